@@ -1,0 +1,718 @@
+/*
+ * lqcd_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU statement of what the hot path of arXiv:2111.05012 computes, written
+ * from the paper's equations with the readings of SURVEY.md §8(c) / DESIGN.md
+ * "Readings".  It shares no code with the CUDA path (paper_2111_05012_b200/csrc) and is only
+ * ever called from tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs.
+ *
+ * Every routine is the plain definition evaluated with straightforward loops on the canonical
+ * layouts (lqcd_inputs.py docstring): no blocking, no fusion, no spin-projection trick, no
+ * reordering beyond `#pragma omp parallel for` over independent output sites.
+ *
+ * The file is compiled twice (oracle/build.py):
+ *     -DIN_REAL=double -DSUFFIX=_ref        inputs are fp64
+ *     -DIN_REAL=float  -DSUFFIX=_ref_f32in  inputs are fp32-rounded values (parity protocol O9:
+ *                                           promoted to fp64 on load; ALL arithmetic is fp64)
+ * Outputs are always fp64.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): free-field plane waves (closed form),
+ * constant-abelian-background plane waves, gamma algebra, gamma5-hermiticity (Eq. 2), gauge
+ * covariance, constant-field clover closed form, R P = 1, adjointness of R and P, dense
+ * brute-force P^dag D P, coarse gamma5-hermiticity, coarse_mult == restrict(D(prolong)).
+ * No routine in this file is "parity unpinned".
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef double _Complex zc;
+#ifndef IN_REAL
+#define IN_REAL double
+#endif
+#ifndef SUFFIX
+#define SUFFIX _ref
+#endif
+typedef IN_REAL _Complex inc;
+#define CAT_(a, b) a##b
+#define CAT(a, b) CAT_(a, b)
+#define FN(name) CAT(name, SUFFIX)
+
+#define LQCD_REF_DAGGER 1u
+
+/* ------------------------------------------------------------------------------------------
+ * O1. Gamma matrices: chiral (Weyl) basis, Hermitian, {g_mu, g_nu} = 2 delta  (reading Q2: the
+ * paper gives no representation; only gamma5 = -g1 g2 g3 g4, Eq. 2).
+ * ---------------------------------------------------------------------------------------- */
+static const zc GAMMA[4][4][4] = {
+    /* gamma_x */ {{0, 0, 0, -I}, {0, 0, -I, 0}, {0, I, 0, 0}, {I, 0, 0, 0}},
+    /* gamma_y */ {{0, 0, 0, -1}, {0, 0, 1, 0}, {0, 1, 0, 0}, {-1, 0, 0, 0}},
+    /* gamma_z */ {{0, 0, -I, 0}, {0, 0, 0, I}, {I, 0, 0, 0}, {0, -I, 0, 0}},
+    /* gamma_t */ {{0, 0, 1, 0}, {0, 0, 0, 1}, {1, 0, 0, 0}, {0, 1, 0, 0}},
+};
+
+static void mat4_mul(zc c[4][4], const zc a[4][4], const zc b[4][4]) {
+    zc t[4][4];
+    for (int i = 0; i < 4; i++)
+        for (int j = 0; j < 4; j++) {
+            zc s = 0;
+            for (int k = 0; k < 4; k++) s += a[i][k] * b[k][j];
+            t[i][j] = s;
+        }
+    memcpy(c, t, sizeof(t));
+}
+
+/* gamma5 = - gamma_1 gamma_2 gamma_3 gamma_4   (Eq. 2) */
+static void gamma5(zc g5[4][4]) {
+    zc t[4][4];
+    mat4_mul(t, GAMMA[0], GAMMA[1]);
+    mat4_mul(t, t, GAMMA[2]);
+    mat4_mul(t, t, GAMMA[3]);
+    for (int i = 0; i < 4; i++)
+        for (int j = 0; j < 4; j++) g5[i][j] = -t[i][j];
+}
+
+/* g[0..3] = gamma_x..gamma_t, g[4] = gamma5 (for the algebra pins). */
+void FN(lqcd_gamma)(zc g[5][4][4]) {
+    memcpy(g, GAMMA, sizeof(GAMMA));
+    gamma5(g[4]);
+}
+
+int FN(lqcd_oracle_threads)(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Geometry: s = x + Lx (y + Ly (z + Lz t))   (reading Q3: 0-based, x fastest)
+ * ---------------------------------------------------------------------------------------- */
+static void coords_of(const int L[4], long s, int x[4]) {
+    x[0] = (int)(s % L[0]);
+    s /= L[0];
+    x[1] = (int)(s % L[1]);
+    s /= L[1];
+    x[2] = (int)(s % L[2]);
+    s /= L[2];
+    x[3] = (int)s;
+}
+
+static long index_of(const int L[4], const int x[4]) {
+    return x[0] + (long)L[0] * (x[1] + (long)L[1] * (x[2] + (long)L[2] * x[3]));
+}
+
+/* site x + sign*mu_hat modulo L; *wrapped = 1 if the hop crosses the lattice boundary */
+static long neighbour(const int L[4], long s, int mu, int sign, int* wrapped) {
+    int x[4];
+    coords_of(L, s, x);
+    int y = x[mu] + sign;
+    *wrapped = 0;
+    if (y >= L[mu]) {
+        y -= L[mu];
+        *wrapped = 1;
+    }
+    if (y < 0) {
+        y += L[mu];
+        *wrapped = 1;
+    }
+    x[mu] = y;
+    return index_of(L, x);
+}
+
+static long volume_of(const int L[4]) { return (long)L[0] * L[1] * L[2] * L[3]; }
+
+/* ------------------------------------------------------------------------------------------
+ * O2. Fine operator, Eq. 1:
+ *   D psi(x) = [1 + F(x)] psi(x)
+ *              - kappa sum_mu [ (1 - g_mu) U_mu(x) psi(x+mu) + (1 + g_mu) U_mu^dag(x-mu) psi(x-mu) ]
+ * Boundary condition (reading Q4): psi(x + L_mu mu_hat) = bc[mu] psi(x), i.e. a hop that wraps
+ * carries the factor bc[mu] (forward and backward alike).
+ * Dagger (Eq. 2): D^dag = gamma5 D gamma5 -- input multiplied by gamma5, D applied, output
+ * multiplied by gamma5.
+ * ---------------------------------------------------------------------------------------- */
+static void load_spinor(zc psi[4][3], const inc* in, long y, const zc (*g5)[4]) {
+    zc raw[4][3];
+    for (int a = 0; a < 4; a++)
+        for (int c = 0; c < 3; c++) raw[a][c] = (zc)in[(y * 4 + a) * 3 + c];
+    if (!g5) {
+        memcpy(psi, raw, sizeof(raw));
+        return;
+    }
+    for (int a = 0; a < 4; a++)
+        for (int c = 0; c < 3; c++) {
+            zc s = 0;
+            for (int b = 0; b < 4; b++) s += g5[a][b] * raw[b][c];
+            psi[a][c] = s;
+        }
+}
+
+static inline zc link_elem(const inc* U, long V, int mu, long s, int a, int b) {
+    return (zc)U[(((long)mu * V + s) * 3 + a) * 3 + b];
+}
+
+/* D (or D^dag) at one site s; result in out[4][3]. */
+static void dirac_site(zc out[4][3], const inc* in, const inc* U, const inc* clover, double kappa,
+                       const int L[4], const int bc[4], int dagger, long s) {
+    const long V = volume_of(L);
+    zc g5m[4][4];
+    gamma5(g5m);
+    const zc(*g5)[4] = dagger ? g5m : NULL;
+
+    zc psi[4][3], acc[4][3];
+    load_spinor(psi, in, s, g5);
+    /* 1 * psi */
+    memcpy(acc, psi, sizeof(acc));
+    /* F(x) psi: two 6x6 blocks, in-block index k = 3*(alpha mod 2) + c, alpha = 2*chi + k/3 */
+    for (int chi = 0; chi < 2; chi++)
+        for (int k = 0; k < 6; k++) {
+            zc sum = 0;
+            for (int l = 0; l < 6; l++)
+                sum += (zc)clover[((s * 2 + chi) * 6 + k) * 6 + l] * psi[2 * chi + l / 3][l % 3];
+            acc[2 * chi + k / 3][k % 3] += sum;
+        }
+    for (int mu = 0; mu < 4; mu++) {
+        int wrapped;
+        zc nb[4][3], t[4][3];
+        /* forward hop: (1 - g_mu) U_mu(x) psi(x + mu) */
+        long y = neighbour(L, s, mu, +1, &wrapped);
+        double phase = wrapped ? (double)bc[mu] : 1.0;
+        load_spinor(nb, in, y, g5);
+        for (int be = 0; be < 4; be++)
+            for (int a = 0; a < 3; a++) {
+                zc sum = 0;
+                for (int b = 0; b < 3; b++) sum += link_elem(U, V, mu, s, a, b) * nb[be][b];
+                t[be][a] = sum;
+            }
+        for (int al = 0; al < 4; al++)
+            for (int a = 0; a < 3; a++) {
+                zc sum = 0;
+                for (int be = 0; be < 4; be++) sum += ((al == be ? 1.0 : 0.0) - GAMMA[mu][al][be]) * t[be][a];
+                acc[al][a] -= kappa * phase * sum;
+            }
+        /* backward hop: (1 + g_mu) U_mu^dag(x - mu) psi(x - mu) */
+        y = neighbour(L, s, mu, -1, &wrapped);
+        phase = wrapped ? (double)bc[mu] : 1.0;
+        load_spinor(nb, in, y, g5);
+        for (int be = 0; be < 4; be++)
+            for (int a = 0; a < 3; a++) {
+                zc sum = 0;
+                for (int b = 0; b < 3; b++) sum += conj(link_elem(U, V, mu, y, b, a)) * nb[be][b];
+                t[be][a] = sum;
+            }
+        for (int al = 0; al < 4; al++)
+            for (int a = 0; a < 3; a++) {
+                zc sum = 0;
+                for (int be = 0; be < 4; be++) sum += ((al == be ? 1.0 : 0.0) + GAMMA[mu][al][be]) * t[be][a];
+                acc[al][a] -= kappa * phase * sum;
+            }
+    }
+    if (!dagger) {
+        memcpy(out, acc, sizeof(acc));
+        return;
+    }
+    for (int a = 0; a < 4; a++)
+        for (int c = 0; c < 3; c++) {
+            zc sum = 0;
+            for (int b = 0; b < 4; b++) sum += g5m[a][b] * acc[b][c];
+            out[a][c] = sum;
+        }
+}
+
+static int check_dims_bc(const int L[4], const int bc[4]) {
+    for (int mu = 0; mu < 4; mu++) {
+        if (L[mu] < 1) return -1;
+        if (bc && bc[mu] != 1 && bc[mu] != -1) return -1;
+    }
+    return 0;
+}
+
+/* out[V][4][3] = D in  (flags & 1: D^dag in) */
+int FN(lqcd_wilson_clover_mult)(zc* out, const inc* in, const inc* U, const inc* clover, double kappa,
+                                const int L[4], const int bc[4], unsigned flags) {
+    if (!out || !in || !U || !clover || check_dims_bc(L, bc)) return -1;
+    const long V = volume_of(L);
+    const int dagger = (flags & LQCD_REF_DAGGER) != 0;
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < V; s++) {
+        zc r[4][3];
+        dirac_site(r, in, U, clover, kappa, L, bc, dagger, s);
+        memcpy(out + s * 12, r, sizeof(r));
+    }
+    return 0;
+}
+
+/* Same operator evaluated only at the listed sites: out[n][4][3] = (D in)(sites[n]).
+ * Used for sampled parity at the full BASELINE sizes and for the bounded cpu_baseline sample. */
+int FN(lqcd_wilson_clover_mult_sites)(zc* out, const inc* in, const inc* U, const inc* clover, double kappa,
+                                      const int L[4], const int bc[4], unsigned flags, const long* sites,
+                                      long nsites) {
+    if (!out || !in || !U || !clover || !sites || check_dims_bc(L, bc)) return -1;
+    const long V = volume_of(L);
+    const int dagger = (flags & LQCD_REF_DAGGER) != 0;
+    for (long n = 0; n < nsites; n++)
+        if (sites[n] < 0 || sites[n] >= V) return -1;
+#pragma omp parallel for schedule(static)
+    for (long n = 0; n < nsites; n++) {
+        zc r[4][3];
+        dirac_site(r, in, U, clover, kappa, L, bc, dagger, sites[n]);
+        memcpy(out + n * 12, r, sizeof(r));
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O3. Clover term (input preparation; reading Q1 -- the paper says only "12x12 Hermitian matrix
+ * made of link variables"):
+ *   F(x) = kappa c_sw sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}(x),
+ *   sigma_{mu nu} = [g_mu, g_nu] / (2i),   F_{mu nu} = (Q - Q^dag) / (8i),
+ *   Q_{mu nu}(x) = sum of the four plaquette leaves in the mu-nu plane starting and ending at x,
+ *   all with the same orientation.  Gauge links are periodic (bc acts on fermion hops only).
+ * Output: clover[s][chi][6][6], the two chirality-diagonal 6x6 blocks; *offdiag_max receives the
+ * largest |entry| of the chirality-off-diagonal part (must be 0: F commutes with gamma5).
+ * ---------------------------------------------------------------------------------------- */
+typedef zc m3[3][3];
+
+static void m3_load(m3 r, const inc* U, long V, int mu, long s) {
+    for (int a = 0; a < 3; a++)
+        for (int b = 0; b < 3; b++) r[a][b] = link_elem(U, V, mu, s, a, b);
+}
+static void m3_dag(m3 r, const m3 a) {
+    m3 t;
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) t[i][j] = conj(a[j][i]);
+    memcpy(r, t, sizeof(m3));
+}
+static void m3_mul(m3 r, const m3 a, const m3 b) {
+    m3 t;
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) {
+            zc s = 0;
+            for (int k = 0; k < 3; k++) s += a[i][k] * b[k][j];
+            t[i][j] = s;
+        }
+    memcpy(r, t, sizeof(m3));
+}
+/* r = a b c d */
+static void m3_mul4(m3 r, const m3 a, const m3 b, const m3 c, const m3 d) {
+    m3 t;
+    m3_mul(t, a, b);
+    m3_mul(t, t, c);
+    m3_mul(r, t, d);
+}
+
+static long shift(const int L[4], long s, int mu, int dmu, int nu, int dnu) {
+    int w;
+    long y = s;
+    if (dmu) y = neighbour(L, y, mu, dmu, &w);
+    if (dnu) y = neighbour(L, y, nu, dnu, &w);
+    return y;
+}
+
+int FN(lqcd_clover_from_links)(zc* clover, const inc* U, double kappa, double csw, const int L[4],
+                               double* offdiag_max) {
+    if (!clover || !U || check_dims_bc(L, NULL)) return -1;
+    const long V = volume_of(L);
+    double offmax = 0.0;
+#pragma omp parallel for schedule(static) reduction(max : offmax)
+    for (long s = 0; s < V; s++) {
+        zc F[12][12];
+        memset(F, 0, sizeof(F));
+        for (int mu = 0; mu < 4; mu++)
+            for (int nu = mu + 1; nu < 4; nu++) {
+                m3 a, b, c, d, leaf, Q;
+                memset(Q, 0, sizeof(Q));
+                /* leaf 1: U_mu(x) U_nu(x+mu) U_mu^dag(x+nu) U_nu^dag(x) */
+                m3_load(a, U, V, mu, s);
+                m3_load(b, U, V, nu, shift(L, s, mu, +1, nu, 0));
+                m3_load(c, U, V, mu, shift(L, s, mu, 0, nu, +1));
+                m3_dag(c, c);
+                m3_load(d, U, V, nu, s);
+                m3_dag(d, d);
+                m3_mul4(leaf, a, b, c, d);
+                for (int i = 0; i < 3; i++)
+                    for (int j = 0; j < 3; j++) Q[i][j] += leaf[i][j];
+                /* leaf 2: U_nu(x) U_mu^dag(x-mu+nu) U_nu^dag(x-mu) U_mu(x-mu) */
+                m3_load(a, U, V, nu, s);
+                m3_load(b, U, V, mu, shift(L, s, mu, -1, nu, +1));
+                m3_dag(b, b);
+                m3_load(c, U, V, nu, shift(L, s, mu, -1, nu, 0));
+                m3_dag(c, c);
+                m3_load(d, U, V, mu, shift(L, s, mu, -1, nu, 0));
+                m3_mul4(leaf, a, b, c, d);
+                for (int i = 0; i < 3; i++)
+                    for (int j = 0; j < 3; j++) Q[i][j] += leaf[i][j];
+                /* leaf 3: U_mu^dag(x-mu) U_nu^dag(x-mu-nu) U_mu(x-mu-nu) U_nu(x-nu) */
+                m3_load(a, U, V, mu, shift(L, s, mu, -1, nu, 0));
+                m3_dag(a, a);
+                m3_load(b, U, V, nu, shift(L, s, mu, -1, nu, -1));
+                m3_dag(b, b);
+                m3_load(c, U, V, mu, shift(L, s, mu, -1, nu, -1));
+                m3_load(d, U, V, nu, shift(L, s, mu, 0, nu, -1));
+                m3_mul4(leaf, a, b, c, d);
+                for (int i = 0; i < 3; i++)
+                    for (int j = 0; j < 3; j++) Q[i][j] += leaf[i][j];
+                /* leaf 4: U_nu^dag(x-nu) U_mu(x-nu) U_nu(x+mu-nu) U_mu^dag(x) */
+                m3_load(a, U, V, nu, shift(L, s, mu, 0, nu, -1));
+                m3_dag(a, a);
+                m3_load(b, U, V, mu, shift(L, s, mu, 0, nu, -1));
+                m3_load(c, U, V, nu, shift(L, s, mu, +1, nu, -1));
+                m3_load(d, U, V, mu, s);
+                m3_dag(d, d);
+                m3_mul4(leaf, a, b, c, d);
+                for (int i = 0; i < 3; i++)
+                    for (int j = 0; j < 3; j++) Q[i][j] += leaf[i][j];
+                /* F_{mu nu} = (Q - Q^dag) / (8 i) */
+                m3 Fmn;
+                for (int i = 0; i < 3; i++)
+                    for (int j = 0; j < 3; j++) Fmn[i][j] = (Q[i][j] - conj(Q[j][i])) / (8.0 * I);
+                /* sigma_{mu nu} = (g_mu g_nu - g_nu g_mu) / (2 i) */
+                zc gm[4][4], gn[4][4], sig[4][4];
+                mat4_mul(gm, GAMMA[mu], GAMMA[nu]);
+                mat4_mul(gn, GAMMA[nu], GAMMA[mu]);
+                for (int i = 0; i < 4; i++)
+                    for (int j = 0; j < 4; j++) sig[i][j] = (gm[i][j] - gn[i][j]) / (2.0 * I);
+                for (int al = 0; al < 4; al++)
+                    for (int be = 0; be < 4; be++)
+                        for (int i = 0; i < 3; i++)
+                            for (int j = 0; j < 3; j++)
+                                F[3 * al + i][3 * be + j] += kappa * csw * sig[al][be] * Fmn[i][j];
+            }
+        /* split into the two chirality blocks; record the off-diagonal remainder */
+        for (int al = 0; al < 4; al++)
+            for (int be = 0; be < 4; be++)
+                for (int i = 0; i < 3; i++)
+                    for (int j = 0; j < 3; j++) {
+                        zc f = F[3 * al + i][3 * be + j];
+                        if (al / 2 == be / 2) {
+                            int chi = al / 2, k = 3 * (al % 2) + i, l = 3 * (be % 2) + j;
+                            clover[((s * 2 + chi) * 6 + k) * 6 + l] = f;
+                        } else if (cabs(f) > offmax) {
+                            offmax = cabs(f);
+                        }
+                    }
+    }
+    if (offdiag_max) *offdiag_max = offmax;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Aggregates: block b[4] divides L; coarse dims Lc = L / b; X_mu = floor(x_mu / b_mu);
+ * coarse component c = chi * nvec + i, chi = alpha / 2   (readings Q5, Q9).
+ * ---------------------------------------------------------------------------------------- */
+static int check_block(const int L[4], const int b[4], int nvec, int Lc[4]) {
+    if (nvec < 1) return -1;
+    for (int mu = 0; mu < 4; mu++) {
+        if (L[mu] < 1 || b[mu] < 1 || L[mu] % b[mu]) return -1;
+        Lc[mu] = L[mu] / b[mu];
+    }
+    return 0;
+}
+
+/* fine site of local coordinate index l (x fastest) inside coarse site X */
+static long block_site(const int L[4], const int b[4], const int Lc[4], long X, long l) {
+    int Xc[4], lc[4], x[4];
+    coords_of(Lc, X, Xc);
+    coords_of(b, l, lc);
+    for (int mu = 0; mu < 4; mu++) x[mu] = Xc[mu] * b[mu] + lc[mu];
+    return index_of(L, x);
+}
+
+static long coarse_site_of(const int L[4], const int b[4], const int Lc[4], long s) {
+    int x[4], Xc[4];
+    coords_of(L, s, x);
+    for (int mu = 0; mu < 4; mu++) Xc[mu] = x[mu] / b[mu];
+    return index_of(Lc, Xc);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O4. Block orthonormalisation (input preparation; reading Q6): within each
+ * (X, chi) the nvec vectors restricted to the sites of X and the two spin components of chi are
+ * orthonormalised in index order by modified Gram-Schmidt, each vector projected twice against
+ * its predecessors before it is normalised.  In place, fp64 only.
+ * ---------------------------------------------------------------------------------------- */
+#ifdef LQCD_ORACLE_FP64_BUILD
+int FN(lqcd_orthonormalize_blocks)(zc* v, const int L[4], const int b[4], int nvec) {
+    int Lc[4];
+    if (!v || check_block(L, b, nvec, Lc)) return -1;
+    const long V = volume_of(L), Vc = volume_of(Lc), bv = volume_of(b);
+    if (bv * 6 < nvec) return -1;
+    int fail = 0;
+#pragma omp parallel for schedule(dynamic) collapse(2)
+    for (long X = 0; X < Vc; X++)
+        for (int chi = 0; chi < 2; chi++) {
+            for (int i = 0; i < nvec; i++) {
+                for (int pass = 0; pass < 2; pass++)
+                    for (int j = 0; j < i; j++) {
+                        zc r = 0; /* r = <w_j | w_i> */
+                        for (long l = 0; l < bv; l++) {
+                            long s = block_site(L, b, Lc, X, l);
+                            for (int k = 0; k < 6; k++) {
+                                long o = (s * 4 + 2 * chi + k / 3) * 3 + k % 3;
+                                r += conj(v[(long)j * V * 12 + o]) * v[(long)i * V * 12 + o];
+                            }
+                        }
+                        for (long l = 0; l < bv; l++) {
+                            long s = block_site(L, b, Lc, X, l);
+                            for (int k = 0; k < 6; k++) {
+                                long o = (s * 4 + 2 * chi + k / 3) * 3 + k % 3;
+                                v[(long)i * V * 12 + o] -= r * v[(long)j * V * 12 + o];
+                            }
+                        }
+                    }
+                double n2 = 0;
+                for (long l = 0; l < bv; l++) {
+                    long s = block_site(L, b, Lc, X, l);
+                    for (int k = 0; k < 6; k++) {
+                        long o = (s * 4 + 2 * chi + k / 3) * 3 + k % 3;
+                        zc z = v[(long)i * V * 12 + o];
+                        n2 += creal(z) * creal(z) + cimag(z) * cimag(z);
+                    }
+                }
+                if (!(n2 > 0)) {
+                    fail = 1;
+                    continue;
+                }
+                double inv = 1.0 / sqrt(n2);
+                for (long l = 0; l < bv; l++) {
+                    long s = block_site(L, b, Lc, X, l);
+                    for (int k = 0; k < 6; k++) {
+                        long o = (s * 4 + 2 * chi + k / 3) * 3 + k % 3;
+                        v[(long)i * V * 12 + o] *= inv;
+                    }
+                }
+            }
+        }
+    return fail ? -2 : 0;
+}
+#endif
+
+/* ------------------------------------------------------------------------------------------
+ * O5. Restriction, Eq. 5:  x_c(I) = <I|x>,  I = {s(chi), i, X}:
+ *   out[X][chi][i] = sum_{x in X} sum_{alpha in chi} sum_c conj(v_i(x,alpha,c)) in(x,alpha,c)
+ * ---------------------------------------------------------------------------------------- */
+int FN(lqcd_restrict)(zc* out_c, const inc* in_f, const inc* v, const int L[4], const int b[4], int nvec) {
+    int Lc[4];
+    if (!out_c || !in_f || !v || check_block(L, b, nvec, Lc)) return -1;
+    const long V = volume_of(L), Vc = volume_of(Lc), bv = volume_of(b);
+#pragma omp parallel for schedule(static)
+    for (long X = 0; X < Vc; X++)
+        for (int chi = 0; chi < 2; chi++)
+            for (int i = 0; i < nvec; i++) {
+                zc sum = 0;
+                for (long l = 0; l < bv; l++) {
+                    long s = block_site(L, b, Lc, X, l);
+                    for (int al = 2 * chi; al < 2 * chi + 2; al++)
+                        for (int c = 0; c < 3; c++) {
+                            long o = (s * 4 + al) * 3 + c;
+                            sum += conj((zc)v[(long)i * V * 12 + o]) * (zc)in_f[o];
+                        }
+                }
+                out_c[(X * 2 + chi) * nvec + i] = sum;
+            }
+    return 0;
+}
+
+/* Prolongation, Eq. 6:  |x'> = sum_I x_c(I) |I>:
+ *   out(x,alpha,c) = sum_i v_i(x,alpha,c) in[X(x)][chi(alpha)][i] */
+int FN(lqcd_prolong)(zc* out_f, const inc* in_c, const inc* v, const int L[4], const int b[4], int nvec) {
+    int Lc[4];
+    if (!out_f || !in_c || !v || check_block(L, b, nvec, Lc)) return -1;
+    const long V = volume_of(L);
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < V; s++) {
+        long X = coarse_site_of(L, b, Lc, s);
+        for (int al = 0; al < 4; al++)
+            for (int c = 0; c < 3; c++) {
+                long o = (s * 4 + al) * 3 + c;
+                zc sum = 0;
+                for (int i = 0; i < nvec; i++)
+                    sum += (zc)v[(long)i * V * 12 + o] * (zc)in_c[(X * 2 + al / 2) * nvec + i];
+                out_f[o] = sum;
+            }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O6. Galerkin coarse operator, Eq. 7:  D_c(I,J) = <I|D|J>, stored as nine dense
+ * N x N blocks per coarse site (reading Q7), N = 2 nvec.  D is split into its site-diagonal part
+ * and its eight directed hops,
+ *     D = D_diag + sum_mu (D_{+mu} + D_{-mu}),
+ *     D_diag = 1 + F,
+ *     (D_{+mu} w)(x) = -kappa beta+ (1 - g_mu) U_mu(x) w(x+mu),
+ *     (D_{-mu} w)(x) = -kappa beta- (1 + g_mu) U_mu^dag(x-mu) w(x-mu),
+ * and
+ *     A[X][0]      = P_X^dag [ D_diag + hops with both ends inside X ] P_X
+ *     A[X][1+2mu]  = P_X^dag D_{+mu} P_{X+mu}   (only hops that leave X in +mu)
+ *     A[X][2+2mu]  = P_X^dag D_{-mu} P_{X-mu}   (only hops that leave X in -mu)
+ * A hop from y = x+mu into x leaves the block iff x is on the block's high edge in mu
+ * (x_mu mod b_mu == b_mu - 1); backward iff x_mu mod b_mu == 0.  Keeping the DIRECTED split is what
+ * makes this right when the coarse extent is 2 and X+mu == X-mu (reading Q8).  Column (chi',i') of
+ * P_Y is v_i' on block Y with the spin components outside chi' zeroed.
+ * ---------------------------------------------------------------------------------------- */
+int FN(lqcd_galerkin_coarse)(zc* A, const inc* U, const inc* clover, const inc* v, double kappa, const int L[4],
+                             const int bc[4], const int b[4], int nvec) {
+    int Lc[4];
+    if (!A || !U || !clover || !v || check_block(L, b, nvec, Lc) || check_dims_bc(L, bc)) return -1;
+    for (int mu = 0; mu < 4; mu++)
+        if (Lc[mu] < 2) return -1;
+    const long V = volume_of(L), Vc = volume_of(Lc), bv = volume_of(b);
+    const int N = 2 * nvec;
+#pragma omp parallel
+    {
+        zc* T = (zc*)malloc(sizeof(zc) * N * 12); /* T[J][alpha*3+c] = (D_piece P)(x) column J */
+#pragma omp for schedule(dynamic)
+        for (long X = 0; X < Vc; X++) {
+            zc* AX = A + X * 9 * (long)N * N;
+            memset(AX, 0, sizeof(zc) * 9 * (size_t)N * N);
+            for (long l = 0; l < bv; l++) {
+                const long s = block_site(L, b, Lc, X, l);
+                int x[4];
+                coords_of(L, s, x);
+                for (int piece = 0; piece < 9; piece++) {
+                    long y; /* source site */
+                    int d;  /* which of the nine blocks receives this piece */
+                    if (piece == 0) {
+                        y = s;
+                        d = 0;
+                    } else {
+                        const int mu = (piece - 1) / 2, fwd = (piece - 1) % 2 == 0;
+                        int wrapped;
+                        y = neighbour(L, s, mu, fwd ? +1 : -1, &wrapped);
+                        const int leaves =
+                            fwd ? (x[mu] % b[mu] == b[mu] - 1) : (x[mu] % b[mu] == 0);
+                        d = leaves ? piece : 0;
+                    }
+                    /* T[J] = piece applied to column J of P at source site y */
+                    for (int J = 0; J < N; J++) {
+                        const int chiJ = J / nvec, iJ = J % nvec;
+                        zc src[4][3], res[4][3];
+                        for (int al = 0; al < 4; al++)
+                            for (int c = 0; c < 3; c++)
+                                src[al][c] = (al / 2 == chiJ) ? (zc)v[(long)iJ * V * 12 + (y * 4 + al) * 3 + c] : 0;
+                        if (piece == 0) {
+                            memcpy(res, src, sizeof(res));
+                            for (int chi = 0; chi < 2; chi++)
+                                for (int k = 0; k < 6; k++) {
+                                    zc sum = 0;
+                                    for (int m = 0; m < 6; m++)
+                                        sum += (zc)clover[((s * 2 + chi) * 6 + k) * 6 + m] *
+                                               src[2 * chi + m / 3][m % 3];
+                                    res[2 * chi + k / 3][k % 3] += sum;
+                                }
+                        } else {
+                            const int mu = (piece - 1) / 2, fwd = (piece - 1) % 2 == 0;
+                            int wrapped;
+                            (void)neighbour(L, s, mu, fwd ? +1 : -1, &wrapped);
+                            const double phase = wrapped ? (double)bc[mu] : 1.0;
+                            zc t[4][3];
+                            for (int be = 0; be < 4; be++)
+                                for (int a = 0; a < 3; a++) {
+                                    zc sum = 0;
+                                    for (int c = 0; c < 3; c++)
+                                        sum += (fwd ? link_elem(U, V, mu, s, a, c)
+                                                    : conj(link_elem(U, V, mu, y, c, a))) *
+                                               src[be][c];
+                                    t[be][a] = sum;
+                                }
+                            for (int al = 0; al < 4; al++)
+                                for (int a = 0; a < 3; a++) {
+                                    zc sum = 0;
+                                    for (int be = 0; be < 4; be++)
+                                        sum += ((al == be ? 1.0 : 0.0) + (fwd ? -1.0 : 1.0) * GAMMA[mu][al][be]) *
+                                               t[be][a];
+                                    res[al][a] = -kappa * phase * sum;
+                                }
+                        }
+                        memcpy(T + (long)J * 12, res, sizeof(res));
+                    }
+                    /* A[X][d][I][J] += sum_{alpha in chi_I, c} conj(v_iI(x,alpha,c)) T[J][alpha,c] */
+                    zc* Ad = AX + (long)d * N * N;
+                    for (int Irow = 0; Irow < N; Irow++) {
+                        const int chiI = Irow / nvec, iI = Irow % nvec;
+                        zc w[6];
+                        for (int k = 0; k < 6; k++)
+                            w[k] = conj((zc)v[(long)iI * V * 12 + (s * 4 + 2 * chiI + k / 3) * 3 + k % 3]);
+                        for (int J = 0; J < N; J++) {
+                            const zc* tj = T + (long)J * 12 + 6 * chiI;
+                            zc sum = 0;
+                            for (int k = 0; k < 6; k++) sum += w[k] * tj[k];
+                            Ad[(long)Irow * N + J] += sum;
+                        }
+                    }
+                }
+            }
+        }
+        free(T);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O7. Coarse operator application, Eqs. 4, 7:
+ *   out(X) = A[X][0] in(X) + sum_mu ( A[X][1+2mu] in(X+mu) + A[X][2+2mu] in(X-mu) ),
+ * neighbours modulo Lc, always periodic (boundary phases live inside A).
+ * Dagger: Gamma5c D_c Gamma5c, Gamma5c = diag(gamma5 sign of chi) (x) 1_nvec.
+ * ---------------------------------------------------------------------------------------- */
+/* AX = the nine blocks A[X][0..8] of this coarse site */
+static void coarse_site(zc* out, const inc* in, const inc* AX, const int Lc[4], int nvec, int dagger, long X) {
+    const int N = 2 * nvec;
+    zc g5m[4][4];
+    gamma5(g5m);
+    double sgn[2] = {1.0, 1.0};
+    if (dagger) {
+        sgn[0] = creal(g5m[0][0]);
+        sgn[1] = creal(g5m[2][2]);
+    }
+    for (int r = 0; r < N; r++) out[r] = 0;
+    for (int d = 0; d < 9; d++) {
+        long Y = X;
+        int w;
+        if (d > 0) Y = neighbour(Lc, X, (d - 1) / 2, (d - 1) % 2 == 0 ? +1 : -1, &w);
+        const inc* Ad = AX + (long)d * N * N;
+        for (int r = 0; r < N; r++) {
+            zc sum = 0;
+            for (int c = 0; c < N; c++) sum += (zc)Ad[(long)r * N + c] * (sgn[c / nvec] * (zc)in[Y * N + c]);
+            out[r] += sum;
+        }
+    }
+    for (int r = 0; r < N; r++) out[r] *= sgn[r / nvec];
+}
+
+int FN(lqcd_coarse_mult)(zc* out, const inc* in, const inc* A, const int Lc[4], int nvec, unsigned flags) {
+    if (!out || !in || !A || nvec < 1) return -1;
+    for (int mu = 0; mu < 4; mu++)
+        if (Lc[mu] < 2) return -1;
+    const long Vc = volume_of(Lc);
+    const int N = 2 * nvec;
+#pragma omp parallel for schedule(static)
+    for (long X = 0; X < Vc; X++)
+        coarse_site(out + X * N, in, A + X * 9 * (long)N * N, Lc, nvec, (flags & LQCD_REF_DAGGER) != 0, X);
+    return 0;
+}
+
+/* The same at listed coarse sites only; A_sites holds ONLY the blocks of those sites
+ * ([n][9][N][N]) so that a sample of a 12 GB coarse matrix can be checked. */
+int FN(lqcd_coarse_mult_sites)(zc* out, const inc* in, const inc* A_sites, const int Lc[4], int nvec,
+                               unsigned flags, const long* sites, long nsites) {
+    if (!out || !in || !A_sites || !sites || nvec < 1) return -1;
+    for (int mu = 0; mu < 4; mu++)
+        if (Lc[mu] < 2) return -1;
+    const long Vc = volume_of(Lc);
+    const int N = 2 * nvec;
+    for (long n = 0; n < nsites; n++)
+        if (sites[n] < 0 || sites[n] >= Vc) return -1;
+#pragma omp parallel for schedule(static)
+    for (long n = 0; n < nsites; n++) {
+        coarse_site(out + n * N, in, A_sites + n * 9 * (long)N * N, Lc, nvec, (flags & LQCD_REF_DAGGER) != 0,
+                    sites[n]);
+    }
+    return 0;
+}

@@ -1,0 +1,434 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (-m "not gpu").
+
+The paper prints no operator input/output values, so every pin is a closed form,
+an invariant, a special case or a brute-force evaluation -- never the oracle's own formula retyped.
+Each test names the mistake it is there to catch.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import lqcd_inputs as li
+import oracle
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def rel(a, b):
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+def zero_clover(V):
+    return np.zeros((V, 2, 6, 6), dtype=np.complex128)
+
+
+# ------------------------------------------------------------------------------------------------
+# O1  gamma algebra (Eq. 2)
+# ------------------------------------------------------------------------------------------------
+
+
+def test_gamma_algebra():
+    g = oracle.gamma()
+    eye = np.eye(4)
+    for mu in range(4):
+        assert np.array_equal(g[mu], g[mu].conj().T), "gamma_mu Hermitian"
+        for nu in range(4):
+            anti = g[mu] @ g[nu] + g[nu] @ g[mu]
+            assert np.array_equal(anti, 2 * eye * (mu == nu)), "Clifford algebra"
+        for sign in (+1, -1):
+            proj = 0.5 * (eye + sign * g[mu])
+            assert np.array_equal(proj @ proj, proj), "(1 +- gamma)/2 is a projector"
+            assert np.linalg.matrix_rank(proj) == 2, "of rank 2"
+    g5 = g[4]
+    assert np.array_equal(g5, -g[0] @ g[1] @ g[2] @ g[3]), "gamma5 = -g1 g2 g3 g4 (Eq. 2)"
+    assert np.array_equal(g5 @ g5, eye), "(gamma5)^2 = 1 (footnote 4, PAPER.md:90)"
+    assert np.array_equal(g5, np.diag([-1, -1, 1, 1])), "chiral basis: gamma5 diagonal, chi=0 <-> spins 0,1"
+    for mu in range(4):
+        assert np.array_equal(g5 @ g[mu], -g[mu] @ g5), "gamma5 anticommutes with gamma_mu"
+
+
+# ------------------------------------------------------------------------------------------------
+# A1  free field: plane waves and the closed-form momentum-space operator
+#     D psi = e^{ipx} M(p) chi,  M(p) = (1 - 2 kappa sum cos p) + 2 i kappa sum gamma_mu sin p_mu
+#     (from Eq. 1 with U = 1, F = 0), eigenvalues 1 - 2k sum cos p +- 2 i k sqrt(sum sin^2 p), each x6.
+#     Catches: wrong hop sign, wrong (1 -+ gamma) assignment, wrong neighbour, wrong bc phase, kappa.
+# ------------------------------------------------------------------------------------------------
+
+
+def plane_wave(dims, p):
+    return np.exp(1j * (li.site_coords(dims) @ np.asarray(p)))
+
+
+def momentum(dims, n, bc):
+    return np.array([2 * np.pi * (n[mu] + (0.5 if bc[mu] == -1 else 0.0)) / dims[mu] for mu in range(4)])
+
+
+def momentum_matrix(p, kappa, colour_phase=None):
+    """12x12 M(p) in (spin, colour) order; colour_phase[mu][c] adds a constant abelian background."""
+    g = oracle.gamma()
+    M = np.zeros((4, 3, 4, 3), dtype=np.complex128)
+    for c in range(3):
+        q = p + (0 if colour_phase is None else colour_phase[:, c])
+        m = (1 - 2 * kappa * np.sum(np.cos(q))) * np.eye(4) + 2j * kappa * sum(g[mu] * np.sin(q[mu]) for mu in range(4))
+        M[:, c, :, c] = m
+    return M.reshape(12, 12)
+
+
+@pytest.mark.parametrize("dims,n,bc", [
+    ((4, 4, 4, 4), (1, 2, 0, 1), (1, 1, 1, -1)),
+    ((4, 6, 2, 8), (3, 1, 1, 5), (1, 1, 1, -1)),
+    ((6, 4, 4, 2), (2, 3, 1, 0), (-1, 1, -1, 1)),
+    ((3, 5, 2, 4), (1, 4, 1, 2), (1, -1, 1, -1)),
+])
+def test_free_field_plane_waves(dims, n, bc):
+    kappa = 0.13
+    V = int(np.prod(dims))
+    U = li.gauge_unit(V)
+    p = momentum(dims, n, bc)
+    wave = plane_wave(dims, p)
+    M = momentum_matrix(p, kappa)
+    got = np.zeros((12, 12), dtype=np.complex128)
+    for k in range(12):
+        chi = np.zeros(12, dtype=np.complex128)
+        chi[k] = 1.0
+        psi = (wave[:, None] * chi[None, :]).reshape(V, 4, 3)
+        out = oracle.wilson_clover_mult(psi, U, zero_clover(V), kappa, dims, bc)
+        expect = (wave[:, None] * M[:, k][None, :]).reshape(V, 4, 3)
+        assert rel(out, expect) < 1e-14
+        got[:, k] = out.reshape(V, 12)[0] / wave[0]
+    # representation-independent: spectrum of the extracted 12x12 equals the closed form
+    lam = np.linalg.eigvals(got)
+    a = 1 - 2 * kappa * np.sum(np.cos(p))
+    b = 2 * kappa * np.sqrt(np.sum(np.sin(p) ** 2))
+    assert np.allclose(lam.real, a, atol=1e-12)
+    assert np.allclose(np.sort(lam.imag), np.array([-b] * 6 + [b] * 6), atol=1e-12)
+
+
+def test_free_field_golden_eigenvalues():
+    """tests/golden/free_field_eigenvalues.txt: closed-form values written by
+    tests/golden/make_free_field_golden.py (pure math, no oracle, no CUDA)."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "free_field_eigenvalues.txt")) if l.strip() and l[0] != "#"]
+    for r in rows:
+        dims = tuple(int(v) for v in r[0:4])
+        n = tuple(int(v) for v in r[4:8])
+        bc = tuple(int(v) for v in r[8:12])
+        kappa, re, im = float(r[12]), float(r[13]), float(r[14])
+        V = int(np.prod(dims))
+        p = momentum(dims, n, bc)
+        wave = plane_wave(dims, p)
+        got = np.zeros((12, 12), dtype=np.complex128)
+        for k in range(12):
+            chi = np.zeros(12, dtype=np.complex128)
+            chi[k] = 1.0
+            psi = (wave[:, None] * chi[None, :]).reshape(V, 4, 3)
+            out = oracle.wilson_clover_mult(psi, li.gauge_unit(V), zero_clover(V), kappa, dims, bc)
+            got[:, k] = out.reshape(V, 12)[5] / wave[5]
+        lam = np.linalg.eigvals(got)
+        assert np.allclose(np.sort(lam.real), re, atol=2e-6)
+        assert np.allclose(np.sort(np.abs(lam.imag)), im, atol=2e-6)
+
+
+def test_kappa_mass_relation():
+    """kappa = 1/(8 + 2 m0): at p = 0, periodic free field, D = (1 - 8 kappa) 1."""
+    dims, bc = (4, 2, 3, 2), (1, 1, 1, 1)
+    V = int(np.prod(dims))
+    m0 = 0.37
+    kappa = 1 / (8 + 2 * m0)
+    psi = np.ones((V, 4, 3), dtype=np.complex128) * (0.3 - 0.8j)
+    out = oracle.wilson_clover_mult(psi, li.gauge_unit(V), zero_clover(V), kappa, dims, bc)
+    assert rel(out, (1 - 8 * kappa) * psi) < 1e-15
+    assert abs((1 - 8 * kappa) - 2 * m0 * kappa) < 1e-15
+
+
+def test_constant_abelian_background():
+    """U_mu = diag(e^{i th_mu,c}) constant: colour c sees momentum p + theta_c.
+    Catches U <-> U^dagger swapped between forward and backward hop, and colour-index mix-ups."""
+    dims, bc, n = (4, 4, 2, 6), (1, 1, 1, -1), (1, 3, 1, 2)
+    V = int(np.prod(dims))
+    rng = np.random.default_rng(7)
+    theta = rng.uniform(-1, 1, size=(4, 3))
+    theta[:, 2] = -theta[:, 0] - theta[:, 1]  # det = 1
+    U = np.zeros((4, V, 3, 3), dtype=np.complex128)
+    for mu in range(4):
+        for c in range(3):
+            U[mu, :, c, c] = np.exp(1j * theta[mu, c])
+    clov, off = oracle.clover_from_links(U, 0.13, 1.3, dims, return_offdiag=True)
+    assert np.max(np.abs(clov)) < 1e-15 and off < 1e-15, "constant abelian field has zero field strength"
+    kappa = 0.124
+    p = momentum(dims, n, bc)
+    wave = plane_wave(dims, p)
+    M = momentum_matrix(p, kappa, colour_phase=theta)
+    for k in (0, 4, 8, 11):
+        chi = np.zeros(12, dtype=np.complex128)
+        chi[k] = 1.0
+        psi = (wave[:, None] * chi[None, :]).reshape(V, 4, 3)
+        out = oracle.wilson_clover_mult(psi, U, clov, kappa, dims, bc)
+        expect = (wave[:, None] * M[:, k][None, :]).reshape(V, 4, 3)
+        assert rel(out, expect) < 1e-14
+
+
+# ------------------------------------------------------------------------------------------------
+# interacting field: config-1-like inputs
+# ------------------------------------------------------------------------------------------------
+
+
+@pytest.fixture(scope="module")
+def c1():
+    cfg = li.CONFIGS["c1"]
+    f = li.make_host_fields(cfg, n_rhs=2)
+    clov = oracle.clover_from_links(f.U, cfg.kappa, cfg.csw, cfg.dims)
+    v = oracle.orthonormalize_blocks(f.v, cfg.dims, cfg.block)
+    A = oracle.galerkin_coarse(f.U, clov, v, cfg.kappa, cfg.dims, cfg.bc, cfg.block)
+    return dict(cfg=cfg, U=f.U, psi=f.psi, clov=clov, v=v, A=A)
+
+
+def test_inputs_are_su3(c1):
+    U = c1["U"]
+    uu = U @ U.conj().swapaxes(-1, -2)
+    assert np.max(np.abs(uu - np.eye(3))) < 1e-14
+    assert np.max(np.abs(np.linalg.det(U) - 1)) < 1e-14
+    # O8: third row = conj(row0 x row1) -- what the 12-real link compression relies on
+    assert np.max(np.abs(np.conj(np.cross(U[..., 0, :], U[..., 1, :])) - U[..., 2, :])) < 1e-14
+    Uh = li.gauge_haar(np.random.default_rng(3), 64)
+    assert np.max(np.abs(Uh @ Uh.conj().swapaxes(-1, -2) - np.eye(3))) < 1e-13
+    assert np.max(np.abs(np.linalg.det(Uh) - 1)) < 1e-13
+
+
+def test_gamma5_hermiticity(c1):
+    """Eq. 2: <x, D^dag y> = <D x, y>, D^dag via the DAGGER flag (gamma5 D gamma5)."""
+    cfg = c1["cfg"]
+    x, y = c1["psi"]
+    Dx = oracle.wilson_clover_mult(x, c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc)
+    Ddy = oracle.wilson_clover_mult(y, c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc, dagger=True)
+    lhs = np.vdot(x, Ddy)
+    rhs = np.vdot(Dx, y)
+    assert abs(lhs - rhs) / abs(rhs) < 1e-13
+    # and the flag really is gamma5 D gamma5
+    g5 = np.array([-1, -1, 1, 1])[None, :, None]
+    manual = g5 * oracle.wilson_clover_mult(g5 * y, c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc)
+    assert rel(Ddy, manual) < 1e-15
+
+
+def test_dagger_is_dense_adjoint():
+    """On a 2x2x2x4 lattice (extent 2: x+mu == x-mu) build dense D and D^dag from unit vectors."""
+    dims, bc = (2, 2, 2, 4), (1, 1, 1, -1)
+    V = int(np.prod(dims))
+    rng = np.random.default_rng(11)
+    U = li.gauge_exp(rng, V, 0.6)
+    clov = oracle.clover_from_links(U, 0.13, 1.2, dims)
+    n = 12 * V
+    D = np.zeros((n, n), dtype=np.complex128)
+    Dd = np.zeros((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1
+        D[:, k] = oracle.wilson_clover_mult(e.reshape(V, 4, 3), U, clov, 0.13, dims, bc).ravel()
+        Dd[:, k] = oracle.wilson_clover_mult(e.reshape(V, 4, 3), U, clov, 0.13, dims, bc, dagger=True).ravel()
+    assert np.max(np.abs(Dd - D.conj().T)) < 1e-14
+
+
+def test_gauge_covariance(c1):
+    """U'_mu(x) = g(x) U_mu(x) g^dag(x+mu), F' from U':  D[U'](g psi) = g D[U] psi.
+    Catches a wrong link site/dagger in the hops and a mis-routed clover leaf."""
+    cfg = c1["cfg"]
+    V = cfg.volume
+    rng = np.random.default_rng(5)
+    g = li.random_gauge_transform(rng, V)
+    Ug = np.empty_like(c1["U"])
+    for mu in range(4):
+        fwd = li.neighbour_index(cfg.dims, mu, +1)
+        Ug[mu] = g @ c1["U"][mu] @ g[fwd].conj().swapaxes(-1, -2)
+    clov_g = oracle.clover_from_links(Ug, cfg.kappa, cfg.csw, cfg.dims)
+    psi = c1["psi"][0]
+    gpsi = np.einsum("sab,sxb->sxa", g, psi)
+    lhs = oracle.wilson_clover_mult(gpsi, Ug, clov_g, cfg.kappa, cfg.dims, cfg.bc)
+    rhs = np.einsum("sab,sxb->sxa", g, oracle.wilson_clover_mult(psi, c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc))
+    assert rel(lhs, rhs) < 1e-14
+
+
+def test_clover_properties(c1):
+    cfg = c1["cfg"]
+    clov, off = oracle.clover_from_links(c1["U"], cfg.kappa, cfg.csw, cfg.dims, return_offdiag=True)
+    assert off < 1e-16, "F commutes with gamma5: chirality-off-diagonal part vanishes"
+    assert np.max(np.abs(clov - clov.conj().swapaxes(-1, -2))) < 1e-16, "F Hermitian (PAPER.md:50)"
+    tr = np.trace(clov, axis1=-2, axis2=-1)
+    assert np.max(np.abs(tr)) < 1e-15, "each chirality block traceless"
+    assert 0.01 < np.max(np.abs(clov)) < 0.5
+    free = oracle.clover_from_links(li.gauge_unit(cfg.volume), cfg.kappa, cfg.csw, cfg.dims)
+    assert np.max(np.abs(free)) == 0.0, "F = 0 at U = 1"
+
+
+def test_clover_constant_field_closed_form():
+    """U_y(x) = exp(i B x_x T), T = diag(1,-1,0), B = 2 pi k / Lx, other links 1: all four xy leaves equal
+    exp(i B T)  =>  F(x) = kappa c_sw sigma_xy (x) sin(B T), other planes 0.
+    Catches a mis-oriented leaf, a wrong 1/8, a wrong mu<nu factor."""
+    dims = (4, 4, 2, 2)
+    V = int(np.prod(dims))
+    kappa, csw, k = 0.13, 1.7, 1
+    B = 2 * np.pi * k / dims[0]
+    T = np.array([1.0, -1.0, 0.0])
+    U = li.gauge_unit(V)
+    xx = li.site_coords(dims)[:, 0]
+    for c in range(3):
+        U[1, :, c, c] = np.exp(1j * B * xx * T[c])
+    clov = oracle.clover_from_links(U, kappa, csw, dims)
+    g = oracle.gamma()
+    sig_xy = (g[0] @ g[1] - g[1] @ g[0]) / 2j
+    assert np.array_equal(sig_xy, np.diag([1, -1, 1, -1])), "sigma_xy = (tau3, tau3) in the chiral basis"
+    F12 = np.kron(sig_xy, np.diag(np.sin(B * T))) * kappa * csw   # index = 3*alpha + c
+    expect = np.stack([F12[0:6, 0:6], F12[6:12, 6:12]])
+    assert np.max(np.abs(clov - expect[None])) < 1e-15
+
+
+# ------------------------------------------------------------------------------------------------
+# O4/O5  aggregates, restriction, prolongation (Eqs. 5, 6)
+# ------------------------------------------------------------------------------------------------
+
+
+def test_block_orthonormality_and_RP_identity(c1):
+    cfg, v = c1["cfg"], c1["v"]
+    rng = np.random.default_rng(9)
+    xc = li.coarse_vector(rng, cfg.cvolume, cfg.nvec)
+    back = oracle.restrict(oracle.prolong(xc, v, cfg.dims, cfg.block), v, cfg.dims, cfg.block)
+    assert rel(back, xc) < 1e-14, "<I|J> = delta_IJ  =>  R P = 1 (PAPER.md:92)"
+    psi = c1["psi"][0]
+    pr = oracle.prolong(oracle.restrict(psi, v, cfg.dims, cfg.block), v, cfg.dims, cfg.block)
+    pr2 = oracle.prolong(oracle.restrict(pr, v, cfg.dims, cfg.block), v, cfg.dims, cfg.block)
+    assert rel(pr2, pr) < 1e-14, "P R idempotent"
+    ratio = np.linalg.norm(pr) / np.linalg.norm(psi)
+    assert 0.05 < ratio < 0.9, "x and x' are in general different (PAPER.md:101)"
+    # explicit Gram matrix of one aggregate, straight from the definition
+    X = 5
+    Xc = np.array([X % 2, (X // 2) % 2, (X // 4) % 2, X // 8])
+    co = li.site_coords(cfg.dims)
+    mask = np.all(co // np.array(cfg.block) == Xc, axis=1)
+    for chi in range(2):
+        W = v[:, mask][:, :, 2 * chi:2 * chi + 2, :].reshape(cfg.nvec, -1)
+        assert np.max(np.abs(W.conj() @ W.T - np.eye(cfg.nvec))) < 1e-14
+
+
+def test_restrict_prolong_adjoint_and_definition(c1):
+    cfg, v = c1["cfg"], c1["v"]
+    rng = np.random.default_rng(10)
+    psi = c1["psi"][1]
+    xc = li.coarse_vector(rng, cfg.cvolume, cfg.nvec)
+    lhs = np.vdot(oracle.restrict(psi, v, cfg.dims, cfg.block), xc)
+    rhs = np.vdot(psi, oracle.prolong(xc, v, cfg.dims, cfg.block))
+    assert abs(lhs - rhs) / abs(rhs) < 1e-14, "<R psi, x_c> = <psi, P x_c>"
+    # dense P (3072 x 128) assembled column by column from Eq. 6 and used for Eq. 5
+    co = li.site_coords(cfg.dims)
+    Xof = (co // np.array(cfg.block)) @ np.array([1, 2, 4, 8])
+    P = np.zeros((cfg.volume, 4, 3, cfg.cvolume, 2, cfg.nvec), dtype=np.complex128)
+    for i in range(cfg.nvec):
+        for chi in range(2):
+            P[np.arange(cfg.volume), 2 * chi:2 * chi + 2, :, Xof, chi, i] = v[i][:, 2 * chi:2 * chi + 2, :]
+    P = P.reshape(cfg.volume * 12, cfg.cvolume * 2 * cfg.nvec)
+    assert rel(oracle.prolong(xc, v, cfg.dims, cfg.block).ravel(), P @ xc.ravel()) < 1e-14
+    assert rel(oracle.restrict(psi, v, cfg.dims, cfg.block).ravel(), P.conj().T @ psi.ravel()) < 1e-14
+
+
+# ------------------------------------------------------------------------------------------------
+# O6/O7  Galerkin coarse operator (Eq. 7) and its application
+# ------------------------------------------------------------------------------------------------
+
+
+def test_coarse_equals_dense_PdagDP(c1):
+    """Brute force on config 1: dense D (3072^2) from unit vectors, dense P, y = P^dag D P x_c
+    against the 9-point apply of the Galerkin blocks.  Coarse extent 2 in every direction
+    (X+mu == X-mu), antiperiodic time."""
+    cfg, v = c1["cfg"], c1["v"]
+    n = cfg.volume * 12
+    D = np.zeros((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1
+        D[:, k] = oracle.wilson_clover_mult(e.reshape(-1, 4, 3), c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc).ravel()
+    nc = cfg.cvolume * 2 * cfg.nvec
+    P = np.zeros((n, nc), dtype=np.complex128)
+    for k in range(nc):
+        e = np.zeros(nc, dtype=np.complex128)
+        e[k] = 1
+        P[:, k] = oracle.prolong(e.reshape(cfg.cvolume, 2, cfg.nvec), v, cfg.dims, cfg.block).ravel()
+    Dc = P.conj().T @ D @ P
+    rng = np.random.default_rng(12)
+    xc = li.coarse_vector(rng, cfg.cvolume, cfg.nvec)
+    got = oracle.coarse_mult(xc, c1["A"], cfg.cdims)
+    assert rel(got.ravel(), Dc @ xc.ravel()) < 1e-14
+    gotd = oracle.coarse_mult(xc, c1["A"], cfg.cdims, dagger=True)
+    assert rel(gotd.ravel(), Dc.conj().T @ xc.ravel()) < 1e-13, "Gamma5c D_c Gamma5c = D_c^dag"
+
+
+def test_coarse_gamma5_block_relations(c1):
+    """Gamma5c A0 Gamma5c = A0^dag and A_{-mu}(X+mu) = Gamma5c A_{+mu}(X)^dag Gamma5c."""
+    cfg, A = c1["cfg"], c1["A"]
+    nv = cfg.nvec
+    g5c = np.diag(np.concatenate([-np.ones(nv), np.ones(nv)]))
+    for X in range(cfg.cvolume):
+        assert np.max(np.abs(g5c @ A[X, 0] @ g5c - A[X, 0].conj().T)) < 1e-15
+    for mu in range(4):
+        fwd = li.neighbour_index(cfg.cdims, mu, +1)
+        for X in range(cfg.cvolume):
+            lhs = A[fwd[X], 2 + 2 * mu]
+            rhs = g5c @ A[X, 1 + 2 * mu].conj().T @ g5c
+            assert np.max(np.abs(lhs - rhs)) < 1e-15
+
+
+@pytest.mark.parametrize("dims,block,nvec,bc", [
+    ((8, 4, 4, 8), (4, 2, 2, 2), 5, (1, 1, 1, -1)),
+    ((4, 6, 4, 4), (2, 3, 1, 2), 3, (-1, 1, 1, -1)),
+])
+def test_galerkin_identity_as_operators(dims, block, nvec, bc):
+    """coarse_mult(x_c) == restrict(D prolong(x_c)) without dense matrices."""
+    V = int(np.prod(dims))
+    rng = np.random.default_rng(21)
+    U = li.gauge_haar(rng, V)
+    kappa, csw = 0.135, 1.4
+    clov = oracle.clover_from_links(U, kappa, csw, dims)
+    v = oracle.orthonormalize_blocks(li.null_vectors(rng, nvec, V), dims, block)
+    A = oracle.galerkin_coarse(U, clov, v, kappa, dims, bc, block)
+    cdims = tuple(l // b for l, b in zip(dims, block))
+    xc = li.coarse_vector(rng, int(np.prod(cdims)), nvec)
+    lhs = oracle.coarse_mult(xc, A, cdims)
+    rhs = oracle.restrict(oracle.wilson_clover_mult(oracle.prolong(xc, v, dims, block), U, clov, kappa, dims, bc), v, dims, block)
+    assert rel(lhs, rhs) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# entry-point variants agree with the pinned ones
+# ------------------------------------------------------------------------------------------------
+
+
+def test_f32in_and_sites_variants(c1):
+    cfg = c1["cfg"]
+    U32, psi32, clov32 = (li.round_to_f32(a) for a in (c1["U"], c1["psi"][0], c1["clov"]))
+    v32, A32 = li.round_to_f32(c1["v"]), li.round_to_f32(c1["A"])
+    up = lambda a: a.astype(np.complex128)
+    for dag in (False, True):
+        a = oracle.wilson_clover_mult(psi32, U32, clov32, cfg.kappa, cfg.dims, cfg.bc, dagger=dag)
+        b = oracle.wilson_clover_mult(up(psi32), up(U32), up(clov32), cfg.kappa, cfg.dims, cfg.bc, dagger=dag)
+        assert np.array_equal(a, b), "fp32-input entry point = fp64 arithmetic on the rounded values"
+        sites = np.array([0, 17, 255, 64, 3])
+        c = oracle.wilson_clover_mult_sites(psi32, U32, clov32, cfg.kappa, cfg.dims, cfg.bc, sites, dagger=dag)
+        assert np.array_equal(c, a[sites])
+    rng = np.random.default_rng(2)
+    xc32 = li.round_to_f32(li.coarse_vector(rng, cfg.cvolume, cfg.nvec))
+    for dag in (False, True):
+        a = oracle.coarse_mult(xc32, A32, cfg.cdims, dagger=dag)
+        assert np.array_equal(a, oracle.coarse_mult(up(xc32), up(A32), cfg.cdims, dagger=dag))
+        sites = np.array([3, 0, 15])
+        assert np.array_equal(oracle.coarse_mult_sites(xc32, A32[sites], cfg.cdims, sites, dagger=dag), a[sites])
+    assert np.array_equal(oracle.restrict(psi32, v32, cfg.dims, cfg.block), oracle.restrict(up(psi32), up(v32), cfg.dims, cfg.block))
+    assert np.array_equal(oracle.prolong(xc32, v32, cfg.dims, cfg.block), oracle.prolong(up(xc32), up(v32), cfg.dims, cfg.block))
+    assert np.array_equal(oracle.galerkin_coarse(U32, clov32, v32, cfg.kappa, cfg.dims, cfg.bc, cfg.block),
+                          oracle.galerkin_coarse(up(U32), up(clov32), up(v32), cfg.kappa, cfg.dims, cfg.bc, cfg.block))
+
+
+def test_oracle_rejects_bad_arguments(c1):
+    cfg = c1["cfg"]
+    with pytest.raises(ValueError):
+        oracle.wilson_clover_mult(c1["psi"][0], c1["U"], c1["clov"], cfg.kappa, cfg.dims, (1, 1, 1, 0))
+    with pytest.raises(ValueError):
+        oracle.restrict(c1["psi"][0], c1["v"], cfg.dims, (3, 2, 2, 2))
+    with pytest.raises(ValueError):
+        oracle.coarse_mult(np.zeros((4, 2, 2), dtype=np.complex128), np.zeros((4, 9, 4, 4), dtype=np.complex128), (1, 2, 2, 1))
