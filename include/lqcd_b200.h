@@ -1,0 +1,170 @@
+/*
+ * lqcd_b200.h -- C ABI of the B200 (sm_100a) hot path of arXiv:2111.05012:
+ * the Dirac-operator matrix-vector products of the multigrid-preconditioned solve.
+ *
+ * Citations are PAPER.md:<line> (the paper text) and SURVEY.md section 8 (the scope contract);
+ * every reading of a point the paper leaves open is listed in DESIGN.md "Readings".
+ *
+ * Conventions (the paper fixes none of them):
+ *   dims = {Lx, Ly, Lz, Lt}; mu = 0..3 <-> x, y, z, t (paper's mu = 1..4); sites 0-based;
+ *   canonical site index  s = x + Lx (y + Ly (z + Lz t)),  V = Lx Ly Lz Lt;
+ *   block b[4] divides dims; coarse dims Lc = dims / b (each >= 2); coarse site
+ *   X = Xx + Lcx (Xy + Lcy (Xz + Lcz Xt)), Vc = prod Lc; N = 2 nvec coarse dofs per coarse site,
+ *   coarse component  c = chi * nvec + i,  chi = alpha / 2 the chirality block of spin alpha.
+ *   Gamma matrices: chiral basis of DESIGN.md (gamma5 = -g1 g2 g3 g4 = diag(-1,-1,+1,+1), Eq. 2,
+ *   PAPER.md:54).  Complex numbers are interleaved (re, im).
+ *
+ * CANONICAL layouts (what the pack kernels read / unpack kernels write; x = fastest index last):
+ *   spinor      psi[s][alpha][c]                 V*12 complex
+ *   gauge       U[mu][s][a][b], (U psi)_a = sum_b U_ab psi_b     4*V*9 complex
+ *   clover      F[s][chi][k][l], k = 3*(alpha%2)+c, Hermitian 6x6 blocks       V*2*36 complex
+ *   null vecs   v[i][s][alpha][c]                nvec*V*12 complex
+ *   coarse vec  x[X][chi][i]                     Vc*N complex
+ *   coarse mat  A[X][d][row][col], d = 0 diag, 1+2mu forward, 2+2mu backward   Vc*9*N*N complex
+ *
+ * NATIVE layouts (what the mult kernels consume; sizes from lqcd_native_*_reals; R = real type,
+ * a "vec16" is 16 bytes = 4 floats or 2 doubles; sites are grouped in chunks of 32 canonical-
+ * consecutive sites, chunk = s / 32, lane = s % 32, nchunk = ceil(V / 32)):
+ *   spinor   [chunk][j][lane] vec16, j = 0..24/nv-1 over the 24 reals r = 2*(3 alpha + c) + reim
+ *   gauge18  [chunk][mu][18 reals as 18/nv full vec16 rows of 32 lanes, then (f32 only) one row of
+ *            32 float2 holding reals 16,17], reals r = 2*(3a+b)+reim
+ *   gauge12  [chunk][mu][j][lane] vec16 over the 12 reals of rows a = 0,1; the third row is rebuilt
+ *            in the kernel as conj(row0 x row1)
+ *   clover   [chunk][j][lane] vec16 over 72 reals: per chi 6 real diagonal entries then the 15
+ *            complex entries below the diagonal in row-major order (1,0),(2,0),(2,1),(3,0),...
+ *            (only the Hermitian part of the canonical input is kept)
+ *   null vecs [X][chi][i][l][k] complex, l = local site index inside the block (x fastest),
+ *            k = 3*(alpha%2)+c -- one contiguous (|block|*6)-complex vector per (X, chi, i)
+ *   coarse vec, coarse mat: identical to canonical.
+ *
+ * All pointers named *_dev / without suffix are DEVICE pointers owned by the caller and must be
+ * 16-byte aligned; *_host are HOST pointers.  No call allocates device memory, none keeps state
+ * beyond a thread-local error string and the tuning knobs below.  Every call enqueues its work on
+ * `stream` (a cudaStream_t passed as void*; NULL = legacy default stream) and returns without
+ * synchronising, except the *_host_* calls, which synchronise the stream before returning.
+ *
+ * Return value: 0 = LQCD_OK; negative = error and NOTHING was enqueued:
+ *   LQCD_EINVAL (-1)        null pointer, misaligned pointer, non-positive dim, block not dividing
+ *                           dims, coarse extent < 2, bc[mu] not in {+1,-1}, nvec < 1, out == in
+ *   LQCD_EUNSUPPORTED (-2)  size outside a kernel's compiled range
+ *   LQCD_ECUDA (-3)         the launch reported an error (text in lqcd_last_error())
+ * There is no CPU fallback and no other GPU architecture.
+ */
+#ifndef LQCD_B200_H
+#define LQCD_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LQCD_OK 0
+#define LQCD_EINVAL (-1)
+#define LQCD_EUNSUPPORTED (-2)
+#define LQCD_ECUDA (-3)
+
+/* flags */
+#define LQCD_DAGGER 1u   /* apply gamma5 D gamma5 = D^dag (Eq. 2) / Gamma5c D_c Gamma5c */
+#define LQCD_LINKS_12 2u /* U holds the 12-real compressed native gauge layout */
+
+/* ---- diagnostics ------------------------------------------------------------------------- */
+int lqcd_version(void);
+/* Text of the last error on this thread ("" if none).  Owned by the library. */
+const char* lqcd_last_error(void);
+/* Number of kernel launches this library has enqueued so far (all threads). */
+unsigned long long lqcd_launch_count(void);
+
+/* ---- tuning knobs (process-wide; defaults chosen for B200; results never depend on them) --- */
+/* Thread tile of the fine kernel: tile[mu] sites per CTA in direction mu, product <= 256,
+ * each dividing dims[mu] at call time (otherwise the call falls back to the automatic choice).
+ * tile = NULL or tile[0] = 0 restores the automatic choice. */
+int lqcd_set_fine_tile(const int tile[4]);
+/* Generic integer knob by name; returns LQCD_EINVAL for an unknown name. */
+int lqcd_set_knob(const char* name, int value);
+
+/* ---- native sizes, in reals of the precision in use -------------------------------------- */
+size_t lqcd_native_spinor_reals(const int dims[4]);
+size_t lqcd_native_gauge_reals(const int dims[4], unsigned flags /* LQCD_LINKS_12 or 0 */);
+size_t lqcd_native_clover_reals(const int dims[4]);
+size_t lqcd_native_nullvecs_reals(const int dims[4], const int block[4], int nvec);
+size_t lqcd_native_coarse_vec_reals(const int cdims[4], int nvec);
+size_t lqcd_native_coarse_mat_reals(const int cdims[4], int nvec);
+
+/* ---- layout helpers: device -> device re-layout kernels (not on the timed path) ---------- */
+int lqcd_pack_spinor_f32(float* dst_native, const float* src_canonical, const int dims[4], void* stream);
+int lqcd_pack_spinor_f64(double* dst_native, const double* src_canonical, const int dims[4], void* stream);
+int lqcd_unpack_spinor_f32(float* dst_canonical, const float* src_native, const int dims[4], void* stream);
+int lqcd_unpack_spinor_f64(double* dst_canonical, const double* src_native, const int dims[4], void* stream);
+/* flags: LQCD_LINKS_12 packs rows 0,1 only */
+int lqcd_pack_gauge_f32(float* dst_native, const float* src_canonical, const int dims[4], unsigned flags,
+                        void* stream);
+int lqcd_pack_gauge_f64(double* dst_native, const double* src_canonical, const int dims[4], unsigned flags,
+                        void* stream);
+int lqcd_pack_clover_f32(float* dst_native, const float* src_canonical, const int dims[4], void* stream);
+int lqcd_pack_clover_f64(double* dst_native, const double* src_canonical, const int dims[4], void* stream);
+/* Packs ONE canonical null vector v_i[s][alpha][c] into slot i of the native array (so that a
+ * 32-vector set never has to exist twice in HBM). */
+int lqcd_pack_nullvec_f32(float* dst_native, const float* src_canonical_vi, int i, const int dims[4],
+                          const int block[4], int nvec, void* stream);
+int lqcd_pack_nullvec_f64(double* dst_native, const double* src_canonical_vi, int i, const int dims[4],
+                          const int block[4], int nvec, void* stream);
+int lqcd_unpack_nullvec_f32(float* dst_canonical_vi, const float* src_native, int i, const int dims[4],
+                            const int block[4], int nvec, void* stream);
+int lqcd_unpack_nullvec_f64(double* dst_canonical_vi, const double* src_native, int i, const int dims[4],
+                            const int block[4], int nvec, void* stream);
+
+/* ---- A1 / A2: fine Wilson-clover operator, Eq. 1, dagger Eq. 2 ---
+ *   out(x) = in(x) + F(x) in(x)
+ *            - kappa sum_mu [ (1 - g_mu) U_mu(x) beta+ in(x+mu) + (1 + g_mu) U_mu^dag(x-mu) beta- in(x-mu) ]
+ * neighbours modulo dims (halo-free); beta+- = bc[mu] when the hop wraps around the lattice, else 1
+ * (psi(x + L_mu mu) = bc[mu] psi(x); "periodic or anti-periodic").
+ * out, in: native spinor; U: native gauge (18-real, or 12-real with LQCD_LINKS_12); clover: native
+ * clover.  out must not alias in.  flags: LQCD_DAGGER, LQCD_LINKS_12. */
+int lqcd_wilson_clover_mult_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
+                                const int dims[4], const int bc[4], unsigned flags, void* stream);
+int lqcd_wilson_clover_mult_f64(double* out, const double* in, const double* U, const double* clover,
+                                double kappa, const int dims[4], const int bc[4], unsigned flags, void* stream);
+
+/* ---- A3: coarse operator, Eqs. 4, 7 ---------------------------------------
+ *   out(X) = A[X][0] in(X) + sum_mu ( A[X][1+2mu] in(X+mu) + A[X][2+2mu] in(X-mu) ),
+ * neighbours modulo cdims, always periodic (boundary phases live inside A).  LQCD_DAGGER applies
+ * Gamma5c D_c Gamma5c, Gamma5c = diag(gamma5 sign of chi) (x) 1_nvec.  out must not alias in. */
+int lqcd_coarse_mult_f32(float* out, const float* in, const float* A, const int cdims[4], int nvec,
+                         unsigned flags, void* stream);
+int lqcd_coarse_mult_f64(double* out, const double* in, const double* A, const int cdims[4], int nvec,
+                         unsigned flags, void* stream);
+
+/* ---- A4: restriction, Eq. 5:  out_c[X][chi][i] = <v_i restricted to (X,chi) | in_f> -- */
+int lqcd_restrict_f32(float* out_c, const float* in_f, const float* nullvecs, const int dims[4],
+                      const int block[4], int nvec, void* stream);
+int lqcd_restrict_f64(double* out_c, const double* in_f, const double* nullvecs, const int dims[4],
+                      const int block[4], int nvec, void* stream);
+/* ---- A5: prolongation, Eq. 6:  out_f(x,alpha,c) = sum_i v_i(x,alpha,c) in_c[X(x)][chi(alpha)][i];
+ * overwrites out_f (no accumulate). */
+int lqcd_prolong_f32(float* out_f, const float* in_c, const float* nullvecs, const int dims[4],
+                     const int block[4], int nvec, void* stream);
+int lqcd_prolong_f64(double* out_f, const double* in_c, const double* nullvecs, const int dims[4],
+                     const int block[4], int nvec, void* stream);
+
+/* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
+ * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
+ * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned
+ * memory recommended).  Each call: cudaMemcpyAsync H2D -> pack -> the mult kernel -> unpack ->
+ * cudaMemcpyAsync D2H -> cudaStreamSynchronize.  ws_dev is caller-owned device scratch of at least
+ * lqcd_host_workspace_bytes(...) bytes. */
+size_t lqcd_host_workspace_bytes(const int dims[4], const int block[4], int nvec);
+int lqcd_wilson_clover_mult_host_f32(float* out_host, const float* in_host, const float* U, const float* clover,
+                                     float kappa, const int dims[4], const int bc[4], unsigned flags,
+                                     void* ws_dev, void* stream);
+int lqcd_coarse_mult_host_f32(float* out_host, const float* in_host, const float* A, const int cdims[4],
+                              int nvec, unsigned flags, void* ws_dev, void* stream);
+int lqcd_restrict_host_f32(float* out_c_host, const float* in_f_host, const float* nullvecs, const int dims[4],
+                           const int block[4], int nvec, void* ws_dev, void* stream);
+int lqcd_prolong_host_f32(float* out_f_host, const float* in_c_host, const float* nullvecs, const int dims[4],
+                          const int block[4], int nvec, void* ws_dev, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_B200_H */

@@ -1,0 +1,268 @@
+"""paper_2111_05012_b200 -- thin Python binding of the C ABI in include/lqcd_b200.h.
+
+B200 (sm_100a) hot path of arXiv:2111.05012: fine Wilson-clover operator (Eq. 1) and its
+gamma5-conjugate (Eq. 2), coarse 9-point block operator (Eqs. 4, 7),
+restriction / prolongation (Eqs. 5, 6).  Functions have the names of the C entry points
+without the `lqcd_` prefix and the precision suffix (picked from the tensor dtype).  This module marshals
+arguments only: every step runs in the CUDA kernels of csrc/.  torch supplies device memory and streams.
+There is no CPU fallback; nothing here imports oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import torch
+
+from . import _lib
+from ._lib import c_int4
+
+DAGGER = 1
+LINKS_12 = 2
+
+OK, EINVAL, EUNSUPPORTED, ECUDA = 0, -1, -2, -3
+
+
+class LqcdError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        self.code = code
+        msg = _lib.load().lqcd_last_error().decode()
+        super().__init__(f"{what} failed with code {code}: {msg}")
+
+
+def lib():
+    return _lib.load()
+
+
+def _i4(a):
+    return c_int4(*[int(v) for v in a])
+
+
+def _sfx(t: torch.Tensor) -> str:
+    if t.dtype in (torch.float32, torch.complex64):
+        return "f32"
+    if t.dtype in (torch.float64, torch.complex128):
+        return "f64"
+    raise TypeError(f"unsupported dtype {t.dtype}")
+
+
+def _real(t: torch.Tensor) -> torch.Tensor:
+    """Real view of a contiguous real or complex tensor (no copy)."""
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    return torch.view_as_real(t) if t.is_complex() else t
+
+
+def _dev_ptr(t: torch.Tensor):
+    if not t.is_cuda:
+        raise ValueError("expected a CUDA tensor (there is no CPU path)")
+    return C.c_void_p(_real(t).data_ptr())
+
+
+def _host_ptr(t: torch.Tensor):
+    if t.is_cuda:
+        raise ValueError("expected a host tensor")
+    return C.c_void_p(_real(t).data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise LqcdError(rc, what)
+
+
+def _same_dtype(*ts):
+    sf = {_sfx(t) for t in ts}
+    if len(sf) != 1:
+        raise TypeError("all tensors of one call must share one precision")
+    return sf.pop()
+
+
+def _rdtype(sfx: str):
+    return torch.float32 if sfx == "f32" else torch.float64
+
+
+# ---- diagnostics / knobs ---------------------------------------------------------------------------
+def version() -> int:
+    return lib().lqcd_version()
+
+
+def last_error() -> str:
+    return lib().lqcd_last_error().decode()
+
+
+def launch_count() -> int:
+    return int(lib().lqcd_launch_count())
+
+
+def set_fine_tile(tile=None):
+    _check(lib().lqcd_set_fine_tile(_i4(tile) if tile is not None else None), "lqcd_set_fine_tile")
+
+
+def set_knob(name: str, value: int):
+    _check(lib().lqcd_set_knob(name.encode(), int(value)), "lqcd_set_knob")
+
+
+# ---- native sizes ------------------------------------------------------------------------------------
+def native_spinor_reals(dims) -> int:
+    return int(lib().lqcd_native_spinor_reals(_i4(dims)))
+
+
+def native_gauge_reals(dims, links12=False) -> int:
+    return int(lib().lqcd_native_gauge_reals(_i4(dims), LINKS_12 if links12 else 0))
+
+
+def native_clover_reals(dims) -> int:
+    return int(lib().lqcd_native_clover_reals(_i4(dims)))
+
+
+def native_nullvecs_reals(dims, block, nvec) -> int:
+    return int(lib().lqcd_native_nullvecs_reals(_i4(dims), _i4(block), int(nvec)))
+
+
+def native_coarse_vec_reals(cdims, nvec) -> int:
+    return int(lib().lqcd_native_coarse_vec_reals(_i4(cdims), int(nvec)))
+
+
+def native_coarse_mat_reals(cdims, nvec) -> int:
+    return int(lib().lqcd_native_coarse_mat_reals(_i4(cdims), int(nvec)))
+
+
+def host_workspace_bytes(dims, block, nvec) -> int:
+    return int(lib().lqcd_host_workspace_bytes(_i4(dims), _i4(block), int(nvec)))
+
+
+def empty_spinor(dims, dtype=torch.float32, device="cuda") -> torch.Tensor:
+    return torch.zeros(native_spinor_reals(dims), dtype=dtype, device=device)
+
+
+# ---- layout helpers (allocate the destination, then one C call) ------------------------------------------
+def pack_spinor(src: torch.Tensor, dims, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    sfx = _sfx(src)
+    dst = out if out is not None else torch.zeros(native_spinor_reals(dims), dtype=_rdtype(sfx), device=src.device)
+    _check(getattr(lib(), f"lqcd_pack_spinor_{sfx}")(_dev_ptr(dst), _dev_ptr(src), _i4(dims), _stream(stream)),
+           "lqcd_pack_spinor")
+    return dst
+
+
+def unpack_spinor(src: torch.Tensor, dims, stream=None) -> torch.Tensor:
+    """native -> canonical complex tensor of shape (V, 4, 3)"""
+    sfx = _sfx(src)
+    v = 1
+    for d in dims:
+        v *= int(d)
+    dst = torch.empty((v, 4, 3, 2), dtype=_rdtype(sfx), device=src.device)
+    _check(getattr(lib(), f"lqcd_unpack_spinor_{sfx}")(_dev_ptr(dst), _dev_ptr(src), _i4(dims), _stream(stream)),
+           "lqcd_unpack_spinor")
+    return torch.view_as_complex(dst)
+
+
+def pack_gauge(src: torch.Tensor, dims, links12=False, stream=None) -> torch.Tensor:
+    sfx = _sfx(src)
+    dst = torch.zeros(native_gauge_reals(dims, links12), dtype=_rdtype(sfx), device=src.device)
+    _check(getattr(lib(), f"lqcd_pack_gauge_{sfx}")(_dev_ptr(dst), _dev_ptr(src), _i4(dims),
+                                                    LINKS_12 if links12 else 0, _stream(stream)), "lqcd_pack_gauge")
+    return dst
+
+
+def pack_clover(src: torch.Tensor, dims, stream=None) -> torch.Tensor:
+    sfx = _sfx(src)
+    dst = torch.zeros(native_clover_reals(dims), dtype=_rdtype(sfx), device=src.device)
+    _check(getattr(lib(), f"lqcd_pack_clover_{sfx}")(_dev_ptr(dst), _dev_ptr(src), _i4(dims), _stream(stream)),
+           "lqcd_pack_clover")
+    return dst
+
+
+def pack_nullvec(dst: torch.Tensor, src_vi: torch.Tensor, i: int, dims, block, nvec, stream=None):
+    sfx = _same_dtype(dst, src_vi)
+    _check(getattr(lib(), f"lqcd_pack_nullvec_{sfx}")(_dev_ptr(dst), _dev_ptr(src_vi), int(i), _i4(dims), _i4(block),
+                                                      int(nvec), _stream(stream)), "lqcd_pack_nullvec")
+
+
+def unpack_nullvec(src_native: torch.Tensor, i: int, dims, block, nvec, stream=None) -> torch.Tensor:
+    sfx = _sfx(src_native)
+    v = 1
+    for d in dims:
+        v *= int(d)
+    dst = torch.empty((v, 4, 3, 2), dtype=_rdtype(sfx), device=src_native.device)
+    _check(getattr(lib(), f"lqcd_unpack_nullvec_{sfx}")(_dev_ptr(dst), _dev_ptr(src_native), int(i), _i4(dims),
+                                                        _i4(block), int(nvec), _stream(stream)), "lqcd_unpack_nullvec")
+    return torch.view_as_complex(dst)
+
+
+def pack_nullvecs(v: torch.Tensor, dims, block) -> torch.Tensor:
+    """canonical (nvec, V, 4, 3) complex -> native; one lqcd_pack_nullvec call per vector."""
+    sfx = _sfx(v)
+    nvec = v.shape[0]
+    dst = torch.zeros(native_nullvecs_reals(dims, block, nvec), dtype=_rdtype(sfx), device=v.device)
+    for i in range(nvec):
+        pack_nullvec(dst, v[i], i, dims, block, nvec)
+    return dst
+
+
+# ---- the hot path -------------------------------------------------------------------------------------
+def wilson_clover_mult(out, inp, U, clover, kappa, dims, bc, dagger=False, links12=False, stream=None):
+    """A1/A2: out = D in (or D^dag in), Eq. 1 / Eq. 2; all tensors native layout."""
+    sfx = _same_dtype(out, inp, U, clover)
+    flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_wilson_clover_mult_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(U), _dev_ptr(clover),
+                                                            k, _i4(dims), _i4(bc), flags, _stream(stream)),
+           "lqcd_wilson_clover_mult")
+    return out
+
+
+def coarse_mult(out, inp, A, cdims, nvec, dagger=False, stream=None):
+    """A3: out = D_c in, Eqs. 4, 7."""
+    sfx = _same_dtype(out, inp, A)
+    _check(getattr(lib(), f"lqcd_coarse_mult_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(A), _i4(cdims), int(nvec),
+                                                     DAGGER if dagger else 0, _stream(stream)), "lqcd_coarse_mult")
+    return out
+
+
+def restrict(out_c, in_f, nullvecs, dims, block, nvec, stream=None):
+    """A4: Eq. 5.  (`restrict` is the paper's name; it shadows nothing in Python.)"""
+    sfx = _same_dtype(out_c, in_f, nullvecs)
+    _check(getattr(lib(), f"lqcd_restrict_{sfx}")(_dev_ptr(out_c), _dev_ptr(in_f), _dev_ptr(nullvecs), _i4(dims),
+                                                  _i4(block), int(nvec), _stream(stream)), "lqcd_restrict")
+    return out_c
+
+
+def prolong(out_f, in_c, nullvecs, dims, block, nvec, stream=None):
+    """A5: Eq. 6."""
+    sfx = _same_dtype(out_f, in_c, nullvecs)
+    _check(getattr(lib(), f"lqcd_prolong_{sfx}")(_dev_ptr(out_f), _dev_ptr(in_c), _dev_ptr(nullvecs), _i4(dims),
+                                                 _i4(block), int(nvec), _stream(stream)), "lqcd_prolong")
+    return out_f
+
+
+# ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
+def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
+                            stream=None):
+    flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)
+    _check(lib().lqcd_wilson_clover_mult_host_f32(_host_ptr(out_host), _host_ptr(in_host), _dev_ptr(U),
+                                                  _dev_ptr(clover), C.c_float(kappa), _i4(dims), _i4(bc), flags,
+                                                  _dev_ptr(ws), _stream(stream)), "lqcd_wilson_clover_mult_host_f32")
+    return out_host
+
+
+def coarse_mult_host(out_host, in_host, A, cdims, nvec, ws, dagger=False, stream=None):
+    _check(lib().lqcd_coarse_mult_host_f32(_host_ptr(out_host), _host_ptr(in_host), _dev_ptr(A), _i4(cdims), int(nvec),
+                                           DAGGER if dagger else 0, _dev_ptr(ws), _stream(stream)),
+           "lqcd_coarse_mult_host_f32")
+    return out_host
+
+
+def restrict_host(out_c_host, in_f_host, nullvecs, dims, block, nvec, ws, stream=None):
+    _check(lib().lqcd_restrict_host_f32(_host_ptr(out_c_host), _host_ptr(in_f_host), _dev_ptr(nullvecs), _i4(dims),
+                                        _i4(block), int(nvec), _dev_ptr(ws), _stream(stream)), "lqcd_restrict_host_f32")
+    return out_c_host
+
+
+def prolong_host(out_f_host, in_c_host, nullvecs, dims, block, nvec, ws, stream=None):
+    _check(lib().lqcd_prolong_host_f32(_host_ptr(out_f_host), _host_ptr(in_c_host), _dev_ptr(nullvecs), _i4(dims),
+                                       _i4(block), int(nvec), _dev_ptr(ws), _stream(stream)), "lqcd_prolong_host_f32")
+    return out_f_host

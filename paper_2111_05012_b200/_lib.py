@@ -1,0 +1,77 @@
+"""ctypes loader for liblqcd_b200.so (the C ABI of include/lqcd_b200.h).
+
+There is no CPU fallback: if the library is missing and cannot be built with nvcc, loading raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from . import build as _build
+
+_lib = None
+
+c_int4 = C.c_int * 4
+_vp, _ci, _cu, _cf, _cd = C.c_void_p, C.c_int, C.c_uint, C.c_float, C.c_double
+_i4 = C.POINTER(C.c_int)
+
+# name -> (restype, argtypes); every symbol include/lqcd_b200.h declares
+SIGNATURES = {
+    "lqcd_version": (_ci, []),
+    "lqcd_last_error": (C.c_char_p, []),
+    "lqcd_launch_count": (C.c_ulonglong, []),
+    "lqcd_set_fine_tile": (_ci, [_i4]),
+    "lqcd_set_knob": (_ci, [C.c_char_p, _ci]),
+    "lqcd_native_spinor_reals": (C.c_size_t, [_i4]),
+    "lqcd_native_gauge_reals": (C.c_size_t, [_i4, _cu]),
+    "lqcd_native_clover_reals": (C.c_size_t, [_i4]),
+    "lqcd_native_nullvecs_reals": (C.c_size_t, [_i4, _i4, _ci]),
+    "lqcd_native_coarse_vec_reals": (C.c_size_t, [_i4, _ci]),
+    "lqcd_native_coarse_mat_reals": (C.c_size_t, [_i4, _ci]),
+    "lqcd_host_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
+}
+for _p, _k in (("f32", _cf), ("f64", _cd)):
+    SIGNATURES.update({
+        f"lqcd_pack_spinor_{_p}": (_ci, [_vp, _vp, _i4, _vp]),
+        f"lqcd_unpack_spinor_{_p}": (_ci, [_vp, _vp, _i4, _vp]),
+        f"lqcd_pack_gauge_{_p}": (_ci, [_vp, _vp, _i4, _cu, _vp]),
+        f"lqcd_pack_clover_{_p}": (_ci, [_vp, _vp, _i4, _vp]),
+        f"lqcd_pack_nullvec_{_p}": (_ci, [_vp, _vp, _ci, _i4, _i4, _ci, _vp]),
+        f"lqcd_unpack_nullvec_{_p}": (_ci, [_vp, _vp, _ci, _i4, _i4, _ci, _vp]),
+        f"lqcd_wilson_clover_mult_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _vp]),
+        f"lqcd_coarse_mult_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _vp]),
+        f"lqcd_restrict_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp]),
+        f"lqcd_prolong_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp]),
+    })
+SIGNATURES.update({
+    "lqcd_wilson_clover_mult_host_f32": (_ci, [_vp, _vp, _vp, _vp, _cf, _i4, _i4, _cu, _vp, _vp]),
+    "lqcd_coarse_mult_host_f32": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _vp, _vp]),
+    "lqcd_restrict_host_f32": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp, _vp]),
+    "lqcd_prolong_host_f32": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp, _vp]),
+})
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load():
+    """Load (building first if the sources are newer and nvcc is present) and type every entry point."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.stale():
+        try:
+            _build.build()
+        except Exception as e:  # no nvcc on this box
+            if not os.path.exists(path):
+                raise RuntimeError(
+                    f"liblqcd_b200.so is missing and could not be built ({e}); there is no CPU fallback") from e
+    lib = C.CDLL(path)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(lib, name)  # AttributeError if the header and the library disagree
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib

@@ -1,0 +1,112 @@
+// common.cuh -- shared plumbing of the sm_100a kernels: error reporting, argument checks,
+// the 16-byte vector type per precision, cache-hinted loads/stores, lattice geometry.
+// Product code: never includes or links anything under oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdarg.h>
+
+#include "../../include/lqcd_b200.h"
+
+namespace lqcd {
+
+constexpr int CH = 32;  // sites per native chunk (one warp-wide row of vec16)
+
+// ---- error reporting -------------------------------------------------------------------------
+void set_error(const char* fmt, ...);
+void clear_error();
+void count_launch(int n = 1);
+int check_launch(const char* what);  // cudaGetLastError -> LQCD_ECUDA / LQCD_OK
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+inline int check_dims(const int dims[4]) {
+    if (!dims) return LQCD_EINVAL;
+    for (int mu = 0; mu < 4; mu++)
+        if (dims[mu] < 1) return LQCD_EINVAL;
+    return LQCD_OK;
+}
+inline long long volume(const int d[4]) { return (long long)d[0] * d[1] * d[2] * d[3]; }
+inline long long nchunks(const int d[4]) { return (volume(d) + CH - 1) / CH; }
+
+// block must divide dims, coarse extents >= 2 (reading Q8)
+inline int check_block(const int dims[4], const int block[4], int nvec, int cdims[4]) {
+    if (check_dims(dims) || !block || nvec < 1) return LQCD_EINVAL;
+    for (int mu = 0; mu < 4; mu++) {
+        if (block[mu] < 1 || dims[mu] % block[mu]) return LQCD_EINVAL;
+        cdims[mu] = dims[mu] / block[mu];
+        if (cdims[mu] < 2) return LQCD_EINVAL;
+    }
+    return LQCD_OK;
+}
+
+// ---- 16-byte vectors ----------------------------------------------------------------------------
+template <typename T> struct VecOf;
+template <> struct VecOf<float> {
+    typedef float4 type;
+    static constexpr int NV = 4;
+};
+template <> struct VecOf<double> {
+    typedef double2 type;
+    static constexpr int NV = 2;
+};
+
+// A 16-byte register bundle addressable by compile-time index.
+template <typename T> struct V16;
+template <> struct alignas(16) V16<float> {
+    float r[4];
+};
+template <> struct alignas(16) V16<double> {
+    double r[2];
+};
+
+// Default-cached 128-bit load (L1 + L2): data with reuse (spinors, links).
+template <typename T> __device__ __forceinline__ V16<T> ld16(const T* p) {
+    return *reinterpret_cast<const V16<T>*>(p);
+}
+// Read-only, L1 no-allocate, L2 evict-first: data streamed exactly once (clover, coarse blocks, null vectors).
+// (The plain .L2::evict_first qualifier exists only for 256-bit loads on sm_100a, hence the policy operand;
+// createpolicy is loop-invariant and gets hoisted.)
+template <typename T> __device__ __forceinline__ V16<T> ld16_stream(const T* p);
+__device__ __forceinline__ uint64_t evict_first_policy() {
+    uint64_t pol;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+template <> __device__ __forceinline__ V16<float> ld16_stream<float>(const float* p) {
+    V16<float> v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=f"(v.r[0]), "=f"(v.r[1]), "=f"(v.r[2]), "=f"(v.r[3])
+                 : "l"(p), "l"(evict_first_policy()));
+    return v;
+}
+template <> __device__ __forceinline__ V16<double> ld16_stream<double>(const double* p) {
+    V16<double> v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
+                 : "=d"(v.r[0]), "=d"(v.r[1])
+                 : "l"(p), "l"(evict_first_policy()));
+    return v;
+}
+// Streaming store (written once, not re-read by this kernel).
+template <typename T> __device__ __forceinline__ void st16_stream(T* p, const V16<T>& v);
+template <> __device__ __forceinline__ void st16_stream<float>(float* p, const V16<float>& v) {
+    asm volatile("st.global.cs.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(v.r[0]), "f"(v.r[1]), "f"(v.r[2]),
+                 "f"(v.r[3])
+                 : "memory");
+}
+template <> __device__ __forceinline__ void st16_stream<double>(double* p, const V16<double>& v) {
+    asm volatile("st.global.cs.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(v.r[0]), "d"(v.r[1]) : "memory");
+}
+template <typename T> __device__ __forceinline__ void st16(T* p, const V16<T>& v) {
+    *reinterpret_cast<V16<T>*>(p) = v;
+}
+
+// ---- geometry passed to kernels by value ---------------------------------------------------------
+struct Geom {
+    int L[4];        // fine dims
+    int V;           // volume (fits in int: the largest supported lattice is < 2^31 sites)
+};
+
+}  // namespace lqcd

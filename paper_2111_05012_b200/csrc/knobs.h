@@ -1,0 +1,13 @@
+// knobs.h -- process-wide tuning knobs (lqcd_set_fine_tile / lqcd_set_knob). Results never depend on them.
+#pragma once
+namespace lqcd {
+struct Knobs {
+    int fine_tile[4] = {0, 0, 0, 0};  // 0 = automatic
+    int fine_variant = 0;             // 0 = automatic choice of fine-kernel variant
+    int fine_tslab = 0;               // 0 = automatic; >0 = z-extent of the traversal slab
+    int coarse_rows_per_warp = 0;     // 0 = automatic
+    int coarse_warps = 0;             // warps per CTA of the coarse kernel, 0 = automatic
+    int transfer_warps = 0;           // warps per CTA of restrict, 0 = automatic
+};
+extern Knobs g_knobs;
+}  // namespace lqcd

@@ -1,0 +1,249 @@
+// transfer.cu -- rows A4/A5 of the hot path: block restriction and prolongation with chirality-split null
+// vectors (Eqs. 5, 6):
+//   restrict:  out_c[X][chi][i]    = sum_{x in X} sum_{alpha in chi, c} conj(v_i(x,alpha,c)) in_f(x,alpha,c)
+//   prolong:   out_f(x,alpha,c)    = sum_i v_i(x,alpha,c) in_c[X(x)][chi(alpha)][i]
+//
+// Design: both are a single pass over the null vectors (nvec*96 B per fine site
+// in fp32 -- 97% of the traffic), so the native null-vector layout [X][chi][i][l][k] makes the part of v_i
+// that belongs to one aggregate (X, chi) ONE contiguous vector of |block|*6 complex, read with full-width
+// 128-bit coalesced, L1::no_allocate / L2 evict-first loads by both kernels.  One CTA per aggregate (X, chi):
+//   restrict: the aggregate's slice of in_f is staged once in shared memory; each warp owns null vectors
+//             i = w, w+W, ... and finishes its dot product with a warp-shuffle tree (fixed order, no atomics);
+//   prolong:  the nvec coarse coefficients sit in shared memory; each thread owns 16-byte slices of the
+//             aggregate and accumulates over i, no reduction across threads.
+// The paper's GPU version bounced these two steps through the host; here they stay on the device.
+#include "common.cuh"
+#include "knobs.h"
+
+namespace lqcd {
+
+struct TransferParams {
+    int L[4], b[4], Lc[4];
+    int bv;    // sites per block
+    int nvec;
+    int LV;    // vec16 per (X, chi, i) vector = bv * 12 / NV
+};
+
+// canonical fine site of local index l inside coarse site X
+__device__ __forceinline__ int fine_site(const TransferParams& P, int X, int l) {
+    int s = 0, stride = 1;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        const int Xmu = X % P.Lc[mu];
+        X /= P.Lc[mu];
+        const int lmu = l % P.b[mu];
+        l /= P.b[mu];
+        s += (Xmu * P.b[mu] + lmu) * stride;
+        stride *= P.L[mu];
+    }
+    return s;
+}
+
+template <typename T> __device__ __forceinline__ void cdot_acc(T& sr, T& si, const V16<T>& a, const V16<T>& x);
+// sum conj(a) x over the complex entries of one vec16
+template <> __device__ __forceinline__ void cdot_acc<float>(float& sr, float& si, const V16<float>& a,
+                                                            const V16<float>& x) {
+    sr = fmaf(a.r[0], x.r[0], sr);
+    sr = fmaf(a.r[1], x.r[1], sr);
+    si = fmaf(a.r[0], x.r[1], si);
+    si = fmaf(-a.r[1], x.r[0], si);
+    sr = fmaf(a.r[2], x.r[2], sr);
+    sr = fmaf(a.r[3], x.r[3], sr);
+    si = fmaf(a.r[2], x.r[3], si);
+    si = fmaf(-a.r[3], x.r[2], si);
+}
+template <> __device__ __forceinline__ void cdot_acc<double>(double& sr, double& si, const V16<double>& a,
+                                                             const V16<double>& x) {
+    sr = fma(a.r[0], x.r[0], sr);
+    sr = fma(a.r[1], x.r[1], sr);
+    si = fma(a.r[0], x.r[1], si);
+    si = fma(-a.r[1], x.r[0], si);
+}
+
+// acc += a * (cr + i ci) for each complex entry of the vec16
+template <typename T> __device__ __forceinline__ void caxpy(V16<T>& acc, const V16<T>& a, T cr, T ci) {
+    constexpr int NV = VecOf<T>::NV;
+#pragma unroll
+    for (int e = 0; e < NV / 2; e++) {
+        acc.r[2 * e] = fma(a.r[2 * e], cr, acc.r[2 * e]);
+        acc.r[2 * e] = fma(-a.r[2 * e + 1], ci, acc.r[2 * e]);
+        acc.r[2 * e + 1] = fma(a.r[2 * e], ci, acc.r[2 * e + 1]);
+        acc.r[2 * e + 1] = fma(a.r[2 * e + 1], cr, acc.r[2 * e + 1]);
+    }
+}
+
+template <typename T, int UNROLL>
+__global__ void __launch_bounds__(256) k_restrict(T* __restrict__ out_c, const T* __restrict__ in_f,
+                                                  const T* __restrict__ v, TransferParams P) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, JH = 12 / NV;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sm = reinterpret_cast<T*>(smem_raw);  // [l][12 reals of chirality chi]
+    const int agg = blockIdx.x;              // (X, chi)
+    const int X = agg >> 1, chi = agg & 1;
+    // stage the aggregate's slice of in_f
+    for (int idx = threadIdx.x; idx < P.LV; idx += blockDim.x) {
+        const int l = idx / JH, jj = idx % JH;
+        const int s = fine_site(P, X, l);
+        const T* src = in_f + (((long long)(s >> 5) * NJ + chi * JH + jj) * CH + (s & 31)) * NV;
+        st16(sm + (long long)idx * NV, ld16(src));
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, W = blockDim.x >> 5;
+    const T* vagg = v + (long long)agg * P.nvec * P.LV * NV;
+    for (int i = w; i < P.nvec; i += W) {
+        const T* vi = vagg + (long long)i * P.LV * NV;
+        T sr[UNROLL], si[UNROLL];
+#pragma unroll
+        for (int u = 0; u < UNROLL; u++) sr[u] = si[u] = 0;
+        int p = lane;
+        for (; p + 32 * (UNROLL - 1) < P.LV; p += 32 * UNROLL) {
+            V16<T> a[UNROLL];
+#pragma unroll
+            for (int u = 0; u < UNROLL; u++) a[u] = ld16_stream(vi + (long long)(p + 32 * u) * NV);
+#pragma unroll
+            for (int u = 0; u < UNROLL; u++)
+                cdot_acc<T>(sr[u], si[u], a[u], *reinterpret_cast<const V16<T>*>(sm + (p + 32 * u) * NV));
+        }
+        for (; p < P.LV; p += 32)
+            cdot_acc<T>(sr[0], si[0], ld16_stream(vi + (long long)p * NV), *reinterpret_cast<const V16<T>*>(sm + p * NV));
+        T tr = 0, ti = 0;
+#pragma unroll
+        for (int u = 0; u < UNROLL; u++) {
+            tr += sr[u];
+            ti += si[u];
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            tr += __shfl_xor_sync(0xffffffffu, tr, off);
+            ti += __shfl_xor_sync(0xffffffffu, ti, off);
+        }
+        if (lane == 0) {
+            T* o = out_c + ((long long)agg * P.nvec + i) * 2;
+            o[0] = tr;
+            o[1] = ti;
+        }
+    }
+}
+
+template <typename T, int UNROLL>
+__global__ void __launch_bounds__(256) k_prolong(T* __restrict__ out_f, const T* __restrict__ in_c,
+                                                 const T* __restrict__ v, TransferParams P) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, JH = 12 / NV;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* xc = reinterpret_cast<T*>(smem_raw);  // nvec complex
+    const int agg = blockIdx.x;
+    const int X = agg >> 1, chi = agg & 1;
+    for (int i = threadIdx.x; i < 2 * P.nvec; i += blockDim.x) xc[i] = in_c[(long long)agg * P.nvec * 2 + i];
+    __syncthreads();
+    const T* vagg = v + (long long)agg * P.nvec * P.LV * NV;
+    for (int p = threadIdx.x; p < P.LV; p += blockDim.x) {
+        V16<T> acc;
+#pragma unroll
+        for (int e = 0; e < NV; e++) acc.r[e] = 0;
+        const T* vp = vagg + (long long)p * NV;
+        int i = 0;
+        for (; i + UNROLL <= P.nvec; i += UNROLL) {
+            V16<T> a[UNROLL];
+#pragma unroll
+            for (int u = 0; u < UNROLL; u++) a[u] = ld16_stream(vp + (long long)(i + u) * P.LV * NV);
+#pragma unroll
+            for (int u = 0; u < UNROLL; u++) caxpy<T>(acc, a[u], xc[2 * (i + u)], xc[2 * (i + u) + 1]);
+        }
+        for (; i < P.nvec; i++) caxpy<T>(acc, ld16_stream(vp + (long long)i * P.LV * NV), xc[2 * i], xc[2 * i + 1]);
+        const int l = p / JH, jj = p % JH;
+        const int s = fine_site(P, X, l);
+        T* dst = out_f + (((long long)(s >> 5) * NJ + chi * JH + jj) * CH + (s & 31)) * NV;
+        st16_stream(dst, acc);
+    }
+}
+
+template <typename T>
+static int transfer_setup(TransferParams& P, const void* a, const void* b, const void* c, const int dims[4],
+                          const int block[4], int nvec, const char* what) {
+    clear_error();
+    if (!a || !b || !c) {
+        set_error("%s: null pointer", what);
+        return LQCD_EINVAL;
+    }
+    if (!aligned16(a) || !aligned16(b) || !aligned16(c)) {
+        set_error("%s: pointers must be 16-byte aligned", what);
+        return LQCD_EINVAL;
+    }
+    if (check_block(dims, block, nvec, P.Lc)) {
+        set_error("%s: bad dims/block/nvec (block must divide dims, coarse extents >= 2, nvec >= 1)", what);
+        return LQCD_EINVAL;
+    }
+    if (volume(dims) > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
+    P.bv = 1;
+    for (int mu = 0; mu < 4; mu++) {
+        P.L[mu] = dims[mu];
+        P.b[mu] = block[mu];
+        P.bv *= block[mu];
+    }
+    P.nvec = nvec;
+    P.LV = P.bv * 12 / VecOf<T>::NV;
+    return LQCD_OK;
+}
+
+template <typename T>
+static int restrict_call(T* out_c, const T* in_f, const T* v, const int dims[4], const int block[4], int nvec,
+                         void* stream, const char* what) {
+    TransferParams P;
+    int rc = transfer_setup<T>(P, out_c, in_f, v, dims, block, nvec, what);
+    if (rc) return rc;
+    const size_t smem = (size_t)P.bv * 12 * sizeof(T);
+    if (smem > 200 * 1024) {
+        set_error("%s: block of %d sites does not fit in shared memory", what, P.bv);
+        return LQCD_EUNSUPPORTED;
+    }
+    auto kern = k_restrict<T, 8>;
+    if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    int warps = g_knobs.transfer_warps > 0 ? g_knobs.transfer_warps : 8;
+    if (warps > 8) warps = 8;
+    if (warps > nvec) warps = nvec;
+    const long long nagg = 2 * volume(P.Lc);
+    kern<<<(unsigned)nagg, warps * 32, smem, (cudaStream_t)stream>>>(out_c, in_f, v, P);
+    count_launch();
+    return check_launch(what);
+}
+
+template <typename T>
+static int prolong_call(T* out_f, const T* in_c, const T* v, const int dims[4], const int block[4], int nvec,
+                        void* stream, const char* what) {
+    TransferParams P;
+    int rc = transfer_setup<T>(P, out_f, in_c, v, dims, block, nvec, what);
+    if (rc) return rc;
+    const size_t smem = (size_t)nvec * 2 * sizeof(T);
+    if (smem > 48 * 1024) {
+        set_error("%s: nvec = %d outside the compiled range", what, nvec);
+        return LQCD_EUNSUPPORTED;
+    }
+    int threads = P.LV >= 256 ? 256 : (P.LV + 31) / 32 * 32;
+    const long long nagg = 2 * volume(P.Lc);
+    k_prolong<T, 8><<<(unsigned)nagg, threads, smem, (cudaStream_t)stream>>>(out_f, in_c, v, P);
+    count_launch();
+    return check_launch(what);
+}
+
+}  // namespace lqcd
+
+using namespace lqcd;
+
+extern "C" {
+int lqcd_restrict_f32(float* o, const float* i, const float* v, const int dims[4], const int block[4], int nvec,
+                      void* st) {
+    return restrict_call<float>(o, i, v, dims, block, nvec, st, "lqcd_restrict_f32");
+}
+int lqcd_restrict_f64(double* o, const double* i, const double* v, const int dims[4], const int block[4], int nvec,
+                      void* st) {
+    return restrict_call<double>(o, i, v, dims, block, nvec, st, "lqcd_restrict_f64");
+}
+int lqcd_prolong_f32(float* o, const float* i, const float* v, const int dims[4], const int block[4], int nvec,
+                     void* st) {
+    return prolong_call<float>(o, i, v, dims, block, nvec, st, "lqcd_prolong_f32");
+}
+int lqcd_prolong_f64(double* o, const double* i, const double* v, const int dims[4], const int block[4], int nvec,
+                     void* st) {
+    return prolong_call<double>(o, i, v, dims, block, nvec, st, "lqcd_prolong_f64");
+}
+}

@@ -1,0 +1,432 @@
+// wilson_clover.cu -- rows A1/A2 of the hot path: the fine-lattice Wilson-clover operator,
+//   out(x) = in(x) + F(x) in(x) - kappa sum_mu [ (1 - g_mu) U_mu(x) in(x+mu) + (1 + g_mu) U_mu^dag(x-mu) in(x-mu) ]
+// (Eq. 1) and its gamma5-conjugate D^dag = gamma5 D gamma5 (Eq. 2).
+//
+// Design: one thread per lattice site (as the paper's GPU mapping),
+// but each CTA owns a compact 4-D tile of sites so that most neighbour spinors and backward links are
+// served by L1/L2 rather than HBM; native chunk-of-32 SoA layouts give 128-bit fully coalesced accesses;
+// the clover term and the output are streamed with evict-first / streaming hints so that they do not
+// displace the spinor and link lines that still have reuse; halo-free neighbour indexing modulo L with the
+// boundary phase bc[mu] applied on hops that wrap.  Spin projection uses the rank-2 structure of
+// (1 -+ g_mu) in the chiral basis: only two colour vectors per hop are multiplied by the link.
+// The dagger variant swaps the two projectors (gamma5 (1 -+ g_mu) gamma5 = (1 +- g_mu), [F, gamma5] = 0),
+// so it costs exactly the same traffic and arithmetic.
+#include "common.cuh"
+#include "knobs.h"
+#include "layout.cuh"
+
+namespace lqcd {
+
+struct FineParams {
+    int L[4];      // lattice extents
+    int tile[4];   // sites per CTA per direction
+    int ntile[4];  // tiles per direction
+    int bc[4];     // +1 / -1
+    int tilevol;   // threads that own a site (<= blockDim.x)
+    int zslab;     // traversal slab extent in z tiles (0 = canonical tile order)
+};
+
+template <typename T> struct Cx {
+    T re, im;
+};
+
+// ---- loads --------------------------------------------------------------------------------------------
+template <typename T> __device__ __forceinline__ void load_spinor(T p[24], const T* __restrict__ f, int s) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+    const T* base = f + ((long long)(s >> 5) * NJ * CH + (s & 31)) * NV;
+#pragma unroll
+    for (int j = 0; j < NJ; j++) {
+        V16<T> v = ld16(base + (long long)j * CH * NV);
+#pragma unroll
+        for (int q = 0; q < NV; q++) p[j * NV + q] = v.r[q];
+    }
+}
+
+template <typename T> __device__ __forceinline__ void store_spinor(T* __restrict__ f, int s, const T p[24]) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+    T* base = f + ((long long)(s >> 5) * NJ * CH + (s & 31)) * NV;
+#pragma unroll
+    for (int j = 0; j < NJ; j++) {
+        V16<T> v;
+#pragma unroll
+        for (int q = 0; q < NV; q++) v.r[q] = p[j * NV + q];
+        st16_stream(base + (long long)j * CH * NV, v);
+    }
+}
+
+// link U_mu(s) as 18 reals u[2*(3a+b)+reim]; with L12 the third row is conj(row0 x row1)
+template <typename T, bool L12>
+__device__ __forceinline__ void load_link(T u[18], const T* __restrict__ U, int s, int mu) {
+    constexpr int NV = VecOf<T>::NV;
+    const long long chunk = s >> 5;
+    const int lane = s & 31;
+    if (L12) {
+        const T* base = U + (chunk * 4 + mu) * (12LL * CH) + lane * NV;
+#pragma unroll
+        for (int j = 0; j < 12 / NV; j++) {
+            V16<T> v = ld16(base + j * CH * NV);
+#pragma unroll
+            for (int q = 0; q < NV; q++) u[j * NV + q] = v.r[q];
+        }
+        // row2 = conj(row0 x row1)
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+            const T ar = u[2 * c1], ai = u[2 * c1 + 1];          // row0[c1]
+            const T br = u[6 + 2 * c2], bi = u[6 + 2 * c2 + 1];  // row1[c2]
+            const T cr = u[2 * c2], ci = u[2 * c2 + 1];          // row0[c2]
+            const T dr = u[6 + 2 * c1], di = u[6 + 2 * c1 + 1];  // row1[c1]
+            u[12 + 2 * c] = (ar * br - ai * bi) - (cr * dr - ci * di);
+            u[12 + 2 * c + 1] = -((ar * bi + ai * br) - (cr * di + ci * dr));
+        }
+    } else {
+        constexpr int NFULL = 18 / NV;
+        const T* base = U + (chunk * 4 + mu) * (18LL * CH);
+#pragma unroll
+        for (int j = 0; j < NFULL; j++) {
+            V16<T> v = ld16(base + (j * CH + lane) * NV);
+#pragma unroll
+            for (int q = 0; q < NV; q++) u[j * NV + q] = v.r[q];
+        }
+        if (NFULL * NV < 18) {  // f32: reals 16, 17 in a float2 row
+            const T* tail = base + NFULL * NV * CH + lane * 2;
+            const float2 v = *reinterpret_cast<const float2*>(tail);
+            u[16] = (T)v.x;
+            u[17] = (T)v.y;
+        }
+    }
+}
+
+// ---- spin projection / reconstruction (chiral basis; table in DESIGN.md "Spin projectors") ------------
+// SGN = -1: (1 - g_mu), SGN = +1: (1 + g_mu).  h[2][3] complex stored as h[sp*6 + 2c + reim].
+template <int MU, int SGN, typename T> __device__ __forceinline__ void project(T h[12], const T p[24]) {
+    constexpr T sg = (T)SGN;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const T p0r = p[2 * c], p0i = p[2 * c + 1];
+        const T p1r = p[6 + 2 * c], p1i = p[6 + 2 * c + 1];
+        const T p2r = p[12 + 2 * c], p2i = p[12 + 2 * c + 1];
+        const T p3r = p[18 + 2 * c], p3i = p[18 + 2 * c + 1];
+        if (MU == 0) {  // h0 = p0 - sg i p3 ; h1 = p1 - sg i p2
+            h[2 * c] = p0r + sg * p3i;
+            h[2 * c + 1] = p0i - sg * p3r;
+            h[6 + 2 * c] = p1r + sg * p2i;
+            h[6 + 2 * c + 1] = p1i - sg * p2r;
+        } else if (MU == 1) {  // h0 = p0 - sg p3 ; h1 = p1 + sg p2
+            h[2 * c] = p0r - sg * p3r;
+            h[2 * c + 1] = p0i - sg * p3i;
+            h[6 + 2 * c] = p1r + sg * p2r;
+            h[6 + 2 * c + 1] = p1i + sg * p2i;
+        } else if (MU == 2) {  // h0 = p0 - sg i p2 ; h1 = p1 + sg i p3
+            h[2 * c] = p0r + sg * p2i;
+            h[2 * c + 1] = p0i - sg * p2r;
+            h[6 + 2 * c] = p1r - sg * p3i;
+            h[6 + 2 * c + 1] = p1i + sg * p3r;
+        } else {  // h0 = p0 + sg p2 ; h1 = p1 + sg p3
+            h[2 * c] = p0r + sg * p2r;
+            h[2 * c + 1] = p0i + sg * p2i;
+            h[6 + 2 * c] = p1r + sg * p3r;
+            h[6 + 2 * c + 1] = p1i + sg * p3i;
+        }
+    }
+}
+
+// acc += ph * (1 + SGN g_mu)-reconstruction of g (g = link times projected half spinor)
+template <int MU, int SGN, typename T> __device__ __forceinline__ void reconstruct(T acc[24], const T g[12], T ph) {
+    const T sp = (T)SGN * ph;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const T g0r = g[2 * c], g0i = g[2 * c + 1], g1r = g[6 + 2 * c], g1i = g[6 + 2 * c + 1];
+        acc[2 * c] = fma(ph, g0r, acc[2 * c]);
+        acc[2 * c + 1] = fma(ph, g0i, acc[2 * c + 1]);
+        acc[6 + 2 * c] = fma(ph, g1r, acc[6 + 2 * c]);
+        acc[6 + 2 * c + 1] = fma(ph, g1i, acc[6 + 2 * c + 1]);
+        if (MU == 0) {  // r2 = sg i g1 ; r3 = sg i g0
+            acc[12 + 2 * c] = fma(-sp, g1i, acc[12 + 2 * c]);
+            acc[12 + 2 * c + 1] = fma(sp, g1r, acc[12 + 2 * c + 1]);
+            acc[18 + 2 * c] = fma(-sp, g0i, acc[18 + 2 * c]);
+            acc[18 + 2 * c + 1] = fma(sp, g0r, acc[18 + 2 * c + 1]);
+        } else if (MU == 1) {  // r2 = sg g1 ; r3 = -sg g0
+            acc[12 + 2 * c] = fma(sp, g1r, acc[12 + 2 * c]);
+            acc[12 + 2 * c + 1] = fma(sp, g1i, acc[12 + 2 * c + 1]);
+            acc[18 + 2 * c] = fma(-sp, g0r, acc[18 + 2 * c]);
+            acc[18 + 2 * c + 1] = fma(-sp, g0i, acc[18 + 2 * c + 1]);
+        } else if (MU == 2) {  // r2 = sg i g0 ; r3 = -sg i g1
+            acc[12 + 2 * c] = fma(-sp, g0i, acc[12 + 2 * c]);
+            acc[12 + 2 * c + 1] = fma(sp, g0r, acc[12 + 2 * c + 1]);
+            acc[18 + 2 * c] = fma(sp, g1i, acc[18 + 2 * c]);
+            acc[18 + 2 * c + 1] = fma(-sp, g1r, acc[18 + 2 * c + 1]);
+        } else {  // r2 = sg g0 ; r3 = sg g1
+            acc[12 + 2 * c] = fma(sp, g0r, acc[12 + 2 * c]);
+            acc[12 + 2 * c + 1] = fma(sp, g0i, acc[12 + 2 * c + 1]);
+            acc[18 + 2 * c] = fma(sp, g1r, acc[18 + 2 * c]);
+            acc[18 + 2 * c + 1] = fma(sp, g1i, acc[18 + 2 * c + 1]);
+        }
+    }
+}
+
+// g = U h (FWD) or U^dag h (!FWD) for the two colour vectors of the half spinor
+template <bool FWD, typename T> __device__ __forceinline__ void su3_mult(T g[12], const T u[18], const T h[12]) {
+#pragma unroll
+    for (int sp = 0; sp < 2; sp++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            T gr = 0, gi = 0;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                const T hr = h[sp * 6 + 2 * b], hi = h[sp * 6 + 2 * b + 1];
+                if (FWD) {
+                    const T ur = u[2 * (3 * a + b)], ui = u[2 * (3 * a + b) + 1];
+                    gr = fma(ur, hr, gr);
+                    gr = fma(-ui, hi, gr);
+                    gi = fma(ur, hi, gi);
+                    gi = fma(ui, hr, gi);
+                } else {  // conj(U_ba)
+                    const T ur = u[2 * (3 * b + a)], ui = u[2 * (3 * b + a) + 1];
+                    gr = fma(ur, hr, gr);
+                    gr = fma(ui, hi, gr);
+                    gi = fma(ur, hi, gi);
+                    gi = fma(-ui, hr, gi);
+                }
+            }
+            g[sp * 6 + 2 * a] = gr;
+            g[sp * 6 + 2 * a + 1] = gi;
+        }
+}
+
+// one directed hop: FWD: (1 + SGN g_mu) U_mu(x) in(x+mu);  !FWD: (1 + SGN g_mu) U_mu^dag(x-mu) in(x-mu)
+template <int MU, bool FWD, int SGN, bool L12, typename T>
+__device__ __forceinline__ void hop(T acc[24], const T* __restrict__ in, const T* __restrict__ U, int s_self, int s_nb,
+                                    T ph) {
+    T p[24], h[12], u[18], g[12];
+    load_spinor<T>(p, in, s_nb);
+    load_link<T, L12>(u, U, FWD ? s_self : s_nb, MU);
+    project<MU, SGN, T>(h, p);
+    su3_mult<FWD, T>(g, u, h);
+    reconstruct<MU, SGN, T>(acc, g, ph);
+}
+
+// out6 += Hermitian 6x6 block (36 reals: 6 diagonal, 15 complex strictly-lower row-major) times in6
+template <typename T> __device__ __forceinline__ void herm6_madd(T out[12], const T cl[36], const T in[12]) {
+#pragma unroll
+    for (int k = 0; k < 6; k++) {
+        T sr = fma(cl[k], in[2 * k], out[2 * k]);
+        T si = fma(cl[k], in[2 * k + 1], out[2 * k + 1]);
+#pragma unroll
+        for (int l = 0; l < 6; l++) {
+            if (l == k) continue;
+            const T xr = in[2 * l], xi = in[2 * l + 1];
+            if (l < k) {  // L_kl
+                const T ar = cl[6 + 2 * tri(k, l)], ai = cl[6 + 2 * tri(k, l) + 1];
+                sr = fma(ar, xr, sr);
+                sr = fma(-ai, xi, sr);
+                si = fma(ar, xi, si);
+                si = fma(ai, xr, si);
+            } else {  // conj(L_lk)
+                const T ar = cl[6 + 2 * tri(l, k)], ai = cl[6 + 2 * tri(l, k) + 1];
+                sr = fma(ar, xr, sr);
+                sr = fma(ai, xi, sr);
+                si = fma(ar, xi, si);
+                si = fma(-ai, xr, si);
+            }
+        }
+        out[2 * k] = sr;
+        out[2 * k + 1] = si;
+    }
+}
+
+template <typename T> __device__ __forceinline__ void load_clover_block(T cl[36], const T* __restrict__ C, int s, int chi) {
+    constexpr int NV = VecOf<T>::NV, NJ = 72 / NV;
+    const T* base = C + (((long long)(s >> 5) * NJ + chi * (36 / NV)) * CH + (s & 31)) * NV;
+#pragma unroll
+    for (int j = 0; j < 36 / NV; j++) {
+        V16<T> v = ld16_stream(base + (long long)j * CH * NV);
+#pragma unroll
+        for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
+    }
+}
+
+template <typename T, bool DAG, bool L12, int MAXTHREADS, int MINBLOCKS>
+__global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
+    k_wilson_clover(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ U, const T* __restrict__ clover,
+                    T kappa, FineParams P) {
+    // ---- which site is mine: CTA -> tile (x tiles fastest; optionally z-slabbed traversal), thread -> site in tile
+    int tid = threadIdx.x;
+    if (tid >= P.tilevol) return;
+    int b = blockIdx.x;
+    int tc[4];
+    tc[0] = b % P.ntile[0]; b /= P.ntile[0];
+    tc[1] = b % P.ntile[1]; b /= P.ntile[1];
+    if (P.zslab > 0) {
+        // order: x, y, z within slab, t, slab  (keeps the +-t neighbours of a slab resident in L2)
+        const int nslab_full = P.ntile[2] / P.zslab;          // slabs of full height
+        const int per_slab = P.zslab * P.ntile[3];
+        int slab = b / per_slab;
+        int zs = P.zslab;
+        int r = b - slab * per_slab;
+        if (slab >= nslab_full) {  // ragged last slab
+            slab = nslab_full;
+            r = b - nslab_full * per_slab;
+            zs = P.ntile[2] - nslab_full * P.zslab;
+        }
+        tc[2] = slab * P.zslab + r % zs;
+        tc[3] = r / zs;
+    } else {
+        tc[2] = b % P.ntile[2];
+        tc[3] = b / P.ntile[2];
+    }
+    int x[4];
+    x[0] = tc[0] * P.tile[0] + tid % P.tile[0]; tid /= P.tile[0];
+    x[1] = tc[1] * P.tile[1] + tid % P.tile[1]; tid /= P.tile[1];
+    x[2] = tc[2] * P.tile[2] + tid % P.tile[2]; tid /= P.tile[2];
+    x[3] = tc[3] * P.tile[3] + tid;
+    const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
+    const int s = x[0] + st1 * x[1] + st2 * x[2] + st3 * x[3];
+
+    // neighbour sites (halo-free, modulo L) and wrap phases
+    int sf[4], sb[4];
+    T pf[4], pb[4];
+    {
+        const int stride[4] = {1, st1, st2, st3};
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const bool wf = (x[mu] == P.L[mu] - 1), wb = (x[mu] == 0);
+            sf[mu] = wf ? s - (P.L[mu] - 1) * stride[mu] : s + stride[mu];
+            sb[mu] = wb ? s + (P.L[mu] - 1) * stride[mu] : s - stride[mu];
+            pf[mu] = wf ? (T)P.bc[mu] : (T)1;
+            pb[mu] = wb ? (T)P.bc[mu] : (T)1;
+        }
+    }
+
+    T acc[24];
+#pragma unroll
+    for (int r = 0; r < 24; r++) acc[r] = 0;
+
+    // D: forward hops carry (1 - g_mu), backward (1 + g_mu); D^dag: the two are swapped.
+    constexpr int SF = DAG ? +1 : -1, SB = DAG ? -1 : +1;
+    hop<0, true, SF, L12, T>(acc, in, U, s, sf[0], pf[0]);
+    hop<0, false, SB, L12, T>(acc, in, U, s, sb[0], pb[0]);
+    hop<1, true, SF, L12, T>(acc, in, U, s, sf[1], pf[1]);
+    hop<1, false, SB, L12, T>(acc, in, U, s, sb[1], pb[1]);
+    hop<2, true, SF, L12, T>(acc, in, U, s, sf[2], pf[2]);
+    hop<2, false, SB, L12, T>(acc, in, U, s, sb[2], pb[2]);
+    hop<3, true, SF, L12, T>(acc, in, U, s, sf[3], pf[3]);
+    hop<3, false, SB, L12, T>(acc, in, U, s, sb[3], pb[3]);
+
+    // site-diagonal part: (1 + F) in, then out = that - kappa * hops
+    T p[24], o[24];
+    load_spinor<T>(p, in, s);
+#pragma unroll
+    for (int r = 0; r < 24; r++) o[r] = fma(-kappa, acc[r], p[r]);
+#pragma unroll
+    for (int chi = 0; chi < 2; chi++) {
+        T cl[36];
+        load_clover_block<T>(cl, clover, s, chi);
+        herm6_madd<T>(o + 12 * chi, cl, p + 12 * chi);
+    }
+    store_spinor<T>(out, s, o);
+}
+
+// Automatic CTA tile: powers of two dividing L, x first (128-byte lines hold 8 consecutive x sites of one
+// vec16 row), up to 128 threads.
+static void auto_tile(const int L[4], int tile[4]) {
+    const int cap[4] = {8, 4, 4, 4};
+    int vol = 1;
+    for (int mu = 0; mu < 4; mu++) {
+        int t = 1;
+        while (t * 2 <= cap[mu] && L[mu] % (t * 2) == 0 && vol * t * 2 <= 128) t *= 2;
+        tile[mu] = t;
+        vol *= t;
+    }
+    // use left-over thread budget (small or odd lattices)
+    for (int mu = 0; mu < 4 && vol < 128; mu++)
+        while (L[mu] % (tile[mu] * 2) == 0 && vol * 2 <= 128) {
+            tile[mu] *= 2;
+            vol *= 2;
+        }
+}
+
+template <typename T>
+static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4],
+                              const int bc[4], unsigned flags, void* stream, const char* what) {
+    clear_error();
+    if (!out || !in || !U || !clover || check_dims(dims) || !bc) {
+        set_error("%s: null pointer or non-positive dim", what);
+        return LQCD_EINVAL;
+    }
+    if (!aligned16(out) || !aligned16(in) || !aligned16(U) || !aligned16(clover)) {
+        set_error("%s: pointers must be 16-byte aligned", what);
+        return LQCD_EINVAL;
+    }
+    if (out == in) {
+        set_error("%s: out must not alias in", what);
+        return LQCD_EINVAL;
+    }
+    if (flags & ~(LQCD_DAGGER | LQCD_LINKS_12)) {
+        set_error("%s: unknown flag bits 0x%x", what, flags);
+        return LQCD_EINVAL;
+    }
+    if (volume(dims) > 0x7fffffffLL) {
+        set_error("%s: volume exceeds 2^31-1 sites", what);
+        return LQCD_EUNSUPPORTED;
+    }
+    FineParams P;
+    for (int mu = 0; mu < 4; mu++) {
+        if (bc[mu] != 1 && bc[mu] != -1) {
+            set_error("%s: bc[%d] = %d not in {+1,-1}", what, mu, bc[mu]);
+            return LQCD_EINVAL;
+        }
+        P.L[mu] = dims[mu];
+        P.bc[mu] = bc[mu];
+    }
+    bool user_ok = g_knobs.fine_tile[0] > 0;
+    for (int mu = 0; mu < 4 && user_ok; mu++) user_ok = dims[mu] % g_knobs.fine_tile[mu] == 0;
+    if (user_ok)
+        for (int mu = 0; mu < 4; mu++) P.tile[mu] = g_knobs.fine_tile[mu];
+    else
+        auto_tile(dims, P.tile);
+    P.tilevol = 1;
+    long long ntiles = 1;
+    for (int mu = 0; mu < 4; mu++) {
+        P.ntile[mu] = dims[mu] / P.tile[mu];
+        P.tilevol *= P.tile[mu];
+        ntiles *= P.ntile[mu];
+    }
+    P.zslab = g_knobs.fine_tslab > 0 ? g_knobs.fine_tslab : 0;
+    if (P.zslab >= P.ntile[2]) P.zslab = 0;
+    int threads = (P.tilevol + 31) / 32 * 32;
+    const bool dag = flags & LQCD_DAGGER, l12 = flags & LQCD_LINKS_12;
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned grid = (unsigned)ntiles;
+#define LAUNCH(DAG, L12)                                                                                  \
+    do {                                                                                                  \
+        if (threads <= 128)                                                                               \
+            k_wilson_clover<T, DAG, L12, 128, (sizeof(T) == 4 ? 4 : 2)>                                   \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
+        else                                                                                              \
+            k_wilson_clover<T, DAG, L12, 256, (sizeof(T) == 4 ? 2 : 1)>                                   \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
+    } while (0)
+    if (dag && l12) LAUNCH(true, true);
+    else if (dag) LAUNCH(true, false);
+    else if (l12) LAUNCH(false, true);
+    else LAUNCH(false, false);
+#undef LAUNCH
+    count_launch();
+    return check_launch(what);
+}
+
+}  // namespace lqcd
+
+using namespace lqcd;
+
+extern "C" {
+int lqcd_wilson_clover_mult_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
+                                const int dims[4], const int bc[4], unsigned flags, void* stream) {
+    return wilson_clover_call<float>(out, in, U, clover, kappa, dims, bc, flags, stream, "lqcd_wilson_clover_mult_f32");
+}
+int lqcd_wilson_clover_mult_f64(double* out, const double* in, const double* U, const double* clover, double kappa,
+                                const int dims[4], const int bc[4], unsigned flags, void* stream) {
+    return wilson_clover_call<double>(out, in, U, clover, kappa, dims, bc, flags, stream, "lqcd_wilson_clover_mult_f64");
+}
+}

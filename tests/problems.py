@@ -1,0 +1,56 @@
+"""Test problems: the BASELINE.json configs (and edge-case lattices) with every input the hot path needs.
+
+Input preparation that is part of the method (clover term O3, block orthonormalisation O4, Galerkin blocks O6)
+is done by the ORACLE and handed identically to both sides; the CUDA path never produces an oracle input.
+"""
+from __future__ import annotations
+
+import functools
+from dataclasses import dataclass
+
+import numpy as np
+
+import lqcd_inputs as li
+import oracle
+
+
+@dataclass
+class Problem:
+    cfg: li.Config
+    U: np.ndarray         # (4, V, 3, 3) complex128
+    psi: list             # n_rhs x (V, 4, 3)
+    clover: np.ndarray    # (V, 2, 6, 6)
+    v: np.ndarray | None  # (nvec, V, 4, 3), block-orthonormal
+    A: np.ndarray | None  # (Vc, 9, N, N)
+    xc: np.ndarray | None  # (Vc, 2, nvec) coarse test vector
+
+
+def make_problem(cfg: li.Config, n_rhs: int = 1, coarse: str = "galerkin") -> Problem:
+    """coarse: 'galerkin' (true P^dag D P), 'synthetic' (SURVEY 8(d) recipe) or 'none'."""
+    hf = li.make_host_fields(cfg, n_rhs=n_rhs, with_nullvecs=coarse != "none")
+    clover = oracle.clover_from_links(hf.U, cfg.kappa, cfg.csw, cfg.dims)
+    v = A = xc = None
+    rng = np.random.default_rng(cfg.seed + 1000)
+    if coarse != "none":
+        v = oracle.orthonormalize_blocks(hf.v, cfg.dims, cfg.block)
+        xc = li.coarse_vector(rng, cfg.cvolume, cfg.nvec)
+        if coarse == "galerkin":
+            A = oracle.galerkin_coarse(hf.U, clover, v, cfg.kappa, cfg.dims, cfg.bc, cfg.block)
+        else:
+            A = li.coarse_matrix_synthetic(rng, cfg.cvolume, cfg.nvec)
+    return Problem(cfg, hf.U, hf.psi, clover, v, A, xc)
+
+
+@functools.lru_cache(maxsize=4)
+def config_problem(name: str, n_rhs: int = 1) -> Problem:
+    return make_problem(li.CONFIGS[name], n_rhs=n_rhs)
+
+
+def custom_config(dims, block, nvec, bc=(1, 1, 1, -1), gauge="exp", eps=0.4, kappa=0.13, csw=1.3, seed=11):
+    return li.Config("custom", tuple(dims), tuple(block), nvec, gauge, eps, kappa, csw, seed=seed, bc=tuple(bc))
+
+
+def rel_l2(a, b) -> float:
+    a = np.asarray(a, dtype=np.complex128).ravel()
+    b = np.asarray(b, dtype=np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))

@@ -1,0 +1,323 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element, on the same
+seeded inputs (-m gpu).  Bars (BASELINE.json north_star): relative L2 per application <= 1e-12 in fp64 and
+<= 2e-6 in fp32.  fp32 protocol (O9): every input is rounded to fp32 once, BOTH sides consume the
+rounded values, the oracle promotes them and does all arithmetic in fp64.
+"""
+import numpy as np
+import pytest
+
+import lqcd_inputs as li
+import oracle
+from problems import config_problem, custom_config, make_problem, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 2e-6}
+CDT = {"f64": np.complex128, "f32": np.complex64}
+
+
+@pytest.fixture(scope="module")
+def lq():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_2111_05012_b200 as lq  # raises if the CUDA library is missing: no fallback
+    return lq
+
+
+def to_dev(a, prec):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(np.asarray(a).astype(CDT[prec]))).cuda()
+
+
+def rounded(a, prec):
+    """the values both sides consume"""
+    return np.ascontiguousarray(np.asarray(a).astype(CDT[prec]))
+
+
+class Dev:
+    """Device-resident native operator fields of a Problem in one precision."""
+
+    def __init__(self, lq, prob, prec, links12=False, coarse=True):
+        cfg = prob.cfg
+        self.lq, self.prob, self.prec, self.cfg, self.links12 = lq, prob, prec, cfg, links12
+        self.U = lq.pack_gauge(to_dev(prob.U, prec), cfg.dims, links12=links12)
+        self.clover = lq.pack_clover(to_dev(prob.clover, prec), cfg.dims)
+        self.v = self.A = None
+        if coarse and prob.v is not None:
+            self.v = lq.pack_nullvecs(to_dev(prob.v, prec), cfg.dims, cfg.block)
+            self.A = to_dev(prob.A, prec)
+
+    def D(self, psi, dagger=False):
+        lq, cfg = self.lq, self.cfg
+        x = lq.pack_spinor(to_dev(psi, self.prec), cfg.dims)
+        y = lq.empty_spinor(cfg.dims, dtype=x.dtype)
+        lq.wilson_clover_mult(y, x, self.U, self.clover, cfg.kappa, cfg.dims, cfg.bc, dagger=dagger,
+                              links12=self.links12)
+        return lq.unpack_spinor(y, cfg.dims).cpu().numpy()
+
+    def Dc(self, xc, dagger=False):
+        import torch
+        x = to_dev(xc, self.prec)
+        y = torch.empty_like(x)
+        self.lq.coarse_mult(y, x, self.A, self.cfg.cdims, self.cfg.nvec, dagger=dagger)
+        return y.cpu().numpy()
+
+    def R(self, psi):
+        import torch
+        lq, cfg = self.lq, self.cfg
+        x = lq.pack_spinor(to_dev(psi, self.prec), cfg.dims)
+        y = torch.empty((cfg.cvolume, 2, cfg.nvec), dtype=to_dev(np.zeros(1), self.prec).dtype, device="cuda")
+        lq.restrict(y, x, self.v, cfg.dims, cfg.block, cfg.nvec)
+        return y.cpu().numpy()
+
+    def P(self, xc):
+        lq, cfg = self.lq, self.cfg
+        x = to_dev(xc, self.prec)
+        y = lq.empty_spinor(cfg.dims, dtype=self.U.dtype)
+        lq.prolong(y, x, self.v, cfg.dims, cfg.block, cfg.nvec)
+        return lq.unpack_spinor(y, cfg.dims).cpu().numpy()
+
+
+def oracle_D(prob, psi, prec, dagger=False):
+    cfg = prob.cfg
+    return oracle.wilson_clover_mult(rounded(psi, prec), rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa,
+                                     cfg.dims, cfg.bc, dagger=dagger)
+
+
+# ------------------------------------------------------------------------------------------------------
+# layout helpers: bit-exact round trips
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 5, 2, 7), (6, 4, 2, 10)])
+def test_pack_unpack_spinor_roundtrip(lq, prec, dims):
+    rng = np.random.default_rng(5)
+    psi = rounded(li.spinor(rng, int(np.prod(dims))), prec)
+    back = lq.unpack_spinor(lq.pack_spinor(to_dev(psi, prec), dims), dims).cpu().numpy()
+    assert np.array_equal(back, psi)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_pack_unpack_nullvec_roundtrip(lq, prec):
+    dims, block, nvec = (8, 4, 4, 6), (4, 2, 2, 3), 3
+    rng = np.random.default_rng(6)
+    v = rounded(li.null_vectors(rng, nvec, int(np.prod(dims))), prec)
+    nat = lq.pack_nullvecs(to_dev(v, prec), dims, block)
+    for i in range(nvec):
+        assert np.array_equal(lq.unpack_nullvec(nat, i, dims, block, nvec).cpu().numpy(), v[i])
+
+
+# ------------------------------------------------------------------------------------------------------
+# config 1: every row, fp64 and fp32
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("links12", [False, True])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_c1_wilson_clover(lq, prec, links12, dagger):
+    prob = config_problem("c1")
+    d = Dev(lq, prob, prec, links12=links12, coarse=False)
+    got = d.D(prob.psi[0], dagger=dagger)
+    ref = oracle_D(prob, prob.psi[0], prec, dagger=dagger)
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_c1_coarse(lq, prec, dagger):
+    prob = config_problem("c1")
+    d = Dev(lq, prob, prec)
+    got = d.Dc(prob.xc, dagger=dagger)
+    ref = oracle.coarse_mult(rounded(prob.xc, prec), rounded(prob.A, prec), prob.cfg.cdims, dagger=dagger)
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_c1_restrict_prolong(lq, prec):
+    prob = config_problem("c1")
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    got = d.R(prob.psi[0])
+    ref = oracle.restrict(rounded(prob.psi[0], prec), rounded(prob.v, prec), cfg.dims, cfg.block)
+    assert rel_l2(got, ref) <= TOL[prec]
+    got = d.P(prob.xc)
+    ref = oracle.prolong(rounded(prob.xc, prec), rounded(prob.v, prec), cfg.dims, cfg.block)
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+# ------------------------------------------------------------------------------------------------------
+# config 2: 8^4, block 4^4, nvec 16, fp32, 16 right-hand sides one at a time
+# ------------------------------------------------------------------------------------------------------
+def test_c2_sixteen_rhs(lq):
+    prec = "f32"
+    prob = config_problem("c2", 16)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    rng = np.random.default_rng(77)
+    for k, psi in enumerate(prob.psi):
+        assert rel_l2(d.D(psi), oracle_D(prob, psi, prec)) <= TOL[prec], f"D rhs {k}"
+        xc = li.coarse_vector(rng, cfg.cvolume, cfg.nvec)
+        ref = oracle.coarse_mult(rounded(xc, prec), rounded(prob.A, prec), cfg.cdims)
+        assert rel_l2(d.Dc(xc), ref) <= TOL[prec], f"D_c rhs {k}"
+    psi = prob.psi[3]
+    assert rel_l2(d.D(psi, dagger=True), oracle_D(prob, psi, prec, dagger=True)) <= TOL[prec]
+    assert rel_l2(d.R(psi), oracle.restrict(rounded(psi, prec), rounded(prob.v, prec), cfg.dims, cfg.block)) <= TOL[prec]
+    assert rel_l2(d.P(prob.xc), oracle.prolong(rounded(prob.xc, prec), rounded(prob.v, prec), cfg.dims, cfg.block)) <= \
+        TOL[prec]
+
+
+# ------------------------------------------------------------------------------------------------------
+# config 3: 16^3 x 32, Haar links, nvec 32, true Galerkin A; restrict -> coarse_mult -> prolong chained on the
+# device as in a V-cycle (row A6), no host copies between the three kernels
+# ------------------------------------------------------------------------------------------------------
+def test_c3_vcycle_chain(lq):
+    import torch
+    prec = "f32"
+    prob = config_problem("c3")
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    psi = prob.psi[0]
+    # each step against the oracle on the same (rounded) input
+    assert rel_l2(d.D(psi), oracle_D(prob, psi, prec)) <= TOL[prec]
+    v32, A32 = rounded(prob.v, prec), rounded(prob.A, prec)
+    r_ref = oracle.restrict(rounded(psi, prec), v32, cfg.dims, cfg.block)
+    assert rel_l2(d.R(psi), r_ref) <= TOL[prec]
+    c_ref = oracle.coarse_mult(rounded(prob.xc, prec), A32, cfg.cdims)
+    assert rel_l2(d.Dc(prob.xc), c_ref) <= TOL[prec]
+    p_ref = oracle.prolong(rounded(prob.xc, prec), v32, cfg.dims, cfg.block)
+    assert rel_l2(d.P(prob.xc), p_ref) <= TOL[prec]
+    # the chain, device-resident; the oracle chain runs in fp64 from the same fp32 input, so the bar is three
+    # applications' worth of fp32 rounding
+    x = lq.pack_spinor(to_dev(psi, prec), cfg.dims)
+    xc = torch.empty((cfg.cvolume, 2, cfg.nvec), dtype=torch.complex64, device="cuda")
+    yc = torch.empty_like(xc)
+    y = lq.empty_spinor(cfg.dims)
+    n0 = lq.launch_count()
+    lq.restrict(xc, x, d.v, cfg.dims, cfg.block, cfg.nvec)
+    lq.coarse_mult(yc, xc, d.A, cfg.cdims, cfg.nvec)
+    lq.prolong(y, yc, d.v, cfg.dims, cfg.block, cfg.nvec)
+    assert lq.launch_count() - n0 == 3
+    got = lq.unpack_spinor(y, cfg.dims).cpu().numpy()
+    ref = oracle.prolong(oracle.coarse_mult(r_ref, prob.A.astype(np.complex64).astype(np.complex128), cfg.cdims),
+                         v32.astype(np.complex128), cfg.dims, cfg.block)
+    assert rel_l2(got, ref) <= 3 * TOL[prec]
+
+
+# ------------------------------------------------------------------------------------------------------
+# edge cases: odd / ragged lattices (V not a multiple of 32), other boundary conditions, odd nvec, 8x4x4x4
+# blocks (the paper's production block), coarse extent 2 with X+mu == X-mu
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,bc", [
+    ((3, 3, 3, 3), (1, 1, 1, -1)),       # V = 81: ragged last chunk, no power-of-two tile
+    ((6, 4, 2, 10), (-1, 1, -1, 1)),     # extent 2 (x+mu == x-mu), mixed boundary conditions
+    ((2, 2, 2, 2), (-1, -1, -1, -1)),    # smallest lattice, all antiperiodic
+    ((16, 4, 4, 4), (1, 1, 1, 1)),       # all periodic
+])
+def test_wilson_clover_edge_lattices(lq, prec, dims, bc):
+    cfg = custom_config(dims, (1, 1, 1, 1), 1, bc=bc)
+    prob = make_problem(cfg, coarse="none")
+    for links12 in (False, True):
+        d = Dev(lq, prob, prec, links12=links12, coarse=False)
+        for dagger in (False, True):
+            got = d.D(prob.psi[0], dagger=dagger)
+            assert rel_l2(got, oracle_D(prob, prob.psi[0], prec, dagger=dagger)) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,block,nvec", [
+    ((16, 8, 8, 8), (8, 4, 4, 4), 4),    # the paper's 8x4x4x4 block; coarse 2^4
+    ((4, 6, 4, 6), (2, 3, 2, 2), 3),     # odd nvec, non-power-of-two block
+    ((4, 4, 4, 8), (2, 2, 2, 2), 1),     # nvec = 1 (N = 2)
+    ((8, 4, 4, 4), (2, 2, 2, 2), 20),    # N = 40: rows not a power of two
+    ((4, 4, 4, 4), (2, 2, 2, 2), 40),    # N = 80 > 64: several vec16 per lane per row
+])
+def test_coarse_and_transfer_edge_sizes(lq, prec, dims, block, nvec):
+    cfg = custom_config(dims, block, nvec)
+    prob = make_problem(cfg, coarse="galerkin" if nvec <= 4 else "synthetic")
+    d = Dev(lq, prob, prec)
+    psi = prob.psi[0]
+    v, A = rounded(prob.v, prec), rounded(prob.A, prec)
+    for dagger in (False, True):
+        ref = oracle.coarse_mult(rounded(prob.xc, prec), A, cfg.cdims, dagger=dagger)
+        assert rel_l2(d.Dc(prob.xc, dagger=dagger), ref) <= TOL[prec]
+    assert rel_l2(d.R(psi), oracle.restrict(rounded(psi, prec), v, cfg.dims, cfg.block)) <= TOL[prec]
+    assert rel_l2(d.P(prob.xc), oracle.prolong(rounded(prob.xc, prec), v, cfg.dims, cfg.block)) <= TOL[prec]
+
+
+def test_results_do_not_depend_on_tuning_knobs(lq):
+    prob = config_problem("c2", 16)
+    d = Dev(lq, prob, "f32")
+    base = d.D(prob.psi[0])
+    base_c = d.Dc(prob.xc)
+    try:
+        for tile in [(8, 4, 4, 1), (4, 4, 4, 4), (8, 8, 2, 2), (2, 2, 2, 2), (8, 1, 1, 1)]:
+            lq.set_fine_tile(tile)
+            assert np.array_equal(d.D(prob.psi[0]), base), tile
+        lq.set_fine_tile(None)
+        lq.set_knob("fine_tslab", 1)
+        assert np.array_equal(d.D(prob.psi[0]), base)
+        for rpw in (1, 2, 4):
+            lq.set_knob("coarse_rows_per_warp", rpw)
+            assert np.array_equal(d.Dc(prob.xc), base_c)
+    finally:
+        lq.set_fine_tile(None)
+        lq.set_knob("fine_tslab", 0)
+        lq.set_knob("coarse_rows_per_warp", 0)
+
+
+# ------------------------------------------------------------------------------------------------------
+# error behaviour of the C ABI (nothing is enqueued on error)
+# ------------------------------------------------------------------------------------------------------
+def test_error_codes(lq):
+    import torch
+    prob = config_problem("c1")
+    cfg = prob.cfg
+    d = Dev(lq, prob, "f32")
+    x = lq.pack_spinor(to_dev(prob.psi[0], "f32"), cfg.dims)
+    y = lq.empty_spinor(cfg.dims)
+    n0 = lq.launch_count()
+
+    def code(fn):
+        with pytest.raises(lq.LqcdError) as e:
+            fn()
+        return e.value.code
+
+    assert code(lambda: lq.wilson_clover_mult(x, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc)) == lq.EINVAL
+    assert code(lambda: lq.wilson_clover_mult(y, x, d.U, d.clover, cfg.kappa, cfg.dims, (1, 1, 1, 0))) == lq.EINVAL
+    assert code(lambda: lq.wilson_clover_mult(y, x, d.U, d.clover, cfg.kappa, (4, 4, 4, 0), cfg.bc)) == lq.EINVAL
+    assert code(lambda: lq.wilson_clover_mult(y[1:], x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc)) == lq.EINVAL
+    xc = to_dev(prob.xc, "f32")
+    yc = torch.empty_like(xc)
+    assert code(lambda: lq.coarse_mult(yc, xc, d.A, (2, 2, 2, 1), cfg.nvec)) == lq.EINVAL
+    assert code(lambda: lq.coarse_mult(xc, xc, d.A, cfg.cdims, cfg.nvec)) == lq.EINVAL
+    assert code(lambda: lq.restrict(yc, x, d.v, cfg.dims, (3, 2, 2, 2), cfg.nvec)) == lq.EINVAL
+    assert code(lambda: lq.restrict(yc, x, d.v, cfg.dims, (4, 4, 4, 4), cfg.nvec)) == lq.EINVAL  # coarse extent 1
+    assert code(lambda: lq.prolong(y, yc, d.v, cfg.dims, cfg.block, 0)) == lq.EINVAL
+    assert "lqcd_prolong_f32" in lq.last_error()
+    assert lq.launch_count() == n0, "an erroring call must not enqueue anything"
+    with pytest.raises(ValueError):
+        lq.wilson_clover_mult(y.cpu(), x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc)  # no CPU path
+
+
+# ------------------------------------------------------------------------------------------------------
+# host-vector entry points give the same numbers as the device-pointer ones
+# ------------------------------------------------------------------------------------------------------
+def test_host_entry_points(lq):
+    import torch
+    prob = config_problem("c2", 16)
+    cfg = prob.cfg
+    d = Dev(lq, prob, "f32")
+    ws = torch.empty(lq.host_workspace_bytes(cfg.dims, cfg.block, cfg.nvec), dtype=torch.uint8, device="cuda")
+    psi = torch.from_numpy(rounded(prob.psi[0], "f32")).pin_memory()
+    out = torch.empty_like(psi).pin_memory()
+    lq.wilson_clover_mult_host(out, psi, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, ws)
+    assert np.array_equal(out.numpy(), d.D(prob.psi[0]))
+    lq.wilson_clover_mult_host(out, psi, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, ws, dagger=True)
+    assert np.array_equal(out.numpy(), d.D(prob.psi[0], dagger=True))
+    xc = torch.from_numpy(rounded(prob.xc, "f32")).pin_memory()
+    yc = torch.empty_like(xc).pin_memory()
+    lq.coarse_mult_host(yc, xc, d.A, cfg.cdims, cfg.nvec, ws)
+    assert np.array_equal(yc.numpy(), d.Dc(prob.xc))
+    lq.restrict_host(yc, psi, d.v, cfg.dims, cfg.block, cfg.nvec, ws)
+    assert np.array_equal(yc.numpy(), d.R(prob.psi[0]))
+    lq.prolong_host(out, xc, d.v, cfg.dims, cfg.block, cfg.nvec, ws)
+    assert np.array_equal(out.numpy(), d.P(prob.xc))
