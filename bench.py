@@ -1,0 +1,539 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path on synthetic lattices shaped like the
+paper's workloads.
+
+    python bench.py --gpus N --steps K --warmup W [--workload c5|c4|c3|c2] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one right-hand side:
+    D x (A1, 18-real links), D^dag x (A2), restrict x (A4), coarse_mult (A3), prolong (A5)  [A4->A3->A5 chained = A6]
+Metric (BASELINE.json): fp32 Wilson-clover & coarse mat-vec GB/s and GFLOP/s; % of HBM roofline.  `value` is the
+ALGORITHMIC GB/s of the whole step (compulsory bytes of section 8(d) / measured time), inputs resident in HBM;
+`kernels` carries sites/s, GFLOP/s, GB/s and roofline fraction per kernel; `e2e` is the same metric through the
+host-vector C-ABI calls with the H2D/D2H copies inside the timed region.
+
+Multi-GPU: the path is single-GPU by the north_star ("replicas only"): --gpus N runs N independent
+replicas, one process per GPU under torchrun, barrier + max-over-ranks timing, no data-path collective.
+
+--impl reference times the CPU oracle as it stands on the host cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import lqcd_inputs as li
+
+METRIC = "fp32 Wilson-clover & coarse mat-vec GB/s and GFLOP/s; % of HBM roofline"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+
+# ----------------------------------------------------------------------------------------------------------
+# algorithmic bytes / nominal flops per launch (restated in DESIGN.md "Roofline model")
+# ----------------------------------------------------------------------------------------------------------
+def model(cfg: li.Config, links12: bool = False) -> dict:
+    V, Vc, N, nv = cfg.volume, cfg.cvolume, 2 * cfg.nvec, cfg.nvec
+    bv = V // Vc
+    fine_b = (96 + 96 + (192 if links12 else 288) + 288) * V
+    fine_f = 1872 * V
+    coarse_b = (9 * N * N * 8 + 2 * N * 8) * Vc
+    coarse_f = 9 * N * N * 8 * Vc
+    tr_b = (nv * 96 + 96) * V + N * 8 * Vc
+    tr_f = nv * 96 * V
+    return {
+        "wilson_clover": {"bytes": fine_b, "flops": fine_f, "units": V},
+        "wilson_clover_dagger": {"bytes": fine_b, "flops": fine_f, "units": V},
+        "restrict": {"bytes": tr_b, "flops": tr_f, "units": V},
+        "coarse_mult": {"bytes": coarse_b, "flops": coarse_f, "units": Vc},
+        "prolong": {"bytes": tr_b, "flops": tr_f, "units": V},
+        "_block_sites": bv,
+    }
+
+
+STEP_ORDER = ["wilson_clover", "wilson_clover_dagger", "restrict", "coarse_mult", "prolong"]
+KERNEL_SYMBOL = {  # the __global__ each row launches (for the ncu launch list)
+    "wilson_clover": "k_wilson_clover", "wilson_clover_dagger": "k_wilson_clover", "restrict": "k_restrict",
+    "coarse_mult": "k_coarse", "prolong": "k_prolong",
+}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def recorded_traffic(workload: str, kernel: str):
+    """dram bytes per launch from the committed ncu --set full capture (profiles/ncu_traffic.json), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f)[workload][kernel]["dram_bytes_per_launch"]
+    except Exception:
+        return None
+
+
+# ----------------------------------------------------------------------------------------------------------
+# ranks: one process per GPU, replicas only
+# ----------------------------------------------------------------------------------------------------------
+class Ranks:
+    """torch.distributed plumbing: barrier and max-over-ranks.  backend nccl on GPUs, gloo in the CPU tests."""
+
+    def __init__(self, backend: str | None = None):
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29511")
+            self.backend = backend or "nccl"
+            if self.backend == "nccl":
+                import torch
+                torch.cuda.set_device(self.local_rank)
+            dist.init_process_group(self.backend, rank=self.rank, world_size=self.world)
+            self.dist = dist
+
+    def _tensor(self, x):
+        import torch
+        dev = "cuda" if (self.dist is not None and self.backend == "nccl") else "cpu"
+        return torch.tensor([float(x)], dtype=torch.float64, device=dev)
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+
+    def max(self, x: float) -> float:
+        if self.dist is None:
+            return float(x)
+        t = self._tensor(x)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum(self, x: float) -> float:
+        if self.dist is None:
+            return float(x)
+        t = self._tensor(x)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
+        return float(t.item())
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
+def whole_job_value(units_per_rank: float, world: int, max_seconds: float) -> float:
+    """weak scaling, replicas: every rank processes units_per_rank in (at most) max_seconds."""
+    return units_per_rank * world / max_seconds
+
+
+# ----------------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ----------------------------------------------------------------------------------------------------------
+_REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+            0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+
+class ClockSampler(threading.Thread):
+    def __init__(self, device_index: int, period_s: float = 0.004):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.reasons, self.max_mhz = period_s, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            try:
+                uuid = "GPU-" + str(torch.cuda.get_device_properties(device_index).uuid)
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode() if hasattr(uuid, "encode") else uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(device_index)
+            self.nv = pynvml
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    bits = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    bits = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for b, name in _REASONS.items():
+                    if bits & b:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self) -> dict:
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2)
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "note": "nvml unavailable"}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ----------------------------------------------------------------------------------------------------------
+# the workload on the device (synthetic, seeded)
+# ----------------------------------------------------------------------------------------------------------
+class Workload:
+    """Device-resident native operator fields + rotating right-hand sides of one config."""
+
+    NBUF = 4  # distinct input/output buffer sets rotated across steps (and every buffer is >> L2 at c4/c5)
+
+    def __init__(self, cfg: li.Config, device, seed: int):
+        import torch
+        import paper_2111_05012_b200 as lq
+        self.cfg, self.lq, self.dev = cfg, lq, device
+        gen = torch.Generator(device=device)
+        gen.manual_seed(seed)
+        V, Vc, nv = cfg.volume, cfg.cvolume, cfg.nvec
+        # gauge: the config's recipe, fp64 on the device, rounded to fp32 once, packed (18-real and 12-real)
+        U = li.t_gauge_field(cfg, gen, device).to(torch.complex64)
+        self.U18 = lq.pack_gauge(U, cfg.dims)
+        self.U12 = lq.pack_gauge(U, cfg.dims, links12=True)
+        del U
+        cl = li.t_clover_synthetic(gen, V, device)
+        self.clover = lq.pack_clover(cl, cfg.dims)
+        del cl
+        self.x = [lq.pack_spinor(li.t_spinor(gen, V, device, torch.float32), cfg.dims) for _ in range(self.NBUF)]
+        self.y = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
+        self.yd = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
+        self.z = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
+        self.xc = [torch.empty((Vc, 2, nv), dtype=torch.complex64, device=device) for _ in range(self.NBUF)]
+        self.yc = [torch.empty((Vc, 2, nv), dtype=torch.complex64, device=device) for _ in range(self.NBUF)]
+        self.A = li.t_coarse_matrix_synthetic(gen, Vc, nv, device)
+        # null vectors: Gaussian, one canonical vector at a time into its native slot (never twice in HBM)
+        self.v = torch.empty(lq.native_nullvecs_reals(cfg.dims, cfg.block, nv), dtype=torch.float32, device=device)
+        scale = 1.0 / np.sqrt(2.0 * 6 * (V // Vc))  # unit-norm aggregates on average, like orthonormal ones
+        for i in range(nv):
+            vi = li.t_spinor(gen, V, device, torch.float32) * scale
+            lq.pack_nullvec(self.v, vi, i, cfg.dims, cfg.block, nv)
+            del vi
+        torch.cuda.synchronize()
+
+    # one launch per row; `i` picks the buffer set
+    def wilson_clover(self, i):
+        c = self.cfg
+        self.lq.wilson_clover_mult(self.y[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc)
+
+    def wilson_clover_dagger(self, i):
+        c = self.cfg
+        self.lq.wilson_clover_mult(self.yd[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, dagger=True)
+
+    def wilson_clover_12(self, i):
+        c = self.cfg
+        self.lq.wilson_clover_mult(self.y[i], self.x[i], self.U12, self.clover, c.kappa, c.dims, c.bc, links12=True)
+
+    def restrict(self, i):
+        c = self.cfg
+        self.lq.restrict(self.xc[i], self.x[i], self.v, c.dims, c.block, c.nvec)
+
+    def coarse_mult(self, i):
+        c = self.cfg
+        self.lq.coarse_mult(self.yc[i], self.xc[i], self.A, c.cdims, c.nvec)
+
+    def prolong(self, i):
+        c = self.cfg
+        self.lq.prolong(self.z[i], self.yc[i], self.v, c.dims, c.block, c.nvec)
+
+
+def time_steps(W: Workload, steps: int, warmup: int, ranks: Ranks):
+    """K steps between one pair of events (whole-step time) with an event after every launch (per-kernel times)."""
+    import torch
+    fns = [getattr(W, n) for n in STEP_ORDER]
+    for k in range(warmup):
+        for f in fns:
+            f(k % W.NBUF)
+    torch.cuda.synchronize()
+    ranks.barrier()
+    torch.cuda.synchronize()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(len(fns) + 1)] for _ in range(steps)]
+    n0 = W.lq.launch_count()
+    for k in range(steps):
+        ev[k][0].record()
+        for j, f in enumerate(fns):
+            f(k % W.NBUF)
+            ev[k][j + 1].record()
+    torch.cuda.synchronize()
+    launches = W.lq.launch_count() - n0
+    ranks.barrier()
+    total_s = ev[0][0].elapsed_time(ev[-1][-1]) * 1e-3
+    per_kernel = {}
+    for j, name in enumerate(STEP_ORDER):
+        per_kernel[name] = [ev[k][j].elapsed_time(ev[k][j + 1]) * 1e-3 for k in range(steps)]
+    return total_s, per_kernel, launches
+
+
+def time_single(W: Workload, name: str, reps: int, warmup: int = 3):
+    """one row alone, rotating buffers (used for the 12-real-link variant and the sweep)"""
+    import torch
+    f = getattr(W, name)
+    for k in range(warmup):
+        f(k % W.NBUF)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(reps):
+        f(k % W.NBUF)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e-3 / reps
+
+
+def time_e2e(W: Workload, steps: int, warmup: int, ranks: Ranks):
+    """The same step through the host-vector C-ABI calls: canonical fp32 vectors in pinned host memory, H2D and D2H
+    inside the timed region, every call synchronising."""
+    import torch
+    c, lq = W.cfg, W.lq
+    V, Vc, nv = c.volume, c.cvolume, c.nvec
+    ws = torch.empty(lq.host_workspace_bytes(c.dims, c.block, nv), dtype=torch.uint8, device=W.dev)
+    g = torch.Generator()
+    g.manual_seed(99)
+    x_h = torch.randn((V, 4, 3, 2), generator=g, dtype=torch.float32).pin_memory()
+    y_h = torch.empty((V, 4, 3, 2), dtype=torch.float32).pin_memory()
+    xc_h = torch.empty((Vc, 2, nv, 2), dtype=torch.float32).pin_memory()
+    yc_h = torch.empty((Vc, 2, nv, 2), dtype=torch.float32).pin_memory()
+
+    def one():
+        lq.wilson_clover_mult_host(y_h, x_h, W.U18, W.clover, c.kappa, c.dims, c.bc, ws)
+        lq.wilson_clover_mult_host(y_h, x_h, W.U18, W.clover, c.kappa, c.dims, c.bc, ws, dagger=True)
+        lq.restrict_host(xc_h, x_h, W.v, c.dims, c.block, nv, ws)
+        lq.coarse_mult_host(yc_h, xc_h, W.A, c.cdims, nv, ws)
+        lq.prolong_host(y_h, yc_h, W.v, c.dims, c.block, nv, ws)
+
+    fine_b, coarse_b = V * 96, Vc * 2 * nv * 8
+    h2d = 3 * fine_b + 2 * coarse_b          # x (three times), xc, yc
+    d2h = 3 * fine_b + 2 * coarse_b          # D x, D^dag x, prolong out, xc, yc
+    for _ in range(warmup):
+        one()
+    torch.cuda.synchronize()
+    ranks.barrier()
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        one()
+    e1.record()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    dev_s = e0.elapsed_time(e1) * 1e-3
+    return max(wall, dev_s) / steps, h2d, d2h
+
+
+# ----------------------------------------------------------------------------------------------------------
+# the CPU oracle as a baseline (the only place outside tests/ and smoke() that executes oracle/)
+# ----------------------------------------------------------------------------------------------------------
+def sample_config(cfg: li.Config) -> li.Config:
+    """The bounded sample of a workload the oracle is timed on: the same recipe (links, kappa, c_sw, block, nvec,
+    boundary conditions) on a lattice of at most 16^3 x 32 sites."""
+    cap = (16, 16, 16, 32)
+    dims = tuple(min(l, c) for l, c in zip(cfg.dims, cap))
+    return li.Config(cfg.name + "-sample", dims, cfg.block, cfg.nvec, cfg.gauge, cfg.eps, cfg.kappa, cfg.csw,
+                     seed=cfg.seed, bc=cfg.bc)
+
+
+class OracleSample:
+    """Host fields of the sample, fp32-rounded (the oracle promotes them and computes in fp64)."""
+
+    def __init__(self, cfg: li.Config):
+        import oracle
+        self.oracle = oracle
+        self.scfg = s = sample_config(cfg)
+        rng = np.random.default_rng(s.seed)
+        c64 = lambda a: np.ascontiguousarray(a.astype(np.complex64))
+        self.U = c64(li.gauge_field(s, rng))
+        self.psi = c64(li.spinor(rng, s.volume))
+        g = li._cgauss(rng, (s.volume, 2, 6, 6))
+        self.clover = c64(0.025 * (g + np.conj(np.swapaxes(g, -1, -2))))
+        self.v = c64(li.null_vectors(rng, s.nvec, s.volume) / np.sqrt(2.0 * 6 * (s.volume // s.cvolume)))
+        self.A = c64(li.coarse_matrix_synthetic(rng, s.cvolume, s.nvec))
+        self.threads = oracle.threads()
+
+    def step(self):
+        o, s = self.oracle, self.scfg
+        o.wilson_clover_mult(self.psi, self.U, self.clover, s.kappa, s.dims, s.bc)
+        o.wilson_clover_mult(self.psi, self.U, self.clover, s.kappa, s.dims, s.bc, dagger=True)
+        xc = o.restrict(self.psi, self.v, s.dims, s.block)
+        yc = o.coarse_mult(np.ascontiguousarray(xc.astype(np.complex64)), self.A, s.cdims)
+        o.prolong(np.ascontiguousarray(yc.astype(np.complex64)), self.v, s.dims, s.block)
+
+    def time(self, steps: int, warmup: int) -> float:
+        for _ in range(warmup):
+            self.step()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            self.step()
+        return (time.perf_counter() - t0) / steps
+
+    def describe(self) -> str:
+        s = self.scfg
+        return (f"whole 5-row step on a {'x'.join(map(str, s.dims))} lattice ({s.volume} sites) of the same recipe, "
+                f"block {'x'.join(map(str, s.block))}, nvec {s.nvec}, fp32-rounded inputs, fp64 arithmetic")
+
+
+def step_bytes(cfg: li.Config) -> int:
+    m = model(cfg)
+    return sum(m[k]["bytes"] for k in STEP_ORDER)
+
+
+def step_flops(cfg: li.Config) -> int:
+    m = model(cfg)
+    return sum(m[k]["flops"] for k in STEP_ORDER)
+
+
+def config_dict(cfg: li.Config, n_gpus: int) -> dict:
+    return {
+        "workload": (f"{cfg.name}: fine {'x'.join(map(str, cfg.dims))} ({cfg.volume} sites), block "
+                     f"{'x'.join(map(str, cfg.block))} -> coarse {'x'.join(map(str, cfg.cdims))}, nvec {cfg.nvec} "
+                     f"(N={2 * cfg.nvec}), {cfg.gauge} links, kappa {cfg.kappa}, bc {list(cfg.bc)}; step = D, D^dag, "
+                     f"restrict, coarse_mult, prolong on one right-hand side"),
+        "replicas": n_gpus, "parallelism": "replicas only (single-GPU path)",
+        "l2": "every operand stream of the timed kernels is larger than L2 at c4/c5; 4 rotating buffer sets",
+    }
+
+
+def run_reference(args, cfg: li.Config, ranks: Ranks):
+    if ranks.rank != 0:
+        return
+    smp = OracleSample(cfg)
+    sec = smp.time(args.steps, args.warmup)
+    val = step_bytes(smp.scfg) / sec / 1e9
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(cfg, args.gpus),
+        "gflops": step_flops(smp.scfg) / sec / 1e9,
+        "cpu_baseline": {"value": val, "unit": "GB/s", "cores": smp.threads, "kind": "oracle",
+                         "sample": smp.describe()},
+        "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, cfg: li.Config, ranks: Ranks):
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    dev_index = ranks.local_rank if ranks.world > 1 else 0
+    torch.cuda.set_device(dev_index)
+    device = torch.device("cuda", dev_index)
+    import paper_2111_05012_b200 as lq
+    W = Workload(cfg, device, seed=cfg.seed + 17 * ranks.rank)
+    m = model(cfg)
+    peak, peak_src = measured_peak()
+
+    sampler = ClockSampler(dev_index)
+    sampler.start()
+    total_s, per_kernel, launches = time_steps(W, args.steps, args.warmup, ranks)
+    clocks = sampler.stop()
+    max_s = ranks.max(total_s)
+    sec_per_step = max_s / args.steps
+    sbytes, sflops = step_bytes(cfg), step_flops(cfg)
+    value = whole_job_value(sbytes, ranks.world, sec_per_step) / 1e9
+
+    kernels = {}
+    for name in STEP_ORDER:
+        t = statistics.mean(per_kernel[name])
+        kernels[name] = {
+            "us": t * 1e6, "us_min": min(per_kernel[name]) * 1e6, "share": t * args.steps / total_s,
+            "GBps": m[name]["bytes"] / t / 1e9, "GFLOPs": m[name]["flops"] / t / 1e9,
+            "units_per_s": m[name]["units"] / t, "frac_of_hbm_peak": m[name]["bytes"] / t / 1e9 / peak,
+            "bytes_per_launch": m[name]["bytes"], "symbol": KERNEL_SYMBOL[name],
+        }
+    dominant = max(STEP_ORDER, key=lambda n: kernels[n]["us"])
+    roofline = {
+        "bound": "hbm", "kernel": dominant, "achieved": kernels[dominant]["GBps"], "peak": peak, "unit": "GB/s",
+        "frac": kernels[dominant]["GBps"] / peak, "traffic": recorded_traffic(cfg.name, dominant),
+        "peak_source": peak_src, "algorithmic_bytes_per_launch": m[dominant]["bytes"],
+    }
+    # the 12-real-link variant of A1 (config 4 asks for both storages), timed alone
+    extra = {}
+    if not args.no_extras:
+        t12 = time_single(W, "wilson_clover_12", reps=max(10, args.steps))
+        m12 = model(cfg, links12=True)["wilson_clover"]
+        extra["wilson_clover_links12"] = {"us": t12 * 1e6, "GBps": m12["bytes"] / t12 / 1e9,
+                                          "GFLOPs": m12["flops"] / t12 / 1e9, "units_per_s": m12["units"] / t12,
+                                          "frac_of_hbm_peak": m12["bytes"] / t12 / 1e9 / peak}
+
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)
+    e2e_s = ranks.max(e2e_s)
+    e2e = {"value": whole_job_value(sbytes, ranks.world, e2e_s) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps,
+           "note": "host-vector C-ABI calls, pinned canonical vectors; PCIe copies dominate"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": ranks.world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config_dict(cfg, ranks.world),
+        "gflops": whole_job_value(sflops, ranks.world, sec_per_step) / 1e9,
+        "fine_sites_per_s": whole_job_value(2 * cfg.volume, ranks.world, sec_per_step),
+        "frac_of_hbm_peak": value / ranks.world / peak,
+        "kernels": kernels, "extra": extra, "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if ranks.rank == 0 and ranks.world == 1 and not args.no_cpu_baseline:
+        smp = OracleSample(cfg)
+        sec = smp.time(3, 1)
+        line["cpu_baseline"] = {"value": step_bytes(smp.scfg) / sec / 1e9, "unit": "GB/s", "cores": smp.threads,
+                                "kind": "oracle", "sample": smp.describe(), "ms_per_step": sec * 1e3,
+                                "gflops": step_flops(smp.scfg) / sec / 1e9}
+    if ranks.rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", choices=sorted(li.CONFIGS), default="c5")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true")
+    args = ap.parse_args()
+    cfg = li.CONFIGS[args.workload]
+    if args.impl == "reference":
+        # rank 0 alone runs the oracle; the other ranks exit 0 without work (no process group needed)
+        if int(os.environ.get("RANK", "0")) == 0:
+            r = Ranks.__new__(Ranks)
+            r.rank, r.world, r.local_rank, r.dist = 0, 1, 0, None
+            run_reference(args, cfg, r)
+        return
+    ranks = Ranks()
+    if ranks.world != args.gpus and ranks.rank == 0:
+        print(f"[bench] note: --gpus {args.gpus} but WORLD_SIZE={ranks.world}; using WORLD_SIZE", file=sys.stderr)
+    try:
+        run_ours(args, cfg, ranks)
+    finally:
+        ranks.close()
+
+
+if __name__ == "__main__":
+    main()

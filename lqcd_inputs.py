@@ -273,3 +273,42 @@ def t_gauge_field(cfg: Config, gen, device):
     if cfg.gauge == "exp":
         return t_gauge_exp(gen, cfg.volume, cfg.eps, device)
     return t_gauge_haar(gen, cfg.volume, device)
+
+
+def t_spinor(gen, volume: int, device, dtype=None):
+    """Gaussian spinor (V, 4, 3); dtype = real dtype of the parts (float32 -> complex64)."""
+    return t_cgauss(gen, (volume, 4, 3), device, dtype)
+
+
+def t_coarse_vector(gen, cvolume: int, nvec: int, device, dtype=None):
+    return t_cgauss(gen, (cvolume, 2, nvec), device, dtype)
+
+
+def t_clover_synthetic(gen, volume: int, device, scale: float = 0.05, chunk: int = 1 << 20):
+    """Synthetic clover term for the two largest configs: per site two Hermitian 6x6
+    blocks F = scale * (G + G^dag) / 2, G complex Gaussian -- the magnitude of the true term at these kappa, c_sw
+    (|F| ~ 0.05-0.15).  complex64, canonical (V, 2, 6, 6).  The operator takes F as an input, so parity and
+    throughput do not depend on where F comes from."""
+    torch = _torch()
+    out = torch.empty((volume, 2, 6, 6), dtype=torch.complex64, device=device)
+    for lo in range(0, volume, chunk):
+        hi = min(lo + chunk, volume)
+        g = t_cgauss(gen, (hi - lo, 2, 6, 6), device, torch.float32)
+        out[lo:hi] = (0.5 * scale) * (g + torch.conj(g.transpose(-1, -2)))
+    return out
+
+
+def t_coarse_matrix_synthetic(gen, cvolume: int, nvec: int, device, chunk: int = 1 << 10):
+    """Device version of coarse_matrix_synthetic: A0 = 1 + 0.1 G, hop blocks 0.05 G; complex64 (Vc, 9, N, N)."""
+    torch = _torch()
+    n = 2 * nvec
+    out = torch.empty((cvolume, 9, n, n), dtype=torch.complex64, device=device)
+    eye = torch.eye(n, dtype=torch.complex64, device=device)
+    for lo in range(0, cvolume, chunk):
+        hi = min(lo + chunk, cvolume)
+        g = t_cgauss(gen, (hi - lo, 9, n, n), device, torch.float32)
+        g[:, 0] *= 0.1
+        g[:, 0] += eye
+        g[:, 1:] *= 0.05
+        out[lo:hi] = g
+    return out
