@@ -77,12 +77,17 @@ def measured_peak():
 
 
 def recorded_traffic(workload: str, kernel: str):
-    """dram bytes per launch from the committed ncu --set full capture (profiles/ncu_traffic.json), or None."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+    (profiles/ncu_traffic.csv: workload,kernel,dram_bytes_per_launch,...), or None if that row is absent."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f)[workload][kernel]["dram_bytes_per_launch"]
+        import csv
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and row["kernel"] == kernel:
+                    return float(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 # ----------------------------------------------------------------------------------------------------------

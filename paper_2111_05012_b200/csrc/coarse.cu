@@ -49,8 +49,10 @@ template <> __device__ __forceinline__ void cmadd<double>(double& sr, double& si
 }
 
 // LPR lanes per row (power of two <= 32), CPL vec16 per lane per row, R rows in flight per lane.
-template <typename T, int LPR, int CPL, int R>
-__global__ void __launch_bounds__(256) k_coarse(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ A,
+// FULL: N is a multiple of the row tile and a row is exactly LPR*CPL vec16 -- no bounds predicates, so the loads of
+// a tile are unconditional and stay batched at the top of the tile.
+template <typename T, int LPR, int CPL, int R, bool FULL>
+__global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ A,
                                                 CoarseParams P) {
     constexpr int NV = VecOf<T>::NV;
     constexpr int CPV = NV / 2;  // complex per vec16
@@ -86,7 +88,7 @@ __global__ void __launch_bounds__(256) k_coarse(T* __restrict__ out, const T* __
 #pragma unroll
         for (int c = 0; c < CPL; c++) {
             const int v = q + LPR * c;
-            if (v < P.RV) {
+            if (FULL || v < P.RV) {
                 xv[d][c] = ld16(in + ((long long)src[d] * P.RV + v) * NV);
                 if (P.dagger) {
 #pragma unroll
@@ -118,7 +120,7 @@ __global__ void __launch_bounds__(256) k_coarse(T* __restrict__ out, const T* __
 #pragma unroll
                 for (int c = 0; c < CPL; c++) {
                     const int v = q + LPR * c;
-                    if (row < P.N && v < P.RV)
+                    if (FULL || (row < P.N && v < P.RV))
                         a[r][d][c] = ld16_stream(Asite + (((long long)d * P.N + row) * P.RV + v) * NV);
                     else {
 #pragma unroll
@@ -141,7 +143,7 @@ __global__ void __launch_bounds__(256) k_coarse(T* __restrict__ out, const T* __
                 si[r] += __shfl_xor_sync(0xffffffffu, si[r], off);
             }
             const int row = rbase + r * G + g;
-            if (q == 0 && row < P.N) {
+            if (q == 0 && (FULL || row < P.N)) {
                 T s = (P.dagger && row >= P.nvec) ? (T)-1 : (T)1;
                 T* o = out + ((long long)X * P.N + row) * 2;
                 o[0] = s * sr[r];
@@ -155,18 +157,21 @@ template <typename T, int LPR, int CPL, int R>
 static void launch_coarse(T* out, const T* in, const T* A, CoarseParams P, cudaStream_t st) {
     constexpr int G = 32 / LPR;
     P.ntile = (P.N + G * R - 1) / (G * R);
-    // rows tiles per warp: as many as possible while the grid still fills the machine (>= 148 SMs x 32 warps)
+    // row tiles per warp: as many as possible (the nine source slices are loaded once per warp) while the grid
+    // still has several waves of warps (>= 148 SMs x 256 warp tasks)
     int tpw = g_knobs.coarse_rows_per_warp > 0 ? g_knobs.coarse_rows_per_warp : P.ntile;
     if (tpw > P.ntile) tpw = P.ntile;
     while (tpw > 1 && (P.ntile % tpw != 0 ||
-                       (g_knobs.coarse_rows_per_warp <= 0 && (long long)P.Vc * (P.ntile / tpw) < 148LL * 32)))
+                       (g_knobs.coarse_rows_per_warp <= 0 && (long long)P.Vc * (P.ntile / tpw) < 148LL * 256)))
         tpw--;
     P.tpw = tpw;
     P.ntask = (long long)P.Vc * (P.ntile / tpw);
     int warps = g_knobs.coarse_warps > 0 ? g_knobs.coarse_warps : 4;
     if (warps > 8) warps = 8;
     const long long grid = (P.ntask + warps - 1) / warps;
-    k_coarse<T, LPR, CPL, R><<<(unsigned)grid, warps * 32, 0, st>>>(out, in, A, P);
+    const bool full = (P.N % (G * R) == 0) && (P.RV == LPR * CPL);
+    if (full) k_coarse<T, LPR, CPL, R, true><<<(unsigned)grid, warps * 32, 0, st>>>(out, in, A, P);
+    else k_coarse<T, LPR, CPL, R, false><<<(unsigned)grid, warps * 32, 0, st>>>(out, in, A, P);
 }
 
 template <typename T>
@@ -215,7 +220,11 @@ static int coarse_call(T* out, const T* in, const T* A, const int cdims[4], int 
     else if (RV <= 4) launch_coarse<T, 4, 1, 2>(out, in, A, P, st);
     else if (RV <= 8) launch_coarse<T, 8, 1, 2>(out, in, A, P, st);
     else if (RV <= 16) launch_coarse<T, 16, 1, 2>(out, in, A, P, st);
-    else if (RV <= 32) launch_coarse<T, 32, 1, 2>(out, in, A, P, st);
+    else if (RV <= 32) {
+        if (g_knobs.coarse_R == 1) launch_coarse<T, 32, 1, 1>(out, in, A, P, st);
+        else if (g_knobs.coarse_R == 4) launch_coarse<T, 32, 1, 4>(out, in, A, P, st);
+        else launch_coarse<T, 32, 1, 2>(out, in, A, P, st);
+    }
     else if (RV <= 64) launch_coarse<T, 32, 2, 1>(out, in, A, P, st);
     else if (RV <= 96) launch_coarse<T, 32, 3, 1>(out, in, A, P, st);
     else launch_coarse<T, 32, 4, 1>(out, in, A, P, st);

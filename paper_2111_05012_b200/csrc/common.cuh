@@ -68,7 +68,8 @@ template <typename T> __device__ __forceinline__ V16<T> ld16(const T* p) {
 }
 // Read-only, L1 no-allocate, L2 evict-first: data streamed exactly once (clover, coarse blocks, null vectors).
 // (The plain .L2::evict_first qualifier exists only for 256-bit loads on sm_100a, hence the policy operand;
-// createpolicy is loop-invariant and gets hoisted.)
+// createpolicy is loop-invariant and gets hoisted.)  The loads are `volatile` so that a batch of them written
+// back to back stays back to back (front-loaded memory-level parallelism) instead of being sunk to their uses.
 template <typename T> __device__ __forceinline__ V16<T> ld16_stream(const T* p);
 __device__ __forceinline__ uint64_t evict_first_policy() {
     uint64_t pol;
@@ -77,14 +78,14 @@ __device__ __forceinline__ uint64_t evict_first_policy() {
 }
 template <> __device__ __forceinline__ V16<float> ld16_stream<float>(const float* p) {
     V16<float> v;
-    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
                  : "=f"(v.r[0]), "=f"(v.r[1]), "=f"(v.r[2]), "=f"(v.r[3])
                  : "l"(p), "l"(evict_first_policy()));
     return v;
 }
 template <> __device__ __forceinline__ V16<double> ld16_stream<double>(const double* p) {
     V16<double> v;
-    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
                  : "=d"(v.r[0]), "=d"(v.r[1])
                  : "l"(p), "l"(evict_first_policy()));
     return v;

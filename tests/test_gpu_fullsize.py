@@ -1,0 +1,196 @@
+"""Parity at BASELINE.json's full sizes (configs 4 and 5), in the launch configuration bench.py times (default
+knobs), on SAMPLED outputs the oracle computes one by one, plus properties that hold at any size (-m gpu).
+
+Inputs are generated on the device with the seeded generators of lqcd_inputs.py; the
+oracle gets the very same fp32 values:
+  * fine operator: time-slabs of the canonical fields are copied into lazily-committed full-size host arrays
+    (only the touched pages exist), the oracle's *_sites entry point evaluates Eq. 1 at sampled sites whose
+    neighbours all lie in those slabs (both t boundaries, the lattice corners and the bulk are covered);
+  * coarse operator: the oracle's *_sites entry point takes only the nine blocks of the sampled coarse sites;
+  * restrict / prolong are aggregate-local, so 16 sampled aggregates are gathered into a fake 8^4 lattice of
+    4^4 blocks on which the oracle runs as it stands.
+"""
+import numpy as np
+import pytest
+
+import lqcd_inputs as li
+import oracle
+
+pytestmark = pytest.mark.gpu
+TOL32 = 2e-6
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.complex128).ravel()
+    b = np.asarray(b, dtype=np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def site_index(dims, c):
+    return c[..., 0] + dims[0] * (c[..., 1] + dims[1] * (c[..., 2] + dims[2] * c[..., 3]))
+
+
+def sample_fine_sites(cfg, rng, n):
+    """sites with t in {0, 1, Lt/2, Lt-1} (both sides of the antiperiodic boundary and the bulk) + the corners"""
+    L = np.array(cfg.dims)
+    ts = np.array([0, 1, L[3] // 2, L[3] - 1])
+    c = np.stack([rng.integers(0, L[0], n), rng.integers(0, L[1], n), rng.integers(0, L[2], n),
+                  ts[rng.integers(0, len(ts), n)]], axis=1)
+    corners = np.array([[x, y, z, t] for x in (0, L[0] - 1) for y in (0, L[1] - 1) for z in (0, L[2] - 1)
+                        for t in (0, L[3] - 1)])
+    c = np.concatenate([corners, c])
+    slabs = sorted({int(v) % int(L[3]) for t in ts for v in (t - 1, t, t + 1)})
+    return site_index(cfg.dims, c).astype(np.int64), slabs
+
+
+def lazily_filled(shape, dtype, dev_tensor, slabs, v3, site_axis):
+    """full-size host array (uninitialised, pages committed on touch) holding only the given time-slabs"""
+    host = np.empty(shape, dtype=dtype)
+    for t in slabs:
+        sl = [slice(None)] * len(shape)
+        sl[site_axis] = slice(t * v3, (t + 1) * v3)
+        host[tuple(sl)] = dev_tensor[tuple(sl)].cpu().numpy()
+    return host
+
+
+@pytest.fixture(scope="module")
+def lq():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2111_05012_b200 as lq
+    return lq
+
+
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_fullsize_wilson_clover_sampled(lq, name):
+    import torch
+    cfg = li.CONFIGS[name]
+    V, L = cfg.volume, cfg.dims
+    v3 = L[0] * L[1] * L[2]
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed)
+    U = li.t_gauge_field(cfg, gen, "cuda").to(torch.complex64)
+    cl = li.t_clover_synthetic(gen, V, "cuda")
+    psi = li.t_spinor(gen, V, "cuda", torch.float32)
+    chi = li.t_spinor(gen, V, "cuda", torch.float32)
+    U18, U12 = lq.pack_gauge(U, L), lq.pack_gauge(U, L, links12=True)
+    Cn = lq.pack_clover(cl, L)
+    x, w = lq.pack_spinor(psi, L), lq.pack_spinor(chi, L)
+    y = lq.empty_spinor(L)
+
+    rng = np.random.default_rng(cfg.seed)
+    sites, slabs = sample_fine_sites(cfg, rng, 3000)
+    U_h = lazily_filled((4, V, 3, 3), np.complex64, U, slabs, v3, 1)
+    cl_h = lazily_filled((V, 2, 6, 6), np.complex64, cl, slabs, v3, 0)
+    psi_h = lazily_filled((V, 4, 3), np.complex64, psi, slabs, v3, 0)
+    sites_d = torch.from_numpy(sites).cuda()
+
+    results = {}
+    for label, Un, dag, l12 in (("D", U18, False, False), ("Ddag", U18, True, False), ("D_links12", U12, False, True)):
+        lq.wilson_clover_mult(y, x, Un, Cn, cfg.kappa, L, cfg.bc, dagger=dag, links12=l12)
+        yc = lq.unpack_spinor(y, L)
+        got = yc[sites_d].cpu().numpy()
+        ref = oracle.wilson_clover_mult_sites(psi_h, U_h, cl_h, cfg.kappa, L, cfg.bc, sites, dagger=dag)
+        assert np.isfinite(got).all()
+        assert rel_l2(got, ref) <= TOL32, label
+        # no sampled site is individually off either (catches a wrong neighbour at a single boundary site)
+        per_site = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / np.linalg.norm(
+            ref.reshape(len(sites), -1), axis=1)
+        assert per_site.max() <= 5 * TOL32, (label, int(sites[per_site.argmax()]))
+        results[label] = yc
+    # property at full size: gamma5-hermiticity <chi, D psi> = <D^dag chi, psi> (Eq. 2), fp64 sums
+    lq.wilson_clover_mult(y, w, U18, Cn, cfg.kappa, L, cfg.bc, dagger=True)
+    ddag_chi = lq.unpack_spinor(y, L)
+    lhs = torch.sum(torch.conj(chi.to(torch.complex128)) * results["D"].to(torch.complex128))
+    rhs = torch.sum(torch.conj(ddag_chi.to(torch.complex128)) * psi.to(torch.complex128))
+    assert abs((lhs - rhs).item()) <= 1e-5 * abs(lhs.item())
+    # 12-real links reproduce the 18-real result up to fp32 rounding of the rebuilt third row
+    d = (results["D_links12"] - results["D"]).to(torch.complex128)
+    assert (torch.linalg.vector_norm(d) / torch.linalg.vector_norm(results["D"].to(torch.complex128))).item() <= TOL32
+
+
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_fullsize_coarse_sampled(lq, name):
+    import torch
+    cfg = li.CONFIGS[name]
+    Lc, Vc, nv = cfg.cdims, cfg.cvolume, cfg.nvec
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed + 1)
+    A = li.t_coarse_matrix_synthetic(gen, Vc, nv, "cuda")
+    xc = li.t_coarse_vector(gen, Vc, nv, "cuda", torch.float32)
+    yc = torch.empty_like(xc)
+    rng = np.random.default_rng(cfg.seed + 1)
+    Lca = np.array(Lc)
+    corners = np.array([[x, y, z, t] for x in (0, Lca[0] - 1) for y in (0, Lca[1] - 1) for z in (0, Lca[2] - 1)
+                        for t in (0, Lca[3] - 1)])
+    rnd = np.stack([rng.integers(0, Lca[mu], 112) for mu in range(4)], axis=1)
+    sites = site_index(Lc, np.concatenate([corners, rnd])).astype(np.int64)
+    A_s = A[torch.from_numpy(sites).cuda()].cpu().numpy()
+    xc_h = xc.cpu().numpy()
+    for dag in (False, True):
+        lq.coarse_mult(yc, xc, A, Lc, nv, dagger=dag)
+        got = yc[torch.from_numpy(sites).cuda()].cpu().numpy()
+        ref = oracle.coarse_mult_sites(xc_h, A_s, Lc, sites, dagger=dag)
+        assert rel_l2(got, ref) <= TOL32, dag
+        per_site = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / np.linalg.norm(
+            ref.reshape(len(sites), -1), axis=1)
+        assert per_site.max() <= 5 * TOL32
+    # property at full size: linearity D_c(a x + z) = a D_c x + D_c z on the whole lattice
+    z = li.t_coarse_vector(gen, Vc, nv, "cuda", torch.float32)
+    a = 0.5 - 0.25j
+    y1, y2, y3 = torch.empty_like(xc), torch.empty_like(xc), torch.empty_like(xc)
+    lq.coarse_mult(y1, xc, A, Lc, nv)
+    lq.coarse_mult(y2, z, A, Lc, nv)
+    lq.coarse_mult(y3, (a * xc + z).contiguous(), A, Lc, nv)
+    err = torch.linalg.vector_norm((y3 - (a * y1 + y2)).to(torch.complex128)) / torch.linalg.vector_norm(
+        y3.to(torch.complex128))
+    assert err.item() <= 4 * TOL32
+
+
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_fullsize_restrict_prolong_sampled(lq, name):
+    import torch
+    cfg = li.CONFIGS[name]
+    L, b, nv, V, Vc, Lc = cfg.dims, cfg.block, cfg.nvec, cfg.volume, cfg.cvolume, cfg.cdims
+    assert tuple(b) == (4, 4, 4, 4)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed + 2)
+    rng = np.random.default_rng(cfg.seed + 2)
+    # 16 sampled aggregates (the two opposite corners included) -> fake 8^4 lattice of 2^4 blocks
+    Lca = np.array(Lc)
+    Xs = np.stack([rng.integers(0, Lca[mu], 16) for mu in range(4)], axis=1)
+    Xs[0] = 0
+    Xs[1] = Lca - 1
+    fdims = (8, 8, 8, 8)
+    fc = li.site_coords(fdims)                       # fake fine coords
+    k = site_index((2, 2, 2, 2), fc // 4)            # fake coarse site of each fake fine site
+    real = site_index(L, Xs[k] * 4 + fc % 4)         # the real fine site it stands for
+    real_d = torch.from_numpy(real.astype(np.int64)).cuda()
+    Xreal = site_index(Lc, Xs).astype(np.int64)      # real coarse index of fake coarse site k
+    Xreal_d = torch.from_numpy(Xreal).cuda()
+
+    vn = torch.empty(lq.native_nullvecs_reals(L, b, nv), dtype=torch.float32, device="cuda")
+    v_fake = np.empty((nv, 4096, 4, 3), dtype=np.complex64)
+    scale = 1.0 / np.sqrt(2.0 * 6 * 256)
+    for i in range(nv):
+        vi = li.t_spinor(gen, V, "cuda", torch.float32) * scale
+        lq.pack_nullvec(vn, vi, i, L, b, nv)
+        v_fake[i] = vi[real_d].cpu().numpy()
+        del vi
+    psi = li.t_spinor(gen, V, "cuda", torch.float32)
+    xc = li.t_coarse_vector(gen, Vc, nv, "cuda", torch.float32)
+    x = lq.pack_spinor(psi, L)
+    out_c = torch.empty((Vc, 2, nv), dtype=torch.complex64, device="cuda")
+    out_f = lq.empty_spinor(L)
+    lq.restrict(out_c, x, vn, L, b, nv)
+    lq.prolong(out_f, xc, vn, L, b, nv)
+    got_r = out_c[Xreal_d].cpu().numpy()
+    ref_r = oracle.restrict(psi[real_d].cpu().numpy(), v_fake, fdims, b)
+    assert rel_l2(got_r, ref_r) <= TOL32
+    got_p = lq.unpack_spinor(out_f, L)[real_d].cpu().numpy()
+    ref_p = oracle.prolong(xc[Xreal_d].cpu().numpy(), v_fake, fdims, b)
+    assert rel_l2(got_p, ref_p) <= TOL32
+    # property at full size: adjointness <restrict(psi), xc> = <psi, prolong(xc)> (Eqs. 5, 6), fp64 sums
+    lhs = torch.sum(torch.conj(out_c.to(torch.complex128)) * xc.to(torch.complex128))
+    rhs = torch.sum(torch.conj(psi.to(torch.complex128)) * lq.unpack_spinor(out_f, L).to(torch.complex128))
+    assert abs((lhs - rhs).item()) <= 1e-5 * abs(lhs.item())
