@@ -512,6 +512,63 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """Config 5's bandwidth-roofline sweep: the fp32 fine operator (and D^dag) and the coarse operator over volumes
+    8^3x16 ... 48^3x96 (and the matching coarse lattices, block 4^4, nvec 32): algorithmic GB/s versus footprint,
+    showing the L2 -> HBM transition.  Operator fields are random numbers written straight into the native layouts
+    (throughput does not depend on values); two buffer sets alternate.  One JSON line."""
+    import torch
+    import paper_2111_05012_b200 as lq
+    torch.cuda.set_device(0)
+    peak, peak_src = measured_peak()
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5)
+    rnd = lambda n, s=1.0: torch.randn(n, device="cuda", dtype=torch.float32, generator=gen) * s
+    out = []
+    for l in (8, 16, 24, 32, 40, 48):
+        dims, cd, nv = (l, l, l, 2 * l), (l // 4, l // 4, l // 4, l // 2), 32
+        cfg = li.Config(f"sweep{l}", dims, (4, 4, 4, 4), nv, "haar", 0.0, 0.1372, 1.7)
+        m = model(cfg)
+        U, cl = rnd(lq.native_gauge_reals(dims)), rnd(lq.native_clover_reals(dims), 0.05)
+        x = [rnd(lq.native_spinor_reals(dims)) for _ in range(2)]
+        y = [torch.empty_like(x[0]) for _ in range(2)]
+        A = rnd(lq.native_coarse_mat_reals(cd, nv), 0.05)
+        xc = [rnd(lq.native_coarse_vec_reals(cd, nv)) for _ in range(2)]
+        yc = [torch.empty_like(xc[0]) for _ in range(2)]
+        reps = max(20, min(400, int(2e9 / m["wilson_clover"]["bytes"]) * 10))
+
+        def timed(f):
+            for k in range(5):
+                f(k % 2)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for k in range(reps):
+                f(k % 2)
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) * 1e-3 / reps
+
+        t_d = timed(lambda i: lq.wilson_clover_mult(y[i], x[i], U, cl, cfg.kappa, dims, cfg.bc))
+        t_dd = timed(lambda i: lq.wilson_clover_mult(y[i], x[i], U, cl, cfg.kappa, dims, cfg.bc, dagger=True))
+        t_c = timed(lambda i: lq.coarse_mult(yc[i], xc[i], A, cd, nv))
+        fb, cb = m["wilson_clover"]["bytes"], m["coarse_mult"]["bytes"]
+        out.append({
+            "fine_dims": list(dims), "coarse_dims": list(cd), "reps": reps,
+            "fine_footprint_MB": (fb + 96 * cfg.volume) / 1e6, "coarse_footprint_MB": cb / 1e6,
+            "wilson_clover": {"us": t_d * 1e6, "GBps": fb / t_d / 1e9, "GFLOPs": m["wilson_clover"]["flops"] / t_d / 1e9,
+                              "frac_of_hbm_peak": fb / t_d / 1e9 / peak},
+            "wilson_clover_dagger": {"us": t_dd * 1e6, "GBps": fb / t_dd / 1e9, "frac_of_hbm_peak": fb / t_dd / 1e9 / peak},
+            "coarse_mult": {"us": t_c * 1e6, "GBps": cb / t_c / 1e9, "GFLOPs": m["coarse_mult"]["flops"] / t_c / 1e9,
+                            "frac_of_hbm_peak": cb / t_c / 1e9 / peak},
+        })
+        del U, cl, x, y, A, xc, yc
+    print(json.dumps({"metric": METRIC, "sweep": out, "unit": "GB/s", "peak": peak, "peak_source": peak_src,
+                      "dtype": "f32", "data": "synthetic",
+                      "note": "footprints below ~126 MB are L2-resident across repetitions: GB/s there is not an HBM figure"}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -522,8 +579,12 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="config 5's bandwidth-roofline sweep over volumes (1 GPU)")
     args = ap.parse_args()
     cfg = li.CONFIGS[args.workload]
+    if args.sweep:
+        run_sweep(args)
+        return
     if args.impl == "reference":
         # rank 0 alone runs the oracle; the other ranks exit 0 without work (no process group needed)
         if int(os.environ.get("RANK", "0")) == 0:

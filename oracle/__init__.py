@@ -184,3 +184,30 @@ def coarse_mult_sites(xc, A_sites, cdims, sites, dagger=False) -> np.ndarray:
             _ptr(sites), C.c_long(len(sites)))
     _check(rc, "coarse_mult_sites")
     return out
+
+
+def wilson_clover_dd_mult(psi, U, clover, kappa, dims, bc, domain, parity=0, dagger=False) -> np.ndarray:
+    """F1, D_SAP: D with the hops across domain boundaries off; parity 0/1/2 = all/even/odd domains."""
+    psi, U, clover = _c(psi), _c(U), _c(clover)
+    V = int(np.prod(dims))
+    assert psi.shape == (V, 4, 3) and U.shape == (4, V, 3, 3) and clover.shape == (V, 2, 6, 6)
+    out = np.empty((V, 4, 3), dtype=np.complex128)
+    fn = getattr(lib(), "lqcd_wilson_clover_dd_mult" + _kind(psi, U, clover))
+    fn.restype = C.c_int
+    rc = fn(_ptr(out), _ptr(psi), _ptr(U), _ptr(clover), C.c_double(kappa), _i4(dims), _i4(bc), _i4(domain),
+            C.c_int(parity), C.c_uint(DAGGER if dagger else 0))
+    _check(rc, "wilson_clover_dd_mult")
+    return out
+
+
+def wilson_clover_dd_mult_sites(psi, U, clover, kappa, dims, bc, domain, sites, parity=0, dagger=False) -> np.ndarray:
+    """D_SAP at the listed canonical site indices only -> (len(sites), 4, 3)."""
+    psi, U, clover = _c(psi), _c(U), _c(clover)
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.empty((len(sites), 4, 3), dtype=np.complex128)
+    fn = getattr(lib(), "lqcd_wilson_clover_dd_mult_sites" + _kind(psi, U, clover))
+    fn.restype = C.c_int
+    rc = fn(_ptr(out), _ptr(psi), _ptr(U), _ptr(clover), C.c_double(kappa), _i4(dims), _i4(bc), _i4(domain),
+            C.c_int(parity), C.c_uint(DAGGER if dagger else 0), _ptr(sites), C.c_long(len(sites)))
+    _check(rc, "wilson_clover_dd_mult_sites")
+    return out

@@ -20,7 +20,9 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): free-field plane waves (closed form),
  * constant-abelian-background plane waves, gamma algebra, gamma5-hermiticity (Eq. 2), gauge
  * covariance, constant-field clover closed form, R P = 1, adjointness of R and P, dense
- * brute-force P^dag D P, coarse gamma5-hermiticity, coarse_mult == restrict(D(prolong)).
+ * brute-force P^dag D P, coarse gamma5-hermiticity, coarse_mult == restrict(D(prolong));
+ * D_SAP (F1): dense D masked by "same domain", single-domain and one-site-domain limits, block
+ * structure, even + odd = all, gamma5-hermiticity.
  * No routine in this file is "parity unpinned".
  */
 #include <complex.h>
@@ -713,6 +715,130 @@ int FN(lqcd_coarse_mult_sites)(zc* out, const inc* in, const inc* A_sites, const
     for (long n = 0; n < nsites; n++) {
         coarse_site(out + n * N, in, A_sites + n * 9 * (long)N * N, Lc, nvec, (flags & LQCD_REF_DAGGER) != 0,
                     sites[n]);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * F1. Domain-decomposed operator D_SAP: "the Dirac matrix D_SAP [is defined] by turning
+ * off the interaction across the domains"; the domains are the aggregation blocks b[4] ("We set the SAP
+ * domain to be the same as the domain of coarsening").  Eq. 1 with every hop whose two ends lie in
+ * different domains dropped; everything else (clover, kappa, boundary phase on hops that wrap inside a
+ * domain spanning the whole direction) as in D.
+ * "Splitting the domains into even and odd groups, D_SAP^(e) and D_SAP^(o)": the parity of a domain is
+ * (X_x + X_y + X_z + X_t) mod 2 of its coarse coordinates; D_SAP^(e) = P_e D_SAP P_e with P_e the projector
+ * on the sites of even domains (D_SAP is block diagonal, so this is D_SAP on even domains and 0 elsewhere).
+ *   parity: 0 = all domains, 1 = even domains only, 2 = odd domains only (output 0 on the others).
+ * Dagger as for D (gamma5 commutes with the domain projectors).
+ * Here a coarse extent of 1 is allowed (a single domain in that direction: no hop is dropped).
+ * ---------------------------------------------------------------------------------------- */
+static int domain_parity(const int L[4], const int b[4], long s) {
+    int x[4], p = 0;
+    coords_of(L, s, x);
+    for (int mu = 0; mu < 4; mu++) p += x[mu] / b[mu];
+    return p & 1;
+}
+
+static void dirac_dd_site(zc out[4][3], const inc* in, const inc* U, const inc* clover, double kappa,
+                          const int L[4], const int bc[4], const int b[4], const int Lc[4], int parity, int dagger,
+                          long s) {
+    const long V = volume_of(L);
+    if ((parity == 1 && domain_parity(L, b, s) != 0) || (parity == 2 && domain_parity(L, b, s) != 1)) {
+        memset(out, 0, sizeof(zc) * 12);
+        return;
+    }
+    zc g5m[4][4];
+    gamma5(g5m);
+    const zc(*g5)[4] = dagger ? g5m : NULL;
+    const long X = coarse_site_of(L, b, Lc, s);
+    zc psi[4][3], acc[4][3];
+    load_spinor(psi, in, s, g5);
+    memcpy(acc, psi, sizeof(acc));
+    for (int chi = 0; chi < 2; chi++)
+        for (int k = 0; k < 6; k++) {
+            zc sum = 0;
+            for (int l = 0; l < 6; l++)
+                sum += (zc)clover[((s * 2 + chi) * 6 + k) * 6 + l] * psi[2 * chi + l / 3][l % 3];
+            acc[2 * chi + k / 3][k % 3] += sum;
+        }
+    for (int mu = 0; mu < 4; mu++)
+        for (int dir = +1; dir >= -1; dir -= 2) {
+            int wrapped;
+            const long y = neighbour(L, s, mu, dir, &wrapped);
+            if (coarse_site_of(L, b, Lc, y) != X) continue; /* the hop crosses a domain boundary: off */
+            const double phase = wrapped ? (double)bc[mu] : 1.0;
+            zc nb[4][3], t[4][3];
+            load_spinor(nb, in, y, g5);
+            for (int be = 0; be < 4; be++)
+                for (int a = 0; a < 3; a++) {
+                    zc sum = 0;
+                    for (int c = 0; c < 3; c++)
+                        sum += (dir > 0 ? link_elem(U, V, mu, s, a, c) : conj(link_elem(U, V, mu, y, c, a))) * nb[be][c];
+                    t[be][a] = sum;
+                }
+            for (int al = 0; al < 4; al++)
+                for (int a = 0; a < 3; a++) {
+                    zc sum = 0;
+                    for (int be = 0; be < 4; be++)
+                        sum += ((al == be ? 1.0 : 0.0) - (double)dir * GAMMA[mu][al][be]) * t[be][a];
+                    acc[al][a] -= kappa * phase * sum;
+                }
+        }
+    if (!dagger) {
+        memcpy(out, acc, sizeof(acc));
+        return;
+    }
+    for (int a = 0; a < 4; a++)
+        for (int c = 0; c < 3; c++) {
+            zc sum = 0;
+            for (int be = 0; be < 4; be++) sum += g5m[a][be] * acc[be][c];
+            out[a][c] = sum;
+        }
+}
+
+static int check_domain(const int L[4], const int b[4], int Lc[4]) {
+    for (int mu = 0; mu < 4; mu++) {
+        if (L[mu] < 1 || b[mu] < 1 || L[mu] % b[mu]) return -1;
+        Lc[mu] = L[mu] / b[mu];
+    }
+    return 0;
+}
+
+/* out[V][4][3] = D_SAP in;  flags & 1: dagger;  parity 0 / 1 / 2 = all / even / odd domains */
+int FN(lqcd_wilson_clover_dd_mult)(zc* out, const inc* in, const inc* U, const inc* clover, double kappa,
+                                   const int L[4], const int bc[4], const int b[4], int parity, unsigned flags) {
+    int Lc[4];
+    if (!out || !in || !U || !clover || !b || check_dims_bc(L, bc) || check_domain(L, b, Lc) || parity < 0 ||
+        parity > 2)
+        return -1;
+    const long V = volume_of(L);
+    const int dagger = (flags & LQCD_REF_DAGGER) != 0;
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < V; s++) {
+        zc r[4][3];
+        dirac_dd_site(r, in, U, clover, kappa, L, bc, b, Lc, parity, dagger, s);
+        memcpy(out + s * 12, r, sizeof(r));
+    }
+    return 0;
+}
+
+/* the same at listed sites only (sampled parity at full size) */
+int FN(lqcd_wilson_clover_dd_mult_sites)(zc* out, const inc* in, const inc* U, const inc* clover, double kappa,
+                                         const int L[4], const int bc[4], const int b[4], int parity, unsigned flags,
+                                         const long* sites, long nsites) {
+    int Lc[4];
+    if (!out || !in || !U || !clover || !b || !sites || check_dims_bc(L, bc) || check_domain(L, b, Lc) ||
+        parity < 0 || parity > 2)
+        return -1;
+    const long V = volume_of(L);
+    const int dagger = (flags & LQCD_REF_DAGGER) != 0;
+    for (long n = 0; n < nsites; n++)
+        if (sites[n] < 0 || sites[n] >= V) return -1;
+#pragma omp parallel for schedule(static)
+    for (long n = 0; n < nsites; n++) {
+        zc r[4][3];
+        dirac_dd_site(r, in, U, clover, kappa, L, bc, b, Lc, parity, dagger, sites[n]);
+        memcpy(out + n * 12, r, sizeof(r));
     }
     return 0;
 }

@@ -418,10 +418,18 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
     const unsigned grid = (unsigned)ntiles;
 #define LAUNCH(DAG, L12)                                                                                  \
     do {                                                                                                  \
-        if (threads <= 128)                                                                               \
-            k_wilson_clover<T, DAG, L12, 128, (sizeof(T) == 4 ? 4 : 2)>                                   \
+        /* registers per thread: fp32 128 (4 CTAs/SM), fp64 168 (3 CTAs/SM) measured best on B200;      */ \
+        /* fine_variant 1 / 2 select fewer / more resident CTAs for experiments                          */ \
+        if (threads <= 128 && g_knobs.fine_variant == 1)                                                  \
+            k_wilson_clover<T, DAG, L12, 128, (sizeof(T) == 4 ? 3 : 2)>                                   \
                 <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
-        else                                                                                              \
+        else if (threads <= 128 && g_knobs.fine_variant == 2)                                             \
+            k_wilson_clover<T, DAG, L12, 128, (sizeof(T) == 4 ? 5 : 4)>                                   \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
+        else if (threads <= 128)                                                                          \
+            k_wilson_clover<T, DAG, L12, 128, (sizeof(T) == 4 ? 4 : 3)>                                   \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
+        else                                                                                           \
             k_wilson_clover<T, DAG, L12, 256, (sizeof(T) == 4 ? 2 : 1)>                                   \
                 <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
     } while (0)

@@ -432,3 +432,88 @@ def test_oracle_rejects_bad_arguments(c1):
         oracle.restrict(c1["psi"][0], c1["v"], cfg.dims, (3, 2, 2, 2))
     with pytest.raises(ValueError):
         oracle.coarse_mult(np.zeros((4, 2, 2), dtype=np.complex128), np.zeros((4, 9, 4, 4), dtype=np.complex128), (1, 2, 2, 1))
+
+
+# ------------------------------------------------------------------------------------------------
+# F1  D_SAP: D with the interaction across domains switched off; even/odd domain groups.
+#     Pinned to the (already pinned) D: dense D masked by "same domain", single-domain limit, block
+#     structure, e + o = all, gamma5-hermiticity.
+# ------------------------------------------------------------------------------------------------
+
+
+def domain_index(dims, block):
+    c = li.site_coords(dims) // np.array(block)
+    lc = [d // b for d, b in zip(dims, block)]
+    return c[:, 0] + lc[0] * (c[:, 1] + lc[1] * (c[:, 2] + lc[2] * c[:, 3])), c.sum(axis=1) % 2
+
+
+@pytest.mark.parametrize("dims,block,bc", [
+    ((4, 4, 2, 4), (2, 2, 1, 2), (1, 1, 1, -1)),   # extent-2 direction with two domains (x+mu == x-mu, both cross)
+    ((4, 2, 2, 6), (2, 2, 2, 3), (-1, 1, 1, -1)),  # directions spanned by a single domain keep their wrapping hops
+])
+def test_dsap_is_dense_D_masked_by_domain(dims, block, bc):
+    """Brute force: dense D from unit vectors (pinned above), entries between different domains zeroed."""
+    V = int(np.prod(dims))
+    rng = np.random.default_rng(21)
+    U = li.gauge_exp(rng, V, 0.6)
+    clov = oracle.clover_from_links(U, 0.13, 1.2, dims)
+    n = 12 * V
+    D = np.zeros((n, n), dtype=np.complex128)
+    Ds = np.zeros((n, n), dtype=np.complex128)
+    Dsd = np.zeros((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1
+        e = e.reshape(V, 4, 3)
+        D[:, k] = oracle.wilson_clover_mult(e, U, clov, 0.13, dims, bc).ravel()
+        Ds[:, k] = oracle.wilson_clover_dd_mult(e, U, clov, 0.13, dims, bc, block).ravel()
+        Dsd[:, k] = oracle.wilson_clover_dd_mult(e, U, clov, 0.13, dims, bc, block, dagger=True).ravel()
+    dom, par = domain_index(dims, block)
+    dom12, par12 = np.repeat(dom, 12), np.repeat(par, 12)
+    same = dom12[:, None] == dom12[None, :]
+    assert np.max(np.abs(Ds - np.where(same, D, 0))) < 1e-15
+    assert np.max(np.abs(D - Ds)) > 1e-3, "the mask removes something"
+    assert np.max(np.abs(Dsd - Ds.conj().T)) < 1e-14, "D_SAP^dag via gamma5 is the dense adjoint"
+    # even / odd groups: P_e D_SAP P_e
+    x = li.spinor(rng, V)
+    for parity in (1, 2):
+        keep = (par12 == parity - 1)
+        ref = np.where(keep, Ds @ np.where(keep, x.ravel(), 0), 0)
+        got = oracle.wilson_clover_dd_mult(x, U, clov, 0.13, dims, bc, block, parity=parity).ravel()
+        assert np.max(np.abs(got - ref)) < 1e-14
+
+
+def test_dsap_limits_and_structure(c1):
+    cfg = c1["cfg"]
+    U, clov, x, y = c1["U"], c1["clov"], c1["psi"][0], c1["psi"][1]
+    args = (U, clov, cfg.kappa, cfg.dims, cfg.bc)
+    # one domain = the whole lattice: nothing is switched off
+    assert rel(oracle.wilson_clover_dd_mult(x, *args, cfg.dims), oracle.wilson_clover_mult(x, *args)) < 1e-15
+    # domains of one site: only the site-diagonal part 1 + F survives
+    site_diag = x + np.einsum("schkl,schl->schk", clov.reshape(-1, 2, 6, 6)[:, :, None].repeat(1, 2),
+                              x.reshape(-1, 2, 1, 6)).reshape(x.shape)
+    assert rel(oracle.wilson_clover_dd_mult(x, *args, (1, 1, 1, 1)), site_diag) < 1e-15
+    # block structure: a source inside one domain stays inside it
+    dom, par = domain_index(cfg.dims, cfg.block)
+    src = np.where((dom == 5)[:, None, None], x, 0)
+    out = oracle.wilson_clover_dd_mult(src, *args, cfg.block)
+    assert np.max(np.abs(out[dom != 5])) == 0.0 and np.max(np.abs(out[dom == 5])) > 0.1
+    # even + odd = all; gamma5-hermiticity <x, Dsap^dag y> = <Dsap x, y>
+    full = oracle.wilson_clover_dd_mult(x, *args, cfg.block)
+    e = oracle.wilson_clover_dd_mult(x, *args, cfg.block, parity=1)
+    o = oracle.wilson_clover_dd_mult(x, *args, cfg.block, parity=2)
+    assert np.array_equal(e + o, full)
+    assert np.max(np.abs(e[par == 1])) == 0.0 and np.max(np.abs(o[par == 0])) == 0.0
+    lhs = np.vdot(x, oracle.wilson_clover_dd_mult(y, *args, cfg.block, dagger=True))
+    rhs = np.vdot(oracle.wilson_clover_dd_mult(x, *args, cfg.block), y)
+    assert abs(lhs - rhs) < 1e-12 * abs(rhs)
+    # f32-input and sampled-site variants agree with the full fp64-input call on fp32-representable data
+    x32, U32, c32 = li.round_to_f32(x), li.round_to_f32(U), li.round_to_f32(clov)
+    a = oracle.wilson_clover_dd_mult(x32, U32, c32, cfg.kappa, cfg.dims, cfg.bc, cfg.block, parity=2, dagger=True)
+    b = oracle.wilson_clover_dd_mult(x32.astype(np.complex128), U32.astype(np.complex128), c32.astype(np.complex128),
+                                     cfg.kappa, cfg.dims, cfg.bc, cfg.block, parity=2, dagger=True)
+    assert np.array_equal(a, b)
+    sites = np.array([0, 7, 100, 255])
+    s = oracle.wilson_clover_dd_mult_sites(x32, U32, c32, cfg.kappa, cfg.dims, cfg.bc, cfg.block, sites, parity=2,
+                                           dagger=True)
+    assert np.array_equal(s, a[sites])
