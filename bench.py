@@ -60,6 +60,18 @@ def model(cfg: li.Config, links12: bool = False) -> dict:
     }
 
 
+def model_dsap(cfg: li.Config, parity: int = 0) -> dict:
+    """F1, D_SAP with the aggregation block as domain: links and hops that cross a domain face are never touched."""
+    V = cfg.volume
+    kept = [(b - 1) / b if l // b > 1 else 1.0 for l, b in zip(cfg.dims, cfg.block)]   # per direction
+    link_b = sum(72 * k for k in kept)
+    hop_f = sum(2 * 165 * k for k in kept)
+    active_b, active_f = 96 + 96 + link_b + 288, hop_f + 504 + 48
+    if parity == 0:
+        return {"bytes": active_b * V, "flops": active_f * V, "units": V}
+    return {"bytes": (active_b + 96) * V / 2, "flops": active_f * V / 2, "units": V}   # other group: zeros written
+
+
 STEP_ORDER = ["wilson_clover", "wilson_clover_dagger", "restrict", "coarse_mult", "prolong"]
 KERNEL_SYMBOL = {  # the __global__ each row launches (for the ncu launch list)
     "wilson_clover": "k_wilson_clover", "wilson_clover_dagger": "k_wilson_clover", "restrict": "k_restrict",
@@ -252,6 +264,15 @@ class Workload:
     def wilson_clover_12(self, i):
         c = self.cfg
         self.lq.wilson_clover_mult(self.y[i], self.x[i], self.U12, self.clover, c.kappa, c.dims, c.bc, links12=True)
+
+    def wilson_clover_dd(self, i):
+        c = self.cfg
+        self.lq.wilson_clover_dd_mult(self.y[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block)
+
+    def wilson_clover_dd_even(self, i):
+        c = self.cfg
+        self.lq.wilson_clover_dd_mult(self.y[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block,
+                                      parity=1)
 
     def restrict(self, i):
         c = self.cfg
@@ -484,6 +505,13 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         extra["wilson_clover_links12"] = {"us": t12 * 1e6, "GBps": m12["bytes"] / t12 / 1e9,
                                           "GFLOPs": m12["flops"] / t12 / 1e9, "units_per_s": m12["units"] / t12,
                                           "frac_of_hbm_peak": m12["bytes"] / t12 / 1e9 / peak}
+        # F1 (next row of SURVEY 8(f)): the domain-decomposed operator D_SAP, all domains and the even group
+        for name, par in (("wilson_clover_dd", 0), ("wilson_clover_dd_even", 1)):
+            t = time_single(W, name, reps=max(10, args.steps))
+            md = model_dsap(cfg, par)
+            extra[name] = {"us": t * 1e6, "GBps": md["bytes"] / t / 1e9, "GFLOPs": md["flops"] / t / 1e9,
+                           "units_per_s": md["units"] / t, "frac_of_hbm_peak": md["bytes"] / t / 1e9 / peak,
+                           "bytes_per_launch": md["bytes"]}
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)

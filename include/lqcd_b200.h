@@ -67,6 +67,8 @@ extern "C" {
 /* flags */
 #define LQCD_DAGGER 1u   /* apply gamma5 D gamma5 = D^dag (Eq. 2) / Gamma5c D_c Gamma5c */
 #define LQCD_LINKS_12 2u /* U holds the 12-real compressed native gauge layout */
+#define LQCD_DOMAIN_EVEN 4u /* lqcd_wilson_clover_dd_mult only: compute even domains, zero elsewhere */
+#define LQCD_DOMAIN_ODD 8u  /* lqcd_wilson_clover_dd_mult only: compute odd domains, zero elsewhere */
 
 /* ---- diagnostics ------------------------------------------------------------------------- */
 int lqcd_version(void);
@@ -125,6 +127,20 @@ int lqcd_wilson_clover_mult_f32(float* out, const float* in, const float* U, con
                                 const int dims[4], const int bc[4], unsigned flags, void* stream);
 int lqcd_wilson_clover_mult_f64(double* out, const double* in, const double* U, const double* clover,
                                 double kappa, const int dims[4], const int bc[4], unsigned flags, void* stream);
+
+/* ---- F1: domain-decomposed operator D_SAP: "the Dirac matrix D_SAP [is defined] by turning off
+ * the interaction across the domains" -- Eq. 1 with every hop whose two ends lie in different domains dropped.
+ * domain[4] divides dims (the paper sets the SAP domain equal to the aggregation block); a direction spanned
+ * by a single domain keeps all its hops, including the wrapping one with its boundary phase.
+ * "Splitting the domains into even and odd groups, D_SAP^(e) and D_SAP^(o)": with LQCD_DOMAIN_EVEN (ODD) only
+ * the sites of domains with (X_x+X_y+X_z+X_t) even (odd) are computed, out is set to ZERO on the others
+ * (P_e D_SAP P_e).  Other flags and all argument rules as for lqcd_wilson_clover_mult. */
+int lqcd_wilson_clover_dd_mult_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
+                                   const int dims[4], const int bc[4], const int domain[4], unsigned flags,
+                                   void* stream);
+int lqcd_wilson_clover_dd_mult_f64(double* out, const double* in, const double* U, const double* clover,
+                                   double kappa, const int dims[4], const int bc[4], const int domain[4],
+                                   unsigned flags, void* stream);
 
 /* ---- A3: coarse operator, Eqs. 4, 7 ---------------------------------------
  *   out(X) = A[X][0] in(X) + sum_mu ( A[X][1+2mu] in(X+mu) + A[X][2+2mu] in(X-mu) ),

@@ -18,6 +18,8 @@ from ._lib import c_int4
 
 DAGGER = 1
 LINKS_12 = 2
+DOMAIN_EVEN = 4
+DOMAIN_ODD = 8
 
 OK, EINVAL, EUNSUPPORTED, ECUDA = 0, -1, -2, -3
 
@@ -212,6 +214,18 @@ def wilson_clover_mult(out, inp, U, clover, kappa, dims, bc, dagger=False, links
     _check(getattr(lib(), f"lqcd_wilson_clover_mult_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(U), _dev_ptr(clover),
                                                             k, _i4(dims), _i4(bc), flags, _stream(stream)),
            "lqcd_wilson_clover_mult")
+    return out
+
+
+def wilson_clover_dd_mult(out, inp, U, clover, kappa, dims, bc, domain, parity=0, dagger=False, links12=False,
+                          stream=None):
+    """F1: out = D_SAP in; parity 0 / 1 / 2 = all / even / odd domains (zero elsewhere)."""
+    sfx = _same_dtype(out, inp, U, clover)
+    flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0) | {0: 0, 1: DOMAIN_EVEN, 2: DOMAIN_ODD}[parity]
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_wilson_clover_dd_mult_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(U),
+                                                               _dev_ptr(clover), k, _i4(dims), _i4(bc), _i4(domain),
+                                                               flags, _stream(stream)), "lqcd_wilson_clover_dd_mult")
     return out
 
 

@@ -39,6 +39,7 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_pack_nullvec_{_p}": (_ci, [_vp, _vp, _ci, _i4, _i4, _ci, _vp]),
         f"lqcd_unpack_nullvec_{_p}": (_ci, [_vp, _vp, _ci, _i4, _i4, _ci, _vp]),
         f"lqcd_wilson_clover_mult_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _vp]),
+        f"lqcd_wilson_clover_dd_mult_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _cu, _vp]),
         f"lqcd_coarse_mult_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _vp]),
         f"lqcd_restrict_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp]),
         f"lqcd_prolong_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp]),

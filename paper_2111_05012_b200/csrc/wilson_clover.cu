@@ -24,6 +24,10 @@ struct FineParams {
     int bc[4];     // +1 / -1
     int tilevol;   // threads that own a site (<= blockDim.x)
     int zslab;     // traversal slab extent in z tiles (0 = canonical tile order)
+    // domain-decomposed variant D_SAP; unused by the plain operator
+    int dom[4];    // domain extents (the aggregation block)
+    int multi[4];  // 1 if there is more than one domain in that direction (else no hop is ever cut)
+    int parity;    // 0 = all domains, 1 = even domains only, 2 = odd domains only
 };
 
 template <typename T> struct Cx {
@@ -246,7 +250,10 @@ template <typename T> __device__ __forceinline__ void load_clover_block(T cl[36]
     }
 }
 
-template <typename T, bool DAG, bool L12, int MAXTHREADS, int MINBLOCKS>
+// DD: the domain-decomposed operator D_SAP -- hops whose two ends lie in different domains are switched off
+// (no load is issued for them), and with P.parity != 0 only the sites of even (odd) domains are computed, the
+// others are set to zero (D_SAP^(e/o) = P_e/o D_SAP P_e/o).
+template <typename T, bool DAG, bool L12, bool DD, int MAXTHREADS, int MINBLOCKS>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
     k_wilson_clover(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ U, const T* __restrict__ clover,
                     T kappa, FineParams P) {
@@ -302,16 +309,33 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
 #pragma unroll
     for (int r = 0; r < 24; r++) acc[r] = 0;
 
+    // domain decomposition: which of my eight hops leave my domain, and is my domain in the selected group
+    bool cutf[4] = {false, false, false, false}, cutb[4] = {false, false, false, false};
+    if (DD) {
+        int par = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const int X = x[mu] / P.dom[mu], lx = x[mu] - X * P.dom[mu];
+            par += X;
+            cutf[mu] = P.multi[mu] && lx == P.dom[mu] - 1;
+            cutb[mu] = P.multi[mu] && lx == 0;
+        }
+        if (P.parity != 0 && (par & 1) != P.parity - 1) {
+            store_spinor<T>(out, s, acc);  // zeros
+            return;
+        }
+    }
+
     // D: forward hops carry (1 - g_mu), backward (1 + g_mu); D^dag: the two are swapped.
     constexpr int SF = DAG ? +1 : -1, SB = DAG ? -1 : +1;
-    hop<0, true, SF, L12, T>(acc, in, U, s, sf[0], pf[0]);
-    hop<0, false, SB, L12, T>(acc, in, U, s, sb[0], pb[0]);
-    hop<1, true, SF, L12, T>(acc, in, U, s, sf[1], pf[1]);
-    hop<1, false, SB, L12, T>(acc, in, U, s, sb[1], pb[1]);
-    hop<2, true, SF, L12, T>(acc, in, U, s, sf[2], pf[2]);
-    hop<2, false, SB, L12, T>(acc, in, U, s, sb[2], pb[2]);
-    hop<3, true, SF, L12, T>(acc, in, U, s, sf[3], pf[3]);
-    hop<3, false, SB, L12, T>(acc, in, U, s, sb[3], pb[3]);
+    if (!DD || !cutf[0]) hop<0, true, SF, L12, T>(acc, in, U, s, sf[0], pf[0]);
+    if (!DD || !cutb[0]) hop<0, false, SB, L12, T>(acc, in, U, s, sb[0], pb[0]);
+    if (!DD || !cutf[1]) hop<1, true, SF, L12, T>(acc, in, U, s, sf[1], pf[1]);
+    if (!DD || !cutb[1]) hop<1, false, SB, L12, T>(acc, in, U, s, sb[1], pb[1]);
+    if (!DD || !cutf[2]) hop<2, true, SF, L12, T>(acc, in, U, s, sf[2], pf[2]);
+    if (!DD || !cutb[2]) hop<2, false, SB, L12, T>(acc, in, U, s, sb[2], pb[2]);
+    if (!DD || !cutf[3]) hop<3, true, SF, L12, T>(acc, in, U, s, sf[3], pf[3]);
+    if (!DD || !cutb[3]) hop<3, false, SB, L12, T>(acc, in, U, s, sb[3], pb[3]);
 
     // site-diagonal part: (1 + F) in, then out = that - kappa * hops
     T p[24], o[24];
@@ -346,9 +370,10 @@ static void auto_tile(const int L[4], int tile[4]) {
         }
 }
 
+// domain == NULL: the plain operator D; otherwise D_SAP with those domains
 template <typename T>
 static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4],
-                              const int bc[4], unsigned flags, void* stream, const char* what) {
+                              const int bc[4], const int* domain, unsigned flags, void* stream, const char* what) {
     clear_error();
     if (!out || !in || !U || !clover || check_dims(dims) || !bc) {
         set_error("%s: null pointer or non-positive dim", what);
@@ -362,8 +387,9 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
         set_error("%s: out must not alias in", what);
         return LQCD_EINVAL;
     }
-    if (flags & ~(LQCD_DAGGER | LQCD_LINKS_12)) {
-        set_error("%s: unknown flag bits 0x%x", what, flags);
+    const unsigned allowed = LQCD_DAGGER | LQCD_LINKS_12 | (domain ? (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD) : 0u);
+    if ((flags & ~allowed) || ((flags & LQCD_DOMAIN_EVEN) && (flags & LQCD_DOMAIN_ODD))) {
+        set_error("%s: unknown or contradictory flag bits 0x%x", what, flags);
         return LQCD_EINVAL;
     }
     if (volume(dims) > 0x7fffffffLL) {
@@ -378,7 +404,18 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
         }
         P.L[mu] = dims[mu];
         P.bc[mu] = bc[mu];
+        P.dom[mu] = dims[mu];
+        P.multi[mu] = 0;
+        if (domain) {
+            if (domain[mu] < 1 || dims[mu] % domain[mu]) {
+                set_error("%s: domain[%d] = %d does not divide dims[%d] = %d", what, mu, domain[mu], mu, dims[mu]);
+                return LQCD_EINVAL;
+            }
+            P.dom[mu] = domain[mu];
+            P.multi[mu] = dims[mu] / domain[mu] > 1;
+        }
     }
+    P.parity = (flags & LQCD_DOMAIN_EVEN) ? 1 : (flags & LQCD_DOMAIN_ODD) ? 2 : 0;
     bool user_ok = g_knobs.fine_tile[0] > 0;
     for (int mu = 0; mu < 4 && user_ok; mu++) user_ok = dims[mu] % g_knobs.fine_tile[mu] == 0;
     if (user_ok)
@@ -416,27 +453,26 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
     const bool dag = flags & LQCD_DAGGER, l12 = flags & LQCD_LINKS_12;
     cudaStream_t st = (cudaStream_t)stream;
     const unsigned grid = (unsigned)ntiles;
-#define LAUNCH(DAG, L12)                                                                                  \
-    do {                                                                                                  \
-        /* registers per thread: fp32 128 (4 CTAs/SM), fp64 168 (3 CTAs/SM) measured best on B200;      */ \
-        /* fine_variant 1 / 2 select fewer / more resident CTAs for experiments                          */ \
-        if (threads <= 128 && g_knobs.fine_variant == 1)                                                  \
-            k_wilson_clover<T, DAG, L12, 128, (sizeof(T) == 4 ? 3 : 2)>                                   \
-                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
-        else if (threads <= 128 && g_knobs.fine_variant == 2)                                             \
-            k_wilson_clover<T, DAG, L12, 128, (sizeof(T) == 4 ? 5 : 4)>                                   \
-                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
-        else if (threads <= 128)                                                                          \
-            k_wilson_clover<T, DAG, L12, 128, (sizeof(T) == 4 ? 4 : 3)>                                   \
-                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
-        else                                                                                           \
-            k_wilson_clover<T, DAG, L12, 256, (sizeof(T) == 4 ? 2 : 1)>                                   \
-                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                 \
+    // registers per thread: fp32 128 (4 CTAs/SM), fp64 168 (3 CTAs/SM) -- measured best on B200
+#define LAUNCH(DAG, L12, DD)                                                                                 \
+    do {                                                                                                     \
+        if (threads <= 128)                                                                                  \
+            k_wilson_clover<T, DAG, L12, DD, 128, (sizeof(T) == 4 ? 4 : 3)>                                  \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                    \
+        else                                                                                                 \
+            k_wilson_clover<T, DAG, L12, DD, 256, (sizeof(T) == 4 ? 2 : 1)>                                  \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                    \
     } while (0)
-    if (dag && l12) LAUNCH(true, true);
-    else if (dag) LAUNCH(true, false);
-    else if (l12) LAUNCH(false, true);
-    else LAUNCH(false, false);
+#define LAUNCH_DD(DAG, L12)                                                                                  \
+    do {                                                                                                     \
+        if (domain) LAUNCH(DAG, L12, true);                                                                  \
+        else LAUNCH(DAG, L12, false);                                                                        \
+    } while (0)
+    if (dag && l12) LAUNCH_DD(true, true);
+    else if (dag) LAUNCH_DD(true, false);
+    else if (l12) LAUNCH_DD(false, true);
+    else LAUNCH_DD(false, false);
+#undef LAUNCH_DD
 #undef LAUNCH
     count_launch();
     return check_launch(what);
@@ -449,10 +485,32 @@ using namespace lqcd;
 extern "C" {
 int lqcd_wilson_clover_mult_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
                                 const int dims[4], const int bc[4], unsigned flags, void* stream) {
-    return wilson_clover_call<float>(out, in, U, clover, kappa, dims, bc, flags, stream, "lqcd_wilson_clover_mult_f32");
+    return wilson_clover_call<float>(out, in, U, clover, kappa, dims, bc, nullptr, flags, stream,
+                                     "lqcd_wilson_clover_mult_f32");
 }
 int lqcd_wilson_clover_mult_f64(double* out, const double* in, const double* U, const double* clover, double kappa,
                                 const int dims[4], const int bc[4], unsigned flags, void* stream) {
-    return wilson_clover_call<double>(out, in, U, clover, kappa, dims, bc, flags, stream, "lqcd_wilson_clover_mult_f64");
+    return wilson_clover_call<double>(out, in, U, clover, kappa, dims, bc, nullptr, flags, stream,
+                                      "lqcd_wilson_clover_mult_f64");
+}
+int lqcd_wilson_clover_dd_mult_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
+                                   const int dims[4], const int bc[4], const int domain[4], unsigned flags,
+                                   void* stream) {
+    if (!domain) {
+        set_error("lqcd_wilson_clover_dd_mult_f32: null domain");
+        return LQCD_EINVAL;
+    }
+    return wilson_clover_call<float>(out, in, U, clover, kappa, dims, bc, domain, flags, stream,
+                                     "lqcd_wilson_clover_dd_mult_f32");
+}
+int lqcd_wilson_clover_dd_mult_f64(double* out, const double* in, const double* U, const double* clover, double kappa,
+                                   const int dims[4], const int bc[4], const int domain[4], unsigned flags,
+                                   void* stream) {
+    if (!domain) {
+        set_error("lqcd_wilson_clover_dd_mult_f64: null domain");
+        return LQCD_EINVAL;
+    }
+    return wilson_clover_call<double>(out, in, U, clover, kappa, dims, bc, domain, flags, stream,
+                                      "lqcd_wilson_clover_dd_mult_f64");
 }
 }

@@ -98,6 +98,14 @@ def test_fullsize_wilson_clover_sampled(lq, name):
             ref.reshape(len(sites), -1), axis=1)
         assert per_site.max() <= 5 * TOL32, (label, int(sites[per_site.argmax()]))
         results[label] = yc
+    # F1: D_SAP with the aggregation block as domain, all domains and the even group
+    for parity, dag in ((0, False), (1, True), (2, False)):
+        lq.wilson_clover_dd_mult(y, x, U18, Cn, cfg.kappa, L, cfg.bc, cfg.block, parity=parity, dagger=dag)
+        got = lq.unpack_spinor(y, L)[sites_d].cpu().numpy()
+        ref = oracle.wilson_clover_dd_mult_sites(psi_h, U_h, cl_h, cfg.kappa, L, cfg.bc, cfg.block, sites,
+                                                 parity=parity, dagger=dag)
+        assert rel_l2(got, ref) <= TOL32, ("D_SAP", parity)
+        assert np.array_equal(got == 0, ref == 0)
     # property at full size: gamma5-hermiticity <chi, D psi> = <D^dag chi, psi> (Eq. 2), fp64 sums
     lq.wilson_clover_mult(y, w, U18, Cn, cfg.kappa, L, cfg.bc, dagger=True)
     ddag_chi = lq.unpack_spinor(y, L)

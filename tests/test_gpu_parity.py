@@ -55,6 +55,15 @@ class Dev:
                               links12=self.links12)
         return lq.unpack_spinor(y, cfg.dims).cpu().numpy()
 
+    def Dsap(self, psi, domain, parity=0, dagger=False):
+        lq, cfg = self.lq, self.cfg
+        x = lq.pack_spinor(to_dev(psi, self.prec), cfg.dims)
+        y = lq.empty_spinor(cfg.dims, dtype=x.dtype)
+        y.fill_(7.0)  # the kernel must overwrite every site, also the zeroed ones of the other domain group
+        lq.wilson_clover_dd_mult(y, x, self.U, self.clover, cfg.kappa, cfg.dims, cfg.bc, domain, parity=parity,
+                                 dagger=dagger, links12=self.links12)
+        return lq.unpack_spinor(y, cfg.dims).cpu().numpy()
+
     def Dc(self, xc, dagger=False):
         import torch
         x = to_dev(xc, self.prec)
@@ -141,6 +150,50 @@ def test_c1_restrict_prolong(lq, prec):
     got = d.P(prob.xc)
     ref = oracle.prolong(rounded(prob.xc, prec), rounded(prob.v, prec), cfg.dims, cfg.block)
     assert rel_l2(got, ref) <= TOL[prec]
+
+
+# ------------------------------------------------------------------------------------------------------
+# F1: domain-decomposed operator D_SAP, all / even / odd domain groups
+# ------------------------------------------------------------------------------------------------------
+def oracle_Dsap(prob, psi, prec, domain, parity=0, dagger=False):
+    cfg = prob.cfg
+    return oracle.wilson_clover_dd_mult(rounded(psi, prec), rounded(prob.U, prec), rounded(prob.clover, prec),
+                                        cfg.kappa, cfg.dims, cfg.bc, domain, parity=parity, dagger=dagger)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("links12", [False, True])
+def test_c1_dsap(lq, prec, links12):
+    prob = config_problem("c1")
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec, links12=links12, coarse=False)
+    psi = prob.psi[0]
+    for parity in (0, 1, 2):
+        for dagger in (False, True):
+            got = d.Dsap(psi, cfg.block, parity=parity, dagger=dagger)
+            ref = oracle_Dsap(prob, psi, prec, cfg.block, parity=parity, dagger=dagger)
+            assert rel_l2(got, ref) <= TOL[prec], (parity, dagger)
+            assert np.array_equal(got == 0, ref == 0), "exact zeros on the domains of the other group"
+    # one domain spanning the lattice: D_SAP is D, bit for bit
+    assert np.array_equal(d.Dsap(psi, cfg.dims), d.D(psi))
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,domain,bc", [
+    ((8, 8, 8, 8), (4, 4, 4, 4), (1, 1, 1, -1)),       # config 2's lattice and domains
+    ((16, 8, 8, 8), (8, 4, 4, 4), (1, 1, 1, -1)),      # the paper's 8x4x4x4 domain
+    ((6, 4, 2, 10), (3, 4, 1, 5), (-1, 1, -1, 1)),     # odd domains, single domain in y, one-site domains in z
+    ((3, 3, 3, 3), (3, 1, 3, 1), (1, 1, 1, -1)),       # V = 81: ragged chunk
+])
+def test_dsap_edge_lattices(lq, prec, dims, domain, bc):
+    cfg = custom_config(dims, (1, 1, 1, 1), 1, bc=bc)
+    prob = make_problem(cfg, coarse="none")
+    d = Dev(lq, prob, prec, coarse=False)
+    for parity, dagger in ((0, False), (1, True), (2, False)):
+        got = d.Dsap(prob.psi[0], domain, parity=parity, dagger=dagger)
+        ref = oracle_Dsap(prob, prob.psi[0], prec, domain, parity=parity, dagger=dagger)
+        assert rel_l2(got, ref) <= TOL[prec], (parity, dagger)
+        assert np.array_equal(got == 0, ref == 0)
 
 
 # ------------------------------------------------------------------------------------------------------
@@ -293,6 +346,16 @@ def test_error_codes(lq):
     assert code(lambda: lq.restrict(yc, x, d.v, cfg.dims, (4, 4, 4, 4), cfg.nvec)) == lq.EINVAL  # coarse extent 1
     assert code(lambda: lq.prolong(y, yc, d.v, cfg.dims, cfg.block, 0)) == lq.EINVAL
     assert "lqcd_prolong_f32" in lq.last_error()
+    dd = lambda **kw: lq.wilson_clover_dd_mult(y, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, **kw)
+    assert code(lambda: dd(domain=(3, 2, 2, 2))) == lq.EINVAL          # does not divide
+    assert code(lambda: dd(domain=(2, 2, 2, 0))) == lq.EINVAL
+    rc = lq.lib().lqcd_wilson_clover_dd_mult_f32(y.data_ptr(), x.data_ptr(), d.U.data_ptr(), d.clover.data_ptr(),
+                                                 cfg.kappa, lq._i4(cfg.dims), lq._i4(cfg.bc), lq._i4(cfg.block),
+                                                 lq.DOMAIN_EVEN | lq.DOMAIN_ODD, None)
+    assert rc == lq.EINVAL, "even and odd at once"
+    rc = lq.lib().lqcd_wilson_clover_mult_f32(y.data_ptr(), x.data_ptr(), d.U.data_ptr(), d.clover.data_ptr(),
+                                              cfg.kappa, lq._i4(cfg.dims), lq._i4(cfg.bc), lq.DOMAIN_EVEN, None)
+    assert rc == lq.EINVAL, "domain flags are not accepted by the plain operator"
     assert lq.launch_count() == n0, "an erroring call must not enqueue anything"
     with pytest.raises(ValueError):
         lq.wilson_clover_mult(y.cpu(), x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc)  # no CPU path
