@@ -35,12 +35,14 @@ template <typename T> struct Cx {
 };
 
 // ---- loads --------------------------------------------------------------------------------------------
-template <typename T> __device__ __forceinline__ void load_spinor(T p[24], const T* __restrict__ f, int s) {
+// G64: 64-byte L2 fetch granularity (even/odd-domain mode, see common.cuh)
+template <typename T, bool G64 = false>
+__device__ __forceinline__ void load_spinor(T p[24], const T* __restrict__ f, int s) {
     constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
     const T* base = f + ((long long)(s >> 5) * NJ * CH + (s & 31)) * NV;
 #pragma unroll
     for (int j = 0; j < NJ; j++) {
-        V16<T> v = ld16(base + (long long)j * CH * NV);
+        V16<T> v = G64 ? ld16_g64(base + (long long)j * CH * NV) : ld16(base + (long long)j * CH * NV);
 #pragma unroll
         for (int q = 0; q < NV; q++) p[j * NV + q] = v.r[q];
     }
@@ -59,7 +61,7 @@ template <typename T> __device__ __forceinline__ void store_spinor(T* __restrict
 }
 
 // link U_mu(s) as 18 reals u[2*(3a+b)+reim]; with L12 the third row is conj(row0 x row1)
-template <typename T, bool L12>
+template <typename T, bool L12, bool G64 = false>
 __device__ __forceinline__ void load_link(T u[18], const T* __restrict__ U, int s, int mu) {
     constexpr int NV = VecOf<T>::NV;
     const long long chunk = s >> 5;
@@ -68,7 +70,7 @@ __device__ __forceinline__ void load_link(T u[18], const T* __restrict__ U, int 
         const T* base = U + (chunk * 4 + mu) * (12LL * CH) + lane * NV;
 #pragma unroll
         for (int j = 0; j < 12 / NV; j++) {
-            V16<T> v = ld16(base + j * CH * NV);
+            V16<T> v = G64 ? ld16_g64(base + j * CH * NV) : ld16(base + j * CH * NV);
 #pragma unroll
             for (int q = 0; q < NV; q++) u[j * NV + q] = v.r[q];
         }
@@ -88,7 +90,7 @@ __device__ __forceinline__ void load_link(T u[18], const T* __restrict__ U, int 
         const T* base = U + (chunk * 4 + mu) * (18LL * CH);
 #pragma unroll
         for (int j = 0; j < NFULL; j++) {
-            V16<T> v = ld16(base + (j * CH + lane) * NV);
+            V16<T> v = G64 ? ld16_g64(base + (j * CH + lane) * NV) : ld16(base + (j * CH + lane) * NV);
 #pragma unroll
             for (int q = 0; q < NV; q++) u[j * NV + q] = v.r[q];
         }
@@ -199,12 +201,12 @@ template <bool FWD, typename T> __device__ __forceinline__ void su3_mult(T g[12]
 }
 
 // one directed hop: FWD: (1 + SGN g_mu) U_mu(x) in(x+mu);  !FWD: (1 + SGN g_mu) U_mu^dag(x-mu) in(x-mu)
-template <int MU, bool FWD, int SGN, bool L12, typename T>
-__device__ __forceinline__ void hop(T acc[24], const T* __restrict__ in, const T* __restrict__ U, int s_self, int s_nb,
+template <int MU, bool FWD, int SGN, bool L12, bool G64, typename T>
+__device__ __forceinline__ void hop(T acc[24], const T* __restrict__ in, const T* __restrict__ U, int s_link, int s_nb,
                                     T ph) {
     T p[24], h[12], u[18], g[12];
-    load_spinor<T>(p, in, s_nb);
-    load_link<T, L12>(u, U, FWD ? s_self : s_nb, MU);
+    load_spinor<T, G64>(p, in, s_nb);
+    load_link<T, L12, G64>(u, U, s_link, MU);
     project<MU, SGN, T>(h, p);
     su3_mult<FWD, T>(g, u, h);
     reconstruct<MU, SGN, T>(acc, g, ph);
@@ -239,12 +241,13 @@ template <typename T> __device__ __forceinline__ void herm6_madd(T out[12], cons
     }
 }
 
-template <typename T> __device__ __forceinline__ void load_clover_block(T cl[36], const T* __restrict__ C, int s, int chi) {
+template <typename T, bool G64 = false>
+__device__ __forceinline__ void load_clover_block(T cl[36], const T* __restrict__ C, int s, int chi) {
     constexpr int NV = VecOf<T>::NV, NJ = 72 / NV;
     const T* base = C + (((long long)(s >> 5) * NJ + chi * (36 / NV)) * CH + (s & 31)) * NV;
 #pragma unroll
     for (int j = 0; j < 36 / NV; j++) {
-        V16<T> v = ld16_stream(base + (long long)j * CH * NV);
+        V16<T> v = G64 ? ld16_stream_g64(base + (long long)j * CH * NV) : ld16_stream(base + (long long)j * CH * NV);
 #pragma unroll
         for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
     }
@@ -253,7 +256,8 @@ template <typename T> __device__ __forceinline__ void load_clover_block(T cl[36]
 // DD: the domain-decomposed operator D_SAP -- hops whose two ends lie in different domains are switched off
 // (no load is issued for them), and with P.parity != 0 only the sites of even (odd) domains are computed, the
 // others are set to zero (D_SAP^(e/o) = P_e/o D_SAP P_e/o).
-template <typename T, bool DAG, bool L12, bool DD, int MAXTHREADS, int MINBLOCKS>
+// DD = 2: the even/odd mode; active data then comes in alternate 64-byte half lines -> 64-byte L2 granularity.
+template <typename T, bool DAG, bool L12, int DD, int MAXTHREADS, int MINBLOCKS>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
     k_wilson_clover(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ U, const T* __restrict__ clover,
                     T kappa, FineParams P) {
@@ -309,43 +313,57 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
 #pragma unroll
     for (int r = 0; r < 24; r++) acc[r] = 0;
 
-    // domain decomposition: which of my eight hops leave my domain, and is my domain in the selected group
-    bool cutf[4] = {false, false, false, false}, cutb[4] = {false, false, false, false};
+    // link sites: U_mu(x) for the forward hop, U_mu(x - mu) for the backward hop
+    int lf[4] = {s, s, s, s}, lb[4] = {sb[0], sb[1], sb[2], sb[3]};
+    // Domain decomposition: a hop that leaves my domain is switched off.  Control flow stays uniform (the eight
+    // hops are one straight-line, software-pipelined instruction stream, as in D): a cut hop gets phase 0 and is
+    // redirected to operands this thread needs anyway -- its own spinor and the link of the opposite hop of the
+    // same direction -- so it costs L1 hits and idle flops but no DRAM traffic (the links and neighbour spinors
+    // across a domain face are never touched).
     if (DD) {
         int par = 0;
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) {
             const int X = x[mu] / P.dom[mu], lx = x[mu] - X * P.dom[mu];
             par += X;
-            cutf[mu] = P.multi[mu] && lx == P.dom[mu] - 1;
-            cutb[mu] = P.multi[mu] && lx == 0;
+            if (P.multi[mu] && lx == P.dom[mu] - 1) {  // forward hop leaves the domain
+                sf[mu] = s;
+                lf[mu] = sb[mu];
+                pf[mu] = 0;
+            }
+            if (P.multi[mu] && lx == 0) {  // backward hop leaves the domain
+                lb[mu] = s;
+                sb[mu] = s;
+                pb[mu] = 0;
+            }
         }
-        if (P.parity != 0 && (par & 1) != P.parity - 1) {
-            store_spinor<T>(out, s, acc);  // zeros
+        if (P.parity != 0 && (par & 1) != P.parity - 1) {  // my domain is not in the selected group: zero
+            store_spinor<T>(out, s, acc);
             return;
         }
     }
 
     // D: forward hops carry (1 - g_mu), backward (1 + g_mu); D^dag: the two are swapped.
     constexpr int SF = DAG ? +1 : -1, SB = DAG ? -1 : +1;
-    if (!DD || !cutf[0]) hop<0, true, SF, L12, T>(acc, in, U, s, sf[0], pf[0]);
-    if (!DD || !cutb[0]) hop<0, false, SB, L12, T>(acc, in, U, s, sb[0], pb[0]);
-    if (!DD || !cutf[1]) hop<1, true, SF, L12, T>(acc, in, U, s, sf[1], pf[1]);
-    if (!DD || !cutb[1]) hop<1, false, SB, L12, T>(acc, in, U, s, sb[1], pb[1]);
-    if (!DD || !cutf[2]) hop<2, true, SF, L12, T>(acc, in, U, s, sf[2], pf[2]);
-    if (!DD || !cutb[2]) hop<2, false, SB, L12, T>(acc, in, U, s, sb[2], pb[2]);
-    if (!DD || !cutf[3]) hop<3, true, SF, L12, T>(acc, in, U, s, sf[3], pf[3]);
-    if (!DD || !cutb[3]) hop<3, false, SB, L12, T>(acc, in, U, s, sb[3], pb[3]);
+    constexpr bool G64 = (DD == 2);
+    hop<0, true, SF, L12, G64, T>(acc, in, U, lf[0], sf[0], pf[0]);
+    hop<0, false, SB, L12, G64, T>(acc, in, U, lb[0], sb[0], pb[0]);
+    hop<1, true, SF, L12, G64, T>(acc, in, U, lf[1], sf[1], pf[1]);
+    hop<1, false, SB, L12, G64, T>(acc, in, U, lb[1], sb[1], pb[1]);
+    hop<2, true, SF, L12, G64, T>(acc, in, U, lf[2], sf[2], pf[2]);
+    hop<2, false, SB, L12, G64, T>(acc, in, U, lb[2], sb[2], pb[2]);
+    hop<3, true, SF, L12, G64, T>(acc, in, U, lf[3], sf[3], pf[3]);
+    hop<3, false, SB, L12, G64, T>(acc, in, U, lb[3], sb[3], pb[3]);
 
     // site-diagonal part: (1 + F) in, then out = that - kappa * hops
     T p[24], o[24];
-    load_spinor<T>(p, in, s);
+    load_spinor<T, (DD == 2)>(p, in, s);
 #pragma unroll
     for (int r = 0; r < 24; r++) o[r] = fma(-kappa, acc[r], p[r]);
 #pragma unroll
     for (int chi = 0; chi < 2; chi++) {
         T cl[36];
-        load_clover_block<T>(cl, clover, s, chi);
+        load_clover_block<T, (DD == 2)>(cl, clover, s, chi);
         herm6_madd<T>(o + 12 * chi, cl, p + 12 * chi);
     }
     store_spinor<T>(out, s, o);
@@ -420,6 +438,8 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
     for (int mu = 0; mu < 4 && user_ok; mu++) user_ok = dims[mu] % g_knobs.fine_tile[mu] == 0;
     if (user_ok)
         for (int mu = 0; mu < 4; mu++) P.tile[mu] = g_knobs.fine_tile[mu];
+    else if (P.parity != 0)
+        auto_tile(P.dom, P.tile);  // tiles inside one domain: a whole CTA is either computed or zero-filled
     else
         auto_tile(dims, P.tile);
     P.tilevol = 1;
@@ -465,8 +485,9 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
     } while (0)
 #define LAUNCH_DD(DAG, L12)                                                                                  \
     do {                                                                                                     \
-        if (domain) LAUNCH(DAG, L12, true);                                                                  \
-        else LAUNCH(DAG, L12, false);                                                                        \
+        if (domain && P.parity != 0) LAUNCH(DAG, L12, 2);                                                    \
+        else if (domain) LAUNCH(DAG, L12, 1);                                                                \
+        else LAUNCH(DAG, L12, 0);                                                                            \
     } while (0)
     if (dag && l12) LAUNCH_DD(true, true);
     else if (dag) LAUNCH_DD(true, false);
