@@ -221,7 +221,7 @@ class Workload:
 
     NBUF = 4  # distinct input/output buffer sets rotated across steps (and every buffer is >> L2 at c4/c5)
 
-    def __init__(self, cfg: li.Config, device, seed: int):
+    def __init__(self, cfg: li.Config, device, seed: int, synthetic_operators: bool = False):
         import torch
         import paper_2111_05012_b200 as lq
         self.cfg, self.lq, self.dev = cfg, lq, device
@@ -233,16 +233,28 @@ class Workload:
         self.U18 = lq.pack_gauge(U, cfg.dims)
         self.U12 = lq.pack_gauge(U, cfg.dims, links12=True)
         del U
-        cl = li.t_clover_synthetic(gen, V, device)
-        self.clover = lq.pack_clover(cl, cfg.dims)
-        del cl
+        self.setup_ms = {}
+
+        def timed(name, fn):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            r = fn()
+            torch.cuda.synchronize()
+            self.setup_ms[name] = (time.perf_counter() - t0) * 1e3
+            return r
+
+        if synthetic_operators:
+            cl = li.t_clover_synthetic(gen, V, device)
+            self.clover = lq.pack_clover(cl, cfg.dims)
+            del cl
+        else:  # the true clover term of these links, built by the device set-up kernel (F2)
+            self.clover = timed("clover_from_links", lambda: lq.clover_from_links(self.U18, cfg.kappa, cfg.csw, cfg.dims))
         self.x = [lq.pack_spinor(li.t_spinor(gen, V, device, torch.float32), cfg.dims) for _ in range(self.NBUF)]
         self.y = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
         self.yd = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
         self.z = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
         self.xc = [torch.empty((Vc, 2, nv), dtype=torch.complex64, device=device) for _ in range(self.NBUF)]
         self.yc = [torch.empty((Vc, 2, nv), dtype=torch.complex64, device=device) for _ in range(self.NBUF)]
-        self.A = li.t_coarse_matrix_synthetic(gen, Vc, nv, device)
         # null vectors: Gaussian, one canonical vector at a time into its native slot (never twice in HBM)
         self.v = torch.empty(lq.native_nullvecs_reals(cfg.dims, cfg.block, nv), dtype=torch.float32, device=device)
         scale = 1.0 / np.sqrt(2.0 * 6 * (V // Vc))  # unit-norm aggregates on average, like orthonormal ones
@@ -250,6 +262,12 @@ class Workload:
             vi = li.t_spinor(gen, V, device, torch.float32) * scale
             lq.pack_nullvec(self.v, vi, i, cfg.dims, cfg.block, nv)
             del vi
+        if synthetic_operators:
+            self.A = li.t_coarse_matrix_synthetic(gen, Vc, nv, device)
+        else:  # block-orthonormal null vectors and the true Galerkin coarse operator P^dag D P (F2)
+            timed("orthonormalize_blocks", lambda: lq.orthonormalize_blocks(self.v, cfg.dims, cfg.block, nv))
+            self.A = timed("galerkin_coarse", lambda: lq.galerkin_coarse(self.U18, self.clover, self.v, cfg.kappa,
+                                                                          cfg.dims, cfg.bc, cfg.block, nv))
         torch.cuda.synchronize()
 
     # one launch per row; `i` picks the buffer set
@@ -469,7 +487,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     torch.cuda.set_device(dev_index)
     device = torch.device("cuda", dev_index)
     import paper_2111_05012_b200 as lq
-    W = Workload(cfg, device, seed=cfg.seed + 17 * ranks.rank)
+    W = Workload(cfg, device, seed=cfg.seed + 17 * ranks.rank, synthetic_operators=args.synthetic_operators)
     m = model(cfg)
     peak, peak_src = measured_peak()
 
@@ -527,7 +545,8 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         "gflops": whole_job_value(sflops, ranks.world, sec_per_step) / 1e9,
         "fine_sites_per_s": whole_job_value(2 * cfg.volume, ranks.world, sec_per_step),
         "frac_of_hbm_peak": value / ranks.world / peak,
-        "kernels": kernels, "extra": extra, "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches),
+        "kernels": kernels, "extra": extra, "setup_ms": W.setup_ms,
+        "operators": "synthetic" if args.synthetic_operators else "device-built (clover from links, Galerkin P^dag D P)", "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches),
         "clocks": clocks,
     }
     if ranks.rank == 0 and ranks.world == 1 and not args.no_cpu_baseline:
@@ -607,6 +626,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--synthetic-operators", action="store_true",
+                    help="random clover term and coarse matrix instead of the device-built ones (DESIGN.md section 4)")
     ap.add_argument("--sweep", action="store_true", help="config 5's bandwidth-roofline sweep over volumes (1 GPU)")
     args = ap.parse_args()
     cfg = li.CONFIGS[args.workload]

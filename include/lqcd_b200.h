@@ -105,6 +105,8 @@ int lqcd_pack_gauge_f64(double* dst_native, const double* src_canonical, const i
                         void* stream);
 int lqcd_pack_clover_f32(float* dst_native, const float* src_canonical, const int dims[4], void* stream);
 int lqcd_pack_clover_f64(double* dst_native, const double* src_canonical, const int dims[4], void* stream);
+int lqcd_unpack_clover_f32(float* dst_canonical, const float* src_native, const int dims[4], void* stream);
+int lqcd_unpack_clover_f64(double* dst_canonical, const double* src_native, const int dims[4], void* stream);
 /* Packs ONE canonical null vector v_i[s][alpha][c] into slot i of the native array (so that a
  * 32-vector set never has to exist twice in HBM). */
 int lqcd_pack_nullvec_f32(float* dst_native, const float* src_canonical_vi, int i, const int dims[4],
@@ -162,6 +164,35 @@ int lqcd_prolong_f32(float* out_f, const float* in_c, const float* nullvecs, con
                      const int block[4], int nvec, void* stream);
 int lqcd_prolong_f64(double* out_f, const double* in_c, const double* nullvecs, const int dims[4],
                      const int block[4], int nvec, void* stream);
+
+/* ---- F2: set-up of the operator fields on the device (not on the timed path) ------------------------------
+ * Clover term from the links (formula: DESIGN.md reading Q1):
+ *   F(x) = kappa csw sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}(x), sigma_{mu nu} = [g_mu, g_nu]/(2i),
+ *   F_{mu nu} = (Q - Q^dag)/(8i), Q = the four plaquette leaves in the mu-nu plane (links periodic).
+ * U: native 18-real gauge; clover: native clover (output). */
+int lqcd_clover_from_links_f32(float* clover_native, const float* U_native18, float kappa, float csw,
+                               const int dims[4], void* stream);
+int lqcd_clover_from_links_f64(double* clover_native, const double* U_native18, double kappa, double csw,
+                               const int dims[4], void* stream);
+
+/* Block orthonormalisation of the null vectors, in place on the NATIVE null-vector array: within
+ * every aggregate (X, chi) the nvec vectors are orthonormalised in index order (Gram-Schmidt, each vector projected
+ * twice against its predecessors; the result is the unique Q of the QR factorisation with positive diagonal).
+ * Requires |block| * 6 >= nvec; linearly dependent input yields non-finite output. */
+int lqcd_orthonormalize_blocks_f32(float* nullvecs, const int dims[4], const int block[4], int nvec, void* stream);
+int lqcd_orthonormalize_blocks_f64(double* nullvecs, const int dims[4], const int block[4], int nvec, void* stream);
+/* Galerkin coarse operator, Eq. 7: A[X][d][I][J] = <I| D_d |J> for the nine pieces of D (d = 0: the
+ * site-diagonal term and the hops inside the aggregate; 1 + 2 mu / 2 + 2 mu: the forward / backward hops that leave
+ * it), coarse-matrix layout as consumed by lqcd_coarse_mult.  U: native 18-real gauge; nullvecs: native, block-
+ * orthonormal.  ws_dev: device scratch of lqcd_galerkin_workspace_bytes(dims, block, nvec, sizeof(real)) bytes.
+ * Built column by column from the hot-path kernels: 2 nvec * 28 launches. */
+size_t lqcd_galerkin_workspace_bytes(const int dims[4], const int block[4], int nvec, int real_bytes);
+int lqcd_galerkin_coarse_f32(float* A, const float* U, const float* clover, const float* nullvecs, float kappa,
+                             const int dims[4], const int bc[4], const int block[4], int nvec, void* ws_dev,
+                             void* stream);
+int lqcd_galerkin_coarse_f64(double* A, const double* U, const double* clover, const double* nullvecs, double kappa,
+                             const int dims[4], const int bc[4], const int block[4], int nvec, void* ws_dev,
+                             void* stream);
 
 /* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the

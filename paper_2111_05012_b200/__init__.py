@@ -178,6 +178,53 @@ def pack_clover(src: torch.Tensor, dims, stream=None) -> torch.Tensor:
     return dst
 
 
+def unpack_clover(src: torch.Tensor, dims, stream=None) -> torch.Tensor:
+    """native -> canonical complex tensor of shape (V, 2, 6, 6) (full Hermitian blocks)"""
+    sfx = _sfx(src)
+    v = 1
+    for d in dims:
+        v *= int(d)
+    dst = torch.empty((v, 2, 6, 6, 2), dtype=_rdtype(sfx), device=src.device)
+    _check(getattr(lib(), f"lqcd_unpack_clover_{sfx}")(_dev_ptr(dst), _dev_ptr(src), _i4(dims), _stream(stream)),
+           "lqcd_unpack_clover")
+    return torch.view_as_complex(dst)
+
+
+def clover_from_links(U_native18: torch.Tensor, kappa, csw, dims, stream=None) -> torch.Tensor:
+    """F2: the native clover field built on the device from the native 18-real links (Q1)."""
+    sfx = _sfx(U_native18)
+    dst = torch.zeros(native_clover_reals(dims), dtype=_rdtype(sfx), device=U_native18.device)
+    k = (C.c_float if sfx == "f32" else C.c_double)
+    _check(getattr(lib(), f"lqcd_clover_from_links_{sfx}")(_dev_ptr(dst), _dev_ptr(U_native18), k(kappa), k(csw),
+                                                           _i4(dims), _stream(stream)), "lqcd_clover_from_links")
+    return dst
+
+
+def orthonormalize_blocks(nullvecs_native: torch.Tensor, dims, block, nvec, stream=None) -> torch.Tensor:
+    """F2: in-place block/chirality-wise orthonormalisation of the native null vectors."""
+    sfx = _sfx(nullvecs_native)
+    _check(getattr(lib(), f"lqcd_orthonormalize_blocks_{sfx}")(_dev_ptr(nullvecs_native), _i4(dims), _i4(block),
+                                                               int(nvec), _stream(stream)), "lqcd_orthonormalize_blocks")
+    return nullvecs_native
+
+
+def galerkin_coarse(U_native18, clover, nullvecs, kappa, dims, bc, block, nvec, stream=None) -> torch.Tensor:
+    """F2: the coarse matrix A[X][d][I][J] = <I|D_d|J> (Eq. 7) as a complex (Vc, 9, N, N) tensor."""
+    sfx = _same_dtype(U_native18, clover, nullvecs)
+    rdt = _rdtype(sfx)
+    cd = [int(l) // int(b) for l, b in zip(dims, block)]
+    vc, n = cd[0] * cd[1] * cd[2] * cd[3], 2 * int(nvec)
+    A = torch.zeros((vc, 9, n, n, 2), dtype=rdt, device=nullvecs.device)
+    nbytes = int(lib().lqcd_galerkin_workspace_bytes(_i4(dims), _i4(block), int(nvec), 4 if sfx == "f32" else 8))
+    ws = torch.empty(max(nbytes, 16), dtype=torch.uint8, device=nullvecs.device)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_galerkin_coarse_{sfx}")(_dev_ptr(A), _dev_ptr(U_native18), _dev_ptr(clover),
+                                                         _dev_ptr(nullvecs), k, _i4(dims), _i4(bc), _i4(block),
+                                                         int(nvec), _dev_ptr(ws), _stream(stream)),
+           "lqcd_galerkin_coarse")
+    return torch.view_as_complex(A)
+
+
 def pack_nullvec(dst: torch.Tensor, src_vi: torch.Tensor, i: int, dims, block, nvec, stream=None):
     sfx = _same_dtype(dst, src_vi)
     _check(getattr(lib(), f"lqcd_pack_nullvec_{sfx}")(_dev_ptr(dst), _dev_ptr(src_vi), int(i), _i4(dims), _i4(block),

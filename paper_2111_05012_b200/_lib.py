@@ -29,6 +29,7 @@ SIGNATURES = {
     "lqcd_native_coarse_vec_reals": (C.c_size_t, [_i4, _ci]),
     "lqcd_native_coarse_mat_reals": (C.c_size_t, [_i4, _ci]),
     "lqcd_host_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
+    "lqcd_galerkin_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
 }
 for _p, _k in (("f32", _cf), ("f64", _cd)):
     SIGNATURES.update({
@@ -36,6 +37,10 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_unpack_spinor_{_p}": (_ci, [_vp, _vp, _i4, _vp]),
         f"lqcd_pack_gauge_{_p}": (_ci, [_vp, _vp, _i4, _cu, _vp]),
         f"lqcd_pack_clover_{_p}": (_ci, [_vp, _vp, _i4, _vp]),
+        f"lqcd_unpack_clover_{_p}": (_ci, [_vp, _vp, _i4, _vp]),
+        f"lqcd_clover_from_links_{_p}": (_ci, [_vp, _vp, _k, _k, _i4, _vp]),
+        f"lqcd_orthonormalize_blocks_{_p}": (_ci, [_vp, _i4, _i4, _ci, _vp]),
+        f"lqcd_galerkin_coarse_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _vp, _vp]),
         f"lqcd_pack_nullvec_{_p}": (_ci, [_vp, _vp, _ci, _i4, _i4, _ci, _vp]),
         f"lqcd_unpack_nullvec_{_p}": (_ci, [_vp, _vp, _ci, _i4, _i4, _ci, _vp]),
         f"lqcd_wilson_clover_mult_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _vp]),

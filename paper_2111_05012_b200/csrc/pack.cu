@@ -61,6 +61,29 @@ template <typename T> __global__ void k_clover(T* __restrict__ dst, const T* __r
     }
 }
 
+// native 72 reals -> canonical full Hermitian blocks F[s][chi][k][l] complex
+template <typename T> __global__ void k_clover_unpack(T* __restrict__ dst, const T* __restrict__ src, long long V) {
+    const long long n = V * 72;  // one thread per (site, chi, k, l)
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const long long s = idx / 72;
+        const int e = (int)(idx % 72), chi = e / 36, k = (e % 36) / 6, l = e % 6;
+        T re, im;
+        if (k == l) {
+            re = src[clover_off<T>(s, clover_diag_r(chi, k))];
+            im = 0;
+        } else if (k > l) {
+            re = src[clover_off<T>(s, clover_low_r(chi, k, l, 0))];
+            im = src[clover_off<T>(s, clover_low_r(chi, k, l, 1))];
+        } else {
+            re = src[clover_off<T>(s, clover_low_r(chi, l, k, 0))];
+            im = -src[clover_off<T>(s, clover_low_r(chi, l, k, 1))];
+        }
+        dst[idx * 2] = re;
+        dst[idx * 2 + 1] = im;
+    }
+}
+
 struct BlockGeom {
     int L[4], b[4], Lc[4];
     int bv;
@@ -140,6 +163,19 @@ template <typename T> static int clover_call(T* dst, const T* src, const int dim
     return check_launch(what);
 }
 
+template <typename T>
+static int clover_unpack_call(T* dst, const T* src, const int dims[4], void* stream, const char* what) {
+    clear_error();
+    if (!dst || !src || check_dims(dims) || !aligned16(dst) || !aligned16(src) || dst == src) {
+        set_error("%s: invalid argument", what);
+        return LQCD_EINVAL;
+    }
+    const long long V = volume(dims);
+    k_clover_unpack<T><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V);
+    count_launch();
+    return check_launch(what);
+}
+
 template <typename T, bool UNPACK>
 static int nullvec_call(T* native, T* canon, int i, const int dims[4], const int block[4], int nvec, void* stream,
                         const char* what) {
@@ -190,6 +226,12 @@ int lqcd_pack_clover_f32(float* d, const float* s, const int dims[4], void* st) 
 }
 int lqcd_pack_clover_f64(double* d, const double* s, const int dims[4], void* st) {
     return clover_call<double>(d, s, dims, st, "lqcd_pack_clover_f64");
+}
+int lqcd_unpack_clover_f32(float* d, const float* s, const int dims[4], void* st) {
+    return clover_unpack_call<float>(d, s, dims, st, "lqcd_unpack_clover_f32");
+}
+int lqcd_unpack_clover_f64(double* d, const double* s, const int dims[4], void* st) {
+    return clover_unpack_call<double>(d, s, dims, st, "lqcd_unpack_clover_f64");
 }
 int lqcd_pack_nullvec_f32(float* d, const float* s, int i, const int dims[4], const int block[4], int nvec, void* st) {
     return nullvec_call<float, false>(d, const_cast<float*>(s), i, dims, block, nvec, st, "lqcd_pack_nullvec_f32");

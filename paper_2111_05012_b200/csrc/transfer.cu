@@ -12,32 +12,11 @@
 //   prolong:  the nvec coarse coefficients sit in shared memory; each thread owns 16-byte slices of the
 //             aggregate and accumulates over i, no reduction across threads.
 // The paper's GPU version bounced these two steps through the host; here they stay on the device.
+#include "aggregate.cuh"
 #include "common.cuh"
 #include "knobs.h"
 
 namespace lqcd {
-
-struct TransferParams {
-    int L[4], b[4], Lc[4];
-    int bv;    // sites per block
-    int nvec;
-    int LV;    // vec16 per (X, chi, i) vector = bv * 12 / NV
-};
-
-// canonical fine site of local index l inside coarse site X
-__device__ __forceinline__ int fine_site(const TransferParams& P, int X, int l) {
-    int s = 0, stride = 1;
-#pragma unroll
-    for (int mu = 0; mu < 4; mu++) {
-        const int Xmu = X % P.Lc[mu];
-        X /= P.Lc[mu];
-        const int lmu = l % P.b[mu];
-        l /= P.b[mu];
-        s += (Xmu * P.b[mu] + lmu) * stride;
-        stride *= P.L[mu];
-    }
-    return s;
-}
 
 template <typename T> __device__ __forceinline__ void cdot_acc(T& sr, T& si, const V16<T>& a, const V16<T>& x);
 // sum conj(a) x over the complex entries of one vec16
@@ -155,34 +134,6 @@ __global__ void __launch_bounds__(256) k_prolong(T* __restrict__ out_f, const T*
         T* dst = out_f + (((long long)(s >> 5) * NJ + chi * JH + jj) * CH + (s & 31)) * NV;
         st16_stream(dst, acc);
     }
-}
-
-template <typename T>
-static int transfer_setup(TransferParams& P, const void* a, const void* b, const void* c, const int dims[4],
-                          const int block[4], int nvec, const char* what) {
-    clear_error();
-    if (!a || !b || !c) {
-        set_error("%s: null pointer", what);
-        return LQCD_EINVAL;
-    }
-    if (!aligned16(a) || !aligned16(b) || !aligned16(c)) {
-        set_error("%s: pointers must be 16-byte aligned", what);
-        return LQCD_EINVAL;
-    }
-    if (check_block(dims, block, nvec, P.Lc)) {
-        set_error("%s: bad dims/block/nvec (block must divide dims, coarse extents >= 2, nvec >= 1)", what);
-        return LQCD_EINVAL;
-    }
-    if (volume(dims) > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
-    P.bv = 1;
-    for (int mu = 0; mu < 4; mu++) {
-        P.L[mu] = dims[mu];
-        P.b[mu] = block[mu];
-        P.bv *= block[mu];
-    }
-    P.nvec = nvec;
-    P.LV = P.bv * 12 / VecOf<T>::NV;
-    return LQCD_OK;
 }
 
 template <typename T>
