@@ -129,6 +129,19 @@ template <typename T> __device__ __forceinline__ void st16(T* p, const V16<T>& v
     *reinterpret_cast<V16<T>*>(p) = v;
 }
 
+// ---- division by a run-time constant: q = n / d for 0 <= n with n * d < 2^32 (block and thread indices by lattice
+// extents), as one multiply-high (+ one multiply-add for d = 1) instead of the ~20-instruction integer division.
+// m = ceil(2^32 / d); floor(n m / 2^32) = floor(n / d) whenever n (m d - 2^32) < 2^32, which n d < 2^32 implies.
+struct FastDiv {
+    unsigned m;    // ceil(2^32 / d) for d >= 2, 0 for d = 1
+    unsigned one;  // 1 if d == 1
+    __host__ void set(int d) {
+        one = d == 1;
+        m = d == 1 ? 0u : (unsigned)((0x100000000ull + (unsigned)d - 1) / (unsigned)d);
+    }
+    __device__ __forceinline__ int div(int n) const { return (int)(__umulhi((unsigned)n, m) + (unsigned)n * one); }
+};
+
 // ---- geometry passed to kernels by value ---------------------------------------------------------
 struct Geom {
     int L[4];        // fine dims

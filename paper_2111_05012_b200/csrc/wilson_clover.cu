@@ -25,6 +25,8 @@ struct FineParams {
     int bc[4];     // +1 / -1
     int tilevol;   // threads that own a site (<= blockDim.x)
     int zslab;     // traversal slab extent in z tiles (0 = canonical tile order)
+    int per_slab, nslab_full;  // zslab * ntile[3]; number of slabs of full height
+    FastDiv d_ntile[3], d_tile[3], d_per_slab, d_zslab, d_dom[4];
     // domain-decomposed variant D_SAP; unused by the plain operator
     int dom[4];    // domain extents (the aggregation block)
     int multi[4];  // 1 if there is more than one domain in that direction (else no hop is ever cut)
@@ -93,34 +95,35 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
     k_wilson_clover(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ U, const T* __restrict__ clover,
                     T kappa, FineParams P) {
     // ---- which site is mine: CTA -> tile (x tiles fastest; optionally z-slabbed traversal), thread -> site in tile
+    // (all divisions by run-time extents are multiply-high with host-computed reciprocals: the index decode was a
+    // quarter of the integer work of this kernel)
     int tid = threadIdx.x;
     if (tid >= P.tilevol) return;
-    int b = blockIdx.x;
+    int b = blockIdx.x, q;
     int tc[4];
-    tc[0] = b % P.ntile[0]; b /= P.ntile[0];
-    tc[1] = b % P.ntile[1]; b /= P.ntile[1];
+    q = P.d_ntile[0].div(b); tc[0] = b - q * P.ntile[0]; b = q;
+    q = P.d_ntile[1].div(b); tc[1] = b - q * P.ntile[1]; b = q;
     if (P.zslab > 0) {
         // order: x, y, z within slab, t, slab  (keeps the +-t neighbours of a slab resident in L2)
-        const int nslab_full = P.ntile[2] / P.zslab;          // slabs of full height
-        const int per_slab = P.zslab * P.ntile[3];
-        int slab = b / per_slab;
-        int zs = P.zslab;
-        int r = b - slab * per_slab;
-        if (slab >= nslab_full) {  // ragged last slab
-            slab = nslab_full;
-            r = b - nslab_full * per_slab;
-            zs = P.ntile[2] - nslab_full * P.zslab;
+        const int slab = P.d_per_slab.div(b);
+        const int r = b - slab * P.per_slab;
+        if (slab >= P.nslab_full) {  // ragged last slab (rare: slabs are chosen of equal height when possible)
+            const int zs = P.ntile[2] - P.nslab_full * P.zslab;
+            const int rr = b - P.nslab_full * P.per_slab;
+            tc[2] = P.nslab_full * P.zslab + rr % zs;
+            tc[3] = rr / zs;
+        } else {
+            tc[3] = P.d_zslab.div(r);
+            tc[2] = slab * P.zslab + (r - tc[3] * P.zslab);
         }
-        tc[2] = slab * P.zslab + r % zs;
-        tc[3] = r / zs;
     } else {
-        tc[2] = b % P.ntile[2];
-        tc[3] = b / P.ntile[2];
+        tc[3] = P.d_ntile[2].div(b);
+        tc[2] = b - tc[3] * P.ntile[2];
     }
     int x[4];
-    x[0] = tc[0] * P.tile[0] + tid % P.tile[0]; tid /= P.tile[0];
-    x[1] = tc[1] * P.tile[1] + tid % P.tile[1]; tid /= P.tile[1];
-    x[2] = tc[2] * P.tile[2] + tid % P.tile[2]; tid /= P.tile[2];
+    q = P.d_tile[0].div(tid); x[0] = tc[0] * P.tile[0] + (tid - q * P.tile[0]); tid = q;
+    q = P.d_tile[1].div(tid); x[1] = tc[1] * P.tile[1] + (tid - q * P.tile[1]); tid = q;
+    q = P.d_tile[2].div(tid); x[2] = tc[2] * P.tile[2] + (tid - q * P.tile[2]); tid = q;
     x[3] = tc[3] * P.tile[3] + tid;
     const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
     const int s = x[0] + st1 * x[1] + st2 * x[2] + st3 * x[3];
@@ -155,7 +158,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
         int par = 0;
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) {
-            const int X = x[mu] / P.dom[mu], lx = x[mu] - X * P.dom[mu];
+            const int X = P.d_dom[mu].div(x[mu]), lx = x[mu] - X * P.dom[mu];
             par += X;
             if (P.multi[mu] && lx == P.dom[mu] - 1) {  // forward hop leaves the domain
                 sf[mu] = s;
@@ -300,6 +303,24 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
         }
     }
     if (P.zslab >= P.ntile[2]) P.zslab = 0;
+    // reciprocals for the index decode (exact while n * d < 2^32: n is a tile index or a thread index)
+    P.per_slab = (P.zslab > 0 ? P.zslab : 1) * P.ntile[3];
+    P.nslab_full = P.zslab > 0 ? P.ntile[2] / P.zslab : 0;
+    {
+        long long dmax = P.per_slab;
+        for (int mu = 0; mu < 3; mu++) dmax = P.ntile[mu] > dmax ? P.ntile[mu] : dmax;
+        if (ntiles * dmax >= 0x100000000LL) {
+            set_error("%s: lattice too large for the 32-bit index decode", what);
+            return LQCD_EUNSUPPORTED;
+        }
+    }
+    for (int mu = 0; mu < 3; mu++) {
+        P.d_ntile[mu].set(P.ntile[mu]);
+        P.d_tile[mu].set(P.tile[mu]);
+    }
+    P.d_per_slab.set(P.per_slab);
+    P.d_zslab.set(P.zslab > 0 ? P.zslab : 1);
+    for (int mu = 0; mu < 4; mu++) P.d_dom[mu].set(P.dom[mu]);
     int threads = (P.tilevol + 31) / 32 * 32;
     const bool dag = flags & LQCD_DAGGER, l12 = flags & LQCD_LINKS_12;
     cudaStream_t st = (cudaStream_t)stream;
