@@ -211,3 +211,49 @@ def wilson_clover_dd_mult_sites(psi, U, clover, kappa, dims, bc, domain, sites, 
             C.c_int(parity), C.c_uint(DAGGER if dagger else 0), _ptr(sites), C.c_long(len(sites)))
     _check(rc, "wilson_clover_dd_mult_sites")
     return out
+
+
+def _c128(a):
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def block_dotc(a, b, dims, domain) -> np.ndarray:
+    """F3, blocked BLAS-1: out[X] = <a|b> restricted to domain X (fp64 only)."""
+    a, b = _c128(a), _c128(b)
+    Vc = int(np.prod([l // d for l, d in zip(dims, domain)]))
+    out = np.empty(Vc, dtype=np.complex128)
+    fn = lib().lqcd_block_dotc_ref
+    fn.restype = C.c_int
+    _check(fn(_ptr(out), _ptr(a), _ptr(b), _i4(dims), _i4(domain)), "block_dotc")
+    return out
+
+
+def block_caxpy(y, coef, a, dims, domain) -> np.ndarray:
+    """y + coef[X(x)] * a, one complex coefficient per domain; returns a new array."""
+    y, coef, a = np.array(y, dtype=np.complex128, order="C", copy=True), _c128(coef), _c128(a)
+    fn = lib().lqcd_block_caxpy_ref
+    fn.restype = C.c_int
+    _check(fn(_ptr(y), _ptr(coef), _ptr(a), _i4(dims), _i4(domain)), "block_caxpy")
+    return y
+
+
+def mr_domain_solve(r, U, clover, kappa, dims, bc, domain, parity, niter) -> np.ndarray:
+    """z = M_SAP^(e/o) r: `niter` minimal-residual iterations per domain (Q17)."""
+    r, U, clover = _c128(r), _c128(U), _c128(clover)
+    z = np.empty_like(r)
+    fn = lib().lqcd_mr_domain_solve_ref
+    fn.restype = C.c_int
+    _check(fn(_ptr(z), _ptr(r), _ptr(U), _ptr(clover), C.c_double(kappa), _i4(dims), _i4(bc), _i4(domain),
+              C.c_int(parity), C.c_int(niter)), "mr_domain_solve")
+    return z
+
+
+def sap(b, U, clover, kappa, dims, bc, domain, n_sap=4, n_mr=6):
+    """SAP with fixed iterations -> (x, final residual b - D x)."""
+    b, U, clover = _c128(b), _c128(U), _c128(clover)
+    x, r = np.empty_like(b), np.empty_like(b)
+    fn = lib().lqcd_sap_ref
+    fn.restype = C.c_int
+    _check(fn(_ptr(x), _ptr(r), _ptr(b), _ptr(U), _ptr(clover), C.c_double(kappa), _i4(dims), _i4(bc), _i4(domain),
+              C.c_int(n_sap), C.c_int(n_mr)), "sap")
+    return x, r

@@ -842,3 +842,114 @@ int FN(lqcd_wilson_clover_dd_mult_sites)(zc* out, const inc* in, const inc* U, c
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * F3. Blocked linear algebra, the inner-domain solver and the SAP smoother.
+ *
+ * Blocked BLAS-1 ("dotc, axpy, ... per block"): the same operations restricted to each domain X,
+ * giving one number per domain:
+ *    block_dotc[X]  = sum_{x in X} sum_{alpha,c} conj(a(x,alpha,c)) b(x,alpha,c)
+ *    block_caxpy:     y(x) += coef[X(x)] a(x)
+ *
+ * Inner-domain solver M_SAP^(e/o) ~ (D_SAP^(e/o))^-1 "MINRES algorithm with fixed number of iterations, 6"
+ * (PAPER.md:133).  D_SAP is not Hermitian, so the reading (Q17) is the minimal-residual iteration of the
+ * SAP literature the paper cites ([10, 11]), run independently in every domain of the selected group with z_0 = 0:
+ *    rho := P_g r ;  z := 0
+ *    repeat niter times:   p := D_SAP^(g) rho
+ *                          alpha[X] := <p|rho>_X / <p|p>_X      (0 if <p|p>_X = 0)
+ *                          z += alpha rho ;  rho -= alpha p
+ *
+ * SAP with fixed iterations, the listing of PAPER.md:127-131:
+ *    x := 0, r := b;  for i = 1..n:  x += M^(e) r;  r := b - D x;  x += M^(o) r;  r := b - D x
+ * ---------------------------------------------------------------------------------------- */
+#ifdef LQCD_ORACLE_FP64_BUILD
+int FN(lqcd_block_dotc)(zc* out, const zc* a, const zc* b, const int L[4], const int blk[4]) {
+    int Lc[4];
+    if (!out || !a || !b || check_domain(L, blk, Lc)) return -1;
+    const long Vc = volume_of(Lc), bv = volume_of(blk);
+#pragma omp parallel for schedule(static)
+    for (long X = 0; X < Vc; X++) {
+        zc sum = 0;
+        for (long l = 0; l < bv; l++) {
+            const long s = block_site(L, blk, Lc, X, l);
+            for (int k = 0; k < 12; k++) sum += conj(a[s * 12 + k]) * b[s * 12 + k];
+        }
+        out[X] = sum;
+    }
+    return 0;
+}
+
+int FN(lqcd_block_caxpy)(zc* y, const zc* coef, const zc* a, const int L[4], const int blk[4]) {
+    int Lc[4];
+    if (!y || !coef || !a || check_domain(L, blk, Lc)) return -1;
+    const long V = volume_of(L);
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < V; s++) {
+        const zc c = coef[coarse_site_of(L, blk, Lc, s)];
+        for (int k = 0; k < 12; k++) y[s * 12 + k] += c * a[s * 12 + k];
+    }
+    return 0;
+}
+
+/* z = M_SAP^(g) r: niter minimal-residual iterations per domain of group g (1 = even, 2 = odd, 0 = all) */
+int FN(lqcd_mr_domain_solve)(zc* z, const zc* r, const zc* U, const zc* clover, double kappa, const int L[4],
+                             const int bc[4], const int blk[4], int parity, int niter) {
+    int Lc[4];
+    if (!z || !r || !U || !clover || check_dims_bc(L, bc) || check_domain(L, blk, Lc) || parity < 0 || parity > 2 ||
+        niter < 0)
+        return -1;
+    const long V = volume_of(L), Vc = volume_of(Lc);
+    zc* rho = (zc*)malloc(sizeof(zc) * V * 12);
+    zc* p = (zc*)malloc(sizeof(zc) * V * 12);
+    zc* pr = (zc*)malloc(sizeof(zc) * Vc);
+    zc* pp = (zc*)malloc(sizeof(zc) * Vc);
+    zc* alpha = (zc*)malloc(sizeof(zc) * Vc);
+    if (!rho || !p || !pr || !pp || !alpha) return -3;
+    for (long s = 0; s < V; s++) {
+        const int keep = parity == 0 || domain_parity(L, blk, s) == parity - 1;
+        for (int k = 0; k < 12; k++) {
+            rho[s * 12 + k] = keep ? r[s * 12 + k] : 0;
+            z[s * 12 + k] = 0;
+        }
+    }
+    for (int it = 0; it < niter; it++) {
+        FN(lqcd_wilson_clover_dd_mult)(p, (const inc*)rho, (const inc*)U, (const inc*)clover, kappa, L, bc, blk, parity,
+                                       0);
+        FN(lqcd_block_dotc)(pr, p, rho, L, blk);
+        FN(lqcd_block_dotc)(pp, p, p, L, blk);
+        for (long X = 0; X < Vc; X++) alpha[X] = creal(pp[X]) > 0 ? pr[X] / creal(pp[X]) : 0;
+        FN(lqcd_block_caxpy)(z, alpha, rho, L, blk);
+        for (long X = 0; X < Vc; X++) alpha[X] = -alpha[X];
+        FN(lqcd_block_caxpy)(rho, alpha, p, L, blk);
+    }
+    free(rho); free(p); free(pr); free(pp); free(alpha);
+    return 0;
+}
+
+/* x = SAP_n(b); r_out (may be NULL) receives the final residual b - D x */
+int FN(lqcd_sap)(zc* x, zc* r_out, const zc* b, const zc* U, const zc* clover, double kappa, const int L[4],
+                 const int bc[4], const int blk[4], int n_sap, int n_mr) {
+    int Lc[4];
+    if (!x || !b || !U || !clover || check_dims_bc(L, bc) || check_domain(L, blk, Lc) || n_sap < 0 || n_mr < 0)
+        return -1;
+    const long V = volume_of(L);
+    zc* r = (zc*)malloc(sizeof(zc) * V * 12);
+    zc* z = (zc*)malloc(sizeof(zc) * V * 12);
+    zc* t = (zc*)malloc(sizeof(zc) * V * 12);
+    if (!r || !z || !t) return -3;
+    for (long k = 0; k < V * 12; k++) {
+        x[k] = 0;
+        r[k] = b[k];
+    }
+    for (int i = 0; i < n_sap; i++)
+        for (int g = 1; g <= 2; g++) {
+            FN(lqcd_mr_domain_solve)(z, r, U, clover, kappa, L, bc, blk, g, n_mr); /* z = M^(e/o) r */
+            for (long k = 0; k < V * 12; k++) x[k] += z[k];
+            FN(lqcd_wilson_clover_mult)(t, (const inc*)x, (const inc*)U, (const inc*)clover, kappa, L, bc, 0);
+            for (long k = 0; k < V * 12; k++) r[k] = b[k] - t[k];
+        }
+    if (r_out) memcpy(r_out, r, sizeof(zc) * V * 12);
+    free(r); free(z); free(t);
+    return 0;
+}
+#endif

@@ -517,3 +517,109 @@ def test_dsap_limits_and_structure(c1):
     s = oracle.wilson_clover_dd_mult_sites(x32, U32, c32, cfg.kappa, cfg.dims, cfg.bc, cfg.block, sites, parity=2,
                                            dagger=True)
     assert np.array_equal(s, a[sites])
+
+
+# ------------------------------------------------------------------------------------------------
+# F3  blocked BLAS-1, the inner-domain minimal-residual solver and SAP
+# ------------------------------------------------------------------------------------------------
+
+
+def test_block_blas_against_numpy(c1):
+    cfg = c1["cfg"]
+    a, b = c1["psi"]
+    dims, dom = cfg.dims, (2, 4, 1, 2)
+    idx, _ = domain_index(dims, dom)
+    nd = idx.max() + 1
+    ref = np.array([np.vdot(a[idx == X], b[idx == X]) for X in range(nd)])
+    assert np.max(np.abs(oracle.block_dotc(a, b, dims, dom) - ref)) < 1e-12
+    coef = np.random.default_rng(4).standard_normal(nd) + 1j * np.random.default_rng(5).standard_normal(nd)
+    assert np.max(np.abs(oracle.block_caxpy(b, coef, a, dims, dom) - (b + coef[idx][:, None, None] * a))) < 1e-13
+
+
+def dense_of(apply, V):
+    n = 12 * V
+    M = np.zeros((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1
+        M[:, k] = apply(e.reshape(V, 4, 3)).ravel()
+    return M
+
+
+def numpy_mr(A, r, niter):
+    """textbook minimal-residual iteration on a dense matrix, z0 = 0"""
+    z, rho = np.zeros_like(r), r.copy()
+    for _ in range(niter):
+        p = A @ rho
+        alpha = np.vdot(p, rho) / np.vdot(p, p)
+        z += alpha * rho
+        rho -= alpha * p
+    return z
+
+
+def test_mr_domain_solve_is_mr_on_each_domain_block():
+    """Brute force: dense D_SAP (pinned above) cut into its domain blocks, textbook MR on each block separately."""
+    dims, dom, bc = (4, 2, 2, 4), (2, 2, 2, 2), (1, 1, 1, -1)
+    V = int(np.prod(dims))
+    rng = np.random.default_rng(31)
+    U = li.gauge_exp(rng, V, 0.6)
+    clov = oracle.clover_from_links(U, 0.13, 1.2, dims)
+    r = li.spinor(rng, V)
+    Ds = dense_of(lambda e: oracle.wilson_clover_dd_mult(e, U, clov, 0.13, dims, bc, dom), V)
+    idx, par = domain_index(dims, dom)
+    idx12, par12 = np.repeat(idx, 12), np.repeat(par, 12)
+    for parity in (0, 1, 2):
+        for niter in (1, 6):
+            ref = np.zeros(12 * V, dtype=np.complex128)
+            for X in range(idx.max() + 1):
+                m = idx12 == X
+                if parity and par12[m][0] != parity - 1:
+                    continue
+                ref[m] = numpy_mr(Ds[np.ix_(m, m)], r.ravel()[m], niter)
+            got = oracle.mr_domain_solve(r, U, clov, 0.13, dims, bc, dom, parity, niter).ravel()
+            assert np.max(np.abs(got - ref)) < 1e-13, (parity, niter)
+    # enough iterations converge to the exact inverse on the selected group: D_SAP^(e) M^(e) r = P_e r
+    z = oracle.mr_domain_solve(r, U, clov, 0.13, dims, bc, dom, 1, 200)
+    keep = par12 == 0
+    assert np.max(np.abs((Ds @ z.ravel())[keep] - r.ravel()[keep])) < 1e-10
+    assert np.max(np.abs(z.ravel()[~keep])) == 0.0
+
+
+def test_sap_listing(c1):
+    """The listing of PAPER.md:127-131 retyped on top of dense matrices, and its invariants."""
+    dims, dom, bc = (4, 2, 2, 4), (2, 2, 2, 2), (1, 1, 1, -1)
+    V = int(np.prod(dims))
+    rng = np.random.default_rng(32)
+    U = li.gauge_exp(rng, V, 0.6)
+    clov = oracle.clover_from_links(U, 0.13, 1.2, dims)
+    b = li.spinor(rng, V)
+    D = dense_of(lambda e: oracle.wilson_clover_mult(e, U, clov, 0.13, dims, bc), V)
+    Ds = dense_of(lambda e: oracle.wilson_clover_dd_mult(e, U, clov, 0.13, dims, bc, dom), V)
+    idx, par = domain_index(dims, dom)
+    idx12, par12 = np.repeat(idx, 12), np.repeat(par, 12)
+
+    def M(group, r, n_mr):  # block-wise textbook MR on the domains of one group
+        z = np.zeros_like(r)
+        for X in range(idx.max() + 1):
+            m = idx12 == X
+            if par12[m][0] == group:
+                z[m] = numpy_mr(Ds[np.ix_(m, m)], r[m], n_mr)
+        return z
+
+    n_sap, n_mr = 3, 4
+    x, r = np.zeros(12 * V, dtype=np.complex128), b.ravel().copy()
+    norms = [np.linalg.norm(r)]
+    for _ in range(n_sap):
+        for group in (0, 1):
+            x += M(group, r, n_mr)
+            r = b.ravel() - D @ x
+            norms.append(np.linalg.norm(r))
+    gx, gr = oracle.sap(b, U, clov, 0.13, dims, bc, dom, n_sap=n_sap, n_mr=n_mr)
+    assert np.max(np.abs(gx.ravel() - x)) < 1e-13 and np.max(np.abs(gr.ravel() - r)) < 1e-13
+    assert all(b2 < b1 for b1, b2 in zip(norms, norms[1:])), "every half sweep reduces the residual here"
+    assert norms[-1] < 0.05 * norms[0]
+    # config 1 with the paper's parameters (n = 4, 6 MR iterations): the returned residual is the true residual
+    cfg = c1["cfg"]
+    x1, r1 = oracle.sap(c1["psi"][0], c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc, cfg.block)
+    true_r = c1["psi"][0] - oracle.wilson_clover_mult(x1, c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc)
+    assert rel(r1, true_r) < 1e-13 and np.linalg.norm(r1) < 0.05 * np.linalg.norm(c1["psi"][0])
