@@ -69,6 +69,9 @@ extern "C" {
 #define LQCD_LINKS_12 2u /* U holds the 12-real compressed native gauge layout */
 #define LQCD_DOMAIN_EVEN 4u /* lqcd_wilson_clover_dd_mult only: compute even domains, zero elsewhere */
 #define LQCD_DOMAIN_ODD 8u  /* lqcd_wilson_clover_dd_mult only: compute odd domains, zero elsewhere */
+#define LQCD_ACCUMULATE 16u /* lqcd_mr_domain_solve: z += M r on the selected domains, other sites untouched */
+#define LQCD_SAP_INITIAL_GUESS 32u     /* lqcd_sap: x holds x0 on entry; start from r = b - D x0 instead of x = 0 */
+#define LQCD_SAP_NO_FINAL_RESIDUAL 64u /* lqcd_sap: skip the last r = b - D x (r is then NOT the final residual) */
 
 /* ---- diagnostics ------------------------------------------------------------------------- */
 int lqcd_version(void);
@@ -193,6 +196,66 @@ int lqcd_galerkin_coarse_f32(float* A, const float* U, const float* clover, cons
 int lqcd_galerkin_coarse_f64(double* A, const double* U, const double* clover, const double* nullvecs, double kappa,
                              const int dims[4], const int bc[4], const int block[4], int nvec, void* ws_dev,
                              void* stream);
+
+/* ---- F3: Richardson residual, blocked BLAS-1, inner-domain solver, SAP --------
+ * Residual of one Richardson refinement "|x> + M_i(|b> - D|x>)" and of the SAP listing (PAPER.md:
+ * 128-131) in one pass:  r = b - D x.  r must not alias x (it may alias b).  flags: LQCD_LINKS_12 only. */
+int lqcd_wilson_clover_residual_f32(float* r, const float* b, const float* x, const float* U, const float* clover,
+                                    float kappa, const int dims[4], const int bc[4], unsigned flags, void* stream);
+int lqcd_wilson_clover_residual_f64(double* r, const double* b, const double* x, const double* U,
+                                    const double* clover, double kappa, const int dims[4], const int bc[4],
+                                    unsigned flags, void* stream);
+
+/* Blocked linear algebra ("a set of blocked version of linear algebraic functions such as dotc and axpy",
+ * PAPER.md:155-157): the BLAS-1 operation restricted to each domain X (domain[4] divides dims; any number of
+ * domains per direction, including 1), one number per domain, X in canonical coarse order.
+ *   dotc:  out[X] = sum_{x in X} sum_{alpha,c} conj(a(x,alpha,c)) b(x,alpha,c)      out: Vc complex (re, im)
+ *   caxpy: y(x) += coef[X(x)] a(x)                                                  coef: Vc complex
+ * a, b, y: native spinors.  Fixed summation order (bit-reproducible). */
+int lqcd_block_dotc_f32(float* out, const float* a, const float* b, const int dims[4], const int domain[4],
+                        void* stream);
+int lqcd_block_dotc_f64(double* out, const double* a, const double* b, const int dims[4], const int domain[4],
+                        void* stream);
+int lqcd_block_caxpy_f32(float* y, const float* coef, const float* a, const int dims[4], const int domain[4],
+                         void* stream);
+int lqcd_block_caxpy_f64(double* y, const double* coef, const double* a, const int dims[4], const int domain[4],
+                         void* stream);
+
+/* Inner-domain solver z = M_SAP^(g) r ~ (D_SAP^(g))^-1 r: "the MINRES algorithm with fixed number of iterations"
+ * (PAPER.md:133).  D_SAP is not Hermitian, so this is the minimal-residual iteration of the SAP literature the paper
+ * cites (reading Q17), run independently in every domain X of the selected group, from z = 0:
+ *   rho = P_g r;  repeat niter times:  p = D_SAP^(g) rho;  alpha[X] = <p|rho>_X / <p|p>_X (0 if <p|p>_X = 0);
+ *                                      z += alpha rho;  rho -= alpha p.
+ * flags: LQCD_DOMAIN_EVEN / LQCD_DOMAIN_ODD select the group (neither: all domains); without LQCD_ACCUMULATE z is
+ * overwritten (zero outside the group), with it z += M r on the group's sites and the others are left untouched.
+ * U: native 18-real gauge.  z must not alias r.  When a domain's residual, links and clover term fit in the shared
+ * memory of one SM (fp32: |domain| <= 256 sites, e.g. 4^4) all niter iterations run inside ONE kernel with the
+ * operator read from HBM once; other sizes take a generic path that needs ws_dev, device scratch of
+ * lqcd_mr_workspace_bytes(dims, domain, sizeof(real)) bytes (0 when the resident kernel applies; then ws_dev may be
+ * NULL).  Both paths compute the same iteration; results agree to rounding. */
+size_t lqcd_mr_workspace_bytes(const int dims[4], const int domain[4], int real_bytes);
+int lqcd_mr_domain_solve_f32(float* z, const float* r, const float* U, const float* clover, float kappa,
+                             const int dims[4], const int bc[4], const int domain[4], unsigned flags, int niter,
+                             void* ws_dev, void* stream);
+int lqcd_mr_domain_solve_f64(double* z, const double* r, const double* U, const double* clover, double kappa,
+                             const int dims[4], const int bc[4], const int domain[4], unsigned flags, int niter,
+                             void* ws_dev, void* stream);
+
+/* Schwarz alternating procedure with fixed iterations, the listing of PAPER.md:127-131:
+ *   |x> := 0, |r> := |b>;  for i = 1..n_sap:  |x> += M_SAP^(e)|r>;  |r> := |b> - D|x>;
+ *                                             |x> += M_SAP^(o)|r>;  |r> := |b> - D|x>
+ * with M_SAP^(e/o) = lqcd_mr_domain_solve with n_mr iterations (paper: n_sap = 4, n_mr = 6).
+ * x: the result; r: caller-owned scratch spinor that receives the final residual b - D x; b: right-hand side; all
+ * three distinct native spinors.  flags: LQCD_SAP_INITIAL_GUESS starts from the x passed in (|r> := |b> - D|x>
+ * first): x0 + SAP(b - D x0), the Richardson refinement with M_2 = SAP in one call;
+ * LQCD_SAP_NO_FINAL_RESIDUAL omits the last residual (saves one application of D when r is not needed).
+ * ws_dev as for lqcd_mr_domain_solve.  2 n_sap solver launches + 2 n_sap residual launches on `stream`. */
+int lqcd_sap_f32(float* x, float* r, const float* b, const float* U, const float* clover, float kappa,
+                 const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
+                 void* ws_dev, void* stream);
+int lqcd_sap_f64(double* x, double* r, const double* b, const double* U, const double* clover, double kappa,
+                 const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
+                 void* ws_dev, void* stream);
 
 /* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the

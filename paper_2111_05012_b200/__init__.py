@@ -20,6 +20,9 @@ DAGGER = 1
 LINKS_12 = 2
 DOMAIN_EVEN = 4
 DOMAIN_ODD = 8
+ACCUMULATE = 16
+SAP_INITIAL_GUESS = 32
+SAP_NO_FINAL_RESIDUAL = 64
 
 OK, EINVAL, EUNSUPPORTED, ECUDA = 0, -1, -2, -3
 
@@ -299,6 +302,75 @@ def prolong(out_f, in_c, nullvecs, dims, block, nvec, stream=None):
                                                  _i4(block), int(nvec), _stream(stream)), "lqcd_prolong")
     return out_f
 
+
+# ---- F3: residual, blocked BLAS-1, inner-domain solver, SAP ------------------------------------------------------
+def wilson_clover_residual(r, b, x, U, clover, kappa, dims, bc, links12=False, stream=None):
+    """r = b - D x in one pass."""
+    sfx = _same_dtype(r, b, x, U, clover)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_wilson_clover_residual_{sfx}")(_dev_ptr(r), _dev_ptr(b), _dev_ptr(x), _dev_ptr(U),
+                                                                _dev_ptr(clover), k, _i4(dims), _i4(bc),
+                                                                LINKS_12 if links12 else 0, _stream(stream)),
+           "lqcd_wilson_clover_residual")
+    return r
+
+
+def _ndomains(dims, domain) -> int:
+    n = 1
+    for l, d in zip(dims, domain):
+        n *= int(l) // int(d)
+    return n
+
+
+def block_dotc(a, b, dims, domain, stream=None) -> torch.Tensor:
+    """out[X] = <a|b> restricted to domain X; complex tensor of one entry per domain."""
+    sfx = _same_dtype(a, b)
+    out = torch.zeros((_ndomains(dims, domain), 2), dtype=_rdtype(sfx), device=a.device)
+    _check(getattr(lib(), f"lqcd_block_dotc_{sfx}")(_dev_ptr(out), _dev_ptr(a), _dev_ptr(b), _i4(dims), _i4(domain),
+                                                    _stream(stream)), "lqcd_block_dotc")
+    return torch.view_as_complex(out)
+
+
+def block_caxpy(y, coef, a, dims, domain, stream=None):
+    """y(x) += coef[X(x)] a(x) (PAPER.md:155)."""
+    sfx = _same_dtype(y, coef, a)
+    _check(getattr(lib(), f"lqcd_block_caxpy_{sfx}")(_dev_ptr(y), _dev_ptr(coef), _dev_ptr(a), _i4(dims), _i4(domain),
+                                                     _stream(stream)), "lqcd_block_caxpy")
+    return y
+
+
+def mr_workspace(dims, domain, dtype=torch.float32, device="cuda"):
+    """Scratch for mr_domain_solve / sap (None when the shared-memory-resident kernel applies)."""
+    n = int(lib().lqcd_mr_workspace_bytes(_i4(dims), _i4(domain), 4 if dtype == torch.float32 else 8))
+    return torch.empty(n, dtype=torch.uint8, device=device) if n else None
+
+
+def _ws_ptr(ws):
+    return C.c_void_p(None) if ws is None else _dev_ptr(ws)
+
+
+def mr_domain_solve(z, r, U, clover, kappa, dims, bc, domain, parity=0, niter=6, accumulate=False, ws=None,
+                    stream=None):
+    """z (+)= M_SAP^(g) r: niter minimal-residual iterations in every domain of group `parity`."""
+    sfx = _same_dtype(z, r, U, clover)
+    flags = {0: 0, 1: DOMAIN_EVEN, 2: DOMAIN_ODD}[parity] | (ACCUMULATE if accumulate else 0)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_mr_domain_solve_{sfx}")(_dev_ptr(z), _dev_ptr(r), _dev_ptr(U), _dev_ptr(clover), k,
+                                                         _i4(dims), _i4(bc), _i4(domain), flags, int(niter),
+                                                         _ws_ptr(ws), _stream(stream)), "lqcd_mr_domain_solve")
+    return z
+
+
+def sap(x, r, b, U, clover, kappa, dims, bc, domain, n_sap=4, n_mr=6, initial_guess=False, final_residual=True,
+        ws=None, stream=None):
+    """SAP with fixed iterations: x = SAP_n(b) (or x0 + SAP_n(b - D x0)); r = b - D x."""
+    sfx = _same_dtype(x, r, b, U, clover)
+    flags = (SAP_INITIAL_GUESS if initial_guess else 0) | (0 if final_residual else SAP_NO_FINAL_RESIDUAL)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_sap_{sfx}")(_dev_ptr(x), _dev_ptr(r), _dev_ptr(b), _dev_ptr(U), _dev_ptr(clover), k,
+                                             _i4(dims), _i4(bc), _i4(domain), int(n_sap), int(n_mr), flags,
+                                             _ws_ptr(ws), _stream(stream)), "lqcd_sap")
+    return x
 
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,

@@ -30,6 +30,7 @@ SIGNATURES = {
     "lqcd_native_coarse_mat_reals": (C.c_size_t, [_i4, _ci]),
     "lqcd_host_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_galerkin_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
+    "lqcd_mr_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
 }
 for _p, _k in (("f32", _cf), ("f64", _cd)):
     SIGNATURES.update({
@@ -48,6 +49,11 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_coarse_mult_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _vp]),
         f"lqcd_restrict_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp]),
         f"lqcd_prolong_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp]),
+        f"lqcd_wilson_clover_residual_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _vp]),
+        f"lqcd_block_dotc_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _vp]),
+        f"lqcd_block_caxpy_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _vp]),
+        f"lqcd_mr_domain_solve_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _cu, _ci, _vp, _vp]),
+        f"lqcd_sap_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _cu, _vp, _vp]),
     })
 SIGNATURES.update({
     "lqcd_wilson_clover_mult_host_f32": (_ci, [_vp, _vp, _vp, _vp, _cf, _i4, _i4, _cu, _vp, _vp]),

@@ -173,4 +173,45 @@ template <bool FWD, typename T> __device__ __forceinline__ void su3_mult(T g[12]
         }
 }
 
+// out6 += Hermitian 6x6 block (36 reals: 6 diagonal, 15 complex strictly-lower row-major) times in6
+template <typename T> __device__ __forceinline__ void herm6_madd(T out[12], const T cl[36], const T in[12]) {
+#pragma unroll
+    for (int k = 0; k < 6; k++) {
+        T sr = fma(cl[k], in[2 * k], out[2 * k]);
+        T si = fma(cl[k], in[2 * k + 1], out[2 * k + 1]);
+#pragma unroll
+        for (int l = 0; l < 6; l++) {
+            if (l == k) continue;
+            const T xr = in[2 * l], xi = in[2 * l + 1];
+            if (l < k) {  // L_kl
+                const T ar = cl[6 + 2 * tri(k, l)], ai = cl[6 + 2 * tri(k, l) + 1];
+                sr = fma(ar, xr, sr);
+                sr = fma(-ai, xi, sr);
+                si = fma(ar, xi, si);
+                si = fma(ai, xr, si);
+            } else {  // conj(L_lk)
+                const T ar = cl[6 + 2 * tri(l, k)], ai = cl[6 + 2 * tri(l, k) + 1];
+                sr = fma(ar, xr, sr);
+                sr = fma(ai, xi, sr);
+                si = fma(ar, xi, si);
+                si = fma(-ai, xr, si);
+            }
+        }
+        out[2 * k] = sr;
+        out[2 * k + 1] = si;
+    }
+}
+
+template <typename T, bool G64 = false>
+__device__ __forceinline__ void load_clover_block(T cl[36], const T* __restrict__ C, int s, int chi) {
+    constexpr int NV = VecOf<T>::NV, NJ = 72 / NV;
+    const T* base = C + (((long long)(s >> 5) * NJ + chi * (36 / NV)) * CH + (s & 31)) * NV;
+#pragma unroll
+    for (int j = 0; j < 36 / NV; j++) {
+        V16<T> v = G64 ? ld16_stream_g64(base + (long long)j * CH * NV) : ld16_stream(base + (long long)j * CH * NV);
+#pragma unroll
+        for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
+    }
+}
+
 }  // namespace lqcd

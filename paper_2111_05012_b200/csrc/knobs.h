@@ -9,6 +9,7 @@ struct Knobs {
     int coarse_R = 0;                 // rows in flight per lane (1, 2, 4), 0 = automatic (2)
     int coarse_warps = 0;             // warps per CTA of the coarse kernel, 0 = automatic
     int transfer_warps = 0;           // warps per CTA of restrict, 0 = automatic
+    int sap_fused = 0;                // 0 = shared-memory-resident inner-domain solver when it fits; -1 = never
 };
 extern Knobs g_knobs;
 }  // namespace lqcd

@@ -1,0 +1,693 @@
+// sap.cu -- row F3 of SURVEY.md section 8(f): blocked BLAS-1, the inner-domain solver
+// M_SAP^(e/o) ~ (D_SAP^(e/o))^-1 ("MINRES algorithm with fixed number of iterations, 6"; reading Q17
+// of DESIGN.md: the minimal-residual iteration, run independently in every domain) and the Schwarz alternating
+// procedure with fixed iterations (listing PAPER.md:127-131).
+//
+// B200 design: a 4^4 domain's residual, links and clover term are 168 KB in fp32 -- they
+// fit the 227 KB of shared memory of one SM.  k_mr_domain therefore runs ALL n_mr iterations of one domain inside
+// one CTA: the operator fields are read from HBM once per half sweep instead of once per iteration, the blocked
+// dot products are CTA reductions, the blocked axpys are register updates, and nothing but the solution goes back
+// to HBM.  Domains that do not fit (fp64 4^4, 8x4^3) take the generic path: D_SAP^(e/o) by k_wilson_clover and
+// one fused blocked dotc/dotc/axpy/axpy kernel per iteration.
+#include "common.cuh"
+#include "fermion.cuh"
+#include "knobs.h"
+#include "layout.cuh"
+
+namespace lqcd {
+
+template <typename T>
+int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
+                       const int bc[4], const int* domain, unsigned flags, void* stream, const char* what);
+
+struct DomParams {
+    int L[4], dom[4], Lc[4], bc[4], multi[4];
+    int bv, Vc;
+    int parity;    // 0 = all domains, 1 = even, 2 = odd
+    int halfgrid;  // 1: the grid enumerates only the domains of the selected group (needs Lc[0] even)
+};
+
+// Coarse coordinates of the domain of CTA b; false if that domain is not in the selected group.
+__device__ __forceinline__ bool domain_of_cta(const DomParams& P, int b, int Xc[4]) {
+    if (P.halfgrid) {
+        const int h = P.Lc[0] >> 1;
+        const int hx = b % h;
+        b /= h;
+        Xc[1] = b % P.Lc[1];
+        b /= P.Lc[1];
+        Xc[2] = b % P.Lc[2];
+        Xc[3] = b / P.Lc[2];
+        Xc[0] = 2 * hx + ((Xc[1] + Xc[2] + Xc[3] + P.parity - 1) & 1);
+        return true;
+    }
+    Xc[0] = b % P.Lc[0];
+    b /= P.Lc[0];
+    Xc[1] = b % P.Lc[1];
+    b /= P.Lc[1];
+    Xc[2] = b % P.Lc[2];
+    Xc[3] = b / P.Lc[2];
+    return P.parity == 0 || ((Xc[0] + Xc[1] + Xc[2] + Xc[3]) & 1) == P.parity - 1;
+}
+
+// local coordinates of local index l (x fastest) and the canonical fine site
+__device__ __forceinline__ int domain_site(const DomParams& P, const int Xc[4], int l, int lx[4]) {
+    int s = 0, stride = 1;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        lx[mu] = l % P.dom[mu];
+        l /= P.dom[mu];
+        s += (Xc[mu] * P.dom[mu] + lx[mu]) * stride;
+        stride *= P.L[mu];
+    }
+    return s;
+}
+
+// Sum of NRED partial sums per thread over the CTA, same bits in every thread; fixed order (warp tree, then warps in
+// index order).  red: shared scratch of (blockDim.x / 32) * NRED values.  Contains one __syncthreads().
+template <int NRED, typename T> __device__ __forceinline__ void cta_sum(T v[NRED], T* red) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+    for (int q = 0; q < NRED; q++) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+        if (lane == 0) red[w * NRED + q] = v[q];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < NRED; q++) {
+        T s = red[q];
+        for (int i = 1; i < nw; i++) s += red[i * NRED + q];
+        v[q] = s;
+    }
+}
+
+// ---- the shared-memory-resident inner-domain solver ------------------------------------------------------
+// One directed hop of D_SAP with every operand in shared memory: rho_s[j][l] vec16 rows of the residual,
+// U_s[row][l] vec16 rows over the 72 reals (mu, 18) of the four forward links of local site l.
+template <int MU, bool FWD, int SGN, typename T>
+__device__ __forceinline__ void hop_smem(T acc[24], const V16<T>* __restrict__ rho_s, const V16<T>* __restrict__ U_s,
+                                         int bv, int l_link, int l_nb, T ph) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+    T p[24], h[12], u[18], g[12];
+#pragma unroll
+    for (int j = 0; j < NJ; j++) {
+        const V16<T> v = rho_s[j * bv + l_nb];
+#pragma unroll
+        for (int q = 0; q < NV; q++) p[j * NV + q] = v.r[q];
+    }
+    constexpr int R0 = 18 * MU / NV, R1 = (18 * MU + 17) / NV;
+#pragma unroll
+    for (int row = R0; row <= R1; row++) {
+        const V16<T> v = U_s[row * bv + l_link];
+#pragma unroll
+        for (int q = 0; q < NV; q++) {
+            const int idx = row * NV + q - 18 * MU;
+            if (idx >= 0 && idx < 18) u[idx] = v.r[q];
+        }
+    }
+    project<MU, SGN, T>(h, p);
+    su3_mult<FWD, T>(g, u, h);
+    reconstruct<MU, SGN, T>(acc, g, ph);
+}
+
+// x (+)= M_SAP^(g) r for one domain per CTA, thread l <-> local site l; ACC: accumulate into x.
+template <typename T, bool ACC>
+__global__ void __launch_bounds__(256, 1)
+    k_mr_domain(T* __restrict__ x, const T* __restrict__ r, const T* __restrict__ U, const T* __restrict__ clover,
+                T kappa, DomParams P, int niter) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, NR = 72 / NV;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int bv = P.bv;
+    V16<T>* rho_s = reinterpret_cast<V16<T>*>(smem_raw);  // [NJ][bv]
+    V16<T>* U_s = rho_s + NJ * bv;                        // [NR][bv]
+    V16<T>* C_s = U_s + NR * bv;                          // [NR][bv]
+    T* red = reinterpret_cast<T*>(C_s + NR * bv);         // [warps][3]
+
+    int Xc[4], lx[4];
+    const bool selected = domain_of_cta(P, blockIdx.x, Xc);
+    const bool active = (int)threadIdx.x < bv;
+    const int l = active ? (int)threadIdx.x : 0;
+    const int s = domain_site(P, Xc, l, lx);
+    if (!selected) {  // only reached without ACC: M^(g) r vanishes outside the group
+        if (active) {
+            T zero[24];
+#pragma unroll
+            for (int q = 0; q < 24; q++) zero[q] = 0;
+            store_spinor<T>(x, s, zero);
+        }
+        return;
+    }
+
+    // ---- stage the domain: residual -> registers + shared, links and clover -> shared (read ONCE from HBM)
+    T rho[24];
+    load_spinor<T, true>(rho, r, s);
+    if (active) {
+        {
+            T ul[72];
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++) load_link<T, false, true>(ul + 18 * mu, U, s, mu);
+#pragma unroll
+            for (int j = 0; j < NR; j++) {
+                V16<T> v;
+#pragma unroll
+                for (int q = 0; q < NV; q++) v.r[q] = ul[j * NV + q];
+                U_s[j * bv + l] = v;
+            }
+        }
+        const T* cbase = clover + ((long long)(s >> 5) * NR * CH + (s & 31)) * NV;
+#pragma unroll
+        for (int j = 0; j < NR; j++) C_s[j * bv + l] = ld16_stream_g64(cbase + (long long)j * CH * NV);
+    }
+
+    // neighbours inside the domain (local index, wrapped) and hop phases: a hop that leaves the domain is cut
+    // (phase 0); in a direction spanned by ONE domain the wrap is the lattice's own and carries bc[mu].
+    int nf[4], nb[4];
+    T pf[4], pb[4];
+    {
+        int ls = 1;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const bool wf = lx[mu] == P.dom[mu] - 1, wb = lx[mu] == 0;
+            nf[mu] = wf ? l - (P.dom[mu] - 1) * ls : l + ls;
+            nb[mu] = wb ? l + (P.dom[mu] - 1) * ls : l - ls;
+            const T wrap = P.multi[mu] ? (T)0 : (T)P.bc[mu];
+            pf[mu] = wf ? wrap : (T)1;
+            pb[mu] = wb ? wrap : (T)1;
+            ls *= P.dom[mu];
+        }
+    }
+
+    T z[24];
+#pragma unroll
+    for (int q = 0; q < 24; q++) z[q] = 0;
+
+    for (int it = 0; it < niter; it++) {
+        if (active) {
+#pragma unroll
+            for (int j = 0; j < NJ; j++) {
+                V16<T> v;
+#pragma unroll
+                for (int q = 0; q < NV; q++) v.r[q] = rho[j * NV + q];
+                rho_s[j * bv + l] = v;
+            }
+        }
+        __syncthreads();
+        // p = D_SAP rho
+        T acc[24];
+#pragma unroll
+        for (int q = 0; q < 24; q++) acc[q] = 0;
+        hop_smem<0, true, -1, T>(acc, rho_s, U_s, bv, l, nf[0], pf[0]);
+        hop_smem<0, false, +1, T>(acc, rho_s, U_s, bv, nb[0], nb[0], pb[0]);
+        hop_smem<1, true, -1, T>(acc, rho_s, U_s, bv, l, nf[1], pf[1]);
+        hop_smem<1, false, +1, T>(acc, rho_s, U_s, bv, nb[1], nb[1], pb[1]);
+        hop_smem<2, true, -1, T>(acc, rho_s, U_s, bv, l, nf[2], pf[2]);
+        hop_smem<2, false, +1, T>(acc, rho_s, U_s, bv, nb[2], nb[2], pb[2]);
+        hop_smem<3, true, -1, T>(acc, rho_s, U_s, bv, l, nf[3], pf[3]);
+        hop_smem<3, false, +1, T>(acc, rho_s, U_s, bv, nb[3], nb[3], pb[3]);
+        T p[24];
+#pragma unroll
+        for (int q = 0; q < 24; q++) p[q] = fma(-kappa, acc[q], rho[q]);
+#pragma unroll
+        for (int chi = 0; chi < 2; chi++) {
+            T cl[36];
+#pragma unroll
+            for (int j = 0; j < 36 / NV; j++) {
+                const V16<T> v = C_s[(chi * (36 / NV) + j) * bv + l];
+#pragma unroll
+                for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
+            }
+            herm6_madd<T>(p + 12 * chi, cl, rho + 12 * chi);
+        }
+        // alpha = <p|rho>_X / <p|p>_X  (blocked dotc)
+        T d[3] = {0, 0, 0};
+        if (active) {
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                d[0] = fma(p[2 * k], rho[2 * k], d[0]);
+                d[0] = fma(p[2 * k + 1], rho[2 * k + 1], d[0]);
+                d[1] = fma(p[2 * k], rho[2 * k + 1], d[1]);
+                d[1] = fma(-p[2 * k + 1], rho[2 * k], d[1]);
+                d[2] = fma(p[2 * k], p[2 * k], d[2]);
+                d[2] = fma(p[2 * k + 1], p[2 * k + 1], d[2]);
+            }
+        }
+        cta_sum<3, T>(d, red);
+        const T ar = d[2] > 0 ? d[0] / d[2] : (T)0, ai = d[2] > 0 ? d[1] / d[2] : (T)0;
+        // z += alpha rho ; rho -= alpha p  (blocked axpy)
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            const T rr = rho[2 * k], ri = rho[2 * k + 1];
+            z[2 * k] = fma(ar, rr, z[2 * k]);
+            z[2 * k] = fma(-ai, ri, z[2 * k]);
+            z[2 * k + 1] = fma(ar, ri, z[2 * k + 1]);
+            z[2 * k + 1] = fma(ai, rr, z[2 * k + 1]);
+            rho[2 * k] = fma(-ar, p[2 * k], rho[2 * k]);
+            rho[2 * k] = fma(ai, p[2 * k + 1], rho[2 * k]);
+            rho[2 * k + 1] = fma(-ar, p[2 * k + 1], rho[2 * k + 1]);
+            rho[2 * k + 1] = fma(-ai, p[2 * k], rho[2 * k + 1]);
+        }
+        // (the barrier inside cta_sum ordered every read of rho_s and red before the next iteration's writes of
+        // rho_s; red is rewritten only after the next __syncthreads)
+    }
+
+    if (active) {
+        if (ACC) {
+            T xo[24];
+            load_spinor<T, true>(xo, x, s);
+#pragma unroll
+            for (int q = 0; q < 24; q++) z[q] += xo[q];
+        }
+        T* base = x + ((long long)(s >> 5) * NJ * CH + (s & 31)) * NV;
+#pragma unroll
+        for (int j = 0; j < NJ; j++) {
+            V16<T> v;
+#pragma unroll
+            for (int q = 0; q < NV; q++) v.r[q] = z[j * NV + q];
+            st16(base + (long long)j * CH * NV, v);
+        }
+    }
+}
+
+// ---- blocked BLAS-1: one CTA per domain, sites strided over the threads ------------------------
+// native spinor row j of site s
+template <typename T> __device__ __forceinline__ const T* srow(const T* f, int s, int j) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+    return f + (((long long)(s >> 5) * NJ + j) * CH + (s & 31)) * NV;
+}
+template <typename T> __device__ __forceinline__ T* srow(T* f, int s, int j) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+    return f + (((long long)(s >> 5) * NJ + j) * CH + (s & 31)) * NV;
+}
+
+// out[X] = <a|b>_X = sum over the sites of domain X of conj(a) b   (complex, interleaved)
+template <typename T>
+__global__ void __launch_bounds__(128) k_block_dotc(T* __restrict__ out, const T* __restrict__ a,
+                                                     const T* __restrict__ b, DomParams P) {
+    __shared__ T red[4 * 2];
+    int Xc[4], lx[4];
+    domain_of_cta(P, blockIdx.x, Xc);
+    T d[2] = {0, 0};
+    for (int l = threadIdx.x; l < P.bv; l += blockDim.x) {
+        const int s = domain_site(P, Xc, l, lx);
+        T va[24], vb[24];
+        load_spinor<T>(va, a, s);
+        load_spinor<T>(vb, b, s);
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            d[0] = fma(va[2 * k], vb[2 * k], d[0]);
+            d[0] = fma(va[2 * k + 1], vb[2 * k + 1], d[0]);
+            d[1] = fma(va[2 * k], vb[2 * k + 1], d[1]);
+            d[1] = fma(-va[2 * k + 1], vb[2 * k], d[1]);
+        }
+    }
+    cta_sum<2, T>(d, red);
+    if (threadIdx.x == 0) {
+        out[2 * blockIdx.x] = d[0];
+        out[2 * blockIdx.x + 1] = d[1];
+    }
+}
+
+// y(x) += coef[X(x)] a(x)
+template <typename T>
+__global__ void __launch_bounds__(128) k_block_caxpy(T* __restrict__ y, const T* __restrict__ coef,
+                                                      const T* __restrict__ a, DomParams P) {
+    int Xc[4], lx[4];
+    domain_of_cta(P, blockIdx.x, Xc);
+    const T cr = coef[2 * blockIdx.x], ci = coef[2 * blockIdx.x + 1];
+    for (int l = threadIdx.x; l < P.bv; l += blockDim.x) {
+        const int s = domain_site(P, Xc, l, lx);
+        T va[24], vy[24];
+        load_spinor<T>(va, a, s);
+        load_spinor<T>(vy, y, s);
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            vy[2 * k] = fma(cr, va[2 * k], vy[2 * k]);
+            vy[2 * k] = fma(-ci, va[2 * k + 1], vy[2 * k]);
+            vy[2 * k + 1] = fma(cr, va[2 * k + 1], vy[2 * k + 1]);
+            vy[2 * k + 1] = fma(ci, va[2 * k], vy[2 * k + 1]);
+        }
+        constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+#pragma unroll
+        for (int j = 0; j < NJ; j++) {
+            V16<T> v;
+#pragma unroll
+            for (int q = 0; q < NV; q++) v.r[q] = vy[j * NV + q];
+            st16(srow(y, s, j), v);
+        }
+    }
+}
+
+// ---- generic inner-domain solver (domains that do not fit in shared memory) ------------------------------------
+// rho = P_g r; z = 0 (when z != nullptr)
+template <typename T>
+__global__ void __launch_bounds__(128) k_mr_init(T* __restrict__ rho, T* __restrict__ z, const T* __restrict__ r,
+                                                  DomParams P) {
+    int Xc[4], lx[4];
+    const bool selected = domain_of_cta(P, blockIdx.x, Xc);
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+    for (int l = threadIdx.x; l < P.bv; l += blockDim.x) {
+        const int s = domain_site(P, Xc, l, lx);
+#pragma unroll
+        for (int j = 0; j < NJ; j++) {
+            V16<T> v = ld16(srow(r, s, j));
+            V16<T> zero;
+#pragma unroll
+            for (int q = 0; q < NV; q++) {
+                zero.r[q] = 0;
+                if (!selected) v.r[q] = 0;
+            }
+            st16(srow(rho, s, j), v);
+            if (z) st16(srow(z, s, j), zero);
+        }
+    }
+}
+
+// one minimal-residual update per domain: alpha = <p|rho>_X / <p|p>_X; z += alpha rho; rho -= alpha p
+template <typename T>
+__global__ void __launch_bounds__(128) k_mr_update(T* __restrict__ z, T* __restrict__ rho, const T* __restrict__ p,
+                                                    DomParams P) {
+    __shared__ T red[4 * 3];
+    int Xc[4], lx[4];
+    if (!domain_of_cta(P, blockIdx.x, Xc)) return;
+    T d[3] = {0, 0, 0};
+    for (int l = threadIdx.x; l < P.bv; l += blockDim.x) {
+        const int s = domain_site(P, Xc, l, lx);
+        T vp[24], vr[24];
+        load_spinor<T>(vp, p, s);
+        load_spinor<T>(vr, rho, s);
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            d[0] = fma(vp[2 * k], vr[2 * k], d[0]);
+            d[0] = fma(vp[2 * k + 1], vr[2 * k + 1], d[0]);
+            d[1] = fma(vp[2 * k], vr[2 * k + 1], d[1]);
+            d[1] = fma(-vp[2 * k + 1], vr[2 * k], d[1]);
+            d[2] = fma(vp[2 * k], vp[2 * k], d[2]);
+            d[2] = fma(vp[2 * k + 1], vp[2 * k + 1], d[2]);
+        }
+    }
+    cta_sum<3, T>(d, red);
+    const T ar = d[2] > 0 ? d[0] / d[2] : (T)0, ai = d[2] > 0 ? d[1] / d[2] : (T)0;
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+    for (int l = threadIdx.x; l < P.bv; l += blockDim.x) {
+        const int s = domain_site(P, Xc, l, lx);
+        T vp[24], vr[24], vz[24];
+        load_spinor<T>(vp, p, s);
+        load_spinor<T>(vr, rho, s);
+        load_spinor<T>(vz, z, s);
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            const T rr = vr[2 * k], ri = vr[2 * k + 1];
+            vz[2 * k] = fma(ar, rr, vz[2 * k]);
+            vz[2 * k] = fma(-ai, ri, vz[2 * k]);
+            vz[2 * k + 1] = fma(ar, ri, vz[2 * k + 1]);
+            vz[2 * k + 1] = fma(ai, rr, vz[2 * k + 1]);
+            vr[2 * k] = fma(-ar, vp[2 * k], vr[2 * k]);
+            vr[2 * k] = fma(ai, vp[2 * k + 1], vr[2 * k]);
+            vr[2 * k + 1] = fma(-ar, vp[2 * k + 1], vr[2 * k + 1]);
+            vr[2 * k + 1] = fma(-ai, vp[2 * k], vr[2 * k + 1]);
+        }
+#pragma unroll
+        for (int j = 0; j < NJ; j++) {
+            V16<T> a, b;
+#pragma unroll
+            for (int q = 0; q < NV; q++) {
+                a.r[q] = vz[j * NV + q];
+                b.r[q] = vr[j * NV + q];
+            }
+            st16(srow(z, s, j), a);
+            st16(srow(rho, s, j), b);
+        }
+    }
+}
+
+// ---- host side ----------------------------------------------------------------------------------------------------
+static int dom_setup(DomParams& P, const int dims[4], const int bc[4], const int domain[4], const char* what) {
+    if (check_dims(dims) || !domain) {
+        set_error("%s: null or non-positive dims/domain", what);
+        return LQCD_EINVAL;
+    }
+    if (volume(dims) > 0x7fffffffLL) {
+        set_error("%s: volume exceeds 2^31-1 sites", what);
+        return LQCD_EUNSUPPORTED;
+    }
+    P.bv = 1;
+    P.Vc = 1;
+    for (int mu = 0; mu < 4; mu++) {
+        if (domain[mu] < 1 || dims[mu] % domain[mu]) {
+            set_error("%s: domain[%d] = %d does not divide dims[%d] = %d", what, mu, domain[mu], mu, dims[mu]);
+            return LQCD_EINVAL;
+        }
+        if (bc && bc[mu] != 1 && bc[mu] != -1) {
+            set_error("%s: bc[%d] = %d not in {+1,-1}", what, mu, bc[mu]);
+            return LQCD_EINVAL;
+        }
+        P.L[mu] = dims[mu];
+        P.dom[mu] = domain[mu];
+        P.Lc[mu] = dims[mu] / domain[mu];
+        P.bc[mu] = bc ? bc[mu] : 1;
+        P.multi[mu] = P.Lc[mu] > 1;
+        P.bv *= domain[mu];
+        P.Vc *= P.Lc[mu];
+    }
+    P.parity = 0;
+    P.halfgrid = 0;
+    return LQCD_OK;
+}
+
+template <typename T> static size_t mr_smem_bytes(int bv) {
+    return (size_t)bv * (24 + 72 + 72) * sizeof(T) + 8 * 3 * sizeof(T);
+}
+
+static int max_optin_smem() {
+    static int v = -1;
+    if (v < 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) v = 0;
+        cudaGetLastError();
+    }
+    return v;
+}
+
+template <typename T> static bool mr_fits_smem(int bv) {
+    return g_knobs.sap_fused >= 0 && bv <= 256 && mr_smem_bytes<T>(bv) <= (size_t)max_optin_smem();
+}
+
+// z (+)= M_SAP^(g) r.  ws: two native spinors of scratch (rho, p) when the generic path is taken.
+template <typename T>
+static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa, const int dims[4], const int bc[4],
+                          const int domain[4], unsigned flags, int niter, void* ws, void* stream, const char* what) {
+    clear_error();
+    if (!z || !r || !U || !clover || !bc) {
+        set_error("%s: null pointer", what);
+        return LQCD_EINVAL;
+    }
+    if (!aligned16(z) || !aligned16(r) || !aligned16(U) || !aligned16(clover) || !aligned16(ws)) {
+        set_error("%s: pointers must be 16-byte aligned", what);
+        return LQCD_EINVAL;
+    }
+    if (z == r) {
+        set_error("%s: z must not alias r", what);
+        return LQCD_EINVAL;
+    }
+    if ((flags & ~(LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD | LQCD_ACCUMULATE)) ||
+        ((flags & LQCD_DOMAIN_EVEN) && (flags & LQCD_DOMAIN_ODD)) || niter < 0) {
+        set_error("%s: bad flags 0x%x or niter %d", what, flags, niter);
+        return LQCD_EINVAL;
+    }
+    DomParams P;
+    int rc = dom_setup(P, dims, bc, domain, what);
+    if (rc) return rc;
+    P.parity = (flags & LQCD_DOMAIN_EVEN) ? 1 : (flags & LQCD_DOMAIN_ODD) ? 2 : 0;
+    const bool acc = flags & LQCD_ACCUMULATE;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    if (mr_fits_smem<T>(P.bv)) {
+        const size_t smem = mr_smem_bytes<T>(P.bv);
+        const int threads = (P.bv + 31) / 32 * 32;
+        unsigned grid = (unsigned)P.Vc;
+        if (acc && P.parity != 0 && P.Lc[0] % 2 == 0) {  // no CTA for the domains of the other group
+            P.halfgrid = 1;
+            grid = (unsigned)(P.Vc / 2);
+        }
+        if (acc) {
+            static bool attr = false;
+            if (!attr) {
+                cudaFuncSetAttribute(k_mr_domain<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     max_optin_smem());
+                attr = true;
+            }
+            k_mr_domain<T, true><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter);
+        } else {
+            static bool attr = false;
+            if (!attr) {
+                cudaFuncSetAttribute(k_mr_domain<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     max_optin_smem());
+                attr = true;
+            }
+            k_mr_domain<T, false><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter);
+        }
+        count_launch();
+        return check_launch(what);
+    }
+
+    // generic path
+    if (!ws) {
+        set_error("%s: this domain size needs the workspace of lqcd_mr_workspace_bytes()", what);
+        return LQCD_EINVAL;
+    }
+    const size_t nreal = (size_t)nchunks(dims) * CH * 24;
+    T* rho = reinterpret_cast<T*>(ws);
+    T* p = rho + nreal;
+    k_mr_init<T><<<(unsigned)P.Vc, 128, 0, st>>>(rho, acc ? nullptr : z, r, P);
+    count_launch();
+    const unsigned ddflags = flags & (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD);
+    for (int it = 0; it < niter; it++) {
+        rc = wilson_clover_call<T>(p, rho, U, clover, nullptr, kappa, dims, bc, domain, ddflags, stream, what);
+        if (rc) return rc;
+        k_mr_update<T><<<(unsigned)P.Vc, 128, 0, st>>>(z, rho, p, P);
+        count_launch();
+    }
+    return check_launch(what);
+}
+
+// SAP with fixed iterations.  x: solution; r: scratch, receives the residual; b: right-hand side.
+template <typename T>
+static int sap_call(T* x, T* r, const T* b, const T* U, const T* clover, T kappa, const int dims[4], const int bc[4],
+                    const int domain[4], int n_sap, int n_mr, unsigned flags, void* ws, void* stream,
+                    const char* what) {
+    clear_error();
+    if (!x || !r || !b || !U || !clover || !bc || check_dims(dims) || !domain) {
+        set_error("%s: null pointer or non-positive dim", what);
+        return LQCD_EINVAL;
+    }
+    if (x == r || x == b || r == b) {
+        set_error("%s: x, r and b must be distinct", what);
+        return LQCD_EINVAL;
+    }
+    if ((flags & ~(LQCD_SAP_INITIAL_GUESS | LQCD_SAP_NO_FINAL_RESIDUAL)) || n_sap < 0 || n_mr < 0) {
+        set_error("%s: bad flags 0x%x, n_sap %d or n_mr %d", what, flags, n_sap, n_mr);
+        return LQCD_EINVAL;
+    }
+    {  // validate everything before the first enqueue ("nothing enqueued on error")
+        DomParams P;
+        int rc = dom_setup(P, dims, bc, domain, what);
+        if (rc) return rc;
+        if (!aligned16(x) || !aligned16(r) || !aligned16(b) || !aligned16(U) || !aligned16(clover) || !aligned16(ws)) {
+            set_error("%s: pointers must be 16-byte aligned", what);
+            return LQCD_EINVAL;
+        }
+        if (!mr_fits_smem<T>(P.bv) && !ws) {
+            set_error("%s: this domain size needs the workspace of lqcd_mr_workspace_bytes()", what);
+            return LQCD_EINVAL;
+        }
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)nchunks(dims) * CH * 24 * sizeof(T);
+    int rc;
+    const T* res = r;
+    if (flags & LQCD_SAP_INITIAL_GUESS) {  // |r> := |b> - D|x>
+        rc = wilson_clover_call<T>(r, x, U, clover, b, kappa, dims, bc, nullptr, 0, stream, what);
+        if (rc) return rc;
+    } else {  // |x> := 0, |r> := |b>: the first half sweep reads b itself
+        if (cudaMemsetAsync(x, 0, bytes, st) != cudaSuccess) return check_launch(what);
+        res = b;
+        if (n_sap == 0 && !(flags & LQCD_SAP_NO_FINAL_RESIDUAL))
+            if (cudaMemcpyAsync(r, b, bytes, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return check_launch(what);
+    }
+    for (int i = 0; i < n_sap; i++)
+        for (int g = 0; g < 2; g++) {
+            // |x> := |x> + M_SAP^(e/o)|r>
+            rc = mr_domain_call<T>(x, res, U, clover, kappa, dims, bc, domain,
+                                   (g == 0 ? LQCD_DOMAIN_EVEN : LQCD_DOMAIN_ODD) | LQCD_ACCUMULATE, n_mr, ws, stream,
+                                   what);
+            if (rc) return rc;
+            const bool last = (i == n_sap - 1 && g == 1);
+            if (last && (flags & LQCD_SAP_NO_FINAL_RESIDUAL)) break;
+            // |r> := |b> - D|x>
+            rc = wilson_clover_call<T>(r, x, U, clover, b, kappa, dims, bc, nullptr, 0, stream, what);
+            if (rc) return rc;
+            res = r;
+        }
+    return LQCD_OK;
+}
+
+template <typename T>
+static int block_blas_call(int which, T* out, const T* a, const T* b, const int dims[4], const int domain[4],
+                           void* stream, const char* what) {
+    clear_error();
+    if (!out || !a || !b) {
+        set_error("%s: null pointer", what);
+        return LQCD_EINVAL;
+    }
+    if (!aligned16(a) || !aligned16(b) || (which == 1 && !aligned16(out))) {
+        set_error("%s: spinor pointers must be 16-byte aligned", what);
+        return LQCD_EINVAL;
+    }
+    DomParams P;
+    int rc = dom_setup(P, dims, nullptr, domain, what);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (which == 0) k_block_dotc<T><<<(unsigned)P.Vc, 128, 0, st>>>(out, a, b, P);
+    else k_block_caxpy<T><<<(unsigned)P.Vc, 128, 0, st>>>(out, a, b, P);
+    count_launch();
+    return check_launch(what);
+}
+
+}  // namespace lqcd
+
+using namespace lqcd;
+
+extern "C" {
+
+size_t lqcd_mr_workspace_bytes(const int dims[4], const int domain[4], int real_bytes) {
+    DomParams P;
+    if (dom_setup(P, dims, nullptr, domain, "lqcd_mr_workspace_bytes")) return 0;
+    if (real_bytes != 4 && real_bytes != 8) return 0;
+    const bool fits = real_bytes == 4 ? mr_fits_smem<float>(P.bv) : mr_fits_smem<double>(P.bv);
+    return fits ? 0 : 2 * (size_t)nchunks(dims) * CH * 24 * (size_t)real_bytes;
+}
+
+int lqcd_block_dotc_f32(float* out, const float* a, const float* b, const int dims[4], const int domain[4],
+                        void* stream) {
+    return block_blas_call<float>(0, out, a, b, dims, domain, stream, "lqcd_block_dotc_f32");
+}
+int lqcd_block_dotc_f64(double* out, const double* a, const double* b, const int dims[4], const int domain[4],
+                        void* stream) {
+    return block_blas_call<double>(0, out, a, b, dims, domain, stream, "lqcd_block_dotc_f64");
+}
+int lqcd_block_caxpy_f32(float* y, const float* coef, const float* a, const int dims[4], const int domain[4],
+                         void* stream) {
+    return block_blas_call<float>(1, y, coef, a, dims, domain, stream, "lqcd_block_caxpy_f32");
+}
+int lqcd_block_caxpy_f64(double* y, const double* coef, const double* a, const int dims[4], const int domain[4],
+                         void* stream) {
+    return block_blas_call<double>(1, y, coef, a, dims, domain, stream, "lqcd_block_caxpy_f64");
+}
+
+int lqcd_mr_domain_solve_f32(float* z, const float* r, const float* U, const float* clover, float kappa,
+                             const int dims[4], const int bc[4], const int domain[4], unsigned flags, int niter,
+                             void* ws_dev, void* stream) {
+    return mr_domain_call<float>(z, r, U, clover, kappa, dims, bc, domain, flags, niter, ws_dev, stream,
+                                 "lqcd_mr_domain_solve_f32");
+}
+int lqcd_mr_domain_solve_f64(double* z, const double* r, const double* U, const double* clover, double kappa,
+                             const int dims[4], const int bc[4], const int domain[4], unsigned flags, int niter,
+                             void* ws_dev, void* stream) {
+    return mr_domain_call<double>(z, r, U, clover, kappa, dims, bc, domain, flags, niter, ws_dev, stream,
+                                  "lqcd_mr_domain_solve_f64");
+}
+
+int lqcd_sap_f32(float* x, float* r, const float* b, const float* U, const float* clover, float kappa,
+                 const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
+                 void* ws_dev, void* stream) {
+    return sap_call<float>(x, r, b, U, clover, kappa, dims, bc, domain, n_sap, n_mr, flags, ws_dev, stream,
+                           "lqcd_sap_f32");
+}
+int lqcd_sap_f64(double* x, double* r, const double* b, const double* U, const double* clover, double kappa,
+                 const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
+                 void* ws_dev, void* stream) {
+    return sap_call<double>(x, r, b, U, clover, kappa, dims, bc, domain, n_sap, n_mr, flags, ws_dev, stream,
+                            "lqcd_sap_f64");
+}
+}

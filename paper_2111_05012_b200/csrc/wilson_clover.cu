@@ -45,55 +45,15 @@ __device__ __forceinline__ void hop(T acc[24], const T* __restrict__ in, const T
     reconstruct<MU, SGN, T>(acc, g, ph);
 }
 
-// out6 += Hermitian 6x6 block (36 reals: 6 diagonal, 15 complex strictly-lower row-major) times in6
-template <typename T> __device__ __forceinline__ void herm6_madd(T out[12], const T cl[36], const T in[12]) {
-#pragma unroll
-    for (int k = 0; k < 6; k++) {
-        T sr = fma(cl[k], in[2 * k], out[2 * k]);
-        T si = fma(cl[k], in[2 * k + 1], out[2 * k + 1]);
-#pragma unroll
-        for (int l = 0; l < 6; l++) {
-            if (l == k) continue;
-            const T xr = in[2 * l], xi = in[2 * l + 1];
-            if (l < k) {  // L_kl
-                const T ar = cl[6 + 2 * tri(k, l)], ai = cl[6 + 2 * tri(k, l) + 1];
-                sr = fma(ar, xr, sr);
-                sr = fma(-ai, xi, sr);
-                si = fma(ar, xi, si);
-                si = fma(ai, xr, si);
-            } else {  // conj(L_lk)
-                const T ar = cl[6 + 2 * tri(l, k)], ai = cl[6 + 2 * tri(l, k) + 1];
-                sr = fma(ar, xr, sr);
-                sr = fma(ai, xi, sr);
-                si = fma(ar, xi, si);
-                si = fma(-ai, xr, si);
-            }
-        }
-        out[2 * k] = sr;
-        out[2 * k + 1] = si;
-    }
-}
-
-template <typename T, bool G64 = false>
-__device__ __forceinline__ void load_clover_block(T cl[36], const T* __restrict__ C, int s, int chi) {
-    constexpr int NV = VecOf<T>::NV, NJ = 72 / NV;
-    const T* base = C + (((long long)(s >> 5) * NJ + chi * (36 / NV)) * CH + (s & 31)) * NV;
-#pragma unroll
-    for (int j = 0; j < 36 / NV; j++) {
-        V16<T> v = G64 ? ld16_stream_g64(base + (long long)j * CH * NV) : ld16_stream(base + (long long)j * CH * NV);
-#pragma unroll
-        for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
-    }
-}
-
 // DD: the domain-decomposed operator D_SAP -- hops whose two ends lie in different domains are switched off
 // (no load is issued for them), and with P.parity != 0 only the sites of even (odd) domains are computed, the
 // others are set to zero (D_SAP^(e/o) = P_e/o D_SAP P_e/o).
 // DD = 2: the even/odd mode; active data then comes in alternate 64-byte half lines -> 64-byte L2 granularity.
-template <typename T, bool DAG, bool L12, int DD, int MAXTHREADS, int MINBLOCKS>
+// RES: the Richardson residual out = rhs - D in in the same pass: one more streamed read.
+template <typename T, bool DAG, bool L12, int DD, bool RES, int MAXTHREADS, int MINBLOCKS>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
     k_wilson_clover(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ U, const T* __restrict__ clover,
-                    T kappa, FineParams P) {
+                    const T* __restrict__ rhs, T kappa, FineParams P) {
     // ---- which site is mine: CTA -> tile (x tiles fastest; optionally z-slabbed traversal), thread -> site in tile
     // (all divisions by run-time extents are multiply-high with host-computed reciprocals: the index decode was a
     // quarter of the integer work of this kernel)
@@ -200,6 +160,16 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
         load_clover_block<T, (DD == 2)>(cl, clover, s, chi);
         herm6_madd<T>(o + 12 * chi, cl, p + 12 * chi);
     }
+    if (RES) {
+        constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+        const T* base = rhs + ((long long)(s >> 5) * NJ * CH + (s & 31)) * NV;
+#pragma unroll
+        for (int j = 0; j < NJ; j++) {
+            const V16<T> v = ld16_stream(base + (long long)j * CH * NV);
+#pragma unroll
+            for (int q = 0; q < NV; q++) o[j * NV + q] = v.r[q] - o[j * NV + q];
+        }
+    }
     store_spinor<T>(out, s, o);
 }
 
@@ -224,8 +194,8 @@ static void auto_tile(const int L[4], int tile[4]) {
 
 // domain == NULL: the plain operator D; otherwise D_SAP with those domains
 template <typename T>
-static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4],
-                              const int bc[4], const int* domain, unsigned flags, void* stream, const char* what) {
+int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
+                       const int bc[4], const int* domain, unsigned flags, void* stream, const char* what) {
     clear_error();
     if (!out || !in || !U || !clover || check_dims(dims) || !bc) {
         set_error("%s: null pointer or non-positive dim", what);
@@ -237,6 +207,10 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
     }
     if (out == in) {
         set_error("%s: out must not alias in", what);
+        return LQCD_EINVAL;
+    }
+    if (rhs && (!aligned16(rhs) || domain || (flags & LQCD_DAGGER))) {
+        set_error("%s: the residual form needs an aligned rhs and takes neither a domain nor LQCD_DAGGER", what);
         return LQCD_EINVAL;
     }
     const unsigned allowed = LQCD_DAGGER | LQCD_LINKS_12 | (domain ? (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD) : 0u);
@@ -326,30 +300,38 @@ static int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, 
     cudaStream_t st = (cudaStream_t)stream;
     const unsigned grid = (unsigned)ntiles;
     // registers per thread: fp32 128 (4 CTAs/SM), fp64 168 (3 CTAs/SM) -- measured best on B200
-#define LAUNCH(DAG, L12, DD)                                                                                 \
+#define LAUNCH_R(DAG, L12, DD, RES)                                                                          \
     do {                                                                                                     \
         if (threads <= 128)                                                                                  \
-            k_wilson_clover<T, DAG, L12, DD, 128, (sizeof(T) == 4 ? 4 : 3)>                                  \
-                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                    \
+            k_wilson_clover<T, DAG, L12, DD, RES, 128, (sizeof(T) == 4 ? 4 : 3)>                             \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);                               \
         else                                                                                                 \
-            k_wilson_clover<T, DAG, L12, DD, 256, (sizeof(T) == 4 ? 2 : 1)>                                  \
-                <<<grid, threads, 0, st>>>(out, in, U, clover, kappa, P);                                    \
+            k_wilson_clover<T, DAG, L12, DD, RES, 256, (sizeof(T) == 4 ? 2 : 1)>                             \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);                               \
     } while (0)
+#define LAUNCH(DAG, L12, DD) LAUNCH_R(DAG, L12, DD, false)
 #define LAUNCH_DD(DAG, L12)                                                                                  \
     do {                                                                                                     \
         if (domain && P.parity != 0) LAUNCH(DAG, L12, 2);                                                    \
         else if (domain) LAUNCH(DAG, L12, 1);                                                                \
         else LAUNCH(DAG, L12, 0);                                                                            \
     } while (0)
-    if (dag && l12) LAUNCH_DD(true, true);
+    if (rhs && l12) LAUNCH_R(false, true, 0, true);
+    else if (rhs) LAUNCH_R(false, false, 0, true);
+    else if (dag && l12) LAUNCH_DD(true, true);
     else if (dag) LAUNCH_DD(true, false);
     else if (l12) LAUNCH_DD(false, true);
     else LAUNCH_DD(false, false);
 #undef LAUNCH_DD
 #undef LAUNCH
+#undef LAUNCH_R
     count_launch();
     return check_launch(what);
 }
+template int wilson_clover_call<float>(float*, const float*, const float*, const float*, const float*, float,
+                                       const int*, const int*, const int*, unsigned, void*, const char*);
+template int wilson_clover_call<double>(double*, const double*, const double*, const double*, const double*, double,
+                                        const int*, const int*, const int*, unsigned, void*, const char*);
 
 }  // namespace lqcd
 
@@ -358,12 +340,12 @@ using namespace lqcd;
 extern "C" {
 int lqcd_wilson_clover_mult_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
                                 const int dims[4], const int bc[4], unsigned flags, void* stream) {
-    return wilson_clover_call<float>(out, in, U, clover, kappa, dims, bc, nullptr, flags, stream,
+    return wilson_clover_call<float>(out, in, U, clover, nullptr, kappa, dims, bc, nullptr, flags, stream,
                                      "lqcd_wilson_clover_mult_f32");
 }
 int lqcd_wilson_clover_mult_f64(double* out, const double* in, const double* U, const double* clover, double kappa,
                                 const int dims[4], const int bc[4], unsigned flags, void* stream) {
-    return wilson_clover_call<double>(out, in, U, clover, kappa, dims, bc, nullptr, flags, stream,
+    return wilson_clover_call<double>(out, in, U, clover, nullptr, kappa, dims, bc, nullptr, flags, stream,
                                       "lqcd_wilson_clover_mult_f64");
 }
 int lqcd_wilson_clover_dd_mult_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
@@ -373,7 +355,7 @@ int lqcd_wilson_clover_dd_mult_f32(float* out, const float* in, const float* U, 
         set_error("lqcd_wilson_clover_dd_mult_f32: null domain");
         return LQCD_EINVAL;
     }
-    return wilson_clover_call<float>(out, in, U, clover, kappa, dims, bc, domain, flags, stream,
+    return wilson_clover_call<float>(out, in, U, clover, nullptr, kappa, dims, bc, domain, flags, stream,
                                      "lqcd_wilson_clover_dd_mult_f32");
 }
 int lqcd_wilson_clover_dd_mult_f64(double* out, const double* in, const double* U, const double* clover, double kappa,
@@ -383,7 +365,29 @@ int lqcd_wilson_clover_dd_mult_f64(double* out, const double* in, const double* 
         set_error("lqcd_wilson_clover_dd_mult_f64: null domain");
         return LQCD_EINVAL;
     }
-    return wilson_clover_call<double>(out, in, U, clover, kappa, dims, bc, domain, flags, stream,
+    return wilson_clover_call<double>(out, in, U, clover, nullptr, kappa, dims, bc, domain, flags, stream,
                                       "lqcd_wilson_clover_dd_mult_f64");
+}
+}
+
+extern "C" {
+int lqcd_wilson_clover_residual_f32(float* r, const float* b, const float* x, const float* U, const float* clover,
+                                    float kappa, const int dims[4], const int bc[4], unsigned flags, void* stream) {
+    if (!b) {
+        set_error("lqcd_wilson_clover_residual_f32: null rhs");
+        return LQCD_EINVAL;
+    }
+    return wilson_clover_call<float>(r, x, U, clover, b, kappa, dims, bc, nullptr, flags, stream,
+                                     "lqcd_wilson_clover_residual_f32");
+}
+int lqcd_wilson_clover_residual_f64(double* r, const double* b, const double* x, const double* U,
+                                    const double* clover, double kappa, const int dims[4], const int bc[4],
+                                    unsigned flags, void* stream) {
+    if (!b) {
+        set_error("lqcd_wilson_clover_residual_f64: null rhs");
+        return LQCD_EINVAL;
+    }
+    return wilson_clover_call<double>(r, x, U, clover, b, kappa, dims, bc, nullptr, flags, stream,
+                                      "lqcd_wilson_clover_residual_f64");
 }
 }

@@ -1,0 +1,254 @@
+"""F3 on the GPU against the oracle (-m gpu): Richardson residual, blocked BLAS-1, the inner-domain minimal-residual
+solver M_SAP^(e/o) and the SAP listing, through the C ABI.
+
+Bars.  A single operator application keeps the north_star bars (1e-12 fp64, 2e-6 fp32).  The iterations chain
+applications with fixed counts; their rounding errors add at most linearly (the minimal-residual coefficient is a
+ratio of two sums over the same data, so its relative perturbation is that of p = D_SAP rho), hence
+  mr_domain_solve(n_mr):  n_mr x the single-application bar,
+  sap(n_sap, n_mr):       2 n_sap (n_mr + 1) x the single-application bar
+(DESIGN.md section 6.6).  Both code paths of the solver (shared-memory-resident and generic) are held to them.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from problems import config_problem, custom_config, make_problem, rel_l2
+from test_gpu_parity import CDT, Dev, rounded, to_dev
+
+pytestmark = pytest.mark.gpu
+
+TOL1 = {"f64": 1e-12, "f32": 2e-6}
+
+
+@pytest.fixture(scope="module")
+def lq():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_2111_05012_b200 as lq
+    return lq
+
+
+@pytest.fixture(params=[0, -1], ids=["resident", "generic"])
+def path(lq, request):
+    """both implementations of the inner-domain solver"""
+    lq.set_knob("sap_fused", request.param)
+    yield request.param
+    lq.set_knob("sap_fused", 0)
+
+
+def fields(prob, prec):
+    return rounded(prob.U, prec), rounded(prob.clover, prec)
+
+
+def rdtype(lq, prec):
+    import torch
+    return torch.float32 if prec == "f32" else torch.float64
+
+
+def gpu_mr(lq, d, r, domain, parity, niter, accumulate_into=None):
+    import torch
+    cfg = d.cfg
+    rn = lq.pack_spinor(to_dev(r, d.prec), cfg.dims)
+    ws = lq.mr_workspace(cfg.dims, domain, dtype=rdtype(lq, d.prec))
+    if accumulate_into is None:
+        z = lq.empty_spinor(cfg.dims, dtype=rn.dtype)
+        z.fill_(5.0)  # must be overwritten everywhere
+        lq.mr_domain_solve(z, rn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, domain, parity=parity, niter=niter, ws=ws)
+    else:
+        z = lq.pack_spinor(to_dev(accumulate_into, d.prec), cfg.dims)
+        lq.mr_domain_solve(z, rn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, domain, parity=parity, niter=niter,
+                           accumulate=True, ws=ws)
+    torch.cuda.synchronize()
+    return lq.unpack_spinor(z, cfg.dims).cpu().numpy()
+
+
+def gpu_sap(lq, d, b, domain, n_sap, n_mr, x0=None, final_residual=True):
+    cfg = d.cfg
+    bn = lq.pack_spinor(to_dev(b, d.prec), cfg.dims)
+    x = lq.empty_spinor(cfg.dims, dtype=bn.dtype) if x0 is None else lq.pack_spinor(to_dev(x0, d.prec), cfg.dims)
+    if x0 is None:
+        x.fill_(3.0)
+    r = lq.empty_spinor(cfg.dims, dtype=bn.dtype)
+    ws = lq.mr_workspace(cfg.dims, domain, dtype=rdtype(lq, d.prec))
+    lq.sap(x, r, bn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, domain, n_sap=n_sap, n_mr=n_mr,
+           initial_guess=x0 is not None, final_residual=final_residual, ws=ws)
+    return lq.unpack_spinor(x, cfg.dims).cpu().numpy(), lq.unpack_spinor(r, cfg.dims).cpu().numpy()
+
+
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("links12", [False, True])
+def test_residual(lq, prec, links12):
+    prob = config_problem("c1", 2)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec, links12=links12, coarse=False)
+    b, x = prob.psi
+    bn, xn = (lq.pack_spinor(to_dev(a, prec), cfg.dims) for a in (b, x))
+    r = lq.empty_spinor(cfg.dims, dtype=bn.dtype)
+    lq.wilson_clover_residual(r, bn, xn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, links12=links12)
+    U, clov = fields(prob, prec)
+    ref = rounded(b, prec) - oracle.wilson_clover_mult(rounded(x, prec), U, clov, cfg.kappa, cfg.dims, cfg.bc)
+    assert rel_l2(lq.unpack_spinor(r, cfg.dims).cpu().numpy(), ref) <= TOL1[prec]
+    # r may alias b
+    lq.wilson_clover_residual(bn, bn, xn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, links12=links12)
+    assert rel_l2(lq.unpack_spinor(bn, cfg.dims).cpu().numpy(), ref) <= TOL1[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,domain", [
+    ((4, 4, 4, 4), (2, 2, 2, 2)),
+    ((8, 8, 8, 8), (4, 4, 4, 4)),
+    ((6, 4, 2, 10), (3, 4, 1, 5)),
+    ((3, 3, 3, 3), (3, 1, 3, 1)),     # V = 81: ragged chunk
+    ((16, 8, 8, 8), (8, 4, 4, 4)),    # the paper's 8x4x4x4: 512 sites per domain
+    ((4, 4, 4, 4), (4, 4, 4, 4)),     # one domain: the global dotc / axpy
+])
+def test_block_blas(lq, prec, dims, domain):
+    import torch
+    rng = np.random.default_rng(5)
+    V = int(np.prod(dims))
+    a, b = (rounded(rng.standard_normal((V, 4, 3)) + 1j * rng.standard_normal((V, 4, 3)), prec) for _ in range(2))
+    an, bn = (lq.pack_spinor(to_dev(v, prec), dims) for v in (a, b))
+    got = lq.block_dotc(an, bn, dims, domain).cpu().numpy()
+    ref = oracle.block_dotc(a, b, dims, domain)
+    # a dot product is compared on the scale of its terms: |<a|b>_X| <= |a|_X |b|_X
+    scale = np.sqrt(oracle.block_dotc(a, a, dims, domain).real * oracle.block_dotc(b, b, dims, domain).real)
+    assert np.max(np.abs(got - ref) / scale) <= TOL1[prec]
+    nd = ref.size
+    coef = rounded(rng.standard_normal(nd) + 1j * rng.standard_normal(nd), prec)
+    lq.block_caxpy(bn, to_dev(coef, prec), an, dims, domain)
+    assert rel_l2(lq.unpack_spinor(bn, dims).cpu().numpy(), oracle.block_caxpy(b, coef, a, dims, domain)) <= TOL1[prec]
+    torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_c1_mr_domain_solve(lq, prec, path):
+    prob = config_problem("c1", 2)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec, coarse=False)
+    U, clov = fields(prob, prec)
+    r, y = prob.psi
+    for parity in (0, 1, 2):
+        for niter in (0, 1, 6):
+            ref = oracle.mr_domain_solve(rounded(r, prec), U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block, parity,
+                                         niter)
+            got = gpu_mr(lq, d, r, cfg.block, parity, niter)
+            if niter == 0:
+                assert np.all(got == 0)
+                continue
+            assert rel_l2(got, ref) <= niter * TOL1[prec], (parity, niter)
+            assert np.array_equal(got == 0, ref == 0), "exact zeros outside the selected group"
+    # accumulate: y + M^(e) r, sites of odd domains untouched (bit for bit)
+    ref = rounded(y, prec) + oracle.mr_domain_solve(rounded(r, prec), U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block,
+                                                    1, 6)
+    got = gpu_mr(lq, d, r, cfg.block, 1, 6, accumulate_into=y)
+    assert rel_l2(got, ref) <= 6 * TOL1[prec]
+    untouched = oracle.mr_domain_solve(rounded(r, prec), U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block, 1, 1) == 0
+    assert np.array_equal(got[untouched], rounded(y, prec)[untouched])
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,domain,bc", [
+    ((8, 8, 8, 8), (4, 4, 4, 4), (1, 1, 1, -1)),       # config 2's lattice, the paper's typical 4^4 domain
+    ((16, 8, 8, 8), (8, 4, 4, 4), (1, 1, 1, -1)),      # 8x4x4x4: generic path in both precisions
+    ((6, 4, 2, 10), (3, 4, 1, 5), (-1, 1, -1, 1)),     # 60-site domains, single domain in y (wrap with bc), odd Lc[0]
+    ((3, 3, 3, 3), (3, 1, 3, 1), (1, 1, 1, -1)),       # V = 81, 9-site domains, 9 domains (odd count)
+    ((4, 4, 4, 8), (4, 4, 4, 8), (1, 1, 1, -1)),       # ONE domain: global minimal residual on D itself
+])
+def test_mr_edge_lattices(lq, prec, dims, domain, bc, path):
+    cfg = custom_config(dims, (1, 1, 1, 1), 1, bc=bc)
+    prob = make_problem(cfg, coarse="none")
+    if np.prod(domain) >= 512 and path == -1 and prec == "f64":
+        pytest.skip("same path as the resident parametrisation")
+    d = Dev(lq, prob, prec, coarse=False)
+    U, clov = fields(prob, prec)
+    r = prob.psi[0]
+    for parity in (0, 1, 2):
+        ref = oracle.mr_domain_solve(rounded(r, prec), U, clov, cfg.kappa, dims, bc, domain, parity, 6)
+        got = gpu_mr(lq, d, r, domain, parity, 6)
+        if not np.any(ref):  # e.g. odd group of a single-domain lattice
+            assert not np.any(got)
+            continue
+        assert rel_l2(got, ref) <= 6 * TOL1[prec], parity
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_c1_sap(lq, prec, path):
+    """config 1 with the paper's parameters n = 4, 6 inner iterations"""
+    prob = config_problem("c1", 2)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec, coarse=False)
+    U, clov = fields(prob, prec)
+    b, x0 = prob.psi
+    bar = 2 * 4 * 7 * TOL1[prec]
+    rx, rr = oracle.sap(rounded(b, prec), U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=4, n_mr=6)
+    gx, gr = gpu_sap(lq, d, b, cfg.block, 4, 6)
+    assert rel_l2(gx, rx) <= bar
+    assert np.linalg.norm(gr - rr) / np.linalg.norm(rounded(b, prec)) <= bar  # the residual on the scale of b
+    assert np.linalg.norm(gr) < 0.05 * np.linalg.norm(b), "SAP(4) reduces the residual as in the oracle pin"
+    # without the final residual the solution is the same, bit for bit
+    gx2, _ = gpu_sap(lq, d, b, cfg.block, 4, 6, final_residual=False)
+    assert np.array_equal(gx, gx2)
+    # with an initial guess: x0 + SAP(b - D x0), i.e. the Richardson refinement with M_2 = SAP
+    x0 = 0.1 * rounded(x0, prec)
+    r0 = rounded(b, prec) - oracle.wilson_clover_mult(x0, U, clov, cfg.kappa, cfg.dims, cfg.bc)
+    sx, sr = oracle.sap(r0, U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=3)
+    gx, gr = gpu_sap(lq, d, b, cfg.block, 2, 3, x0=x0)
+    assert rel_l2(gx, x0 + sx) <= bar
+    assert np.linalg.norm(gr - sr) / np.linalg.norm(rounded(b, prec)) <= bar
+    # n_sap = 0: x = 0, r = b
+    gx, gr = gpu_sap(lq, d, b, cfg.block, 0, 6)
+    assert not np.any(gx) and np.array_equal(gr, rounded(b, prec))
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_c2_lattice_sap(lq, prec):
+    """8^4 with 4^4 domains: fp32 takes the shared-memory-resident kernel at its design size (256 sites, 168 KB),
+    fp64 does not fit and takes the generic path."""
+    cfg = custom_config((8, 8, 8, 8), (4, 4, 4, 4), 1, gauge="exp", eps=0.5, kappa=0.135, csw=1.0)
+    prob = make_problem(cfg, coarse="none")
+    d = Dev(lq, prob, prec, coarse=False)
+    nbytes = lq.lib().lqcd_mr_workspace_bytes(lq._i4(cfg.dims), lq._i4(cfg.block), 4 if prec == "f32" else 8)
+    assert (nbytes == 0) == (prec == "f32")
+    U, clov = fields(prob, prec)
+    b = prob.psi[0]
+    rx, rr = oracle.sap(rounded(b, prec), U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=4, n_mr=6)
+    gx, gr = gpu_sap(lq, d, b, cfg.block, 4, 6)
+    bar = 2 * 4 * 7 * TOL1[prec]
+    assert rel_l2(gx, rx) <= bar
+    assert np.linalg.norm(gr - rr) / np.linalg.norm(b) <= bar
+    assert np.linalg.norm(gr) < np.linalg.norm(b)
+
+
+def test_sap_error_codes(lq):
+    prob = config_problem("c1")
+    cfg = prob.cfg
+    d = Dev(lq, prob, "f32", coarse=False)
+    x, r, b = (lq.empty_spinor(cfg.dims) for _ in range(3))
+
+    def code(fn):
+        try:
+            fn()
+        except lq.LqcdError as e:
+            return e.code
+        return 0
+
+    n0 = lq.launch_count()
+    sap = lambda **kw: lq.sap(x, r, b, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, **{"domain": cfg.block, **kw})
+    assert code(lambda: sap(domain=(3, 2, 2, 2))) == lq.EINVAL
+    assert code(lambda: sap(n_sap=-1)) == lq.EINVAL
+    assert code(lambda: lq.sap(x, x, b, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block)) == lq.EINVAL
+    assert code(lambda: lq.sap(x, r, b, d.U, d.clover, cfg.kappa, cfg.dims, (1, 1, 1, 0), cfg.block)) == lq.EINVAL
+    assert "lqcd_sap_f32" in lq.last_error()
+    mr = lambda **kw: lq.mr_domain_solve(x, r, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, **kw)
+    assert code(lambda: mr(niter=-2)) == lq.EINVAL
+    assert code(lambda: lq.mr_domain_solve(x, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block)) == lq.EINVAL
+    assert code(lambda: lq.wilson_clover_residual(x, b, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc)) == lq.EINVAL
+    assert code(lambda: lq.block_dotc(x, b, cfg.dims, (3, 1, 1, 1))) == lq.EINVAL
+    # the generic path without its workspace
+    lq.set_knob("sap_fused", -1)
+    try:
+        assert code(lambda: sap()) == lq.EINVAL and "workspace" in lq.last_error()
+    finally:
+        lq.set_knob("sap_fused", 0)
+    assert lq.launch_count() == n0, "nothing is enqueued on error"
