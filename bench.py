@@ -72,6 +72,19 @@ def model_dsap(cfg: li.Config, parity: int = 0) -> dict:
     return {"bytes": (active_b + 96) * V / 2, "flops": active_f * V / 2, "units": V}   # other group: zeros written
 
 
+def model_sap(cfg: li.Config, n_sap: int = 4, n_mr: int = 6) -> dict:
+    """F3: the inner-domain solver on one domain group (x += M^(g) r, the operator read once for all n_mr iterations)
+    and SAP(n_sap) = 2 n_sap half sweeps, each one solver launch and one residual r = b - D x."""
+    V = cfg.volume
+    d = model_dsap(cfg, 0)
+    site_b = d["bytes"] / V + 96           # r, links inside the domain, clover, x read + x written
+    site_f = n_mr * (d["flops"] / V + 336)  # D_SAP + two blocked dots (96 + 48) + two blocked axpys (2 x 96)
+    mr = {"bytes": site_b * V / 2, "flops": site_f * V / 2, "units": V / 2}
+    res = {"bytes": (768 + 96) * V, "flops": (1872 + 24) * V}
+    return {"mr": mr, "sap": {"bytes": 2 * n_sap * (mr["bytes"] + res["bytes"]),
+                              "flops": 2 * n_sap * (mr["flops"] + res["flops"]), "units": V}}
+
+
 STEP_ORDER = ["wilson_clover", "wilson_clover_dagger", "restrict", "coarse_mult", "prolong"]
 KERNEL_SYMBOL = {  # the __global__ each row launches (for the ncu launch list)
     "wilson_clover": "k_wilson_clover", "wilson_clover_dagger": "k_wilson_clover", "restrict": "k_restrict",
@@ -291,6 +304,16 @@ class Workload:
         c = self.cfg
         self.lq.wilson_clover_dd_mult(self.y[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block,
                                       parity=1)
+
+    def mr_even(self, i):
+        c = self.cfg
+        self.lq.mr_domain_solve(self.y[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block, parity=1,
+                                niter=6, accumulate=True, ws=getattr(self, "mr_ws", None))
+
+    def sap(self, i):
+        c = self.cfg
+        self.lq.sap(self.y[i], self.z[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block, n_sap=4,
+                    n_mr=6, ws=getattr(self, "mr_ws", None))
 
     def restrict(self, i):
         c = self.cfg
@@ -530,6 +553,25 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             extra[name] = {"us": t * 1e6, "GBps": md["bytes"] / t / 1e9, "GFLOPs": md["flops"] / t / 1e9,
                            "units_per_s": md["units"] / t, "frac_of_hbm_peak": md["bytes"] / t / 1e9 / peak,
                            "bytes_per_launch": md["bytes"]}
+
+        # F3: the inner-domain solver (6 minimal-residual iterations, even domains), shared-memory-resident and
+        # generic, and the SAP smoother with the paper's parameters (n = 4, 6 inner iterations)
+        import torch
+        ms = model_sap(cfg)
+        for name, knob, key in (("mr_even", 0, "mr"), ("mr_even", -1, "mr"), ("sap", 0, "sap")):
+            W.lq.set_knob("sap_fused", knob)
+            nb = int(W.lq.lib().lqcd_mr_workspace_bytes(W.lq._i4(cfg.dims), W.lq._i4(cfg.block), 4))
+            W.mr_ws = torch.empty(nb, dtype=torch.uint8, device=W.dev) if nb else None
+            t = time_single(W, name, reps=max(3, min(10, args.steps)), warmup=1)
+            W.mr_ws = None
+            md = ms[key]
+            label = {("mr_even", 0): "mr_domain_solve_even", ("mr_even", -1): "mr_domain_solve_even_generic",
+                     ("sap", 0): "sap_4_6"}[(name, knob)]
+            extra[label] = {"us": t * 1e6, "GBps": md["bytes"] / t / 1e9, "GFLOPs": md["flops"] / t / 1e9,
+                            "units_per_s": md["units"] / t, "frac_of_hbm_peak": md["bytes"] / t / 1e9 / peak,
+                            "bytes_per_launch": md["bytes"],
+                            "path": "generic" if nb else "shared-memory-resident"}
+        W.lq.set_knob("sap_fused", 0)
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)

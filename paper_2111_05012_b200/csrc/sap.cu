@@ -4,7 +4,7 @@
 // procedure with fixed iterations (listing PAPER.md:127-131).
 //
 // B200 design: a 4^4 domain's residual, links and clover term are 168 KB in fp32 -- they
-// fit the 227 KB of shared memory of one SM.  k_mr_domain therefore runs ALL n_mr iterations of one domain inside
+// fit the 227 KB of shared memory of one SM (192 KB with the exchange buffer of the two-threads-per-site split).  k_mr_domain therefore runs ALL n_mr iterations of one domain inside
 // one CTA: the operator fields are read from HBM once per half sweep instead of once per iteration, the blocked
 // dot products are CTA reductions, the blocked axpys are register updates, and nothing but the solution goes back
 // to HBM.  Domains that do not fit (fp64 4^4, 8x4^3) take the generic path: D_SAP^(e/o) by k_wilson_clover and
@@ -82,82 +82,134 @@ template <int NRED, typename T> __device__ __forceinline__ void cta_sum(T v[NRED
 }
 
 // ---- the shared-memory-resident inner-domain solver ------------------------------------------------------
-// One directed hop of D_SAP with every operand in shared memory: rho_s[j][l] vec16 rows of the residual,
-// U_s[row][l] vec16 rows over the 72 reals (mu, 18) of the four forward links of local site l.
+// Shared-memory image of one domain (bv sites, local index l, x fastest):
+//   rho_s [NJ][bv]  vec16            the current residual (every thread reads its neighbours' from here)
+//   U_s   [mu][NFULL][bv] vec16      the four forward links of site l, laid out as in HBM:
+//   U_t   [mu][bv] float2 (fp32)     18 reals = NFULL full vec16 rows (+ one 8-byte tail in fp32)
+//   C_s   [NR][bv]  vec16            the clover term (Hermitian storage, 72 reals)
+//   xch_s [NJ/2][2 bvp] vec16        exchange of the partial hop sums between the two threads of a site
+// fp32, 4^4: 24 + 72 + 72 + 24 KB = 192 KB of the SM's 227 KB.
+//
+// TWO threads per site (l, h): with one thread per site the kernel needs 255 registers, i.e. 8 warps per SM, and
+// was latency-bound on shared-memory loads (ncu: 2 warps per scheduler, issue slots 41 % busy).  Thread h = 0
+// computes the x and y hops, h = 1 the z and t hops (h is warp-uniform: threads l and l + bvp, so the direction
+// templates do not diverge); the halves of the two partial sums are exchanged through xch_s, after which thread h
+// owns the chirality block chi = h of the site (spin components 2h, 2h+1): its clover block, its 12 reals of rho, z
+// and p, its share of the blocked dot products.  128 registers, 16 warps per SM.
+template <typename T> __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global.L2::64B [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global.L2::64B [%0], [%1], 8;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
+template <typename T> struct MrSmem {
+    static constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, NR = 72 / NV, NFULL = 18 / NV, TAIL = 18 - NFULL * NV;
+    static __host__ __device__ size_t bytes(int bv, int bvp) {
+        return (size_t)bv * (NJ + 4 * NFULL + NR) * 16 + (size_t)bv * 4 * TAIL * sizeof(T) +
+               (size_t)bvp * 2 * (NJ / 2) * 16 + 16 * 3 * sizeof(T);
+    }
+};
+
+// One directed hop of D_SAP with every operand in shared memory.
 template <int MU, bool FWD, int SGN, typename T>
 __device__ __forceinline__ void hop_smem(T acc[24], const V16<T>* __restrict__ rho_s, const V16<T>* __restrict__ U_s,
-                                         int bv, int l_link, int l_nb, T ph) {
-    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV;
+                                         const T* __restrict__ U_t, int bv, int l_link, int l_nb, T ph) {
+    using S = MrSmem<T>;
+    constexpr int NV = S::NV;
     T p[24], h[12], u[18], g[12];
 #pragma unroll
-    for (int j = 0; j < NJ; j++) {
+    for (int j = 0; j < S::NJ; j++) {
         const V16<T> v = rho_s[j * bv + l_nb];
 #pragma unroll
         for (int q = 0; q < NV; q++) p[j * NV + q] = v.r[q];
     }
-    constexpr int R0 = 18 * MU / NV, R1 = (18 * MU + 17) / NV;
 #pragma unroll
-    for (int row = R0; row <= R1; row++) {
-        const V16<T> v = U_s[row * bv + l_link];
+    for (int j = 0; j < S::NFULL; j++) {
+        const V16<T> v = U_s[(MU * S::NFULL + j) * bv + l_link];
 #pragma unroll
-        for (int q = 0; q < NV; q++) {
-            const int idx = row * NV + q - 18 * MU;
-            if (idx >= 0 && idx < 18) u[idx] = v.r[q];
-        }
+        for (int q = 0; q < NV; q++) u[j * NV + q] = v.r[q];
+    }
+    if (S::TAIL) {
+        const float2 v = *reinterpret_cast<const float2*>(U_t + (MU * bv + l_link) * 2);
+        u[16] = (T)v.x;
+        u[17] = (T)v.y;
     }
     project<MU, SGN, T>(h, p);
     su3_mult<FWD, T>(g, u, h);
     reconstruct<MU, SGN, T>(acc, g, ph);
 }
 
-// x (+)= M_SAP^(g) r for one domain per CTA, thread l <-> local site l; ACC: accumulate into x.
-template <typename T, bool ACC>
-__global__ void __launch_bounds__(256, 1)
+// x (+)= M_SAP^(g) r: one domain per CTA, two threads per site (see above); ACC: accumulate into x.
+// BVC: sites per domain as a compile-time constant (a multiple of 32; every shared-memory row offset then folds into
+// the immediate field of LDS/STS: -12 % instructions), 0 = run-time P.bv.
+template <typename T, bool ACC, int BVC>
+__global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits at most 151 sites (320 threads)
     k_mr_domain(T* __restrict__ x, const T* __restrict__ r, const T* __restrict__ U, const T* __restrict__ clover,
                 T kappa, DomParams P, int niter) {
-    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, NR = 72 / NV;
+    using S = MrSmem<T>;
+    constexpr int NV = S::NV, NJ = S::NJ, NH = S::NJ / 2, NR = S::NR, NFULL = S::NFULL;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int bv = P.bv;
-    V16<T>* rho_s = reinterpret_cast<V16<T>*>(smem_raw);  // [NJ][bv]
-    V16<T>* U_s = rho_s + NJ * bv;                        // [NR][bv]
-    V16<T>* C_s = U_s + NR * bv;                          // [NR][bv]
-    T* red = reinterpret_cast<T*>(C_s + NR * bv);         // [warps][3]
+    const int bv = BVC ? BVC : P.bv, bvp = BVC ? BVC : (int)(blockDim.x >> 1), tid = threadIdx.x;
+    V16<T>* rho_s = reinterpret_cast<V16<T>*>(smem_raw);
+    V16<T>* U_s = rho_s + NJ * bv;
+    V16<T>* C_s = U_s + 4 * NFULL * bv;
+    V16<T>* xch_s = C_s + NR * bv;
+    T* U_t = reinterpret_cast<T*>(xch_s + NH * 2 * bvp);
+    T* red = U_t + 4 * bv * S::TAIL;
 
+    const int h = tid >= bvp;  // warp-uniform (bvp is a multiple of 32)
+    const int l0 = tid - h * bvp;
+    const bool active = l0 < bv;
+    const int l = active ? l0 : 0;
     int Xc[4], lx[4];
     const bool selected = domain_of_cta(P, blockIdx.x, Xc);
-    const bool active = (int)threadIdx.x < bv;
-    const int l = active ? (int)threadIdx.x : 0;
     const int s = domain_site(P, Xc, l, lx);
+    const int lane = s & 31;
+    const long long chunk = s >> 5;
+    const long long sp_off = (chunk * NJ * CH + lane) * NV;  // native spinor row 0 of site s
     if (!selected) {  // only reached without ACC: M^(g) r vanishes outside the group
         if (active) {
-            T zero[24];
+            V16<T> zero;
 #pragma unroll
-            for (int q = 0; q < 24; q++) zero[q] = 0;
-            store_spinor<T>(x, s, zero);
+            for (int q = 0; q < NV; q++) zero.r[q] = 0;
+#pragma unroll
+            for (int j = 0; j < NH; j++) st16_stream(x + sp_off + (long long)(NH * h + j) * CH * NV, zero);
         }
         return;
     }
 
-    // ---- stage the domain: residual -> registers + shared, links and clover -> shared (read ONCE from HBM)
-    T rho[24];
-    load_spinor<T, true>(rho, r, s);
-    if (active) {
-        {
-            T ul[72];
+    // ---- stage the domain (every operand is read ONCE from HBM): links and clover straight into shared memory
+    // (cp.async, 64-byte L2 granularity: a 4-site x-run of a domain is half a 128-byte line), my half of r in registers
+    T rho[12];
 #pragma unroll
-            for (int mu = 0; mu < 4; mu++) load_link<T, false, true>(ul + 18 * mu, U, s, mu);
+    for (int j = 0; j < NH; j++) {
+        const V16<T> v = ld16_g64(r + sp_off + (long long)(NH * h + j) * CH * NV);
 #pragma unroll
-            for (int j = 0; j < NR; j++) {
-                V16<T> v;
-#pragma unroll
-                for (int q = 0; q < NV; q++) v.r[q] = ul[j * NV + q];
-                U_s[j * bv + l] = v;
-            }
-        }
-        const T* cbase = clover + ((long long)(s >> 5) * NR * CH + (s & 31)) * NV;
-#pragma unroll
-        for (int j = 0; j < NR; j++) C_s[j * bv + l] = ld16_stream_g64(cbase + (long long)j * CH * NV);
+        for (int q = 0; q < NV; q++) rho[j * NV + q] = v.r[q];
     }
+    if (active) {
+#pragma unroll
+        for (int m = 0; m < 2; m++) {
+            const int mu = 2 * h + m;
+            const T* g = U + (chunk * 4 + mu) * (18LL * CH);
+#pragma unroll
+            for (int j = 0; j < NFULL; j++) cp_async16<T>(&U_s[(mu * NFULL + j) * bv + l], g + (j * CH + lane) * NV);
+            if (S::TAIL) cp_async8(U_t + (mu * bv + l) * 2, g + NFULL * NV * CH + lane * 2);
+        }
+        const T* cbase = clover + (chunk * NR * CH + lane) * NV;
+#pragma unroll
+        for (int j = 0; j < NR / 2; j++) {
+            const int row = h * (NR / 2) + j;
+            cp_async16<T>(&C_s[row * bv + l], cbase + (long long)row * CH * NV);
+        }
+    }
+    cp_async_wait_all();
 
     // neighbours inside the domain (local index, wrapped) and hop phases: a hop that leaves the domain is cut
     // (phase 0); in a direction spanned by ONE domain the wrap is the lattice's own and carries bc[mu].
@@ -176,53 +228,84 @@ __global__ void __launch_bounds__(256, 1)
             ls *= P.dom[mu];
         }
     }
+    const int partner = h ? tid - bvp : tid + bvp;
 
-    T z[24];
+    T z[12];
 #pragma unroll
-    for (int q = 0; q < 24; q++) z[q] = 0;
+    for (int q = 0; q < 12; q++) z[q] = 0;
 
     for (int it = 0; it < niter; it++) {
         if (active) {
 #pragma unroll
-            for (int j = 0; j < NJ; j++) {
+            for (int j = 0; j < NH; j++) {
                 V16<T> v;
 #pragma unroll
                 for (int q = 0; q < NV; q++) v.r[q] = rho[j * NV + q];
-                rho_s[j * bv + l] = v;
+                rho_s[(NH * h + j) * bv + l] = v;
+            }
+        }
+        __syncthreads();  // rho_s complete (first pass: also the cp.async data of every thread)
+        // my four hops of D_SAP rho; the half of the partial sum that belongs to the other chirality goes to the partner
+        T mine[12];
+        {
+            T acc[24];
+#pragma unroll
+            for (int q = 0; q < 24; q++) acc[q] = 0;
+            if (h == 0) {
+                hop_smem<0, true, -1, T>(acc, rho_s, U_s, U_t, bv, l, nf[0], pf[0]);
+                hop_smem<0, false, +1, T>(acc, rho_s, U_s, U_t, bv, nb[0], nb[0], pb[0]);
+                hop_smem<1, true, -1, T>(acc, rho_s, U_s, U_t, bv, l, nf[1], pf[1]);
+                hop_smem<1, false, +1, T>(acc, rho_s, U_s, U_t, bv, nb[1], nb[1], pb[1]);
+#pragma unroll
+                for (int j = 0; j < NH; j++) {
+                    V16<T> v;
+#pragma unroll
+                    for (int q = 0; q < NV; q++) {
+                        v.r[q] = acc[12 + j * NV + q];
+                        mine[j * NV + q] = acc[j * NV + q];
+                    }
+                    xch_s[j * 2 * bvp + tid] = v;
+                }
+            } else {
+                hop_smem<2, true, -1, T>(acc, rho_s, U_s, U_t, bv, l, nf[2], pf[2]);
+                hop_smem<2, false, +1, T>(acc, rho_s, U_s, U_t, bv, nb[2], nb[2], pb[2]);
+                hop_smem<3, true, -1, T>(acc, rho_s, U_s, U_t, bv, l, nf[3], pf[3]);
+                hop_smem<3, false, +1, T>(acc, rho_s, U_s, U_t, bv, nb[3], nb[3], pb[3]);
+#pragma unroll
+                for (int j = 0; j < NH; j++) {
+                    V16<T> v;
+#pragma unroll
+                    for (int q = 0; q < NV; q++) {
+                        v.r[q] = acc[j * NV + q];
+                        mine[j * NV + q] = acc[12 + j * NV + q];
+                    }
+                    xch_s[j * 2 * bvp + tid] = v;
+                }
             }
         }
         __syncthreads();
-        // p = D_SAP rho
-        T acc[24];
+        T p[12];
 #pragma unroll
-        for (int q = 0; q < 24; q++) acc[q] = 0;
-        hop_smem<0, true, -1, T>(acc, rho_s, U_s, bv, l, nf[0], pf[0]);
-        hop_smem<0, false, +1, T>(acc, rho_s, U_s, bv, nb[0], nb[0], pb[0]);
-        hop_smem<1, true, -1, T>(acc, rho_s, U_s, bv, l, nf[1], pf[1]);
-        hop_smem<1, false, +1, T>(acc, rho_s, U_s, bv, nb[1], nb[1], pb[1]);
-        hop_smem<2, true, -1, T>(acc, rho_s, U_s, bv, l, nf[2], pf[2]);
-        hop_smem<2, false, +1, T>(acc, rho_s, U_s, bv, nb[2], nb[2], pb[2]);
-        hop_smem<3, true, -1, T>(acc, rho_s, U_s, bv, l, nf[3], pf[3]);
-        hop_smem<3, false, +1, T>(acc, rho_s, U_s, bv, nb[3], nb[3], pb[3]);
-        T p[24];
+        for (int j = 0; j < NH; j++) {
+            const V16<T> v = xch_s[j * 2 * bvp + partner];
 #pragma unroll
-        for (int q = 0; q < 24; q++) p[q] = fma(-kappa, acc[q], rho[q]);
-#pragma unroll
-        for (int chi = 0; chi < 2; chi++) {
+            for (int q = 0; q < NV; q++) p[j * NV + q] = fma(-kappa, mine[j * NV + q] + v.r[q], rho[j * NV + q]);
+        }
+        {
             T cl[36];
 #pragma unroll
             for (int j = 0; j < 36 / NV; j++) {
-                const V16<T> v = C_s[(chi * (36 / NV) + j) * bv + l];
+                const V16<T> v = C_s[(h * (36 / NV) + j) * bv + l];
 #pragma unroll
                 for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
             }
-            herm6_madd<T>(p + 12 * chi, cl, rho + 12 * chi);
+            herm6_madd<T>(p, cl, rho);
         }
         // alpha = <p|rho>_X / <p|p>_X  (blocked dotc)
         T d[3] = {0, 0, 0};
         if (active) {
 #pragma unroll
-            for (int k = 0; k < 12; k++) {
+            for (int k = 0; k < 6; k++) {
                 d[0] = fma(p[2 * k], rho[2 * k], d[0]);
                 d[0] = fma(p[2 * k + 1], rho[2 * k + 1], d[0]);
                 d[1] = fma(p[2 * k], rho[2 * k + 1], d[1]);
@@ -235,7 +318,7 @@ __global__ void __launch_bounds__(256, 1)
         const T ar = d[2] > 0 ? d[0] / d[2] : (T)0, ai = d[2] > 0 ? d[1] / d[2] : (T)0;
         // z += alpha rho ; rho -= alpha p  (blocked axpy)
 #pragma unroll
-        for (int k = 0; k < 12; k++) {
+        for (int k = 0; k < 6; k++) {
             const T rr = rho[2 * k], ri = rho[2 * k + 1];
             z[2 * k] = fma(ar, rr, z[2 * k]);
             z[2 * k] = fma(-ai, ri, z[2 * k]);
@@ -246,24 +329,23 @@ __global__ void __launch_bounds__(256, 1)
             rho[2 * k + 1] = fma(-ar, p[2 * k + 1], rho[2 * k + 1]);
             rho[2 * k + 1] = fma(-ai, p[2 * k], rho[2 * k + 1]);
         }
-        // (the barrier inside cta_sum ordered every read of rho_s and red before the next iteration's writes of
-        // rho_s; red is rewritten only after the next __syncthreads)
+        // hazards: rho_s and xch_s are rewritten only after the barrier in cta_sum (all reads done) and, for
+        // red, after the two barriers of the next iteration.
     }
 
     if (active) {
-        if (ACC) {
-            T xo[24];
-            load_spinor<T, true>(xo, x, s);
 #pragma unroll
-            for (int q = 0; q < 24; q++) z[q] += xo[q];
-        }
-        T* base = x + ((long long)(s >> 5) * NJ * CH + (s & 31)) * NV;
-#pragma unroll
-        for (int j = 0; j < NJ; j++) {
+        for (int j = 0; j < NH; j++) {
+            T* px = x + sp_off + (long long)(NH * h + j) * CH * NV;
             V16<T> v;
 #pragma unroll
             for (int q = 0; q < NV; q++) v.r[q] = z[j * NV + q];
-            st16(base + (long long)j * CH * NV, v);
+            if (ACC) {
+                const V16<T> xo = ld16_g64(px);
+#pragma unroll
+                for (int q = 0; q < NV; q++) v.r[q] += xo.r[q];
+            }
+            st16(px, v);
         }
     }
 }
@@ -454,9 +536,7 @@ static int dom_setup(DomParams& P, const int dims[4], const int bc[4], const int
     return LQCD_OK;
 }
 
-template <typename T> static size_t mr_smem_bytes(int bv) {
-    return (size_t)bv * (24 + 72 + 72) * sizeof(T) + 8 * 3 * sizeof(T);
-}
+template <typename T> static size_t mr_smem_bytes(int bv) { return MrSmem<T>::bytes(bv, (bv + 31) / 32 * 32); }
 
 static int max_optin_smem() {
     static int v = -1;
@@ -504,29 +584,30 @@ static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa
 
     if (mr_fits_smem<T>(P.bv)) {
         const size_t smem = mr_smem_bytes<T>(P.bv);
-        const int threads = (P.bv + 31) / 32 * 32;
+        const int threads = 2 * ((P.bv + 31) / 32 * 32);  // two threads per site
         unsigned grid = (unsigned)P.Vc;
         if (acc && P.parity != 0 && P.Lc[0] % 2 == 0) {  // no CTA for the domains of the other group
             P.halfgrid = 1;
             grid = (unsigned)(P.Vc / 2);
         }
-        if (acc) {
-            static bool attr = false;
-            if (!attr) {
-                cudaFuncSetAttribute(k_mr_domain<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     max_optin_smem());
-                attr = true;
-            }
-            k_mr_domain<T, true><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter);
+#define LAUNCH_MR(ACC, BVC)                                                                                   \
+    do {                                                                                                      \
+        static bool attr = false;                                                                             \
+        if (!attr) {                                                                                          \
+            cudaFuncSetAttribute(k_mr_domain<T, ACC, BVC>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
+                                 max_optin_smem());                                                           \
+            attr = true;                                                                                      \
+        }                                                                                                     \
+        k_mr_domain<T, ACC, BVC><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter);               \
+    } while (0)
+        if (sizeof(T) == 4 && P.bv == 256) {  // the paper's typical 4^4 domain
+            if (acc) LAUNCH_MR(true, (sizeof(T) == 4 ? 256 : 0));
+            else LAUNCH_MR(false, (sizeof(T) == 4 ? 256 : 0));
         } else {
-            static bool attr = false;
-            if (!attr) {
-                cudaFuncSetAttribute(k_mr_domain<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     max_optin_smem());
-                attr = true;
-            }
-            k_mr_domain<T, false><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter);
+            if (acc) LAUNCH_MR(true, 0);
+            else LAUNCH_MR(false, 0);
         }
+#undef LAUNCH_MR
         count_launch();
         return check_launch(what);
     }
