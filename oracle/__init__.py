@@ -257,3 +257,25 @@ def sap(b, U, clover, kappa, dims, bc, domain, n_sap=4, n_mr=6):
     _check(fn(_ptr(x), _ptr(r), _ptr(b), _ptr(U), _ptr(clover), C.c_double(kappa), _i4(dims), _i4(bc), _i4(domain),
               C.c_int(n_sap), C.c_int(n_mr)), "sap")
     return x, r
+
+
+def coarse_bicgstab(b, A, cdims, nvec, niter):
+    """(1b) of PAPER.md:116: `niter` BiCGStab iterations (listing PAPER.md:71 with M = 1, x0 = 0; Q18)
+    for D_c x = b -> (x, recurrence residual)."""
+    b, A = _c128(b), _c128(A)
+    x, r = np.empty_like(b), np.empty_like(b)
+    fn = lib().lqcd_coarse_bicgstab_ref
+    fn.restype = C.c_int
+    _check(fn(_ptr(x), _ptr(r), _ptr(b), _ptr(A), _i4(cdims), C.c_int(nvec), C.c_int(niter)), "coarse_bicgstab")
+    return x, r
+
+
+def mg_vcycle(b, U, clover, kappa, dims, bc, block, v, A, n_coarse=8, n_sap=4, n_mr=6) -> np.ndarray:
+    """x = M b: one V-cycle of the multigrid preconditioner."""
+    b, U, clover, v, A = _c128(b), _c128(U), _c128(clover), _c128(v), _c128(A)
+    x = np.empty_like(b)
+    fn = lib().lqcd_mg_vcycle_ref
+    fn.restype = C.c_int
+    _check(fn(_ptr(x), _ptr(b), _ptr(U), _ptr(clover), C.c_double(kappa), _i4(dims), _i4(bc), _i4(block),
+              C.c_int(v.shape[0]), _ptr(v), _ptr(A), C.c_int(n_coarse), C.c_int(n_sap), C.c_int(n_mr)), "mg_vcycle")
+    return x

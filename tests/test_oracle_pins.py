@@ -623,3 +623,72 @@ def test_sap_listing(c1):
     x1, r1 = oracle.sap(c1["psi"][0], c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc, cfg.block)
     true_r = c1["psi"][0] - oracle.wilson_clover_mult(x1, c1["U"], c1["clov"], cfg.kappa, cfg.dims, cfg.bc)
     assert rel(r1, true_r) < 1e-13 and np.linalg.norm(r1) < 0.05 * np.linalg.norm(c1["psi"][0])
+
+
+# ------------------------------------------------------------------------------------------------
+# F3 (continued)  coarse BiCGStab with fixed iterations and the V-cycle
+# ------------------------------------------------------------------------------------------------
+def dense_coarse(A, cdims, nvec):
+    n = int(np.prod(cdims)) * 2 * nvec
+    M = np.zeros((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1
+        M[:, k] = oracle.coarse_mult(e.reshape(-1, 2, nvec), A, cdims).ravel()
+    return M
+
+
+def test_coarse_bicgstab_against_scipy_and_dense_solve(c1):
+    """An independent library routine (scipy.sparse.linalg.bicgstab, stopped after the same number of iterations) on
+    the dense coarse matrix (itself pinned by brute force above), and the exact solution for many iterations."""
+    import scipy.sparse.linalg as spla
+    cfg = c1["cfg"]
+    Dc = dense_coarse(c1["A"], cfg.cdims, cfg.nvec)
+    rng = np.random.default_rng(41)
+    b = li.coarse_vector(rng, cfg.cvolume, cfg.nvec)
+    for niter in (1, 2, 5, 9):
+        ref, info = spla.bicgstab(Dc, b.ravel(), x0=np.zeros(Dc.shape[0], dtype=np.complex128), rtol=1e-300, atol=0.0,
+                                  maxiter=niter)
+        assert info == niter  # stopped by the iteration count, not by convergence
+        x, r = oracle.coarse_bicgstab(b, c1["A"], cfg.cdims, cfg.nvec, niter)
+        assert rel(x.ravel(), ref) < 1e-11, niter
+        assert np.linalg.norm(r.ravel() - (b.ravel() - Dc @ x.ravel())) < 1e-12 * np.linalg.norm(b), \
+            "the recurrence residual is the true residual"
+    x0, r0 = oracle.coarse_bicgstab(b, c1["A"], cfg.cdims, cfg.nvec, 0)
+    assert not np.any(x0) and np.array_equal(r0, b)
+    x, r = oracle.coarse_bicgstab(b, c1["A"], cfg.cdims, cfg.nvec, 60)
+    assert rel(x.ravel(), np.linalg.solve(Dc, b.ravel())) < 1e-10
+    # residual norms fall by orders of magnitude within the paper-like iteration counts ("not necessarily ... high
+    # precision", PAPER.md:116)
+    assert np.linalg.norm(oracle.coarse_bicgstab(b, c1["A"], cfg.cdims, cfg.nvec, 8)[1]) < 1e-2 * np.linalg.norm(b)
+
+
+def test_vcycle_structure_and_convergence(c1):
+    cfg = c1["cfg"]
+    U, clov, v, A = c1["U"], c1["clov"], c1["v"], c1["A"]
+    b = c1["psi"][0]
+    D = lambda y: oracle.wilson_clover_mult(y, U, clov, cfg.kappa, cfg.dims, cfg.bc)
+    args = (U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block, v, A)
+    # (1) alone with an accurate coarse solve: Galerkin orthogonality R (b - D P D_c^-1 R b) = 0 because D_c = R D P
+    x1 = oracle.mg_vcycle(b, *args, n_coarse=60, n_sap=0)
+    assert np.linalg.norm(oracle.restrict(b - D(x1), v, cfg.dims, cfg.block)) < 1e-9 * np.linalg.norm(b)
+    # ... and x1 lies in the range of P: P R x1 = x1
+    assert rel(oracle.prolong(oracle.restrict(x1, v, cfg.dims, cfg.block), v, cfg.dims, cfg.block), x1) < 1e-13
+    # (2) alone (no coarse iterations): the V-cycle is SAP
+    assert rel(oracle.mg_vcycle(b, *args, n_coarse=0, n_sap=2, n_mr=3),
+               oracle.sap(b, U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=3)[0]) < 1e-14
+    # both: the two Richardson refinements of PAPER.md:112 from the pinned parts
+    xc, _ = oracle.coarse_bicgstab(oracle.restrict(b, v, cfg.dims, cfg.block), A, cfg.cdims, cfg.nvec, 8)
+    y = oracle.prolong(xc, v, cfg.dims, cfg.block)
+    y = y + oracle.sap(b - D(y), U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block)[0]
+    x = oracle.mg_vcycle(b, *args)
+    assert rel(x, y) < 1e-13
+    # M ~ D^-1: as a stationary iteration x += M (b - D x) the error against the DENSE solve contracts every cycle
+    V = cfg.volume
+    Dd = dense_of(D, V)
+    exact = np.linalg.solve(Dd, b.ravel()).reshape(V, 4, 3)
+    xk, errs = np.zeros_like(b), []
+    for _ in range(4):
+        xk = xk + oracle.mg_vcycle(b - D(xk), *args)
+        errs.append(rel(xk, exact))
+    assert errs[0] < 0.1 and all(e2 < 0.25 * e1 for e1, e2 in zip(errs, errs[1:])), errs
