@@ -257,6 +257,37 @@ int lqcd_sap_f64(double* x, double* r, const double* b, const double* U, const d
                  const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
                  void* ws_dev, void* stream);
 
+/* Coarse solver (1b) of PAPER.md:116 ("We employ the BiCGStab algorithm ... not necessarily performed with high
+ * precision"): the BiCGStab recurrence of the listing PAPER.md:71 with M = 1 and x_0 = 0 for D_c x = b, with a FIXED
+ * number of iterations instead of the listing's two "small enough" break points (reading Q18):
+ *   r = rt = p = b;  repeat niter times:  v = D_c p;  alpha = <rt|r>/<rt|v>;  s = r - alpha v;  t = D_c s;
+ *     omega = <t|s>/<t|t>;  x += alpha p + omega s;  r' = s - omega t;  beta = (alpha/omega) <rt|r'>/<rt|r>;
+ *     p = r' + beta (p - omega v);  r = r'.        (a vanishing denominator sets its quotient to 0)
+ * x, b: coarse vectors; r_out (may be NULL): receives the recurrence residual; A as for lqcd_coarse_mult.  All scalars
+ * stay on the device (no host synchronisation); dot products have a fixed summation order.  ws_dev: device scratch of
+ * lqcd_coarse_bicgstab_workspace_bytes(cdims, nvec, sizeof(real)) bytes.  7 launches per iteration. */
+size_t lqcd_coarse_bicgstab_workspace_bytes(const int cdims[4], int nvec, int real_bytes);
+int lqcd_coarse_bicgstab_f32(float* x, float* r_out, const float* b, const float* A, const int cdims[4], int nvec,
+                             int niter, void* ws_dev, void* stream);
+int lqcd_coarse_bicgstab_f64(double* x, double* r_out, const double* b, const double* A, const int cdims[4], int nvec,
+                             int niter, void* ws_dev, void* stream);
+
+/* One V-cycle x = M b of the multigrid preconditioner, two Richardson refinements
+ * "|x> + M_i(|b> - D|x>) -> |x>" from |x> = 0:
+ *   (1) M_1 = prolong o BiCGStab(D_c, n_coarse iterations) o restrict     steps (1a)-(1c)
+ *   (2) M_2 = SAP(n_sap, n_mr) with the aggregation block as SAP domain   ("We set the SAP domain to be the same as
+ *                                                                          the domain of coarsening")
+ * x, b: native spinors, distinct; U: native 18-real gauge; nullvecs: native, block-orthonormal; A: coarse matrix.
+ * Everything is enqueued on `stream`, device-resident, no host synchronisation or copy.  ws_dev: device scratch of
+ * lqcd_mg_workspace_bytes(dims, block, nvec, sizeof(real)) bytes. */
+size_t lqcd_mg_workspace_bytes(const int dims[4], const int block[4], int nvec, int real_bytes);
+int lqcd_mg_vcycle_f32(float* x, const float* b, const float* U, const float* clover, float kappa, const int dims[4],
+                       const int bc[4], const int block[4], int nvec, const float* nullvecs, const float* A,
+                       int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
+int lqcd_mg_vcycle_f64(double* x, const double* b, const double* U, const double* clover, double kappa,
+                       const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
+                       const double* A, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
+
 /* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
  * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned

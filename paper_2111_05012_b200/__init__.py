@@ -372,6 +372,36 @@ def sap(x, r, b, U, clover, kappa, dims, bc, domain, n_sap=4, n_mr=6, initial_gu
                                              _ws_ptr(ws), _stream(stream)), "lqcd_sap")
     return x
 
+def coarse_bicgstab(x, b, A, cdims, nvec, niter, r_out=None, ws=None, stream=None):
+    """(1b) of PAPER.md:116: niter BiCGStab iterations (listing PAPER.md:71, M = 1, x0 = 0) for D_c x = b."""
+    sfx = _same_dtype(x, b, A)
+    if ws is None:
+        nb = int(lib().lqcd_coarse_bicgstab_workspace_bytes(_i4(cdims), int(nvec), 4 if sfx == "f32" else 8))
+        ws = torch.empty(nb, dtype=torch.uint8, device=x.device)
+    _check(getattr(lib(), f"lqcd_coarse_bicgstab_{sfx}")(_dev_ptr(x), _ws_ptr(r_out), _dev_ptr(b), _dev_ptr(A),
+                                                         _i4(cdims), int(nvec), int(niter), _dev_ptr(ws),
+                                                         _stream(stream)), "lqcd_coarse_bicgstab")
+    return x
+
+
+def mg_workspace(dims, block, nvec, dtype=torch.float32, device="cuda") -> torch.Tensor:
+    nb = int(lib().lqcd_mg_workspace_bytes(_i4(dims), _i4(block), int(nvec), 4 if dtype == torch.float32 else 8))
+    return torch.empty(nb, dtype=torch.uint8, device=device)
+
+
+def mg_vcycle(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, n_coarse=8, n_sap=4, n_mr=6, ws=None,
+              stream=None):
+    """x = M b: one V-cycle of the multigrid preconditioner."""
+    sfx = _same_dtype(x, b, U, clover, nullvecs, A)
+    if ws is None:
+        ws = mg_workspace(dims, block, nvec, dtype=_rdtype(sfx), device=x.device)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_mg_vcycle_{sfx}")(_dev_ptr(x), _dev_ptr(b), _dev_ptr(U), _dev_ptr(clover), k,
+                                                   _i4(dims), _i4(bc), _i4(block), int(nvec), _dev_ptr(nullvecs),
+                                                   _dev_ptr(A), int(n_coarse), int(n_sap), int(n_mr), _dev_ptr(ws),
+                                                   _stream(stream)), "lqcd_mg_vcycle")
+    return x
+
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):

@@ -31,6 +31,8 @@ SIGNATURES = {
     "lqcd_host_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_galerkin_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
     "lqcd_mr_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
+    "lqcd_coarse_bicgstab_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci]),
+    "lqcd_mg_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
 }
 for _p, _k in (("f32", _cf), ("f64", _cd)):
     SIGNATURES.update({
@@ -53,6 +55,8 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_block_dotc_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _vp]),
         f"lqcd_block_caxpy_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _vp]),
         f"lqcd_mr_domain_solve_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _cu, _ci, _vp, _vp]),
+        f"lqcd_coarse_bicgstab_{_p}": (_ci, [_vp, _vp, _vp, _vp, _i4, _ci, _ci, _vp, _vp]),
+        f"lqcd_mg_vcycle_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _vp, _vp, _ci, _ci, _ci, _vp, _vp]),
         f"lqcd_sap_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _cu, _vp, _vp]),
     })
 SIGNATURES.update({

@@ -1,0 +1,169 @@
+"""F3, second half, on the GPU against the oracle (-m gpu): the coarse BiCGStab with fixed iterations
+and one V-cycle of the multigrid preconditioner, through the C ABI.
+
+Bars.  One operator application keeps the north_star bars TOL1 (1e-12 fp64, 2e-6 fp32).
+A k-iteration BiCGStab applies D_c 2k times; its iterate is a rational function of inner products, so the forward
+error is bounded by (number of applications) x cond(D_c) x TOL1 -- cond(D_c) is computed in the test from the oracle's
+dense coarse matrix where that is small enough, else the bound 30 (cond <= 17 measured on configs 1-2).  The V-cycle
+adds the restriction, the prolongation and SAP's 2 n_sap (n_mr + 1) fine applications.
+"""
+import numpy as np
+import pytest
+
+import lqcd_inputs as li
+import oracle
+from problems import config_problem, rel_l2
+from test_gpu_parity import Dev, rounded, to_dev
+
+pytestmark = pytest.mark.gpu
+
+TOL1 = {"f64": 1e-12, "f32": 2e-6}
+
+
+@pytest.fixture(scope="module")
+def lq():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_2111_05012_b200 as lq
+    return lq
+
+
+def cond_coarse(prob, prec):
+    cfg = prob.cfg
+    n = cfg.cvolume * 2 * cfg.nvec
+    if n > 1024:
+        return 30.0
+    A = rounded(prob.A, prec).astype(np.complex128)
+    M = np.zeros((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1
+        M[:, k] = oracle.coarse_mult(e.reshape(-1, 2, cfg.nvec), A, cfg.cdims).ravel()
+    return float(np.linalg.cond(M))
+
+
+def gpu_bicgstab(lq, d, b, niter, want_r=True):
+    import torch
+    cfg = d.cfg
+    bd = to_dev(b, d.prec)
+    x = torch.full_like(bd, 9.0)
+    r = torch.full_like(bd, 9.0) if want_r else None
+    lq.coarse_bicgstab(x, bd, d.A, cfg.cdims, cfg.nvec, niter, r_out=r)
+    return x.cpu().numpy(), (r.cpu().numpy() if want_r else None)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_coarse_bicgstab(lq, prec, name):
+    prob = config_problem(name)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    cond = cond_coarse(prob, prec)
+    assert cond < 30
+    b = prob.xc
+    A = rounded(prob.A, prec)
+    for niter in (0, 1, 3, 8):
+        rx, rr = oracle.coarse_bicgstab(rounded(b, prec), A, cfg.cdims, cfg.nvec, niter)
+        gx, gr = gpu_bicgstab(lq, d, b, niter)
+        if niter == 0:
+            assert not np.any(gx) and np.array_equal(gr, rounded(b, prec))
+            continue
+        bar = 2 * niter * cond * TOL1[prec]
+        assert rel_l2(gx, rx) <= bar, (niter, rel_l2(gx, rx), bar)
+        assert np.linalg.norm(gr - rr) / np.linalg.norm(b) <= bar, niter  # the residual on the scale of b
+    # without r_out: the same solution, bit for bit (fixed summation order)
+    gx2, _ = gpu_bicgstab(lq, d, b, 8, want_r=False)
+    assert np.array_equal(gx, gx2)
+    # b = 0: every quotient has a vanishing denominator -> x = 0, no NaN
+    gx0, gr0 = gpu_bicgstab(lq, d, np.zeros_like(b), 3)
+    assert not np.any(gx0) and not np.any(gr0)
+
+
+def gpu_vcycle(lq, d, b, n_coarse, n_sap, n_mr):
+    cfg = d.cfg
+    bn = lq.pack_spinor(to_dev(b, d.prec), cfg.dims)
+    x = lq.empty_spinor(cfg.dims, dtype=bn.dtype)
+    x.fill_(2.0)
+    lq.mg_vcycle(x, bn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, cfg.nvec, d.v, d.A, n_coarse=n_coarse,
+                 n_sap=n_sap, n_mr=n_mr)
+    return lq.unpack_spinor(x, cfg.dims).cpu().numpy()
+
+
+def oracle_vcycle(prob, prec, b, n_coarse, n_sap, n_mr):
+    cfg = prob.cfg
+    return oracle.mg_vcycle(rounded(b, prec), rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa, cfg.dims,
+                            cfg.bc, cfg.block, rounded(prob.v, prec), rounded(prob.A, prec), n_coarse=n_coarse,
+                            n_sap=n_sap, n_mr=n_mr)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("path", [0, -1], ids=["resident", "generic"])
+def test_c1_vcycle(lq, prec, path):
+    prob = config_problem("c1")
+    d = Dev(lq, prob, prec)
+    cond = cond_coarse(prob, prec)
+    b = prob.psi[0]
+    lq.set_knob("sap_fused", path)
+    try:
+        for n_coarse, n_sap, n_mr in ((8, 4, 6), (3, 0, 6), (0, 2, 3), (0, 0, 0)):
+            ref = oracle_vcycle(prob, prec, b, n_coarse, n_sap, n_mr)
+            got = gpu_vcycle(lq, d, b, n_coarse, n_sap, n_mr)
+            if not np.any(ref):
+                assert not np.any(got)
+                continue
+            bar = (2 * n_coarse * cond + 2 + 2 * n_sap * (n_mr + 1)) * TOL1[prec]
+            assert rel_l2(got, ref) <= bar, (n_coarse, n_sap, n_mr, rel_l2(got, ref), bar)
+    finally:
+        lq.set_knob("sap_fused", 0)
+    # M ~ D^-1: the V-cycle with the paper's parameters reduces the residual of D x = b
+    x = gpu_vcycle(lq, d, b, 8, 4, 6)
+    cfg = prob.cfg
+    res = rounded(b, prec) - oracle.wilson_clover_mult(x, rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa,
+                                                       cfg.dims, cfg.bc)
+    assert np.linalg.norm(res) < 0.1 * np.linalg.norm(b)
+
+
+@pytest.mark.parametrize("name", ["c2", "c3"])
+def test_vcycle_fp32_configs(lq, name):
+    """config 2 (8^4, N_nv = 16) and config 3 (16^3 x 32, N_nv = 32, the V-cycle config): 4^4 domains, i.e. the
+    shared-memory-resident smoother at its design size, the paper's parameters n_sap = 4, n_mr = 6."""
+    prob = config_problem(name)
+    d = Dev(lq, prob, "f32")
+    b = prob.psi[0]
+    n_coarse = 8 if name == "c2" else 4
+    ref = oracle_vcycle(prob, "f32", b, n_coarse, 4, 6)
+    got = gpu_vcycle(lq, d, b, n_coarse, 4, 6)
+    bar = (2 * n_coarse * 30.0 + 2 + 2 * 4 * 7) * TOL1["f32"]
+    assert rel_l2(got, ref) <= bar, (rel_l2(got, ref), bar)
+
+
+def test_mg_error_codes(lq):
+    import torch
+    prob = config_problem("c1")
+    cfg = prob.cfg
+    d = Dev(lq, prob, "f32")
+    x, b = lq.empty_spinor(cfg.dims), lq.empty_spinor(cfg.dims)
+    xc = torch.zeros((cfg.cvolume, 2, cfg.nvec), dtype=torch.complex64, device="cuda")
+    bc_ = torch.zeros_like(xc)
+
+    def code(fn):
+        try:
+            fn()
+        except lq.LqcdError as e:
+            return e.code
+        return 0
+
+    n0 = lq.launch_count()
+    vc = lambda **kw: lq.mg_vcycle(x, b, d.U, d.clover, cfg.kappa, cfg.dims, **{"bc": cfg.bc, "block": cfg.block,
+                                                                                 "nvec": cfg.nvec, "nullvecs": d.v,
+                                                                                 "A": d.A, **kw})
+    assert code(lambda: vc(bc=(1, 1, 1, 2))) == lq.EINVAL
+    assert code(lambda: vc(block=(4, 4, 4, 4))) == lq.EINVAL      # coarse extent 1
+    assert code(lambda: vc(n_coarse=-1)) == lq.EINVAL
+    assert code(lambda: lq.mg_vcycle(x, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, cfg.nvec, d.v,
+                                     d.A)) == lq.EINVAL
+    assert "lqcd_mg_vcycle_f32" in lq.last_error()
+    assert code(lambda: lq.coarse_bicgstab(xc, xc, d.A, cfg.cdims, cfg.nvec, 3)) == lq.EINVAL
+    assert code(lambda: lq.coarse_bicgstab(xc, bc_, d.A, cfg.cdims, cfg.nvec, -1)) == lq.EINVAL
+    assert code(lambda: lq.coarse_bicgstab(xc, bc_, d.A, (2, 2, 2, 1), cfg.nvec, 1)) == lq.EINVAL
+    assert lq.launch_count() == n0, "nothing is enqueued on error"
