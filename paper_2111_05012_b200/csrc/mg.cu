@@ -272,7 +272,7 @@ static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims
         if ((rc = coarse_mult_any<T>(W.t, W.s, A, cdims, nvec, stream))) return rc;                // t = D_c s
         k_cdot<T><<<RED_CTAS, RED_THREADS, 0, st>>>(W.part_a, W.t, W.s, n);                        // <t|s>, <t|t>
         k_bicg_xr<T><<<RED_CTAS, RED_THREADS, 0, st>>>(x, W.r, p, W.s, W.t, b, W.part_a, W.part_b, W.sc, it == 0, n);
-        count_launch(3);
+        count_launch(4);
         if (it + 1 < niter) {  // the last p is never used
             k_bicg_p<T><<<RED_CTAS, RED_THREADS, 0, st>>>(W.p, p, W.r, W.v, W.part_b, W.sc, it, n);
             count_launch();
