@@ -288,6 +288,19 @@ int lqcd_mg_vcycle_f64(double* x, const double* b, const double* U, const double
                        const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
                        const double* A, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
 
+/* ---- F4: the coarse operator on K right-hand sides at once (many right-hand sides are "a typical
+ * situation") ----------------------------------------------------------------------------------------------------
+ *   out_k = D_c in_k,  k = 0 .. nrhs-1     (Eqs. 4, 7; the definition of lqcd_coarse_mult, K times)
+ * in, out: nrhs coarse vectors back to back, [k][X][chi][i]; A as for lqcd_coarse_mult; out must not alias in.
+ * fp32 with nvec = 32 (N = 64) and flags = 0 runs on the tensor cores (tcgen05, 3xTF32 split of both operands with
+ * fp32 accumulation in short TMEM chains added in registers: fp32 accuracy; A is read from HBM ONCE per launch of up
+ * to 32 right-hand sides);
+ * every other case (other nvec, LQCD_DAGGER, fp64) applies lqcd_coarse_mult once per right-hand side. */
+int lqcd_coarse_mult_mrhs_f32(float* out, const float* in, const float* A, const int cdims[4], int nvec, int nrhs,
+                              unsigned flags, void* stream);
+int lqcd_coarse_mult_mrhs_f64(double* out, const double* in, const double* A, const int cdims[4], int nvec, int nrhs,
+                              unsigned flags, void* stream);
+
 /* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
  * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned

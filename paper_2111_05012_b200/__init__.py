@@ -402,6 +402,15 @@ def mg_vcycle(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, n_coar
                                                    _stream(stream)), "lqcd_mg_vcycle")
     return x
 
+def coarse_mult_mrhs(out, inp, A, cdims, nvec, dagger=False, stream=None):
+    """F4: out[k] = D_c in[k] for all k at once; in, out of shape (K, Vc, 2, nvec) complex."""
+    sfx = _same_dtype(out, inp, A)
+    nrhs = int(inp.shape[0])
+    _check(getattr(lib(), f"lqcd_coarse_mult_mrhs_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(A), _i4(cdims),
+                                                          int(nvec), nrhs, DAGGER if dagger else 0, _stream(stream)),
+           "lqcd_coarse_mult_mrhs")
+    return out
+
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):

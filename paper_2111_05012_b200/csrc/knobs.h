@@ -9,6 +9,8 @@ struct Knobs {
     int coarse_R = 0;                 // rows in flight per lane (1, 2, 4), 0 = automatic (2)
     int coarse_warps = 0;             // warps per CTA of the coarse kernel, 0 = automatic
     int transfer_warps = 0;           // warps per CTA of restrict, 0 = automatic
+    int mrhs_tensor = 0;              // 0 = tcgen05 path of coarse_mult_mrhs when it applies; -1 = never
+    int mrhs_stages = 0;              // pipeline stages of coarse_mult_mrhs, 0 = as many as fit
     int sap_fused = 0;                // 0 = shared-memory-resident inner-domain solver when it fits; -1 = never
 };
 extern Knobs g_knobs;

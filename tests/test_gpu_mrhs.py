@@ -1,0 +1,120 @@
+"""F4 on the GPU against the oracle (-m gpu): the coarse operator on K right-hand sides at once.  The definition is K
+independent applications of Eq. 4/7, so the expected value is the oracle's coarse_mult per right-
+hand side; the bar is the north_star's per-application bar (2e-6 fp32 -- also for the tensor-core path, whose 3xTF32
+operand split is there to keep fp32 accuracy; 1e-12 fp64)."""
+import numpy as np
+import pytest
+
+import lqcd_inputs as li
+import oracle
+from problems import config_problem, rel_l2
+from test_gpu_parity import Dev, rounded, to_dev
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 2e-6}
+
+
+@pytest.fixture(scope="module")
+def lq():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_2111_05012_b200 as lq
+    return lq
+
+
+def rhs_set(cfg, nrhs, seed=77):
+    rng = np.random.default_rng(seed)
+    return np.stack([li.coarse_vector(rng, cfg.cvolume, cfg.nvec) for _ in range(nrhs)])
+
+
+def gpu_mrhs(lq, d, xs, dagger=False):
+    import torch
+    x = to_dev(xs, d.prec)
+    y = torch.full_like(x, 3.0)
+    lq.coarse_mult_mrhs(y, x, d.A, d.cfg.cdims, d.cfg.nvec, dagger=dagger)
+    torch.cuda.synchronize()
+    return y.cpu().numpy()
+
+
+@pytest.mark.parametrize("nrhs", [1, 3, 4, 16, 21, 64, 70])
+def test_c3_tensor_core_path(lq, nrhs):
+    """config 3 (coarse 4^3 x 8, N = 64, true Galerkin blocks): tcgen05 path, also ragged K and K > 32 (several launches)"""
+    prob = config_problem("c3")
+    cfg = prob.cfg
+    d = Dev(lq, prob, "f32")
+    xs = rhs_set(cfg, nrhs)
+    n0 = lq.launch_count()
+    got = gpu_mrhs(lq, d, xs)
+    assert lq.launch_count() - n0 == (nrhs + 31) // 32, "one tensor-core launch per 32 right-hand sides"
+    A = rounded(prob.A, "f32")
+    worst = 0.0
+    for k in range(nrhs):
+        ref = oracle.coarse_mult(rounded(xs[k], "f32"), A, cfg.cdims)
+        worst = max(worst, rel_l2(got[k], ref))
+    assert worst <= TOL["f32"], worst
+    # the tensor-core path and the single-right-hand-side kernel agree to rounding
+    lq.set_knob("mrhs_tensor", -1)
+    try:
+        alt = gpu_mrhs(lq, d, xs)
+    finally:
+        lq.set_knob("mrhs_tensor", 0)
+    assert rel_l2(got, alt) <= TOL["f32"]
+
+
+def test_c3_structured_inputs(lq):
+    """unit vectors and a constant vector: a wrong neighbour, a transposed block or a swapped (re, im) row of the
+    operand matrix cannot hide behind random data"""
+    prob = config_problem("c3")
+    cfg = prob.cfg
+    d = Dev(lq, prob, "f32")
+    xs = np.zeros((8, cfg.cvolume, 2, cfg.nvec), dtype=np.complex128)
+    sites = [0, 1, cfg.cdims[0], cfg.cvolume - 1]
+    for k, X in enumerate(sites):
+        xs[k, X, k % 2, (5 * k) % cfg.nvec] = 1.0        # real unit vector at one site
+        xs[4 + k, X, (k + 1) % 2, (7 * k + 3) % cfg.nvec] = 1j  # imaginary unit vector
+    got = gpu_mrhs(lq, d, xs)
+    A = rounded(prob.A, "f32")
+    for k in range(8):
+        ref = oracle.coarse_mult(xs[k], A.astype(np.complex128), cfg.cdims)
+        assert rel_l2(got[k], ref) <= TOL["f32"], k
+        assert np.array_equal(got[k] == 0, ref == 0), "exact zeros outside the stencil"
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_generic_sizes(lq, prec, name):
+    """N = 8 and N = 32 (and fp64): one single-right-hand-side application per vector; dagger form too"""
+    prob = config_problem(name)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    xs = rhs_set(cfg, 5)
+    A = rounded(prob.A, prec)
+    for dagger in (False, True):
+        got = gpu_mrhs(lq, d, xs, dagger=dagger)
+        for k in range(5):
+            ref = oracle.coarse_mult(rounded(xs[k], prec), A, cfg.cdims, dagger=dagger)
+            assert rel_l2(got[k], ref) <= TOL[prec], (k, dagger)
+
+
+def test_mrhs_error_codes(lq):
+    import torch
+    prob = config_problem("c1")
+    cfg = prob.cfg
+    d = Dev(lq, prob, "f32")
+    x = torch.zeros((2, cfg.cvolume, 2, cfg.nvec), dtype=torch.complex64, device="cuda")
+    y = torch.zeros_like(x)
+
+    def code(fn):
+        try:
+            fn()
+        except lq.LqcdError as e:
+            return e.code
+        return 0
+
+    n0 = lq.launch_count()
+    assert code(lambda: lq.coarse_mult_mrhs(x, x, d.A, cfg.cdims, cfg.nvec)) == lq.EINVAL
+    assert code(lambda: lq.coarse_mult_mrhs(y, x, d.A, (2, 2, 1, 2), cfg.nvec)) == lq.EINVAL
+    assert code(lambda: lq.coarse_mult_mrhs(y, x, d.A, cfg.cdims, 0)) == lq.EINVAL
+    assert "lqcd_coarse_mult_mrhs_f32" in lq.last_error()
+    assert lq.launch_count() == n0
