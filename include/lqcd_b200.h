@@ -294,7 +294,7 @@ int lqcd_mg_vcycle_f64(double* x, const double* b, const double* U, const double
  * in, out: nrhs coarse vectors back to back, [k][X][chi][i]; A as for lqcd_coarse_mult; out must not alias in.
  * fp32 with nvec = 32 (N = 64) and flags = 0 runs on the tensor cores (tcgen05, 3xTF32 split of both operands with
  * fp32 accumulation in short TMEM chains added in registers: fp32 accuracy; A is read from HBM ONCE per launch of up
- * to 32 right-hand sides);
+ * to 16 right-hand sides);
  * every other case (other nvec, LQCD_DAGGER, fp64) applies lqcd_coarse_mult once per right-hand side. */
 int lqcd_coarse_mult_mrhs_f32(float* out, const float* in, const float* A, const int cdims[4], int nvec, int nrhs,
                               unsigned flags, void* stream);

@@ -33,17 +33,19 @@ namespace lqcd {
 constexpr int MR_ROWS = 64;          // N = 2 nvec = 64 rows per block; hi and lo stacked: UMMA M = 128
 constexpr int MR_KT = 64;            // reals of the contraction index per stage (half a block)
 constexpr int MR_HALVES = 18;        // 9 blocks x 2 halves per coarse site
+constexpr int MR_AS = 2;             // pipeline stages accumulated into one TMEM slot (chain of MR_AS * 8 MMAs)
 constexpr int MR_EPI_WARPS = 4, MR_PROD_GROUPS = 4, MR_PROD_WARPS = 4 * MR_PROD_GROUPS;
-constexpr int MR_ISSUERS = 1;         // MMA-issuing warps (one elected lane)
+constexpr int MR_ISSUERS = 2;         // MMA-issuing warps (one elected lane each); stages in turn, like the producers
 constexpr int MR_THREADS = (MR_EPI_WARPS + MR_ISSUERS + MR_PROD_WARPS) * 32;  // 672
 constexpr int MR_TMEM_COLS = 512;    // all of TMEM: one accumulator slot of 2 NCOL columns per pipeline stage
 
 struct MrhsParams {
     int Lc[4];
+    FastDiv dLc[3];  // division by Lc[0..2] as a multiply-high
     int Vc;
     int nrhs;     // K
-    int stages;      // shared-memory pipeline stages = TMEM accumulator slots
-    int groups;      // active producer groups; divides stages, so that every stage is always filled by the same group
+    int stages;      // shared-memory pipeline stages
+    int slots;       // TMEM accumulator slots (2 NCOL columns each); a multiple of groups
     long long vstride;  // reals between consecutive right-hand sides: Vc * 128
 };
 
@@ -163,20 +165,21 @@ __device__ __forceinline__ void split_tf32(const V16<float>& x, V16<float>& hi, 
     }
 }
 
-// neighbour of coarse site X for block d (0 diag, 1+2mu forward, 2+2mu backward), periodic
+// neighbour of coarse site X for block d (0 diag, 1+2mu forward, 2+2mu backward), periodic.  No dynamic indexing of
+// the parameter struct (that would put it in local memory) and no run-time division: this sits on the producers'
+// critical path (with a generic version the address arithmetic took longer than the loads it precedes).
 __device__ __forceinline__ int coarse_neighbour(const MrhsParams& P, int X, int d) {
     if (d == 0) return X;
-    const int mu = (d - 1) >> 1, fwd = (d - 1) & 1 ? -1 : +1;
-    int stride = 1, xc = X;
-    for (int nu = 0; nu < mu; nu++) {
-        stride *= P.Lc[nu];
-        xc /= P.Lc[nu];
-    }
-    const int c = xc % P.Lc[mu];
-    int cn = c + fwd;
-    if (cn < 0) cn += P.Lc[mu];
-    if (cn >= P.Lc[mu]) cn -= P.Lc[mu];
-    return X + (cn - c) * stride;
+    const int mu = (d - 1) >> 1;
+    const int q0 = P.dLc[0].div(X), x0 = X - q0 * P.Lc[0];
+    const int q1 = P.dLc[1].div(q0), x1 = q0 - q1 * P.Lc[1];
+    const int q2 = P.dLc[2].div(q1), x2 = q1 - q2 * P.Lc[2];
+    const int s1 = P.Lc[0], s2 = s1 * P.Lc[1], s3 = s2 * P.Lc[2];
+    const int c = mu == 0 ? x0 : mu == 1 ? x1 : mu == 2 ? x2 : q2;
+    const int L = mu == 0 ? P.Lc[0] : mu == 1 ? P.Lc[1] : mu == 2 ? P.Lc[2] : P.Lc[3];
+    const int stride = mu == 0 ? 1 : mu == 1 ? s1 : mu == 2 ? s2 : s3;
+    if ((d - 1) & 1) return c == 0 ? X + (L - 1) * stride : X - stride;  // backward
+    return c == L - 1 ? X - (L - 1) * stride : X + stride;               // forward
 }
 
 // shared memory: [stages][ A: 128 rows (hi, lo) x 64 reals = 32 KB | B_hi ncol*256 B | B_lo ncol*256 B ], then the
@@ -211,16 +214,21 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
     constexpr unsigned stage_bytes = mr_stage_bytes(NCOL);
     float* xbuf = reinterpret_cast<float*>(smem + (size_t)S * stage_bytes);           // [64][NCOL]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(xbuf + MR_ROWS * NCOL);
-    unsigned long long* full = bars;            // [S] producers -> issuer: operands of the stage are in shared memory
-    unsigned long long* done = bars + S;        // [S] tcgen05.commit -> producers (stage free) and epilogue (slot ready)
-    unsigned long long* tfree = bars + 2 * S;   // [S] epilogue -> issuer: the stage's TMEM slot has been read
-    unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 3 * S);
+    const int T = P.slots;
+    unsigned long long* full = bars;               // [S] producers -> issuer: operands of the stage are in shared memory
+    unsigned long long* done = bars + S;           // [S] tcgen05.commit -> producers: the MMAs have read the stage
+    unsigned long long* tfull = bars + 2 * S;      // [T] tcgen05.commit -> epilogue: the slot's accumulators are complete
+    unsigned long long* tfree = bars + 2 * S + T;  // [T] epilogue -> issuer: the slot has been read
+    unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 2 * S + 2 * T);
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < S; i++) {
-            mbar_init(&full[i], 4);              // one arrival per warp of the producer group that owns the stage
-            mbar_init(&done[i], 1);              // one tcgen05.commit
-            mbar_init(&tfree[i], MR_EPI_WARPS);  // one arrival per epilogue warp
+            mbar_init(&full[i], 4);  // one arrival per warp of the producer group that owns the stage
+            mbar_init(&done[i], 1);  // one tcgen05.commit
+        }
+        for (int i = 0; i < T; i++) {
+            mbar_init(&tfull[i], 1);              // one tcgen05.commit
+            mbar_init(&tfree[i], MR_EPI_WARPS);   // one arrival per epilogue warp
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -245,23 +253,29 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
             float acc[NCOL];
 #pragma unroll
             for (int q = 0; q < NCOL; q++) acc[q] = 0.f;
-            for (int hb = 0; hb < MR_HALVES; hb++, g++) {
-                const int st = g % S;
+            for (int ch = 0; ch < MR_HALVES / MR_AS; ch++, g++) {  // g counts accumulator chains here
+                const int st = g % T;  // TMEM slot
                 if (warp == 0) MR_TRACE(2, g, 0);
-                mbar_wait(&done[st], (g / S) & 1, 1, g);
+                mbar_wait(&tfull[st], (g / T) & 1, 1, g);
                 if (warp == 0) MR_TRACE(2, g, 1);
                 tc_fence_after();
                 const unsigned taddr = tmem_base + ((unsigned)(32 * warp) << 16) + (unsigned)(st * 2 * NCOL);
 #pragma unroll
-                for (int c0 = 0; c0 < 2 * NCOL; c0 += 8) {
-                    unsigned v[8];
-                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]),
-                                   "=r"(v[7])
-                                 : "r"(taddr + c0));
+                for (int c0 = 0; c0 < 2 * NCOL; c0 += 32) {  // 32 columns per round trip
+                    unsigned v[32];
+#pragma unroll
+                    for (int h = 0; h < 2; h++)
+                        asm volatile(
+                            "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                            "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                            : "=r"(v[16 * h + 0]), "=r"(v[16 * h + 1]), "=r"(v[16 * h + 2]), "=r"(v[16 * h + 3]),
+                              "=r"(v[16 * h + 4]), "=r"(v[16 * h + 5]), "=r"(v[16 * h + 6]), "=r"(v[16 * h + 7]),
+                              "=r"(v[16 * h + 8]), "=r"(v[16 * h + 9]), "=r"(v[16 * h + 10]), "=r"(v[16 * h + 11]),
+                              "=r"(v[16 * h + 12]), "=r"(v[16 * h + 13]), "=r"(v[16 * h + 14]), "=r"(v[16 * h + 15])
+                            : "r"(taddr + c0 + 16 * h));
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-                    for (int q = 0; q < 8; q++) acc[(c0 + q) % NCOL] += __uint_as_float(v[q]);
+                    for (int q = 0; q < 32; q++) acc[(c0 + q) % NCOL] += __uint_as_float(v[q]);
                 }
                 tc_fence_before();
                 __syncwarp();
@@ -287,7 +301,7 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
             asm volatile("bar.sync 1, 128;" ::: "memory");
         }
     } else if (warp < MR_EPI_WARPS + MR_ISSUERS) {
-        // ===== MMA issuer (one elected lane of warp 4; the other issuer warps idle) =====
+        // ===== MMA issuers (one elected lane per warp) =====
         // instruction descriptor: D fp32, A and B TF32, both K-major, M = 128 (hi rows | lo rows of A),
         // N = 2 ncol (B'_hi rows | B'_lo rows): ONE MMA per k-step yields all four products hi.hi, lo.hi, hi.lo, lo.lo
         const unsigned idesc =
@@ -295,28 +309,42 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
         const unsigned s0 = smem_u32(smem);
         const unsigned long long dA = umma_desc_sw128(s0);
         const unsigned long long dB = umma_desc_sw128(s0 + 2 * MR_ROWS * MR_KT * 4);
-        if (warp == MR_EPI_WARPS && lane == 0) {
-            for (int g = 0; g < G; g++) {
-                const int st = g % S;
-                const unsigned ph = (g / S) & 1;
-                MR_TRACE(1, g, 0);
-                mbar_wait_lane(&tfree[st], ph ^ 1, 2, g);
-                MR_TRACE(1, g, 1);
-                mbar_wait_lane(&full[st], ph, 3, g);
-                MR_TRACE(1, g, 2);
-                tc_fence_after();
-                const unsigned tmem_d = tmem_base + (unsigned)(st * 2 * NCOL);
-                // descriptors differ from those of (stage 0, k-step 0) only in the 14-bit address field
-                const unsigned long long so = (unsigned long long)(((unsigned)st * stage_bytes) >> 4);
+        // Issuer warp m takes the stages g = m, m + NG, ... (NG = P.groups divides S and T: a stage and a slot always
+        // have the same issuer).  A wait on a ready mbarrier still costs ~300 cycles of shared-memory latency under the producers'
+        // store traffic, a commit as much again: one issuer alone paced the kernel at ~1700 cycles per stage.
+        // Issuer warp m takes the accumulator chains c = m, m + MR_ISSUERS, ... (MR_AS stages each).  MR_ISSUERS * MR_AS
+        // divides S and MR_ISSUERS divides T, so a stage and a slot always have the same issuer (a parity wait cannot
+        // tell one completed phase from the one two phases earlier).  One issuer alone cannot keep up: a wait on a ready
+        // mbarrier costs ~300 cycles under the producers' store traffic, issuing 8 small MMAs ~500, a commit ~100.
+        const int mi = warp - MR_EPI_WARPS;
+        if (lane == 0) {
+            for (int c = mi; c < G / MR_AS; c += MR_ISSUERS) {
+                const int sl = c % T;
+                MR_TRACE(1, c * MR_AS, 0);
+                mbar_wait_lane(&tfree[sl], ((c / T) & 1) ^ 1, 2, c);
+                MR_TRACE(1, c * MR_AS, 1);
+                const unsigned tmem_d = tmem_base + (unsigned)(sl * 2 * NCOL);
 #pragma unroll
-                for (int ks = 0; ks < MR_KT / 8; ks++) {  // 8 reals = 32 bytes of the 128-byte swizzled row
-                    const unsigned long long ao = so + (unsigned long long)(((ks >> 2) * 2 * MR_ROWS * 128 + (ks & 3) * 32) >> 4);
-                    const unsigned long long bo = so + (unsigned long long)(((ks >> 2) * 2 * ncol * 128 + (ks & 3) * 32) >> 4);
-                    tc_mma_tf32(tmem_d, dA + ao, dB + bo, idesc, ks != 0);
+                for (int hs = 0; hs < MR_AS; hs++) {
+                    const int g = c * MR_AS + hs, st = g % S;
+                    mbar_wait_lane(&full[st], (g / S) & 1, 3, g);
+                    MR_TRACE(1, g, 2);
+                    tc_fence_after();
+                    // descriptors differ from those of (stage 0, k-step 0) only in the 14-bit address field
+                    const unsigned long long so = (unsigned long long)(((unsigned)st * stage_bytes) >> 4);
+#pragma unroll
+                    for (int ks = 0; ks < MR_KT / 8; ks++) {  // 8 reals = 32 bytes of the 128-byte swizzled row
+                        const unsigned long long ao =
+                            so + (unsigned long long)(((ks >> 2) * 2 * MR_ROWS * 128 + (ks & 3) * 32) >> 4);
+                        const unsigned long long bo =
+                            so + (unsigned long long)(((ks >> 2) * 2 * ncol * 128 + (ks & 3) * 32) >> 4);
+                        tc_mma_tf32(tmem_d, dA + ao, dB + bo, idesc, (hs | ks) != 0);
+                    }
+                    MR_TRACE(1, g, 3);
+                    tc_commit(&done[st]);
+                    MR_TRACE(1, g, 4);
                 }
-                MR_TRACE(1, g, 3);
-                tc_commit(&done[st]);
-                MR_TRACE(1, g, 4);
+                tc_commit(&tfull[sl]);
             }
         }
         __syncwarp();
@@ -326,6 +354,8 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
         // full round (MR_PROD_GROUPS stage times, > the HBM latency) later.  Why not a deeper register prefetch inside
         // one group: fence.proxy.async / the releasing mbarrier arrive drain every outstanding load of the thread,
         // so loads in flight across a hand-over serialise the pipeline (measured: ~2000 cycles per stage).
+        // Stage ownership: MR_PROD_GROUPS divides S, so a stage is always filled by the same group (a parity wait
+        // cannot tell one completed phase from the one two phases earlier).
         const int pw = warp - MR_EPI_WARPS - MR_ISSUERS;  // 0..15
         const int pg = pw >> 2, wq = pw & 3;              // group, warp in group
         const int ptg = wq * 32 + lane;                   // 0..127
@@ -363,11 +393,9 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
                     bq[j].r[0] = bq[j].r[1] = bq[j].r[2] = bq[j].r[3] = 0.f;
             }
         };
-        // A parity wait cannot tell "the previous use of this stage is over" from "the use before that is over", so
-        // consecutive uses of a stage must be ordered by program order of ONE group: P.groups divides P.stages.
-        const int NG = P.groups;
-        if (pg < NG && pg < G) issue(pg);
-        for (int g = pg; g < G && pg < NG; g += NG) {
+        constexpr int NG = MR_PROD_GROUPS;
+        if (pg < G) issue(pg);
+        for (int g = pg; g < G; g += NG) {
             const int st = g % S;
             if (wq == 0) MR_TRACE(0, g, 0);
             mbar_wait(&done[st], ((g / S) & 1) ^ 1, 4, g);
@@ -437,22 +465,20 @@ static int mrhs_sm_count() {
     return v;
 }
 
-// one tensor-core launch for up to 32 right-hand sides
+// one tensor-core launch for up to 16 right-hand sides
 template <int NCOL>
 static int mrhs_launch_ncol(float* out, const float* in, const float* A, MrhsParams P, cudaStream_t st, const char* what) {
     constexpr size_t stage = mr_stage_bytes(NCOL);
-    int S = (int)((mrhs_max_smem() - 1024 - MR_ROWS * NCOL * 4) / stage);
-    if (S > mr_max_stages(NCOL)) S = mr_max_stages(NCOL);
-    if (g_knobs.mrhs_stages >= 2 && g_knobs.mrhs_stages < S) S = g_knobs.mrhs_stages;
-    if (S >= 2 * MR_PROD_GROUPS) S = 2 * MR_PROD_GROUPS;
-    else if (S >= MR_PROD_GROUPS) S = MR_PROD_GROUPS;
-    P.groups = S < MR_PROD_GROUPS ? S : MR_PROD_GROUPS;
-    if (S < 2) {
-        set_error("%s: not enough shared memory for two pipeline stages", what);
+    // S = 4 stages: a multiple of the producer groups and of MR_ISSUERS * MR_AS (stage ownership, see the kernel)
+    const int S = 4;
+    static_assert(4 % MR_PROD_GROUPS == 0 && 4 % (MR_ISSUERS * MR_AS) == 0, "stage ownership");
+    if ((size_t)mrhs_max_smem() < S * stage + MR_ROWS * NCOL * 4 + 1024) {
+        set_error("%s: not enough shared memory for the pipeline", what);
         return LQCD_EUNSUPPORTED;
     }
+    P.slots = mr_max_stages(NCOL) / MR_ISSUERS * MR_ISSUERS;
     P.stages = S;
-    const size_t smem = S * stage + MR_ROWS * NCOL * 4 + 3 * S * 8 + 16;
+    const size_t smem = S * stage + MR_ROWS * NCOL * 4 + (2 * S + 2 * 8) * 8 + 16;
     static bool attr = false;
     if (!attr) {
         cudaFuncSetAttribute(k_coarse_mrhs<NCOL>, cudaFuncAttributeMaxDynamicSharedMemorySize, mrhs_max_smem());
@@ -468,13 +494,13 @@ static int mrhs_tensor_launch(float* out, const float* in, const float* A, const
                               cudaStream_t st, const char* what) {
     MrhsParams P;
     for (int mu = 0; mu < 4; mu++) P.Lc[mu] = cdims[mu];
+    for (int mu = 0; mu < 3; mu++) P.dLc[mu].set(cdims[mu]);
     P.Vc = (int)volume(cdims);
     P.nrhs = nrhs;
     P.vstride = vstride;
     P.stages = 0;
     if (nrhs <= 8)  // UMMA with M = 128 needs N to be a multiple of 16 return mrhs_launch_ncol<16>(out, in, A, P, st, what);
-    if (nrhs <= 16) return mrhs_launch_ncol<32>(out, in, A, P, st, what);
-    return mrhs_launch_ncol<64>(out, in, A, P, st, what);
+    return mrhs_launch_ncol<32>(out, in, A, P, st, what);
 }
 
 }  // namespace lqcd
@@ -521,8 +547,8 @@ int lqcd_coarse_mult_mrhs_f32(float* out, const float* in, const float* A, const
     if (volume(cdims) * 9 * 64 * 64 > 0x7fffffffffffLL || volume(cdims) > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
     const long long vstride = volume(cdims) * 4 * nvec;  // reals per coarse vector
     if (nvec == 32 && flags == 0 && g_knobs.mrhs_tensor >= 0) {
-        for (int k0 = 0; k0 < nrhs; k0 += 32) {
-            const int kn = nrhs - k0 < 32 ? nrhs - k0 : 32;
+        for (int k0 = 0; k0 < nrhs; k0 += 16) {  // 16 right-hand sides per launch (TMEM slots and registers)
+            const int kn = nrhs - k0 < 16 ? nrhs - k0 : 16;
             int rc = mrhs_tensor_launch(out + k0 * vstride, in + k0 * vstride, A, cdims, kn, vstride,
                                         (cudaStream_t)stream, what);
             if (rc) return rc;
