@@ -315,6 +315,10 @@ class Workload:
         self.lq.sap(self.y[i], self.z[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block, n_sap=4,
                     n_mr=6, ws=getattr(self, "mr_ws", None))
 
+    def coarse_mrhs(self, i):
+        c = self.cfg
+        self.lq.coarse_mult_mrhs(self.ycK, self.xcK, self.A, c.cdims, c.nvec)
+
     def vcycle(self, i):
         c = self.cfg
         self.lq.mg_vcycle(self.y[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block, c.nvec, self.v,
@@ -589,6 +593,23 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
                                     "units_per_s": cfg.volume / t, "launches": int(nl),
                                     "frac_of_hbm_peak": mvc["bytes"] / t / 1e9 / peak, "bytes_per_launch": mvc["bytes"]}
         W.mg_ws = None
+        # F4: the coarse operator on 16 right-hand sides at once (tcgen05, 3xTF32): A is read from HBM once
+        K = 16
+        gk = torch.Generator(device=W.dev)
+        gk.manual_seed(4242)
+        W.xcK = torch.view_as_complex(torch.randn((K, cfg.cvolume, 2, cfg.nvec, 2), generator=gk, device=W.dev,
+                                                  dtype=torch.float32))
+        W.ycK = torch.empty_like(W.xcK)
+        t = time_single(W, "coarse_mrhs", reps=max(5, min(20, args.steps)), warmup=2)
+        mc = m["coarse_mult"]
+        vec_b = 2 * K * cfg.cvolume * 2 * cfg.nvec * 8
+        extra["coarse_mult_mrhs_16"] = {
+            "us": t * 1e6, "us_per_rhs": t * 1e6 / K, "GBps": (mc["bytes"] + vec_b) / t / 1e9,
+            "GFLOPs": K * mc["flops"] / t / 1e9, "units_per_s": K * cfg.cvolume / t,
+            "speedup_vs_16_single_applications": K * kernels["coarse_mult"]["us"] * 1e-6 / t,
+            "frac_of_hbm_peak": (mc["bytes"] + vec_b) / t / 1e9 / peak, "bytes_per_launch": mc["bytes"] + vec_b,
+            "path": "tcgen05 kind::tf32, hi/lo split of both operands (3xTF32), fp32 accumulation"}
+        del W.xcK, W.ycK
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)
