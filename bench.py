@@ -315,6 +315,10 @@ class Workload:
         self.lq.sap(self.y[i], self.z[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block, n_sap=4,
                     n_mr=6, ws=getattr(self, "mr_ws", None))
 
+    def fine_mrhs(self, i):
+        c = self.cfg
+        self.lq.wilson_clover_mult_mrhs(self.y2[i % 2], self.x2[i % 2], self.U18, self.clover, c.kappa, c.dims, c.bc)
+
     def coarse_mrhs(self, i):
         c = self.cfg
         self.lq.coarse_mult_mrhs(self.ycK, self.xcK, self.A, c.cdims, c.nvec)
@@ -610,6 +614,17 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "frac_of_hbm_peak": (mc["bytes"] + vec_b) / t / 1e9 / peak, "bytes_per_launch": mc["bytes"] + vec_b,
             "path": "tcgen05 kind::tf32, hi/lo split of both operands (3xTF32), fp32 accumulation"}
         del W.xcK, W.ycK
+        # F4, fine half: D on two right-hand sides at once (links and clover read once for both)
+        W.x2 = [torch.stack([W.x[0], W.x[1]]), torch.stack([W.x[2], W.x[3]])]
+        W.y2 = [torch.empty_like(W.x2[0]), torch.empty_like(W.x2[1])]
+        t = time_single(W, "fine_mrhs", reps=max(10, args.steps))
+        fb, ff = (576 + 2 * 192) * cfg.volume, 2 * m["wilson_clover"]["flops"]
+        extra["wilson_clover_mrhs_2"] = {
+            "us": t * 1e6, "us_per_rhs": t * 1e6 / 2, "GBps": fb / t / 1e9, "GFLOPs": ff / t / 1e9,
+            "units_per_s": 2 * cfg.volume / t,
+            "speedup_vs_2_single_applications": 2 * kernels["wilson_clover"]["us"] * 1e-6 / t,
+            "frac_of_hbm_peak": fb / t / 1e9 / peak, "bytes_per_launch": fb}
+        del W.x2, W.y2
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)

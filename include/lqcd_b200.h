@@ -301,6 +301,17 @@ int lqcd_coarse_mult_mrhs_f32(float* out, const float* in, const float* A, const
 int lqcd_coarse_mult_mrhs_f64(double* out, const double* in, const double* A, const int cdims[4], int nvec, int nrhs,
                               unsigned flags, void* stream);
 
+/* The fine operator on nrhs right-hand sides at once: out_k = D in_k (or D^dag in_k), k = 0 .. nrhs-1 (Eq. 1, nrhs
+ * times).  in, out: nrhs native spinors back to back (stride lqcd_native_spinor_reals(dims)); out must not alias in.
+ * Right-hand sides are taken two at a time by a kernel that loads every link and clover block once for both
+ * (576 + 2 x 192 instead of 2 x 768 compulsory bytes per site); an odd one out takes the single-right-hand-side
+ * kernel.  flags: LQCD_DAGGER, LQCD_LINKS_12. */
+int lqcd_wilson_clover_mult_mrhs_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
+                                     const int dims[4], const int bc[4], int nrhs, unsigned flags, void* stream);
+int lqcd_wilson_clover_mult_mrhs_f64(double* out, const double* in, const double* U, const double* clover,
+                                     double kappa, const int dims[4], const int bc[4], int nrhs, unsigned flags,
+                                     void* stream);
+
 /* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
  * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned

@@ -411,6 +411,17 @@ def coarse_mult_mrhs(out, inp, A, cdims, nvec, dagger=False, stream=None):
            "lqcd_coarse_mult_mrhs")
     return out
 
+def wilson_clover_mult_mrhs(out, inp, U, clover, kappa, dims, bc, dagger=False, links12=False, stream=None):
+    """F4: out[k] = D in[k] for all k at once; in, out of shape (K, native_spinor_reals(dims))."""
+    sfx = _same_dtype(out, inp, U, clover)
+    flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_wilson_clover_mult_mrhs_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(U),
+                                                                 _dev_ptr(clover), k, _i4(dims), _i4(bc),
+                                                                 int(inp.shape[0]), flags, _stream(stream)),
+           "lqcd_wilson_clover_mult_mrhs")
+    return out
+
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):

@@ -11,6 +11,7 @@ struct Knobs {
     int transfer_warps = 0;           // warps per CTA of restrict, 0 = automatic
     int mrhs_tensor = 0;              // 0 = tcgen05 path of coarse_mult_mrhs when it applies; -1 = never
     int mrhs_stages = 0;              // pipeline stages of coarse_mult_mrhs, 0 = as many as fit
+    int fine_mrhs = 0;                // -1 = wilson_clover_mult_mrhs applies the single-right-hand-side kernel per vector
     int sap_fused = 0;                // 0 = shared-memory-resident inner-domain solver when it fits; -1 = never
 };
 extern Knobs g_knobs;

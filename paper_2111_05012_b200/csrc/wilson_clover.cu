@@ -33,32 +33,12 @@ struct FineParams {
     int parity;    // 0 = all domains, 1 = even domains only, 2 = odd domains only
 };
 
-// one directed hop: FWD: (1 + SGN g_mu) U_mu(x) in(x+mu);  !FWD: (1 + SGN g_mu) U_mu^dag(x-mu) in(x-mu)
-template <int MU, bool FWD, int SGN, bool L12, bool G64, typename T>
-__device__ __forceinline__ void hop(T acc[24], const T* __restrict__ in, const T* __restrict__ U, int s_link, int s_nb,
-                                    T ph) {
-    T p[24], h[12], u[18], g[12];
-    load_spinor<T, G64>(p, in, s_nb);
-    load_link<T, L12, G64>(u, U, s_link, MU);
-    project<MU, SGN, T>(h, p);
-    su3_mult<FWD, T>(g, u, h);
-    reconstruct<MU, SGN, T>(acc, g, ph);
-}
-
-// DD: the domain-decomposed operator D_SAP -- hops whose two ends lie in different domains are switched off
-// (no load is issued for them), and with P.parity != 0 only the sites of even (odd) domains are computed, the
-// others are set to zero (D_SAP^(e/o) = P_e/o D_SAP P_e/o).
-// DD = 2: the even/odd mode; active data then comes in alternate 64-byte half lines -> 64-byte L2 granularity.
-// RES: the Richardson residual out = rhs - D in (PAPER.md:112, 128-131) in the same pass: one more streamed read.
-template <typename T, bool DAG, bool L12, int DD, bool RES, int MAXTHREADS, int MINBLOCKS>
-__global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
-    k_wilson_clover(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ U, const T* __restrict__ clover,
-                    const T* __restrict__ rhs, T kappa, FineParams P) {
-    // ---- which site is mine: CTA -> tile (x tiles fastest; optionally z-slabbed traversal), thread -> site in tile
-    // (all divisions by run-time extents are multiply-high with host-computed reciprocals: the index decode was a
-    // quarter of the integer work of this kernel)
+// Which site is mine: CTA -> tile (x tiles fastest; optionally z-slabbed traversal), thread -> site in tile.  All
+// divisions by run-time extents are multiply-high with host-computed reciprocals (the index decode was a quarter of
+// the integer work of the fine kernel).  False for the padding threads of a CTA.
+__device__ __forceinline__ bool fine_decode(const FineParams& P, int x[4], int& s_out) {
     int tid = threadIdx.x;
-    if (tid >= P.tilevol) return;
+    if (tid >= P.tilevol) return false;
     int b = blockIdx.x, q;
     int tc[4];
     q = P.d_ntile[0].div(b); tc[0] = b - q * P.ntile[0]; b = q;
@@ -80,13 +60,40 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
         tc[3] = P.d_ntile[2].div(b);
         tc[2] = b - tc[3] * P.ntile[2];
     }
-    int x[4];
     q = P.d_tile[0].div(tid); x[0] = tc[0] * P.tile[0] + (tid - q * P.tile[0]); tid = q;
     q = P.d_tile[1].div(tid); x[1] = tc[1] * P.tile[1] + (tid - q * P.tile[1]); tid = q;
     q = P.d_tile[2].div(tid); x[2] = tc[2] * P.tile[2] + (tid - q * P.tile[2]); tid = q;
     x[3] = tc[3] * P.tile[3] + tid;
     const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
-    const int s = x[0] + st1 * x[1] + st2 * x[2] + st3 * x[3];
+    s_out = x[0] + st1 * x[1] + st2 * x[2] + st3 * x[3];
+    return true;
+
+}
+
+// one directed hop: FWD: (1 + SGN g_mu) U_mu(x) in(x+mu);  !FWD: (1 + SGN g_mu) U_mu^dag(x-mu) in(x-mu)
+template <int MU, bool FWD, int SGN, bool L12, bool G64, typename T>
+__device__ __forceinline__ void hop(T acc[24], const T* __restrict__ in, const T* __restrict__ U, int s_link, int s_nb,
+                                    T ph) {
+    T p[24], h[12], u[18], g[12];
+    load_spinor<T, G64>(p, in, s_nb);
+    load_link<T, L12, G64>(u, U, s_link, MU);
+    project<MU, SGN, T>(h, p);
+    su3_mult<FWD, T>(g, u, h);
+    reconstruct<MU, SGN, T>(acc, g, ph);
+}
+
+// DD: the domain-decomposed operator D_SAP -- hops whose two ends lie in different domains are switched off
+// (no load is issued for them), and with P.parity != 0 only the sites of even (odd) domains are computed, the
+// others are set to zero (D_SAP^(e/o) = P_e/o D_SAP P_e/o).
+// DD = 2: the even/odd mode; active data then comes in alternate 64-byte half lines -> 64-byte L2 granularity.
+// RES: the Richardson residual out = rhs - D in (PAPER.md:112, 128-131) in the same pass: one more streamed read.
+template <typename T, bool DAG, bool L12, int DD, bool RES, int MAXTHREADS, int MINBLOCKS>
+__global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
+    k_wilson_clover(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ U, const T* __restrict__ clover,
+                    const T* __restrict__ rhs, T kappa, FineParams P) {
+    int x[4], s;
+    if (!fine_decode(P, x, s)) return;
+    const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
 
     // neighbour sites (halo-free, modulo L) and wrap phases
     int sf[4], sb[4];
@@ -192,37 +199,9 @@ static void auto_tile(const int L[4], int tile[4]) {
         }
 }
 
-// domain == NULL: the plain operator D; otherwise D_SAP with those domains
-template <typename T>
-int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
-                       const int bc[4], const int* domain, unsigned flags, void* stream, const char* what) {
-    clear_error();
-    if (!out || !in || !U || !clover || check_dims(dims) || !bc) {
-        set_error("%s: null pointer or non-positive dim", what);
-        return LQCD_EINVAL;
-    }
-    if (!aligned16(out) || !aligned16(in) || !aligned16(U) || !aligned16(clover)) {
-        set_error("%s: pointers must be 16-byte aligned", what);
-        return LQCD_EINVAL;
-    }
-    if (out == in) {
-        set_error("%s: out must not alias in", what);
-        return LQCD_EINVAL;
-    }
-    if (rhs && (!aligned16(rhs) || domain || (flags & LQCD_DAGGER))) {
-        set_error("%s: the residual form needs an aligned rhs and takes neither a domain nor LQCD_DAGGER", what);
-        return LQCD_EINVAL;
-    }
-    const unsigned allowed = LQCD_DAGGER | LQCD_LINKS_12 | (domain ? (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD) : 0u);
-    if ((flags & ~allowed) || ((flags & LQCD_DOMAIN_EVEN) && (flags & LQCD_DOMAIN_ODD))) {
-        set_error("%s: unknown or contradictory flag bits 0x%x", what, flags);
-        return LQCD_EINVAL;
-    }
-    if (volume(dims) > 0x7fffffffLL) {
-        set_error("%s: volume exceeds 2^31-1 sites", what);
-        return LQCD_EUNSUPPORTED;
-    }
-    FineParams P;
+// Launch geometry of the fine kernels: CTA tile, tile traversal, reciprocals of the index decode.  real_bytes = 4 / 8.
+static int fine_setup(FineParams& P, long long& ntiles_out, const int dims[4], const int bc[4], const int* domain,
+                      unsigned flags, int real_bytes, const char* what) {
     for (int mu = 0; mu < 4; mu++) {
         if (bc[mu] != 1 && bc[mu] != -1) {
             set_error("%s: bc[%d] = %d not in {+1,-1}", what, mu, bc[mu]);
@@ -265,7 +244,7 @@ int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T
     } else if (g_knobs.fine_tslab < 0) {
         P.zslab = 0;
     } else {
-        const double site_bytes = 192.0 * sizeof(T);
+        const double site_bytes = 192.0 * real_bytes;
         const double slice = (double)dims[0] * dims[1] * dims[2] * site_bytes;
         P.zslab = 0;
         if (slice > 40e6) {
@@ -295,6 +274,46 @@ int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T
     P.d_per_slab.set(P.per_slab);
     P.d_zslab.set(P.zslab > 0 ? P.zslab : 1);
     for (int mu = 0; mu < 4; mu++) P.d_dom[mu].set(P.dom[mu]);
+    ntiles_out = ntiles;
+    return LQCD_OK;
+}
+
+// domain == NULL: the plain operator D; otherwise D_SAP with those domains
+template <typename T>
+int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
+                       const int bc[4], const int* domain, unsigned flags, void* stream, const char* what) {
+    clear_error();
+    if (!out || !in || !U || !clover || check_dims(dims) || !bc) {
+        set_error("%s: null pointer or non-positive dim", what);
+        return LQCD_EINVAL;
+    }
+    if (!aligned16(out) || !aligned16(in) || !aligned16(U) || !aligned16(clover)) {
+        set_error("%s: pointers must be 16-byte aligned", what);
+        return LQCD_EINVAL;
+    }
+    if (out == in) {
+        set_error("%s: out must not alias in", what);
+        return LQCD_EINVAL;
+    }
+    if (rhs && (!aligned16(rhs) || domain || (flags & LQCD_DAGGER))) {
+        set_error("%s: the residual form needs an aligned rhs and takes neither a domain nor LQCD_DAGGER", what);
+        return LQCD_EINVAL;
+    }
+    const unsigned allowed = LQCD_DAGGER | LQCD_LINKS_12 | (domain ? (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD) : 0u);
+    if ((flags & ~allowed) || ((flags & LQCD_DOMAIN_EVEN) && (flags & LQCD_DOMAIN_ODD))) {
+        set_error("%s: unknown or contradictory flag bits 0x%x", what, flags);
+        return LQCD_EINVAL;
+    }
+    if (volume(dims) > 0x7fffffffLL) {
+        set_error("%s: volume exceeds 2^31-1 sites", what);
+        return LQCD_EUNSUPPORTED;
+    }
+    FineParams P;
+    long long ntiles = 0;
+    {
+        const int rc = fine_setup(P, ntiles, dims, bc, domain, flags, (int)sizeof(T), what);
+        if (rc) return rc;
+    }
     int threads = (P.tilevol + 31) / 32 * 32;
     const bool dag = flags & LQCD_DAGGER, l12 = flags & LQCD_LINKS_12;
     cudaStream_t st = (cudaStream_t)stream;
@@ -332,6 +351,145 @@ template int wilson_clover_call<float>(float*, const float*, const float*, const
                                        const int*, const int*, const int*, unsigned, void*, const char*);
 template int wilson_clover_call<double>(double*, const double*, const double*, const double*, const double*, double,
                                         const int*, const int*, const int*, unsigned, void*, const char*);
+
+
+// ---- F4 (fine half): D on NRHS right-hand sides at once ---------------------------------------------------
+// Every link and clover block is loaded ONCE per site and applied to NRHS spinors: compulsory traffic per site drops
+// from NRHS * 768 B to 576 + NRHS * 192 B (18-real links): 1.6x less at NRHS = 2.  One thread per site as in
+// k_wilson_clover, same tile / traversal geometry; registers, not bandwidth, limit NRHS (24 accumulators per
+// right-hand side).  Right-hand side k lives at in + k * rstride (native spinors back to back).
+template <int MU, bool FWD, int SGN, bool L12, int NRHS, typename T>
+__device__ __forceinline__ void hop_mrhs(T (&acc)[NRHS][24], const T* __restrict__ in, long long rstride,
+                                         const T* __restrict__ U, int s_link, int s_nb, T ph) {
+    T u[18];
+    load_link<T, L12>(u, U, s_link, MU);
+#pragma unroll
+    for (int k = 0; k < NRHS; k++) {
+        T p[24], h[12], g[12];
+        load_spinor<T>(p, in + k * rstride, s_nb);
+        project<MU, SGN, T>(h, p);
+        su3_mult<FWD, T>(g, u, h);
+        reconstruct<MU, SGN, T>(acc[k], g, ph);
+    }
+}
+
+template <typename T, bool DAG, bool L12, int NRHS>
+__global__ void __launch_bounds__(128, sizeof(T) == 4 ? 3 : 2)
+    k_wilson_clover_mrhs(T* __restrict__ out, const T* __restrict__ in, long long rstride, const T* __restrict__ U,
+                         const T* __restrict__ clover, T kappa, FineParams P) {
+    int x[4], s;
+    if (!fine_decode(P, x, s)) return;
+    const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
+    int sf[4], sb[4];
+    T pf[4], pb[4];
+    {
+        const int stride[4] = {1, st1, st2, st3};
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const bool wf = (x[mu] == P.L[mu] - 1), wb = (x[mu] == 0);
+            sf[mu] = wf ? s - (P.L[mu] - 1) * stride[mu] : s + stride[mu];
+            sb[mu] = wb ? s + (P.L[mu] - 1) * stride[mu] : s - stride[mu];
+            pf[mu] = wf ? (T)P.bc[mu] : (T)1;
+            pb[mu] = wb ? (T)P.bc[mu] : (T)1;
+        }
+    }
+    T acc[NRHS][24];
+#pragma unroll
+    for (int k = 0; k < NRHS; k++)
+#pragma unroll
+        for (int r = 0; r < 24; r++) acc[k][r] = 0;
+    constexpr int SF = DAG ? +1 : -1, SB = DAG ? -1 : +1;
+    hop_mrhs<0, true, SF, L12, NRHS, T>(acc, in, rstride, U, s, sf[0], pf[0]);
+    hop_mrhs<0, false, SB, L12, NRHS, T>(acc, in, rstride, U, sb[0], sb[0], pb[0]);
+    hop_mrhs<1, true, SF, L12, NRHS, T>(acc, in, rstride, U, s, sf[1], pf[1]);
+    hop_mrhs<1, false, SB, L12, NRHS, T>(acc, in, rstride, U, sb[1], sb[1], pb[1]);
+    hop_mrhs<2, true, SF, L12, NRHS, T>(acc, in, rstride, U, s, sf[2], pf[2]);
+    hop_mrhs<2, false, SB, L12, NRHS, T>(acc, in, rstride, U, sb[2], sb[2], pb[2]);
+    hop_mrhs<3, true, SF, L12, NRHS, T>(acc, in, rstride, U, s, sf[3], pf[3]);
+    hop_mrhs<3, false, SB, L12, NRHS, T>(acc, in, rstride, U, sb[3], sb[3], pb[3]);
+
+    // site-diagonal part, one chirality block of the clover term at a time (loaded once for all right-hand sides)
+    constexpr int NV = VecOf<T>::NV, NH = 12 / NV;  // vec16 rows per chirality half of a spinor
+    const long long sp_off = ((long long)(s >> 5) * (24 / NV) * CH + (s & 31)) * NV;
+#pragma unroll
+    for (int chi = 0; chi < 2; chi++) {
+        T cl[36];
+        load_clover_block<T>(cl, clover, s, chi);
+#pragma unroll
+        for (int k = 0; k < NRHS; k++) {
+            T p[12], o[12];
+#pragma unroll
+            for (int j = 0; j < NH; j++) {
+                const V16<T> v = ld16(in + k * rstride + sp_off + (long long)(NH * chi + j) * CH * NV);
+#pragma unroll
+                for (int q = 0; q < NV; q++) p[j * NV + q] = v.r[q];
+            }
+#pragma unroll
+            for (int r = 0; r < 12; r++) o[r] = fma(-kappa, acc[k][12 * chi + r], p[r]);
+            herm6_madd<T>(o, cl, p);
+#pragma unroll
+            for (int j = 0; j < NH; j++) {
+                V16<T> v;
+#pragma unroll
+                for (int q = 0; q < NV; q++) v.r[q] = o[j * NV + q];
+                st16_stream(out + k * rstride + sp_off + (long long)(NH * chi + j) * CH * NV, v);
+            }
+        }
+    }
+}
+
+template <typename T>
+static int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4],
+                                   const int bc[4], int nrhs, unsigned flags, void* stream, const char* what) {
+    clear_error();
+    if (!out || !in || !U || !clover || check_dims(dims) || !bc || nrhs < 1) {
+        set_error("%s: null pointer, non-positive dim or nrhs < 1", what);
+        return LQCD_EINVAL;
+    }
+    if (!aligned16(out) || !aligned16(in) || !aligned16(U) || !aligned16(clover) || out == in) {
+        set_error("%s: pointers must be 16-byte aligned and out must not alias in", what);
+        return LQCD_EINVAL;
+    }
+    if (flags & ~(LQCD_DAGGER | LQCD_LINKS_12)) {
+        set_error("%s: unknown flag bits 0x%x", what, flags);
+        return LQCD_EINVAL;
+    }
+    if (volume(dims) > 0x7fffffffLL) {
+        set_error("%s: volume exceeds 2^31-1 sites", what);
+        return LQCD_EUNSUPPORTED;
+    }
+    FineParams P;
+    long long ntiles = 0;
+    {
+        // tiles of at most 128 sites: the kernel is compiled for 128 threads
+        const int rc = fine_setup(P, ntiles, dims, bc, nullptr, flags & (LQCD_DAGGER | LQCD_LINKS_12), (int)sizeof(T), what);
+        if (rc) return rc;
+    }
+    const long long rstride = (long long)nchunks(dims) * CH * 24;
+    const int threads = (P.tilevol + 31) / 32 * 32;
+    const bool dag = flags & LQCD_DAGGER, l12 = flags & LQCD_LINKS_12;
+    cudaStream_t st = (cudaStream_t)stream;
+    int k = 0;
+    if (threads <= 128 && g_knobs.fine_mrhs >= 0) {
+        for (; k + 2 <= nrhs; k += 2) {  // pairs of right-hand sides
+            T* o = out + k * rstride;
+            const T* i = in + k * rstride;
+            if (dag && l12) k_wilson_clover_mrhs<T, true, true, 2><<<(unsigned)ntiles, threads, 0, st>>>(o, i, rstride, U, clover, kappa, P);
+            else if (dag) k_wilson_clover_mrhs<T, true, false, 2><<<(unsigned)ntiles, threads, 0, st>>>(o, i, rstride, U, clover, kappa, P);
+            else if (l12) k_wilson_clover_mrhs<T, false, true, 2><<<(unsigned)ntiles, threads, 0, st>>>(o, i, rstride, U, clover, kappa, P);
+            else k_wilson_clover_mrhs<T, false, false, 2><<<(unsigned)ntiles, threads, 0, st>>>(o, i, rstride, U, clover, kappa, P);
+            count_launch();
+        }
+        const int rc = check_launch(what);
+        if (rc) return rc;
+    }
+    for (; k < nrhs; k++) {  // an odd one out (or a user tile of more than 128 sites): the single-right-hand-side kernel
+        const int rc = wilson_clover_call<T>(out + k * rstride, in + k * rstride, U, clover, nullptr, kappa, dims, bc,
+                                             nullptr, flags, stream, what);
+        if (rc) return rc;
+    }
+    return LQCD_OK;
+}
 
 }  // namespace lqcd
 
@@ -389,5 +547,19 @@ int lqcd_wilson_clover_residual_f64(double* r, const double* b, const double* x,
     }
     return wilson_clover_call<double>(r, x, U, clover, b, kappa, dims, bc, nullptr, flags, stream,
                                       "lqcd_wilson_clover_residual_f64");
+}
+}
+
+extern "C" {
+int lqcd_wilson_clover_mult_mrhs_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
+                                     const int dims[4], const int bc[4], int nrhs, unsigned flags, void* stream) {
+    return wilson_clover_mrhs_call<float>(out, in, U, clover, kappa, dims, bc, nrhs, flags, stream,
+                                          "lqcd_wilson_clover_mult_mrhs_f32");
+}
+int lqcd_wilson_clover_mult_mrhs_f64(double* out, const double* in, const double* U, const double* clover,
+                                     double kappa, const int dims[4], const int bc[4], int nrhs, unsigned flags,
+                                     void* stream) {
+    return wilson_clover_mrhs_call<double>(out, in, U, clover, kappa, dims, bc, nrhs, flags, stream,
+                                           "lqcd_wilson_clover_mult_mrhs_f64");
 }
 }

@@ -118,3 +118,49 @@ def test_mrhs_error_codes(lq):
     assert code(lambda: lq.coarse_mult_mrhs(y, x, d.A, cfg.cdims, 0)) == lq.EINVAL
     assert "lqcd_coarse_mult_mrhs_f32" in lq.last_error()
     assert lq.launch_count() == n0
+
+
+# ---- the fine operator on several right-hand sides -----------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("links12", [False, True])
+def test_c1_fine_mrhs(lq, prec, links12):
+    import torch
+    from problems import make_problem
+    prob = make_problem(li.CONFIGS["c1"], n_rhs=5, coarse="none")
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec, links12=links12, coarse=False)
+    x = torch.stack([lq.pack_spinor(to_dev(p, prec), cfg.dims) for p in prob.psi])
+    for dagger in (False, True):
+        y = torch.full_like(x, 4.0)
+        n0 = lq.launch_count()
+        lq.wilson_clover_mult_mrhs(y, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, dagger=dagger, links12=links12)
+        assert lq.launch_count() - n0 == 3, "two pairs and one odd right-hand side"
+        for k in range(5):
+            ref = oracle.wilson_clover_mult(rounded(prob.psi[k], prec), rounded(prob.U, prec), rounded(prob.clover, prec),
+                                            cfg.kappa, cfg.dims, cfg.bc, dagger=dagger)
+            assert rel_l2(lq.unpack_spinor(y[k], cfg.dims).cpu().numpy(), ref) <= TOL[prec], (k, dagger)
+    # the pair kernel and the single-right-hand-side kernel do the same arithmetic in the same order: bit-identical
+    y1 = torch.empty_like(x)
+    lq.set_knob("fine_mrhs", -1)
+    try:
+        lq.wilson_clover_mult_mrhs(y1, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, dagger=True, links12=links12)
+    finally:
+        lq.set_knob("fine_mrhs", 0)
+    assert torch.equal(y, y1)
+
+
+@pytest.mark.parametrize("dims,bc", [((3, 3, 3, 3), (1, 1, 1, -1)), ((6, 4, 2, 10), (-1, 1, -1, 1)),
+                                     ((16, 8, 8, 8), (1, 1, 1, -1))])
+def test_fine_mrhs_edge_lattices(lq, dims, bc):
+    import torch
+    from problems import custom_config, make_problem
+    cfg = custom_config(dims, (1, 1, 1, 1), 1, bc=bc)
+    prob = make_problem(cfg, n_rhs=2, coarse="none")
+    d = Dev(lq, prob, "f32", coarse=False)
+    x = torch.stack([lq.pack_spinor(to_dev(p, "f32"), dims) for p in prob.psi])
+    y = torch.full_like(x, 4.0)
+    lq.wilson_clover_mult_mrhs(y, x, d.U, d.clover, cfg.kappa, dims, bc)
+    for k in range(2):
+        ref = oracle.wilson_clover_mult(rounded(prob.psi[k], "f32"), rounded(prob.U, "f32"), rounded(prob.clover, "f32"),
+                                        cfg.kappa, dims, bc)
+        assert rel_l2(lq.unpack_spinor(y[k], dims).cpu().numpy(), ref) <= TOL["f32"], k
