@@ -202,3 +202,110 @@ def test_fullsize_restrict_prolong_sampled(lq, name):
     lhs = torch.sum(torch.conj(out_c.to(torch.complex128)) * xc.to(torch.complex128))
     rhs = torch.sum(torch.conj(psi.to(torch.complex128)) * lq.unpack_spinor(out_f, L).to(torch.complex128))
     assert abs((lhs - rhs).item()) <= 1e-5 * abs(lhs.item())
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# F3 / F4 at full size
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_fullsize_mr_domain_and_sap_sampled(lq, name):
+    """The inner-domain solver is domain-local: 16 sampled 4^4 domains (both lattice corners included) are gathered
+    into a fake 8^4 lattice of 2^4 domains on which the oracle runs as it stands (hops between domains are cut, so the
+    fake neighbourhood is irrelevant).  Then SAP at full size: properties that hold at any size."""
+    import torch
+    cfg = li.CONFIGS[name]
+    L, dom, V, Lc = cfg.dims, cfg.block, cfg.volume, cfg.cdims
+    assert tuple(dom) == (4, 4, 4, 4)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed + 3)
+    rng = np.random.default_rng(cfg.seed + 3)
+    U = li.t_gauge_field(cfg, gen, "cuda").to(torch.complex64)
+    cl = li.t_clover_synthetic(gen, V, "cuda")
+    r = li.t_spinor(gen, V, "cuda", torch.float32)
+    U18, Cn, rn = lq.pack_gauge(U, L), lq.pack_clover(cl, L), lq.pack_spinor(r, L)
+    Lca = np.array(Lc)
+    Xs = np.stack([rng.integers(0, Lca[mu], 16) for mu in range(4)], axis=1)
+    Xs[0] = 0
+    Xs[1] = Lca - 1
+    fdims = (8, 8, 8, 8)
+    fc = li.site_coords(fdims)
+    k = site_index((2, 2, 2, 2), fc // 4)
+    real = site_index(L, Xs[k] * 4 + fc % 4)
+    real_d = torch.from_numpy(real.astype(np.int64)).cuda()
+    U_f = U[:, real_d].cpu().numpy()
+    cl_f = cl[real_d].cpu().numpy()
+    r_f = r[real_d].cpu().numpy()
+    ref = oracle.mr_domain_solve(r_f, U_f, cl_f, cfg.kappa, fdims, (1, 1, 1, 1), dom, 0, 6)
+    z = lq.empty_spinor(L)
+    z.fill_(1.0)
+    lq.mr_domain_solve(z, rn, U18, Cn, cfg.kappa, L, cfg.bc, dom, parity=0, niter=6)   # resident kernel, all domains
+    got = lq.unpack_spinor(z, L)[real_d].cpu().numpy()
+    assert rel_l2(got, ref) <= 6 * TOL32
+    # the half-grid accumulate form SAP uses: x += M^(e) r changes exactly the even domains, by the same z
+    x = lq.pack_spinor(li.t_spinor(gen, V, "cuda", torch.float32), L)
+    x0 = lq.unpack_spinor(x, L).clone()
+    lq.mr_domain_solve(x, rn, U18, Cn, cfg.kappa, L, cfg.bc, dom, parity=1, niter=6, accumulate=True)
+    dx = (lq.unpack_spinor(x, L) - x0)[real_d].cpu().numpy()
+    even = (Xs.sum(axis=1) % 2 == 0)[k]
+    assert not np.any(dx[~even]), "odd domains untouched, bit for bit"
+    assert rel_l2(dx[even], ref[even]) <= 10 * TOL32   # (x0 + z) - x0: one more rounding on the scale of x0
+    del x0, dx
+    # SAP(2, 6) at full size: the residual it returns is b - D x of the x it returns (same kernel: bit-identical),
+    # and every quantity is finite and smaller than the right-hand side
+    xs, rs, chk = lq.empty_spinor(L), lq.empty_spinor(L), lq.empty_spinor(L)
+    lq.sap(xs, rs, rn, U18, Cn, cfg.kappa, L, cfg.bc, dom, n_sap=2, n_mr=6)
+    lq.wilson_clover_residual(chk, rn, xs, U18, Cn, cfg.kappa, L, cfg.bc)
+    assert torch.equal(rs, chk)
+    nb, nr = torch.linalg.vector_norm(rn.double()).item(), torch.linalg.vector_norm(rs.double()).item()
+    assert np.isfinite(nr) and nr < 0.5 * nb, (nr, nb)
+
+
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_fullsize_mrhs_sampled(lq, name):
+    """F4 in bench.py's configuration: 16 coarse right-hand sides through the tensor-core kernel, sampled sites
+    against the oracle; the pair kernel of the fine operator against the (sample-checked) single kernel."""
+    import torch
+    cfg = li.CONFIGS[name]
+    Lc, Vc, nv = cfg.cdims, cfg.cvolume, cfg.nvec
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed + 4)
+    A = li.t_coarse_matrix_synthetic(gen, Vc, nv, "cuda")
+    K = 16
+    xs = torch.view_as_complex(torch.randn((K, Vc, 2, nv, 2), generator=gen, device="cuda", dtype=torch.float32))
+    ys = torch.empty_like(xs)
+    lq.coarse_mult_mrhs(ys, xs, A, Lc, nv)
+    rng = np.random.default_rng(cfg.seed + 4)
+    Lca = np.array(Lc)
+    corners = np.array([[x, y, z, t] for x in (0, Lca[0] - 1) for y in (0, Lca[1] - 1) for z in (0, Lca[2] - 1)
+                        for t in (0, Lca[3] - 1)])
+    rnd = np.stack([rng.integers(0, Lca[mu], 48) for mu in range(4)], axis=1)
+    sites = site_index(Lc, np.concatenate([corners, rnd])).astype(np.int64)
+    sites_d = torch.from_numpy(sites).cuda()
+    A_s = A[sites_d].cpu().numpy()
+    for k in (0, 7, 15):
+        ref = oracle.coarse_mult_sites(xs[k].cpu().numpy(), A_s, Lc, sites)
+        got = ys[k][sites_d].cpu().numpy()
+        assert rel_l2(got, ref) <= TOL32, k
+        per_site = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / np.linalg.norm(
+            ref.reshape(len(sites), -1), axis=1)
+        assert per_site.max() <= 5 * TOL32, k
+    # every right-hand side, every site: agreement with the single-right-hand-side kernel to fp32 rounding
+    y1 = torch.empty_like(xs[0])
+    for k in range(K):
+        lq.coarse_mult(y1, xs[k].contiguous(), A, Lc, nv)
+        err = torch.linalg.vector_norm((ys[k] - y1).to(torch.complex128)) / torch.linalg.vector_norm(y1.to(torch.complex128))
+        assert err.item() <= TOL32, k
+    del A, xs, ys
+    # fine operator on a pair of right-hand sides: bit-identical with two single applications
+    L, V = cfg.dims, cfg.volume
+    U = li.t_gauge_field(cfg, gen, "cuda").to(torch.complex64)
+    U18 = lq.pack_gauge(U, L)
+    del U
+    Cn = lq.pack_clover(li.t_clover_synthetic(gen, V, "cuda"), L)
+    x2 = torch.stack([lq.pack_spinor(li.t_spinor(gen, V, "cuda", torch.float32), L) for _ in range(2)])
+    y2, ys1 = torch.empty_like(x2), lq.empty_spinor(L)
+    for dag in (False, True):
+        lq.wilson_clover_mult_mrhs(y2, x2, U18, Cn, cfg.kappa, L, cfg.bc, dagger=dag)
+        for k in range(2):
+            lq.wilson_clover_mult(ys1, x2[k], U18, Cn, cfg.kappa, L, cfg.bc, dagger=dag)
+            assert torch.equal(y2[k], ys1), (dag, k)

@@ -164,3 +164,20 @@ def test_fine_mrhs_edge_lattices(lq, dims, bc):
         ref = oracle.wilson_clover_mult(rounded(prob.psi[k], "f32"), rounded(prob.U, "f32"), rounded(prob.clover, "f32"),
                                         cfg.kappa, dims, bc)
         assert rel_l2(lq.unpack_spinor(y[k], dims).cpu().numpy(), ref) <= TOL["f32"], k
+
+
+def test_tensor_core_path_coarse_extent_two(lq):
+    """8^4 blocked 4^4 with N_nv = 32: coarse extent 2 in every direction (X + mu == X - mu: the forward and the
+    backward block multiply the SAME neighbour vector), 16 coarse sites only -- fewer sites than SMs, one per CTA."""
+    from problems import custom_config, make_problem
+    cfg = custom_config((8, 8, 8, 8), (4, 4, 4, 4), 32, bc=(1, 1, 1, -1), kappa=0.135, csw=1.0)
+    prob = make_problem(cfg)
+    d = Dev(lq, prob, "f32")
+    xs = rhs_set(cfg, 6)
+    n0 = lq.launch_count()
+    got = gpu_mrhs(lq, d, xs)
+    assert lq.launch_count() - n0 == 1
+    A = rounded(prob.A, "f32")
+    for k in range(6):
+        ref = oracle.coarse_mult(rounded(xs[k], "f32"), A, cfg.cdims)
+        assert rel_l2(got[k], ref) <= TOL["f32"], k
