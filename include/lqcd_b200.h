@@ -161,6 +161,13 @@ int lqcd_restrict_f32(float* out_c, const float* in_f, const float* nullvecs, co
                       const int block[4], int nvec, void* stream);
 int lqcd_restrict_f64(double* out_c, const double* in_f, const double* nullvecs, const int dims[4],
                       const int block[4], int nvec, void* stream);
+/* Restriction of nrhs fine vectors at once (native spinors back to back -> coarse vectors back to back): the null
+ * vectors, 97 % of a restriction's traffic, are streamed once per group of up to 9 vectors (as many slices of a 4^4
+ * aggregate as fit in shared memory).  Used by the Galerkin assembly (the nine pieces of D of one column). */
+int lqcd_restrict_mrhs_f32(float* out_c, const float* in_f, const float* nullvecs, const int dims[4],
+                           const int block[4], int nvec, int nrhs, void* stream);
+int lqcd_restrict_mrhs_f64(double* out_c, const double* in_f, const double* nullvecs, const int dims[4],
+                           const int block[4], int nvec, int nrhs, void* stream);
 /* ---- A5: prolongation, Eq. 6:  out_f(x,alpha,c) = sum_i v_i(x,alpha,c) in_c[X(x)][chi(alpha)][i];
  * overwrites out_f (no accumulate). */
 int lqcd_prolong_f32(float* out_f, const float* in_c, const float* nullvecs, const int dims[4],
@@ -188,7 +195,7 @@ int lqcd_orthonormalize_blocks_f64(double* nullvecs, const int dims[4], const in
  * site-diagonal term and the hops inside the aggregate; 1 + 2 mu / 2 + 2 mu: the forward / backward hops that leave
  * it), coarse-matrix layout as consumed by lqcd_coarse_mult.  U: native 18-real gauge; nullvecs: native, block-
  * orthonormal.  ws_dev: device scratch of lqcd_galerkin_workspace_bytes(dims, block, nvec, sizeof(real)) bytes.
- * Built column by column from the hot-path kernels: 2 nvec * 28 launches. */
+ * Built column by column from the hot-path kernels: 2 nvec * 20 launches (one multi-vector restriction per column). */
 size_t lqcd_galerkin_workspace_bytes(const int dims[4], const int block[4], int nvec, int real_bytes);
 int lqcd_galerkin_coarse_f32(float* A, const float* U, const float* clover, const float* nullvecs, float kappa,
                              const int dims[4], const int bc[4], const int block[4], int nvec, void* ws_dev,

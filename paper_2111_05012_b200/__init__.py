@@ -422,6 +422,14 @@ def wilson_clover_mult_mrhs(out, inp, U, clover, kappa, dims, bc, dagger=False, 
            "lqcd_wilson_clover_mult_mrhs")
     return out
 
+def restrict_mrhs(out_c, in_f, nullvecs, dims, block, nvec, stream=None):
+    """Eq. 5 for several fine vectors at once: in_f (K, native spinor), out_c (K, Vc, 2, nvec)."""
+    sfx = _same_dtype(out_c, in_f, nullvecs)
+    _check(getattr(lib(), f"lqcd_restrict_mrhs_{sfx}")(_dev_ptr(out_c), _dev_ptr(in_f), _dev_ptr(nullvecs), _i4(dims),
+                                                       _i4(block), int(nvec), int(in_f.shape[0]), _stream(stream)),
+           "lqcd_restrict_mrhs")
+    return out_c
+
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):

@@ -402,7 +402,8 @@ static inline size_t up256(size_t n) { return (n + 255) & ~(size_t)255; }
 template <typename T> static size_t galerkin_ws_bytes(const int dims[4], const int block[4], int nvec) {
     int cd[4];
     if (check_block(dims, block, nvec, cd)) return 0;
-    return 2 * up256((size_t)nchunks(dims) * CH * 24 * sizeof(T)) + up256((size_t)volume(cd) * 4 * nvec * sizeof(T));
+    // one column of P, its nine images under the pieces of D, their nine restrictions
+    return up256(10 * (size_t)nchunks(dims) * CH * 24 * sizeof(T) + 9 * (size_t)volume(cd) * 4 * nvec * sizeof(T));
 }
 
 template <typename T> int dd_mult(T*, const T*, const T*, const T*, T, const int*, const int*, const int*, void*);
@@ -414,15 +415,10 @@ template <> int dd_mult<double>(double* o, const double* i, const double* U, con
                                 const int* bc, const int* b, void* st) {
     return lqcd_wilson_clover_dd_mult_f64(o, i, U, c, k, d, bc, b, 0, st);
 }
-template <typename T> int restrict_mult(T*, const T*, const T*, const int*, const int*, int, void*);
-template <> int restrict_mult<float>(float* o, const float* i, const float* v, const int* d, const int* b, int n,
-                                     void* st) {
-    return lqcd_restrict_f32(o, i, v, d, b, n, st);
-}
-template <> int restrict_mult<double>(double* o, const double* i, const double* v, const int* d, const int* b, int n,
-                                      void* st) {
-    return lqcd_restrict_f64(o, i, v, d, b, n, st);
-}
+// (transfer.cu) nrhs fine vectors back to back -> nrhs coarse vectors back to back, null vectors streamed once per group
+template <typename T>
+int restrict_mrhs_call(T* out_c, const T* in_f, const T* v, const int dims[4], const int block[4], int nvec, int nrhs,
+                       void* stream, const char* what);
 
 template <typename T>
 static int galerkin_call(T* A, const T* U, const T* clover, const T* v, T kappa, const int dims[4], const int bc[4],
@@ -447,11 +443,12 @@ static int galerkin_call(T* A, const T* U, const T* clover, const T* v, T kappa,
     }
     H.V = (int)volume(dims);
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t fine_b = up256((size_t)nchunks(dims) * CH * 24 * sizeof(T));
-    T* col = (T*)ws;
-    T* img = (T*)((char*)ws + fine_b);
-    T* xc = (T*)((char*)ws + 2 * fine_b);
     const long long Vc = volume(P.Lc);
+    // vectors back to back, as restrict_mrhs_call expects them (every size is a multiple of 16 bytes)
+    const long long fstride = (long long)nchunks(dims) * CH * 24, cstride = Vc * 4 * nvec;
+    T* col = (T*)ws;
+    T* img = col + fstride;        // nine images
+    T* xc = col + 10 * fstride;    // nine restrictions
     const int N = 2 * nvec;
     const unsigned hop_grid = (unsigned)((H.V + 127) / 128);
     long long sgrid = (Vc * N + 255) / 256;
@@ -459,26 +456,20 @@ static int galerkin_call(T* A, const T* U, const T* clover, const T* v, T kappa,
     for (int J = 0; J < N; J++) {
         k_prolongator_column<T><<<(unsigned)Vc, 256, 0, st>>>(col, v, J / nvec, J % nvec, P);
         count_launch();
-        for (int d = 0; d < 9; d++) {
-            if (d == 0) {
-                if ((rc = dd_mult<T>(img, col, U, clover, kappa, dims, bc, block, stream))) return rc;
-            } else {
-                switch (d) {
-                    case 1: k_hop_cross<T, 0, true><<<hop_grid, 128, 0, st>>>(img, col, U, kappa, H); break;
-                    case 2: k_hop_cross<T, 0, false><<<hop_grid, 128, 0, st>>>(img, col, U, kappa, H); break;
-                    case 3: k_hop_cross<T, 1, true><<<hop_grid, 128, 0, st>>>(img, col, U, kappa, H); break;
-                    case 4: k_hop_cross<T, 1, false><<<hop_grid, 128, 0, st>>>(img, col, U, kappa, H); break;
-                    case 5: k_hop_cross<T, 2, true><<<hop_grid, 128, 0, st>>>(img, col, U, kappa, H); break;
-                    case 6: k_hop_cross<T, 2, false><<<hop_grid, 128, 0, st>>>(img, col, U, kappa, H); break;
-                    case 7: k_hop_cross<T, 3, true><<<hop_grid, 128, 0, st>>>(img, col, U, kappa, H); break;
-                    default: k_hop_cross<T, 3, false><<<hop_grid, 128, 0, st>>>(img, col, U, kappa, H); break;
-                }
-                count_launch();
-            }
-            if ((rc = restrict_mult<T>(xc, img, v, dims, block, nvec, stream))) return rc;
-            k_scatter_column<T><<<(unsigned)sgrid, 256, 0, st>>>(A, xc, d, J, N, Vc);
-            count_launch();
-        }
+        if ((rc = dd_mult<T>(img, col, U, clover, kappa, dims, bc, block, stream))) return rc;
+        k_hop_cross<T, 0, true><<<hop_grid, 128, 0, st>>>(img + 1 * fstride, col, U, kappa, H);
+        k_hop_cross<T, 0, false><<<hop_grid, 128, 0, st>>>(img + 2 * fstride, col, U, kappa, H);
+        k_hop_cross<T, 1, true><<<hop_grid, 128, 0, st>>>(img + 3 * fstride, col, U, kappa, H);
+        k_hop_cross<T, 1, false><<<hop_grid, 128, 0, st>>>(img + 4 * fstride, col, U, kappa, H);
+        k_hop_cross<T, 2, true><<<hop_grid, 128, 0, st>>>(img + 5 * fstride, col, U, kappa, H);
+        k_hop_cross<T, 2, false><<<hop_grid, 128, 0, st>>>(img + 6 * fstride, col, U, kappa, H);
+        k_hop_cross<T, 3, true><<<hop_grid, 128, 0, st>>>(img + 7 * fstride, col, U, kappa, H);
+        k_hop_cross<T, 3, false><<<hop_grid, 128, 0, st>>>(img + 8 * fstride, col, U, kappa, H);
+        count_launch(8);
+        // the nine restrictions in one pass over the null vectors (they are 97 % of a restriction's traffic)
+        if ((rc = restrict_mrhs_call<T>(xc, img, v, dims, block, nvec, 9, stream, what))) return rc;
+        for (int d = 0; d < 9; d++) k_scatter_column<T><<<(unsigned)sgrid, 256, 0, st>>>(A, xc + d * cstride, d, J, N, Vc);
+        count_launch(9);
     }
     return check_launch(what);
 }

@@ -181,3 +181,27 @@ def test_tensor_core_path_coarse_extent_two(lq):
     for k in range(6):
         ref = oracle.coarse_mult(rounded(xs[k], "f32"), A, cfg.cdims)
         assert rel_l2(got[k], ref) <= TOL["f32"], k
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("name,nrhs", [("c1", 11), ("c2", 5), ("c3", 9)])
+def test_restrict_mrhs(lq, prec, name, nrhs):
+    """several fine vectors restricted in one pass over the null vectors; groups of up to 9, ragged last group"""
+    import torch
+    if name == "c3" and prec == "f64":
+        pytest.skip("config 3 is an fp32 config")
+    prob = config_problem(name)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    rng = np.random.default_rng(9)
+    psis = [rng.standard_normal((cfg.volume, 4, 3)) + 1j * rng.standard_normal((cfg.volume, 4, 3)) for _ in range(nrhs)]
+    x = torch.stack([lq.pack_spinor(to_dev(p, prec), cfg.dims) for p in psis])
+    out = torch.full((nrhs, cfg.cvolume, 2, cfg.nvec), 3.0, dtype=to_dev(np.zeros(1), prec).dtype, device="cuda")
+    lq.restrict_mrhs(out, x, d.v, cfg.dims, cfg.block, cfg.nvec)
+    got = out.cpu().numpy()
+    one = torch.empty_like(out[0])
+    for k in range(nrhs):
+        ref = oracle.restrict(rounded(psis[k], prec), rounded(prob.v, prec), cfg.dims, cfg.block)
+        assert rel_l2(got[k], ref) <= TOL[prec], k
+        lq.restrict(one, x[k], d.v, cfg.dims, cfg.block, cfg.nvec)
+        assert rel_l2(got[k], one.cpu().numpy()) <= TOL[prec]
