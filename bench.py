@@ -323,6 +323,14 @@ class Workload:
         c = self.cfg
         self.lq.coarse_mult_mrhs(self.ycK, self.xcK, self.A, c.cdims, c.nvec)
 
+    def bicg_mrhs(self, i):
+        c = self.cfg
+        self.lq.coarse_bicgstab_mrhs(self.ycK, self.xcK, self.A, c.cdims, c.nvec, 8, ws=self.bicg_ws)
+
+    def bicg_single(self, i):
+        c = self.cfg
+        self.lq.coarse_bicgstab(self.ycK[i % 4], self.xcK[i % 4], self.A, c.cdims, c.nvec, 8, ws=self.bicg_ws)
+
     def vcycle(self, i):
         c = self.cfg
         self.lq.mg_vcycle(self.y[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, c.block, c.nvec, self.v,
@@ -635,7 +643,16 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "speedup_vs_16_single_applications": K * kernels["coarse_mult"]["us"] * 1e-6 / t,
             "frac_of_hbm_peak": (mc["bytes"] + vec_b) / t / 1e9 / peak, "bytes_per_launch": mc["bytes"] + vec_b,
             "path": "tcgen05 kind::tf32, hi/lo split of both operands (3xTF32), fp32 accumulation"}
-        del W.xcK, W.ycK
+        # the coarse solver (1b) on the same 16 right-hand sides: 8 BiCGStab iterations, batched (D_c through the
+        # tensor-core kernel) against one right-hand side at a time
+        nb = int(W.lq.lib().lqcd_coarse_bicgstab_mrhs_workspace_bytes(W.lq._i4(cfg.cdims), cfg.nvec, K, 4))
+        W.bicg_ws = torch.empty(nb, dtype=torch.uint8, device=W.dev)
+        t1 = time_single(W, "bicg_single", reps=3, warmup=1)
+        tk = time_single(W, "bicg_mrhs", reps=3, warmup=1)
+        extra["coarse_bicgstab_mrhs_16x8"] = {"us": tk * 1e6, "us_single_rhs": t1 * 1e6,
+                                               "speedup_vs_16_single_solves": K * t1 / tk,
+                                               "GFLOPs": K * 16 * mc["flops"] / tk / 1e9}
+        del W.xcK, W.ycK, W.bicg_ws
         # F4, fine half: D on two right-hand sides at once (links and clover read once for both)
         W.x2 = [torch.stack([W.x[0], W.x[1]]), torch.stack([W.x[2], W.x[3]])]
         W.y2 = [torch.empty_like(W.x2[0]), torch.empty_like(W.x2[1])]

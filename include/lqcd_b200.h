@@ -279,6 +279,16 @@ int lqcd_coarse_bicgstab_f32(float* x, float* r_out, const float* b, const float
 int lqcd_coarse_bicgstab_f64(double* x, double* r_out, const double* b, const double* A, const int cdims[4], int nvec,
                              int niter, void* ws_dev, void* stream);
 
+/* The same for nrhs right-hand sides at once (x, r_out, b: nrhs coarse vectors back to back): nrhs independent
+ * recurrences -- every right-hand side has its own alpha, omega, beta -- that share the applications of D_c through
+ * lqcd_coarse_mult_mrhs, i.e. ONE pass over A per application for up to 16 right-hand sides (tensor cores, fp32,
+ * N = 64).  Result k is what lqcd_coarse_bicgstab gives for b_k, up to rounding. */
+size_t lqcd_coarse_bicgstab_mrhs_workspace_bytes(const int cdims[4], int nvec, int nrhs, int real_bytes);
+int lqcd_coarse_bicgstab_mrhs_f32(float* x, float* r_out, const float* b, const float* A, const int cdims[4], int nvec,
+                                  int nrhs, int niter, void* ws_dev, void* stream);
+int lqcd_coarse_bicgstab_mrhs_f64(double* x, double* r_out, const double* b, const double* A, const int cdims[4],
+                                  int nvec, int nrhs, int niter, void* ws_dev, void* stream);
+
 /* One V-cycle x = M b of the multigrid preconditioner, two Richardson refinements
  * "|x> + M_i(|b> - D|x>) -> |x>" from |x> = 0:
  *   (1) M_1 = prolong o BiCGStab(D_c, n_coarse iterations) o restrict     steps (1a)-(1c)

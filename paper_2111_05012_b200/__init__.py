@@ -430,6 +430,19 @@ def restrict_mrhs(out_c, in_f, nullvecs, dims, block, nvec, stream=None):
            "lqcd_restrict_mrhs")
     return out_c
 
+def coarse_bicgstab_mrhs(x, b, A, cdims, nvec, niter, r_out=None, ws=None, stream=None):
+    """niter BiCGStab iterations for D_c x_k = b_k, all k at once; x, b of shape (K, Vc, 2, nvec)."""
+    sfx = _same_dtype(x, b, A)
+    nrhs = int(b.shape[0])
+    if ws is None:
+        nb = int(lib().lqcd_coarse_bicgstab_mrhs_workspace_bytes(_i4(cdims), int(nvec), nrhs,
+                                                                 4 if sfx == "f32" else 8))
+        ws = torch.empty(nb, dtype=torch.uint8, device=x.device)
+    _check(getattr(lib(), f"lqcd_coarse_bicgstab_mrhs_{sfx}")(_dev_ptr(x), _ws_ptr(r_out), _dev_ptr(b), _dev_ptr(A),
+                                                              _i4(cdims), int(nvec), nrhs, int(niter), _dev_ptr(ws),
+                                                              _stream(stream)), "lqcd_coarse_bicgstab_mrhs")
+    return x
+
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):

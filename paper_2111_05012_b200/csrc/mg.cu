@@ -36,12 +36,16 @@ template <typename T> __device__ __forceinline__ Cx<T> cquot(Cx<T> n, Cx<T> d) {
     return {(n.re * d.re + n.im * d.im) / m, (n.im * d.re - n.re * d.im) / m};
 }
 
-// Sum of the RED_CTAS partial triples in a fixed order, same bits in every thread of every CTA.
-// Must be called by all threads of the CTA.  scratch: 3 values of shared memory.
-template <typename T> __device__ __forceinline__ void sum_partials(T out[3], const T* __restrict__ part, T* scratch) {
+// Batched form: every kernel below is launched with grid (nred, K): blockIdx.y is the right-hand side, whose vectors
+// lie K-fold back to back (2 n reals apart), whose partial sums are part + y * nred * 3 and whose scalars sc + y * 8.
+// Sum of the gridDim.x partial triples of this right-hand side in a fixed order, same bits in every thread of every
+// CTA.  Must be called by all threads of the CTA.  scratch: 3 values of shared memory.
+template <typename T>
+__device__ __forceinline__ void sum_partials(T out[3], const T* __restrict__ part, T* scratch, int nred) {
+    part += (long long)blockIdx.y * nred * 3;
     if (threadIdx.x < 32) {
         T s[3] = {0, 0, 0};
-        for (int i = threadIdx.x; i < RED_CTAS; i += 32) {
+        for (int i = threadIdx.x; i < nred; i += 32) {
             s[0] += part[3 * i];
             s[1] += part[3 * i + 1];
             s[2] += part[3 * i + 2];
@@ -75,7 +79,7 @@ template <typename T> __device__ __forceinline__ void write_partial(T d[3], T* _
         for (int q = 0; q < 3; q++) {
             T s = 0;
             for (int i = 0; i < RED_THREADS / 32; i++) s += red[i * 3 + q];
-            part[3 * blockIdx.x + q] = s;
+            part[3 * ((long long)blockIdx.y * gridDim.x + blockIdx.x) + q] = s;
         }
     }
 }
@@ -86,7 +90,9 @@ __global__ void __launch_bounds__(RED_THREADS) k_cdot(T* __restrict__ part, cons
                                                        const T* __restrict__ b, long long n) {
     __shared__ T red[RED_THREADS / 32 * 3];
     T d[3] = {0, 0, 0};
-    for (long long k = blockIdx.x * (long long)RED_THREADS + threadIdx.x; k < n; k += (long long)RED_CTAS * RED_THREADS) {
+    a += (long long)blockIdx.y * 2 * n;
+    b += (long long)blockIdx.y * 2 * n;
+    for (long long k = blockIdx.x * (long long)RED_THREADS + threadIdx.x; k < n; k += (long long)gridDim.x * RED_THREADS) {
         const T ar = a[2 * k], ai = a[2 * k + 1], br = b[2 * k], bi = b[2 * k + 1];
         d[0] = fma(ar, br, d[0]);
         d[0] = fma(ai, bi, d[0]);
@@ -99,10 +105,12 @@ __global__ void __launch_bounds__(RED_THREADS) k_cdot(T* __restrict__ part, cons
 }
 
 // rho[0] = sum of the partials (one CTA)
-template <typename T> __global__ void __launch_bounds__(32) k_set_rho(T* __restrict__ sc, const T* __restrict__ part) {
+template <typename T>
+__global__ void __launch_bounds__(32) k_set_rho(T* __restrict__ sc, const T* __restrict__ part, int nred) {
     __shared__ T scratch[3];
     T s[3];
-    sum_partials<T>(s, part, scratch);
+    sum_partials<T>(s, part, scratch, nred);
+    sc += blockIdx.y * SC_COUNT;
     if (threadIdx.x == 0) {
         sc[SC_RHO] = s[0];
         sc[SC_RHO + 1] = s[1];
@@ -116,7 +124,11 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_s(T* __restrict__ s, const
                                                          T* __restrict__ sc, int it, long long n) {
     __shared__ T scratch[3];
     T d[3];
-    sum_partials<T>(d, part, scratch);
+    sum_partials<T>(d, part, scratch, gridDim.x);
+    sc += blockIdx.y * SC_COUNT;
+    s += (long long)blockIdx.y * 2 * n;
+    r += (long long)blockIdx.y * 2 * n;
+    v += (long long)blockIdx.y * 2 * n;
     const Cx<T> rho = {sc[SC_RHO + 2 * (it & 1)], sc[SC_RHO + 2 * (it & 1) + 1]};
     const Cx<T> alpha = cquot<T>(rho, {d[0], d[1]});
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -140,7 +152,12 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(T* __restrict__ x, T* _
     __shared__ T scratch[3];
     __shared__ T red[RED_THREADS / 32 * 3];
     T d[3];
-    sum_partials<T>(d, part_in, scratch);
+    sum_partials<T>(d, part_in, scratch, gridDim.x);
+    sc += blockIdx.y * SC_COUNT;
+    {
+        const long long bo = (long long)blockIdx.y * 2 * n;
+        x += bo; r += bo; p += bo; s += bo; t += bo; rt += bo;
+    }
     const Cx<T> omega = cquot<T>({d[0], d[1]}, {d[2], 0});
     const Cx<T> alpha = {sc[SC_ALPHA], sc[SC_ALPHA + 1]};
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -148,7 +165,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(T* __restrict__ x, T* _
         sc[SC_OMEGA + 1] = omega.im;
     }
     T q[3] = {0, 0, 0};
-    for (long long k = blockIdx.x * (long long)RED_THREADS + threadIdx.x; k < n; k += (long long)RED_CTAS * RED_THREADS) {
+    for (long long k = blockIdx.x * (long long)RED_THREADS + threadIdx.x; k < n; k += (long long)gridDim.x * RED_THREADS) {
         const Cx<T> sk = {s[2 * k], s[2 * k + 1]};
         const Cx<T> ap = cmul<T>(alpha, {p[2 * k], p[2 * k + 1]}), os = cmul<T>(omega, sk);
         const Cx<T> ot = cmul<T>(omega, {t[2 * k], t[2 * k + 1]});
@@ -175,7 +192,12 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_p(T* __restrict__ p_out, c
                                                          long long n) {
     __shared__ T scratch[3];
     T d[3];
-    sum_partials<T>(d, part, scratch);
+    sum_partials<T>(d, part, scratch, gridDim.x);
+    sc += blockIdx.y * SC_COUNT;
+    {
+        const long long bo = (long long)blockIdx.y * 2 * n;
+        p_out += bo; p_in += bo; r += bo; v += bo;
+    }
     const Cx<T> rho = {sc[SC_RHO + 2 * (it & 1)], sc[SC_RHO + 2 * (it & 1) + 1]};
     const Cx<T> alpha = {sc[SC_ALPHA], sc[SC_ALPHA + 1]}, omega = {sc[SC_OMEGA], sc[SC_OMEGA + 1]};
     const Cx<T> rho_new = {d[0], d[1]};
@@ -195,15 +217,23 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_p(T* __restrict__ p_out, c
 // ---- host side ----------------------------------------------------------------------------------------------------
 static size_t align256(size_t b) { return (b + 255) / 256 * 256; }
 
-template <typename T> struct BicgWs {  // carve-up of the caller's scratch
+// partial sums per dot product and right-hand side: 2 x 148 CTAs for one vector, fewer each for a batch
+static int red_ctas(int nrhs) {
+    int n = 2 * RED_CTAS / nrhs;
+    if (n > RED_CTAS) n = RED_CTAS;
+    if (n < 8) n = 8;
+    return n;
+}
+
+template <typename T> struct BicgWs {  // carve-up of the caller's scratch (K vectors back to back each)
     T *v, *s, *t, *p, *r, *part_a, *part_b, *sc;
-    static size_t bytes(long long n) {
-        return 5 * align256((size_t)n * 2 * sizeof(T)) + 2 * align256(RED_CTAS * 3 * sizeof(T)) +
-               align256(SC_COUNT * sizeof(T));
+    static size_t bytes(long long n, int K) {
+        return 5 * align256((size_t)n * 2 * sizeof(T) * K) + 2 * align256((size_t)red_ctas(K) * K * 3 * sizeof(T)) +
+               align256((size_t)SC_COUNT * K * sizeof(T));
     }
-    void carve(void* ws, long long n) {
+    void carve(void* ws, long long n, int K) {
         char* c = reinterpret_cast<char*>(ws);
-        const size_t vb = align256((size_t)n * 2 * sizeof(T)), pb = align256(RED_CTAS * 3 * sizeof(T));
+        const size_t vb = align256((size_t)n * 2 * sizeof(T) * K), pb = align256((size_t)red_ctas(K) * K * 3 * sizeof(T));
         v = (T*)c; c += vb;
         s = (T*)c; c += vb;
         t = (T*)c; c += vb;
@@ -215,23 +245,29 @@ template <typename T> struct BicgWs {  // carve-up of the caller's scratch
     }
 };
 
-template <typename T> static int coarse_mult_any(T* out, const T* in, const T* A, const int cdims[4], int nvec, void* st);
-template <> int coarse_mult_any<float>(float* out, const float* in, const float* A, const int cdims[4], int nvec,
-                                       void* st) {
-    return lqcd_coarse_mult_f32(out, in, A, cdims, nvec, 0, st);
+// out_k = D_c in_k for K vectors back to back: one pass over A on the tensor cores where that applies (coarse_mrhs.cu)
+template <typename T>
+static int coarse_mult_any(T* out, const T* in, const T* A, const int cdims[4], int nvec, int K, void* st);
+template <>
+int coarse_mult_any<float>(float* out, const float* in, const float* A, const int cdims[4], int nvec, int K, void* st) {
+    if (K == 1) return lqcd_coarse_mult_f32(out, in, A, cdims, nvec, 0, st);
+    return lqcd_coarse_mult_mrhs_f32(out, in, A, cdims, nvec, K, 0, st);
 }
-template <> int coarse_mult_any<double>(double* out, const double* in, const double* A, const int cdims[4], int nvec,
-                                        void* st) {
-    return lqcd_coarse_mult_f64(out, in, A, cdims, nvec, 0, st);
+template <>
+int coarse_mult_any<double>(double* out, const double* in, const double* A, const int cdims[4], int nvec, int K,
+                            void* st) {
+    if (K == 1) return lqcd_coarse_mult_f64(out, in, A, cdims, nvec, 0, st);
+    return lqcd_coarse_mult_mrhs_f64(out, in, A, cdims, nvec, K, 0, st);
 }
 
-// x = niter BiCGStab iterations for D_c x = b from x = 0 (PAPER.md:71 with M = 1); r_out may be NULL
+// x_k = niter BiCGStab iterations for D_c x_k = b_k from x_k = 0 (PAPER.md:71 with M = 1), k = 0 .. K-1: K independent
+// recurrences (own scalars each) that share the applications of D_c; r_out may be NULL
 template <typename T>
-static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims[4], int nvec, int niter, void* ws,
-                         void* stream, const char* what) {
+static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims[4], int nvec, int K, int niter,
+                         void* ws, void* stream, const char* what) {
     clear_error();
-    if (!x || !b || !A || !ws || check_dims(cdims) || nvec < 1 || niter < 0) {
-        set_error("%s: null pointer, non-positive dim, nvec < 1 or niter < 0", what);
+    if (!x || !b || !A || !ws || check_dims(cdims) || nvec < 1 || niter < 0 || K < 1 || K > 65535) {
+        set_error("%s: null pointer, non-positive dim, nvec < 1, niter < 0 or nrhs outside 1..65535", what);
         return LQCD_EINVAL;
     }
     if (!aligned16(x) || !aligned16(b) || !aligned16(A) || !aligned16(ws) || !aligned16(r_out)) {
@@ -248,10 +284,10 @@ static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims
             return LQCD_EINVAL;
         }
     const long long n = volume(cdims) * 2 * nvec;
-    const size_t vbytes = (size_t)n * 2 * sizeof(T);
+    const size_t vbytes = (size_t)n * 2 * sizeof(T) * K;
     cudaStream_t st = (cudaStream_t)stream;
     BicgWs<T> W;
-    W.carve(ws, n);
+    W.carve(ws, n, K);
     int rc;
     if (niter == 0) {
         if (cudaMemsetAsync(x, 0, vbytes, st) != cudaSuccess) return check_launch(what);
@@ -259,22 +295,23 @@ static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims
             return check_launch(what);
         return LQCD_OK;
     }
+    const dim3 grid((unsigned)red_ctas(K), (unsigned)K);
     // r := b, rt := b, p := b, x := 0 -- without copies: the first iteration reads b in their place
-    k_cdot<T><<<RED_CTAS, RED_THREADS, 0, st>>>(W.part_a, b, b, n);
-    k_set_rho<T><<<1, 32, 0, st>>>(W.sc, W.part_a);
+    k_cdot<T><<<grid, RED_THREADS, 0, st>>>(W.part_a, b, b, n);
+    k_set_rho<T><<<dim3(1, (unsigned)K), 32, 0, st>>>(W.sc, W.part_a, (int)grid.x);
     count_launch(2);
     for (int it = 0; it < niter; it++) {
         const T* p = it == 0 ? b : W.p;
         const T* r = it == 0 ? b : W.r;
-        if ((rc = coarse_mult_any<T>(W.v, p, A, cdims, nvec, stream))) return rc;                  // v = D_c p
-        k_cdot<T><<<RED_CTAS, RED_THREADS, 0, st>>>(W.part_a, b, W.v, n);                          // <rt|v>
-        k_bicg_s<T><<<RED_CTAS, RED_THREADS, 0, st>>>(W.s, r, W.v, W.part_a, W.sc, it, n);         // s = r - alpha v
-        if ((rc = coarse_mult_any<T>(W.t, W.s, A, cdims, nvec, stream))) return rc;                // t = D_c s
-        k_cdot<T><<<RED_CTAS, RED_THREADS, 0, st>>>(W.part_a, W.t, W.s, n);                        // <t|s>, <t|t>
-        k_bicg_xr<T><<<RED_CTAS, RED_THREADS, 0, st>>>(x, W.r, p, W.s, W.t, b, W.part_a, W.part_b, W.sc, it == 0, n);
+        if ((rc = coarse_mult_any<T>(W.v, p, A, cdims, nvec, K, stream))) return rc;            // v = D_c p
+        k_cdot<T><<<grid, RED_THREADS, 0, st>>>(W.part_a, b, W.v, n);                           // <rt|v>
+        k_bicg_s<T><<<grid, RED_THREADS, 0, st>>>(W.s, r, W.v, W.part_a, W.sc, it, n);          // s = r - alpha v
+        if ((rc = coarse_mult_any<T>(W.t, W.s, A, cdims, nvec, K, stream))) return rc;          // t = D_c s
+        k_cdot<T><<<grid, RED_THREADS, 0, st>>>(W.part_a, W.t, W.s, n);                         // <t|s>, <t|t>
+        k_bicg_xr<T><<<grid, RED_THREADS, 0, st>>>(x, W.r, p, W.s, W.t, b, W.part_a, W.part_b, W.sc, it == 0, n);
         count_launch(4);
         if (it + 1 < niter) {  // the last p is never used
-            k_bicg_p<T><<<RED_CTAS, RED_THREADS, 0, st>>>(W.p, p, W.r, W.v, W.part_b, W.sc, it, n);
+            k_bicg_p<T><<<grid, RED_THREADS, 0, st>>>(W.p, p, W.r, W.v, W.part_b, W.sc, it, n);
             count_launch();
         }
     }
@@ -315,7 +352,7 @@ static size_t mg_ws_bytes(const int dims[4], const int block[4], int nvec, int r
     const long long n = volume(cd) * 2 * nvec;
     const size_t fine = align256((size_t)nchunks(dims) * CH * 24 * real_bytes);
     const size_t cvec = align256((size_t)n * 2 * real_bytes);
-    const size_t bicg = real_bytes == 4 ? BicgWs<float>::bytes(n) : BicgWs<double>::bytes(n);
+    const size_t bicg = real_bytes == 4 ? BicgWs<float>::bytes(n, 1) : BicgWs<double>::bytes(n, 1);
     return fine + 2 * cvec + bicg + align256(lqcd_mr_workspace_bytes(dims, block, real_bytes));
 }
 
@@ -352,12 +389,12 @@ static int vcycle_call(T* x, const T* b, const T* U, const T* clover, T kappa, c
     T* xcv = (T*)c;
     c += align256((size_t)n * 2 * sizeof(T));
     void* bicg_ws = c;
-    c += BicgWs<T>::bytes(n);
+    c += BicgWs<T>::bytes(n, 1);
     void* mr_ws = lqcd_mr_workspace_bytes(dims, block, (int)sizeof(T)) ? (void*)c : nullptr;
     int rc;
     // (1) |x> := M_1 |b>   (|x> = 0, so the first residual is |b> itself)
     if ((rc = FineCalls<T>::restrict_(bcv, b, nullvecs, dims, block, nvec, stream))) return rc;           // (1a) Eq. 5
-    if ((rc = bicgstab_call<T>(xcv, nullptr, bcv, A, cd, nvec, n_coarse, bicg_ws, stream, what))) return rc;  // (1b)
+    if ((rc = bicgstab_call<T>(xcv, nullptr, bcv, A, cd, nvec, 1, n_coarse, bicg_ws, stream, what))) return rc;  // (1b)
     if ((rc = FineCalls<T>::prolong_(x, xcv, nullvecs, dims, block, nvec, stream))) return rc;            // (1c) Eq. 6
     // (2) |x> := |x> + M_2 (|b> - D|x>): SAP started from |x> (its first step is the residual |b> - D|x>)
     return FineCalls<T>::sap_(x, r, b, U, clover, kappa, dims, bc, block, n_sap, n_mr,
@@ -373,15 +410,30 @@ extern "C" {
 size_t lqcd_coarse_bicgstab_workspace_bytes(const int cdims[4], int nvec, int real_bytes) {
     if (check_dims(cdims) || nvec < 1 || (real_bytes != 4 && real_bytes != 8)) return 0;
     const long long n = volume(cdims) * 2 * nvec;
-    return real_bytes == 4 ? BicgWs<float>::bytes(n) : BicgWs<double>::bytes(n);
+    return real_bytes == 4 ? BicgWs<float>::bytes(n, 1) : BicgWs<double>::bytes(n, 1);
+}
+size_t lqcd_coarse_bicgstab_mrhs_workspace_bytes(const int cdims[4], int nvec, int nrhs, int real_bytes) {
+    if (check_dims(cdims) || nvec < 1 || nrhs < 1 || (real_bytes != 4 && real_bytes != 8)) return 0;
+    const long long n = volume(cdims) * 2 * nvec;
+    return real_bytes == 4 ? BicgWs<float>::bytes(n, nrhs) : BicgWs<double>::bytes(n, nrhs);
+}
+int lqcd_coarse_bicgstab_mrhs_f32(float* x, float* r_out, const float* b, const float* A, const int cdims[4], int nvec,
+                                  int nrhs, int niter, void* ws_dev, void* stream) {
+    return bicgstab_call<float>(x, r_out, b, A, cdims, nvec, nrhs, niter, ws_dev, stream,
+                                "lqcd_coarse_bicgstab_mrhs_f32");
+}
+int lqcd_coarse_bicgstab_mrhs_f64(double* x, double* r_out, const double* b, const double* A, const int cdims[4],
+                                  int nvec, int nrhs, int niter, void* ws_dev, void* stream) {
+    return bicgstab_call<double>(x, r_out, b, A, cdims, nvec, nrhs, niter, ws_dev, stream,
+                                 "lqcd_coarse_bicgstab_mrhs_f64");
 }
 int lqcd_coarse_bicgstab_f32(float* x, float* r_out, const float* b, const float* A, const int cdims[4], int nvec,
                              int niter, void* ws_dev, void* stream) {
-    return bicgstab_call<float>(x, r_out, b, A, cdims, nvec, niter, ws_dev, stream, "lqcd_coarse_bicgstab_f32");
+    return bicgstab_call<float>(x, r_out, b, A, cdims, nvec, 1, niter, ws_dev, stream, "lqcd_coarse_bicgstab_f32");
 }
 int lqcd_coarse_bicgstab_f64(double* x, double* r_out, const double* b, const double* A, const int cdims[4], int nvec,
                              int niter, void* ws_dev, void* stream) {
-    return bicgstab_call<double>(x, r_out, b, A, cdims, nvec, niter, ws_dev, stream, "lqcd_coarse_bicgstab_f64");
+    return bicgstab_call<double>(x, r_out, b, A, cdims, nvec, 1, niter, ws_dev, stream, "lqcd_coarse_bicgstab_f64");
 }
 
 size_t lqcd_mg_workspace_bytes(const int dims[4], const int block[4], int nvec, int real_bytes) {

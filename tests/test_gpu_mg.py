@@ -167,3 +167,32 @@ def test_mg_error_codes(lq):
     assert code(lambda: lq.coarse_bicgstab(xc, bc_, d.A, cfg.cdims, cfg.nvec, -1)) == lq.EINVAL
     assert code(lambda: lq.coarse_bicgstab(xc, bc_, d.A, (2, 2, 2, 1), cfg.nvec, 1)) == lq.EINVAL
     assert lq.launch_count() == n0, "nothing is enqueued on error"
+
+
+@pytest.mark.parametrize("prec,name,nrhs", [("f64", "c1", 3), ("f32", "c1", 5), ("f32", "c2", 4), ("f32", "c3", 18)])
+def test_coarse_bicgstab_mrhs(lq, prec, name, nrhs):
+    """K independent BiCGStab recurrences that share the D_c applications (config 3: through the tensor-core kernel,
+    two launches per application for 18 right-hand sides): every right-hand side against the oracle's single solve."""
+    import torch
+    prob = config_problem(name)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    cond = cond_coarse(prob, prec)
+    rng = np.random.default_rng(123)
+    bs = np.stack([li.coarse_vector(rng, cfg.cvolume, cfg.nvec) for _ in range(nrhs)])
+    bs[-1] *= 1e-3                    # right-hand sides of different scale keep their own scalars
+    niter = 5
+    bd = to_dev(bs, prec)
+    x, r = torch.full_like(bd, 7.0), torch.full_like(bd, 7.0)
+    lq.coarse_bicgstab_mrhs(x, bd, d.A, cfg.cdims, cfg.nvec, niter, r_out=r)
+    gx, gr = x.cpu().numpy(), r.cpu().numpy()
+    A = rounded(prob.A, prec)
+    bar = 2 * niter * cond * TOL1[prec]
+    one = torch.empty_like(bd[0])
+    for k in range(nrhs):
+        rx, rr = oracle.coarse_bicgstab(rounded(bs[k], prec), A, cfg.cdims, cfg.nvec, niter)
+        assert rel_l2(gx[k], rx) <= bar, (k, rel_l2(gx[k], rx), bar)
+        assert np.linalg.norm(gr[k] - rr) / np.linalg.norm(bs[k]) <= bar, k
+    # and against the single-right-hand-side call on the GPU
+    lq.coarse_bicgstab(one, bd[0].contiguous(), d.A, cfg.cdims, cfg.nvec, niter)
+    assert rel_l2(gx[0], one.cpu().numpy()) <= bar
