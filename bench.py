@@ -323,6 +323,11 @@ class Workload:
         c = self.cfg
         self.lq.coarse_mult_mrhs(self.ycK, self.xcK, self.A, c.cdims, c.nvec)
 
+    def vcycle_mrhs(self, i):
+        c = self.cfg
+        self.lq.mg_vcycle_mrhs(self.yK, self.xK, self.U18, self.clover, c.kappa, c.dims, c.bc, c.block, c.nvec, self.v,
+                               self.A, n_coarse=8, n_sap=4, n_mr=6, ws=self.mg_ws)
+
     def bicg_mrhs(self, i):
         c = self.cfg
         self.lq.coarse_bicgstab_mrhs(self.ycK, self.xcK, self.A, c.cdims, c.nvec, 8, ws=self.bicg_ws)
@@ -626,6 +631,16 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         extra["mg_vcycle_8_4_6"] = {"us": t * 1e6, "GBps": mvc["bytes"] / t / 1e9, "GFLOPs": mvc["flops"] / t / 1e9,
                                     "units_per_s": cfg.volume / t, "launches": int(nl),
                                     "frac_of_hbm_peak": mvc["bytes"] / t / 1e9 / peak, "bytes_per_launch": mvc["bytes"]}
+        # ... and on 8 right-hand sides at once: restrictions, coarse solves (tensor cores) and prolongations shared
+        KV = 8
+        W.xK = torch.stack([W.x[k % W.NBUF] for k in range(KV)])
+        W.yK = torch.empty_like(W.xK)
+        nbk = int(W.lq.lib().lqcd_mg_mrhs_workspace_bytes(W.lq._i4(cfg.dims), W.lq._i4(cfg.block), cfg.nvec, KV, 4))
+        W.mg_ws = torch.empty(nbk, dtype=torch.uint8, device=W.dev)
+        tk = time_single(W, "vcycle_mrhs", reps=2, warmup=1)
+        extra["mg_vcycle_mrhs_8"] = {"us": tk * 1e6, "us_per_rhs": tk * 1e6 / KV,
+                                     "speedup_vs_8_single_vcycles": KV * t / tk}
+        del W.xK, W.yK
         W.mg_ws = None
         # F4: the coarse operator on 16 right-hand sides at once (tcgen05, 3xTF32): A is read from HBM once
         K = 16

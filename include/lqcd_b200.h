@@ -175,6 +175,13 @@ int lqcd_prolong_f32(float* out_f, const float* in_c, const float* nullvecs, con
 int lqcd_prolong_f64(double* out_f, const double* in_c, const double* nullvecs, const int dims[4],
                      const int block[4], int nvec, void* stream);
 
+/* Prolongation of nrhs coarse vectors at once (coarse vectors back to back -> native spinors back to back): the null
+ * vectors are streamed once per group of up to 8 vectors. */
+int lqcd_prolong_mrhs_f32(float* out_f, const float* in_c, const float* nullvecs, const int dims[4],
+                          const int block[4], int nvec, int nrhs, void* stream);
+int lqcd_prolong_mrhs_f64(double* out_f, const double* in_c, const double* nullvecs, const int dims[4],
+                          const int block[4], int nvec, int nrhs, void* stream);
+
 /* ---- F2: set-up of the operator fields on the device (not on the timed path) ------------------------------
  * Clover term from the links (formula: DESIGN.md reading Q1):
  *   F(x) = kappa csw sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}(x), sigma_{mu nu} = [g_mu, g_nu]/(2i),
@@ -304,6 +311,18 @@ int lqcd_mg_vcycle_f32(float* x, const float* b, const float* U, const float* cl
 int lqcd_mg_vcycle_f64(double* x, const double* b, const double* U, const double* clover, double kappa,
                        const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
                        const double* A, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
+
+/* The V-cycle on nrhs right-hand sides at once (x, b: nrhs native spinors back to back): the restrictions, the coarse
+ * solves (lqcd_coarse_bicgstab_mrhs, i.e. D_c on the tensor cores) and the prolongations are shared by all right-hand
+ * sides -- one pass over the null vectors / over A per group --, the smoother runs right-hand side by right-hand side.
+ * Result k is what lqcd_mg_vcycle gives for b_k, up to rounding.  ws_dev: lqcd_mg_mrhs_workspace_bytes(...) bytes. */
+size_t lqcd_mg_mrhs_workspace_bytes(const int dims[4], const int block[4], int nvec, int nrhs, int real_bytes);
+int lqcd_mg_vcycle_mrhs_f32(float* x, const float* b, const float* U, const float* clover, float kappa,
+                            const int dims[4], const int bc[4], const int block[4], int nvec, const float* nullvecs,
+                            const float* A, int nrhs, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
+int lqcd_mg_vcycle_mrhs_f64(double* x, const double* b, const double* U, const double* clover, double kappa,
+                            const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
+                            const double* A, int nrhs, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
 
 /* ---- F4: the coarse operator on K right-hand sides at once (many right-hand sides are "a typical
  * situation") ----------------------------------------------------------------------------------------------------

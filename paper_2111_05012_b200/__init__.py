@@ -443,6 +443,30 @@ def coarse_bicgstab_mrhs(x, b, A, cdims, nvec, niter, r_out=None, ws=None, strea
                                                               _stream(stream)), "lqcd_coarse_bicgstab_mrhs")
     return x
 
+def prolong_mrhs(out_f, in_c, nullvecs, dims, block, nvec, stream=None):
+    """Eq. 6 for several coarse vectors at once: in_c (K, Vc, 2, nvec), out_f (K, native spinor)."""
+    sfx = _same_dtype(out_f, in_c, nullvecs)
+    _check(getattr(lib(), f"lqcd_prolong_mrhs_{sfx}")(_dev_ptr(out_f), _dev_ptr(in_c), _dev_ptr(nullvecs), _i4(dims),
+                                                      _i4(block), int(nvec), int(in_c.shape[0]), _stream(stream)),
+           "lqcd_prolong_mrhs")
+    return out_f
+
+
+def mg_vcycle_mrhs(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, n_coarse=8, n_sap=4, n_mr=6, ws=None,
+                   stream=None):
+    """x[k] = M b[k] for all k: restrictions, coarse solves and prolongations shared, the smoother one by one."""
+    sfx = _same_dtype(x, b, U, clover, nullvecs, A)
+    nrhs = int(b.shape[0])
+    if ws is None:
+        nb = int(lib().lqcd_mg_mrhs_workspace_bytes(_i4(dims), _i4(block), int(nvec), nrhs, 4 if sfx == "f32" else 8))
+        ws = torch.empty(nb, dtype=torch.uint8, device=x.device)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_mg_vcycle_mrhs_{sfx}")(_dev_ptr(x), _dev_ptr(b), _dev_ptr(U), _dev_ptr(clover), k,
+                                                        _i4(dims), _i4(bc), _i4(block), int(nvec), _dev_ptr(nullvecs),
+                                                        _dev_ptr(A), nrhs, int(n_coarse), int(n_sap), int(n_mr),
+                                                        _dev_ptr(ws), _stream(stream)), "lqcd_mg_vcycle_mrhs")
+    return x
+
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):

@@ -33,6 +33,7 @@ SIGNATURES = {
     "lqcd_mr_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_coarse_bicgstab_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci]),
     "lqcd_mg_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
+    "lqcd_mg_mrhs_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci, _ci]),
     "lqcd_coarse_bicgstab_mrhs_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci, _ci]),
 }
 for _p, _k in (("f32", _cf), ("f64", _cd)):
@@ -62,6 +63,9 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_wilson_clover_mult_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _ci, _cu, _vp]),
         f"lqcd_restrict_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _ci, _vp]),
         f"lqcd_coarse_bicgstab_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _i4, _ci, _ci, _ci, _vp, _vp]),
+        f"lqcd_prolong_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _ci, _vp]),
+        f"lqcd_mg_vcycle_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _vp, _vp, _ci, _ci, _ci, _ci, _vp,
+                                           _vp]),
         f"lqcd_sap_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _cu, _vp, _vp]),
     })
 SIGNATURES.update({

@@ -328,6 +328,14 @@ template <> struct FineCalls<float> {
     static int prolong_(float* o, const float* i, const float* v, const int* d, const int* b, int nv, void* st) {
         return lqcd_prolong_f32(o, i, v, d, b, nv, st);
     }
+    static int restrict_mrhs_(float* o, const float* i, const float* v, const int* d, const int* b, int nv, int K,
+                              void* st) {
+        return lqcd_restrict_mrhs_f32(o, i, v, d, b, nv, K, st);
+    }
+    static int prolong_mrhs_(float* o, const float* i, const float* v, const int* d, const int* b, int nv, int K,
+                             void* st) {
+        return lqcd_prolong_mrhs_f32(o, i, v, d, b, nv, K, st);
+    }
     static int sap_(float* x, float* r, const float* b, const float* U, const float* c, float k, const int* d,
                     const int* bc, const int* dom, int ns, int nm, unsigned fl, void* ws, void* st) {
         return lqcd_sap_f32(x, r, b, U, c, k, d, bc, dom, ns, nm, fl, ws, st);
@@ -340,35 +348,43 @@ template <> struct FineCalls<double> {
     static int prolong_(double* o, const double* i, const double* v, const int* d, const int* b, int nv, void* st) {
         return lqcd_prolong_f64(o, i, v, d, b, nv, st);
     }
+    static int restrict_mrhs_(double* o, const double* i, const double* v, const int* d, const int* b, int nv, int K,
+                              void* st) {
+        return lqcd_restrict_mrhs_f64(o, i, v, d, b, nv, K, st);
+    }
+    static int prolong_mrhs_(double* o, const double* i, const double* v, const int* d, const int* b, int nv, int K,
+                             void* st) {
+        return lqcd_prolong_mrhs_f64(o, i, v, d, b, nv, K, st);
+    }
     static int sap_(double* x, double* r, const double* b, const double* U, const double* c, double k, const int* d,
                     const int* bc, const int* dom, int ns, int nm, unsigned fl, void* ws, void* st) {
         return lqcd_sap_f64(x, r, b, U, c, k, d, bc, dom, ns, nm, fl, ws, st);
     }
 };
 
-static size_t mg_ws_bytes(const int dims[4], const int block[4], int nvec, int real_bytes) {
+static size_t mg_ws_bytes(const int dims[4], const int block[4], int nvec, int K, int real_bytes) {
     int cd[4];
     if (check_block(dims, block, nvec, cd)) return 0;
     const long long n = volume(cd) * 2 * nvec;
     const size_t fine = align256((size_t)nchunks(dims) * CH * 24 * real_bytes);
-    const size_t cvec = align256((size_t)n * 2 * real_bytes);
-    const size_t bicg = real_bytes == 4 ? BicgWs<float>::bytes(n, 1) : BicgWs<double>::bytes(n, 1);
+    const size_t cvec = align256((size_t)n * 2 * real_bytes * K);
+    const size_t bicg = real_bytes == 4 ? BicgWs<float>::bytes(n, K) : BicgWs<double>::bytes(n, K);
     return fine + 2 * cvec + bicg + align256(lqcd_mr_workspace_bytes(dims, block, real_bytes));
 }
 
 // x = M b: one V-cycle
 template <typename T>
 static int vcycle_call(T* x, const T* b, const T* U, const T* clover, T kappa, const int dims[4], const int bc[4],
-                       const int block[4], int nvec, const T* nullvecs, const T* A, int n_coarse, int n_sap, int n_mr,
-                       void* ws, void* stream, const char* what) {
+                       const int block[4], int nvec, const T* nullvecs, const T* A, int K, int n_coarse, int n_sap,
+                       int n_mr, void* ws, void* stream, const char* what) {
     clear_error();
     int cd[4];
     if (!x || !b || !U || !clover || !nullvecs || !A || !ws || !bc || check_block(dims, block, nvec, cd)) {
         set_error("%s: null pointer or bad dims/block/nvec", what);
         return LQCD_EINVAL;
     }
-    if (x == b || n_coarse < 0 || n_sap < 0 || n_mr < 0 || !aligned16(ws)) {
-        set_error("%s: x must not alias b; iteration counts must be >= 0; ws 16-byte aligned", what);
+    if (x == b || n_coarse < 0 || n_sap < 0 || n_mr < 0 || K < 1 || !aligned16(ws)) {
+        set_error("%s: x must not alias b; iteration counts must be >= 0; nrhs >= 1; ws 16-byte aligned", what);
         return LQCD_EINVAL;
     }
     for (int mu = 0; mu < 4; mu++)
@@ -385,20 +401,32 @@ static int vcycle_call(T* x, const T* b, const T* U, const T* clover, T kappa, c
     T* r = (T*)c;
     c += align256((size_t)nchunks(dims) * CH * 24 * sizeof(T));
     T* bcv = (T*)c;
-    c += align256((size_t)n * 2 * sizeof(T));
+    c += align256((size_t)n * 2 * sizeof(T) * K);
     T* xcv = (T*)c;
-    c += align256((size_t)n * 2 * sizeof(T));
+    c += align256((size_t)n * 2 * sizeof(T) * K);
     void* bicg_ws = c;
-    c += BicgWs<T>::bytes(n, 1);
+    c += BicgWs<T>::bytes(n, K);
     void* mr_ws = lqcd_mr_workspace_bytes(dims, block, (int)sizeof(T)) ? (void*)c : nullptr;
+    const long long fstride = (long long)nchunks(dims) * CH * 24;
     int rc;
-    // (1) |x> := M_1 |b>   (|x> = 0, so the first residual is |b> itself)
-    if ((rc = FineCalls<T>::restrict_(bcv, b, nullvecs, dims, block, nvec, stream))) return rc;           // (1a) Eq. 5
-    if ((rc = bicgstab_call<T>(xcv, nullptr, bcv, A, cd, nvec, 1, n_coarse, bicg_ws, stream, what))) return rc;  // (1b)
-    if ((rc = FineCalls<T>::prolong_(x, xcv, nullvecs, dims, block, nvec, stream))) return rc;            // (1c) Eq. 6
+    // (1) |x> := M_1 |b>   (|x> = 0, so the first residual is |b> itself); all right-hand sides together
+    if (K == 1) {
+        if ((rc = FineCalls<T>::restrict_(bcv, b, nullvecs, dims, block, nvec, stream))) return rc;        // (1a) Eq. 5
+    } else if ((rc = FineCalls<T>::restrict_mrhs_(bcv, b, nullvecs, dims, block, nvec, K, stream))) {
+        return rc;
+    }
+    if ((rc = bicgstab_call<T>(xcv, nullptr, bcv, A, cd, nvec, K, n_coarse, bicg_ws, stream, what))) return rc;  // (1b)
+    if (K == 1) {
+        if ((rc = FineCalls<T>::prolong_(x, xcv, nullvecs, dims, block, nvec, stream))) return rc;         // (1c) Eq. 6
+    } else if ((rc = FineCalls<T>::prolong_mrhs_(x, xcv, nullvecs, dims, block, nvec, K, stream))) {
+        return rc;
+    }
     // (2) |x> := |x> + M_2 (|b> - D|x>): SAP started from |x> (its first step is the residual |b> - D|x>)
-    return FineCalls<T>::sap_(x, r, b, U, clover, kappa, dims, bc, block, n_sap, n_mr,
-                              LQCD_SAP_INITIAL_GUESS | LQCD_SAP_NO_FINAL_RESIDUAL, mr_ws, stream);
+    for (int k = 0; k < K; k++)
+        if ((rc = FineCalls<T>::sap_(x + k * fstride, r, b + k * fstride, U, clover, kappa, dims, bc, block, n_sap, n_mr,
+                                     LQCD_SAP_INITIAL_GUESS | LQCD_SAP_NO_FINAL_RESIDUAL, mr_ws, stream)))
+            return rc;
+    return LQCD_OK;
 }
 
 }  // namespace lqcd
@@ -438,18 +466,34 @@ int lqcd_coarse_bicgstab_f64(double* x, double* r_out, const double* b, const do
 
 size_t lqcd_mg_workspace_bytes(const int dims[4], const int block[4], int nvec, int real_bytes) {
     if (real_bytes != 4 && real_bytes != 8) return 0;
-    return mg_ws_bytes(dims, block, nvec, real_bytes);
+    return mg_ws_bytes(dims, block, nvec, 1, real_bytes);
+}
+size_t lqcd_mg_mrhs_workspace_bytes(const int dims[4], const int block[4], int nvec, int nrhs, int real_bytes) {
+    if ((real_bytes != 4 && real_bytes != 8) || nrhs < 1) return 0;
+    return mg_ws_bytes(dims, block, nvec, nrhs, real_bytes);
+}
+int lqcd_mg_vcycle_mrhs_f32(float* x, const float* b, const float* U, const float* clover, float kappa,
+                            const int dims[4], const int bc[4], const int block[4], int nvec, const float* nullvecs,
+                            const float* A, int nrhs, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream) {
+    return vcycle_call<float>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, nrhs, n_coarse, n_sap, n_mr,
+                              ws_dev, stream, "lqcd_mg_vcycle_mrhs_f32");
+}
+int lqcd_mg_vcycle_mrhs_f64(double* x, const double* b, const double* U, const double* clover, double kappa,
+                            const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
+                            const double* A, int nrhs, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream) {
+    return vcycle_call<double>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, nrhs, n_coarse, n_sap, n_mr,
+                               ws_dev, stream, "lqcd_mg_vcycle_mrhs_f64");
 }
 int lqcd_mg_vcycle_f32(float* x, const float* b, const float* U, const float* clover, float kappa, const int dims[4],
                        const int bc[4], const int block[4], int nvec, const float* nullvecs, const float* A,
                        int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream) {
-    return vcycle_call<float>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, n_coarse, n_sap, n_mr,
+    return vcycle_call<float>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, 1, n_coarse, n_sap, n_mr,
                               ws_dev, stream, "lqcd_mg_vcycle_f32");
 }
 int lqcd_mg_vcycle_f64(double* x, const double* b, const double* U, const double* clover, double kappa,
                        const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
                        const double* A, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream) {
-    return vcycle_call<double>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, n_coarse, n_sap, n_mr,
+    return vcycle_call<double>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, 1, n_coarse, n_sap, n_mr,
                                ws_dev, stream, "lqcd_mg_vcycle_f64");
 }
 }

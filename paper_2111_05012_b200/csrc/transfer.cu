@@ -200,6 +200,58 @@ __global__ void __launch_bounds__(256) k_prolong(T* __restrict__ out_f, const T*
     }
 }
 
+// prolong for up to NRMAX coarse vectors at once: the null vectors are streamed once, every thread keeps NRMAX
+// accumulators for its 16-byte slice of the aggregate
+template <typename T, int UNROLL, int NRMAX>
+__global__ void __launch_bounds__(256) k_prolong_mrhs(T* __restrict__ out_f, long long fstride,
+                                                      const T* __restrict__ in_c, long long cstride, int nr,
+                                                      const T* __restrict__ v, TransferParams P) {
+    constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, JH = 12 / NV;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* xc = reinterpret_cast<T*>(smem_raw);  // [r][nvec] complex
+    const int agg = blockIdx.x;
+    const int X = agg >> 1, chi = agg & 1;
+    for (int q = threadIdx.x; q < nr * 2 * P.nvec; q += blockDim.x) {
+        const int r = q / (2 * P.nvec), i = q % (2 * P.nvec);
+        xc[q] = in_c[r * cstride + (long long)agg * P.nvec * 2 + i];
+    }
+    __syncthreads();
+    const T* vagg = v + (long long)agg * P.nvec * P.LV * NV;
+    for (int p = threadIdx.x; p < P.LV; p += blockDim.x) {
+        V16<T> acc[NRMAX];
+#pragma unroll
+        for (int r = 0; r < NRMAX; r++)
+#pragma unroll
+            for (int e = 0; e < NV; e++) acc[r].r[e] = 0;
+        const T* vp = vagg + (long long)p * NV;
+        int i = 0;
+        for (; i + UNROLL <= P.nvec; i += UNROLL) {
+            V16<T> a[UNROLL];
+#pragma unroll
+            for (int u = 0; u < UNROLL; u++) a[u] = ld16_stream(vp + (long long)(i + u) * P.LV * NV);
+#pragma unroll
+            for (int r = 0; r < NRMAX; r++)
+                if (r < nr) {
+#pragma unroll
+                    for (int u = 0; u < UNROLL; u++)
+                        caxpy<T>(acc[r], a[u], xc[(r * P.nvec + i + u) * 2], xc[(r * P.nvec + i + u) * 2 + 1]);
+                }
+        }
+        for (; i < P.nvec; i++) {
+            const V16<T> a = ld16_stream(vp + (long long)i * P.LV * NV);
+#pragma unroll
+            for (int r = 0; r < NRMAX; r++)
+                if (r < nr) caxpy<T>(acc[r], a, xc[(r * P.nvec + i) * 2], xc[(r * P.nvec + i) * 2 + 1]);
+        }
+        const int l = p / JH, jj = p % JH;
+        const int s = fine_site(P, X, l);
+        const long long off = (((long long)(s >> 5) * NJ + chi * JH + jj) * CH + (s & 31)) * NV;
+#pragma unroll
+        for (int r = 0; r < NRMAX; r++)
+            if (r < nr) st16_stream(out_f + r * fstride + off, acc[r]);
+    }
+}
+
 template <typename T>
 static int restrict_call(T* out_c, const T* in_f, const T* v, const int dims[4], const int block[4], int nvec,
                          void* stream, const char* what) {
@@ -283,6 +335,39 @@ static int prolong_call(T* out_f, const T* in_c, const T* v, const int dims[4], 
     return check_launch(what);
 }
 
+// nrhs coarse vectors back to back -> nrhs fine vectors back to back, null vectors read once per group of 8
+template <typename T>
+int prolong_mrhs_call(T* out_f, const T* in_c, const T* v, const int dims[4], const int block[4], int nvec, int nrhs,
+                      void* stream, const char* what) {
+    TransferParams P;
+    int rc = transfer_setup<T>(P, out_f, in_c, v, dims, block, nvec, what);
+    if (rc) return rc;
+    if (nrhs < 1) {
+        set_error("%s: nrhs < 1", what);
+        return LQCD_EINVAL;
+    }
+    constexpr int NRMAX = 8;
+    const size_t one = (size_t)nvec * 2 * sizeof(T);
+    if (NRMAX * one > 48 * 1024) {
+        set_error("%s: nvec = %d outside the compiled range", what, nvec);
+        return LQCD_EUNSUPPORTED;
+    }
+    const long long fstride = (long long)nchunks(dims) * CH * 24, cstride = volume(P.Lc) * 4 * nvec;
+    const int threads = P.LV >= 256 ? 256 : (P.LV + 31) / 32 * 32;
+    const long long nagg = 2 * volume(P.Lc);
+    for (int k = 0; k < nrhs; k += NRMAX) {
+        const int nr = nrhs - k < NRMAX ? nrhs - k : NRMAX;
+        k_prolong_mrhs<T, 4, NRMAX><<<(unsigned)nagg, threads, nr * one, (cudaStream_t)stream>>>(
+            out_f + k * fstride, fstride, in_c + k * cstride, cstride, nr, v, P);
+        count_launch();
+    }
+    return check_launch(what);
+}
+template int prolong_mrhs_call<float>(float*, const float*, const float*, const int*, const int*, int, int, void*,
+                                      const char*);
+template int prolong_mrhs_call<double>(double*, const double*, const double*, const int*, const int*, int, int, void*,
+                                       const char*);
+
 }  // namespace lqcd
 
 using namespace lqcd;
@@ -311,5 +396,13 @@ int lqcd_restrict_mrhs_f32(float* o, const float* i, const float* v, const int d
 int lqcd_restrict_mrhs_f64(double* o, const double* i, const double* v, const int dims[4], const int block[4],
                            int nvec, int nrhs, void* st) {
     return restrict_mrhs_call<double>(o, i, v, dims, block, nvec, nrhs, st, "lqcd_restrict_mrhs_f64");
+}
+int lqcd_prolong_mrhs_f32(float* o, const float* i, const float* v, const int dims[4], const int block[4], int nvec,
+                          int nrhs, void* st) {
+    return prolong_mrhs_call<float>(o, i, v, dims, block, nvec, nrhs, st, "lqcd_prolong_mrhs_f32");
+}
+int lqcd_prolong_mrhs_f64(double* o, const double* i, const double* v, const int dims[4], const int block[4],
+                          int nvec, int nrhs, void* st) {
+    return prolong_mrhs_call<double>(o, i, v, dims, block, nvec, nrhs, st, "lqcd_prolong_mrhs_f64");
 }
 }

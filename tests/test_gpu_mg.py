@@ -196,3 +196,24 @@ def test_coarse_bicgstab_mrhs(lq, prec, name, nrhs):
     # and against the single-right-hand-side call on the GPU
     lq.coarse_bicgstab(one, bd[0].contiguous(), d.A, cfg.cdims, cfg.nvec, niter)
     assert rel_l2(gx[0], one.cpu().numpy()) <= bar
+
+
+@pytest.mark.parametrize("prec,name,nrhs", [("f64", "c1", 3), ("f32", "c1", 4), ("f32", "c3", 3)])
+def test_vcycle_mrhs(lq, prec, name, nrhs):
+    """the V-cycle on several right-hand sides at once: every one against the oracle's single V-cycle"""
+    import torch
+    from problems import make_problem
+    prob = make_problem(li.CONFIGS[name], n_rhs=nrhs)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    cond = cond_coarse(prob, prec)
+    n_coarse, n_sap, n_mr = 4, 2, 6
+    b = torch.stack([lq.pack_spinor(to_dev(p, prec), cfg.dims) for p in prob.psi])
+    x = torch.full_like(b, 2.0)
+    lq.mg_vcycle_mrhs(x, b, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, cfg.nvec, d.v, d.A,
+                      n_coarse=n_coarse, n_sap=n_sap, n_mr=n_mr)
+    bar = (2 * n_coarse * cond + 2 + 2 * n_sap * (n_mr + 1)) * TOL1[prec]
+    for k in range(nrhs):
+        ref = oracle_vcycle(prob, prec, prob.psi[k], n_coarse, n_sap, n_mr)
+        got = lq.unpack_spinor(x[k], cfg.dims).cpu().numpy()
+        assert rel_l2(got, ref) <= bar, (k, rel_l2(got, ref), bar)

@@ -207,3 +207,21 @@ def test_restrict_mrhs(lq, prec, name, nrhs):
         assert rel_l2(got[k], ref) <= TOL[prec], k
         lq.restrict(one, x[k], d.v, cfg.dims, cfg.block, cfg.nvec)
         assert rel_l2(got[k], one.cpu().numpy()) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("name,nrhs", [("c1", 11), ("c2", 5), ("c3", 9)])
+def test_prolong_mrhs(lq, prec, name, nrhs):
+    import torch
+    if name == "c3" and prec == "f64":
+        pytest.skip("config 3 is an fp32 config")
+    prob = config_problem(name)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    xs = rhs_set(cfg, nrhs, seed=5)
+    xd = to_dev(xs, prec)
+    out = torch.full((nrhs, lq.native_spinor_reals(cfg.dims)), 3.0, dtype=d.U.dtype, device="cuda")
+    lq.prolong_mrhs(out, xd, d.v, cfg.dims, cfg.block, cfg.nvec)
+    for k in range(nrhs):
+        ref = oracle.prolong(rounded(xs[k], prec), rounded(prob.v, prec), cfg.dims, cfg.block)
+        assert rel_l2(lq.unpack_spinor(out[k], cfg.dims).cpu().numpy(), ref) <= TOL[prec], k
