@@ -271,6 +271,17 @@ int lqcd_sap_f64(double* x, double* r, const double* b, const double* U, const d
                  const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
                  void* ws_dev, void* stream);
 
+/* SAP on nrhs right-hand sides at once (x, r, b: nrhs native spinors back to back each): the listing above for every
+ * right-hand side; inside the shared-memory-resident inner-domain solver the right-hand sides are solved one after the
+ * other on the resident links and clover term of the domain, which are read from HBM once per half sweep for all of
+ * them.  Result k is bit-identical with lqcd_sap on (x_k, r_k, b_k). */
+int lqcd_sap_mrhs_f32(float* x, float* r, const float* b, const float* U, const float* clover, float kappa,
+                      const int dims[4], const int bc[4], const int domain[4], int nrhs, int n_sap, int n_mr,
+                      unsigned flags, void* ws_dev, void* stream);
+int lqcd_sap_mrhs_f64(double* x, double* r, const double* b, const double* U, const double* clover, double kappa,
+                      const int dims[4], const int bc[4], const int domain[4], int nrhs, int n_sap, int n_mr,
+                      unsigned flags, void* ws_dev, void* stream);
+
 /* Coarse solver (1b) of PAPER.md:116 ("We employ the BiCGStab algorithm ... not necessarily performed with high
  * precision"): the BiCGStab recurrence of the listing PAPER.md:71 with M = 1 and x_0 = 0 for D_c x = b, with a FIXED
  * number of iterations instead of the listing's two "small enough" break points (reading Q18):
@@ -314,7 +325,7 @@ int lqcd_mg_vcycle_f64(double* x, const double* b, const double* U, const double
 
 /* The V-cycle on nrhs right-hand sides at once (x, b: nrhs native spinors back to back): the restrictions, the coarse
  * solves (lqcd_coarse_bicgstab_mrhs, i.e. D_c on the tensor cores) and the prolongations are shared by all right-hand
- * sides -- one pass over the null vectors / over A per group --, the smoother runs right-hand side by right-hand side.
+ * sides -- one pass over the null vectors / over A per group --, the smoother is lqcd_sap_mrhs.
  * Result k is what lqcd_mg_vcycle gives for b_k, up to rounding.  ws_dev: lqcd_mg_mrhs_workspace_bytes(...) bytes. */
 size_t lqcd_mg_mrhs_workspace_bytes(const int dims[4], const int block[4], int nvec, int nrhs, int real_bytes);
 int lqcd_mg_vcycle_mrhs_f32(float* x, const float* b, const float* U, const float* clover, float kappa,

@@ -467,6 +467,17 @@ def mg_vcycle_mrhs(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, n
                                                         _dev_ptr(ws), _stream(stream)), "lqcd_mg_vcycle_mrhs")
     return x
 
+def sap_mrhs(x, r, b, U, clover, kappa, dims, bc, domain, n_sap=4, n_mr=6, initial_guess=False, final_residual=True,
+             ws=None, stream=None):
+    """SAP for all right-hand sides b[k] at once; x, r, b of shape (K, native spinor)."""
+    sfx = _same_dtype(x, r, b, U, clover)
+    flags = (SAP_INITIAL_GUESS if initial_guess else 0) | (0 if final_residual else SAP_NO_FINAL_RESIDUAL)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_sap_mrhs_{sfx}")(_dev_ptr(x), _dev_ptr(r), _dev_ptr(b), _dev_ptr(U), _dev_ptr(clover),
+                                                  k, _i4(dims), _i4(bc), _i4(domain), int(b.shape[0]), int(n_sap),
+                                                  int(n_mr), flags, _ws_ptr(ws), _stream(stream)), "lqcd_sap_mrhs")
+    return x
+
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):

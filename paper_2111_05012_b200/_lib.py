@@ -66,6 +66,7 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_prolong_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _ci, _vp]),
         f"lqcd_mg_vcycle_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _vp, _vp, _ci, _ci, _ci, _ci, _vp,
                                            _vp]),
+        f"lqcd_sap_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _ci, _cu, _vp, _vp]),
         f"lqcd_sap_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _cu, _vp, _vp]),
     })
 SIGNATURES.update({

@@ -337,8 +337,8 @@ template <> struct FineCalls<float> {
         return lqcd_prolong_mrhs_f32(o, i, v, d, b, nv, K, st);
     }
     static int sap_(float* x, float* r, const float* b, const float* U, const float* c, float k, const int* d,
-                    const int* bc, const int* dom, int ns, int nm, unsigned fl, void* ws, void* st) {
-        return lqcd_sap_f32(x, r, b, U, c, k, d, bc, dom, ns, nm, fl, ws, st);
+                    const int* bc, const int* dom, int K, int ns, int nm, unsigned fl, void* ws, void* st) {
+        return lqcd_sap_mrhs_f32(x, r, b, U, c, k, d, bc, dom, K, ns, nm, fl, ws, st);
     }
 };
 template <> struct FineCalls<double> {
@@ -357,8 +357,8 @@ template <> struct FineCalls<double> {
         return lqcd_prolong_mrhs_f64(o, i, v, d, b, nv, K, st);
     }
     static int sap_(double* x, double* r, const double* b, const double* U, const double* c, double k, const int* d,
-                    const int* bc, const int* dom, int ns, int nm, unsigned fl, void* ws, void* st) {
-        return lqcd_sap_f64(x, r, b, U, c, k, d, bc, dom, ns, nm, fl, ws, st);
+                    const int* bc, const int* dom, int K, int ns, int nm, unsigned fl, void* ws, void* st) {
+        return lqcd_sap_mrhs_f64(x, r, b, U, c, k, d, bc, dom, K, ns, nm, fl, ws, st);
     }
 };
 
@@ -366,7 +366,7 @@ static size_t mg_ws_bytes(const int dims[4], const int block[4], int nvec, int K
     int cd[4];
     if (check_block(dims, block, nvec, cd)) return 0;
     const long long n = volume(cd) * 2 * nvec;
-    const size_t fine = align256((size_t)nchunks(dims) * CH * 24 * real_bytes);
+    const size_t fine = align256((size_t)nchunks(dims) * CH * 24 * real_bytes * K);  // one residual per right-hand side
     const size_t cvec = align256((size_t)n * 2 * real_bytes * K);
     const size_t bicg = real_bytes == 4 ? BicgWs<float>::bytes(n, K) : BicgWs<double>::bytes(n, K);
     return fine + 2 * cvec + bicg + align256(lqcd_mr_workspace_bytes(dims, block, real_bytes));
@@ -399,7 +399,7 @@ static int vcycle_call(T* x, const T* b, const T* U, const T* clover, T kappa, c
     const long long n = volume(cd) * 2 * nvec;
     char* c = reinterpret_cast<char*>(ws);
     T* r = (T*)c;
-    c += align256((size_t)nchunks(dims) * CH * 24 * sizeof(T));
+    c += align256((size_t)nchunks(dims) * CH * 24 * sizeof(T) * K);
     T* bcv = (T*)c;
     c += align256((size_t)n * 2 * sizeof(T) * K);
     T* xcv = (T*)c;
@@ -407,7 +407,6 @@ static int vcycle_call(T* x, const T* b, const T* U, const T* clover, T kappa, c
     void* bicg_ws = c;
     c += BicgWs<T>::bytes(n, K);
     void* mr_ws = lqcd_mr_workspace_bytes(dims, block, (int)sizeof(T)) ? (void*)c : nullptr;
-    const long long fstride = (long long)nchunks(dims) * CH * 24;
     int rc;
     // (1) |x> := M_1 |b>   (|x> = 0, so the first residual is |b> itself); all right-hand sides together
     if (K == 1) {
@@ -422,11 +421,8 @@ static int vcycle_call(T* x, const T* b, const T* U, const T* clover, T kappa, c
         return rc;
     }
     // (2) |x> := |x> + M_2 (|b> - D|x>): SAP started from |x> (its first step is the residual |b> - D|x>)
-    for (int k = 0; k < K; k++)
-        if ((rc = FineCalls<T>::sap_(x + k * fstride, r, b + k * fstride, U, clover, kappa, dims, bc, block, n_sap, n_mr,
-                                     LQCD_SAP_INITIAL_GUESS | LQCD_SAP_NO_FINAL_RESIDUAL, mr_ws, stream)))
-            return rc;
-    return LQCD_OK;
+    return FineCalls<T>::sap_(x, r, b, U, clover, kappa, dims, bc, block, K, n_sap, n_mr,
+                              LQCD_SAP_INITIAL_GUESS | LQCD_SAP_NO_FINAL_RESIDUAL, mr_ws, stream);
 }
 
 }  // namespace lqcd

@@ -151,7 +151,7 @@ __device__ __forceinline__ void hop_smem(T acc[24], const V16<T>* __restrict__ r
 template <typename T, bool ACC, int BVC>
 __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits at most 151 sites (320 threads)
     k_mr_domain(T* __restrict__ x, const T* __restrict__ r, const T* __restrict__ U, const T* __restrict__ clover,
-                T kappa, DomParams P, int niter) {
+                T kappa, DomParams P, int niter, int nrhs, long long rstride) {
     using S = MrSmem<T>;
     constexpr int NV = S::NV, NJ = S::NJ, NH = S::NJ / 2, NR = S::NR, NFULL = S::NFULL;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -179,20 +179,16 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
 #pragma unroll
             for (int q = 0; q < NV; q++) zero.r[q] = 0;
 #pragma unroll
-            for (int j = 0; j < NH; j++) st16_stream(x + sp_off + (long long)(NH * h + j) * CH * NV, zero);
+            for (int k = 0; k < nrhs; k++)
+#pragma unroll
+                for (int j = 0; j < NH; j++)
+                    st16_stream(x + k * rstride + sp_off + (long long)(NH * h + j) * CH * NV, zero);
         }
         return;
     }
 
     // ---- stage the domain (every operand is read ONCE from HBM): links and clover straight into shared memory
-    // (cp.async, 64-byte L2 granularity: a 4-site x-run of a domain is half a 128-byte line), my half of r in registers
-    T rho[12];
-#pragma unroll
-    for (int j = 0; j < NH; j++) {
-        const V16<T> v = ld16_g64(r + sp_off + (long long)(NH * h + j) * CH * NV);
-#pragma unroll
-        for (int q = 0; q < NV; q++) rho[j * NV + q] = v.r[q];
-    }
+    // (cp.async, 64-byte L2 granularity: a 4-site x-run of a domain is half a 128-byte line)
     if (active) {
 #pragma unroll
         for (int m = 0; m < 2; m++) {
@@ -230,6 +226,18 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
     }
     const int partner = h ? tid - bvp : tid + bvp;
 
+    // Right-hand sides one after the other on the resident operator: links and clover (86 % of the staged bytes) are
+    // read from HBM once for all of them.
+    for (int krhs = 0; krhs < nrhs; krhs++) {
+    const T* rk = r + krhs * rstride;
+    T* xk = x + krhs * rstride;
+    T rho[12];  // my half of the residual
+#pragma unroll
+    for (int j = 0; j < NH; j++) {
+        const V16<T> v = ld16_g64(rk + sp_off + (long long)(NH * h + j) * CH * NV);
+#pragma unroll
+        for (int q = 0; q < NV; q++) rho[j * NV + q] = v.r[q];
+    }
     T z[12];
 #pragma unroll
     for (int q = 0; q < 12; q++) z[q] = 0;
@@ -336,7 +344,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
     if (active) {
 #pragma unroll
         for (int j = 0; j < NH; j++) {
-            T* px = x + sp_off + (long long)(NH * h + j) * CH * NV;
+            T* px = xk + sp_off + (long long)(NH * h + j) * CH * NV;
             V16<T> v;
 #pragma unroll
             for (int q = 0; q < NV; q++) v.r[q] = z[j * NV + q];
@@ -348,6 +356,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
             st16(px, v);
         }
     }
+    }  // right-hand sides
 }
 
 // ---- blocked BLAS-1: one CTA per domain, sites strided over the threads ------------------------
@@ -556,9 +565,10 @@ template <typename T> static bool mr_fits_smem(int bv) {
 // z (+)= M_SAP^(g) r.  ws: two native spinors of scratch (rho, p) when the generic path is taken.
 template <typename T>
 static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa, const int dims[4], const int bc[4],
-                          const int domain[4], unsigned flags, int niter, void* ws, void* stream, const char* what) {
+                          const int domain[4], unsigned flags, int niter, int K, void* ws, void* stream,
+                          const char* what) {
     clear_error();
-    if (!z || !r || !U || !clover || !bc) {
+    if (!z || !r || !U || !clover || !bc || K < 1) {
         set_error("%s: null pointer", what);
         return LQCD_EINVAL;
     }
@@ -590,6 +600,7 @@ static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa
             P.halfgrid = 1;
             grid = (unsigned)(P.Vc / 2);
         }
+        const long long rstride = (long long)nchunks(dims) * CH * 24;  // right-hand sides back to back
 #define LAUNCH_MR(ACC, BVC)                                                                                   \
     do {                                                                                                      \
         static bool attr = false;                                                                             \
@@ -598,7 +609,7 @@ static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa
                                  max_optin_smem());                                                           \
             attr = true;                                                                                      \
         }                                                                                                     \
-        k_mr_domain<T, ACC, BVC><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter);               \
+        k_mr_domain<T, ACC, BVC><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter, K, rstride);   \
     } while (0)
         if (sizeof(T) == 4 && P.bv == 256) {  // the paper's typical 4^4 domain
             if (acc) LAUNCH_MR(true, (sizeof(T) == 4 ? 256 : 0));
@@ -620,14 +631,17 @@ static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa
     const size_t nreal = (size_t)nchunks(dims) * CH * 24;
     T* rho = reinterpret_cast<T*>(ws);
     T* p = rho + nreal;
-    k_mr_init<T><<<(unsigned)P.Vc, 128, 0, st>>>(rho, acc ? nullptr : z, r, P);
-    count_launch();
     const unsigned ddflags = flags & (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD);
-    for (int it = 0; it < niter; it++) {
-        rc = wilson_clover_call<T>(p, rho, U, clover, nullptr, kappa, dims, bc, domain, ddflags, stream, what);
-        if (rc) return rc;
-        k_mr_update<T><<<(unsigned)P.Vc, 128, 0, st>>>(z, rho, p, P);
+    for (int k = 0; k < K; k++) {  // one right-hand side after the other
+        T* zk = z + k * nreal;
+        k_mr_init<T><<<(unsigned)P.Vc, 128, 0, st>>>(rho, acc ? nullptr : zk, r + k * nreal, P);
         count_launch();
+        for (int it = 0; it < niter; it++) {
+            rc = wilson_clover_call<T>(p, rho, U, clover, nullptr, kappa, dims, bc, domain, ddflags, stream, what);
+            if (rc) return rc;
+            k_mr_update<T><<<(unsigned)P.Vc, 128, 0, st>>>(zk, rho, p, P);
+            count_launch();
+        }
     }
     return check_launch(what);
 }
@@ -635,10 +649,10 @@ static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa
 // SAP with fixed iterations.  x: solution; r: scratch, receives the residual; b: right-hand side.
 template <typename T>
 static int sap_call(T* x, T* r, const T* b, const T* U, const T* clover, T kappa, const int dims[4], const int bc[4],
-                    const int domain[4], int n_sap, int n_mr, unsigned flags, void* ws, void* stream,
+                    const int domain[4], int n_sap, int n_mr, int K, unsigned flags, void* ws, void* stream,
                     const char* what) {
     clear_error();
-    if (!x || !r || !b || !U || !clover || !bc || check_dims(dims) || !domain) {
+    if (!x || !r || !b || !U || !clover || !bc || check_dims(dims) || !domain || K < 1) {
         set_error("%s: null pointer or non-positive dim", what);
         return LQCD_EINVAL;
     }
@@ -664,12 +678,20 @@ static int sap_call(T* x, T* r, const T* b, const T* U, const T* clover, T kappa
         }
     }
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t bytes = (size_t)nchunks(dims) * CH * 24 * sizeof(T);
+    const long long nreal = (long long)nchunks(dims) * CH * 24;  // K vectors back to back
+    const size_t bytes = (size_t)nreal * sizeof(T) * K;
     int rc;
+    auto residual = [&]() -> int {  // |r_k> := |b_k> - D|x_k>
+        for (int k = 0; k < K; k++) {
+            const int e = wilson_clover_call<T>(r + k * nreal, x + k * nreal, U, clover, b + k * nreal, kappa, dims, bc,
+                                                nullptr, 0, stream, what);
+            if (e) return e;
+        }
+        return LQCD_OK;
+    };
     const T* res = r;
-    if (flags & LQCD_SAP_INITIAL_GUESS) {  // |r> := |b> - D|x>
-        rc = wilson_clover_call<T>(r, x, U, clover, b, kappa, dims, bc, nullptr, 0, stream, what);
-        if (rc) return rc;
+    if (flags & LQCD_SAP_INITIAL_GUESS) {
+        if ((rc = residual())) return rc;
     } else {  // |x> := 0, |r> := |b>: the first half sweep reads b itself
         if (cudaMemsetAsync(x, 0, bytes, st) != cudaSuccess) return check_launch(what);
         res = b;
@@ -678,16 +700,14 @@ static int sap_call(T* x, T* r, const T* b, const T* U, const T* clover, T kappa
     }
     for (int i = 0; i < n_sap; i++)
         for (int g = 0; g < 2; g++) {
-            // |x> := |x> + M_SAP^(e/o)|r>
+            // |x_k> := |x_k> + M_SAP^(e/o)|r_k>, all k on the resident operator of each domain
             rc = mr_domain_call<T>(x, res, U, clover, kappa, dims, bc, domain,
-                                   (g == 0 ? LQCD_DOMAIN_EVEN : LQCD_DOMAIN_ODD) | LQCD_ACCUMULATE, n_mr, ws, stream,
+                                   (g == 0 ? LQCD_DOMAIN_EVEN : LQCD_DOMAIN_ODD) | LQCD_ACCUMULATE, n_mr, K, ws, stream,
                                    what);
             if (rc) return rc;
             const bool last = (i == n_sap - 1 && g == 1);
             if (last && (flags & LQCD_SAP_NO_FINAL_RESIDUAL)) break;
-            // |r> := |b> - D|x>
-            rc = wilson_clover_call<T>(r, x, U, clover, b, kappa, dims, bc, nullptr, 0, stream, what);
-            if (rc) return rc;
+            if ((rc = residual())) return rc;
             res = r;
         }
     return LQCD_OK;
@@ -749,26 +769,38 @@ int lqcd_block_caxpy_f64(double* y, const double* coef, const double* a, const i
 int lqcd_mr_domain_solve_f32(float* z, const float* r, const float* U, const float* clover, float kappa,
                              const int dims[4], const int bc[4], const int domain[4], unsigned flags, int niter,
                              void* ws_dev, void* stream) {
-    return mr_domain_call<float>(z, r, U, clover, kappa, dims, bc, domain, flags, niter, ws_dev, stream,
+    return mr_domain_call<float>(z, r, U, clover, kappa, dims, bc, domain, flags, niter, 1, ws_dev, stream,
                                  "lqcd_mr_domain_solve_f32");
 }
 int lqcd_mr_domain_solve_f64(double* z, const double* r, const double* U, const double* clover, double kappa,
                              const int dims[4], const int bc[4], const int domain[4], unsigned flags, int niter,
                              void* ws_dev, void* stream) {
-    return mr_domain_call<double>(z, r, U, clover, kappa, dims, bc, domain, flags, niter, ws_dev, stream,
+    return mr_domain_call<double>(z, r, U, clover, kappa, dims, bc, domain, flags, niter, 1, ws_dev, stream,
                                   "lqcd_mr_domain_solve_f64");
 }
 
 int lqcd_sap_f32(float* x, float* r, const float* b, const float* U, const float* clover, float kappa,
                  const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
                  void* ws_dev, void* stream) {
-    return sap_call<float>(x, r, b, U, clover, kappa, dims, bc, domain, n_sap, n_mr, flags, ws_dev, stream,
+    return sap_call<float>(x, r, b, U, clover, kappa, dims, bc, domain, n_sap, n_mr, 1, flags, ws_dev, stream,
                            "lqcd_sap_f32");
 }
 int lqcd_sap_f64(double* x, double* r, const double* b, const double* U, const double* clover, double kappa,
                  const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
                  void* ws_dev, void* stream) {
-    return sap_call<double>(x, r, b, U, clover, kappa, dims, bc, domain, n_sap, n_mr, flags, ws_dev, stream,
+    return sap_call<double>(x, r, b, U, clover, kappa, dims, bc, domain, n_sap, n_mr, 1, flags, ws_dev, stream,
                             "lqcd_sap_f64");
+}
+int lqcd_sap_mrhs_f32(float* x, float* r, const float* b, const float* U, const float* clover, float kappa,
+                      const int dims[4], const int bc[4], const int domain[4], int nrhs, int n_sap, int n_mr,
+                      unsigned flags, void* ws_dev, void* stream) {
+    return sap_call<float>(x, r, b, U, clover, kappa, dims, bc, domain, n_sap, n_mr, nrhs, flags, ws_dev, stream,
+                           "lqcd_sap_mrhs_f32");
+}
+int lqcd_sap_mrhs_f64(double* x, double* r, const double* b, const double* U, const double* clover, double kappa,
+                      const int dims[4], const int bc[4], const int domain[4], int nrhs, int n_sap, int n_mr,
+                      unsigned flags, void* ws_dev, void* stream) {
+    return sap_call<double>(x, r, b, U, clover, kappa, dims, bc, domain, n_sap, n_mr, nrhs, flags, ws_dev, stream,
+                            "lqcd_sap_mrhs_f64");
 }
 }

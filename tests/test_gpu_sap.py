@@ -252,3 +252,39 @@ def test_sap_error_codes(lq):
     finally:
         lq.set_knob("sap_fused", 0)
     assert lq.launch_count() == n0, "nothing is enqueued on error"
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_sap_mrhs_is_sap_per_rhs(lq, prec, path):
+    """several right-hand sides on the resident operator: bit-identical with one call per right-hand side (both
+    paths), hence covered by the oracle comparisons above; one right-hand side is checked against the oracle again"""
+    import torch
+    prob = make_problem(__import__("lqcd_inputs").CONFIGS["c1"], n_rhs=3, coarse="none")
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec, coarse=False)
+    b = torch.stack([lq.pack_spinor(to_dev(p, prec), cfg.dims) for p in prob.psi])
+    ws = lq.mr_workspace(cfg.dims, cfg.block, dtype=rdtype(lq, prec))
+    x, r = torch.full_like(b, 3.0), torch.full_like(b, 3.0)
+    lq.sap_mrhs(x, r, b, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=4, ws=ws)
+    x1, r1 = lq.empty_spinor(cfg.dims, dtype=b.dtype), lq.empty_spinor(cfg.dims, dtype=b.dtype)
+    for k in range(3):
+        lq.sap(x1, r1, b[k], d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=4, ws=ws)
+        assert torch.equal(x[k], x1) and torch.equal(r[k], r1), k
+    U, clov = fields(prob, prec)
+    rx, rr = oracle.sap(rounded(prob.psi[2], prec), U, clov, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=4)
+    assert rel_l2(lq.unpack_spinor(x[2], cfg.dims).cpu().numpy(), rx) <= 2 * 2 * 5 * TOL1[prec]
+
+
+def test_sap_mrhs_4x4_domains(lq):
+    """8^4 with 4^4 domains in fp32: the compile-time 256-site resident kernel with its right-hand-side loop"""
+    import torch
+    cfg = custom_config((8, 8, 8, 8), (4, 4, 4, 4), 1, gauge="exp", eps=0.5, kappa=0.135, csw=1.0)
+    prob = make_problem(cfg, n_rhs=4, coarse="none")
+    d = Dev(lq, prob, "f32", coarse=False)
+    b = torch.stack([lq.pack_spinor(to_dev(p, "f32"), cfg.dims) for p in prob.psi])
+    x, r = torch.full_like(b, 3.0), torch.full_like(b, 3.0)
+    lq.sap_mrhs(x, r, b, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=6)
+    x1, r1 = lq.empty_spinor(cfg.dims), lq.empty_spinor(cfg.dims)
+    for k in range(4):
+        lq.sap(x1, r1, b[k], d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=6)
+        assert torch.equal(x[k], x1) and torch.equal(r[k], r1), k
