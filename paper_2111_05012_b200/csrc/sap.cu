@@ -20,6 +20,11 @@ template <typename T>
 int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
                        const int bc[4], const int* domain, unsigned flags, void* stream, const char* what);
 
+// (wilson_clover.cu) out_k = rhs_k - D in_k for nrhs vectors back to back, pairs sharing the links and the clover term
+template <typename T>
+int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
+                            const int bc[4], int nrhs, unsigned flags, void* stream, const char* what);
+
 struct DomParams {
     int L[4], dom[4], Lc[4], bc[4], multi[4];
     int bv, Vc;
@@ -681,13 +686,9 @@ static int sap_call(T* x, T* r, const T* b, const T* U, const T* clover, T kappa
     const long long nreal = (long long)nchunks(dims) * CH * 24;  // K vectors back to back
     const size_t bytes = (size_t)nreal * sizeof(T) * K;
     int rc;
-    auto residual = [&]() -> int {  // |r_k> := |b_k> - D|x_k>
-        for (int k = 0; k < K; k++) {
-            const int e = wilson_clover_call<T>(r + k * nreal, x + k * nreal, U, clover, b + k * nreal, kappa, dims, bc,
-                                                nullptr, 0, stream, what);
-            if (e) return e;
-        }
-        return LQCD_OK;
+    auto residual = [&]() -> int {  // |r_k> := |b_k> - D|x_k>; right-hand sides in pairs (links, clover read once)
+        if (K == 1) return wilson_clover_call<T>(r, x, U, clover, b, kappa, dims, bc, nullptr, 0, stream, what);
+        return wilson_clover_mrhs_call<T>(r, x, U, clover, b, kappa, dims, bc, K, 0, stream, what);
     };
     const T* res = r;
     if (flags & LQCD_SAP_INITIAL_GUESS) {

@@ -373,10 +373,11 @@ __device__ __forceinline__ void hop_mrhs(T (&acc)[NRHS][24], const T* __restrict
     }
 }
 
-template <typename T, bool DAG, bool L12, int NRHS>
+// RES: out_k = rhs_k - D in_k (the residual of SAP / of a Richardson step), rhs_k = rhs + k * rstride
+template <typename T, bool DAG, bool L12, int NRHS, bool RES>
 __global__ void __launch_bounds__(128, sizeof(T) == 4 ? 3 : 2)
     k_wilson_clover_mrhs(T* __restrict__ out, const T* __restrict__ in, long long rstride, const T* __restrict__ U,
-                         const T* __restrict__ clover, T kappa, FineParams P) {
+                         const T* __restrict__ clover, const T* __restrict__ rhs, T kappa, FineParams P) {
     int x[4], s;
     if (!fine_decode(P, x, s)) return;
     const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
@@ -432,6 +433,11 @@ __global__ void __launch_bounds__(128, sizeof(T) == 4 ? 3 : 2)
                 V16<T> v;
 #pragma unroll
                 for (int q = 0; q < NV; q++) v.r[q] = o[j * NV + q];
+                if (RES) {
+                    const V16<T> bb = ld16_stream(rhs + k * rstride + sp_off + (long long)(NH * chi + j) * CH * NV);
+#pragma unroll
+                    for (int q = 0; q < NV; q++) v.r[q] = bb.r[q] - v.r[q];
+                }
                 st16_stream(out + k * rstride + sp_off + (long long)(NH * chi + j) * CH * NV, v);
             }
         }
@@ -439,8 +445,8 @@ __global__ void __launch_bounds__(128, sizeof(T) == 4 ? 3 : 2)
 }
 
 template <typename T>
-static int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4],
-                                   const int bc[4], int nrhs, unsigned flags, void* stream, const char* what) {
+int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
+                            const int bc[4], int nrhs, unsigned flags, void* stream, const char* what) {
     clear_error();
     if (!out || !in || !U || !clover || check_dims(dims) || !bc || nrhs < 1) {
         set_error("%s: null pointer, non-positive dim or nrhs < 1", what);
@@ -450,8 +456,8 @@ static int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clo
         set_error("%s: pointers must be 16-byte aligned and out must not alias in", what);
         return LQCD_EINVAL;
     }
-    if (flags & ~(LQCD_DAGGER | LQCD_LINKS_12)) {
-        set_error("%s: unknown flag bits 0x%x", what, flags);
+    if ((flags & ~(LQCD_DAGGER | LQCD_LINKS_12)) || (rhs && ((flags & LQCD_DAGGER) || !aligned16(rhs)))) {
+        set_error("%s: unknown flag bits 0x%x (the residual form takes no LQCD_DAGGER)", what, flags);
         return LQCD_EINVAL;
     }
     if (volume(dims) > 0x7fffffffLL) {
@@ -474,22 +480,32 @@ static int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clo
         for (; k + 2 <= nrhs; k += 2) {  // pairs of right-hand sides
             T* o = out + k * rstride;
             const T* i = in + k * rstride;
-            if (dag && l12) k_wilson_clover_mrhs<T, true, true, 2><<<(unsigned)ntiles, threads, 0, st>>>(o, i, rstride, U, clover, kappa, P);
-            else if (dag) k_wilson_clover_mrhs<T, true, false, 2><<<(unsigned)ntiles, threads, 0, st>>>(o, i, rstride, U, clover, kappa, P);
-            else if (l12) k_wilson_clover_mrhs<T, false, true, 2><<<(unsigned)ntiles, threads, 0, st>>>(o, i, rstride, U, clover, kappa, P);
-            else k_wilson_clover_mrhs<T, false, false, 2><<<(unsigned)ntiles, threads, 0, st>>>(o, i, rstride, U, clover, kappa, P);
+            const T* bk = rhs ? rhs + k * rstride : nullptr;
+            const unsigned g = (unsigned)ntiles;
+            if (rhs && l12) k_wilson_clover_mrhs<T, false, true, 2, true><<<g, threads, 0, st>>>(o, i, rstride, U, clover, bk, kappa, P);
+            else if (rhs) k_wilson_clover_mrhs<T, false, false, 2, true><<<g, threads, 0, st>>>(o, i, rstride, U, clover, bk, kappa, P);
+            else if (dag && l12) k_wilson_clover_mrhs<T, true, true, 2, false><<<g, threads, 0, st>>>(o, i, rstride, U, clover, bk, kappa, P);
+            else if (dag) k_wilson_clover_mrhs<T, true, false, 2, false><<<g, threads, 0, st>>>(o, i, rstride, U, clover, bk, kappa, P);
+            else if (l12) k_wilson_clover_mrhs<T, false, true, 2, false><<<g, threads, 0, st>>>(o, i, rstride, U, clover, bk, kappa, P);
+            else k_wilson_clover_mrhs<T, false, false, 2, false><<<g, threads, 0, st>>>(o, i, rstride, U, clover, bk, kappa, P);
             count_launch();
         }
         const int rc = check_launch(what);
         if (rc) return rc;
     }
     for (; k < nrhs; k++) {  // an odd one out (or a user tile of more than 128 sites): the single-right-hand-side kernel
-        const int rc = wilson_clover_call<T>(out + k * rstride, in + k * rstride, U, clover, nullptr, kappa, dims, bc,
-                                             nullptr, flags, stream, what);
+        const int rc = wilson_clover_call<T>(out + k * rstride, in + k * rstride, U, clover,
+                                             rhs ? rhs + k * rstride : nullptr, kappa, dims, bc, nullptr, flags, stream,
+                                             what);
         if (rc) return rc;
     }
     return LQCD_OK;
 }
+
+template int wilson_clover_mrhs_call<float>(float*, const float*, const float*, const float*, const float*, float,
+                                            const int*, const int*, int, unsigned, void*, const char*);
+template int wilson_clover_mrhs_call<double>(double*, const double*, const double*, const double*, const double*,
+                                             double, const int*, const int*, int, unsigned, void*, const char*);
 
 }  // namespace lqcd
 
@@ -553,13 +569,13 @@ int lqcd_wilson_clover_residual_f64(double* r, const double* b, const double* x,
 extern "C" {
 int lqcd_wilson_clover_mult_mrhs_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
                                      const int dims[4], const int bc[4], int nrhs, unsigned flags, void* stream) {
-    return wilson_clover_mrhs_call<float>(out, in, U, clover, kappa, dims, bc, nrhs, flags, stream,
+    return wilson_clover_mrhs_call<float>(out, in, U, clover, nullptr, kappa, dims, bc, nrhs, flags, stream,
                                           "lqcd_wilson_clover_mult_mrhs_f32");
 }
 int lqcd_wilson_clover_mult_mrhs_f64(double* out, const double* in, const double* U, const double* clover,
                                      double kappa, const int dims[4], const int bc[4], int nrhs, unsigned flags,
                                      void* stream) {
-    return wilson_clover_mrhs_call<double>(out, in, U, clover, kappa, dims, bc, nrhs, flags, stream,
+    return wilson_clover_mrhs_call<double>(out, in, U, clover, nullptr, kappa, dims, bc, nrhs, flags, stream,
                                            "lqcd_wilson_clover_mult_mrhs_f64");
 }
 }
