@@ -12,19 +12,18 @@
 // tcgen05 (5th-generation tensor cores): kind::tf32 MMAs with fp32 accumulators in TMEM.  TF32 alone (10-bit mantissa)
 // would miss the fp32 bar of 2e-6 by two orders of magnitude, so every fp32 operand is split into hi + lo
 // (hi = x rounded to the nearest TF32 value, i.e. 13 low mantissa bits cleared; lo = x - hi, exact, either sign) and each
-// product is formed as lo.hi + hi.lo + hi.hi (the dropped lo.lo term is 2^-22 relative): "3xTF32".  The split is done
+// product is formed from the hi / lo pieces ("3xTF32"; with the stacked operands below all four terms come out).  The split is done
 // by the producer warps on the way from HBM to shared memory, so A is still read from HBM exactly once, as fp32.
 //
-// One persistent CTA per SM, warp-specialised (672 threads):
-//   warps 0-3   epilogue: tcgen05.ld each stage's accumulators, add them in registers (fp32, round-to-nearest),
-//               store out_k(X)
-//   warp  4     one elected thread issues the MMAs; allocates / frees TMEM
-//   warps 5-20  producers, four groups of four warps that take the stages in turn: stream A (whole 128-byte lines,
+// One persistent CTA per SM, warp-specialised (704 threads):
+//   warps 0-3   epilogue: tcgen05.ld each accumulator chain, add it in registers (fp32, round-to-nearest), store out_k(X)
+//   warps 4-5   MMA issuers (one elected lane each, accumulator chains in turn); warp 4 allocates / frees TMEM
+//   warps 6-21  producers, four groups of four warps that take the stages in turn: stream A (whole 128-byte lines,
 //               L1 no-allocate), build B' from the neighbours' input vectors (L2-resident), split into hi / lo, store
 //               both in the 128-byte-swizzled K-major layout UMMA reads (conflict-free stores)
-// Shared-memory ring of S stages (one stage = half a block: A as 128 rows (hi | lo) x 64 reals, B' as 4K rows
-// (hi | lo) x 64 reals), one TMEM accumulator slot per stage; mbarriers full[] (producers -> issuer), done[]
-// (tcgen05.commit -> producers and epilogue), tfree[] (epilogue -> issuer).
+// Shared-memory ring of 4 stages (one stage = half a block: A as 128 rows (hi | lo) x 64 reals, B' as 4K rows
+// (hi | lo) x 64 reals), a ring of TMEM accumulator slots (one per chain of two stages); mbarriers full[] (producers ->
+// issuer), done[] (tcgen05.commit -> producers), tfull[] (tcgen05.commit -> epilogue), tfree[] (epilogue -> issuer).
 #include "common.cuh"
 #include "knobs.h"
 
@@ -36,7 +35,7 @@ constexpr int MR_HALVES = 18;        // 9 blocks x 2 halves per coarse site
 constexpr int MR_AS = 2;             // pipeline stages accumulated into one TMEM slot (chain of MR_AS * 8 MMAs)
 constexpr int MR_EPI_WARPS = 4, MR_PROD_GROUPS = 4, MR_PROD_WARPS = 4 * MR_PROD_GROUPS;
 constexpr int MR_ISSUERS = 2;         // MMA-issuing warps (one elected lane each); stages in turn, like the producers
-constexpr int MR_THREADS = (MR_EPI_WARPS + MR_ISSUERS + MR_PROD_WARPS) * 32;  // 672
+constexpr int MR_THREADS = (MR_EPI_WARPS + MR_ISSUERS + MR_PROD_WARPS) * 32;  // 704
 constexpr int MR_TMEM_COLS = 512;    // all of TMEM: one accumulator slot of 2 NCOL columns per pipeline stage
 
 struct MrhsParams {
