@@ -5,9 +5,9 @@
 //
 // B200 design: a 4^4 domain's residual, links and clover term are 168 KB in fp32 -- they
 // fit the 227 KB of shared memory of one SM (192 KB with the exchange buffer of the two-threads-per-site split).
-// k_mr_domain therefore runs ALL n_mr iterations of one domain inside one CTA: the operator fields are read from HBM once per half sweep instead of once per iteration, the blocked
-// dot products are CTA reductions, the blocked axpys are register updates, and nothing but the solution goes back
-// to HBM.  Domains that do not fit (fp64 4^4, 8x4^3) take the generic path: D_SAP^(e/o) by k_wilson_clover and
+// k_mr_domain therefore runs ALL n_mr iterations of one domain inside one CTA: the operator fields are read from
+// HBM once per half sweep instead of once per iteration, the blocked dot products are CTA reductions, the blocked
+// axpys are register updates, and nothing but the solution goes back to HBM.  Domains that do not fit (fp64 4^4, 8x4^3) take the generic path: D_SAP^(e/o) by k_wilson_clover and
 // one fused blocked dotc/dotc/axpy/axpy kernel per iteration.
 #include "common.cuh"
 #include "fermion.cuh"
