@@ -178,8 +178,9 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
     const int lane = s & 31;
     const long long chunk = s >> 5;
     const long long sp_off = (chunk * NJ * CH + lane) * NV;  // native spinor row 0 of site s
-    if (!selected) {  // only reached without ACC: M^(g) r vanishes outside the group
-        if (active) {
+    if (!selected) {  // M^(g) r vanishes outside the group: zero without ACC, x untouched with ACC (reached with ACC
+                      // only when Lc[0] is odd and the grid therefore enumerates all domains)
+        if (!ACC && active) {
             V16<T> zero;
 #pragma unroll
             for (int q = 0; q < NV; q++) zero.r[q] = 0;

@@ -288,3 +288,25 @@ def test_sap_mrhs_4x4_domains(lq):
     for k in range(4):
         lq.sap(x1, r1, b[k], d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=6)
         assert torch.equal(x[k], x1) and torch.equal(r[k], r1), k
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,domain,bc", [
+    ((6, 4, 2, 10), (3, 4, 1, 5), (-1, 1, -1, 1)),     # odd domain counts (same-parity neighbours across the wrap),
+                                                       # a direction spanned by one domain, one-site-thick domains
+    ((3, 3, 3, 3), (3, 1, 3, 1), (1, 1, 1, -1)),       # V = 81, 9 domains
+    ((16, 8, 8, 8), (8, 4, 4, 4), (1, 1, 1, -1)),      # the paper's 8x4x4x4 domains: generic path
+])
+def test_sap_edge_lattices(lq, prec, dims, domain, bc, path):
+    cfg = custom_config(dims, (1, 1, 1, 1), 1, bc=bc)
+    prob = make_problem(cfg, coarse="none")
+    if np.prod(domain) >= 512 and path == -1:
+        pytest.skip("same path as the resident parametrisation")
+    d = Dev(lq, prob, prec, coarse=False)
+    U, clov = fields(prob, prec)
+    b = prob.psi[0]
+    rx, rr = oracle.sap(rounded(b, prec), U, clov, cfg.kappa, dims, bc, domain, n_sap=3, n_mr=4)
+    gx, gr = gpu_sap(lq, d, b, domain, 3, 4)
+    bar = 2 * 3 * 5 * TOL1[prec]
+    assert rel_l2(gx, rx) <= bar
+    assert np.linalg.norm(gr - rr) / np.linalg.norm(b) <= bar
