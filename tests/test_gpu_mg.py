@@ -217,3 +217,32 @@ def test_vcycle_mrhs(lq, prec, name, nrhs):
         ref = oracle_vcycle(prob, prec, prob.psi[k], n_coarse, n_sap, n_mr)
         got = lq.unpack_spinor(x[k], cfg.dims).cpu().numpy()
         assert rel_l2(got, ref) <= bar, (k, rel_l2(got, ref), bar)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,block,nvec,bc", [
+    ((6, 4, 6, 4), (2, 2, 2, 2), 3, (1, 1, 1, -1)),     # odd coarse extents (3, 2, 3, 2), odd N_nv, coarse extent 2
+    ((4, 6, 4, 8), (2, 3, 2, 4), 5, (-1, 1, -1, 1)),    # non-cubic blocks, other boundary conditions
+])
+def test_vcycle_edge_lattices(lq, prec, dims, block, nvec, bc):
+    """single and batched V-cycle on odd lattices against the oracle, including the degenerate iteration counts"""
+    import torch
+    from problems import custom_config, make_problem
+    cfg = custom_config(dims, block, nvec, bc=bc)
+    prob = make_problem(cfg, n_rhs=3)
+    d = Dev(lq, prob, prec)
+    cond = cond_coarse(prob, prec)
+    assert cond < 200
+    b = torch.stack([lq.pack_spinor(to_dev(p, prec), cfg.dims) for p in prob.psi])
+    for n_coarse, n_sap, n_mr in ((4, 2, 4), (0, 1, 3), (2, 0, 3)):
+        x = torch.full_like(b, 2.0)
+        lq.mg_vcycle_mrhs(x, b, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, cfg.nvec, d.v, d.A,
+                          n_coarse=n_coarse, n_sap=n_sap, n_mr=n_mr)
+        bar = (2 * n_coarse * cond + 2 + 2 * n_sap * (n_mr + 1)) * TOL1[prec]
+        for k in range(3):
+            ref = oracle_vcycle(prob, prec, prob.psi[k], n_coarse, n_sap, n_mr)
+            got = lq.unpack_spinor(x[k], cfg.dims).cpu().numpy()
+            assert rel_l2(got, ref) <= bar, (n_coarse, n_sap, n_mr, k, rel_l2(got, ref), bar)
+        # the single-right-hand-side call gives the same
+        got1 = gpu_vcycle(lq, d, prob.psi[0], n_coarse, n_sap, n_mr)
+        assert rel_l2(got1, lq.unpack_spinor(x[0], cfg.dims).cpu().numpy()) <= bar

@@ -225,3 +225,28 @@ def test_prolong_mrhs(lq, prec, name, nrhs):
     for k in range(nrhs):
         ref = oracle.prolong(rounded(xs[k], prec), rounded(prob.v, prec), cfg.dims, cfg.block)
         assert rel_l2(lq.unpack_spinor(out[k], cfg.dims).cpu().numpy(), ref) <= TOL[prec], k
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_transfer_mrhs_large_and_odd_blocks(lq, prec):
+    """8x4x4x4 blocks (24 / 48 KB per slice: fewer slices per group) and a 2x3x2x2 block with odd N_nv"""
+    import torch
+    from problems import custom_config, make_problem
+    for dims, block, nvec, nrhs in (((16, 8, 8, 8), (8, 4, 4, 4), 4, 5), ((4, 6, 4, 4), (2, 3, 2, 2), 3, 10)):
+        cfg = custom_config(dims, block, nvec)
+        prob = make_problem(cfg, coarse="synthetic")
+        d = Dev(lq, prob, prec)
+        rng = np.random.default_rng(17)
+        psis = [rng.standard_normal((cfg.volume, 4, 3)) + 1j * rng.standard_normal((cfg.volume, 4, 3))
+                for _ in range(nrhs)]
+        x = torch.stack([lq.pack_spinor(to_dev(p, prec), dims) for p in psis])
+        out = torch.full((nrhs, cfg.cvolume, 2, nvec), 3.0, dtype=to_dev(np.zeros(1), prec).dtype, device="cuda")
+        lq.restrict_mrhs(out, x, d.v, dims, block, nvec)
+        xs = rhs_set(cfg, nrhs, seed=8)
+        fine = torch.full_like(x, 3.0)
+        lq.prolong_mrhs(fine, to_dev(xs, prec), d.v, dims, block, nvec)
+        for k in range(nrhs):
+            assert rel_l2(out[k].cpu().numpy(), oracle.restrict(rounded(psis[k], prec), rounded(prob.v, prec), dims,
+                                                                block)) <= TOL[prec], (dims, k)
+            assert rel_l2(lq.unpack_spinor(fine[k], dims).cpu().numpy(),
+                          oracle.prolong(rounded(xs[k], prec), rounded(prob.v, prec), dims, block)) <= TOL[prec], (dims, k)
