@@ -250,3 +250,23 @@ def test_transfer_mrhs_large_and_odd_blocks(lq, prec):
                                                                 block)) <= TOL[prec], (dims, k)
             assert rel_l2(lq.unpack_spinor(fine[k], dims).cpu().numpy(),
                           oracle.prolong(rounded(xs[k], prec), rounded(prob.v, prec), dims, block)) <= TOL[prec], (dims, k)
+
+
+@pytest.mark.parametrize("cdims", [(3, 2, 3, 2), (2, 5, 3, 4), (7, 3, 2, 3)])
+def test_tensor_core_path_odd_coarse_lattices(lq, cdims):
+    """odd and mixed coarse extents (multiply-high division by 3, 5, 7; wraps in every direction), synthetic blocks"""
+    import torch
+    nv = 32
+    Vc = int(np.prod(cdims))
+    rng = np.random.default_rng(sum(cdims))
+    A = li.coarse_matrix_synthetic(rng, Vc, nv)
+    xs = np.stack([li.coarse_vector(rng, Vc, nv) for _ in range(7)])
+    Ad, xd = to_dev(A, "f32"), to_dev(xs, "f32")
+    y = torch.full_like(xd, 3.0)
+    n0 = lq.launch_count()
+    lq.coarse_mult_mrhs(y, xd, Ad, cdims, nv)
+    assert lq.launch_count() - n0 == 1, "tensor-core path"
+    got = y.cpu().numpy()
+    for k in range(7):
+        ref = oracle.coarse_mult(rounded(xs[k], "f32"), rounded(A, "f32"), cdims)
+        assert rel_l2(got[k], ref) <= TOL["f32"], k
