@@ -132,3 +132,32 @@ def test_clover_from_links_feeds_the_operator(lq):
     ref = oracle.wilson_clover_mult(psi64, U64, oracle.clover_from_links(U64, cfg.kappa, cfg.csw, cfg.dims), cfg.kappa,
                                     cfg.dims, cfg.bc)
     assert rel_l2(got, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,block,nvec,bc", [
+    ((6, 4, 6, 4), (2, 2, 2, 2), 3, (1, 1, 1, -1)),     # odd coarse extents, coarse extent 2, odd N_nv
+    ((4, 6, 4, 8), (2, 3, 2, 4), 5, (-1, 1, -1, 1)),    # non-cubic blocks, other boundary conditions
+])
+def test_setup_chain_edge_lattices(lq, prec, dims, block, nvec, bc):
+    """clover term, block orthonormalisation and Galerkin assembly on odd lattices: each against the oracle"""
+    from problems import custom_config
+    import lqcd_inputs as li_
+    cfg = custom_config(dims, block, nvec, bc=bc)
+    hf = li_.make_host_fields(cfg, n_rhs=1, with_nullvecs=True)
+    Un = lq.pack_gauge(to_dev(hf.U, prec), cfg.dims)
+    Cn = lq.clover_from_links(Un, cfg.kappa, cfg.csw, cfg.dims)
+    clov_ref = oracle.clover_from_links(rounded(hf.U, prec), cfg.kappa, cfg.csw, cfg.dims)
+    assert rel_l2(lq.unpack_clover(Cn, cfg.dims).cpu().numpy(), clov_ref) <= 4 * TOL[prec]
+    # from here on both sides consume the oracle's clover term and the oracle's orthonormal vectors
+    v_ref = oracle.orthonormalize_blocks(rounded(hf.v, prec), cfg.dims, cfg.block)
+    vn = lq.pack_nullvecs(to_dev(hf.v, prec), cfg.dims, cfg.block)
+    lq.orthonormalize_blocks(vn, cfg.dims, cfg.block, cfg.nvec)
+    got_v = np.stack([lq.unpack_nullvec(vn, i, cfg.dims, cfg.block, cfg.nvec).cpu().numpy() for i in range(cfg.nvec)])
+    assert rel_l2(got_v, v_ref) <= 4 * TOL[prec]
+    Cn2 = lq.pack_clover(to_dev(clov_ref, prec), cfg.dims)
+    vn2 = lq.pack_nullvecs(to_dev(v_ref, prec), cfg.dims, cfg.block)
+    got = lq.galerkin_coarse(Un, Cn2, vn2, cfg.kappa, cfg.dims, cfg.bc, cfg.block, cfg.nvec).cpu().numpy()
+    ref = oracle.galerkin_coarse(rounded(hf.U, prec), rounded(clov_ref, prec), rounded(v_ref, prec), cfg.kappa, cfg.dims,
+                                 cfg.bc, cfg.block)
+    assert rel_l2(got, ref) <= TOL[prec]
