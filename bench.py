@@ -319,6 +319,9 @@ class Workload:
         c = self.cfg
         self.lq.wilson_clover_mult_mrhs(self.y2[i % 2], self.x2[i % 2], self.U18, self.clover, c.kappa, c.dims, c.bc)
 
+    def sharded_self(self, i):
+        self.sharded_op.apply(self.y[i], self.x[i])
+
     def coarse_mrhs(self, i):
         c = self.cfg
         self.lq.coarse_mult_mrhs(self.ycK, self.xcK, self.A, c.cdims, c.nvec)
@@ -679,6 +682,20 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "speedup_vs_2_single_applications": 2 * kernels["wilson_clover"]["us"] * 1e-6 / t,
             "frac_of_hbm_peak": fb / t / 1e9 / peak, "bytes_per_launch": fb}
         del W.x2, W.y2
+        # SURVEY 8(e), the sharded operator's own cost on one GPU: all four directions partitioned, the rank its own
+        # neighbour (pack -> interior -> add; no link traffic, so this is the kernels' overhead over the plain D)
+        from paper_2111_05012_b200 import sharded as sh
+        W.sharded_op = sh.ShardedWilsonClover(W.U18, W.clover, cfg.kappa, cfg.dims, cfg.bc, sh.RankGrid((1, 1, 1, 1)),
+                                              part_mask=15)
+        t = time_single(W, "sharded_self", reps=max(10, args.steps))
+        face_b = 2 * 4 * sum(W.lq.halo_face_reals(cfg.dims, mu) for mu in range(4))
+        extra["wilson_clover_sharded_selfhalo"] = {
+            "us": t * 1e6, "overhead_vs_plain": t / (kernels["wilson_clover"]["us"] * 1e-6),
+            "GBps": m["wilson_clover"]["bytes"] / t / 1e9, "halo_bytes_sent_per_application": face_b,
+            "launches_per_application": 6,
+            "note": "one rank exchanging with itself in all 4 directions; a multi-GPU run adds only the transfer of "
+                    "halo_bytes (12 reals per face site), overlapped with the interior pass"}
+        del W.sharded_op
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)

@@ -359,6 +359,44 @@ int lqcd_wilson_clover_mult_mrhs_f64(double* out, const double* in, const double
                                      double kappa, const int dims[4], const int bc[4], int nrhs, unsigned flags,
                                      void* stream);
 
+/* ---- Sharded fine operator: the halo-exchange step (the paper partitions the lattice over
+ * the nodes in 4-D and exchanges the boundary once per application of D) --------------
+ * A rank owns the local lattice dims[4] (all fields in the native layouts of that local lattice).  Bit mu of
+ * part_mask says that direction mu is partitioned: hops that leave the local lattice there are served by the
+ * neighbouring rank (which may be the rank itself).  One application of D (Eq. 1) or D^dag (Eq. 2) is
+ *   lqcd_wilson_clover_halo_pack      in  -> send[8]       (independent of the next line: they overlap on two streams)
+ *   lqcd_wilson_clover_mult_interior  in  -> out           D with the leaving hops switched off
+ *   -- exchange: recv[2 mu + 0] := send[2 mu + 1] of the -mu neighbour, recv[2 mu + 1] := send[2 mu + 0] of the +mu one
+ *   lqcd_wilson_clover_halo_add       out -= kappa * (the hops served by recv[8])
+ * Face 2 mu + dir holds the sites with x_mu = 0 (dir 0) or x_mu = dims[mu] - 1 (dir 1); face site f is the
+ * lexicographic index of the other three coordinates (x fastest); each face site carries the spin-projected half
+ * spinor of its hop, 12 reals (not 24), stored as rows of 16 bytes: buf[(j * Fv + f) * NV + q], Fv = V / dims[mu],
+ * NV = 4 (fp32) / 2 (fp64), real 2 (3 sp + c) + reim = j NV + q.  The dir-1 face is already multiplied by
+ * U_mu^dag(x) (the link of a backward hop lives on the sender); the receiver multiplies the other by its own U_mu(x).
+ * send / recv: HOST arrays of 8 DEVICE pointers, each of lqcd_halo_face_reals(dims, mu) reals, 16-byte aligned,
+ * caller-owned; entries of unpartitioned directions are ignored (may be NULL).  face_phase[2 mu + dir]: +1, or
+ * bc[mu] when that hop wraps the GLOBAL lattice (the rank sits on its edge); bc[] of mult_interior is used in the
+ * unpartitioned directions only.  flags: LQCD_DAGGER, LQCD_LINKS_12 (the same on all three calls).  The sum differs
+ * from lqcd_wilson_clover_mult on the global lattice by rounding order only.  part_mask = 0: pack and add are no-ops
+ * and mult_interior is lqcd_wilson_clover_mult. */
+size_t lqcd_halo_face_reals(const int dims[4], int mu);
+int lqcd_wilson_clover_halo_pack_f32(float* const send[8], const float* in, const float* U, const int dims[4],
+                                     unsigned part_mask, unsigned flags, void* stream);
+int lqcd_wilson_clover_halo_pack_f64(double* const send[8], const double* in, const double* U, const int dims[4],
+                                     unsigned part_mask, unsigned flags, void* stream);
+int lqcd_wilson_clover_mult_interior_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
+                                         const int dims[4], const int bc[4], unsigned part_mask, unsigned flags,
+                                         void* stream);
+int lqcd_wilson_clover_mult_interior_f64(double* out, const double* in, const double* U, const double* clover,
+                                         double kappa, const int dims[4], const int bc[4], unsigned part_mask,
+                                         unsigned flags, void* stream);
+int lqcd_wilson_clover_halo_add_f32(float* out, const float* const recv[8], const float* U, float kappa,
+                                    const int dims[4], const int face_phase[8], unsigned part_mask, unsigned flags,
+                                    void* stream);
+int lqcd_wilson_clover_halo_add_f64(double* out, const double* const recv[8], const double* U, double kappa,
+                                    const int dims[4], const int face_phase[8], unsigned part_mask, unsigned flags,
+                                    void* stream);
+
 /* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
  * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned

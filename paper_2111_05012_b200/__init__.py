@@ -479,6 +479,56 @@ def sap_mrhs(x, r, b, U, clover, kappa, dims, bc, domain, n_sap=4, n_mr=6, initi
     return x
 
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
+def halo_face_reals(dims, mu) -> int:
+    return int(lib().lqcd_halo_face_reals(_i4(dims), int(mu)))
+
+
+def halo_buffers(dims, part_mask, dtype=torch.float32, device="cuda"):
+    """The 8 face buffers of one side of the exchange (None for unpartitioned directions)."""
+    return [torch.empty(halo_face_reals(dims, f >> 1), dtype=dtype, device=device) if (part_mask >> (f >> 1)) & 1
+            else None for f in range(8)]
+
+
+def _p8(bufs):
+    return (C.c_void_p * 8)(*[None if b is None else _real(b).data_ptr() for b in bufs])
+
+
+def wilson_clover_halo_pack(send, inp, U, dims, part_mask, dagger=False, links12=False, stream=None):
+    """Sharded D, step 1: the projected half spinors of the partitioned faces of `inp` into send[8]."""
+    sfx = _same_dtype(inp, U, *[b for b in send if b is not None])
+    flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)
+    _check(getattr(lib(), f"lqcd_wilson_clover_halo_pack_{sfx}")(_p8(send), _dev_ptr(inp), _dev_ptr(U), _i4(dims),
+                                                                 int(part_mask), flags, _stream(stream)),
+           "lqcd_wilson_clover_halo_pack")
+    return send
+
+
+def wilson_clover_mult_interior(out, inp, U, clover, kappa, dims, bc, part_mask, dagger=False, links12=False,
+                                stream=None):
+    """Sharded D, step 2: D on the local lattice with the hops leaving it in partitioned directions switched off."""
+    sfx = _same_dtype(out, inp, U, clover)
+    flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_wilson_clover_mult_interior_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(U),
+                                                                     _dev_ptr(clover), k, _i4(dims), _i4(bc),
+                                                                     int(part_mask), flags, _stream(stream)),
+           "lqcd_wilson_clover_mult_interior")
+    return out
+
+
+def wilson_clover_halo_add(out, recv, U, kappa, dims, face_phase, part_mask, dagger=False, links12=False,
+                           stream=None):
+    """Sharded D, step 3: out -= kappa * (the hops served by the received faces recv[8])."""
+    sfx = _same_dtype(out, U, *[b for b in recv if b is not None])
+    flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    ph = (C.c_int * 8)(*[int(v) for v in face_phase])
+    _check(getattr(lib(), f"lqcd_wilson_clover_halo_add_{sfx}")(_dev_ptr(out), _p8(recv), _dev_ptr(U), k, _i4(dims),
+                                                                ph, int(part_mask), flags, _stream(stream)),
+           "lqcd_wilson_clover_halo_add")
+    return out
+
+
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):
     flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)

@@ -14,6 +14,8 @@ _lib = None
 c_int4 = C.c_int * 4
 _vp, _ci, _cu, _cf, _cd = C.c_void_p, C.c_int, C.c_uint, C.c_float, C.c_double
 _i4 = C.POINTER(C.c_int)
+_i8 = C.POINTER(C.c_int)       # int[8]
+_p8 = C.POINTER(C.c_void_p)    # void*[8]: host array of device pointers
 
 # name -> (restype, argtypes); every symbol include/lqcd_b200.h declares
 SIGNATURES = {
@@ -35,6 +37,7 @@ SIGNATURES = {
     "lqcd_mg_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
     "lqcd_mg_mrhs_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci, _ci]),
     "lqcd_coarse_bicgstab_mrhs_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci, _ci]),
+    "lqcd_halo_face_reals": (C.c_size_t, [_i4, _ci]),
 }
 for _p, _k in (("f32", _cf), ("f64", _cd)):
     SIGNATURES.update({
@@ -68,6 +71,9 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
                                            _vp]),
         f"lqcd_sap_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _ci, _cu, _vp, _vp]),
         f"lqcd_sap_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _cu, _vp, _vp]),
+        f"lqcd_wilson_clover_halo_pack_{_p}": (_ci, [_p8, _vp, _vp, _i4, _cu, _cu, _vp]),
+        f"lqcd_wilson_clover_mult_interior_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _cu, _vp]),
+        f"lqcd_wilson_clover_halo_add_{_p}": (_ci, [_vp, _p8, _vp, _k, _i4, _i8, _cu, _cu, _vp]),
     })
 SIGNATURES.update({
     "lqcd_wilson_clover_mult_host_f32": (_ci, [_vp, _vp, _vp, _vp, _cf, _i4, _i4, _cu, _vp, _vp]),

@@ -1,0 +1,178 @@
+"""The sharded fine operator: D on a lattice partitioned over ranks (the paper's own runs
+partition the lattice in 4-D over the nodes and exchange the boundary once per application).
+
+Host logic only -- which rank owns what, who the neighbours are, which boundary phase a hop carries, and moving the
+face buffers with torch.distributed point-to-point calls (nccl on GPUs, gloo in the CPU tests).  Every arithmetic
+step runs in the library's kernels (csrc/halo.cu, csrc/wilson_clover.cu): pack -> [exchange || interior] -> add.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import (halo_buffers, wilson_clover_halo_add, wilson_clover_halo_pack, wilson_clover_mult_interior)
+
+
+class RankGrid:
+    """A 4-D grid of ranks, x fastest (rank = c0 + R0 (c1 + R1 (c2 + R2 c3))), periodic like the lattice."""
+
+    def __init__(self, ranks, rank: int = 0):
+        self.ranks = tuple(int(r) for r in ranks)
+        if len(self.ranks) != 4 or min(self.ranks) < 1:
+            raise ValueError(f"rank grid {ranks}")
+        self.world = int(np.prod(self.ranks))
+        if not 0 <= rank < self.world:
+            raise ValueError(f"rank {rank} outside a grid of {self.world}")
+        self.rank = int(rank)
+        c, r = [], self.rank
+        for mu in range(4):
+            c.append(r % self.ranks[mu])
+            r //= self.ranks[mu]
+        self.coords = tuple(c)
+
+    def rank_of(self, coords) -> int:
+        r = 0
+        for mu in (3, 2, 1, 0):
+            r = r * self.ranks[mu] + coords[mu] % self.ranks[mu]
+        return r
+
+    def neighbour(self, mu: int, sign: int) -> int:
+        c = list(self.coords)
+        c[mu] += sign
+        return self.rank_of(c)
+
+    @property
+    def part_mask(self) -> int:
+        """Bit mu set: direction mu is split over more than one rank."""
+        return sum(1 << mu for mu in range(4) if self.ranks[mu] > 1)
+
+    def face_phase(self, bc, part_mask=None):
+        """face_phase[2 mu + dir] of lqcd_wilson_clover_halo_add: bc[mu] where that hop wraps the global lattice."""
+        mask = self.part_mask if part_mask is None else part_mask
+        ph = [1] * 8
+        for mu in range(4):
+            if not (mask >> mu) & 1:
+                continue
+            if self.coords[mu] == 0:
+                ph[2 * mu] = int(bc[mu])                      # backward hop from x_mu = 0
+            if self.coords[mu] == self.ranks[mu] - 1:
+                ph[2 * mu + 1] = int(bc[mu])                  # forward hop from x_mu = L - 1
+        return ph
+
+    def local_dims(self, gdims):
+        for mu in range(4):
+            if gdims[mu] % self.ranks[mu]:
+                raise ValueError(f"global extent {gdims[mu]} not divisible by {self.ranks[mu]} ranks in direction {mu}")
+        return tuple(gdims[mu] // self.ranks[mu] for mu in range(4))
+
+    def local_slices(self, gdims):
+        """Slices of a canonical field viewed as (L3, L2, L1, L0, ...) that select this rank's sub-lattice."""
+        ld = self.local_dims(gdims)
+        return tuple(slice(self.coords[mu] * ld[mu], (self.coords[mu] + 1) * ld[mu]) for mu in (3, 2, 1, 0))
+
+
+def split_field(a, gdims, grid: RankGrid, site_axis: int = 0):
+    """This rank's part of a canonical field whose axis `site_axis` runs over the global sites (x fastest)."""
+    shp = tuple(a.shape)
+    view = a.reshape(shp[:site_axis] + (gdims[3], gdims[2], gdims[1], gdims[0]) + shp[site_axis + 1:])
+    idx = (slice(None),) * site_axis + grid.local_slices(gdims)
+    loc = view[idx]
+    ld = grid.local_dims(gdims)
+    loc = loc.reshape(shp[:site_axis] + (int(np.prod(ld)),) + shp[site_axis + 1:])
+    return loc.contiguous() if isinstance(loc, torch.Tensor) else np.ascontiguousarray(loc)
+
+
+def join_field(parts, gdims, ranks, site_axis: int = 0):
+    """Inverse of split_field: parts[rank] -> the global canonical field (numpy)."""
+    g0 = RankGrid(ranks, 0)
+    ld = g0.local_dims(gdims)
+    p0 = np.asarray(parts[0])
+    shp = p0.shape
+    out = np.empty(shp[:site_axis] + (gdims[3], gdims[2], gdims[1], gdims[0]) + shp[site_axis + 1:], dtype=p0.dtype)
+    for r, part in enumerate(parts):
+        g = RankGrid(ranks, r)
+        idx = (slice(None),) * site_axis + g.local_slices(gdims)
+        out[idx] = np.asarray(part).reshape(shp[:site_axis] + (ld[3], ld[2], ld[1], ld[0]) + shp[site_axis + 1:])
+    return out.reshape(shp[:site_axis] + (int(np.prod(gdims)),) + shp[site_axis + 1:])
+
+
+def exchange_faces(send, recv, grid: RankGrid, part_mask=None, group=None):
+    """recv[2 mu] := send[2 mu + 1] of the -mu neighbour; recv[2 mu + 1] := send[2 mu] of the +mu neighbour.
+
+    Returns the list of the 8 buffers that hold the received faces: `recv[f]`, or -- where the neighbour is this very
+    rank -- the send buffer itself (no copy).  Point-to-point operations are posted in one batch, in the same order on
+    every rank (per direction: to +mu, to -mu; from -mu, from +mu), so that the two messages between a pair of ranks
+    that are each other's neighbour on both sides (two ranks in a direction) match up under nccl's per-peer ordering.
+    """
+    import torch.distributed as dist
+    mask = grid.part_mask if part_mask is None else part_mask
+    got = [None] * 8
+    ops = []
+    for mu in range(4):
+        if not (mask >> mu) & 1:
+            continue
+        plus, minus = grid.neighbour(mu, +1), grid.neighbour(mu, -1)
+        if plus == grid.rank and minus == grid.rank:
+            got[2 * mu], got[2 * mu + 1] = send[2 * mu + 1], send[2 * mu]
+            continue
+        ops.append(dist.P2POp(dist.isend, send[2 * mu + 1], plus, group=group, tag=2 * mu))
+        ops.append(dist.P2POp(dist.isend, send[2 * mu], minus, group=group, tag=2 * mu + 1))
+        ops.append(dist.P2POp(dist.irecv, recv[2 * mu], minus, group=group, tag=2 * mu))
+        ops.append(dist.P2POp(dist.irecv, recv[2 * mu + 1], plus, group=group, tag=2 * mu + 1))
+        got[2 * mu], got[2 * mu + 1] = recv[2 * mu], recv[2 * mu + 1]
+    if ops:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+    return got
+
+
+def route_faces(sends, ranks, part_mask):
+    """Single-process stand-in for exchange_faces: sends[rank][8] -> recvs[rank][8] by reference (no copies).
+    Used where several virtual ranks live on one GPU one after the other (tests, the bench's overhead probe)."""
+    recvs = []
+    for r in range(len(sends)):
+        g = RankGrid(ranks, r)
+        got = [None] * 8
+        for mu in range(4):
+            if (part_mask >> mu) & 1:
+                got[2 * mu] = sends[g.neighbour(mu, -1)][2 * mu + 1]
+                got[2 * mu + 1] = sends[g.neighbour(mu, +1)][2 * mu]
+        recvs.append(got)
+    return recvs
+
+
+class ShardedWilsonClover:
+    """D (or D^dag) on this rank's sub-lattice of a lattice split over `grid`.
+
+    U, clover: this rank's native fields (lattice `dims` = the LOCAL extents).  part_mask defaults to the directions
+    the grid really splits; a direction may also be marked partitioned with a single rank in it (the rank is then
+    its own neighbour) -- the result is the same operator, which is how one GPU exercises the whole exchange path.
+    """
+
+    def __init__(self, U, clover, kappa, dims, bc, grid: RankGrid, links12=False, part_mask=None, group=None):
+        self.U, self.clover, self.kappa = U, clover, float(kappa)
+        self.dims, self.bc, self.grid, self.links12, self.group = tuple(dims), tuple(bc), grid, links12, group
+        self.mask = grid.part_mask if part_mask is None else int(part_mask)
+        if grid.part_mask & ~self.mask:
+            raise ValueError("part_mask must include every direction the rank grid splits")
+        self.phase = grid.face_phase(bc, self.mask)
+        self.send = halo_buffers(dims, self.mask, dtype=U.dtype, device=U.device)
+        remote = [mu for mu in range(4) if (self.mask >> mu) & 1 and grid.neighbour(mu, 1) != grid.rank]
+        rmask = sum(1 << mu for mu in remote)
+        self.recv = halo_buffers(dims, rmask, dtype=U.dtype, device=U.device)
+        self.comm = torch.cuda.Stream(device=U.device)
+
+    def apply(self, out, inp, dagger=False):
+        cur = torch.cuda.current_stream(self.U.device)
+        wilson_clover_halo_pack(self.send, inp, self.U, self.dims, self.mask, dagger, self.links12, stream=cur)
+        packed = cur.record_event()
+        with torch.cuda.stream(self.comm):           # the exchange overlaps the interior pass
+            self.comm.wait_event(packed)
+            got = exchange_faces(self.send, self.recv, self.grid, self.mask, self.group)
+            arrived = self.comm.record_event()
+        wilson_clover_mult_interior(out, inp, self.U, self.clover, self.kappa, self.dims, self.bc, self.mask, dagger,
+                                    self.links12, stream=cur)
+        cur.wait_event(arrived)
+        wilson_clover_halo_add(out, got, self.U, self.kappa, self.dims, self.phase, self.mask, dagger, self.links12,
+                               stream=cur)
+        return out
