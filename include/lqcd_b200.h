@@ -397,6 +397,30 @@ int lqcd_wilson_clover_halo_add_f64(double* out, const double* const recv[8], co
                                     const int dims[4], const int face_phase[8], unsigned part_mask, unsigned flags,
                                     void* stream);
 
+/* The same for the coarse operator ("same pattern on the coarse lattice, N complex per face site").
+ * cdims[4]: the LOCAL coarse lattice; A: its blocks (a block of a leaving hop lives on the site it acts on, so no
+ * block is ever exchanged and no boundary phase appears: bc is inside A).  Face 2 mu + dir: the coarse vectors of the
+ * sites with X_mu = 0 (dir 0) / cdims[mu] - 1 (dir 1), [face site][chi][i] complex, face site = lexicographic index of
+ * the other three coordinates; lqcd_coarse_halo_face_reals(cdims, nvec, mu) reals each.  Exchange as above
+ * (recv[2 mu] := send[2 mu + 1] of the -mu neighbour, recv[2 mu + 1] := send[2 mu] of the +mu neighbour).
+ *   lqcd_coarse_halo_pack      in -> send[8]
+ *   lqcd_coarse_mult_interior  out = D_c in without the blocks of leaving hops (neither A nor in is read for them)
+ *   lqcd_coarse_halo_add       out += those blocks applied to recv[8]            (one launch; boundary sites only)
+ * flags: LQCD_DAGGER on mult_interior and halo_add alike.  A partitioned direction may have local extent 1. */
+size_t lqcd_coarse_halo_face_reals(const int cdims[4], int nvec, int mu);
+int lqcd_coarse_halo_pack_f32(float* const send[8], const float* in, const int cdims[4], int nvec, unsigned part_mask,
+                              void* stream);
+int lqcd_coarse_halo_pack_f64(double* const send[8], const double* in, const int cdims[4], int nvec,
+                              unsigned part_mask, void* stream);
+int lqcd_coarse_mult_interior_f32(float* out, const float* in, const float* A, const int cdims[4], int nvec,
+                                  unsigned part_mask, unsigned flags, void* stream);
+int lqcd_coarse_mult_interior_f64(double* out, const double* in, const double* A, const int cdims[4], int nvec,
+                                  unsigned part_mask, unsigned flags, void* stream);
+int lqcd_coarse_halo_add_f32(float* out, const float* const recv[8], const float* A, const int cdims[4], int nvec,
+                             unsigned part_mask, unsigned flags, void* stream);
+int lqcd_coarse_halo_add_f64(double* out, const double* const recv[8], const double* A, const int cdims[4], int nvec,
+                             unsigned part_mask, unsigned flags, void* stream);
+
 /* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
  * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned

@@ -529,6 +529,41 @@ def wilson_clover_halo_add(out, recv, U, kappa, dims, face_phase, part_mask, dag
     return out
 
 
+def coarse_halo_face_reals(cdims, nvec, mu) -> int:
+    return int(lib().lqcd_coarse_halo_face_reals(_i4(cdims), int(nvec), int(mu)))
+
+
+def coarse_halo_buffers(cdims, nvec, part_mask, dtype=torch.float32, device="cuda"):
+    return [torch.empty(coarse_halo_face_reals(cdims, nvec, f >> 1), dtype=dtype, device=device)
+            if (part_mask >> (f >> 1)) & 1 else None for f in range(8)]
+
+
+def coarse_halo_pack(send, inp, cdims, nvec, part_mask, stream=None):
+    """Sharded D_c, step 1: the coarse vectors of the partitioned faces of `inp` into send[8]."""
+    sfx = _same_dtype(inp, *[b for b in send if b is not None])
+    _check(getattr(lib(), f"lqcd_coarse_halo_pack_{sfx}")(_p8(send), _dev_ptr(inp), _i4(cdims), int(nvec),
+                                                          int(part_mask), _stream(stream)), "lqcd_coarse_halo_pack")
+    return send
+
+
+def coarse_mult_interior(out, inp, A, cdims, nvec, part_mask, dagger=False, stream=None):
+    """Sharded D_c, step 2: D_c on the local coarse lattice without the blocks of hops that leave it."""
+    sfx = _same_dtype(out, inp, A)
+    _check(getattr(lib(), f"lqcd_coarse_mult_interior_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(A), _i4(cdims),
+                                                              int(nvec), int(part_mask), DAGGER if dagger else 0,
+                                                              _stream(stream)), "lqcd_coarse_mult_interior")
+    return out
+
+
+def coarse_halo_add(out, recv, A, cdims, nvec, part_mask, dagger=False, stream=None):
+    """Sharded D_c, step 3: out += the blocks of the leaving hops applied to the received faces recv[8]."""
+    sfx = _same_dtype(out, A, *[b for b in recv if b is not None])
+    _check(getattr(lib(), f"lqcd_coarse_halo_add_{sfx}")(_dev_ptr(out), _p8(recv), _dev_ptr(A), _i4(cdims), int(nvec),
+                                                         int(part_mask), DAGGER if dagger else 0, _stream(stream)),
+           "lqcd_coarse_halo_add")
+    return out
+
+
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):
     flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)

@@ -38,6 +38,7 @@ SIGNATURES = {
     "lqcd_mg_mrhs_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci, _ci]),
     "lqcd_coarse_bicgstab_mrhs_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci, _ci]),
     "lqcd_halo_face_reals": (C.c_size_t, [_i4, _ci]),
+    "lqcd_coarse_halo_face_reals": (C.c_size_t, [_i4, _ci, _ci]),
 }
 for _p, _k in (("f32", _cf), ("f64", _cd)):
     SIGNATURES.update({
@@ -71,6 +72,9 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
                                            _vp]),
         f"lqcd_sap_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _ci, _cu, _vp, _vp]),
         f"lqcd_sap_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _cu, _vp, _vp]),
+        f"lqcd_coarse_halo_pack_{_p}": (_ci, [_p8, _vp, _i4, _ci, _cu, _vp]),
+        f"lqcd_coarse_mult_interior_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _cu, _vp]),
+        f"lqcd_coarse_halo_add_{_p}": (_ci, [_vp, _p8, _vp, _i4, _ci, _cu, _cu, _vp]),
         f"lqcd_wilson_clover_halo_pack_{_p}": (_ci, [_p8, _vp, _vp, _i4, _cu, _cu, _vp]),
         f"lqcd_wilson_clover_mult_interior_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _cu, _vp]),
         f"lqcd_wilson_clover_halo_add_{_p}": (_ci, [_vp, _p8, _vp, _k, _i4, _i8, _cu, _cu, _vp]),

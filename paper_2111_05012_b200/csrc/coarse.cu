@@ -27,6 +27,12 @@ struct CoarseParams {
     int tpw;        // row tiles per warp (divides ntile)
     long long ntask;  // Vc * ntile / tpw warp tasks
     int dagger;
+    unsigned part_mask;  // sharded variants only: bit mu = direction mu is partitioned over ranks
+};
+
+// received faces of the sharded operator (MODE 2): face 2 mu + dir, [face site][N complex]
+struct CoarseFaces {
+    const void* p[8];
 };
 
 template <typename T> __device__ __forceinline__ void cmadd(T& sr, T& si, const V16<T>& a, const V16<T>& x);
@@ -51,9 +57,13 @@ template <> __device__ __forceinline__ void cmadd<double>(double& sr, double& si
 // LPR lanes per row (power of two <= 32), CPL vec16 per lane per row, R rows in flight per lane.
 // FULL: N is a multiple of the row tile and a row is exactly LPR*CPL vec16 -- no bounds predicates, so the loads of
 // a tile are unconditional and stay batched at the top of the tile.
-template <typename T, int LPR, int CPL, int R, bool FULL>
+// MODE 0: the operator.  Sharded variants (halo exchange on the coarse lattice): MODE 1 = interior
+// pass, the blocks of hops that leave the local lattice in a partitioned direction are skipped (neither A nor the
+// source is read); MODE 2 = boundary completion, out += exactly those blocks with the sources taken from the received
+// faces (warps of interior sites exit at once).
+template <typename T, int LPR, int CPL, int R, bool FULL, int MODE = 0>
 __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ A,
-                                                CoarseParams P) {
+                                                CoarseParams P, CoarseFaces F = CoarseFaces()) {
     constexpr int NV = VecOf<T>::NV;
     constexpr int CPV = NV / 2;  // complex per vec16
     constexpr int G = 32 / LPR;  // rows side by side in a warp
@@ -67,6 +77,7 @@ __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T*
 
     // the nine source sites
     int src[9];
+    unsigned cut = 0;  // MODE 1, 2: bit d = hop d leaves the local lattice in a partitioned direction
     {
         int xc[4], rem = X;
         xc[0] = rem % P.Lc[0]; rem /= P.Lc[0];
@@ -80,7 +91,32 @@ __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T*
             src[1 + 2 * mu] = (xc[mu] == P.Lc[mu] - 1) ? X - (P.Lc[mu] - 1) * stride[mu] : X + stride[mu];
             src[2 + 2 * mu] = (xc[mu] == 0) ? X + (P.Lc[mu] - 1) * stride[mu] : X - stride[mu];
         }
+        if (MODE != 0) {
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++) {
+                if (!((P.part_mask >> mu) & 1)) continue;
+                // face site: lexicographic index of the other three coordinates
+                int f = 0, fs = 1;
+#pragma unroll
+                for (int nu = 0; nu < 4; nu++)
+                    if (nu != mu) {
+                        f += xc[nu] * fs;
+                        fs *= P.Lc[nu];
+                    }
+                if (xc[mu] == P.Lc[mu] - 1) {
+                    cut |= 1u << (1 + 2 * mu);
+                    if (MODE == 2) src[1 + 2 * mu] = f;
+                }
+                if (xc[mu] == 0) {
+                    cut |= 1u << (2 + 2 * mu);
+                    if (MODE == 2) src[2 + 2 * mu] = f;
+                }
+            }
+            if (MODE == 2 && cut == 0) return;
+        }
     }
+    // does block d take part in this pass?
+    auto live = [&](int d) -> bool { return MODE == 0 ? true : MODE == 1 ? !((cut >> d) & 1) : ((cut >> d) & 1); };
     // my slices of the nine source vectors (with the Gamma5c sign of the column for the dagger variant)
     V16<T> xv[9][CPL];
 #pragma unroll
@@ -88,8 +124,10 @@ __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T*
 #pragma unroll
         for (int c = 0; c < CPL; c++) {
             const int v = q + LPR * c;
-            if (FULL || v < P.RV) {
-                xv[d][c] = ld16(in + ((long long)src[d] * P.RV + v) * NV);
+            if ((FULL || v < P.RV) && live(d)) {
+                // MODE 2: hop d = 1 + 2 mu (forward) is served by face 2 mu + 1, d = 2 + 2 mu (backward) by face 2 mu
+                const T* from = MODE == 2 ? static_cast<const T*>(F.p[d == 0 ? 0 : ((d - 1) >> 1) * 2 + (d & 1)]) : in;
+                xv[d][c] = ld16(from + ((long long)src[d] * P.RV + v) * NV);
                 if (P.dagger) {
 #pragma unroll
                     for (int e = 0; e < CPV; e++)
@@ -120,7 +158,7 @@ __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T*
 #pragma unroll
                 for (int c = 0; c < CPL; c++) {
                     const int v = q + LPR * c;
-                    if (FULL || (row < P.N && v < P.RV))
+                    if ((FULL || (row < P.N && v < P.RV)) && live(d))
                         a[r][d][c] = ld16_stream(Asite + (((long long)d * P.N + row) * P.RV + v) * NV);
                     else {
 #pragma unroll
@@ -146,15 +184,21 @@ __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T*
             if (q == 0 && (FULL || row < P.N)) {
                 T s = (P.dagger && row >= P.nvec) ? (T)-1 : (T)1;
                 T* o = out + ((long long)X * P.N + row) * 2;
-                o[0] = s * sr[r];
-                o[1] = s * si[r];
+                if (MODE == 2) {
+                    o[0] += s * sr[r];
+                    o[1] += s * si[r];
+                } else {
+                    o[0] = s * sr[r];
+                    o[1] = s * si[r];
+                }
             }
         }
     }
 }
 
-template <typename T, int LPR, int CPL, int R>
-static void launch_coarse(T* out, const T* in, const T* A, CoarseParams P, cudaStream_t st) {
+template <typename T, int LPR, int CPL, int R, int MODE>
+static void launch_coarse_mode(T* out, const T* in, const T* A, CoarseParams P, cudaStream_t st,
+                               const CoarseFaces& F) {
     constexpr int G = 32 / LPR;
     P.ntile = (P.N + G * R - 1) / (G * R);
     // row tiles per warp: as many as possible (the nine source slices are loaded once per warp) while the grid
@@ -170,14 +214,29 @@ static void launch_coarse(T* out, const T* in, const T* A, CoarseParams P, cudaS
     if (warps > 8) warps = 8;
     const long long grid = (P.ntask + warps - 1) / warps;
     const bool full = (P.N % (G * R) == 0) && (P.RV == LPR * CPL);
-    if (full) k_coarse<T, LPR, CPL, R, true><<<(unsigned)grid, warps * 32, 0, st>>>(out, in, A, P);
-    else k_coarse<T, LPR, CPL, R, false><<<(unsigned)grid, warps * 32, 0, st>>>(out, in, A, P);
+    if (full) k_coarse<T, LPR, CPL, R, true, MODE><<<(unsigned)grid, warps * 32, 0, st>>>(out, in, A, P, F);
+    else k_coarse<T, LPR, CPL, R, false, MODE><<<(unsigned)grid, warps * 32, 0, st>>>(out, in, A, P, F);
 }
 
+template <typename T, int LPR, int CPL, int R>
+static void launch_coarse(T* out, const T* in, const T* A, const CoarseParams& P, cudaStream_t st, int mode,
+                          const CoarseFaces& F) {
+    if (mode == 0) launch_coarse_mode<T, LPR, CPL, R, 0>(out, in, A, P, st, F);
+    else if (mode == 1) launch_coarse_mode<T, LPR, CPL, R, 1>(out, in, A, P, st, F);
+    else launch_coarse_mode<T, LPR, CPL, R, 2>(out, in, A, P, st, F);
+}
+
+// mode 0: D_c; mode 1: interior pass of the sharded operator; mode 2: its boundary completion (in = NULL, sources from
+// recv[8], out accumulated)
 template <typename T>
 static int coarse_call(T* out, const T* in, const T* A, const int cdims[4], int nvec, unsigned flags, void* stream,
-                       const char* what) {
+                       const char* what, int mode = 0, unsigned part_mask = 0, const T* const* recv = nullptr) {
     clear_error();
+    if (mode == 2 && !in) in = A;  // never read in mode 2; keeps the checks below uniform
+    if (part_mask > 15u || (mode == 2 && !recv)) {
+        set_error("%s: bad part_mask 0x%x or null recv", what, part_mask);
+        return LQCD_EINVAL;
+    }
     if (!out || !in || !A || check_dims(cdims) || nvec < 1) {
         set_error("%s: null pointer, non-positive dim or nvec < 1", what);
         return LQCD_EINVAL;
@@ -195,13 +254,26 @@ static int coarse_call(T* out, const T* in, const T* A, const int cdims[4], int 
         return LQCD_EINVAL;
     }
     CoarseParams P;
+    CoarseFaces F;
+    for (int i = 0; i < 8; i++) F.p[i] = nullptr;
     for (int mu = 0; mu < 4; mu++) {
-        if (cdims[mu] < 2) {
+        const bool part = (part_mask >> mu) & 1;
+        if (cdims[mu] < 2 && !part) {  // (a partitioned direction may be one site thick: both hops leave)
             set_error("%s: coarse extent %d < 2 in direction %d", what, cdims[mu], mu);
             return LQCD_EINVAL;
         }
         P.Lc[mu] = cdims[mu];
+        if (mode == 2 && part)
+            for (int dir = 0; dir < 2; dir++) {
+                if (!recv[2 * mu + dir] || !aligned16(recv[2 * mu + dir])) {
+                    set_error("%s: recv[%d] is null or not 16-byte aligned", what, 2 * mu + dir);
+                    return LQCD_EINVAL;
+                }
+                F.p[2 * mu + dir] = recv[2 * mu + dir];
+            }
     }
+    P.part_mask = part_mask;
+    if (mode == 2 && !part_mask) return LQCD_OK;
     if (volume(cdims) > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
     constexpr int NV = VecOf<T>::NV;
     P.Vc = (int)volume(cdims);
@@ -215,19 +287,89 @@ static int coarse_call(T* out, const T* in, const T* A, const int cdims[4], int 
         set_error("%s: nvec = %d outside the compiled range (row longer than 128 vec16)", what, nvec);
         return LQCD_EUNSUPPORTED;
     }
-    if (RV <= 1) launch_coarse<T, 1, 1, 2>(out, in, A, P, st);
-    else if (RV <= 2) launch_coarse<T, 2, 1, 2>(out, in, A, P, st);
-    else if (RV <= 4) launch_coarse<T, 4, 1, 2>(out, in, A, P, st);
-    else if (RV <= 8) launch_coarse<T, 8, 1, 2>(out, in, A, P, st);
-    else if (RV <= 16) launch_coarse<T, 16, 1, 2>(out, in, A, P, st);
+    if (RV <= 1) launch_coarse<T, 1, 1, 2>(out, in, A, P, st, mode, F);
+    else if (RV <= 2) launch_coarse<T, 2, 1, 2>(out, in, A, P, st, mode, F);
+    else if (RV <= 4) launch_coarse<T, 4, 1, 2>(out, in, A, P, st, mode, F);
+    else if (RV <= 8) launch_coarse<T, 8, 1, 2>(out, in, A, P, st, mode, F);
+    else if (RV <= 16) launch_coarse<T, 16, 1, 2>(out, in, A, P, st, mode, F);
     else if (RV <= 32) {
-        if (g_knobs.coarse_R == 1) launch_coarse<T, 32, 1, 1>(out, in, A, P, st);
-        else if (g_knobs.coarse_R == 4) launch_coarse<T, 32, 1, 4>(out, in, A, P, st);
-        else launch_coarse<T, 32, 1, 2>(out, in, A, P, st);
+        if (g_knobs.coarse_R == 1) launch_coarse<T, 32, 1, 1>(out, in, A, P, st, mode, F);
+        else if (g_knobs.coarse_R == 4) launch_coarse<T, 32, 1, 4>(out, in, A, P, st, mode, F);
+        else launch_coarse<T, 32, 1, 2>(out, in, A, P, st, mode, F);
     }
-    else if (RV <= 64) launch_coarse<T, 32, 2, 1>(out, in, A, P, st);
-    else if (RV <= 96) launch_coarse<T, 32, 3, 1>(out, in, A, P, st);
-    else launch_coarse<T, 32, 4, 1>(out, in, A, P, st);
+    else if (RV <= 64) launch_coarse<T, 32, 2, 1>(out, in, A, P, st, mode, F);
+    else if (RV <= 96) launch_coarse<T, 32, 3, 1>(out, in, A, P, st, mode, F);
+    else launch_coarse<T, 32, 4, 1>(out, in, A, P, st, mode, F);
+    count_launch();
+    return check_launch(what);
+}
+
+// ---- sharded coarse operator: the faces ("same pattern on the coarse lattice, N complex per face
+// site") -- face 2 mu + dir = the coarse vectors of the sites with X_mu = 0 (dir 0) / Lc_mu - 1 (dir 1), face site =
+// lexicographic index of the other three coordinates, [face site][N complex].
+template <typename T>
+__global__ void __launch_bounds__(256) k_coarse_halo_pack(CoarseFaces send_c, const T* __restrict__ in, CoarseParams P) {
+    constexpr int NV = VecOf<T>::NV;
+    const int face = blockIdx.y, mu = face >> 1, dir = face & 1;
+    if (!((P.part_mask >> mu) & 1)) return;
+    T* buf = static_cast<T*>(const_cast<void*>(send_c.p[face]));
+    const long long n = (long long)(P.Vc / P.Lc[mu]) * P.RV;  // vec16 of this face
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        int f = (int)(i / P.RV);
+        const int v = (int)(i - (long long)f * P.RV);
+        int X = 0, stride = 1;
+#pragma unroll
+        for (int nu = 0; nu < 4; nu++) {
+            int c;
+            if (nu == mu) {
+                c = dir ? P.Lc[mu] - 1 : 0;
+            } else {
+                c = f % P.Lc[nu];
+                f /= P.Lc[nu];
+            }
+            X += c * stride;
+            stride *= P.Lc[nu];
+        }
+        st16(buf + i * NV, ld16(in + ((long long)X * P.RV + v) * NV));
+    }
+}
+
+template <typename T>
+static int coarse_halo_pack_call(T* const send[8], const T* in, const int cdims[4], int nvec, unsigned part_mask,
+                                 void* stream, const char* what) {
+    clear_error();
+    if (!send || !in || check_dims(cdims) || nvec < 1 || part_mask > 15u || !aligned16(in)) {
+        set_error("%s: null or misaligned pointer, non-positive dim, nvec < 1 or part_mask 0x%x", what, part_mask);
+        return LQCD_EINVAL;
+    }
+    if (volume(cdims) > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
+    constexpr int NV = VecOf<T>::NV;
+    CoarseParams P;
+    CoarseFaces F;
+    P.Vc = (int)volume(cdims);
+    P.nvec = nvec;
+    P.N = 2 * nvec;
+    P.RV = 2 * P.N / NV;
+    P.part_mask = part_mask;
+    long long nmax = 0;
+    for (int mu = 0; mu < 4; mu++) {
+        P.Lc[mu] = cdims[mu];
+        for (int dir = 0; dir < 2; dir++) {
+            F.p[2 * mu + dir] = nullptr;
+            if (!((part_mask >> mu) & 1)) continue;
+            if (!send[2 * mu + dir] || !aligned16(send[2 * mu + dir])) {
+                set_error("%s: send[%d] is null or not 16-byte aligned", what, 2 * mu + dir);
+                return LQCD_EINVAL;
+            }
+            F.p[2 * mu + dir] = send[2 * mu + dir];
+            const long long n = (long long)(P.Vc / cdims[mu]) * P.RV;
+            nmax = n > nmax ? n : nmax;
+        }
+    }
+    if (!part_mask) return LQCD_OK;
+    long long gx = (nmax + 255) / 256;
+    if (gx > 148 * 8) gx = 148 * 8;
+    k_coarse_halo_pack<T><<<dim3((unsigned)gx, 8), 256, 0, (cudaStream_t)stream>>>(F, in, P);
     count_launch();
     return check_launch(what);
 }
@@ -244,5 +386,36 @@ int lqcd_coarse_mult_f32(float* out, const float* in, const float* A, const int 
 int lqcd_coarse_mult_f64(double* out, const double* in, const double* A, const int cdims[4], int nvec, unsigned flags,
                          void* stream) {
     return coarse_call<double>(out, in, A, cdims, nvec, flags, stream, "lqcd_coarse_mult_f64");
+}
+
+size_t lqcd_coarse_halo_face_reals(const int cdims[4], int nvec, int mu) {
+    if (check_dims(cdims) || nvec < 1 || mu < 0 || mu > 3) return 0;
+    return (size_t)(volume(cdims) / cdims[mu]) * 4 * (size_t)nvec;
+}
+int lqcd_coarse_halo_pack_f32(float* const send[8], const float* in, const int cdims[4], int nvec, unsigned part_mask,
+                              void* stream) {
+    return coarse_halo_pack_call<float>(send, in, cdims, nvec, part_mask, stream, "lqcd_coarse_halo_pack_f32");
+}
+int lqcd_coarse_halo_pack_f64(double* const send[8], const double* in, const int cdims[4], int nvec,
+                              unsigned part_mask, void* stream) {
+    return coarse_halo_pack_call<double>(send, in, cdims, nvec, part_mask, stream, "lqcd_coarse_halo_pack_f64");
+}
+int lqcd_coarse_mult_interior_f32(float* out, const float* in, const float* A, const int cdims[4], int nvec,
+                                  unsigned part_mask, unsigned flags, void* stream) {
+    return coarse_call<float>(out, in, A, cdims, nvec, flags, stream, "lqcd_coarse_mult_interior_f32", 1, part_mask);
+}
+int lqcd_coarse_mult_interior_f64(double* out, const double* in, const double* A, const int cdims[4], int nvec,
+                                  unsigned part_mask, unsigned flags, void* stream) {
+    return coarse_call<double>(out, in, A, cdims, nvec, flags, stream, "lqcd_coarse_mult_interior_f64", 1, part_mask);
+}
+int lqcd_coarse_halo_add_f32(float* out, const float* const recv[8], const float* A, const int cdims[4], int nvec,
+                             unsigned part_mask, unsigned flags, void* stream) {
+    return coarse_call<float>(out, nullptr, A, cdims, nvec, flags, stream, "lqcd_coarse_halo_add_f32", 2, part_mask,
+                              recv);
+}
+int lqcd_coarse_halo_add_f64(double* out, const double* const recv[8], const double* A, const int cdims[4], int nvec,
+                             unsigned part_mask, unsigned flags, void* stream) {
+    return coarse_call<double>(out, nullptr, A, cdims, nvec, flags, stream, "lqcd_coarse_halo_add_f64", 2, part_mask,
+                               recv);
 }
 }

@@ -10,7 +10,8 @@ from __future__ import annotations
 import numpy as np
 import torch
 
-from . import (halo_buffers, wilson_clover_halo_add, wilson_clover_halo_pack, wilson_clover_mult_interior)
+from . import (coarse_halo_add, coarse_halo_buffers, coarse_halo_pack, coarse_mult_interior, halo_buffers,
+               wilson_clover_halo_add, wilson_clover_halo_pack, wilson_clover_mult_interior)
 
 
 class RankGrid:
@@ -175,4 +176,33 @@ class ShardedWilsonClover:
         cur.wait_event(arrived)
         wilson_clover_halo_add(out, got, self.U, self.kappa, self.dims, self.phase, self.mask, dagger, self.links12,
                                stream=cur)
+        return out
+
+
+class ShardedCoarse:
+    """D_c (or its dagger) on this rank's part of a coarse lattice split over `grid`; A: the blocks of the local sites.
+    cdims = the LOCAL coarse extents.  No boundary phases: bc lives inside A."""
+
+    def __init__(self, A, cdims, nvec, grid: RankGrid, part_mask=None, group=None):
+        self.A, self.cdims, self.nvec, self.grid, self.group = A, tuple(cdims), int(nvec), grid, group
+        self.mask = grid.part_mask if part_mask is None else int(part_mask)
+        if grid.part_mask & ~self.mask:
+            raise ValueError("part_mask must include every direction the rank grid splits")
+        rdt = torch.float32 if A.dtype in (torch.complex64, torch.float32) else torch.float64
+        self.send = coarse_halo_buffers(cdims, nvec, self.mask, dtype=rdt, device=A.device)
+        rmask = sum(1 << mu for mu in range(4) if (self.mask >> mu) & 1 and grid.neighbour(mu, 1) != grid.rank)
+        self.recv = coarse_halo_buffers(cdims, nvec, rmask, dtype=rdt, device=A.device)
+        self.comm = torch.cuda.Stream(device=A.device)
+
+    def apply(self, out, inp, dagger=False):
+        cur = torch.cuda.current_stream(self.A.device)
+        coarse_halo_pack(self.send, inp, self.cdims, self.nvec, self.mask, stream=cur)
+        packed = cur.record_event()
+        with torch.cuda.stream(self.comm):
+            self.comm.wait_event(packed)
+            got = exchange_faces(self.send, self.recv, self.grid, self.mask, self.group)
+            arrived = self.comm.record_event()
+        coarse_mult_interior(out, inp, self.A, self.cdims, self.nvec, self.mask, dagger, stream=cur)
+        cur.wait_event(arrived)
+        coarse_halo_add(out, got, self.A, self.cdims, self.nvec, self.mask, dagger, stream=cur)
         return out

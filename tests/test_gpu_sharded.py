@@ -153,3 +153,118 @@ def test_halo_argument_errors(lq, prob8):
     with pytest.raises(lq.LqcdError):
         lq.wilson_clover_mult_interior(y, y, U, U, cfg.kappa, cfg.dims, cfg.bc, 8)               # out aliases in
     assert lq.launch_count() == n0                                       # nothing enqueued on error
+
+
+# ---- the coarse operator and the block-local transfers on sub-lattices --------------------------------------------
+def sharded_Dc(lq, A, xc, cdims, nvec, prec, ranks, part_mask=None, dagger=False):
+    import torch
+    from paper_2111_05012_b200 import sharded as sh
+    world = int(np.prod(ranks))
+    grids = [sh.RankGrid(ranks, r) for r in range(world)]
+    mask = grids[0].part_mask if part_mask is None else part_mask
+    lc = grids[0].local_dims(cdims)
+    loc = []
+    for g in grids:
+        Al = to_dev(sh.split_field(A, cdims, g), prec)
+        xl = to_dev(sh.split_field(xc, cdims, g), prec)
+        send = lq.coarse_halo_buffers(lc, nvec, mask, dtype=torch.float32 if prec == "f32" else torch.float64)
+        lq.coarse_halo_pack(send, xl, lc, nvec, mask)
+        loc.append((Al, xl, send))
+    recvs = sh.route_faces([l[2] for l in loc], ranks, mask)
+    parts = []
+    for (Al, xl, _), recv in zip(loc, recvs):
+        y = torch.full_like(xl, 7.0)
+        lq.coarse_mult_interior(y, xl, Al, lc, nvec, mask, dagger=dagger)
+        lq.coarse_halo_add(y, recv, Al, lc, nvec, mask, dagger=dagger)
+        parts.append(y.cpu().numpy())
+    return sh.join_field(parts, cdims, ranks)
+
+
+@pytest.fixture(scope="module")
+def probc():
+    # coarse lattice 4 x 2 x 6 x 4, N = 12 (a ragged row: 6 float4 / 12 double2 per row)
+    return make_problem(custom_config((8, 4, 12, 8), (2, 2, 2, 2), 6, bc=(1, 1, 1, -1), seed=21))
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_sharded_coarse_matches_global_oracle(lq, probc, prec, dagger):
+    cfg = probc.cfg
+    A, xc = rounded(probc.A, prec), rounded(probc.xc, prec)
+    want = oracle.coarse_mult(xc, A, cfg.cdims, dagger=dagger)
+    for ranks, mask in [((1, 1, 1, 2), None), ((2, 1, 3, 2), None), ((4, 2, 6, 4), None), ((1, 1, 1, 1), 15),
+                        ((2, 2, 1, 1), 15), ((1, 1, 6, 1), 4 | 8)]:
+        got = sharded_Dc(lq, A, xc, cfg.cdims, cfg.nvec, prec, ranks, part_mask=mask, dagger=dagger)
+        assert rel_l2(got, want) <= TOL[prec], (ranks, mask)
+
+
+def test_sharded_coarse_n64_and_class(lq):
+    """N = 64 (the paper's size; the full-row fast path of k_coarse) and the ShardedCoarse class with self exchange."""
+    import torch
+    import lqcd_inputs as li
+    from paper_2111_05012_b200 import sharded as sh
+    cdims, nvec = (4, 4, 2, 6), 32
+    rng = np.random.default_rng(5)
+    Vc = int(np.prod(cdims))
+    A = rounded(li.coarse_matrix_synthetic(rng, Vc, nvec), "f32")
+    xc = rounded(li.coarse_vector(rng, Vc, nvec), "f32")
+    want = oracle.coarse_mult(xc, A, cdims)
+    assert rel_l2(sharded_Dc(lq, A, xc, cdims, nvec, "f32", (2, 1, 1, 3)), want) <= TOL["f32"]
+    op = sh.ShardedCoarse(to_dev(A, "f32"), cdims, nvec, sh.RankGrid((1, 1, 1, 1)), part_mask=15)
+    x = to_dev(xc, "f32")
+    y = torch.empty_like(x)
+    op.apply(y, x)
+    torch.cuda.synchronize()
+    assert rel_l2(y.cpu().numpy(), want) <= TOL["f32"]
+    y1 = torch.empty_like(x)
+    lq.coarse_mult(y1, x, to_dev(A, "f32"), cdims, nvec)
+    y0 = torch.empty_like(x)
+    lq.coarse_mult_interior(y0, x, to_dev(A, "f32"), cdims, nvec, 0)          # nothing partitioned: D_c itself
+    assert torch.equal(y0, y1)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_transfers_are_block_local(lq, probc, prec):
+    """A4/A5 need no exchange when the aggregates do not straddle ranks: restrict and prolong on the
+    sub-lattices, with the null vectors of the local aggregates, reproduce the oracle on the global lattice."""
+    import torch
+    from paper_2111_05012_b200 import sharded as sh
+    cfg = probc.cfg
+    ranks = (2, 1, 3, 2)
+    v, psi, xc = rounded(probc.v, prec), rounded(probc.psi[0], prec), rounded(probc.xc, prec)
+    want_r = oracle.restrict(psi, v, cfg.dims, cfg.block)
+    want_p = oracle.prolong(xc, v, cfg.dims, cfg.block)
+    got_r, got_p = [], []
+    for r in range(int(np.prod(ranks))):
+        g = sh.RankGrid(ranks, r)
+        ld, lc = g.local_dims(cfg.dims), g.local_dims(cfg.cdims)
+        vl = lq.pack_nullvecs(to_dev(sh.split_field(v, cfg.dims, g, site_axis=1), prec), ld, cfg.block)
+        x = lq.pack_spinor(to_dev(sh.split_field(psi, cfg.dims, g), prec), ld)
+        yc = torch.empty((int(np.prod(lc)), 2, cfg.nvec), dtype=to_dev(np.zeros(1), prec).dtype, device="cuda")
+        lq.restrict(yc, x, vl, ld, cfg.block, cfg.nvec)
+        got_r.append(yc.cpu().numpy())
+        yf = lq.empty_spinor(ld, dtype=x.dtype)
+        lq.prolong(yf, to_dev(sh.split_field(xc, cfg.cdims, g), prec), vl, ld, cfg.block, cfg.nvec)
+        got_p.append(lq.unpack_spinor(yf, ld).cpu().numpy())
+    assert rel_l2(sh.join_field(got_r, cfg.cdims, ranks), want_r) <= TOL[prec]
+    assert rel_l2(sh.join_field(got_p, cfg.dims, ranks), want_p) <= TOL[prec]
+
+
+def test_coarse_halo_argument_errors(lq):
+    import torch
+    cdims, nvec = (2, 2, 2, 4), 4
+    A = torch.zeros((32, 9, 8, 8), dtype=torch.complex64, device="cuda")
+    x = torch.zeros((32, 2, 4), dtype=torch.complex64, device="cuda")
+    y = torch.zeros_like(x)
+    send = lq.coarse_halo_buffers(cdims, nvec, 8)
+    assert send[7].numel() == lq.coarse_halo_face_reals(cdims, nvec, 3) == 8 * 16 and send[1] is None
+    n0 = lq.launch_count()
+    with pytest.raises(lq.LqcdError):
+        lq.coarse_halo_pack(send, x, cdims, nvec, 1 | 8)                       # face 0 has no buffer
+    with pytest.raises(lq.LqcdError):
+        lq.coarse_halo_add(y, send, A, cdims, nvec, 4 | 8)                     # recv of direction 2 missing
+    with pytest.raises(lq.LqcdError):
+        lq.coarse_mult_interior(y, x, A, (2, 2, 1, 4), nvec, 8)                # extent 1 in an unpartitioned direction
+    with pytest.raises(lq.LqcdError):
+        lq.coarse_mult_interior(y, x, A, cdims, nvec, 16)
+    assert lq.launch_count() == n0
