@@ -165,6 +165,18 @@ class Ranks:
             self.dist.destroy_process_group()
 
 
+def default_rank_grid(world: int):
+    """Split t first, then z, y, x, by factors of two (an odd remainder goes to t): 2 -> 1x1x1x2, 8 -> 1x2x2x2."""
+    r = [1, 1, 1, 1]
+    mu = 3
+    while world % 2 == 0:
+        r[mu] *= 2
+        world //= 2
+        mu = (mu - 1) % 4
+    r[3] *= world
+    return tuple(r)
+
+
 def whole_job_value(units_per_rank: float, world: int, max_seconds: float) -> float:
     """weak scaling, replicas: every rank processes units_per_rank in (at most) max_seconds."""
     return units_per_rank * world / max_seconds
@@ -238,6 +250,7 @@ class Workload:
         import torch
         import paper_2111_05012_b200 as lq
         self.cfg, self.lq, self.dev = cfg, lq, device
+        self.sh_fine = self.sh_coarse = None
         gen = torch.Generator(device=device)
         gen.manual_seed(seed)
         V, Vc, nv = cfg.volume, cfg.cvolume, cfg.nvec
@@ -283,13 +296,25 @@ class Workload:
                                                                           cfg.dims, cfg.bc, cfg.block, nv))
         torch.cuda.synchronize()
 
+    def enable_sharded(self, grid, part_mask):
+        """--sharded: this rank's fields are one sub-lattice of a lattice split over `grid`; D, D^dag and D_c then run
+        as pack -> [exchange || interior] -> add (paper_2111_05012_b200/sharded.py); restrict / prolong are block-local."""
+        from paper_2111_05012_b200 import sharded as sh
+        c = self.cfg
+        self.sh_fine = sh.ShardedWilsonClover(self.U18, self.clover, c.kappa, c.dims, c.bc, grid, part_mask=part_mask)
+        self.sh_coarse = sh.ShardedCoarse(self.A, c.cdims, c.nvec, grid, part_mask=part_mask)
+
     # one launch per row; `i` picks the buffer set
     def wilson_clover(self, i):
         c = self.cfg
+        if self.sh_fine is not None:
+            return self.sh_fine.apply(self.y[i], self.x[i])
         self.lq.wilson_clover_mult(self.y[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc)
 
     def wilson_clover_dagger(self, i):
         c = self.cfg
+        if self.sh_fine is not None:
+            return self.sh_fine.apply(self.yd[i], self.x[i], dagger=True)
         self.lq.wilson_clover_mult(self.yd[i], self.x[i], self.U18, self.clover, c.kappa, c.dims, c.bc, dagger=True)
 
     def wilson_clover_12(self, i):
@@ -322,6 +347,9 @@ class Workload:
     def sharded_self(self, i):
         self.sharded_op.apply(self.y[i], self.x[i])
 
+    def sharded_self_coarse(self, i):
+        self.sharded_op.apply(self.yc[i], self.xc[i])
+
     def coarse_mrhs(self, i):
         c = self.cfg
         self.lq.coarse_mult_mrhs(self.ycK, self.xcK, self.A, c.cdims, c.nvec)
@@ -350,6 +378,8 @@ class Workload:
 
     def coarse_mult(self, i):
         c = self.cfg
+        if self.sh_coarse is not None:
+            return self.sh_coarse.apply(self.yc[i], self.xc[i])
         self.lq.coarse_mult(self.yc[i], self.xc[i], self.A, c.cdims, c.nvec)
 
     def prolong(self, i):
@@ -564,6 +594,21 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     W = Workload(cfg, device, seed=cfg.seed + 17 * ranks.rank, synthetic_operators=args.synthetic_operators)
     m = model(cfg)
     peak, peak_src = measured_peak()
+    sharded = None
+    if args.sharded is not None:
+        from paper_2111_05012_b200 import sharded as sh
+        rg = tuple(int(v) for v in args.sharded.split(",")) if args.sharded else default_rank_grid(ranks.world)
+        grid = sh.RankGrid(rg, ranks.rank)
+        if grid.world != ranks.world:
+            raise SystemExit(f"--sharded {rg}: {grid.world} ranks, but WORLD_SIZE = {ranks.world}")
+        mask = grid.part_mask | args.sharded_mask
+        W.enable_sharded(grid, mask)
+        sharded = {"rank_grid": list(rg), "part_mask": mask,
+                   "global_dims": [cfg.dims[mu] * rg[mu] for mu in range(4)],
+                   "halo_bytes_sent_per_D": 2 * 4 * sum(lq.halo_face_reals(cfg.dims, mu) for mu in range(4)
+                                                        if (mask >> mu) & 1),
+                   "halo_bytes_sent_per_Dc": 2 * 4 * sum(lq.coarse_halo_face_reals(cfg.cdims, cfg.nvec, mu)
+                                                         for mu in range(4) if (mask >> mu) & 1)}
 
     sampler = ClockSampler(dev_index)
     sampler.start()
@@ -591,7 +636,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     }
     # the 12-real-link variant of A1 (config 4 asks for both storages), timed alone
     extra = {}
-    if not args.no_extras:
+    if not args.no_extras and sharded is None:
         t12 = time_single(W, "wilson_clover_12", reps=max(10, args.steps))
         m12 = model(cfg, links12=True)["wilson_clover"]
         extra["wilson_clover_links12"] = {"us": t12 * 1e6, "GBps": m12["bytes"] / t12 / 1e9,
@@ -682,19 +727,28 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "speedup_vs_2_single_applications": 2 * kernels["wilson_clover"]["us"] * 1e-6 / t,
             "frac_of_hbm_peak": fb / t / 1e9 / peak, "bytes_per_launch": fb}
         del W.x2, W.y2
-        # SURVEY 8(e), the sharded operator's own cost on one GPU: all four directions partitioned, the rank its own
-        # neighbour (pack -> interior -> add; no link traffic, so this is the kernels' overhead over the plain D)
+        # SURVEY 8(e), the sharded operators' own cost on one GPU: directions marked partitioned with the rank as its
+        # own neighbour (pack -> interior -> add; nothing crosses a link, so this is the kernels' overhead over the
+        # plain operator; a multi-GPU run adds only the transfer of the halo bytes, overlapped with the interior pass)
         from paper_2111_05012_b200 import sharded as sh
-        W.sharded_op = sh.ShardedWilsonClover(W.U18, W.clover, cfg.kappa, cfg.dims, cfg.bc, sh.RankGrid((1, 1, 1, 1)),
-                                              part_mask=15)
-        t = time_single(W, "sharded_self", reps=max(10, args.steps))
-        face_b = 2 * 4 * sum(W.lq.halo_face_reals(cfg.dims, mu) for mu in range(4))
-        extra["wilson_clover_sharded_selfhalo"] = {
-            "us": t * 1e6, "overhead_vs_plain": t / (kernels["wilson_clover"]["us"] * 1e-6),
-            "GBps": m["wilson_clover"]["bytes"] / t / 1e9, "halo_bytes_sent_per_application": face_b,
-            "launches_per_application": 6,
-            "note": "one rank exchanging with itself in all 4 directions; a multi-GPU run adds only the transfer of "
-                    "halo_bytes (12 reals per face site), overlapped with the interior pass"}
+        one = sh.RankGrid((1, 1, 1, 1))
+        sd = {"note": "one rank exchanging with itself; masks: t, z+t, all four directions"}
+        for tag, mask in (("t", 8), ("zt", 12), ("xyzt", 15)):
+            W.sharded_op = sh.ShardedWilsonClover(W.U18, W.clover, cfg.kappa, cfg.dims, cfg.bc, one, part_mask=mask)
+            t = time_single(W, "sharded_self", reps=max(10, args.steps))
+            sd[tag] = {"us": t * 1e6, "overhead_vs_plain": t / (kernels["wilson_clover"]["us"] * 1e-6),
+                       "halo_bytes_sent": 2 * 4 * sum(W.lq.halo_face_reals(cfg.dims, mu) for mu in range(4)
+                                                      if (mask >> mu) & 1),
+                       "launches": 2 + bin(mask).count("1")}
+        extra["wilson_clover_sharded_selfhalo"] = sd
+        sc = {}
+        for tag, mask in (("t", 8), ("zt", 12), ("xyzt", 15)):
+            W.sharded_op = sh.ShardedCoarse(W.A, cfg.cdims, cfg.nvec, one, part_mask=mask)
+            t = time_single(W, "sharded_self_coarse", reps=max(10, args.steps))
+            sc[tag] = {"us": t * 1e6, "overhead_vs_plain": t / (kernels["coarse_mult"]["us"] * 1e-6),
+                       "halo_bytes_sent": 2 * 4 * sum(W.lq.coarse_halo_face_reals(cfg.cdims, cfg.nvec, mu)
+                                                      for mu in range(4) if (mask >> mu) & 1), "launches": 3}
+        extra["coarse_mult_sharded_selfhalo"] = sc
         del W.sharded_op
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
@@ -715,6 +769,11 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         "operators": "synthetic" if args.synthetic_operators else "device-built (clover from links, Galerkin P^dag D P)", "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if sharded is not None:  # one lattice over all ranks: the per-rank sub-lattice is the config's lattice (weak)
+        line["config"]["parallelism"] = ("sharded: one lattice of %s over a %s grid of ranks; halo exchange per D, "
+                                         "D^dag, D_c" % ("x".join(map(str, sharded["global_dims"])),
+                                                         "x".join(map(str, sharded["rank_grid"]))))
+        line["sharded"] = sharded
     if ranks.rank == 0 and ranks.world == 1 and not args.no_cpu_baseline:
         smp = OracleSample(cfg)
         sec = smp.time(3, 1)
@@ -792,6 +851,12 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--sharded", nargs="?", const="", default=None, metavar="R0,R1,R2,R3",
+                    help="opt-in: the ranks share ONE lattice (each holds a sub-lattice of the config's size) and "
+                         "exchange halos; default grid splits t, z, y, x in turn")
+    ap.add_argument("--sharded-mask", type=int, default=0,
+                    help="with --sharded: also treat these directions (bit mu) as partitioned, the rank being its own "
+                         "neighbour there (exercises the whole exchange path on one GPU)")
     ap.add_argument("--synthetic-operators", action="store_true",
                     help="random clover term and coarse matrix instead of the device-built ones (DESIGN.md section 4)")
     ap.add_argument("--sweep", action="store_true", help="config 5's bandwidth-roofline sweep over volumes (1 GPU)")

@@ -404,8 +404,8 @@ int lqcd_wilson_clover_halo_add_f64(double* out, const double* const recv[8], co
  * the other three coordinates; lqcd_coarse_halo_face_reals(cdims, nvec, mu) reals each.  Exchange as above
  * (recv[2 mu] := send[2 mu + 1] of the -mu neighbour, recv[2 mu + 1] := send[2 mu] of the +mu neighbour).
  *   lqcd_coarse_halo_pack      in -> send[8]
- *   lqcd_coarse_mult_interior  out = D_c in without the blocks of leaving hops (neither A nor in is read for them)
- *   lqcd_coarse_halo_add       out += those blocks applied to recv[8]            (one launch; boundary sites only)
+ *   lqcd_coarse_mult_interior  out = D_c in without the blocks of leaving hops (their sources are not read)
+ *   lqcd_coarse_halo_add       out += those blocks applied to recv[8]            (one launch per face, over its sites only)
  * flags: LQCD_DAGGER on mult_interior and halo_add alike.  A partitioned direction may have local extent 1. */
 size_t lqcd_coarse_halo_face_reals(const int cdims[4], int nvec, int mu);
 int lqcd_coarse_halo_pack_f32(float* const send[8], const float* in, const int cdims[4], int nvec, unsigned part_mask,

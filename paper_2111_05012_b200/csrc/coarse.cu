@@ -28,6 +28,8 @@ struct CoarseParams {
     long long ntask;  // Vc * ntile / tpw warp tasks
     int dagger;
     unsigned part_mask;  // sharded variants only: bit mu = direction mu is partitioned over ranks
+    int nsites;          // sites the grid enumerates: Vc, or the face volume in MODE 2
+    int face;            // MODE 2: the face 2 mu + dir this launch completes
 };
 
 // received faces of the sharded operator (MODE 2): face 2 mu + dir, [face site][N complex]
@@ -58,9 +60,9 @@ template <> __device__ __forceinline__ void cmadd<double>(double& sr, double& si
 // FULL: N is a multiple of the row tile and a row is exactly LPR*CPL vec16 -- no bounds predicates, so the loads of
 // a tile are unconditional and stay batched at the top of the tile.
 // MODE 0: the operator.  Sharded variants (halo exchange on the coarse lattice): MODE 1 = interior
-// pass, the blocks of hops that leave the local lattice in a partitioned direction are skipped (neither A nor the
-// source is read); MODE 2 = boundary completion, out += exactly those blocks with the sources taken from the received
-// faces (warps of interior sites exit at once).
+// pass, the blocks of hops that leave the local lattice in a partitioned direction act on zero (the source is not
+// read); MODE 2 = boundary completion, one launch per face over its sites only: out += the block of the hop that leaves
+// through that face, applied to the received face.
 template <typename T, int LPR, int CPL, int R, bool FULL, int MODE = 0>
 __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ A,
                                                 CoarseParams P, CoarseFaces F = CoarseFaces()) {
@@ -72,61 +74,68 @@ __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T*
     const long long task = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (task >= P.ntask) return;
     const int wps = P.ntile / P.tpw;  // warps per site
-    const int X = (int)(task / wps);
+    int X = (int)(task / wps);  // MODE 2: the face site
     const int tile0 = (int)(task % wps) * P.tpw;
 
     // the nine source sites
     int src[9];
-    unsigned cut = 0;  // MODE 1, 2: bit d = hop d leaves the local lattice in a partitioned direction
+    unsigned cut = 0;  // MODE 1: bit d = hop d leaves the local lattice in a partitioned direction
+    int blk0 = 0;      // MODE 2: the one block this launch applies (slot 0 of the arrays below)
     {
-        int xc[4], rem = X;
-        xc[0] = rem % P.Lc[0]; rem /= P.Lc[0];
-        xc[1] = rem % P.Lc[1]; rem /= P.Lc[1];
-        xc[2] = rem % P.Lc[2]; rem /= P.Lc[2];
-        xc[3] = rem;
+        int xc[4];
         const int stride[4] = {1, P.Lc[0], P.Lc[0] * P.Lc[1], P.Lc[0] * P.Lc[1] * P.Lc[2]};
-        src[0] = X;
+        if (MODE == 2) {
+            // one launch per face: site from the face index; the only live block is the hop that leaves through it
+            // (X_mu = Lc - 1: forward hop d = 1 + 2 mu, served by face 2 mu + 1; X_mu = 0: d = 2 + 2 mu, face 2 mu)
+            const int mu = P.face >> 1, dir = P.face & 1, f = X;
+            int rem = f;
+            X = 0;
 #pragma unroll
-        for (int mu = 0; mu < 4; mu++) {
-            src[1 + 2 * mu] = (xc[mu] == P.Lc[mu] - 1) ? X - (P.Lc[mu] - 1) * stride[mu] : X + stride[mu];
-            src[2 + 2 * mu] = (xc[mu] == 0) ? X + (P.Lc[mu] - 1) * stride[mu] : X - stride[mu];
+            for (int nu = 0; nu < 4; nu++) {
+                if (nu == mu) {
+                    xc[nu] = dir ? P.Lc[nu] - 1 : 0;
+                } else {
+                    xc[nu] = rem % P.Lc[nu];
+                    rem /= P.Lc[nu];
+                }
+                X += xc[nu] * stride[nu];
+            }
+            blk0 = dir ? 1 + 2 * mu : 2 + 2 * mu;
+            src[0] = f;
+        } else {
+            int rem = X;
+            xc[0] = rem % P.Lc[0]; rem /= P.Lc[0];
+            xc[1] = rem % P.Lc[1]; rem /= P.Lc[1];
+            xc[2] = rem % P.Lc[2]; rem /= P.Lc[2];
+            xc[3] = rem;
+            src[0] = X;
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++) {
+                src[1 + 2 * mu] = (xc[mu] == P.Lc[mu] - 1) ? X - (P.Lc[mu] - 1) * stride[mu] : X + stride[mu];
+                src[2 + 2 * mu] = (xc[mu] == 0) ? X + (P.Lc[mu] - 1) * stride[mu] : X - stride[mu];
+            }
         }
-        if (MODE != 0) {
+        if (MODE == 1) {
 #pragma unroll
             for (int mu = 0; mu < 4; mu++) {
                 if (!((P.part_mask >> mu) & 1)) continue;
-                // face site: lexicographic index of the other three coordinates
-                int f = 0, fs = 1;
-#pragma unroll
-                for (int nu = 0; nu < 4; nu++)
-                    if (nu != mu) {
-                        f += xc[nu] * fs;
-                        fs *= P.Lc[nu];
-                    }
-                if (xc[mu] == P.Lc[mu] - 1) {
-                    cut |= 1u << (1 + 2 * mu);
-                    if (MODE == 2) src[1 + 2 * mu] = f;
-                }
-                if (xc[mu] == 0) {
-                    cut |= 1u << (2 + 2 * mu);
-                    if (MODE == 2) src[2 + 2 * mu] = f;
-                }
+                if (xc[mu] == P.Lc[mu] - 1) cut |= 1u << (1 + 2 * mu);
+                if (xc[mu] == 0) cut |= 1u << (2 + 2 * mu);
             }
-            if (MODE == 2 && cut == 0) return;
         }
     }
-    // does block d take part in this pass?
-    auto live = [&](int d) -> bool { return MODE == 0 ? true : MODE == 1 ? !((cut >> d) & 1) : ((cut >> d) & 1); };
-    // my slices of the nine source vectors (with the Gamma5c sign of the column for the dagger variant)
-    V16<T> xv[9][CPL];
+    constexpr int ND = MODE == 2 ? 1 : 9;  // blocks per site in this pass
+    // does the source of slot d take part in this pass?
+    auto live = [&](int d) -> bool { return MODE == 1 ? !((cut >> d) & 1) : true; };
+    // my slices of the source vectors (with the Gamma5c sign of the column for the dagger variant)
+    V16<T> xv[ND][CPL];
 #pragma unroll
-    for (int d = 0; d < 9; d++)
+    for (int d = 0; d < ND; d++)
 #pragma unroll
         for (int c = 0; c < CPL; c++) {
             const int v = q + LPR * c;
             if ((FULL || v < P.RV) && live(d)) {
-                // MODE 2: hop d = 1 + 2 mu (forward) is served by face 2 mu + 1, d = 2 + 2 mu (backward) by face 2 mu
-                const T* from = MODE == 2 ? static_cast<const T*>(F.p[d == 0 ? 0 : ((d - 1) >> 1) * 2 + (d & 1)]) : in;
+                const T* from = MODE == 2 ? static_cast<const T*>(F.p[0]) : in;  // the launch's face
                 xv[d][c] = ld16(from + ((long long)src[d] * P.RV + v) * NV);
                 if (P.dagger) {
 #pragma unroll
@@ -142,23 +151,25 @@ __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T*
             }
         }
 
-    const T* Asite = A + (long long)X * 9 * P.N * P.RV * NV;
+    const T* Asite = A + ((long long)X * 9 + blk0) * P.N * P.RV * NV;
     for (int t = 0; t < P.tpw; t++) {
         const int rbase = (tile0 + t) * (G * R);
         T sr[R], si[R];
 #pragma unroll
         for (int r = 0; r < R; r++) sr[r] = si[r] = 0;
         // issue all loads of the tile first (R * 9 * CPL independent 16-byte requests per lane)
-        V16<T> a[R][9][CPL];
+        V16<T> a[R][ND][CPL];
 #pragma unroll
         for (int r = 0; r < R; r++) {
             const int row = rbase + r * G + g;
 #pragma unroll
-            for (int d = 0; d < 9; d++)
+            for (int d = 0; d < ND; d++)
 #pragma unroll
                 for (int c = 0; c < CPL; c++) {
                     const int v = q + LPR * c;
-                    if ((FULL || (row < P.N && v < P.RV)) && live(d))
+                    // (MODE 1 streams the blocks of cut hops too -- their sources are zero: a per-block predicate
+                    // breaks the batch of unconditional loads and costs 12 %, the skipped bytes would save < 1 %)
+                    if (FULL || (row < P.N && v < P.RV))
                         a[r][d][c] = ld16_stream(Asite + (((long long)d * P.N + row) * P.RV + v) * NV);
                     else {
 #pragma unroll
@@ -169,7 +180,7 @@ __global__ void __launch_bounds__(256, 2) k_coarse(T* __restrict__ out, const T*
 #pragma unroll
         for (int r = 0; r < R; r++)
 #pragma unroll
-            for (int d = 0; d < 9; d++)
+            for (int d = 0; d < ND; d++)
 #pragma unroll
                 for (int c = 0; c < CPL; c++) cmadd<T>(sr[r], si[r], a[r][d][c], xv[d][c]);
         // finish the row dot products across the LPR lanes of each group
@@ -203,13 +214,15 @@ static void launch_coarse_mode(T* out, const T* in, const T* A, CoarseParams P, 
     P.ntile = (P.N + G * R - 1) / (G * R);
     // row tiles per warp: as many as possible (the nine source slices are loaded once per warp) while the grid
     // still has several waves of warps (>= 148 SMs x 256 warp tasks)
+    // (the thin per-face launches of MODE 2 amortise the per-warp set-up over more rows: one wave of 32 warps per SM)
+    const long long min_tasks = MODE == 2 ? 148LL * 32 : 148LL * 256;
     int tpw = g_knobs.coarse_rows_per_warp > 0 ? g_knobs.coarse_rows_per_warp : P.ntile;
     if (tpw > P.ntile) tpw = P.ntile;
     while (tpw > 1 && (P.ntile % tpw != 0 ||
-                       (g_knobs.coarse_rows_per_warp <= 0 && (long long)P.Vc * (P.ntile / tpw) < 148LL * 256)))
+                       (g_knobs.coarse_rows_per_warp <= 0 && (long long)P.nsites * (P.ntile / tpw) < min_tasks)))
         tpw--;
     P.tpw = tpw;
-    P.ntask = (long long)P.Vc * (P.ntile / tpw);
+    P.ntask = (long long)P.nsites * (P.ntile / tpw);
     int warps = g_knobs.coarse_warps > 0 ? g_knobs.coarse_warps : 4;
     if (warps > 8) warps = 8;
     const long long grid = (P.ntask + warps - 1) / warps;
@@ -287,20 +300,37 @@ static int coarse_call(T* out, const T* in, const T* A, const int cdims[4], int 
         set_error("%s: nvec = %d outside the compiled range (row longer than 128 vec16)", what, nvec);
         return LQCD_EUNSUPPORTED;
     }
-    if (RV <= 1) launch_coarse<T, 1, 1, 2>(out, in, A, P, st, mode, F);
-    else if (RV <= 2) launch_coarse<T, 2, 1, 2>(out, in, A, P, st, mode, F);
-    else if (RV <= 4) launch_coarse<T, 4, 1, 2>(out, in, A, P, st, mode, F);
-    else if (RV <= 8) launch_coarse<T, 8, 1, 2>(out, in, A, P, st, mode, F);
-    else if (RV <= 16) launch_coarse<T, 16, 1, 2>(out, in, A, P, st, mode, F);
-    else if (RV <= 32) {
-        if (g_knobs.coarse_R == 1) launch_coarse<T, 32, 1, 1>(out, in, A, P, st, mode, F);
-        else if (g_knobs.coarse_R == 4) launch_coarse<T, 32, 1, 4>(out, in, A, P, st, mode, F);
-        else launch_coarse<T, 32, 1, 2>(out, in, A, P, st, mode, F);
+    CoarseFaces Fl = F;  // MODE 2: slot 0 = the face of the launch
+    auto launch = [&]() {
+        if (RV <= 1) launch_coarse<T, 1, 1, 2>(out, in, A, P, st, mode, Fl);
+        else if (RV <= 2) launch_coarse<T, 2, 1, 2>(out, in, A, P, st, mode, Fl);
+        else if (RV <= 4) launch_coarse<T, 4, 1, 2>(out, in, A, P, st, mode, Fl);
+        else if (RV <= 8) launch_coarse<T, 8, 1, 2>(out, in, A, P, st, mode, Fl);
+        else if (RV <= 16) launch_coarse<T, 16, 1, 2>(out, in, A, P, st, mode, Fl);
+        else if (RV <= 32) {
+            if (g_knobs.coarse_R == 1) launch_coarse<T, 32, 1, 1>(out, in, A, P, st, mode, Fl);
+            else if (g_knobs.coarse_R == 4 || (mode == 2 && g_knobs.coarse_R == 0))  // thin launch: more rows in flight
+                launch_coarse<T, 32, 1, 4>(out, in, A, P, st, mode, Fl);
+            else launch_coarse<T, 32, 1, 2>(out, in, A, P, st, mode, Fl);
+        }
+        else if (RV <= 64) launch_coarse<T, 32, 2, 1>(out, in, A, P, st, mode, Fl);
+        else if (RV <= 96) launch_coarse<T, 32, 3, 1>(out, in, A, P, st, mode, Fl);
+        else launch_coarse<T, 32, 4, 1>(out, in, A, P, st, mode, Fl);
+        count_launch();
+    };
+    P.nsites = P.Vc;
+    P.face = 0;
+    if (mode != 2) {
+        launch();
+    } else {  // one launch per face, in face order (a site on several faces is completed in a fixed order)
+        for (int face = 0; face < 8; face++) {
+            if (!((part_mask >> (face >> 1)) & 1)) continue;
+            P.face = face;
+            Fl.p[0] = F.p[face];
+            P.nsites = P.Vc / P.Lc[face >> 1];
+            launch();
+        }
     }
-    else if (RV <= 64) launch_coarse<T, 32, 2, 1>(out, in, A, P, st, mode, F);
-    else if (RV <= 96) launch_coarse<T, 32, 3, 1>(out, in, A, P, st, mode, F);
-    else launch_coarse<T, 32, 4, 1>(out, in, A, P, st, mode, F);
-    count_launch();
     return check_launch(what);
 }
 
