@@ -296,13 +296,14 @@ class Workload:
                                                                           cfg.dims, cfg.bc, cfg.block, nv))
         torch.cuda.synchronize()
 
-    def enable_sharded(self, grid, part_mask):
+    def enable_sharded(self, grid, part_mask, transport="p2p"):
         """--sharded: this rank's fields are one sub-lattice of a lattice split over `grid`; D, D^dag and D_c then run
         as pack -> [exchange || interior] -> add (paper_2111_05012_b200/sharded.py); restrict / prolong are block-local."""
         from paper_2111_05012_b200 import sharded as sh
         c = self.cfg
-        self.sh_fine = sh.ShardedWilsonClover(self.U18, self.clover, c.kappa, c.dims, c.bc, grid, part_mask=part_mask)
-        self.sh_coarse = sh.ShardedCoarse(self.A, c.cdims, c.nvec, grid, part_mask=part_mask)
+        self.sh_fine = sh.ShardedWilsonClover(self.U18, self.clover, c.kappa, c.dims, c.bc, grid, part_mask=part_mask,
+                                              transport=transport)
+        self.sh_coarse = sh.ShardedCoarse(self.A, c.cdims, c.nvec, grid, part_mask=part_mask, transport=transport)
 
     # one launch per row; `i` picks the buffer set
     def wilson_clover(self, i):
@@ -602,8 +603,13 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         if grid.world != ranks.world:
             raise SystemExit(f"--sharded {rg}: {grid.world} ranks, but WORLD_SIZE = {ranks.world}")
         mask = grid.part_mask | args.sharded_mask
-        W.enable_sharded(grid, mask)
-        sharded = {"rank_grid": list(rg), "part_mask": mask,
+        if args.sharded_transport == "peer" and ranks.dist is None:  # symmetric memory rendezvous needs a group
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29512")
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=device)
+        W.enable_sharded(grid, mask, args.sharded_transport)
+        sharded = {"rank_grid": list(rg), "part_mask": mask, "transport": args.sharded_transport,
                    "global_dims": [cfg.dims[mu] * rg[mu] for mu in range(4)],
                    "halo_bytes_sent_per_D": 2 * 4 * sum(lq.halo_face_reals(cfg.dims, mu) for mu in range(4)
                                                         if (mask >> mu) & 1),
@@ -854,6 +860,9 @@ def main():
     ap.add_argument("--sharded", nargs="?", const="", default=None, metavar="R0,R1,R2,R3",
                     help="opt-in: the ranks share ONE lattice (each holds a sub-lattice of the config's size) and "
                          "exchange halos; default grid splits t, z, y, x in turn")
+    ap.add_argument("--sharded-transport", choices=("p2p", "peer"), default="p2p",
+                    help="with --sharded: p2p = pack, then torch.distributed send/recv; peer = the pack kernels store "
+                         "into the neighbours' receive buffers over NVLink peer memory (symmetric memory)")
     ap.add_argument("--sharded-mask", type=int, default=0,
                     help="with --sharded: also treat these directions (bit mu) as partitioned, the rank being its own "
                          "neighbour there (exercises the whole exchange path on one GPU)")

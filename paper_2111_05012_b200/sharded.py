@@ -142,6 +142,53 @@ def route_faces(sends, ranks, part_mask):
     return recvs
 
 
+class PeerFaces:
+    """The receive faces of this rank in ONE symmetric-memory allocation (torch.distributed._symmetric_memory), twice
+    (double-buffered), every rank's copy mapped into every other rank's address space over NVLink.
+
+    With it the exchange is no separate step: the pack kernel is handed, as its `send[8]`, the NEIGHBOURS' receive
+    buffers, so its stores are the transfer (compute and communication in one kernel, face site by face site), and
+    what remains is one device-side barrier (`arrive`, stream-ordered) before the add kernel may read.  Double
+    buffering makes that one barrier per application enough: a rank can write application n + 2 only after every
+    rank has passed barrier n + 1, which each rank enqueues after its add kernel of application n.
+    `face_reals[f]`: reals of face f (0 where the direction is not partitioned)."""
+
+    def __init__(self, face_reals, dtype, device, grid: RankGrid, group=None):
+        import torch.distributed as dist
+        import torch.distributed._symmetric_memory as symm
+        off, total = [], 0
+        for n in face_reals:
+            off.append(total)
+            total += (int(n) + 3) // 4 * 4                       # keep every face 16-byte aligned
+        self.total = total
+        self.buf = symm.empty(2 * total, dtype=dtype, device=device)
+        self.hdl = symm.rendezvous(self.buf, dist.group.WORLD if group is None else group)
+        if self.hdl.rank != grid.rank or self.hdl.world_size != grid.world:
+            raise ValueError("the rank grid must enumerate the ranks of the group")
+        self.send, self.recv, self.parity = [[None] * 8, [None] * 8], [[None] * 8, [None] * 8], 0
+        for par in range(2):
+            base = par * total
+            for mu in range(4):
+                lo, hi = 2 * mu, 2 * mu + 1
+                if not face_reals[lo]:
+                    continue
+                n = (int(face_reals[lo]),)
+                plus, minus = grid.neighbour(mu, +1), grid.neighbour(mu, -1)
+                self.recv[par][lo] = self.hdl.get_buffer(grid.rank, n, dtype, base + off[lo])
+                self.recv[par][hi] = self.hdl.get_buffer(grid.rank, n, dtype, base + off[hi])
+                # my forward face feeds the +mu neighbour's recv[2 mu]; my backward face the -mu neighbour's recv[2 mu + 1]
+                self.send[par][hi] = self.hdl.get_buffer(plus, n, dtype, base + off[lo])
+                self.send[par][lo] = self.hdl.get_buffer(minus, n, dtype, base + off[hi])
+
+    def next(self):
+        par, self.parity = self.parity, self.parity ^ 1
+        return self.send[par], self.recv[par]
+
+    def arrive(self):
+        """Every rank's stores issued before this point (on the stream it is called under) are visible after it."""
+        self.hdl.barrier(channel=0)
+
+
 class ShardedWilsonClover:
     """D (or D^dag) on this rank's sub-lattice of a lattice split over `grid`.
 
@@ -150,7 +197,10 @@ class ShardedWilsonClover:
     its own neighbour) -- the result is the same operator, which is how one GPU exercises the whole exchange path.
     """
 
-    def __init__(self, U, clover, kappa, dims, bc, grid: RankGrid, links12=False, part_mask=None, group=None):
+    def __init__(self, U, clover, kappa, dims, bc, grid: RankGrid, links12=False, part_mask=None, group=None,
+                 transport="p2p"):
+        """transport: "p2p" = pack into local buffers, torch.distributed send/recv; "peer" = the pack kernel stores
+        straight into the neighbours' receive buffers over NVLink peer memory (PeerFaces)."""
         self.U, self.clover, self.kappa = U, clover, float(kappa)
         self.dims, self.bc, self.grid, self.links12, self.group = tuple(dims), tuple(bc), grid, links12, group
         self.mask = grid.part_mask if part_mask is None else int(part_mask)
@@ -162,14 +212,25 @@ class ShardedWilsonClover:
         rmask = sum(1 << mu for mu in remote)
         self.recv = halo_buffers(dims, rmask, dtype=U.dtype, device=U.device)
         self.comm = torch.cuda.Stream(device=U.device)
+        self.peer = None
+        if transport == "peer":
+            from . import halo_face_reals
+            self.peer = PeerFaces([halo_face_reals(dims, f >> 1) if (self.mask >> (f >> 1)) & 1 else 0
+                                   for f in range(8)], U.dtype, U.device, grid, group)
+        elif transport != "p2p":
+            raise ValueError(f"transport {transport!r}")
 
     def apply(self, out, inp, dagger=False):
         cur = torch.cuda.current_stream(self.U.device)
-        wilson_clover_halo_pack(self.send, inp, self.U, self.dims, self.mask, dagger, self.links12, stream=cur)
+        send, got = (self.send, None) if self.peer is None else self.peer.next()
+        wilson_clover_halo_pack(send, inp, self.U, self.dims, self.mask, dagger, self.links12, stream=cur)
         packed = cur.record_event()
         with torch.cuda.stream(self.comm):           # the exchange overlaps the interior pass
             self.comm.wait_event(packed)
-            got = exchange_faces(self.send, self.recv, self.grid, self.mask, self.group)
+            if self.peer is None:
+                got = exchange_faces(self.send, self.recv, self.grid, self.mask, self.group)
+            else:
+                self.peer.arrive()
             arrived = self.comm.record_event()
         wilson_clover_mult_interior(out, inp, self.U, self.clover, self.kappa, self.dims, self.bc, self.mask, dagger,
                                     self.links12, stream=cur)
@@ -183,7 +244,7 @@ class ShardedCoarse:
     """D_c (or its dagger) on this rank's part of a coarse lattice split over `grid`; A: the blocks of the local sites.
     cdims = the LOCAL coarse extents.  No boundary phases: bc lives inside A."""
 
-    def __init__(self, A, cdims, nvec, grid: RankGrid, part_mask=None, group=None):
+    def __init__(self, A, cdims, nvec, grid: RankGrid, part_mask=None, group=None, transport="p2p"):
         self.A, self.cdims, self.nvec, self.grid, self.group = A, tuple(cdims), int(nvec), grid, group
         self.mask = grid.part_mask if part_mask is None else int(part_mask)
         if grid.part_mask & ~self.mask:
@@ -193,14 +254,25 @@ class ShardedCoarse:
         rmask = sum(1 << mu for mu in range(4) if (self.mask >> mu) & 1 and grid.neighbour(mu, 1) != grid.rank)
         self.recv = coarse_halo_buffers(cdims, nvec, rmask, dtype=rdt, device=A.device)
         self.comm = torch.cuda.Stream(device=A.device)
+        self.peer = None
+        if transport == "peer":
+            from . import coarse_halo_face_reals
+            self.peer = PeerFaces([coarse_halo_face_reals(cdims, nvec, f >> 1) if (self.mask >> (f >> 1)) & 1 else 0
+                                   for f in range(8)], rdt, A.device, grid, group)
+        elif transport != "p2p":
+            raise ValueError(f"transport {transport!r}")
 
     def apply(self, out, inp, dagger=False):
         cur = torch.cuda.current_stream(self.A.device)
-        coarse_halo_pack(self.send, inp, self.cdims, self.nvec, self.mask, stream=cur)
+        send, got = (self.send, None) if self.peer is None else self.peer.next()
+        coarse_halo_pack(send, inp, self.cdims, self.nvec, self.mask, stream=cur)
         packed = cur.record_event()
         with torch.cuda.stream(self.comm):
             self.comm.wait_event(packed)
-            got = exchange_faces(self.send, self.recv, self.grid, self.mask, self.group)
+            if self.peer is None:
+                got = exchange_faces(self.send, self.recv, self.grid, self.mask, self.group)
+            else:
+                self.peer.arrive()
             arrived = self.comm.record_event()
         coarse_mult_interior(out, inp, self.A, self.cdims, self.nvec, self.mask, dagger, stream=cur)
         cur.wait_event(arrived)

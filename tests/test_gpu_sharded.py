@@ -268,3 +268,60 @@ def test_coarse_halo_argument_errors(lq):
     with pytest.raises(lq.LqcdError):
         lq.coarse_mult_interior(y, x, A, cdims, nvec, 16)
     assert lq.launch_count() == n0
+
+
+# ---- peer-memory transport: the pack kernel stores straight into the neighbour's receive buffer -------------------
+@pytest.fixture(scope="module")
+def pg1():
+    """A one-rank nccl process group (symmetric memory needs a group to rendezvous on)."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    if dist.is_initialized():
+        yield dist.group.WORLD
+        return
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1,
+                            device_id=torch.device("cuda", 0))
+    yield dist.group.WORLD
+    dist.destroy_process_group()
+
+
+def test_peer_transport_fine_and_coarse(lq, prob8, probc, pg1):
+    """transport="peer" on one rank: the faces live in symmetric memory and the pack kernels write them through the
+    peer mapping (here the rank's own); three applications walk both halves of the double buffer."""
+    import torch
+    from paper_2111_05012_b200 import sharded as sh
+    cfg = prob8.cfg
+    U = lq.pack_gauge(to_dev(prob8.U, "f32"), cfg.dims)
+    C = lq.pack_clover(to_dev(prob8.clover, "f32"), cfg.dims)
+    try:
+        op = sh.ShardedWilsonClover(U, C, cfg.kappa, cfg.dims, cfg.bc, sh.RankGrid((1, 1, 1, 1)), part_mask=15,
+                                    transport="peer")
+    except (RuntimeError, ImportError) as e:      # no symmetric-memory support on this box
+        pytest.skip(f"symmetric memory unavailable: {e}")
+    ref = sh.ShardedWilsonClover(U, C, cfg.kappa, cfg.dims, cfg.bc, sh.RankGrid((1, 1, 1, 1)), part_mask=15)
+    rng = np.random.default_rng(77)
+    for k in range(3):
+        psi = rounded(rng.standard_normal((cfg.volume, 4, 3)) + 1j * rng.standard_normal((cfg.volume, 4, 3)), "f32")
+        x = lq.pack_spinor(to_dev(psi, "f32"), cfg.dims)
+        y, y0 = lq.empty_spinor(cfg.dims), lq.empty_spinor(cfg.dims)
+        op.apply(y, x, dagger=bool(k & 1))
+        ref.apply(y0, x, dagger=bool(k & 1))
+        torch.cuda.synchronize()
+        assert torch.equal(y, y0)                                        # same kernels, other buffers
+        got = lq.unpack_spinor(y, cfg.dims).cpu().numpy()
+        assert rel_l2(got, oracle_D(prob8, "f32", dagger=bool(k & 1), psi=psi)) <= TOL["f32"]
+    cc = probc.cfg
+    A, xc = rounded(probc.A, "f32"), rounded(probc.xc, "f32")
+    opc = sh.ShardedCoarse(to_dev(A, "f32"), cc.cdims, cc.nvec, sh.RankGrid((1, 1, 1, 1)), part_mask=15,
+                           transport="peer")
+    xd = to_dev(xc, "f32")
+    for k in range(3):
+        yc = torch.empty_like(xd)
+        opc.apply(yc, xd)
+        torch.cuda.synchronize()
+        assert rel_l2(yc.cpu().numpy(), oracle.coarse_mult(xc, A, cc.cdims)) <= TOL["f32"]
