@@ -516,6 +516,17 @@ def wilson_clover_mult_interior(out, inp, U, clover, kappa, dims, bc, part_mask,
     return out
 
 
+def wilson_clover_residual_interior(r, b, x, U, clover, kappa, dims, bc, part_mask, links12=False, stream=None):
+    """Sharded residual, interior pass: r = b - (D without the leaving hops) x; complete it with
+    wilson_clover_halo_add(r, recv, U, -kappa, ...)."""
+    sfx = _same_dtype(r, b, x, U, clover)
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    _check(getattr(lib(), f"lqcd_wilson_clover_residual_interior_{sfx}")(
+        _dev_ptr(r), _dev_ptr(b), _dev_ptr(x), _dev_ptr(U), _dev_ptr(clover), k, _i4(dims), _i4(bc), int(part_mask),
+        LINKS_12 if links12 else 0, _stream(stream)), "lqcd_wilson_clover_residual_interior")
+    return r
+
+
 def wilson_clover_halo_add(out, recv, U, kappa, dims, face_phase, part_mask, dagger=False, links12=False,
                            stream=None):
     """Sharded D, step 3: out -= kappa * (the hops served by the received faces recv[8])."""

@@ -247,8 +247,9 @@ static int halo_add_call(T* out, const T* const recv[8], const T* U, T kappa, co
 }
 
 template <typename T>
-int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4],
-                                const int bc[4], unsigned part_mask, unsigned flags, void* stream, const char* what);
+int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa,
+                                const int dims[4], const int bc[4], unsigned part_mask, unsigned flags, void* stream,
+                                const char* what);
 
 }  // namespace lqcd
 
@@ -272,14 +273,36 @@ int lqcd_wilson_clover_halo_pack_f64(double* const send[8], const double* in, co
 int lqcd_wilson_clover_mult_interior_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
                                          const int dims[4], const int bc[4], unsigned part_mask, unsigned flags,
                                          void* stream) {
-    return wilson_clover_interior_call<float>(out, in, U, clover, kappa, dims, bc, part_mask, flags, stream,
+    return wilson_clover_interior_call<float>(out, in, U, clover, nullptr, kappa, dims, bc, part_mask, flags, stream,
                                               "lqcd_wilson_clover_mult_interior_f32");
 }
 int lqcd_wilson_clover_mult_interior_f64(double* out, const double* in, const double* U, const double* clover,
                                          double kappa, const int dims[4], const int bc[4], unsigned part_mask,
                                          unsigned flags, void* stream) {
-    return wilson_clover_interior_call<double>(out, in, U, clover, kappa, dims, bc, part_mask, flags, stream,
+    return wilson_clover_interior_call<double>(out, in, U, clover, nullptr, kappa, dims, bc, part_mask, flags, stream,
                                                "lqcd_wilson_clover_mult_interior_f64");
+}
+int lqcd_wilson_clover_residual_interior_f32(float* r, const float* b, const float* x, const float* U,
+                                             const float* clover, float kappa, const int dims[4], const int bc[4],
+                                             unsigned part_mask, unsigned flags, void* stream) {
+    if (!b) {
+        clear_error();
+        set_error("lqcd_wilson_clover_residual_interior_f32: null rhs");
+        return LQCD_EINVAL;
+    }
+    return wilson_clover_interior_call<float>(r, x, U, clover, b, kappa, dims, bc, part_mask, flags, stream,
+                                              "lqcd_wilson_clover_residual_interior_f32");
+}
+int lqcd_wilson_clover_residual_interior_f64(double* r, const double* b, const double* x, const double* U,
+                                             const double* clover, double kappa, const int dims[4], const int bc[4],
+                                             unsigned part_mask, unsigned flags, void* stream) {
+    if (!b) {
+        clear_error();
+        set_error("lqcd_wilson_clover_residual_interior_f64: null rhs");
+        return LQCD_EINVAL;
+    }
+    return wilson_clover_interior_call<double>(r, x, U, clover, b, kappa, dims, bc, part_mask, flags, stream,
+                                               "lqcd_wilson_clover_residual_interior_f64");
 }
 int lqcd_wilson_clover_halo_add_f32(float* out, const float* const recv[8], const float* U, float kappa,
                                     const int dims[4], const int face_phase[8], unsigned part_mask, unsigned flags,

@@ -350,9 +350,11 @@ int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T
 // The interior pass of the sharded operator (halo.cu): D on the LOCAL lattice with every hop that leaves it in a
 // partitioned direction (bit mu of part_mask) switched off -- the D_SAP kernel with the local lattice as its one
 // domain and the cut forced in those directions; the other directions wrap with bc[mu] as in D.
+// rhs != NULL: the residual form out = rhs - (that operator) in.
 template <typename T>
-int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4],
-                                const int bc[4], unsigned part_mask, unsigned flags, void* stream, const char* what) {
+int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa,
+                                const int dims[4], const int bc[4], unsigned part_mask, unsigned flags, void* stream,
+                                const char* what) {
     clear_error();
     if (!out || !in || !U || !clover || check_dims(dims) || !bc) {
         set_error("%s: null pointer or non-positive dim", what);
@@ -364,6 +366,10 @@ int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover
     }
     if ((flags & ~(LQCD_DAGGER | LQCD_LINKS_12)) || part_mask > 15u) {
         set_error("%s: bad flags 0x%x or part_mask 0x%x", what, flags, part_mask);
+        return LQCD_EINVAL;
+    }
+    if (rhs && (!aligned16(rhs) || (flags & LQCD_DAGGER) || rhs == out)) {
+        set_error("%s: the residual form needs an aligned rhs distinct from out and does not take LQCD_DAGGER", what);
         return LQCD_EINVAL;
     }
     if (volume(dims) > 0x7fffffffLL) {
@@ -381,27 +387,30 @@ int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover
     const bool dag = flags & LQCD_DAGGER, l12 = flags & LQCD_LINKS_12;
     cudaStream_t st = (cudaStream_t)stream;
     const unsigned grid = (unsigned)ntiles;
-#define LAUNCH_I(DAG, L12)                                                                                   \
+#define LAUNCH_I(DAG, L12, RES)                                                                              \
     do {                                                                                                     \
         if (threads <= 128)                                                                                  \
-            k_wilson_clover<T, DAG, L12, 1, false, 128, (sizeof(T) == 4 ? 4 : 3)>                            \
-                <<<grid, threads, 0, st>>>(out, in, U, clover, nullptr, kappa, P);                           \
+            k_wilson_clover<T, DAG, L12, 1, RES, 128, (sizeof(T) == 4 ? 4 : 3)>                              \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);                               \
         else                                                                                                 \
-            k_wilson_clover<T, DAG, L12, 1, false, 256, (sizeof(T) == 4 ? 2 : 1)>                            \
-                <<<grid, threads, 0, st>>>(out, in, U, clover, nullptr, kappa, P);                           \
+            k_wilson_clover<T, DAG, L12, 1, RES, 256, (sizeof(T) == 4 ? 2 : 1)>                              \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);                               \
     } while (0)
-    if (dag && l12) LAUNCH_I(true, true);
-    else if (dag) LAUNCH_I(true, false);
-    else if (l12) LAUNCH_I(false, true);
-    else LAUNCH_I(false, false);
+    if (rhs && l12) LAUNCH_I(false, true, true);
+    else if (rhs) LAUNCH_I(false, false, true);
+    else if (dag && l12) LAUNCH_I(true, true, false);
+    else if (dag) LAUNCH_I(true, false, false);
+    else if (l12) LAUNCH_I(false, true, false);
+    else LAUNCH_I(false, false, false);
 #undef LAUNCH_I
     count_launch();
     return check_launch(what);
 }
-template int wilson_clover_interior_call<float>(float*, const float*, const float*, const float*, float, const int*,
-                                                const int*, unsigned, unsigned, void*, const char*);
-template int wilson_clover_interior_call<double>(double*, const double*, const double*, const double*, double,
-                                                 const int*, const int*, unsigned, unsigned, void*, const char*);
+template int wilson_clover_interior_call<float>(float*, const float*, const float*, const float*, const float*, float,
+                                                const int*, const int*, unsigned, unsigned, void*, const char*);
+template int wilson_clover_interior_call<double>(double*, const double*, const double*, const double*, const double*,
+                                                 double, const int*, const int*, unsigned, unsigned, void*,
+                                                 const char*);
 
 template int wilson_clover_call<float>(float*, const float*, const float*, const float*, const float*, float,
                                        const int*, const int*, const int*, unsigned, void*, const char*);

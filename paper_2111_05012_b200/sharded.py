@@ -11,7 +11,8 @@ import numpy as np
 import torch
 
 from . import (coarse_halo_add, coarse_halo_buffers, coarse_halo_pack, coarse_mult_interior, halo_buffers,
-               wilson_clover_halo_add, wilson_clover_halo_pack, wilson_clover_mult_interior)
+               mr_domain_solve, mr_workspace, wilson_clover_halo_add, wilson_clover_halo_pack,
+               wilson_clover_mult_interior, wilson_clover_residual_interior)
 
 
 class RankGrid:
@@ -198,11 +199,12 @@ class ShardedWilsonClover:
     """
 
     def __init__(self, U, clover, kappa, dims, bc, grid: RankGrid, links12=False, part_mask=None, group=None,
-                 transport="p2p"):
+                 transport="p2p", exchange=None):
         """transport: "p2p" = pack into local buffers, torch.distributed send/recv; "peer" = the pack kernel stores
         straight into the neighbours' receive buffers over NVLink peer memory (PeerFaces)."""
         self.U, self.clover, self.kappa = U, clover, float(kappa)
         self.dims, self.bc, self.grid, self.links12, self.group = tuple(dims), tuple(bc), grid, links12, group
+        self.exchange = exchange_faces if exchange is None else exchange   # (send, recv, grid, mask, group) -> got
         self.mask = grid.part_mask if part_mask is None else int(part_mask)
         if grid.part_mask & ~self.mask:
             raise ValueError("part_mask must include every direction the rank grid splits")
@@ -220,7 +222,7 @@ class ShardedWilsonClover:
         elif transport != "p2p":
             raise ValueError(f"transport {transport!r}")
 
-    def apply(self, out, inp, dagger=False):
+    def _run(self, out, inp, dagger, rhs):
         cur = torch.cuda.current_stream(self.U.device)
         send, got = (self.send, None) if self.peer is None else self.peer.next()
         wilson_clover_halo_pack(send, inp, self.U, self.dims, self.mask, dagger, self.links12, stream=cur)
@@ -228,24 +230,88 @@ class ShardedWilsonClover:
         with torch.cuda.stream(self.comm):           # the exchange overlaps the interior pass
             self.comm.wait_event(packed)
             if self.peer is None:
-                got = exchange_faces(self.send, self.recv, self.grid, self.mask, self.group)
+                got = self.exchange(self.send, self.recv, self.grid, self.mask, self.group)
             else:
                 self.peer.arrive()
             arrived = self.comm.record_event()
-        wilson_clover_mult_interior(out, inp, self.U, self.clover, self.kappa, self.dims, self.bc, self.mask, dagger,
-                                    self.links12, stream=cur)
+        if rhs is None:
+            wilson_clover_mult_interior(out, inp, self.U, self.clover, self.kappa, self.dims, self.bc, self.mask,
+                                        dagger, self.links12, stream=cur)
+        else:
+            wilson_clover_residual_interior(out, rhs, inp, self.U, self.clover, self.kappa, self.dims, self.bc,
+                                            self.mask, self.links12, stream=cur)
         cur.wait_event(arrived)
-        wilson_clover_halo_add(out, got, self.U, self.kappa, self.dims, self.phase, self.mask, dagger, self.links12,
-                               stream=cur)
+        # the residual carries -D: the faces enter with the opposite sign
+        wilson_clover_halo_add(out, got, self.U, self.kappa if rhs is None else -self.kappa, self.dims, self.phase,
+                               self.mask, dagger, self.links12, stream=cur)
         return out
+
+    def apply(self, out, inp, dagger=False):
+        """out = D inp (or D^dag inp)."""
+        return self._run(out, inp, dagger, None)
+
+    def residual(self, r, b, x):
+        """r = b - D x; r must not alias b or x."""
+        return self._run(r, x, False, b)
+
+
+class ShardedSAP:
+    """The SAP smoother with fixed iterations (lqcd_sap, Q17) on a lattice split over
+    ranks: the domain solves M_SAP^(e/o) are local -- "D_SAP needs no communication", PAPER.md:125 -- and only the
+    residual r = b - D x between the half sweeps exchanges halos.  Same sequence of kernels as lqcd_sap on one GPU.
+
+    The even/odd colouring of the domains is that of the GLOBAL lattice: a rank whose corner sits at an odd domain
+    coordinate sum swaps the two groups.  Every partitioned direction must hold at least two domains per rank (a
+    single domain would be joined to itself around the local lattice)."""
+
+    def __init__(self, op: ShardedWilsonClover, domain, n_sap=4, n_mr=6):
+        self.op, self.domain, self.n_sap, self.n_mr = op, tuple(int(d) for d in domain), int(n_sap), int(n_mr)
+        self.flip = domain_parity_flip(op.grid, op.dims, self.domain, op.mask)
+        self.ws = mr_workspace(op.dims, self.domain, dtype=op.U.dtype, device=op.U.device)
+
+    def apply(self, x, r, b, initial_guess=False, final_residual=True):
+        """x = SAP_n(b) (or x + SAP_n(b - D x) with initial_guess); r: scratch, receives b - D x."""
+        op = self.op
+        if initial_guess:
+            op.residual(r, b, x)
+            res = r
+        else:
+            x.zero_()
+            res = b
+            if self.n_sap == 0 and final_residual:
+                r.copy_(b)
+        for i in range(self.n_sap):
+            for g in (0, 1):
+                mr_domain_solve(x, res, op.U, op.clover, op.kappa, op.dims, op.bc, self.domain,
+                                parity=1 + (g ^ self.flip), niter=self.n_mr, accumulate=True, ws=self.ws)
+                if i == self.n_sap - 1 and g == 1 and not final_residual:
+                    break
+                op.residual(r, b, x)
+                res = r
+        return x
+
+
+def domain_parity_flip(grid: RankGrid, dims, domain, part_mask=None) -> int:
+    """1 if this rank's local even domains are the global odd ones (its corner has an odd domain-coordinate sum)."""
+    mask = grid.part_mask if part_mask is None else part_mask
+    off = 0
+    for mu in range(4):
+        if dims[mu] % domain[mu]:
+            raise ValueError(f"domain extent {domain[mu]} does not divide the local extent {dims[mu]}")
+        n = dims[mu] // domain[mu]
+        if (mask >> mu) & 1 and n < 2:
+            raise ValueError(f"direction {mu} is partitioned but holds only {n} domain per rank")
+        off += grid.coords[mu] * n
+    return off & 1
 
 
 class ShardedCoarse:
     """D_c (or its dagger) on this rank's part of a coarse lattice split over `grid`; A: the blocks of the local sites.
     cdims = the LOCAL coarse extents.  No boundary phases: bc lives inside A."""
 
-    def __init__(self, A, cdims, nvec, grid: RankGrid, part_mask=None, group=None, transport="p2p"):
+    def __init__(self, A, cdims, nvec, grid: RankGrid, part_mask=None, group=None, transport="p2p", exchange=None):
         self.A, self.cdims, self.nvec, self.grid, self.group = A, tuple(cdims), int(nvec), grid, group
+        self.exchange = exchange_faces if exchange is None else exchange
         self.mask = grid.part_mask if part_mask is None else int(part_mask)
         if grid.part_mask & ~self.mask:
             raise ValueError("part_mask must include every direction the rank grid splits")
@@ -270,7 +336,7 @@ class ShardedCoarse:
         with torch.cuda.stream(self.comm):
             self.comm.wait_event(packed)
             if self.peer is None:
-                got = exchange_faces(self.send, self.recv, self.grid, self.mask, self.group)
+                got = self.exchange(self.send, self.recv, self.grid, self.mask, self.group)
             else:
                 self.peer.arrive()
             arrived = self.comm.record_event()

@@ -325,3 +325,152 @@ def test_peer_transport_fine_and_coarse(lq, prob8, probc, pg1):
         opc.apply(yc, xd)
         torch.cuda.synchronize()
         assert rel_l2(yc.cpu().numpy(), oracle.coarse_mult(xc, A, cc.cdims)) <= TOL["f32"]
+
+
+# ---- the residual and the SAP smoother on a sharded lattice ---------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("links12", [False, True])
+def test_sharded_residual_matches_global_oracle(lq, prob8, prec, links12):
+    """r = b - D x rank by rank: interior pass in residual form, faces added with -kappa."""
+    from paper_2111_05012_b200 import sharded as sh
+    cfg = prob8.cfg
+    rng = np.random.default_rng(3)
+    b = rounded(rng.standard_normal((cfg.volume, 4, 3)) + 1j * rng.standard_normal((cfg.volume, 4, 3)), prec)
+    x = rounded(prob8.psi[0], prec)
+    want = b - oracle.wilson_clover_mult(x, rounded(prob8.U, prec), rounded(prob8.clover, prec), cfg.kappa, cfg.dims,
+                                         cfg.bc)
+    for ranks, mask in [((2, 1, 3, 2), None), ((1, 1, 1, 1), 15)]:
+        grids = [sh.RankGrid(ranks, r) for r in range(int(np.prod(ranks)))]
+        mask = grids[0].part_mask if mask is None else mask
+        ld = grids[0].local_dims(cfg.dims)
+        loc = []
+        for g in grids:
+            U = lq.pack_gauge(to_dev(sh.split_field(prob8.U, cfg.dims, g, site_axis=1), prec), ld, links12=links12)
+            C = lq.pack_clover(to_dev(sh.split_field(prob8.clover, cfg.dims, g), prec), ld)
+            xl = lq.pack_spinor(to_dev(sh.split_field(x, cfg.dims, g), prec), ld)
+            bl = lq.pack_spinor(to_dev(sh.split_field(b, cfg.dims, g), prec), ld)
+            send = lq.halo_buffers(ld, mask, dtype=xl.dtype)
+            lq.wilson_clover_halo_pack(send, xl, U, ld, mask, links12=links12)
+            loc.append((U, C, xl, bl, send))
+        recvs = sh.route_faces([l[4] for l in loc], ranks, mask)
+        parts = []
+        for g, (U, C, xl, bl, _), recv in zip(grids, loc, recvs):
+            r = lq.empty_spinor(ld, dtype=xl.dtype)
+            lq.wilson_clover_residual_interior(r, bl, xl, U, C, cfg.kappa, ld, cfg.bc, mask, links12=links12)
+            lq.wilson_clover_halo_add(r, recv, U, -cfg.kappa, ld, g.face_phase(cfg.bc, mask), mask, links12=links12)
+            parts.append(lq.unpack_spinor(r, ld).cpu().numpy())
+        got = sh.join_field(parts, cfg.dims, ranks)
+        assert np.linalg.norm(got - want) / np.linalg.norm(b) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_sharded_sap_one_rank_self_exchange(lq, prec):
+    """ShardedSAP with every direction partitioned on one rank is lqcd_sap: against the oracle's SAP."""
+    import torch
+    from paper_2111_05012_b200 import sharded as sh
+    cfg = custom_config((8, 4, 4, 8), (2, 2, 2, 2), 1, bc=(1, 1, 1, -1), seed=31)
+    prob = make_problem(cfg, n_rhs=2, coarse="none")
+    U = lq.pack_gauge(to_dev(prob.U, prec), cfg.dims)
+    C = lq.pack_clover(to_dev(prob.clover, prec), cfg.dims)
+    b, x0 = rounded(prob.psi[0], prec), 0.1 * rounded(prob.psi[1], prec)
+    op = sh.ShardedWilsonClover(U, C, cfg.kappa, cfg.dims, cfg.bc, sh.RankGrid((1, 1, 1, 1)), part_mask=15)
+    sap = sh.ShardedSAP(op, cfg.block, n_sap=3, n_mr=4)
+    bd = lq.pack_spinor(to_dev(b, prec), cfg.dims)
+    x, r = lq.empty_spinor(cfg.dims, dtype=bd.dtype), lq.empty_spinor(cfg.dims, dtype=bd.dtype)
+    sap.apply(x, r, bd)
+    torch.cuda.synchronize()
+    rx, rr = oracle.sap(b, rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa, cfg.dims, cfg.bc, cfg.block,
+                        n_sap=3, n_mr=4)
+    bar = 2 * 3 * 5 * TOL[prec]
+    assert rel_l2(lq.unpack_spinor(x, cfg.dims).cpu().numpy(), rx) <= bar
+    assert np.linalg.norm(lq.unpack_spinor(r, cfg.dims).cpu().numpy() - rr) / np.linalg.norm(b) <= bar
+    # with an initial guess: x0 + SAP(b - D x0)
+    r0 = b - oracle.wilson_clover_mult(x0, rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa, cfg.dims,
+                                       cfg.bc)
+    sx, _ = oracle.sap(r0, rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa, cfg.dims, cfg.bc, cfg.block,
+                       n_sap=3, n_mr=4)
+    x = lq.pack_spinor(to_dev(x0, prec), cfg.dims)
+    sap.apply(x, r, bd, initial_guess=True, final_residual=False)
+    torch.cuda.synchronize()
+    assert rel_l2(lq.unpack_spinor(x, cfg.dims).cpu().numpy(), x0 + sx) <= bar
+
+
+class ThreadCluster:
+    """Virtual ranks as host threads of this process on one GPU: the exchange hook of the Sharded* classes meets at a
+    host barrier (after a device synchronize: every rank's pack is complete) and hands each rank a COPY of the faces
+    its neighbours packed.  Host threads wait, kernels never do."""
+
+    def __init__(self, n):
+        import threading
+        self.n, self.barrier, self.board = n, threading.Barrier(n), [None] * n
+
+    def exchange(self, send, recv, grid, mask, group=None):
+        import torch
+        from paper_2111_05012_b200 import sharded as sh
+        torch.cuda.synchronize()
+        self.board[grid.rank] = send
+        self.barrier.wait()
+        got = [None] * 8
+        for mu in range(4):
+            if (mask >> mu) & 1:
+                got[2 * mu] = self.board[grid.neighbour(mu, -1)][2 * mu + 1].clone()
+                got[2 * mu + 1] = self.board[grid.neighbour(mu, +1)][2 * mu].clone()
+        torch.cuda.synchronize()
+        self.barrier.wait()           # nobody repacks before everybody has its copies
+        return got
+
+    def run(self, fn):
+        import threading
+        err, out = [], [None] * self.n
+
+        def body(r):
+            try:
+                out[r] = fn(r)
+            except BaseException as e:   # noqa: BLE001  (release the others, then report)
+                err.append(e)
+                self.barrier.abort()
+
+        ts = [threading.Thread(target=body, args=(r,)) for r in range(self.n)]
+        for t in ts:
+            t.start()
+        for t in ts:
+            t.join(timeout=300)
+        if err:
+            raise err[0]
+        return out
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_sharded_sap_four_ranks_lockstep(lq, prec):
+    """SAP on a 4 x 4 x 12 x 8 lattice over a 1 x 1 x 2 x 2 grid of (thread) ranks against the oracle's SAP on the
+    global lattice.  Three 2^4 domains per rank in z: the ranks with z coordinate 1 see the global colouring flipped."""
+    import torch
+    from paper_2111_05012_b200 import sharded as sh
+    ranks, dom = (1, 1, 2, 2), (2, 2, 2, 2)
+    cfg = custom_config((4, 4, 12, 8), dom, 1, bc=(1, 1, -1, -1), seed=41)
+    prob = make_problem(cfg, coarse="none")
+    b = rounded(prob.psi[0], prec)
+    rx, rr = oracle.sap(b, rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa, cfg.dims, cfg.bc, dom,
+                        n_sap=2, n_mr=3)
+    cluster = ThreadCluster(4)
+    assert [sh.domain_parity_flip(sh.RankGrid(ranks, r), (4, 4, 6, 4), dom) for r in range(4)] == [0, 1, 0, 1]
+
+    def rank_main(rk):
+        torch.cuda.set_device(0)
+        g = sh.RankGrid(ranks, rk)
+        ld = g.local_dims(cfg.dims)
+        U = lq.pack_gauge(to_dev(sh.split_field(prob.U, cfg.dims, g, site_axis=1), prec), ld)
+        C = lq.pack_clover(to_dev(sh.split_field(prob.clover, cfg.dims, g), prec), ld)
+        bl = lq.pack_spinor(to_dev(sh.split_field(b, cfg.dims, g), prec), ld)
+        op = sh.ShardedWilsonClover(U, C, cfg.kappa, ld, cfg.bc, g, exchange=cluster.exchange)
+        x, r = lq.empty_spinor(ld, dtype=bl.dtype), lq.empty_spinor(ld, dtype=bl.dtype)
+        sh.ShardedSAP(op, dom, n_sap=2, n_mr=3).apply(x, r, bl)
+        torch.cuda.synchronize()
+        return lq.unpack_spinor(x, ld).cpu().numpy(), lq.unpack_spinor(r, ld).cpu().numpy()
+
+    out = cluster.run(rank_main)
+    gx = sh.join_field([o[0] for o in out], cfg.dims, ranks)
+    gr = sh.join_field([o[1] for o in out], cfg.dims, ranks)
+    bar = 2 * 2 * 4 * TOL[prec]
+    assert rel_l2(gx, rx) <= bar
+    assert np.linalg.norm(gr - rr) / np.linalg.norm(b) <= bar
