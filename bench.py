@@ -348,6 +348,9 @@ class Workload:
     def sharded_self(self, i):
         self.sharded_op.apply(self.y[i], self.x[i])
 
+    def sharded_sap(self, i):
+        self.sharded_op.apply(self.y[i], self.z[i], self.x[i])
+
     def sharded_self_coarse(self, i):
         self.sharded_op.apply(self.yc[i], self.xc[i])
 
@@ -755,6 +758,12 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
                        "halo_bytes_sent": 2 * 4 * sum(W.lq.coarse_halo_face_reals(cfg.cdims, cfg.nvec, mu)
                                                       for mu in range(4) if (mask >> mu) & 1), "launches": 3}
         extra["coarse_mult_sharded_selfhalo"] = sc
+        # the smoother on a sharded lattice (t partitioned): local domain solves, halo exchange in the residuals only
+        W.sharded_op = sh.ShardedSAP(sh.ShardedWilsonClover(W.U18, W.clover, cfg.kappa, cfg.dims, cfg.bc, one,
+                                                            part_mask=8), cfg.block, n_sap=4, n_mr=6)
+        t = time_single(W, "sharded_sap", reps=5, warmup=1)
+        extra["sap_4_6_sharded_selfhalo_t"] = {"us": t * 1e6, "overhead_vs_sap_4_6": t * 1e6 / extra["sap_4_6"]["us"],
+                                               "launches": 8 + 8 * 3}
         del W.sharded_op
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
