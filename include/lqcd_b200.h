@@ -430,6 +430,23 @@ int lqcd_coarse_halo_add_f32(float* out, const float* const recv[8], const float
 int lqcd_coarse_halo_add_f64(double* out, const double* const recv[8], const double* A, const int cdims[4], int nvec,
                              unsigned part_mask, unsigned flags, void* stream);
 
+/* The coarse solver (1b) on a sharded coarse lattice: the same BiCGStab recurrences (same kernels, scalars resident
+ * on the device) with the two things that cross ranks supplied by the caller as plain C callbacks:
+ *   apply (out, in, stream, user): out = D_c in on this rank's part (pack -> interior -> add above); device pointers
+ *          to vectors of the local coarse lattice cdims[4]; must enqueue on `stream` (or order itself after it);
+ *   reduce(reals, count, real_bytes, stream, user): sum the device array reals[count] element by element over all
+ *          ranks, in place, ordered on `stream` (an NCCL all-reduce); NULL = single rank.  The array holds the
+ *          per-CTA partial sums of one dot product; every rank then adds them in the same fixed order, so all ranks
+ *          hold bit-identical scalars.
+ * Both return 0 on success.  ws_dev: lqcd_coarse_bicgstab_workspace_bytes(cdims, nvec, real_bytes).  x, b, r_out as
+ * for lqcd_coarse_bicgstab; a local extent of 1 is allowed. */
+typedef int (*lqcd_apply_fn)(void* out_dev, const void* in_dev, void* stream, void* user);
+typedef int (*lqcd_reduce_fn)(void* reals_dev, size_t count, int real_bytes, void* stream, void* user);
+int lqcd_coarse_bicgstab_hooks_f32(float* x, float* r_out, const float* b, const int cdims[4], int nvec, int niter,
+                                   lqcd_apply_fn apply, lqcd_reduce_fn reduce, void* user, void* ws_dev, void* stream);
+int lqcd_coarse_bicgstab_hooks_f64(double* x, double* r_out, const double* b, const int cdims[4], int nvec, int niter,
+                                   lqcd_apply_fn apply, lqcd_reduce_fn reduce, void* user, void* ws_dev, void* stream);
+
 /* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
  * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned

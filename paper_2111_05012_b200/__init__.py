@@ -479,6 +479,66 @@ def sap_mrhs(x, r, b, U, clover, kappa, dims, bc, domain, n_sap=4, n_mr=6, initi
     return x
 
 # ---- end-to-end calls on host vectors (fp32) --------------------------------------------------------------
+class DevPtr:
+    """A raw device pointer standing in for a real tensor in this module's calls: what the library's callbacks hand
+    back (lqcd_apply_fn).  dtype: torch.float32 / torch.float64."""
+
+    is_cuda = True
+
+    def __init__(self, ptr, dtype):
+        self._ptr, self.dtype = int(ptr), dtype
+
+    def data_ptr(self):
+        return self._ptr
+
+    def is_contiguous(self):
+        return True
+
+    def is_complex(self):
+        return False
+
+
+def coarse_bicgstab_hooks(x, b, cdims, nvec, niter, apply, reduce=None, r_out=None, ws=None, stream=None):
+    """The coarse solver with the operator and the cross-rank sum supplied by the caller (sharded lattice):
+    apply(out: DevPtr, inp: DevPtr) enqueues out = D_c inp on the current stream; reduce(t: Tensor) sums the real
+    tensor t over the ranks in place (None: single rank).  The BiCGStab recurrences run in the library's kernels."""
+    sfx = _same_dtype(x, b)
+    rdt = _rdtype(sfx)
+    if ws is None:
+        nb = int(lib().lqcd_coarse_bicgstab_workspace_bytes(_i4(cdims), int(nvec), 4 if sfx == "f32" else 8))
+        ws = torch.empty(nb, dtype=torch.uint8, device=x.device)
+    st = _stream(stream)
+    failure = []
+
+    def _apply(out_p, in_p, stream_p, _user):
+        try:
+            if (stream_p or 0) != (st.value or 0):
+                raise RuntimeError("apply hook called on a foreign stream")
+            apply(DevPtr(out_p, rdt), DevPtr(in_p, rdt))
+            return 0
+        except BaseException as e:  # noqa: BLE001 -- must not propagate through the C frame
+            failure.append(e)
+            return 1
+
+    def _reduce(ptr, count, real_bytes, stream_p, _user):
+        try:
+            off = int(ptr) - ws.data_ptr()
+            reduce(ws[off:off + int(count) * int(real_bytes)].view(rdt))
+            return 0
+        except BaseException as e:  # noqa: BLE001
+            failure.append(e)
+            return 1
+
+    a_fn = _lib.APPLY_FN(_apply)
+    r_fn = _lib.REDUCE_FN(_reduce) if reduce is not None else C.cast(None, _lib.REDUCE_FN)
+    rc = getattr(lib(), f"lqcd_coarse_bicgstab_hooks_{sfx}")(_dev_ptr(x), _ws_ptr(r_out), _dev_ptr(b), _i4(cdims),
+                                                            int(nvec), int(niter), a_fn, r_fn, None, _dev_ptr(ws), st)
+    if failure:
+        raise failure[0]
+    _check(rc, "lqcd_coarse_bicgstab_hooks")
+    return x
+
+
 def halo_face_reals(dims, mu) -> int:
     return int(lib().lqcd_halo_face_reals(_i4(dims), int(mu)))
 

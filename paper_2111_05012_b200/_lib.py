@@ -16,6 +16,8 @@ _vp, _ci, _cu, _cf, _cd = C.c_void_p, C.c_int, C.c_uint, C.c_float, C.c_double
 _i4 = C.POINTER(C.c_int)
 _i8 = C.POINTER(C.c_int)       # int[8]
 _p8 = C.POINTER(C.c_void_p)    # void*[8]: host array of device pointers
+APPLY_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p)             # lqcd_apply_fn
+REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_size_t, C.c_int, C.c_void_p, C.c_void_p)   # lqcd_reduce_fn
 
 # name -> (restype, argtypes); every symbol include/lqcd_b200.h declares
 SIGNATURES = {
@@ -72,6 +74,7 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
                                            _vp]),
         f"lqcd_sap_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _ci, _cu, _vp, _vp]),
         f"lqcd_sap_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _ci, _cu, _vp, _vp]),
+        f"lqcd_coarse_bicgstab_hooks_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _ci, APPLY_FN, REDUCE_FN, _vp, _vp, _vp]),
         f"lqcd_coarse_halo_pack_{_p}": (_ci, [_p8, _vp, _i4, _ci, _cu, _vp]),
         f"lqcd_coarse_mult_interior_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _cu, _vp]),
         f"lqcd_coarse_halo_add_{_p}": (_ci, [_vp, _p8, _vp, _i4, _ci, _cu, _cu, _vp]),

@@ -262,10 +262,19 @@ int coarse_mult_any<double>(double* out, const double* in, const double* A, cons
 
 // x_k = niter BiCGStab iterations for D_c x_k = b_k from x_k = 0 (PAPER.md:71 with M = 1), k = 0 .. K-1: K independent
 // recurrences (own scalars each) that share the applications of D_c; r_out may be NULL
+// Hooks (sharded solve, lqcd_coarse_bicgstab_hooks): `apply` replaces the application of D_c (A may then be NULL),
+// `reduce` sums an array of per-CTA partial sums element by element over the ranks, in place, stream-ordered.
+struct BicgHooks {
+    lqcd_apply_fn apply;
+    lqcd_reduce_fn reduce;
+    void* user;
+};
+
 template <typename T>
 static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims[4], int nvec, int K, int niter,
-                         void* ws, void* stream, const char* what) {
+                         void* ws, void* stream, const char* what, const BicgHooks* H = nullptr) {
     clear_error();
+    if (H && H->apply && !A) A = b;  // never read: the hook applies the operator
     if (!x || !b || !A || !ws || check_dims(cdims) || nvec < 1 || niter < 0 || K < 1 || K > 65535) {
         set_error("%s: null pointer, non-positive dim, nvec < 1, niter < 0 or nrhs outside 1..65535", what);
         return LQCD_EINVAL;
@@ -279,7 +288,7 @@ static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims
         return LQCD_EINVAL;
     }
     for (int mu = 0; mu < 4; mu++)
-        if (cdims[mu] < 2) {
+        if (cdims[mu] < 2 && !(H && H->apply)) {  // (a rank's part of a sharded lattice may be one site thick)
             set_error("%s: coarse extent < 2", what);
             return LQCD_EINVAL;
         }
@@ -289,6 +298,24 @@ static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims
     BicgWs<T> W;
     W.carve(ws, n, K);
     int rc;
+    const size_t npart = (size_t)red_ctas(K) * K * 3;
+    auto Dc = [&](T* out, const T* in) -> int {
+        if (H && H->apply) {
+            if (H->apply(out, in, stream, H->user)) {
+                set_error("%s: the apply hook failed", what);
+                return LQCD_ECUDA;
+            }
+            return LQCD_OK;
+        }
+        return coarse_mult_any<T>(out, in, A, cdims, nvec, K, stream);
+    };
+    auto allreduce = [&](T* part) -> int {  // the partial sums of every rank, element by element
+        if (H && H->reduce && H->reduce(part, npart, (int)sizeof(T), stream, H->user)) {
+            set_error("%s: the reduce hook failed", what);
+            return LQCD_ECUDA;
+        }
+        return LQCD_OK;
+    };
     if (niter == 0) {
         if (cudaMemsetAsync(x, 0, vbytes, st) != cudaSuccess) return check_launch(what);
         if (r_out && cudaMemcpyAsync(r_out, b, vbytes, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
@@ -298,19 +325,23 @@ static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims
     const dim3 grid((unsigned)red_ctas(K), (unsigned)K);
     // r := b, rt := b, p := b, x := 0 -- without copies: the first iteration reads b in their place
     k_cdot<T><<<grid, RED_THREADS, 0, st>>>(W.part_a, b, b, n);
+    if ((rc = allreduce(W.part_a))) return rc;
     k_set_rho<T><<<dim3(1, (unsigned)K), 32, 0, st>>>(W.sc, W.part_a, (int)grid.x);
     count_launch(2);
     for (int it = 0; it < niter; it++) {
         const T* p = it == 0 ? b : W.p;
         const T* r = it == 0 ? b : W.r;
-        if ((rc = coarse_mult_any<T>(W.v, p, A, cdims, nvec, K, stream))) return rc;            // v = D_c p
+        if ((rc = Dc(W.v, p))) return rc;                                                        // v = D_c p
         k_cdot<T><<<grid, RED_THREADS, 0, st>>>(W.part_a, b, W.v, n);                           // <rt|v>
+        if ((rc = allreduce(W.part_a))) return rc;
         k_bicg_s<T><<<grid, RED_THREADS, 0, st>>>(W.s, r, W.v, W.part_a, W.sc, it, n);          // s = r - alpha v
-        if ((rc = coarse_mult_any<T>(W.t, W.s, A, cdims, nvec, K, stream))) return rc;          // t = D_c s
+        if ((rc = Dc(W.t, W.s))) return rc;                                                      // t = D_c s
         k_cdot<T><<<grid, RED_THREADS, 0, st>>>(W.part_a, W.t, W.s, n);                         // <t|s>, <t|t>
+        if ((rc = allreduce(W.part_a))) return rc;
         k_bicg_xr<T><<<grid, RED_THREADS, 0, st>>>(x, W.r, p, W.s, W.t, b, W.part_a, W.part_b, W.sc, it == 0, n);
         count_launch(4);
         if (it + 1 < niter) {  // the last p is never used
+            if ((rc = allreduce(W.part_b))) return rc;
             k_bicg_p<T><<<grid, RED_THREADS, 0, st>>>(W.p, p, W.r, W.v, W.part_b, W.sc, it, n);
             count_launch();
         }
@@ -450,6 +481,29 @@ int lqcd_coarse_bicgstab_mrhs_f64(double* x, double* r_out, const double* b, con
                                   int nvec, int nrhs, int niter, void* ws_dev, void* stream) {
     return bicgstab_call<double>(x, r_out, b, A, cdims, nvec, nrhs, niter, ws_dev, stream,
                                  "lqcd_coarse_bicgstab_mrhs_f64");
+}
+int lqcd_coarse_bicgstab_hooks_f32(float* x, float* r_out, const float* b, const int cdims[4], int nvec, int niter,
+                                   lqcd_apply_fn apply, lqcd_reduce_fn reduce, void* user, void* ws_dev, void* stream) {
+    if (!apply) {
+        clear_error();
+        set_error("lqcd_coarse_bicgstab_hooks_f32: null apply hook");
+        return LQCD_EINVAL;
+    }
+    const BicgHooks H = {apply, reduce, user};
+    return bicgstab_call<float>(x, r_out, b, nullptr, cdims, nvec, 1, niter, ws_dev, stream,
+                                "lqcd_coarse_bicgstab_hooks_f32", &H);
+}
+int lqcd_coarse_bicgstab_hooks_f64(double* x, double* r_out, const double* b, const int cdims[4], int nvec, int niter,
+                                   lqcd_apply_fn apply, lqcd_reduce_fn reduce, void* user, void* ws_dev,
+                                   void* stream) {
+    if (!apply) {
+        clear_error();
+        set_error("lqcd_coarse_bicgstab_hooks_f64: null apply hook");
+        return LQCD_EINVAL;
+    }
+    const BicgHooks H = {apply, reduce, user};
+    return bicgstab_call<double>(x, r_out, b, nullptr, cdims, nvec, 1, niter, ws_dev, stream,
+                                 "lqcd_coarse_bicgstab_hooks_f64", &H);
 }
 int lqcd_coarse_bicgstab_f32(float* x, float* r_out, const float* b, const float* A, const int cdims[4], int nvec,
                              int niter, void* ws_dev, void* stream) {

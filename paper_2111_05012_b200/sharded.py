@@ -10,9 +10,9 @@ from __future__ import annotations
 import numpy as np
 import torch
 
-from . import (coarse_halo_add, coarse_halo_buffers, coarse_halo_pack, coarse_mult_interior, halo_buffers,
-               mr_domain_solve, mr_workspace, wilson_clover_halo_add, wilson_clover_halo_pack,
-               wilson_clover_mult_interior, wilson_clover_residual_interior)
+from . import (coarse_bicgstab_hooks, coarse_halo_add, coarse_halo_buffers, coarse_halo_pack, coarse_mult_interior,
+               empty_spinor, halo_buffers, mr_domain_solve, mr_workspace, prolong, restrict, wilson_clover_halo_add,
+               wilson_clover_halo_pack, wilson_clover_mult_interior, wilson_clover_residual_interior)
 
 
 class RankGrid:
@@ -344,3 +344,41 @@ class ShardedCoarse:
         cur.wait_event(arrived)
         coarse_halo_add(out, got, self.A, self.cdims, self.nvec, self.mask, dagger, stream=cur)
         return out
+
+
+def allreduce_sum(group=None):
+    """The cross-rank sum for ShardedVcycle / coarse_bicgstab_hooks: an in-place torch.distributed all-reduce (nccl:
+    ordered on the current stream), or None when there is one rank."""
+    import torch.distributed as dist
+    if not dist.is_available() or not dist.is_initialized() or dist.get_world_size(group) == 1:
+        return None
+    return lambda t: dist.all_reduce(t, group=group)
+
+
+class ShardedVcycle:
+    """x = M b, one V-cycle of the multigrid preconditioner (lqcd_mg_vcycle, Q19) on a
+    lattice split over ranks: restrict (block-local) -> fixed-iteration BiCGStab on the sharded D_c, its dot products
+    summed over the ranks (`reduce`) -> prolong (block-local) -> SAP started from that x (ShardedSAP).
+    nullvecs: the native null vectors of this rank's aggregates; the smoother's domains are the aggregates."""
+
+    def __init__(self, fine: ShardedWilsonClover, coarse: ShardedCoarse, nullvecs, block, nvec, n_coarse=8, n_sap=4,
+                 n_mr=6, reduce=None):
+        self.fine, self.coarse, self.v = fine, coarse, nullvecs
+        self.block, self.nvec, self.n_coarse = tuple(int(v) for v in block), int(nvec), int(n_coarse)
+        self.reduce = reduce
+        self.sap = ShardedSAP(fine, self.block, n_sap, n_mr)
+        cdt = torch.complex64 if fine.U.dtype == torch.float32 else torch.complex128
+        vc = int(np.prod(coarse.cdims))
+        self.bc_ = torch.empty((vc, 2, self.nvec), dtype=cdt, device=fine.U.device)
+        self.xc_ = torch.empty_like(self.bc_)
+        self.r_ = empty_spinor(fine.dims, dtype=fine.U.dtype, device=fine.U.device)
+
+    def apply(self, x, b):
+        f, c = self.fine, self.coarse
+        restrict(self.bc_, b, self.v, f.dims, self.block, self.nvec)                                     # (1a) Eq. 5
+        coarse_bicgstab_hooks(self.xc_, self.bc_, c.cdims, self.nvec, self.n_coarse,                     # (1b)
+                              apply=lambda o, i: c.apply(o, i), reduce=self.reduce)
+        prolong(x, self.xc_, self.v, f.dims, self.block, self.nvec)                                      # (1c) Eq. 6
+        if self.sap.n_sap > 0:                                                                           # (2)
+            self.sap.apply(x, self.r_, b, initial_guess=True, final_residual=False)
+        return x

@@ -474,3 +474,109 @@ def test_sharded_sap_four_ranks_lockstep(lq, prec):
     bar = 2 * 2 * 4 * TOL[prec]
     assert rel_l2(gx, rx) <= bar
     assert np.linalg.norm(gr - rr) / np.linalg.norm(b) <= bar
+
+
+# ---- the coarse solver with hooks and the whole V-cycle on a sharded lattice ------------------------------------------
+def vcycle_bar(prob, prec, n_coarse, n_sap, n_mr):
+    from test_gpu_mg import cond_coarse
+    return (2 * n_coarse * cond_coarse(prob, prec) + 2 + 2 * n_sap * (n_mr + 1)) * TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_bicgstab_hooks_equal_the_plain_solver(lq, probc, prec):
+    """With apply = the library's own D_c and no reduce, the hooked solver IS lqcd_coarse_bicgstab, bit for bit."""
+    import torch
+    cc = probc.cfg
+    A, b = to_dev(rounded(probc.A, prec), prec), to_dev(rounded(probc.xc, prec), prec)
+    x0, x1 = torch.empty_like(b), torch.empty_like(b)
+    lq.coarse_bicgstab(x0, b, A, cc.cdims, cc.nvec, 5)
+    calls = []
+
+    def apply(o, i):
+        calls.append(1)
+        lq.coarse_mult(o, i, A, cc.cdims, cc.nvec)
+
+    lq.coarse_bicgstab_hooks(x1, b, cc.cdims, cc.nvec, 5, apply)
+    torch.cuda.synchronize()
+    assert len(calls) == 10 and torch.equal(x0, x1)
+    with pytest.raises(ZeroDivisionError):          # an exception in a hook surfaces after the C call returns
+        lq.coarse_bicgstab_hooks(x1, b, cc.cdims, cc.nvec, 2, lambda o, i: 1 / 0)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_sharded_vcycle_one_rank_self_exchange(lq, prec):
+    import torch
+    from paper_2111_05012_b200 import sharded as sh
+    cfg = custom_config((8, 4, 4, 8), (2, 2, 2, 2), 3, bc=(1, 1, 1, -1), seed=51)
+    prob = make_problem(cfg)
+    one = sh.RankGrid((1, 1, 1, 1))
+    U = lq.pack_gauge(to_dev(prob.U, prec), cfg.dims)
+    C = lq.pack_clover(to_dev(prob.clover, prec), cfg.dims)
+    V = lq.pack_nullvecs(to_dev(prob.v, prec), cfg.dims, cfg.block)
+    b = rounded(prob.psi[0], prec)
+    fine = sh.ShardedWilsonClover(U, C, cfg.kappa, cfg.dims, cfg.bc, one, part_mask=15)
+    coarse = sh.ShardedCoarse(to_dev(prob.A, prec), cfg.cdims, cfg.nvec, one, part_mask=15)
+    bd = lq.pack_spinor(to_dev(b, prec), cfg.dims)
+    for n_coarse, n_sap, n_mr in ((4, 2, 3), (3, 0, 3)):
+        x = lq.empty_spinor(cfg.dims, dtype=bd.dtype)
+        sh.ShardedVcycle(fine, coarse, V, cfg.block, cfg.nvec, n_coarse, n_sap, n_mr).apply(x, bd)
+        torch.cuda.synchronize()
+        ref = oracle.mg_vcycle(b, rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa, cfg.dims, cfg.bc,
+                               cfg.block, rounded(prob.v, prec), rounded(prob.A, prec), n_coarse=n_coarse, n_sap=n_sap,
+                               n_mr=n_mr)
+        assert rel_l2(lq.unpack_spinor(x, cfg.dims).cpu().numpy(), ref) <= vcycle_bar(prob, prec, n_coarse, n_sap, n_mr)
+
+
+def cluster_reduce(cluster, rank):
+    """Sum of a tensor over the thread-ranks, in rank order, in place (the stand-in for the nccl all-reduce)."""
+    import torch
+
+    def reduce(t):
+        torch.cuda.synchronize()
+        cluster.board[rank] = t
+        cluster.barrier.wait()
+        total = cluster.board[0].clone()
+        for r in range(1, cluster.n):
+            total += cluster.board[r]
+        torch.cuda.synchronize()
+        cluster.barrier.wait()
+        t.copy_(total)
+
+    return reduce
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_sharded_vcycle_four_ranks_lockstep(lq, prec):
+    """The whole V-cycle on a 4 x 4 x 12 x 8 lattice over a 1 x 1 x 2 x 2 grid of thread-ranks (halo exchanges of D,
+    D_c and the residual, dot products summed over the ranks) against the oracle's V-cycle on the global lattice."""
+    import torch
+    from paper_2111_05012_b200 import sharded as sh
+    ranks, block = (1, 1, 2, 2), (2, 2, 2, 2)
+    cfg = custom_config((4, 4, 12, 8), block, 2, bc=(1, 1, -1, -1), seed=61)
+    prob = make_problem(cfg)
+    b = rounded(prob.psi[0], prec)
+    n_coarse, n_sap, n_mr = 4, 2, 3
+    ref = oracle.mg_vcycle(b, rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa, cfg.dims, cfg.bc, block,
+                           rounded(prob.v, prec), rounded(prob.A, prec), n_coarse=n_coarse, n_sap=n_sap, n_mr=n_mr)
+    cluster = ThreadCluster(4)
+
+    def rank_main(rk):
+        torch.cuda.set_device(0)
+        g = sh.RankGrid(ranks, rk)
+        ld, lc = g.local_dims(cfg.dims), g.local_dims(cfg.cdims)
+        U = lq.pack_gauge(to_dev(sh.split_field(prob.U, cfg.dims, g, site_axis=1), prec), ld)
+        C = lq.pack_clover(to_dev(sh.split_field(prob.clover, cfg.dims, g), prec), ld)
+        V = lq.pack_nullvecs(to_dev(sh.split_field(prob.v, cfg.dims, g, site_axis=1), prec), ld, block)
+        A = to_dev(sh.split_field(prob.A, cfg.cdims, g), prec)
+        bl = lq.pack_spinor(to_dev(sh.split_field(b, cfg.dims, g), prec), ld)
+        fine = sh.ShardedWilsonClover(U, C, cfg.kappa, ld, cfg.bc, g, exchange=cluster.exchange)
+        coarse = sh.ShardedCoarse(A, lc, cfg.nvec, g, exchange=cluster.exchange)
+        x = lq.empty_spinor(ld, dtype=bl.dtype)
+        sh.ShardedVcycle(fine, coarse, V, block, cfg.nvec, n_coarse, n_sap, n_mr,
+                         reduce=cluster_reduce(cluster, rk)).apply(x, bl)
+        torch.cuda.synchronize()
+        return lq.unpack_spinor(x, ld).cpu().numpy()
+
+    out = cluster.run(rank_main)
+    got = sh.join_field(out, cfg.dims, ranks)
+    assert rel_l2(got, ref) <= vcycle_bar(prob, prec, n_coarse, n_sap, n_mr)
