@@ -348,6 +348,9 @@ class Workload:
     def sharded_self(self, i):
         self.sharded_op.apply(self.y[i], self.x[i])
 
+    def sharded_vcycle(self, i):
+        self.sharded_op.apply(self.y[i], self.x[i])
+
     def sharded_sap(self, i):
         self.sharded_op.apply(self.y[i], self.z[i], self.x[i])
 
@@ -764,6 +767,13 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         t = time_single(W, "sharded_sap", reps=5, warmup=1)
         extra["sap_4_6_sharded_selfhalo_t"] = {"us": t * 1e6, "overhead_vs_sap_4_6": t * 1e6 / extra["sap_4_6"]["us"],
                                                "launches": 8 + 8 * 3}
+        # ... and the whole V-cycle (restrict, 8 BiCGStab iterations on the sharded D_c through the solver's hooks,
+        # prolong, sharded SAP(4, 6)); one rank: the cross-rank sum of the dot products is the identity
+        W.sharded_op = sh.ShardedVcycle(W.sharded_op.op, sh.ShardedCoarse(W.A, cfg.cdims, cfg.nvec, one, part_mask=8),
+                                        W.v, cfg.block, cfg.nvec, n_coarse=8, n_sap=4, n_mr=6)
+        t = time_single(W, "sharded_vcycle", reps=3, warmup=1)
+        extra["mg_vcycle_8_4_6_sharded_selfhalo_t"] = {
+            "us": t * 1e6, "overhead_vs_mg_vcycle_8_4_6": t * 1e6 / extra["mg_vcycle_8_4_6"]["us"]}
         del W.sharded_op
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
