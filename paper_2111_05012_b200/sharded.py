@@ -365,7 +365,8 @@ class ShardedVcycle:
                  n_mr=6, reduce=None):
         self.fine, self.coarse, self.v = fine, coarse, nullvecs
         self.block, self.nvec, self.n_coarse = tuple(int(v) for v in block), int(nvec), int(n_coarse)
-        self.reduce = reduce
+        # more than one rank and no sum given: the process group's all-reduce
+        self.reduce = allreduce_sum(fine.group) if reduce is None and fine.grid.world > 1 else reduce
         self.sap = ShardedSAP(fine, self.block, n_sap, n_mr)
         cdt = torch.complex64 if fine.U.dtype == torch.float32 else torch.complex128
         vc = int(np.prod(coarse.cdims))
