@@ -76,6 +76,10 @@ def _worker(rank, world, port, q):
                                     clover_pad.reshape(Vp, 2, 6, 6), cfg.kappa, pdims, (BC[0], BC[1], BC[2], 1))
     got = got.reshape((ld[3] + 2,) + lat[1:] + (4, 3))[1:-1].reshape(-1, 4, 3)
     err = float(np.linalg.norm(got - want) / np.linalg.norm(want))
+    # the cross-rank sum ShardedVcycle hands to the coarse solver's reduce hook
+    t = torch.tensor([rank + 1.0, 2.0], dtype=torch.float64)
+    sh.allreduce_sum()(t)
+    assert t.tolist() == [3.0, 4.0], t
     dist.barrier()
     dist.destroy_process_group()
     q.put((rank, err, ph))
