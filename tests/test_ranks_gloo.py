@@ -82,3 +82,18 @@ def test_roofline_model_matches_survey_table():
     assert m["wilson_clover"]["flops"] == 1872 * c5.volume
     assert m["coarse_mult"]["bytes"] == 295936 * c5.cvolume          # 9 N^2 8 + 2 N 8, N = 64
     assert m["restrict"]["bytes"] == 3168 * c5.volume + 512 * c5.cvolume
+
+
+def test_default_rank_grid_splits_t_z_y_first():
+    """bench.py --sharded: the x direction (one 16-byte vector per 128-byte line on its faces) is split last."""
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.default_rank_grid(1) == (1, 1, 1, 1)
+    assert bench.default_rank_grid(2) == (1, 1, 1, 2)
+    assert bench.default_rank_grid(4) == (1, 1, 2, 2)
+    assert bench.default_rank_grid(8) == (1, 2, 2, 2)
+    assert bench.default_rank_grid(16) == (2, 2, 2, 2)
+    assert bench.default_rank_grid(6) == (1, 1, 1, 6)
+    for n in (1, 2, 3, 4, 6, 8, 12, 16):
+        g = bench.default_rank_grid(n)
+        assert g[0] * g[1] * g[2] * g[3] == n
