@@ -13,6 +13,7 @@ struct Knobs {
     int mrhs_stages = 0;              // pipeline stages of coarse_mult_mrhs, 0 = as many as fit
     int fine_mrhs = 0;                // -1 = wilson_clover_mult_mrhs applies the single-right-hand-side kernel per vector
     int sap_fused = 0;                // 0 = shared-memory-resident inner-domain solver when it fits; -1 = never
+    int sap_group_residual = 0;       // 0 = SAP's intermediate residuals on the next group's domains only; -1 = all sites
 };
 extern Knobs g_knobs;
 }  // namespace lqcd

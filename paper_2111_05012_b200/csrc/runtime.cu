@@ -70,6 +70,7 @@ int lqcd_set_knob(const char* name, int value) {
     else if (!strcmp(name, "transfer_warps")) g_knobs.transfer_warps = value;
     else if (!strcmp(name, "fine_tslab")) g_knobs.fine_tslab = value;
     else if (!strcmp(name, "sap_fused")) g_knobs.sap_fused = value;
+    else if (!strcmp(name, "sap_group_residual")) g_knobs.sap_group_residual = value;
     else if (!strcmp(name, "fine_mrhs")) g_knobs.fine_mrhs = value;
     else if (!strcmp(name, "mrhs_tensor")) g_knobs.mrhs_tensor = value;
     else if (!strcmp(name, "mrhs_stages")) g_knobs.mrhs_stages = value;

@@ -31,6 +31,7 @@ struct FineParams {
     int dom[4];    // domain extents (the aggregation block)
     int multi[4];  // 1 if there is more than one domain in that direction (else no hop is ever cut)
     int parity;    // 0 = all domains, 1 = even domains only, 2 = odd domains only
+    int keep;      // with parity != 0: 1 = leave the sites of the other group untouched instead of zeroing them
 };
 
 // Which site is mine: CTA -> tile (x tiles fastest; optionally z-slabbed traversal), thread -> site in tile.  All
@@ -139,7 +140,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
             }
         }
         if (P.parity != 0 && (par & 1) != P.parity - 1) {  // my domain is not in the selected group: zero
-            store_spinor<T>(out, s, acc);
+            if (!P.keep) store_spinor<T>(out, s, acc);
             return;
         }
     }
@@ -221,6 +222,7 @@ static int fine_setup(FineParams& P, long long& ntiles_out, const int dims[4], c
         }
     }
     P.parity = (flags & LQCD_DOMAIN_EVEN) ? 1 : (flags & LQCD_DOMAIN_ODD) ? 2 : 0;
+    P.keep = 0;
     bool user_ok = g_knobs.fine_tile[0] > 0;
     for (int mu = 0; mu < 4 && user_ok; mu++) user_ok = dims[mu] % g_knobs.fine_tile[mu] == 0;
     if (user_ok)
@@ -347,6 +349,49 @@ int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T
     count_launch();
     return check_launch(what);
 }
+// r := b - D x on the domains of ONE group only (flags: LQCD_DOMAIN_EVEN / ODD), the other sites of r untouched: what
+// SAP needs between two half sweeps, where only the group solved next reads the residual (sap.cu).  The full operator
+// (no hop is cut): the even/odd kernel variant with the cut switched off, the residual epilogue and no zero fill.
+template <typename T>
+int wilson_clover_residual_group_call(T* r, const T* x, const T* U, const T* clover, const T* b, T kappa,
+                                      const int dims[4], const int bc[4], const int domain[4], unsigned flags,
+                                      void* stream, const char* what) {
+    // (arguments were validated by the caller, sap_call)
+    FineParams P;
+    long long ntiles = 0;
+    {
+        const int rc = fine_setup(P, ntiles, dims, bc, domain, flags & (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD),
+                                  (int)sizeof(T), what);
+        if (rc) return rc;
+    }
+    for (int mu = 0; mu < 4; mu++) P.multi[mu] = 0;
+    P.keep = 1;
+    const int threads = (P.tilevol + 31) / 32 * 32;
+    const bool l12 = flags & LQCD_LINKS_12;
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned grid = (unsigned)ntiles;
+#define LAUNCH_G(L12)                                                                                        \
+    do {                                                                                                     \
+        if (threads <= 128)                                                                                  \
+            k_wilson_clover<T, false, L12, 2, true, 128, (sizeof(T) == 4 ? 4 : 3)>                           \
+                <<<grid, threads, 0, st>>>(r, x, U, clover, b, kappa, P);                                    \
+        else                                                                                                 \
+            k_wilson_clover<T, false, L12, 2, true, 256, (sizeof(T) == 4 ? 2 : 1)>                           \
+                <<<grid, threads, 0, st>>>(r, x, U, clover, b, kappa, P);                                    \
+    } while (0)
+    if (l12) LAUNCH_G(true);
+    else LAUNCH_G(false);
+#undef LAUNCH_G
+    count_launch();
+    return check_launch(what);
+}
+template int wilson_clover_residual_group_call<float>(float*, const float*, const float*, const float*, const float*,
+                                                      float, const int*, const int*, const int*, unsigned, void*,
+                                                      const char*);
+template int wilson_clover_residual_group_call<double>(double*, const double*, const double*, const double*,
+                                                       const double*, double, const int*, const int*, const int*,
+                                                       unsigned, void*, const char*);
+
 // The interior pass of the sharded operator (halo.cu): D on the LOCAL lattice with every hop that leaves it in a
 // partitioned direction (bit mu of part_mask) switched off -- the D_SAP kernel with the local lattice as its one
 // domain and the cut forced in those directions; the other directions wrap with bc[mu] as in D.

@@ -310,3 +310,36 @@ def test_sap_edge_lattices(lq, prec, dims, domain, bc, path):
     bar = 2 * 3 * 5 * TOL1[prec]
     assert rel_l2(gx, rx) <= bar
     assert np.linalg.norm(gr - rr) / np.linalg.norm(b) <= bar
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,domain,bc", [
+    ((8, 8, 8, 8), (4, 4, 4, 4), (1, 1, 1, -1)),       # the resident kernel's design size (fp32)
+    ((6, 4, 2, 10), (3, 4, 1, 5), (-1, 1, -1, 1)),     # odd domain counts, a direction spanned by one domain
+    ((3, 3, 3, 3), (3, 1, 3, 1), (1, 1, 1, -1)),       # 9 domains, ragged chunk
+    ((4, 4, 4, 8), (4, 4, 4, 8), (1, 1, 1, -1)),       # one domain: the odd group is empty
+])
+def test_sap_group_residual_is_the_full_residual(lq, prec, dims, domain, bc):
+    """Between half sweeps SAP computes r = b - D x on the domains of the NEXT group only (knob sap_group_residual):
+    the same numbers where they are read -- x and the final residual are bit-identical with the all-sites form."""
+    cfg = custom_config(dims, (1, 1, 1, 1), 1, bc=bc, seed=13)
+    prob = make_problem(cfg, n_rhs=2, coarse="none")
+    d = Dev(lq, prob, prec, coarse=False)
+    b, x0 = prob.psi
+    out = {}
+    for knob in (0, -1):
+        lq.set_knob("sap_group_residual", knob)
+        try:
+            out[knob] = (gpu_sap(lq, d, b, domain, 3, 4), gpu_sap(lq, d, b, domain, 2, 3, x0=0.1 * x0),
+                         gpu_sap(lq, d, b, domain, 2, 3, final_residual=False)[0])
+        finally:
+            lq.set_knob("sap_group_residual", 0)
+    (xa, ra), (xb, rb), xc = out[0]
+    (xa1, ra1), (xb1, rb1), xc1 = out[-1]
+    assert np.array_equal(xa, xa1) and np.array_equal(ra, ra1)
+    assert np.array_equal(xb, xb1) and np.array_equal(rb, rb1)
+    assert np.array_equal(xc, xc1)
+    n0 = lq.launch_count()
+    gpu_sap(lq, d, b, domain, 3, 4)
+    # pack b, [zero-fill by memset], 6 half sweeps (one resident launch, or 1 + 2 n_mr generic ones) + 6 residuals
+    assert lq.launch_count() - n0 >= 1 + 6 + 6
