@@ -27,7 +27,8 @@ int wilson_clover_residual_group_call(T* r, const T* x, const T* U, const T* clo
                                       void* stream, const char* what);
 template <typename T>
 int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
-                            const int bc[4], int nrhs, unsigned flags, void* stream, const char* what);
+                            const int bc[4], int nrhs, unsigned flags, void* stream, const char* what,
+                            const int* domain, unsigned group);
 
 struct DomParams {
     int L[4], dom[4], Lc[4], bc[4], multi[4];
@@ -692,14 +693,15 @@ static int sap_call(T* x, T* r, const T* b, const T* U, const T* clover, T kappa
     const size_t bytes = (size_t)nreal * sizeof(T) * K;
     int rc;
     // |r_k> := |b_k> - D|x_k>; right-hand sides in pairs (links, clover read once).  Between two half sweeps only
-    // the group solved NEXT reads the residual, so a single right-hand side computes it on that group's domains alone
-    // (`next` = LQCD_DOMAIN_EVEN / ODD; about 0.6 of the traffic of the full pass); next = 0: all sites.
+    // the group solved NEXT reads the residual, so it is computed on that group's domains alone (`next` =
+    // LQCD_DOMAIN_EVEN / ODD; about 0.6 of the traffic of the full pass); next = 0: all sites.
     auto residual = [&](unsigned next) -> int {
-        if (K == 1 && next && g_knobs.sap_group_residual >= 0)
+        if (g_knobs.sap_group_residual < 0) next = 0;
+        if (K == 1 && next)
             return wilson_clover_residual_group_call<T>(r, x, U, clover, b, kappa, dims, bc, domain, next, stream,
                                                         what);
         if (K == 1) return wilson_clover_call<T>(r, x, U, clover, b, kappa, dims, bc, nullptr, 0, stream, what);
-        return wilson_clover_mrhs_call<T>(r, x, U, clover, b, kappa, dims, bc, K, 0, stream, what);
+        return wilson_clover_mrhs_call<T>(r, x, U, clover, b, kappa, dims, bc, K, 0, stream, what, domain, next);
     };
     const T* res = r;
     if (flags & LQCD_SAP_INITIAL_GUESS) {

@@ -490,6 +490,12 @@ __global__ void __launch_bounds__(128, sizeof(T) == 4 ? 3 : 2)
                          const T* __restrict__ clover, const T* __restrict__ rhs, T kappa, FineParams P) {
     int x[4], s;
     if (!fine_decode(P, x, s)) return;
+    if (P.parity != 0) {  // one group of domains only, the other sites untouched (SAP's intermediate residuals)
+        int par = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) par += P.d_dom[mu].div(x[mu]);
+        if ((par & 1) != P.parity - 1) return;
+    }
     const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
     int sf[4], sb[4];
     T pf[4], pb[4];
@@ -556,7 +562,10 @@ __global__ void __launch_bounds__(128, sizeof(T) == 4 ? 3 : 2)
 
 template <typename T>
 int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa, const int dims[4],
-                            const int bc[4], int nrhs, unsigned flags, void* stream, const char* what) {
+                            const int bc[4], int nrhs, unsigned flags, void* stream, const char* what,
+                            const int* domain, unsigned group) {
+    // domain != NULL and group = LQCD_DOMAIN_EVEN / ODD: only the sites of that group of domains are computed, the
+    // others are left as they are (internal: the residual form between SAP's half sweeps)
     clear_error();
     if (!out || !in || !U || !clover || check_dims(dims) || !bc || nrhs < 1) {
         set_error("%s: null pointer, non-positive dim or nrhs < 1", what);
@@ -578,8 +587,9 @@ int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, co
     long long ntiles = 0;
     {
         // tiles of at most 128 sites: the kernel is compiled for 128 threads
-        const int rc = fine_setup(P, ntiles, dims, bc, nullptr, flags & (LQCD_DAGGER | LQCD_LINKS_12), (int)sizeof(T), what);
+        const int rc = fine_setup(P, ntiles, dims, bc, group ? domain : nullptr, group, (int)sizeof(T), what);
         if (rc) return rc;
+        for (int mu = 0; mu < 4; mu++) P.multi[mu] = 0;  // the full operator: no hop is cut
     }
     const long long rstride = (long long)nchunks(dims) * CH * 24;
     const int threads = (P.tilevol + 31) / 32 * 32;
@@ -604,18 +614,23 @@ int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, co
         if (rc) return rc;
     }
     for (; k < nrhs; k++) {  // an odd one out (or a user tile of more than 128 sites): the single-right-hand-side kernel
-        const int rc = wilson_clover_call<T>(out + k * rstride, in + k * rstride, U, clover,
-                                             rhs ? rhs + k * rstride : nullptr, kappa, dims, bc, nullptr, flags, stream,
-                                             what);
+        const int rc = group ? wilson_clover_residual_group_call<T>(out + k * rstride, in + k * rstride, U, clover,
+                                                                    rhs + k * rstride, kappa, dims, bc, domain,
+                                                                    group | (flags & LQCD_LINKS_12), stream, what)
+                             : wilson_clover_call<T>(out + k * rstride, in + k * rstride, U, clover,
+                                                     rhs ? rhs + k * rstride : nullptr, kappa, dims, bc, nullptr,
+                                                     flags, stream, what);
         if (rc) return rc;
     }
     return LQCD_OK;
 }
 
 template int wilson_clover_mrhs_call<float>(float*, const float*, const float*, const float*, const float*, float,
-                                            const int*, const int*, int, unsigned, void*, const char*);
+                                            const int*, const int*, int, unsigned, void*, const char*, const int*,
+                                            unsigned);
 template int wilson_clover_mrhs_call<double>(double*, const double*, const double*, const double*, const double*,
-                                             double, const int*, const int*, int, unsigned, void*, const char*);
+                                             double, const int*, const int*, int, unsigned, void*, const char*,
+                                             const int*, unsigned);
 
 }  // namespace lqcd
 
@@ -680,12 +695,12 @@ extern "C" {
 int lqcd_wilson_clover_mult_mrhs_f32(float* out, const float* in, const float* U, const float* clover, float kappa,
                                      const int dims[4], const int bc[4], int nrhs, unsigned flags, void* stream) {
     return wilson_clover_mrhs_call<float>(out, in, U, clover, nullptr, kappa, dims, bc, nrhs, flags, stream,
-                                          "lqcd_wilson_clover_mult_mrhs_f32");
+                                          "lqcd_wilson_clover_mult_mrhs_f32", nullptr, 0u);
 }
 int lqcd_wilson_clover_mult_mrhs_f64(double* out, const double* in, const double* U, const double* clover,
                                      double kappa, const int dims[4], const int bc[4], int nrhs, unsigned flags,
                                      void* stream) {
     return wilson_clover_mrhs_call<double>(out, in, U, clover, nullptr, kappa, dims, bc, nrhs, flags, stream,
-                                           "lqcd_wilson_clover_mult_mrhs_f64");
+                                           "lqcd_wilson_clover_mult_mrhs_f64", nullptr, 0u);
 }
 }
