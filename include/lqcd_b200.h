@@ -392,13 +392,16 @@ int lqcd_wilson_clover_mult_interior_f64(double* out, const double* in, const do
                                          unsigned flags, void* stream);
 /* The residual r = b - D x of the sharded operator: the interior pass in residual form,
  * r = b - (D with the leaving hops off) x, then lqcd_wilson_clover_halo_add(r, recv, U, -kappa, ...) on faces packed
- * from x (the sign of kappa turns "out -= kappa hops" into "+=").  r must not alias b or x; flags: LQCD_LINKS_12. */
+ * from x (the sign of kappa turns "out -= kappa hops" into "+=").  r must not alias b or x; flags: LQCD_LINKS_12,
+ * and, with domain[4] != NULL, LQCD_DOMAIN_EVEN or LQCD_DOMAIN_ODD: only the sites of that group of domains (local
+ * colouring) are computed, the others are left as they are -- what SAP needs between two half sweeps (the halo add
+ * then also touches face sites of the other group, whose values are not read).  domain may be NULL without them. */
 int lqcd_wilson_clover_residual_interior_f32(float* r, const float* b, const float* x, const float* U,
                                              const float* clover, float kappa, const int dims[4], const int bc[4],
-                                             unsigned part_mask, unsigned flags, void* stream);
+                                             const int* domain, unsigned part_mask, unsigned flags, void* stream);
 int lqcd_wilson_clover_residual_interior_f64(double* r, const double* b, const double* x, const double* U,
                                              const double* clover, double kappa, const int dims[4], const int bc[4],
-                                             unsigned part_mask, unsigned flags, void* stream);
+                                             const int* domain, unsigned part_mask, unsigned flags, void* stream);
 int lqcd_wilson_clover_halo_add_f32(float* out, const float* const recv[8], const float* U, float kappa,
                                     const int dims[4], const int face_phase[8], unsigned part_mask, unsigned flags,
                                     void* stream);

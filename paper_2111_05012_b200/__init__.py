@@ -576,14 +576,18 @@ def wilson_clover_mult_interior(out, inp, U, clover, kappa, dims, bc, part_mask,
     return out
 
 
-def wilson_clover_residual_interior(r, b, x, U, clover, kappa, dims, bc, part_mask, links12=False, stream=None):
+def wilson_clover_residual_interior(r, b, x, U, clover, kappa, dims, bc, part_mask, links12=False, domain=None,
+                                    parity=0, stream=None):
     """Sharded residual, interior pass: r = b - (D without the leaving hops) x; complete it with
-    wilson_clover_halo_add(r, recv, U, -kappa, ...)."""
+    wilson_clover_halo_add(r, recv, U, -kappa, ...).  parity 1 / 2 with a domain: only the even / odd domains'
+    sites are computed, the others left as they are."""
     sfx = _same_dtype(r, b, x, U, clover)
     k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    flags = (LINKS_12 if links12 else 0) | {0: 0, 1: DOMAIN_EVEN, 2: DOMAIN_ODD}[parity]
     _check(getattr(lib(), f"lqcd_wilson_clover_residual_interior_{sfx}")(
-        _dev_ptr(r), _dev_ptr(b), _dev_ptr(x), _dev_ptr(U), _dev_ptr(clover), k, _i4(dims), _i4(bc), int(part_mask),
-        LINKS_12 if links12 else 0, _stream(stream)), "lqcd_wilson_clover_residual_interior")
+        _dev_ptr(r), _dev_ptr(b), _dev_ptr(x), _dev_ptr(U), _dev_ptr(clover), k, _i4(dims), _i4(bc),
+        None if domain is None else _i4(domain), int(part_mask), flags, _stream(stream)),
+        "lqcd_wilson_clover_residual_interior")
     return r
 
 

@@ -80,7 +80,8 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_coarse_halo_add_{_p}": (_ci, [_vp, _p8, _vp, _i4, _ci, _cu, _cu, _vp]),
         f"lqcd_wilson_clover_halo_pack_{_p}": (_ci, [_p8, _vp, _vp, _i4, _cu, _cu, _vp]),
         f"lqcd_wilson_clover_mult_interior_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _cu, _vp]),
-        f"lqcd_wilson_clover_residual_interior_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _cu, _vp]),
+        f"lqcd_wilson_clover_residual_interior_{_p}": (_ci, [_vp, _vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _cu, _cu,
+                                                             _vp]),
         f"lqcd_wilson_clover_halo_add_{_p}": (_ci, [_vp, _p8, _vp, _k, _i4, _i8, _cu, _cu, _vp]),
     })
 SIGNATURES.update({

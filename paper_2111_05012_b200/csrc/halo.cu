@@ -249,7 +249,7 @@ static int halo_add_call(T* out, const T* const recv[8], const T* U, T kappa, co
 template <typename T>
 int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa,
                                 const int dims[4], const int bc[4], unsigned part_mask, unsigned flags, void* stream,
-                                const char* what);
+                                const char* what, const int* domain);
 
 }  // namespace lqcd
 
@@ -274,35 +274,35 @@ int lqcd_wilson_clover_mult_interior_f32(float* out, const float* in, const floa
                                          const int dims[4], const int bc[4], unsigned part_mask, unsigned flags,
                                          void* stream) {
     return wilson_clover_interior_call<float>(out, in, U, clover, nullptr, kappa, dims, bc, part_mask, flags, stream,
-                                              "lqcd_wilson_clover_mult_interior_f32");
+                                              "lqcd_wilson_clover_mult_interior_f32", nullptr);
 }
 int lqcd_wilson_clover_mult_interior_f64(double* out, const double* in, const double* U, const double* clover,
                                          double kappa, const int dims[4], const int bc[4], unsigned part_mask,
                                          unsigned flags, void* stream) {
     return wilson_clover_interior_call<double>(out, in, U, clover, nullptr, kappa, dims, bc, part_mask, flags, stream,
-                                               "lqcd_wilson_clover_mult_interior_f64");
+                                               "lqcd_wilson_clover_mult_interior_f64", nullptr);
 }
 int lqcd_wilson_clover_residual_interior_f32(float* r, const float* b, const float* x, const float* U,
                                              const float* clover, float kappa, const int dims[4], const int bc[4],
-                                             unsigned part_mask, unsigned flags, void* stream) {
+                                             const int* domain, unsigned part_mask, unsigned flags, void* stream) {
     if (!b) {
         clear_error();
         set_error("lqcd_wilson_clover_residual_interior_f32: null rhs");
         return LQCD_EINVAL;
     }
     return wilson_clover_interior_call<float>(r, x, U, clover, b, kappa, dims, bc, part_mask, flags, stream,
-                                              "lqcd_wilson_clover_residual_interior_f32");
+                                              "lqcd_wilson_clover_residual_interior_f32", domain);
 }
 int lqcd_wilson_clover_residual_interior_f64(double* r, const double* b, const double* x, const double* U,
                                              const double* clover, double kappa, const int dims[4], const int bc[4],
-                                             unsigned part_mask, unsigned flags, void* stream) {
+                                             const int* domain, unsigned part_mask, unsigned flags, void* stream) {
     if (!b) {
         clear_error();
         set_error("lqcd_wilson_clover_residual_interior_f64: null rhs");
         return LQCD_EINVAL;
     }
     return wilson_clover_interior_call<double>(r, x, U, clover, b, kappa, dims, bc, part_mask, flags, stream,
-                                               "lqcd_wilson_clover_residual_interior_f64");
+                                               "lqcd_wilson_clover_residual_interior_f64", domain);
 }
 int lqcd_wilson_clover_halo_add_f32(float* out, const float* const recv[8], const float* U, float kappa,
                                     const int dims[4], const int face_phase[8], unsigned part_mask, unsigned flags,

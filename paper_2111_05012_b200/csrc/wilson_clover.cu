@@ -32,6 +32,7 @@ struct FineParams {
     int multi[4];  // 1 if there is more than one domain in that direction (else no hop is ever cut)
     int parity;    // 0 = all domains, 1 = even domains only, 2 = odd domains only
     int keep;      // with parity != 0: 1 = leave the sites of the other group untouched instead of zeroing them
+    int cut_lat;   // 1 = hops are cut where they leave the LATTICE (sharded interior pass), not where they leave a domain
 };
 
 // Which site is mine: CTA -> tile (x tiles fastest; optionally z-slabbed traversal), thread -> site in tile.  All
@@ -128,12 +129,14 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
         for (int mu = 0; mu < 4; mu++) {
             const int X = P.d_dom[mu].div(x[mu]), lx = x[mu] - X * P.dom[mu];
             par += X;
-            if (P.multi[mu] && lx == P.dom[mu] - 1) {  // forward hop leaves the domain
+            const bool ef = P.cut_lat ? x[mu] == P.L[mu] - 1 : lx == P.dom[mu] - 1;
+            const bool eb = P.cut_lat ? x[mu] == 0 : lx == 0;
+            if (P.multi[mu] && ef) {  // forward hop leaves the domain
                 sf[mu] = s;
                 lf[mu] = sb[mu];
                 pf[mu] = 0;
             }
-            if (P.multi[mu] && lx == 0) {  // backward hop leaves the domain
+            if (P.multi[mu] && eb) {  // backward hop leaves the domain
                 lb[mu] = s;
                 sb[mu] = s;
                 pb[mu] = 0;
@@ -223,6 +226,7 @@ static int fine_setup(FineParams& P, long long& ntiles_out, const int dims[4], c
     }
     P.parity = (flags & LQCD_DOMAIN_EVEN) ? 1 : (flags & LQCD_DOMAIN_ODD) ? 2 : 0;
     P.keep = 0;
+    P.cut_lat = 0;
     bool user_ok = g_knobs.fine_tile[0] > 0;
     for (int mu = 0; mu < 4 && user_ok; mu++) user_ok = dims[mu] % g_knobs.fine_tile[mu] == 0;
     if (user_ok)
@@ -399,8 +403,16 @@ template int wilson_clover_residual_group_call<double>(double*, const double*, c
 template <typename T>
 int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover, const T* rhs, T kappa,
                                 const int dims[4], const int bc[4], unsigned part_mask, unsigned flags, void* stream,
-                                const char* what) {
+                                const char* what, const int* domain) {
+    // flags may carry LQCD_DOMAIN_EVEN / ODD with rhs and domain: the residual on that group of domains only, the
+    // other sites untouched (the sharded SAP's intermediate residuals)
     clear_error();
+    const unsigned group = flags & (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD);
+    flags &= ~group;
+    if (group && (!rhs || !domain || group == (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD))) {
+        set_error("%s: a domain group needs the residual form, a domain and ONE of LQCD_DOMAIN_EVEN / ODD", what);
+        return LQCD_EINVAL;
+    }
     if (!out || !in || !U || !clover || check_dims(dims) || !bc) {
         set_error("%s: null pointer or non-positive dim", what);
         return LQCD_EINVAL;
@@ -424,10 +436,12 @@ int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover
     FineParams P;
     long long ntiles = 0;
     {
-        const int rc = fine_setup(P, ntiles, dims, bc, dims, 0, (int)sizeof(T), what);
+        const int rc = fine_setup(P, ntiles, dims, bc, group ? domain : dims, group, (int)sizeof(T), what);
         if (rc) return rc;
     }
     for (int mu = 0; mu < 4; mu++) P.multi[mu] = (part_mask >> mu) & 1;
+    P.cut_lat = 1;
+    P.keep = group ? 1 : 0;
     const int threads = (P.tilevol + 31) / 32 * 32;
     const bool dag = flags & LQCD_DAGGER, l12 = flags & LQCD_LINKS_12;
     cudaStream_t st = (cudaStream_t)stream;
@@ -441,7 +455,22 @@ int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover
             k_wilson_clover<T, DAG, L12, 1, RES, 256, (sizeof(T) == 4 ? 2 : 1)>                              \
                 <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);                               \
     } while (0)
-    if (rhs && l12) LAUNCH_I(false, true, true);
+    if (group && l12) {
+        if (threads <= 128)
+            k_wilson_clover<T, false, true, 2, true, 128, (sizeof(T) == 4 ? 4 : 3)>
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);
+        else
+            k_wilson_clover<T, false, true, 2, true, 256, (sizeof(T) == 4 ? 2 : 1)>
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);
+    } else if (group) {
+        if (threads <= 128)
+            k_wilson_clover<T, false, false, 2, true, 128, (sizeof(T) == 4 ? 4 : 3)>
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);
+        else
+            k_wilson_clover<T, false, false, 2, true, 256, (sizeof(T) == 4 ? 2 : 1)>
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);
+    }
+    else if (rhs && l12) LAUNCH_I(false, true, true);
     else if (rhs) LAUNCH_I(false, false, true);
     else if (dag && l12) LAUNCH_I(true, true, false);
     else if (dag) LAUNCH_I(true, false, false);
@@ -452,10 +481,11 @@ int wilson_clover_interior_call(T* out, const T* in, const T* U, const T* clover
     return check_launch(what);
 }
 template int wilson_clover_interior_call<float>(float*, const float*, const float*, const float*, const float*, float,
-                                                const int*, const int*, unsigned, unsigned, void*, const char*);
+                                                const int*, const int*, unsigned, unsigned, void*, const char*,
+                                                const int*);
 template int wilson_clover_interior_call<double>(double*, const double*, const double*, const double*, const double*,
                                                  double, const int*, const int*, unsigned, unsigned, void*,
-                                                 const char*);
+                                                 const char*, const int*);
 
 template int wilson_clover_call<float>(float*, const float*, const float*, const float*, const float*, float,
                                        const int*, const int*, const int*, unsigned, void*, const char*);

@@ -222,7 +222,7 @@ class ShardedWilsonClover:
         elif transport != "p2p":
             raise ValueError(f"transport {transport!r}")
 
-    def _run(self, out, inp, dagger, rhs):
+    def _run(self, out, inp, dagger, rhs, domain=None, parity=0):
         cur = torch.cuda.current_stream(self.U.device)
         send, got = (self.send, None) if self.peer is None else self.peer.next()
         wilson_clover_halo_pack(send, inp, self.U, self.dims, self.mask, dagger, self.links12, stream=cur)
@@ -239,7 +239,7 @@ class ShardedWilsonClover:
                                         dagger, self.links12, stream=cur)
         else:
             wilson_clover_residual_interior(out, rhs, inp, self.U, self.clover, self.kappa, self.dims, self.bc,
-                                            self.mask, self.links12, stream=cur)
+                                            self.mask, self.links12, domain, parity, stream=cur)
         cur.wait_event(arrived)
         # the residual carries -D: the faces enter with the opposite sign
         wilson_clover_halo_add(out, got, self.U, self.kappa if rhs is None else -self.kappa, self.dims, self.phase,
@@ -250,9 +250,10 @@ class ShardedWilsonClover:
         """out = D inp (or D^dag inp)."""
         return self._run(out, inp, dagger, None)
 
-    def residual(self, r, b, x):
-        """r = b - D x; r must not alias b or x."""
-        return self._run(r, x, False, b)
+    def residual(self, r, b, x, domain=None, parity=0):
+        """r = b - D x; r must not alias b or x.  parity 1 / 2 with a domain: only on the
+        even / odd domains (LOCAL colouring) -- the rest of r is then not meaningful."""
+        return self._run(r, x, False, b, domain, parity)
 
 
 class ShardedSAP:
@@ -272,8 +273,10 @@ class ShardedSAP:
     def apply(self, x, r, b, initial_guess=False, final_residual=True):
         """x = SAP_n(b) (or x + SAP_n(b - D x) with initial_guess); r: scratch, receives b - D x."""
         op = self.op
+        # between two half sweeps only the group solved next reads the residual (as in lqcd_sap)
+        group = lambda g: 1 + (g ^ self.flip)
         if initial_guess:
-            op.residual(r, b, x)
+            op.residual(r, b, x, self.domain, group(0) if self.n_sap > 0 else 0)
             res = r
         else:
             x.zero_()
@@ -283,10 +286,11 @@ class ShardedSAP:
         for i in range(self.n_sap):
             for g in (0, 1):
                 mr_domain_solve(x, res, op.U, op.clover, op.kappa, op.dims, op.bc, self.domain,
-                                parity=1 + (g ^ self.flip), niter=self.n_mr, accumulate=True, ws=self.ws)
-                if i == self.n_sap - 1 and g == 1 and not final_residual:
+                                parity=group(g), niter=self.n_mr, accumulate=True, ws=self.ws)
+                last = i == self.n_sap - 1 and g == 1
+                if last and not final_residual:
                     break
-                op.residual(r, b, x)
+                op.residual(r, b, x, self.domain, 0 if last else group(g ^ 1))
                 res = r
         return x
 
