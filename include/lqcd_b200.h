@@ -262,7 +262,9 @@ int lqcd_mr_domain_solve_f64(double* z, const double* r, const double* U, const 
  * x: the result; r: caller-owned scratch spinor that receives the final residual b - D x; b: right-hand side; all
  * three distinct native spinors.  flags: LQCD_SAP_INITIAL_GUESS starts from the x passed in (|r> := |b> - D|x>
  * first): x0 + SAP(b - D x0), the Richardson refinement with M_2 = SAP in one call;
- * LQCD_SAP_NO_FINAL_RESIDUAL omits the last residual (saves one application of D when r is not needed).
+ * LQCD_SAP_NO_FINAL_RESIDUAL omits the last residual (saves one application of D when r is not needed; r then holds
+ * no defined value).  The intermediate |r> := |b> - D|x> are evaluated only where the next half sweep reads them, on
+ * the domains of its group (same arithmetic there; x and the final r do not depend on it).
  * ws_dev as for lqcd_mr_domain_solve.  2 n_sap solver launches + 2 n_sap residual launches on `stream`. */
 int lqcd_sap_f32(float* x, float* r, const float* b, const float* U, const float* clover, float kappa,
                  const int dims[4], const int bc[4], const int domain[4], int n_sap, int n_mr, unsigned flags,
