@@ -13,6 +13,8 @@ host-vector C-ABI calls with the H2D/D2H copies inside the timed region.
 
 Multi-GPU: the path is single-GPU by the north_star ("replicas only"): --gpus N runs N independent
 replicas, one process per GPU under torchrun, barrier + max-over-ranks timing, no data-path collective.
+Opt-in: --sharded makes the ranks share ONE lattice instead (each holds a sub-lattice of the config's size) with a
+halo exchange inside D, D^dag and D_c (--sharded-transport p2p | peer).
 
 --impl reference times the CPU oracle as it stands on the host cores on a bounded sample of the same workload.
 """
