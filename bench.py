@@ -2,7 +2,7 @@
 """bench.py -- throughput of the hot path on synthetic lattices shaped like the
 paper's workloads.
 
-    python bench.py --gpus N --steps K --warmup W [--workload c5|c4|c3|c2] [--impl ours|reference]
+    python bench.py --gpus N --steps K --warmup W [--workload c5|c4|c3|c2] [--precision f32|f64] [--impl ours|reference]
 
 One "step" = one pass of the whole hot path over one right-hand side:
     D x (A1, 18-real links), D^dag x (A2), restrict x (A4), coarse_mult (A3), prolong (A5)  [A4->A3->A5 chained = A6]
@@ -43,14 +43,16 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if 
 # ----------------------------------------------------------------------------------------------------------
 # algorithmic bytes / nominal flops per launch (restated in DESIGN.md "Roofline model")
 # ----------------------------------------------------------------------------------------------------------
-def model(cfg: li.Config, links12: bool = False) -> dict:
+def model(cfg: li.Config, links12: bool = False, real_bytes: int = 4) -> dict:
+    """real_bytes: 4 for the fp32 kernels (the figures of SURVEY 8(d)), 8 for the fp64 variants (twice the bytes)."""
     V, Vc, N, nv = cfg.volume, cfg.cvolume, 2 * cfg.nvec, cfg.nvec
     bv = V // Vc
-    fine_b = (96 + 96 + (192 if links12 else 288) + 288) * V
+    w = real_bytes // 4
+    fine_b = (96 + 96 + (192 if links12 else 288) + 288) * V * w
     fine_f = 1872 * V
-    coarse_b = (9 * N * N * 8 + 2 * N * 8) * Vc
+    coarse_b = (9 * N * N * 8 + 2 * N * 8) * Vc * w
     coarse_f = 9 * N * N * 8 * Vc
-    tr_b = (nv * 96 + 96) * V + N * 8 * Vc
+    tr_b = ((nv * 96 + 96) * V + N * 8 * Vc) * w
     tr_f = nv * 96 * V
     return {
         "wilson_clover": {"bytes": fine_b, "flops": fine_f, "units": V},
@@ -248,16 +250,17 @@ class Workload:
 
     NBUF = 4  # distinct input/output buffer sets rotated across steps (and every buffer is >> L2 at c4/c5)
 
-    def __init__(self, cfg: li.Config, device, seed: int, synthetic_operators: bool = False):
+    def __init__(self, cfg: li.Config, device, seed: int, synthetic_operators: bool = False, precision: str = "f32"):
         import torch
         import paper_2111_05012_b200 as lq
         self.cfg, self.lq, self.dev = cfg, lq, device
+        rdt, cdt = (torch.float32, torch.complex64) if precision == "f32" else (torch.float64, torch.complex128)
         self.sh_fine = self.sh_coarse = None
         gen = torch.Generator(device=device)
         gen.manual_seed(seed)
         V, Vc, nv = cfg.volume, cfg.cvolume, cfg.nvec
         # gauge: the config's recipe, fp64 on the device, rounded to fp32 once, packed (18-real and 12-real)
-        U = li.t_gauge_field(cfg, gen, device).to(torch.complex64)
+        U = li.t_gauge_field(cfg, gen, device).to(cdt)
         self.U18 = lq.pack_gauge(U, cfg.dims)
         self.U12 = lq.pack_gauge(U, cfg.dims, links12=True)
         del U
@@ -272,26 +275,26 @@ class Workload:
             return r
 
         if synthetic_operators:
-            cl = li.t_clover_synthetic(gen, V, device)
+            cl = li.t_clover_synthetic(gen, V, device).to(cdt)
             self.clover = lq.pack_clover(cl, cfg.dims)
             del cl
         else:  # the true clover term of these links, built by the device set-up kernel (F2)
             self.clover = timed("clover_from_links", lambda: lq.clover_from_links(self.U18, cfg.kappa, cfg.csw, cfg.dims))
-        self.x = [lq.pack_spinor(li.t_spinor(gen, V, device, torch.float32), cfg.dims) for _ in range(self.NBUF)]
-        self.y = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
-        self.yd = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
-        self.z = [lq.empty_spinor(cfg.dims) for _ in range(self.NBUF)]
-        self.xc = [torch.empty((Vc, 2, nv), dtype=torch.complex64, device=device) for _ in range(self.NBUF)]
-        self.yc = [torch.empty((Vc, 2, nv), dtype=torch.complex64, device=device) for _ in range(self.NBUF)]
+        self.x = [lq.pack_spinor(li.t_spinor(gen, V, device, rdt), cfg.dims) for _ in range(self.NBUF)]
+        self.y = [lq.empty_spinor(cfg.dims, dtype=rdt) for _ in range(self.NBUF)]
+        self.yd = [lq.empty_spinor(cfg.dims, dtype=rdt) for _ in range(self.NBUF)]
+        self.z = [lq.empty_spinor(cfg.dims, dtype=rdt) for _ in range(self.NBUF)]
+        self.xc = [torch.empty((Vc, 2, nv), dtype=cdt, device=device) for _ in range(self.NBUF)]
+        self.yc = [torch.empty((Vc, 2, nv), dtype=cdt, device=device) for _ in range(self.NBUF)]
         # null vectors: Gaussian, one canonical vector at a time into its native slot (never twice in HBM)
-        self.v = torch.empty(lq.native_nullvecs_reals(cfg.dims, cfg.block, nv), dtype=torch.float32, device=device)
+        self.v = torch.empty(lq.native_nullvecs_reals(cfg.dims, cfg.block, nv), dtype=rdt, device=device)
         scale = 1.0 / np.sqrt(2.0 * 6 * (V // Vc))  # unit-norm aggregates on average, like orthonormal ones
         for i in range(nv):
-            vi = li.t_spinor(gen, V, device, torch.float32) * scale
+            vi = li.t_spinor(gen, V, device, rdt) * scale
             lq.pack_nullvec(self.v, vi, i, cfg.dims, cfg.block, nv)
             del vi
         if synthetic_operators:
-            self.A = li.t_coarse_matrix_synthetic(gen, Vc, nv, device)
+            self.A = li.t_coarse_matrix_synthetic(gen, Vc, nv, device).to(cdt)
         else:  # block-orthonormal null vectors and the true Galerkin coarse operator P^dag D P (F2)
             timed("orthonormalize_blocks", lambda: lq.orthonormalize_blocks(self.v, cfg.dims, cfg.block, nv))
             self.A = timed("galerkin_coarse", lambda: lq.galerkin_coarse(self.U18, self.clover, self.v, cfg.kappa,
@@ -454,10 +457,11 @@ def time_e2e(W: Workload, steps: int, warmup: int, ranks: Ranks):
     streams = [torch.cuda.Stream(device=W.dev) for _ in range(3)]
     g = torch.Generator()
     g.manual_seed(99)
-    x_h = torch.randn((V, 4, 3, 2), generator=g, dtype=torch.float32).pin_memory()
-    y_h = [torch.empty((V, 4, 3, 2), dtype=torch.float32).pin_memory() for _ in range(3)]
-    xc_h = torch.empty((Vc, 2, nv, 2), dtype=torch.float32).pin_memory()
-    yc_h = torch.empty((Vc, 2, nv, 2), dtype=torch.float32).pin_memory()
+    rdt = W.v.dtype
+    x_h = torch.randn((V, 4, 3, 2), generator=g, dtype=rdt).pin_memory()
+    y_h = [torch.empty((V, 4, 3, 2), dtype=rdt).pin_memory() for _ in range(3)]
+    xc_h = torch.empty((Vc, 2, nv, 2), dtype=rdt).pin_memory()
+    yc_h = torch.empty((Vc, 2, nv, 2), dtype=rdt).pin_memory()
 
     def chain_d():
         torch.cuda.set_device(W.dev)  # worker threads start on device 0
@@ -481,7 +485,7 @@ def time_e2e(W: Workload, steps: int, warmup: int, ranks: Ranks):
         for f in futs:
             f.result()
 
-    fine_b, coarse_b = V * 96, Vc * 2 * nv * 8
+    fine_b, coarse_b = V * 24 * x_h.element_size(), Vc * 2 * nv * 2 * x_h.element_size()
     h2d = 3 * fine_b + 2 * coarse_b          # x (three times), xc, yc
     d2h = 3 * fine_b + 2 * coarse_b          # D x, D^dag x, prolong out, xc, yc
     for _ in range(warmup):
@@ -600,8 +604,11 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     torch.cuda.set_device(dev_index)
     device = torch.device("cuda", dev_index)
     import paper_2111_05012_b200 as lq
-    W = Workload(cfg, device, seed=cfg.seed + 17 * ranks.rank, synthetic_operators=args.synthetic_operators)
-    m = model(cfg)
+    f64 = args.precision == "f64"
+    rb = 8 if f64 else 4
+    W = Workload(cfg, device, seed=cfg.seed + 17 * ranks.rank, synthetic_operators=args.synthetic_operators,
+                 precision=args.precision)
+    m = model(cfg, real_bytes=rb)
     peak, peak_src = measured_peak()
     sharded = None
     if args.sharded is not None:
@@ -630,7 +637,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     clocks = sampler.stop()
     max_s = ranks.max(total_s)
     sec_per_step = max_s / args.steps
-    sbytes, sflops = step_bytes(cfg), step_flops(cfg)
+    sbytes, sflops = step_bytes(cfg) * (rb // 4), step_flops(cfg)
     value = whole_job_value(sbytes, ranks.world, sec_per_step) / 1e9
 
     kernels = {}
@@ -645,17 +652,18 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     dominant = max(STEP_ORDER, key=lambda n: kernels[n]["us"])
     roofline = {
         "bound": "hbm", "kernel": dominant, "achieved": kernels[dominant]["GBps"], "peak": peak, "unit": "GB/s",
-        "frac": kernels[dominant]["GBps"] / peak, "traffic": recorded_traffic(cfg.name, dominant),
+        "frac": kernels[dominant]["GBps"] / peak, "traffic": None if f64 else recorded_traffic(cfg.name, dominant),
         "peak_source": peak_src, "algorithmic_bytes_per_launch": m[dominant]["bytes"],
     }
     # the 12-real-link variant of A1 (config 4 asks for both storages), timed alone
     extra = {}
     if not args.no_extras and sharded is None:
         t12 = time_single(W, "wilson_clover_12", reps=max(10, args.steps))
-        m12 = model(cfg, links12=True)["wilson_clover"]
+        m12 = model(cfg, links12=True, real_bytes=rb)["wilson_clover"]
         extra["wilson_clover_links12"] = {"us": t12 * 1e6, "GBps": m12["bytes"] / t12 / 1e9,
                                           "GFLOPs": m12["flops"] / t12 / 1e9, "units_per_s": m12["units"] / t12,
                                           "frac_of_hbm_peak": m12["bytes"] / t12 / 1e9 / peak}
+    if not args.no_extras and sharded is None and not f64:
         # F1 (next row of SURVEY 8(f)): the domain-decomposed operator D_SAP, all domains and the even group
         for name, par in (("wilson_clover_dd", 0), ("wilson_clover_dd_even", 1)):
             t = time_single(W, name, reps=max(10, args.steps))
@@ -778,6 +786,26 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "us": t * 1e6, "overhead_vs_mg_vcycle_8_4_6": t * 1e6 / extra["mg_vcycle_8_4_6"]["us"]}
         del W.sharded_op
 
+    if not args.no_extras and sharded is None and not f64:
+        # the fp64 variants of the five rows (north_star: "fp64 and fp32 kernel variants"), on config 4's lattice when
+        # the workload is larger (the fp64 fields of config 5 do not fit beside its fp32 ones): twice the bytes
+        c64 = cfg if cfg.volume <= li.CONFIGS["c4"].volume else li.CONFIGS["c4"]
+        W64 = Workload(c64, device, seed=c64.seed + 5, synthetic_operators=args.synthetic_operators, precision="f64")
+        m64 = model(c64, real_bytes=8)
+        _, pk64, _ = time_steps(W64, max(5, min(20, args.steps)), 3, ranks)
+        rows = {}
+        for name in STEP_ORDER:
+            t = statistics.mean(pk64[name])
+            rows[name] = {"us": t * 1e6, "GBps": m64[name]["bytes"] / t / 1e9, "GFLOPs": m64[name]["flops"] / t / 1e9,
+                          "units_per_s": m64[name]["units"] / t, "frac_of_hbm_peak": m64[name]["bytes"] / t / 1e9 / peak}
+        t64 = sum(r["us"] for r in rows.values()) * 1e-6
+        extra["fp64_five_rows"] = {"workload": c64.name, "dtype": "f64", "ms_per_step": t64 * 1e3,
+                                   "GBps": sum(m64[n]["bytes"] for n in STEP_ORDER) / t64 / 1e9,
+                                   "frac_of_hbm_peak": sum(m64[n]["bytes"] for n in STEP_ORDER) / t64 / 1e9 / peak,
+                                   "kernels": rows}
+        del W64
+        torch.cuda.empty_cache()
+
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)
     e2e_s = ranks.max(e2e_s)
@@ -788,7 +816,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     line = {
         "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": ranks.world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config_dict(cfg, ranks.world),
+        "vs_baseline": None, "dtype": args.precision, "data": "synthetic", "config": config_dict(cfg, ranks.world),
         "gflops": whole_job_value(sflops, ranks.world, sec_per_step) / 1e9,
         "fine_sites_per_s": whole_job_value(2 * cfg.volume, ranks.world, sec_per_step),
         "frac_of_hbm_peak": value / ranks.world / peak,
@@ -876,6 +904,9 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", choices=sorted(li.CONFIGS), default="c5")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--precision", choices=("f32", "f64"), default="f32",
+                    help="f64: the fp64 kernel variants on the same step (twice the algorithmic bytes; the headline "
+                         "metric is fp32)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--sharded", nargs="?", const="", default=None, metavar="R0,R1,R2,R3",

@@ -82,6 +82,9 @@ def test_roofline_model_matches_survey_table():
     assert m["wilson_clover"]["flops"] == 1872 * c5.volume
     assert m["coarse_mult"]["bytes"] == 295936 * c5.cvolume          # 9 N^2 8 + 2 N 8, N = 64
     assert m["restrict"]["bytes"] == 3168 * c5.volume + 512 * c5.cvolume
+    m64 = bench.model(c5, real_bytes=8)                              # fp64 variants: twice the bytes, same flops
+    for k in bench.STEP_ORDER:
+        assert m64[k]["bytes"] == 2 * m[k]["bytes"] and m64[k]["flops"] == m[k]["flops"]
 
 
 def test_default_rank_grid_splits_t_z_y_first():
