@@ -452,7 +452,7 @@ def time_e2e(W: Workload, steps: int, warmup: int, ranks: Ranks):
     # with its own scratch, driven by its own host thread (the C calls release the GIL and synchronise their stream):
     # uploads of one chain overlap downloads of another, PCIe being full duplex.
     from concurrent.futures import ThreadPoolExecutor
-    nws = lq.host_workspace_bytes(c.dims, c.block, nv)
+    nws = lq.host_workspace_bytes(c.dims, c.block, nv, dtype=W.v.dtype)
     ws = [torch.empty(nws, dtype=torch.uint8, device=W.dev) for _ in range(3)]
     streams = [torch.cuda.Stream(device=W.dev) for _ in range(3)]
     g = torch.Generator()
@@ -652,7 +652,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     dominant = max(STEP_ORDER, key=lambda n: kernels[n]["us"])
     roofline = {
         "bound": "hbm", "kernel": dominant, "achieved": kernels[dominant]["GBps"], "peak": peak, "unit": "GB/s",
-        "frac": kernels[dominant]["GBps"] / peak, "traffic": None if f64 else recorded_traffic(cfg.name, dominant),
+        "frac": kernels[dominant]["GBps"] / peak, "traffic": recorded_traffic(cfg.name + (":f64" if f64 else ""), dominant),
         "peak_source": peak_src, "algorithmic_bytes_per_launch": m[dominant]["bytes"],
     }
     # the 12-real-link variant of A1 (config 4 asks for both storages), timed alone

@@ -452,13 +452,15 @@ int lqcd_coarse_bicgstab_hooks_f32(float* x, float* r_out, const float* b, const
 int lqcd_coarse_bicgstab_hooks_f64(double* x, double* r_out, const double* b, const int cdims[4], int nvec, int niter,
                                    lqcd_apply_fn apply, lqcd_reduce_fn reduce, void* user, void* ws_dev, void* stream);
 
-/* ---- end-to-end entry points on HOST vectors (fp32) -----------------------------------------
+/* ---- end-to-end entry points on HOST vectors (fp32 and fp64) ---------------------------------
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
  * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned
  * memory recommended).  Each call: cudaMemcpyAsync H2D -> pack -> the mult kernel -> unpack ->
  * cudaMemcpyAsync D2H -> cudaStreamSynchronize.  ws_dev is caller-owned device scratch of at least
- * lqcd_host_workspace_bytes(...) bytes. */
+ * lqcd_host_workspace_bytes(...) bytes (the _f32 calls) or lqcd_host_workspace_bytes_f64(...) bytes
+ * (the _f64 calls; host and device data are then all double).  Same errors as the device calls. */
 size_t lqcd_host_workspace_bytes(const int dims[4], const int block[4], int nvec);
+size_t lqcd_host_workspace_bytes_f64(const int dims[4], const int block[4], int nvec);
 int lqcd_wilson_clover_mult_host_f32(float* out_host, const float* in_host, const float* U, const float* clover,
                                      float kappa, const int dims[4], const int bc[4], unsigned flags,
                                      void* ws_dev, void* stream);
@@ -467,6 +469,15 @@ int lqcd_coarse_mult_host_f32(float* out_host, const float* in_host, const float
 int lqcd_restrict_host_f32(float* out_c_host, const float* in_f_host, const float* nullvecs, const int dims[4],
                            const int block[4], int nvec, void* ws_dev, void* stream);
 int lqcd_prolong_host_f32(float* out_f_host, const float* in_c_host, const float* nullvecs, const int dims[4],
+                          const int block[4], int nvec, void* ws_dev, void* stream);
+int lqcd_wilson_clover_mult_host_f64(double* out_host, const double* in_host, const double* U, const double* clover,
+                                     double kappa, const int dims[4], const int bc[4], unsigned flags,
+                                     void* ws_dev, void* stream);
+int lqcd_coarse_mult_host_f64(double* out_host, const double* in_host, const double* A, const int cdims[4],
+                              int nvec, unsigned flags, void* ws_dev, void* stream);
+int lqcd_restrict_host_f64(double* out_c_host, const double* in_f_host, const double* nullvecs, const int dims[4],
+                           const int block[4], int nvec, void* ws_dev, void* stream);
+int lqcd_prolong_host_f64(double* out_f_host, const double* in_c_host, const double* nullvecs, const int dims[4],
                           const int block[4], int nvec, void* ws_dev, void* stream);
 
 #ifdef __cplusplus

@@ -136,8 +136,9 @@ def native_coarse_mat_reals(cdims, nvec) -> int:
     return int(lib().lqcd_native_coarse_mat_reals(_i4(cdims), int(nvec)))
 
 
-def host_workspace_bytes(dims, block, nvec) -> int:
-    return int(lib().lqcd_host_workspace_bytes(_i4(dims), _i4(block), int(nvec)))
+def host_workspace_bytes(dims, block, nvec, dtype=torch.float32) -> int:
+    fn = lib().lqcd_host_workspace_bytes if dtype == torch.float32 else lib().lqcd_host_workspace_bytes_f64
+    return int(fn(_i4(dims), _i4(block), int(nvec)))
 
 
 def empty_spinor(dims, dtype=torch.float32, device="cuda") -> torch.Tensor:
@@ -641,27 +642,31 @@ def coarse_halo_add(out, recv, A, cdims, nvec, part_mask, dagger=False, stream=N
 
 def wilson_clover_mult_host(out_host, in_host, U, clover, kappa, dims, bc, ws, dagger=False, links12=False,
                             stream=None):
+    sfx = _same_dtype(out_host, in_host, U, clover)
     flags = (DAGGER if dagger else 0) | (LINKS_12 if links12 else 0)
-    _check(lib().lqcd_wilson_clover_mult_host_f32(_host_ptr(out_host), _host_ptr(in_host), _dev_ptr(U),
-                                                  _dev_ptr(clover), C.c_float(kappa), _i4(dims), _i4(bc), flags,
-                                                  _dev_ptr(ws), _stream(stream)), "lqcd_wilson_clover_mult_host_f32")
+    k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
+    what = f"lqcd_wilson_clover_mult_host_{sfx}"
+    _check(getattr(lib(), what)(_host_ptr(out_host), _host_ptr(in_host), _dev_ptr(U), _dev_ptr(clover), k, _i4(dims),
+                                _i4(bc), flags, _dev_ptr(ws), _stream(stream)), what)
     return out_host
 
 
 def coarse_mult_host(out_host, in_host, A, cdims, nvec, ws, dagger=False, stream=None):
-    _check(lib().lqcd_coarse_mult_host_f32(_host_ptr(out_host), _host_ptr(in_host), _dev_ptr(A), _i4(cdims), int(nvec),
-                                           DAGGER if dagger else 0, _dev_ptr(ws), _stream(stream)),
-           "lqcd_coarse_mult_host_f32")
+    what = f"lqcd_coarse_mult_host_{_same_dtype(out_host, in_host, A)}"
+    _check(getattr(lib(), what)(_host_ptr(out_host), _host_ptr(in_host), _dev_ptr(A), _i4(cdims), int(nvec),
+                                DAGGER if dagger else 0, _dev_ptr(ws), _stream(stream)), what)
     return out_host
 
 
 def restrict_host(out_c_host, in_f_host, nullvecs, dims, block, nvec, ws, stream=None):
-    _check(lib().lqcd_restrict_host_f32(_host_ptr(out_c_host), _host_ptr(in_f_host), _dev_ptr(nullvecs), _i4(dims),
-                                        _i4(block), int(nvec), _dev_ptr(ws), _stream(stream)), "lqcd_restrict_host_f32")
+    what = f"lqcd_restrict_host_{_same_dtype(out_c_host, in_f_host, nullvecs)}"
+    _check(getattr(lib(), what)(_host_ptr(out_c_host), _host_ptr(in_f_host), _dev_ptr(nullvecs), _i4(dims),
+                                _i4(block), int(nvec), _dev_ptr(ws), _stream(stream)), what)
     return out_c_host
 
 
 def prolong_host(out_f_host, in_c_host, nullvecs, dims, block, nvec, ws, stream=None):
-    _check(lib().lqcd_prolong_host_f32(_host_ptr(out_f_host), _host_ptr(in_c_host), _dev_ptr(nullvecs), _i4(dims),
-                                       _i4(block), int(nvec), _dev_ptr(ws), _stream(stream)), "lqcd_prolong_host_f32")
+    what = f"lqcd_prolong_host_{_same_dtype(out_f_host, in_c_host, nullvecs)}"
+    _check(getattr(lib(), what)(_host_ptr(out_f_host), _host_ptr(in_c_host), _dev_ptr(nullvecs), _i4(dims),
+                                _i4(block), int(nvec), _dev_ptr(ws), _stream(stream)), what)
     return out_f_host

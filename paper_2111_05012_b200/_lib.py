@@ -33,6 +33,7 @@ SIGNATURES = {
     "lqcd_native_coarse_vec_reals": (C.c_size_t, [_i4, _ci]),
     "lqcd_native_coarse_mat_reals": (C.c_size_t, [_i4, _ci]),
     "lqcd_host_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
+    "lqcd_host_workspace_bytes_f64": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_galerkin_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
     "lqcd_mr_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_coarse_bicgstab_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci]),
@@ -84,12 +85,13 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
                                                              _vp]),
         f"lqcd_wilson_clover_halo_add_{_p}": (_ci, [_vp, _p8, _vp, _k, _i4, _i8, _cu, _cu, _vp]),
     })
-SIGNATURES.update({
-    "lqcd_wilson_clover_mult_host_f32": (_ci, [_vp, _vp, _vp, _vp, _cf, _i4, _i4, _cu, _vp, _vp]),
-    "lqcd_coarse_mult_host_f32": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _vp, _vp]),
-    "lqcd_restrict_host_f32": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp, _vp]),
-    "lqcd_prolong_host_f32": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp, _vp]),
-})
+for _p, _k in (("f32", _cf), ("f64", _cd)):
+    SIGNATURES.update({
+        f"lqcd_wilson_clover_mult_host_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _vp, _vp]),
+        f"lqcd_coarse_mult_host_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _vp, _vp]),
+        f"lqcd_restrict_host_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp, _vp]),
+        f"lqcd_prolong_host_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _vp, _vp]),
+    })
 
 
 def lib_path() -> str:

@@ -364,20 +364,26 @@ def test_error_codes(lq):
 # ------------------------------------------------------------------------------------------------------
 # host-vector entry points give the same numbers as the device-pointer ones
 # ------------------------------------------------------------------------------------------------------
-def test_host_entry_points(lq):
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_host_entry_points(lq, prec):
     import torch
     prob = config_problem("c2", 16)
     cfg = prob.cfg
-    d = Dev(lq, prob, "f32")
-    ws = torch.empty(lq.host_workspace_bytes(cfg.dims, cfg.block, cfg.nvec), dtype=torch.uint8, device="cuda")
-    psi = torch.from_numpy(rounded(prob.psi[0], "f32")).pin_memory()
+    d = Dev(lq, prob, prec)
+    rdt = torch.float32 if prec == "f32" else torch.float64
+    ws = torch.empty(lq.host_workspace_bytes(cfg.dims, cfg.block, cfg.nvec, dtype=rdt), dtype=torch.uint8,
+                     device="cuda")
+    psi = torch.from_numpy(rounded(prob.psi[0], prec)).pin_memory()
     out = torch.empty_like(psi).pin_memory()
     lq.wilson_clover_mult_host(out, psi, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, ws)
     assert np.array_equal(out.numpy(), d.D(prob.psi[0]))
     lq.wilson_clover_mult_host(out, psi, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, ws, dagger=True)
     assert np.array_equal(out.numpy(), d.D(prob.psi[0], dagger=True))
-    xc = torch.from_numpy(rounded(prob.xc, "f32")).pin_memory()
+    xc = torch.from_numpy(rounded(prob.xc, prec)).pin_memory()
     yc = torch.empty_like(xc).pin_memory()
+    with pytest.raises(TypeError):  # host and device data of one call share one precision
+        lq.coarse_mult_host(yc.to(torch.complex64 if prec == "f64" else torch.complex128), xc, d.A, cfg.cdims,
+                            cfg.nvec, ws)
     lq.coarse_mult_host(yc, xc, d.A, cfg.cdims, cfg.nvec, ws)
     assert np.array_equal(yc.numpy(), d.Dc(prob.xc))
     lq.restrict_host(yc, psi, d.v, cfg.dims, cfg.block, cfg.nvec, ws)
