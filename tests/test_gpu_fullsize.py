@@ -309,3 +309,93 @@ def test_fullsize_mrhs_sampled(lq, name):
         for k in range(2):
             lq.wilson_clover_mult(ys1, x2[k], U18, Cn, cfg.kappa, L, cfg.bc, dagger=dag)
             assert torch.equal(y2[k], ys1), (dag, k)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# the fp64 kernel variants at full size (config 4; `bench.py --precision f64` times them), bar 1e-12 (north_star)
+# ------------------------------------------------------------------------------------------------------------------
+TOL64 = 1e-12
+
+
+def test_fullsize_fp64_five_rows_sampled(lq):
+    """Same sampling as the fp32 tests above, on complex128 inputs: the oracle's fp64-input entry points."""
+    import torch
+    cfg = li.CONFIGS["c4"]
+    V, L, b, nv, Vc, Lc = cfg.volume, cfg.dims, cfg.block, cfg.nvec, cfg.cvolume, cfg.cdims
+    v3 = L[0] * L[1] * L[2]
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed + 7)
+    rng = np.random.default_rng(cfg.seed + 7)
+    c128 = torch.complex128
+
+    # ---- A1 / A2: D, D^dag, 12-real links ----
+    U = li.t_gauge_field(cfg, gen, "cuda")
+    assert U.dtype == c128
+    cl = li.t_clover_synthetic(gen, V, "cuda").to(c128)
+    psi = li.t_spinor(gen, V, "cuda", torch.float64)
+    U18, U12 = lq.pack_gauge(U, L), lq.pack_gauge(U, L, links12=True)
+    Cn = lq.pack_clover(cl, L)
+    x = lq.pack_spinor(psi, L)
+    y = lq.empty_spinor(L, dtype=torch.float64)
+    assert U18.dtype == torch.float64 and x.dtype == torch.float64
+    sites, slabs = sample_fine_sites(cfg, rng, 2000)
+    U_h = lazily_filled((4, V, 3, 3), np.complex128, U, slabs, v3, 1)
+    cl_h = lazily_filled((V, 2, 6, 6), np.complex128, cl, slabs, v3, 0)
+    psi_h = lazily_filled((V, 4, 3), np.complex128, psi, slabs, v3, 0)
+    sites_d = torch.from_numpy(sites).cuda()
+    for label, Un, dag, l12 in (("D", U18, False, False), ("Ddag", U18, True, False), ("D_links12", U12, False, True)):
+        lq.wilson_clover_mult(y, x, Un, Cn, cfg.kappa, L, cfg.bc, dagger=dag, links12=l12)
+        got = lq.unpack_spinor(y, L)[sites_d].cpu().numpy()
+        ref = oracle.wilson_clover_mult_sites(psi_h, U_h, cl_h, cfg.kappa, L, cfg.bc, sites, dagger=dag)
+        assert got.dtype == np.complex128 and np.isfinite(got).all()
+        assert rel_l2(got, ref) <= TOL64, label
+        per_site = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / np.linalg.norm(
+            ref.reshape(len(sites), -1), axis=1)
+        assert per_site.max() <= 5 * TOL64, (label, int(sites[per_site.argmax()]))
+    del U, cl, U18, U12, Cn, U_h, cl_h
+
+    # ---- A3: coarse operator and its dagger ----
+    A = li.t_coarse_matrix_synthetic(gen, Vc, nv, "cuda").to(c128)
+    xc = li.t_coarse_vector(gen, Vc, nv, "cuda", torch.float64)
+    yc = torch.empty_like(xc)
+    Lca = np.array(Lc)
+    corners = np.array([[x_, y_, z_, t_] for x_ in (0, Lca[0] - 1) for y_ in (0, Lca[1] - 1) for z_ in (0, Lca[2] - 1)
+                        for t_ in (0, Lca[3] - 1)])
+    rnd = np.stack([rng.integers(0, Lca[mu], 48) for mu in range(4)], axis=1)
+    csites = site_index(Lc, np.concatenate([corners, rnd])).astype(np.int64)
+    csites_d = torch.from_numpy(csites).cuda()
+    A_s = A[csites_d].cpu().numpy()
+    xc_h = xc.cpu().numpy()
+    for dag in (False, True):
+        lq.coarse_mult(yc, xc, A, Lc, nv, dagger=dag)
+        got = yc[csites_d].cpu().numpy()
+        ref = oracle.coarse_mult_sites(xc_h, A_s, Lc, csites, dagger=dag)
+        assert rel_l2(got, ref) <= TOL64, dag
+    del A, A_s
+
+    # ---- A4 / A5: 16 sampled aggregates gathered into a fake 8^4 lattice of 2^4 blocks (see the fp32 test) ----
+    Xs = np.stack([rng.integers(0, Lca[mu], 16) for mu in range(4)], axis=1)
+    Xs[0] = 0
+    Xs[1] = Lca - 1
+    fdims = (8, 8, 8, 8)
+    fc = li.site_coords(fdims)
+    k = site_index((2, 2, 2, 2), fc // 4)
+    real = site_index(L, Xs[k] * 4 + fc % 4)
+    real_d = torch.from_numpy(real.astype(np.int64)).cuda()
+    Xreal_d = torch.from_numpy(site_index(Lc, Xs).astype(np.int64)).cuda()
+    vn = torch.empty(lq.native_nullvecs_reals(L, b, nv), dtype=torch.float64, device="cuda")
+    v_fake = np.empty((nv, 4096, 4, 3), dtype=np.complex128)
+    scale = 1.0 / np.sqrt(2.0 * 6 * 256)
+    for i in range(nv):
+        vi = li.t_spinor(gen, V, "cuda", torch.float64) * scale
+        lq.pack_nullvec(vn, vi, i, L, b, nv)
+        v_fake[i] = vi[real_d].cpu().numpy()
+        del vi
+    out_c = torch.empty((Vc, 2, nv), dtype=c128, device="cuda")
+    out_f = lq.empty_spinor(L, dtype=torch.float64)
+    lq.restrict(out_c, x, vn, L, b, nv)
+    lq.prolong(out_f, xc, vn, L, b, nv)
+    ref_r = oracle.restrict(psi[real_d].cpu().numpy(), v_fake, fdims, b)
+    assert rel_l2(out_c[Xreal_d].cpu().numpy(), ref_r) <= TOL64
+    ref_p = oracle.prolong(xc[Xreal_d].cpu().numpy(), v_fake, fdims, b)
+    assert rel_l2(lq.unpack_spinor(out_f, L)[real_d].cpu().numpy(), ref_p) <= TOL64
