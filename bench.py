@@ -839,6 +839,67 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         print(json.dumps(line), flush=True)
 
 
+ROW_MODELS = {  # rows that --rows can time alone -> (Workload method, model of its algorithmic bytes / flops)
+    "wilson_clover": lambda c, m: m["wilson_clover"], "wilson_clover_dagger": lambda c, m: m["wilson_clover"],
+    "restrict": lambda c, m: m["restrict"], "coarse_mult": lambda c, m: m["coarse_mult"],
+    "prolong": lambda c, m: m["prolong"],
+    "wilson_clover_12": lambda c, m: model(c, links12=True)["wilson_clover"],
+    "wilson_clover_dd": lambda c, m: model_dsap(c, 0), "wilson_clover_dd_even": lambda c, m: model_dsap(c, 1),
+    "mr_even": lambda c, m: model_sap(c)["mr"], "sap": lambda c, m: model_sap(c)["sap"],
+    "fine_mrhs": lambda c, m: {"bytes": (576 + 2 * 192) * c.volume, "flops": 2 * m["wilson_clover"]["flops"]},
+    "coarse_mrhs": lambda c, m: {"bytes": m["coarse_mult"]["bytes"] + 2 * 16 * c.cvolume * 2 * c.nvec * 8,
+                                 "flops": 16 * m["coarse_mult"]["flops"]},
+    "coarse_mult_half": lambda c, m: model_coarse_half(c),
+}
+
+
+def model_coarse_half(cfg: li.Config, real_bytes: int = 4) -> dict:
+    """Half-storage coarse operator: A_0 and the four forward blocks are stored, the backward blocks
+    come from the neighbour's forward block (A_-mu(X) = G5c A_+mu(X-mu)^dag G5c): 5 blocks per coarse site."""
+    Vc, N = cfg.cvolume, 2 * cfg.nvec
+    w = real_bytes // 4
+    return {"bytes": (5 * N * N * 8 + 2 * N * 8) * Vc * w, "flops": 9 * N * N * 8 * Vc, "units": Vc}
+
+
+def prepare_row(W: Workload, name: str):
+    """Buffers that some rows need beside the Workload's own (fp32)."""
+    import torch
+    cfg = W.cfg
+    if name == "fine_mrhs" and not hasattr(W, "x2"):
+        W.x2 = [torch.stack([W.x[0], W.x[1]]), torch.stack([W.x[2], W.x[3]])]
+        W.y2 = [torch.empty_like(W.x2[0]), torch.empty_like(W.x2[1])]
+    if name == "coarse_mrhs" and not hasattr(W, "xcK"):
+        gk = torch.Generator(device=W.dev)
+        gk.manual_seed(4242)
+        W.xcK = torch.view_as_complex(torch.randn((16, cfg.cvolume, 2, cfg.nvec, 2), generator=gk, device=W.dev,
+                                                  dtype=torch.float32))
+        W.ycK = torch.empty_like(W.xcK)
+
+
+def run_rows(args, cfg: li.Config):
+    """--rows a,b,...: each named row timed alone (CUDA events, rotating buffers); one JSON line.  This is the command
+    the per-kernel ncu captures under profiles/ run."""
+    import torch
+    torch.cuda.set_device(0)
+    device = torch.device("cuda", 0)
+    W = Workload(cfg, device, seed=cfg.seed, synthetic_operators=args.synthetic_operators, precision=args.precision)
+    m = model(cfg, real_bytes=8 if args.precision == "f64" else 4)
+    peak, peak_src = measured_peak()
+    sampler = ClockSampler(0)
+    sampler.start()
+    out = {}
+    for name in args.rows.split(","):
+        prepare_row(W, name)
+        t = time_single(W, name, reps=args.steps, warmup=args.warmup)
+        md = ROW_MODELS[name](cfg, m)
+        out[name] = {"us": t * 1e6, "GBps": md["bytes"] / t / 1e9, "GFLOPs": md["flops"] / t / 1e9,
+                     "frac_of_hbm_peak": md["bytes"] / t / 1e9 / peak, "bytes_per_launch": md["bytes"]}
+    clocks = sampler.stop()
+    print(json.dumps({"metric": METRIC, "rows": out, "unit": "GB/s", "peak": peak, "peak_source": peak_src,
+                      "workload": cfg.name, "dtype": args.precision, "data": "synthetic", "steps": args.steps,
+                      "warmup": args.warmup, "clocks": clocks}), flush=True)
+
+
 def run_sweep(args):
     """Config 5's bandwidth-roofline sweep: the fp32 fine operator (and D^dag) and the coarse operator over volumes
     8^3x16 ... 48^3x96 (and the matching coarse lattices, block 4^4, nvec 32): algorithmic GB/s versus footprint,
@@ -921,10 +982,15 @@ def main():
     ap.add_argument("--synthetic-operators", action="store_true",
                     help="random clover term and coarse matrix instead of the device-built ones (DESIGN.md section 4)")
     ap.add_argument("--sweep", action="store_true", help="config 5's bandwidth-roofline sweep over volumes (1 GPU)")
+    ap.add_argument("--rows", default=None, metavar="ROW[,ROW...]",
+                    help="time the named rows alone (1 GPU; %s)" % ", ".join(sorted(ROW_MODELS)))
     args = ap.parse_args()
     cfg = li.CONFIGS[args.workload]
     if args.sweep:
         run_sweep(args)
+        return
+    if args.rows:
+        run_rows(args, cfg)
         return
     if args.impl == "reference":
         # rank 0 alone runs the oracle; the other ranks exit 0 without work (no process group needed)

@@ -195,9 +195,13 @@ int lqcd_clover_from_links_f64(double* clover_native, const double* U_native18, 
 /* Block orthonormalisation of the null vectors, in place on the NATIVE null-vector array: within
  * every aggregate (X, chi) the nvec vectors are orthonormalised in index order (Gram-Schmidt, each vector projected
  * twice against its predecessors; the result is the unique Q of the QR factorisation with positive diagonal).
- * Requires |block| * 6 >= nvec; linearly dependent input yields non-finite output. */
+ * Requires |block| * 6 >= nvec.  Aggregate-local: any coarse extent >= 1.  A vector with nothing left after the
+ * projections (zero or non-finite norm: e.g. a zero input vector) is written as ZERO, never Inf/NaN, and counted;
+ * lqcd_orthonormalize_degenerate_count synchronises `stream`, returns the number of such (aggregate, vector) pairs of
+ * the current device since the last query (0 = P has full rank everywhere) and resets it; < 0 on a CUDA error. */
 int lqcd_orthonormalize_blocks_f32(float* nullvecs, const int dims[4], const int block[4], int nvec, void* stream);
 int lqcd_orthonormalize_blocks_f64(double* nullvecs, const int dims[4], const int block[4], int nvec, void* stream);
+long long lqcd_orthonormalize_degenerate_count(void* stream);
 /* Galerkin coarse operator, Eq. 7: A[X][d][I][J] = <I| D_d |J> for the nine pieces of D (d = 0: the
  * site-diagonal term and the hops inside the aggregate; 1 + 2 mu / 2 + 2 mu: the forward / backward hops that leave
  * it), coarse-matrix layout as consumed by lqcd_coarse_mult.  U: native 18-real gauge; nullvecs: native, block-
@@ -213,7 +217,8 @@ int lqcd_galerkin_coarse_f64(double* A, const double* U, const double* clover, c
 
 /* ---- F3: Richardson residual, blocked BLAS-1, inner-domain solver, SAP --------
  * Residual of one Richardson refinement "|x> + M_i(|b> - D|x>)" and of the SAP listing (PAPER.md:
- * 128-131) in one pass:  r = b - D x.  r must not alias x (it may alias b).  flags: LQCD_LINKS_12 only. */
+ * 128-131) in one pass:  r = b - D x.  r must alias neither x nor b (b is read through the read-only data path;
+ * LQCD_EINVAL otherwise).  flags: LQCD_LINKS_12 only. */
 int lqcd_wilson_clover_residual_f32(float* r, const float* b, const float* x, const float* U, const float* clover,
                                     float kappa, const int dims[4], const int bc[4], unsigned flags, void* stream);
 int lqcd_wilson_clover_residual_f64(double* r, const double* b, const double* x, const double* U,

@@ -35,6 +35,7 @@ SIGNATURES = {
     "lqcd_host_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_host_workspace_bytes_f64": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_galerkin_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
+    "lqcd_orthonormalize_degenerate_count": (C.c_longlong, [_vp]),
     "lqcd_mr_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_coarse_bicgstab_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci]),
     "lqcd_mg_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
@@ -111,6 +112,11 @@ def load():
             if not os.path.exists(path):
                 raise RuntimeError(
                     f"liblqcd_b200.so is missing and could not be built ({e}); there is no CPU fallback") from e
+            if os.environ.get("LQCD_REQUIRE_FRESH"):
+                raise RuntimeError(f"liblqcd_b200.so is older than its sources and the rebuild failed ({e})") from e
+            import warnings
+            warnings.warn(f"liblqcd_b200.so is OLDER than its sources and the rebuild failed ({e}): loading the stale "
+                          "library (set LQCD_REQUIRE_FRESH=1 to make this an error)", RuntimeWarning, stacklevel=2)
     lib = C.CDLL(path)
     for name, (res, args) in SIGNATURES.items():
         fn = getattr(lib, name)  # AttributeError if the header and the library disagree

@@ -40,8 +40,8 @@ inline int transfer_setup(TransferParams& P, const void* a, const void* b, const
         set_error("%s: pointers must be 16-byte aligned", what);
         return LQCD_EINVAL;
     }
-    if (check_block(dims, block, nvec, P.Lc)) {
-        set_error("%s: bad dims/block/nvec (block must divide dims, coarse extents >= 2, nvec >= 1)", what);
+    if (check_block_local(dims, block, nvec, P.Lc)) {  // aggregate-local: any coarse extent >= 1
+        set_error("%s: bad dims/block/nvec (block must divide dims, nvec >= 1)", what);
         return LQCD_EINVAL;
     }
     if (volume(dims) > 0x7fffffffLL) return LQCD_EUNSUPPORTED;

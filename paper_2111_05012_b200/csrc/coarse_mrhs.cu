@@ -443,26 +443,8 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
     }
 }
 
-static int mrhs_max_smem() {
-    static int v = -1;
-    if (v < 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) v = 0;
-        cudaGetLastError();
-    }
-    return v;
-}
-static int mrhs_sm_count() {
-    static int v = -1;
-    if (v < 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v < 1) v = 148;
-        cudaGetLastError();
-    }
-    return v;
-}
+static int mrhs_max_smem() { return max_optin_smem(); }
+static int mrhs_sm_count() { return sm_count(); }
 
 // one tensor-core launch for up to 16 right-hand sides
 template <int NCOL>
@@ -478,11 +460,8 @@ static int mrhs_launch_ncol(float* out, const float* in, const float* A, MrhsPar
     P.slots = mr_max_stages(NCOL) / MR_ISSUERS * MR_ISSUERS;
     P.stages = S;
     const size_t smem = S * stage + MR_ROWS * NCOL * 4 + (2 * S + 2 * 8) * 8 + 16;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(k_coarse_mrhs<NCOL>, cudaFuncAttributeMaxDynamicSharedMemorySize, mrhs_max_smem());
-        attr = true;
-    }
+    static unsigned long long attr = 0;
+    ensure_dynamic_smem(k_coarse_mrhs<NCOL>, mrhs_max_smem(), attr);
     const int grid = P.Vc < mrhs_sm_count() ? P.Vc : mrhs_sm_count();
     k_coarse_mrhs<NCOL><<<grid, MR_THREADS, smem, st>>>(out, in, A, P);
     count_launch();

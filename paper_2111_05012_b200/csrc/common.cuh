@@ -31,15 +31,35 @@ inline int check_dims(const int dims[4]) {
 inline long long volume(const int d[4]) { return (long long)d[0] * d[1] * d[2] * d[3]; }
 inline long long nchunks(const int d[4]) { return (volume(d) + CH - 1) / CH; }
 
-// block must divide dims, coarse extents >= 2 (reading Q8)
-inline int check_block(const int dims[4], const int block[4], int nvec, int cdims[4]) {
+// block must divide dims.  The aggregate-local operations (restrict, prolong, null-vector packing and
+// orthonormalisation) accept any coarse extent >= 1 -- a rank of a sharded lattice may be one aggregate thick;
+// whatever applies the periodic 9-point coarse stencil needs coarse extents >= 2 (reading Q8).
+inline int check_block_local(const int dims[4], const int block[4], int nvec, int cdims[4]) {
     if (check_dims(dims) || !block || nvec < 1) return LQCD_EINVAL;
     for (int mu = 0; mu < 4; mu++) {
         if (block[mu] < 1 || dims[mu] % block[mu]) return LQCD_EINVAL;
         cdims[mu] = dims[mu] / block[mu];
-        if (cdims[mu] < 2) return LQCD_EINVAL;
     }
     return LQCD_OK;
+}
+inline int check_block(const int dims[4], const int block[4], int nvec, int cdims[4]) {
+    if (check_block_local(dims, block, nvec, cdims)) return LQCD_EINVAL;
+    for (int mu = 0; mu < 4; mu++)
+        if (cdims[mu] < 2) return LQCD_EINVAL;
+    return LQCD_OK;
+}
+
+// ---- per-device facts and one-time kernel attributes (a process may drive several devices) -----------
+int max_optin_smem();  // cudaDevAttrMaxSharedMemoryPerBlockOptin of the current device
+int sm_count();        // cudaDevAttrMultiProcessorCount of the current device
+int current_device();
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (kernel instantiation, device): `done` is the call
+// site's static bit mask of devices already served
+template <typename Kern> inline void ensure_dynamic_smem(Kern kern, int bytes, unsigned long long& done) {
+    const int d = current_device();
+    if (d >= 0 && d < 64 && ((done >> d) & 1ull)) return;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (d >= 0 && d < 64) done |= 1ull << d;
 }
 
 // ---- 16-byte vectors ----------------------------------------------------------------------------
@@ -72,11 +92,12 @@ template <typename T> __device__ __forceinline__ V16<T> ld16(const T* p) {
 template <typename T> __device__ __forceinline__ V16<T> ld16_g64(const T* p) {
     V16<T> v;
     if constexpr (sizeof(T) == 4)
-        asm("ld.global.L2::64B.v4.f32 {%0,%1,%2,%3}, [%4];"
-            : "=f"(v.r[0]), "=f"(v.r[1]), "=f"(v.r[2]), "=f"(v.r[3])
-            : "l"(p));
+        asm volatile("ld.global.L2::64B.v4.f32 {%0,%1,%2,%3}, [%4];"
+                     : "=f"(v.r[0]), "=f"(v.r[1]), "=f"(v.r[2]), "=f"(v.r[3])
+                     : "l"(p)
+                     : "memory");  // an ordinary (coherent) load of memory the kernel may also store to
     else
-        asm("ld.global.L2::64B.v2.f64 {%0,%1}, [%2];" : "=d"(v.r[0]), "=d"(v.r[1]) : "l"(p));
+        asm volatile("ld.global.L2::64B.v2.f64 {%0,%1}, [%2];" : "=d"(v.r[0]), "=d"(v.r[1]) : "l"(p) : "memory");
     return v;
 }
 template <typename T> __device__ __forceinline__ V16<T> ld16_stream_g64(const T* p) {

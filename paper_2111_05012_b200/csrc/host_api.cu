@@ -68,7 +68,7 @@ size_t host_ws_bytes(const int dims[4], const int block[4], int nvec, size_t rb)
     size_t fine_n = up256(lqcd_native_spinor_reals(dims) * rb);
     size_t coarse = 0;
     int cd[4];
-    if (block && nvec >= 1 && check_block(dims, block, nvec, cd) == LQCD_OK)
+    if (block && nvec >= 1 && check_block_local(dims, block, nvec, cd) == LQCD_OK)
         coarse = up256((size_t)volume(cd) * 4 * nvec * rb);
     return fine_c + 2 * fine_n + 2 * coarse;
 }
@@ -121,7 +121,7 @@ int restrict_host(const char* what, T* out_c_host, const T* in_f_host, const T* 
                   const int block[4], int nvec, void* ws_dev, void* stream) {
     clear_error();
     int cd[4];
-    if (!out_c_host || !in_f_host || !ws_dev || check_block(dims, block, nvec, cd) || !aligned16(ws_dev)) {
+    if (!out_c_host || !in_f_host || !ws_dev || check_block_local(dims, block, nvec, cd) || !aligned16(ws_dev)) {
         set_error("%s: invalid argument", what);
         return LQCD_EINVAL;
     }
@@ -146,7 +146,7 @@ int prolong_host(const char* what, T* out_f_host, const T* in_c_host, const T* n
                  const int block[4], int nvec, void* ws_dev, void* stream) {
     clear_error();
     int cd[4];
-    if (!out_f_host || !in_c_host || !ws_dev || check_block(dims, block, nvec, cd) || !aligned16(ws_dev)) {
+    if (!out_f_host || !in_c_host || !ws_dev || check_block_local(dims, block, nvec, cd) || !aligned16(ws_dev)) {
         set_error("%s: invalid argument", what);
         return LQCD_EINVAL;
     }

@@ -1,4 +1,5 @@
-// knobs.h -- process-wide tuning knobs (lqcd_set_fine_tile / lqcd_set_knob). Results never depend on them.
+// knobs.h -- tuning knobs (lqcd_set_fine_tile / lqcd_set_knob), one set per calling host thread like the last-error
+// string: two threads with different settings do not race.  Results never depend on them.
 #pragma once
 namespace lqcd {
 struct Knobs {
@@ -15,5 +16,5 @@ struct Knobs {
     int sap_fused = 0;                // 0 = shared-memory-resident inner-domain solver when it fits; -1 = never
     int sap_group_residual = 0;       // 0 = SAP's intermediate residuals on the next group's domains only; -1 = all sites
 };
-extern Knobs g_knobs;
+extern thread_local Knobs g_knobs;
 }  // namespace lqcd

@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bicg_xr(T* __restrict__ x, T* _
 
 // rho' = <rt|r>;  beta = (alpha / omega) (rho' / rho);  p = r + beta (p - omega v);  rho := rho'
 template <typename T>
-__global__ void __launch_bounds__(RED_THREADS) k_bicg_p(T* __restrict__ p_out, const T* __restrict__ p_in,
+__global__ void __launch_bounds__(RED_THREADS) k_bicg_p(T* p_out, const T* p_in,  // may alias (p updated in place)
                                                          const T* __restrict__ r, const T* __restrict__ v,
                                                          const T* __restrict__ part, T* __restrict__ sc, int it,
                                                          long long n) {

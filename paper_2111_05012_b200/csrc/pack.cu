@@ -181,7 +181,7 @@ static int nullvec_call(T* native, T* canon, int i, const int dims[4], const int
                         const char* what) {
     clear_error();
     BlockGeom g;
-    if (!native || !canon || check_block(dims, block, nvec, g.Lc) || i < 0 || i >= nvec || !aligned16(native) ||
+    if (!native || !canon || check_block_local(dims, block, nvec, g.Lc) || i < 0 || i >= nvec || !aligned16(native) ||
         !aligned16(canon)) {
         set_error("%s: invalid argument", what);
         return LQCD_EINVAL;

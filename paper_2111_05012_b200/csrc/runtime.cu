@@ -28,7 +28,36 @@ int check_launch(const char* what) {
     return LQCD_OK;
 }
 
-Knobs g_knobs;
+thread_local Knobs g_knobs;
+
+int current_device() {
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess) {
+        cudaGetLastError();
+        return -1;
+    }
+    return d;
+}
+static int device_attr(cudaDeviceAttr which, int* cache, int fallback) {
+    const int d = current_device();
+    if (d < 0) return fallback;
+    if (d < 64 && cache[d] > 0) return cache[d];
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, which, d) != cudaSuccess || v < 1) {
+        cudaGetLastError();
+        return fallback;
+    }
+    if (d < 64) cache[d] = v;  // racing writers store the same value
+    return v;
+}
+int max_optin_smem() {
+    static int cache[64];
+    return device_attr(cudaDevAttrMaxSharedMemoryPerBlockOptin, cache, 0);
+}
+int sm_count() {
+    static int cache[64];
+    return device_attr(cudaDevAttrMultiProcessorCount, cache, 148);
+}
 
 }  // namespace lqcd
 
@@ -95,7 +124,7 @@ size_t lqcd_native_clover_reals(const int dims[4]) {
 }
 size_t lqcd_native_nullvecs_reals(const int dims[4], const int block[4], int nvec) {
     int cd[4];
-    if (check_block(dims, block, nvec, cd)) return 0;
+    if (check_block_local(dims, block, nvec, cd)) return 0;
     return (size_t)volume(dims) * 24 * (size_t)nvec;
 }
 size_t lqcd_native_coarse_vec_reals(const int cdims[4], int nvec) {

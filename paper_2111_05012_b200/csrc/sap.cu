@@ -558,17 +558,6 @@ static int dom_setup(DomParams& P, const int dims[4], const int bc[4], const int
 
 template <typename T> static size_t mr_smem_bytes(int bv) { return MrSmem<T>::bytes(bv, (bv + 31) / 32 * 32); }
 
-static int max_optin_smem() {
-    static int v = -1;
-    if (v < 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) v = 0;
-        cudaGetLastError();
-    }
-    return v;
-}
-
 template <typename T> static bool mr_fits_smem(int bv) {
     return g_knobs.sap_fused >= 0 && bv <= 256 && mr_smem_bytes<T>(bv) <= (size_t)max_optin_smem();
 }
@@ -614,12 +603,8 @@ static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa
         const long long rstride = (long long)nchunks(dims) * CH * 24;  // right-hand sides back to back
 #define LAUNCH_MR(ACC, BVC)                                                                                   \
     do {                                                                                                      \
-        static bool attr = false;                                                                             \
-        if (!attr) {                                                                                          \
-            cudaFuncSetAttribute(k_mr_domain<T, ACC, BVC>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
-                                 max_optin_smem());                                                           \
-            attr = true;                                                                                      \
-        }                                                                                                     \
+        static unsigned long long attr = 0;                                                                   \
+        ensure_dynamic_smem(k_mr_domain<T, ACC, BVC>, max_optin_smem(), attr);                                \
         k_mr_domain<T, ACC, BVC><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter, K, rstride);   \
     } while (0)
         if (sizeof(T) == 4 && P.bv == 256) {  // the paper's typical 4^4 domain

@@ -215,6 +215,10 @@ static int clover_from_links_call(T* clover, const T* U, T kappa, T csw, const i
 // against its predecessors ("twice is enough"), all predecessors of one pass at once: warps own predecessors j for
 // the dot products <w_j|w_i>, threads own 16-byte slices for the update w_i -= sum_j r_j w_j.
 // ------------------------------------------------------------------------------------------------------------
+// aggregates whose vector had no component left after the projections (zero or non-finite norm): such a vector is
+// written as ZERO instead of Inf/NaN, and counted here (lqcd_orthonormalize_degenerate_count)
+__device__ unsigned long long g_ortho_degenerate;
+
 template <typename T>
 __global__ void __launch_bounds__(256) k_orthonormalize(T* __restrict__ v, TransferParams P) {
     constexpr int NV = VecOf<T>::NV, CPV = NV / 2;
@@ -284,7 +288,9 @@ __global__ void __launch_bounds__(256) k_orthonormalize(T* __restrict__ v, Trans
         __syncthreads();
         T tot = 0;
         for (int k = 0; k < W; k++) tot += red[k];
-        const T inv = (T)1 / sqrt(tot);
+        const bool ok = tot > (T)0 && tot < (T)INFINITY;  // false for 0, Inf and NaN
+        const T inv = ok ? (T)1 / sqrt(tot) : (T)0;
+        if (!ok && threadIdx.x == 0) atomicAdd(&g_ortho_degenerate, 1ull);
         for (int p = threadIdx.x; p < P.LV; p += blockDim.x) {
             V16<T> x = *reinterpret_cast<const V16<T>*>(wi + (size_t)p * NV);
 #pragma unroll
@@ -310,7 +316,8 @@ static int orthonormalize_call(T* v, const int dims[4], const int block[4], int 
         return LQCD_EUNSUPPORTED;
     }
     auto kern = k_orthonormalize<T>;
-    if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static unsigned long long attr = 0;
+    if (smem > 48 * 1024) ensure_dynamic_smem(kern, 200 * 1024, attr);
     kern<<<(unsigned)(2 * volume(P.Lc)), 256, smem, (cudaStream_t)stream>>>(v, P);
     count_launch();
     return check_launch(what);
@@ -426,6 +433,11 @@ static int galerkin_call(T* A, const T* U, const T* clover, const T* v, T kappa,
     TransferParams P;
     int rc = transfer_setup<T>(P, A, U, v, dims, block, nvec, what);
     if (rc) return rc;
+    for (int mu = 0; mu < 4; mu++)
+        if (P.Lc[mu] < 2) {  // the 9-point stencil of directed blocks needs two coarse sites per direction (Q8)
+            set_error("%s: coarse extent < 2 in direction %d", what, mu);
+            return LQCD_EINVAL;
+        }
     if (!clover || !ws || !bc || !aligned16(clover) || !aligned16(ws)) {
         set_error("%s: null or misaligned pointer", what);
         return LQCD_EINVAL;
@@ -484,6 +496,16 @@ int lqcd_orthonormalize_blocks_f32(float* nullvecs, const int dims[4], const int
 }
 int lqcd_orthonormalize_blocks_f64(double* nullvecs, const int dims[4], const int block[4], int nvec, void* stream) {
     return orthonormalize_call<double>(nullvecs, dims, block, nvec, stream, "lqcd_orthonormalize_blocks_f64");
+}
+long long lqcd_orthonormalize_degenerate_count(void* stream) {
+    unsigned long long n = 0, zero = 0;
+    if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess ||
+        cudaMemcpyFromSymbol(&n, g_ortho_degenerate, sizeof(n)) != cudaSuccess ||
+        cudaMemcpyToSymbol(g_ortho_degenerate, &zero, sizeof(zero)) != cudaSuccess) {
+        set_error("lqcd_orthonormalize_degenerate_count: %s", cudaGetErrorString(cudaGetLastError()));
+        return LQCD_ECUDA;
+    }
+    return (long long)n;
 }
 size_t lqcd_galerkin_workspace_bytes(const int dims[4], const int block[4], int nvec, int real_bytes) {
     return real_bytes == 8 ? galerkin_ws_bytes<double>(dims, block, nvec) : galerkin_ws_bytes<float>(dims, block, nvec);

@@ -297,11 +297,8 @@ int restrict_mrhs_call(T* out_c, const T* in_f, const T* v, const int dims[4], c
         return LQCD_OK;
     }
     auto kern = k_restrict_mrhs<T, 4, NRMAX>;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 108 * 1024);
-        attr = true;
-    }
+    static unsigned long long attr = 0;
+    ensure_dynamic_smem(kern, 108 * 1024, attr);
     int warps = nvec < 8 ? nvec : 8;
     const long long nagg = 2 * volume(P.Lc);
     for (int k = 0; k < nrhs; k += per) {

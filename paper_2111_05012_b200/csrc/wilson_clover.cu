@@ -301,8 +301,10 @@ int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T
         set_error("%s: out must not alias in", what);
         return LQCD_EINVAL;
     }
-    if (rhs && (!aligned16(rhs) || domain || (flags & LQCD_DAGGER))) {
-        set_error("%s: the residual form needs an aligned rhs and takes neither a domain nor LQCD_DAGGER", what);
+    if (rhs && (!aligned16(rhs) || domain || (flags & LQCD_DAGGER) || rhs == out)) {  // rhs is read through the
+        // read-only path (ld.global.nc) and out is written: the two must not overlap
+        set_error("%s: the residual form needs an aligned rhs distinct from out and takes neither a domain nor "
+                  "LQCD_DAGGER", what);
         return LQCD_EINVAL;
     }
     const unsigned allowed = LQCD_DAGGER | LQCD_LINKS_12 | (domain ? (LQCD_DOMAIN_EVEN | LQCD_DOMAIN_ODD) : 0u);
@@ -605,8 +607,9 @@ int wilson_clover_mrhs_call(T* out, const T* in, const T* U, const T* clover, co
         set_error("%s: pointers must be 16-byte aligned and out must not alias in", what);
         return LQCD_EINVAL;
     }
-    if ((flags & ~(LQCD_DAGGER | LQCD_LINKS_12)) || (rhs && ((flags & LQCD_DAGGER) || !aligned16(rhs)))) {
-        set_error("%s: unknown flag bits 0x%x (the residual form takes no LQCD_DAGGER)", what, flags);
+    if ((flags & ~(LQCD_DAGGER | LQCD_LINKS_12)) || (rhs && ((flags & LQCD_DAGGER) || !aligned16(rhs) || rhs == out))) {
+        set_error("%s: unknown flag bits 0x%x (the residual form takes no LQCD_DAGGER and needs rhs distinct from out)",
+                  what, flags);
         return LQCD_EINVAL;
     }
     if (volume(dims) > 0x7fffffffLL) {

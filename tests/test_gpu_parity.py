@@ -282,14 +282,20 @@ def test_wilson_clover_edge_lattices(lq, prec, dims, bc):
     ((4, 4, 4, 8), (2, 2, 2, 2), 1),     # nvec = 1 (N = 2)
     ((8, 4, 4, 4), (2, 2, 2, 2), 20),    # N = 40: rows not a power of two
     ((4, 4, 4, 4), (2, 2, 2, 2), 40),    # N = 80 > 64: several vec16 per lane per row
+    ((4, 4, 8, 4), (4, 4, 4, 4), 5),     # one aggregate thick in x, y, t (coarse 1x1x2x1): the transfers only
 ])
 def test_coarse_and_transfer_edge_sizes(lq, prec, dims, block, nvec):
     cfg = custom_config(dims, block, nvec)
+    thin = min(cfg.cdims) < 2    # aggregate-local operations accept it; the coarse stencil does not (Q8)
     prob = make_problem(cfg, coarse="galerkin" if nvec <= 4 else "synthetic")
     d = Dev(lq, prob, prec)
     psi = prob.psi[0]
     v, A = rounded(prob.v, prec), rounded(prob.A, prec)
     for dagger in (False, True):
+        if thin:
+            with pytest.raises(lq.LqcdError):
+                d.Dc(prob.xc, dagger=dagger)
+            continue
         ref = oracle.coarse_mult(rounded(prob.xc, prec), A, cfg.cdims, dagger=dagger)
         assert rel_l2(d.Dc(prob.xc, dagger=dagger), ref) <= TOL[prec]
     assert rel_l2(d.R(psi), oracle.restrict(rounded(psi, prec), v, cfg.dims, cfg.block)) <= TOL[prec]
@@ -337,13 +343,22 @@ def test_error_codes(lq):
     assert code(lambda: lq.wilson_clover_mult(x, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc)) == lq.EINVAL
     assert code(lambda: lq.wilson_clover_mult(y, x, d.U, d.clover, cfg.kappa, cfg.dims, (1, 1, 1, 0))) == lq.EINVAL
     assert code(lambda: lq.wilson_clover_mult(y, x, d.U, d.clover, cfg.kappa, (4, 4, 4, 0), cfg.bc)) == lq.EINVAL
-    assert code(lambda: lq.wilson_clover_mult(y[1:], x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc)) == lq.EINVAL
+    # a tensor of the wrong size never reaches the C call (the binding knows the sizes, tests/test_binding_checks.py) ...
+    with pytest.raises(ValueError, match="needs"):
+        lq.wilson_clover_mult(y[1:], x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc)
+    # ... and the C call itself refuses a pointer that is not 16-byte aligned
+    i4, st = lq._i4, torch.cuda.current_stream().cuda_stream
+    rc = lq.lib().lqcd_wilson_clover_mult_f32(y.data_ptr() + 4, x.data_ptr(), d.U.data_ptr(), d.clover.data_ptr(),
+                                              cfg.kappa, i4(cfg.dims), i4(cfg.bc), 0, st)
+    assert rc == lq.EINVAL and "aligned" in lq.last_error()
     xc = to_dev(prob.xc, "f32")
     yc = torch.empty_like(xc)
-    assert code(lambda: lq.coarse_mult(yc, xc, d.A, (2, 2, 2, 1), cfg.nvec)) == lq.EINVAL
+    with pytest.raises(ValueError, match="needs"):
+        lq.coarse_mult(yc, xc, d.A, (2, 2, 2, 1), cfg.nvec)
+    rc = lq.lib().lqcd_coarse_mult_f32(yc.data_ptr(), xc.data_ptr(), d.A.data_ptr(), i4((2, 2, 2, 1)), cfg.nvec, 0, st)
+    assert rc == lq.EINVAL, "the 9-point coarse stencil needs coarse extents >= 2 (DESIGN.md Q8)"
     assert code(lambda: lq.coarse_mult(xc, xc, d.A, cfg.cdims, cfg.nvec)) == lq.EINVAL
     assert code(lambda: lq.restrict(yc, x, d.v, cfg.dims, (3, 2, 2, 2), cfg.nvec)) == lq.EINVAL
-    assert code(lambda: lq.restrict(yc, x, d.v, cfg.dims, (4, 4, 4, 4), cfg.nvec)) == lq.EINVAL  # coarse extent 1
     assert code(lambda: lq.prolong(y, yc, d.v, cfg.dims, cfg.block, 0)) == lq.EINVAL
     assert "lqcd_prolong_f32" in lq.last_error()
     dd = lambda **kw: lq.wilson_clover_dd_mult(y, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, **kw)

@@ -89,9 +89,11 @@ def test_residual(lq, prec, links12):
     U, clov = fields(prob, prec)
     ref = rounded(b, prec) - oracle.wilson_clover_mult(rounded(x, prec), U, clov, cfg.kappa, cfg.dims, cfg.bc)
     assert rel_l2(lq.unpack_spinor(r, cfg.dims).cpu().numpy(), ref) <= TOL1[prec]
-    # r may alias b
-    lq.wilson_clover_residual(bn, bn, xn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, links12=links12)
-    assert rel_l2(lq.unpack_spinor(bn, cfg.dims).cpu().numpy(), ref) <= TOL1[prec]
+    # r must alias neither b (read through the read-only path) nor x: refused, nothing enqueued
+    for bad in (bn, xn):
+        with pytest.raises(lq.LqcdError) as e:
+            lq.wilson_clover_residual(bad, bn, xn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, links12=links12)
+        assert e.value.code == lq.EINVAL
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
