@@ -2,8 +2,7 @@
 
 `python -m paper_2111_05012_b200.build [--force] [--verbose]`.  nvcc cross-compiles without a GPU.  The
 library is built IN-TREE (git-ignored, but it travels to the GPU box with the repo snapshot).
-Extra nvcc flags for development builds come from the environment variable LQCD_NVCC_EXTRA (e.g.
-"-DLQCD_MRHS_TRACE": per-role clock stamps and a spin watchdog in the tensor-core kernel, csrc/coarse_mrhs.cu).
+Extra nvcc flags for development builds come from the environment variable LQCD_NVCC_EXTRA.
 """
 from __future__ import annotations
 

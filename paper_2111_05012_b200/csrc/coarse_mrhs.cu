@@ -4,47 +4,75 @@
 //
 // With K right-hand sides every block A_d(X) is re-used K times: the arithmetic intensity is K flop/byte and the
 // operation per coarse site is a dense contraction (N x 9N complex) . (9N x K complex) -- the one place of this path
-// where tensor cores belong.  Per site, in REAL arithmetic on the interleaved (re, im)
+// where tensor cores belong.  Per block, in REAL arithmetic on the interleaved (re, im)
 // storage:  C[r][(k,re)] = sum_j (a_r[2j] b_kj.re - a_r[2j+1] b_kj.im),  C[r][(k,im)] = sum_j (a_r[2j] b_kj.im +
-// a_r[2j+1] b_kj.re), i.e. C (64 x 2K) = A (64 x 1152, the rows of the nine blocks as stored) . B' (1152 x 2K) with
+// a_r[2j+1] b_kj.re), i.e. C (64 x 2K) = A (64 x 128, the rows of the block as stored) . B' (128 x 2K) with
 // B'[(2j, 2j+1)][(k,re)] = (b.re, -b.im), B'[(2j, 2j+1)][(k,im)] = (b.im, b.re).
 //
 // tcgen05 (5th-generation tensor cores): kind::tf32 MMAs with fp32 accumulators in TMEM.  TF32 alone (10-bit mantissa)
 // would miss the fp32 bar of 2e-6 by two orders of magnitude, so every fp32 operand is split into hi + lo
-// (hi = x rounded to the nearest TF32 value, i.e. 13 low mantissa bits cleared; lo = x - hi, exact, either sign) and each
-// product is formed from the hi / lo pieces ("3xTF32"; with the stacked operands below all four terms come out).  The split is done
-// by the producer warps on the way from HBM to shared memory, so A is still read from HBM exactly once, as fp32.
+// (hi = x rounded to the nearest TF32 value; lo = x - hi, exact) and the product is hi.hi + lo.hi + hi.lo (lo.lo,
+// 2^-22 relative, is dropped) -- "3xTF32".
 //
-// One persistent CTA per SM, warp-specialised (704 threads):
-//   warps 0-3   epilogue: tcgen05.ld each accumulator chain, add it in registers (fp32, round-to-nearest), store out_k(X)
-//   warps 4-5   MMA issuers (one elected lane each, accumulator chains in turn); warp 4 allocates / frees TMEM
-//   warps 6-21  producers, four groups of four warps that take the stages in turn: stream A (whole 128-byte lines,
-//               L1 no-allocate), build B' from the neighbours' input vectors (L2-resident), split into hi / lo, store
-//               both in the 128-byte-swizzled K-major layout UMMA reads (conflict-free stores)
-// Shared-memory ring of 4 stages (one stage = half a block: A as 128 rows (hi | lo) x 64 reals, B' as 4K rows
-// (hi | lo) x 64 reals), a ring of TMEM accumulator slots (one per chain of two stages); mbarriers full[] (producers ->
-// issuer), done[] (tcgen05.commit -> producers), tfull[] (tcgen05.commit -> epilogue), tfree[] (epilogue -> issuer).
+// Data path of the matrix (DESIGN.md section 6.8 -- why not "split into shared memory"): at the HBM rate an SM takes
+// in ~28 B/clk of A; shared memory moves 128 B/clk.  A split written back to shared memory costs 5 bytes of
+// shared-memory traffic per byte of A (TMA write, read, lo write, two operand reads by the tensor core) plus the
+// traffic of B' -- more than the pipe has.  Here A goes  HBM --TMA--> shared memory (raw fp32, 128B-swizzled, a ring
+// of whole blocks, no register ever holds a load across a hand-over) --ld.shared--> registers (split) --tcgen05.st-->
+// TENSOR MEMORY, and the MMAs take their A operand from tensor memory (hi in columns 0-63, lo in columns 64-127 of
+// the same lane): 2 bytes of shared-memory traffic per byte of A.  Only B' (built from the L2-resident input
+// vectors) is a shared-memory operand.
+//
+// UMMA shape: a block has 64 rows but M = 64 runs at half rate, so the two halves of the contraction index are
+// stacked: TMEM lane 64 h + r holds row r, reals 64 h .. 64 h + 63 (h = 0, 1), and B' carries the rows of both halves
+// side by side (N index = h * NCOL + (k, re|im)); the accumulator is then block-diagonal -- lanes of half h use the
+// columns of half h, the other half of the products is discarded (the tensor pipe has the room: 64 % busy at the
+// HBM roofline for K = 16) -- and the two halves are added by the epilogue.
+//
+// One persistent CTA per SM, warp-specialised (608 threads):
+//   warps 0-3    epilogue: tcgen05.ld the accumulators of every block, add them in registers (fp32, round to
+//                nearest: the tensor core adds by truncation, so chains are kept to one block), store out_k(X)
+//   warps 4-11   converters: raw A tile -> (hi, lo) -> tensor memory (warp w owns TMEM lanes 32 (w % 4) ..)
+//   warps 12-19  B' builders: neighbour's input vectors (L2) -> rows (b.re, -b.im), (b.im, b.re), hi / lo, swizzled
+//   warp 20      MMA issuer  (one lane each): issuer m takes the blocks g = m, m + 2, ... (= accumulator / A / B' slot
+//                m), so every accumulator sees its MMAs in program order.  Two, because ISSUING is the narrow place:
+//                ptxas wraps every tcgen05.mma of a divergent region in an ELECT / BRA.U.ANY loop (~60 cycles per
+//                instruction, measured), more than these small MMAs (32-64 cycles) take to execute.  Warp 16 allocates
+//                and frees tensor memory
+//   warp 18      TMA producer (one lane): cp.async.bulk.tensor of the next block as soon as a ring slot is free
+// mbarriers where the hardware arrives: raw_full[S] (TMA complete_tx -> converters), done[2] (tcgen05.commit ->
+// converters, builders, epilogue); named barriers (bar.arrive / bar.sync) for the hand-overs between warps: converters
+// -> TMA producer (ring slot read), converters + builders -> issuer (operands written), epilogue -> issuer.
+#include <cuda.h>  // CUtensorMap and its enums only: the encoder is fetched through cudaGetDriverEntryPoint
+
 #include "common.cuh"
 #include "knobs.h"
 
 namespace lqcd {
 
-constexpr int MR_ROWS = 64;          // N = 2 nvec = 64 rows per block; hi and lo stacked: UMMA M = 128
-constexpr int MR_KT = 64;            // reals of the contraction index per stage (half a block)
-constexpr int MR_HALVES = 18;        // 9 blocks x 2 halves per coarse site
-constexpr int MR_AS = 2;             // pipeline stages accumulated into one TMEM slot (chain of MR_AS * 8 MMAs)
-constexpr int MR_EPI_WARPS = 4, MR_PROD_GROUPS = 4, MR_PROD_WARPS = 4 * MR_PROD_GROUPS;
-constexpr int MR_ISSUERS = 2;         // MMA-issuing warps (one elected lane each); stages in turn, like the producers
-constexpr int MR_THREADS = (MR_EPI_WARPS + MR_ISSUERS + MR_PROD_WARPS) * 32;  // 704
-constexpr int MR_TMEM_COLS = 512;    // all of TMEM: one accumulator slot of 2 NCOL columns per pipeline stage
+constexpr int MR_ROWS = 64;     // N = 2 nvec = 64 rows per block
+constexpr int MR_REALS = 128;   // reals per row of a block
+constexpr int MR_BLOCKS = 9;    // blocks per coarse site
+constexpr int MR_EPI_WARPS = 4, MR_CONV_WARPS = 8, MR_B_WARPS = 8;
+constexpr int MR_WARP_CONV = MR_EPI_WARPS, MR_WARP_B = MR_WARP_CONV + MR_CONV_WARPS;
+constexpr int MR_B_AHEAD = 4;                       // blocks the B' builders' L2 prefetch runs ahead
+#ifndef LQCD_MR_ISSUERS
+#define LQCD_MR_ISSUERS 1
+#endif
+constexpr int MR_ISSUERS = LQCD_MR_ISSUERS;                       // = accumulator slots = A slots = B' slots
+constexpr int MR_WARP_MMA = MR_WARP_B + MR_B_WARPS, MR_WARP_TMA = MR_WARP_MMA + MR_ISSUERS;
+constexpr int MR_THREADS = (MR_WARP_TMA + 1) * 32;  // 608
+constexpr int MR_TMEM_COLS = 512;                   // all of tensor memory
+constexpr int MR_A_COLS = 128;                      // one A slot: hi (64 columns) | lo (64 columns), 128 lanes
+constexpr unsigned MR_RAW_BYTES = MR_ROWS * MR_REALS * 4;  // 32 KB: one raw block
+static_assert(MR_WARP_CONV % 4 == 0 && MR_CONV_WARPS % 4 == 0, "a warp reaches TMEM lanes 32 (warp % 4) .. only");
 
 struct MrhsParams {
     int Lc[4];
     FastDiv dLc[3];  // division by Lc[0..2] as a multiply-high
     int Vc;
-    int nrhs;     // K
-    int stages;      // shared-memory pipeline stages
-    int slots;       // TMEM accumulator slots (2 NCOL columns each); a multiple of groups
+    int nrhs;           // K
+    int stages;         // raw-block ring slots
     long long vstride;  // reals between consecutive right-hand sides: Vc * 128
 };
 
@@ -56,23 +84,16 @@ __device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
 __device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// Developer aid (compiled only with -DLQCD_MRHS_TRACE): clock64 stamps of CTA 0's three roles for the first 128 stages.
-#ifdef LQCD_MRHS_TRACE
-__device__ long long g_mr_trace[3][128][6];
-#define MR_TRACE(role, idx, which)                                                                \
-    do {                                                                                          \
-        if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (idx) < 128) g_mr_trace[role][idx][which] = clock64(); \
-    } while (0)
-#else
-#define MR_TRACE(role, idx, which)
-#endif
-// spin on the phase parity (one lane; see mbar_wait)
-#ifdef LQCD_MRHS_TRACE
-__device__ int g_mr_hang[64][4];
-__device__ int g_mr_hang_n;
-__device__ __forceinline__ void mbar_wait_lane(unsigned long long* bar, unsigned parity, int tag = 0, int g = 0) {
-    for (int n = 0; n < (1 << 22); n++) {
-        unsigned ok;
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// One lane waits for the phase of parity `parity` to complete (try_wait suspends the thread for a bounded time, so
+// this is not a hot spin).  A wait that lasts longer than ~2 s of SM clock can only be a protocol error: trap, so that
+// the launch fails with an error instead of hanging the device.
+__device__ __forceinline__ void mbar_wait_lane(unsigned long long* bar, unsigned parity) {
+    unsigned ok;
+    long long t0 = 0;
+    for (unsigned n = 0;; n++) {
         asm volatile(
             "{\n"
             ".reg .pred p;\n"
@@ -83,36 +104,47 @@ __device__ __forceinline__ void mbar_wait_lane(unsigned long long* bar, unsigned
             : "r"(smem_u32(bar)), "r"(parity)
             : "memory");
         if (ok) return;
-    }
-    const int i = atomicAdd(&g_mr_hang_n, 1);
-    if (i < 64) {
-        g_mr_hang[i][0] = blockIdx.x * 1000 + (threadIdx.x >> 5);
-        g_mr_hang[i][1] = tag;
-        g_mr_hang[i][2] = g;
-        g_mr_hang[i][3] = (int)parity;
+        if ((n & 1023u) == 1023u) {
+            const long long t = clock64();
+            if (t0 == 0) t0 = t;
+            else if (t - t0 > 4000000000ll) __trap();
+        }
     }
 }
-#else
-__device__ __forceinline__ void mbar_wait_lane(unsigned long long* bar, unsigned parity, int tag = 0, int g = 0) {
-    unsigned ok;
-    do {  // try_wait suspends the thread for a bounded time; no asm labels (they clash when inlined repeatedly)
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-#endif
 // the whole warp waits: lane 0 polls, __syncwarp orders its acquire before the other lanes' later accesses
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity, int tag = 0, int g = 0) {
-    if ((threadIdx.x & 31) == 0) mbar_wait_lane(bar, parity, tag, g);
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    if ((threadIdx.x & 31) == 0) mbar_wait_lane(bar, parity);
     __syncwarp();
 }
+// one lane of the (converged) warp, chosen by the hardware.  ptxas knows that exactly one thread passes an elect.sync
+// predicate and issues the tcgen05 instructions under it directly; under `lane == 0` it wraps every one of them in an
+// ELECT / BRA.U.ANY loop (~60 cycles per MMA, measured)
+__device__ __forceinline__ bool elect_one() {
+    unsigned pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "elect.sync _|p, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(pred));
+    return pred != 0;
+}
+// Named (hardware) barriers for the hand-overs between warps: producers bar.arrive and go on, the consumer warp
+// bar.syncs.  They live in the barrier unit, not in shared memory: an mbarrier operation queues behind the LDS / STS /
+// tensor-core traffic of the shared-memory pipe (300-550 cycles per wait in this kernel, measured, even when the phase
+// is already complete), these take ~50.  mbarriers remain where hardware arrives: TMA complete_tx and tcgen05.commit.
+__device__ __forceinline__ void nbar_arrive(int id, int threads) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+__device__ __forceinline__ void nbar_sync(int id, int threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+constexpr int MR_BAR_EPI = 1;        // the epilogue's exchange of the two halves (128 threads)
+constexpr int MR_BAR_AB = 2;         // + slot: converters and builders -> issuer (A slot in TMEM and B' slot written)
+constexpr int MR_BAR_ACC = 4;        // + slot: epilogue -> issuer (accumulator slot read)
+constexpr int MR_BAR_RAW = 6;        // + ring slot: converters -> TMA producer (raw block read)
+constexpr int MR_MAX_STAGES = 8;     // barrier ids 6 .. 13
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -120,16 +152,27 @@ __device__ __forceinline__ void tc_commit(unsigned long long* bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
                  : "memory");
 }
-// D[tmem] (+)= A[smem] . B[smem]^T, kind::tf32, K = 8 reals per instruction
-__device__ __forceinline__ void tc_mma_tf32(unsigned tmem_d, unsigned long long desc_a, unsigned long long desc_b,
-                                            unsigned idesc, unsigned accumulate) {
+// D[tmem] (+)= A[tmem] . B[smem]^T, kind::tf32, K = 8 reals per instruction.  A: lane = row, 8 consecutive 32-bit
+// columns = the 8 reals; B: K-major shared-memory tile (descriptor); D: lane = row of A, column = row of B.
+__device__ __forceinline__ void tc_mma_tf32_ts(unsigned tmem_d, unsigned tmem_a, unsigned long long desc_b, unsigned idesc,
+                                               unsigned accumulate) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n"
         "}\n" ::"r"(tmem_d),
-        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        "r"(tmem_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// 2-D tiled TMA load: box (32 reals x 64 rows) of the matrix viewed as [rows][128 reals] into 8 KB of shared memory
+// (128-byte swizzle), completion counted in bytes on `bar`; L2 evict-first (A is streamed exactly once).
+__device__ __forceinline__ void tma_load_2d(void* dst, const void* tmap, unsigned long long* bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4}], [%2], %5;" ::"r"(smem_u32(dst)),
+        "l"(reinterpret_cast<unsigned long long>(tmap)), "r"(smem_u32(bar)), "r"(c0), "r"(c1),
+        "l"(0x12F0000000000000ull)
         : "memory");
 }
 // Shared-memory matrix descriptor, K-major, 128-byte swizzle: the tile is stored as rows of 128 bytes (32 reals of
@@ -139,22 +182,15 @@ __device__ __forceinline__ void tc_mma_tf32(unsigned tmem_d, unsigned long long 
 __device__ __forceinline__ unsigned long long umma_desc_sw128(unsigned saddr) {
     unsigned long long d = 0;
     d |= (unsigned long long)((saddr & 0x3FFFFu) >> 4);
-    d |= 1ull << 16;                           // LBO field (ignored for swizzled K-major layouts)
+    d |= 1ull << 16;                             // LBO field (ignored for swizzled K-major layouts)
     d |= (unsigned long long)(1024 >> 4) << 32;  // SBO
-    d |= 1ull << 46;                           // descriptor version of sm_100
-    d |= 2ull << 61;                           // layout type SWIZZLE_128B
+    d |= 1ull << 46;                             // descriptor version of sm_100
+    d |= 2ull << 61;                             // layout type SWIZZLE_128B
     return d;
 }
 // byte offset of 16-byte chunk kc (0..15) of row r in a [2 K-atoms][rows][128 B] swizzled tile
 __device__ __forceinline__ int sw128_off(int rows, int r, int kc) {
     return (kc >> 3) * rows * 128 + r * 128 + (((kc & 7) ^ (r & 7)) << 4);
-}
-__device__ __forceinline__ V16<float> ldg_stream(const float* p) {
-    V16<float> v;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
-                 : "=f"(v.r[0]), "=f"(v.r[1]), "=f"(v.r[2]), "=f"(v.r[3])
-                 : "l"(p));
-    return v;
 }
 __device__ __forceinline__ void split_tf32(const V16<float>& x, V16<float>& hi, V16<float>& lo) {
 #pragma unroll
@@ -163,10 +199,26 @@ __device__ __forceinline__ void split_tf32(const V16<float>& x, V16<float>& hi, 
         lo.r[q] = x.r[q] - hi.r[q];
     }
 }
+// 16 consecutive 32-bit columns of this thread's TMEM lane <- 16 registers / and back
+__device__ __forceinline__ void tmem_st16(unsigned taddr, const float* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+        "r"(__float_as_uint(v[0])), "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])), "r"(__float_as_uint(v[3])),
+        "r"(__float_as_uint(v[4])), "r"(__float_as_uint(v[5])), "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])),
+        "r"(__float_as_uint(v[8])), "r"(__float_as_uint(v[9])), "r"(__float_as_uint(v[10])), "r"(__float_as_uint(v[11])),
+        "r"(__float_as_uint(v[12])), "r"(__float_as_uint(v[13])), "r"(__float_as_uint(v[14])), "r"(__float_as_uint(v[15]))
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(unsigned taddr, unsigned* v) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr));
+}
 
 // neighbour of coarse site X for block d (0 diag, 1+2mu forward, 2+2mu backward), periodic.  No dynamic indexing of
-// the parameter struct (that would put it in local memory) and no run-time division: this sits on the producers'
-// critical path (with a generic version the address arithmetic took longer than the loads it precedes).
+// the parameter struct (that would put it in local memory) and no run-time division.
 __device__ __forceinline__ int coarse_neighbour(const MrhsParams& P, int X, int d) {
     if (d == 0) return X;
     const int mu = (d - 1) >> 1;
@@ -181,57 +233,44 @@ __device__ __forceinline__ int coarse_neighbour(const MrhsParams& P, int X, int 
     return c == L - 1 ? X - (L - 1) * stride : X + stride;               // forward
 }
 
-// shared memory: [stages][ A: 128 rows (hi, lo) x 64 reals = 32 KB | B_hi ncol*256 B | B_lo ncol*256 B ], then the
-// exchange buffer of the epilogue (64 x ncol floats), then the mbarriers
-__host__ __device__ constexpr unsigned mr_stage_bytes(int ncol) {
-    return 2u * MR_ROWS * MR_KT * 4u + 2u * (unsigned)ncol * MR_KT * 4u;
-}
-__host__ __device__ constexpr int mr_max_stages(int ncol) {  // one TMEM slot of 2 ncol columns per stage
-    return MR_TMEM_COLS / (2 * ncol) < 8 ? MR_TMEM_COLS / (2 * ncol) : 8;
+// shared memory: [S raw blocks of 32 KB (TMA destination, 1024-byte aligned)] [2 B' slots] [epilogue exchange
+// buffer 64 x NCOL floats] [mbarriers].  One B' slot: 2 K-atoms x (4 NCOL rows: hi rows of half 0, of half 1, then the
+// lo rows) x 128 B.
+__host__ __device__ constexpr unsigned mr_bslot_bytes(int ncol) { return 2u * 4u * (unsigned)ncol * 128u; }
+__host__ __device__ constexpr size_t mr_smem_bytes(int ncol, int stages) {
+    return (size_t)stages * MR_RAW_BYTES + 2 * mr_bslot_bytes(ncol) + (size_t)MR_ROWS * ncol * 4 + (2 * 8 + 6) * 8 + 16;
 }
 
-// What shaped this kernel (all measured on B200):
-//  * The tensor core adds into its fp32 accumulator with TRUNCATION: a chain of n accumulating MMAs shrinks the result
-//    by about n * 2^-25 (432 MMAs per output -> 1.4e-5 relative, far above the 2e-6 bar).  So chains are short: every
-//    pipeline stage (8 k-steps) starts FRESH accumulators in its own TMEM slot, and the epilogue warps add the slots
-//    into registers in IEEE round-to-nearest fp32 (2.4e-7 relative L2 against the fp64 oracle).
-//  * UMMA with M = 64 and both operands in shared memory exposes the A-read latency (~60-80 cycles per MMA instead of
-//    N/2).  So hi and lo of A are STACKED to M = 128 rows: one MMA with B_hi gives hi.hi (rows 0-63) and lo.hi
-//    (rows 64-127), one with B_lo gives hi.lo and lo.lo -- two full-rate MMAs per k-step instead of three slow ones,
-//    and the fourth product term comes for free.  The small products sit in other TMEM lanes/columns than hi.hi, so
-//    their truncation does not touch the main chain.
-//  * After a tcgen05.commit the issuing thread stalls for several hundred cycles, and the MMAs here are tiny (16
-//    cycles), so one issuer cannot keep up: MR_ISSUERS warps take the stages round-robin (stages are independent: fresh
-//    accumulators), and ONE commit per stage signals both the producers (stage free) and the epilogue (slot ready).
+// NCOL = 2 Kp: accumulator columns per half of the contraction index (Kp = 8 or 16 right-hand sides, zero-padded)
 template <int NCOL>
 __global__ void __launch_bounds__(MR_THREADS, 1)
-    k_coarse_mrhs(float* __restrict__ out, const float* __restrict__ in, const float* __restrict__ A, MrhsParams P) {
+    k_coarse_mrhs(float* __restrict__ out, const float* __restrict__ in, const __grid_constant__ CUtensorMap tmA,
+                  MrhsParams P) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = P.stages;
-    constexpr int ncol = NCOL;
-    constexpr unsigned stage_bytes = mr_stage_bytes(NCOL);
-    float* xbuf = reinterpret_cast<float*>(smem + (size_t)S * stage_bytes);           // [64][NCOL]
+    constexpr unsigned bslot = mr_bslot_bytes(NCOL);
+    constexpr int BROWS = 4 * NCOL;     // rows of a B' slot per K-atom: hi (half 0 | half 1), lo (half 0 | half 1)
+    constexpr int ACC_COLS = 4 * NCOL;  // one accumulator slot: main (2 NCOL columns) | small (2 NCOL columns)
+    constexpr int KP = NCOL / 2;
+    static_assert(2 * MR_A_COLS + 2 * ACC_COLS <= MR_TMEM_COLS, "tensor memory: two A slots and two accumulator slots");
+    unsigned char* sB = smem + (size_t)S * MR_RAW_BYTES;
+    float* xbuf = reinterpret_cast<float*>(sB + 2 * bslot);  // [NCOL][64]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(xbuf + MR_ROWS * NCOL);
-    const int T = P.slots;
-    unsigned long long* full = bars;               // [S] producers -> issuer: operands of the stage are in shared memory
-    unsigned long long* done = bars + S;           // [S] tcgen05.commit -> producers: the MMAs have read the stage
-    unsigned long long* tfull = bars + 2 * S;      // [T] tcgen05.commit -> epilogue: the slot's accumulators are complete
-    unsigned long long* tfree = bars + 2 * S + T;  // [T] epilogue -> issuer: the slot has been read
-    unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 2 * S + 2 * T);
+    unsigned long long* raw_full = bars;   // [<= 8] TMA complete_tx -> converters: the raw block has landed
+    unsigned long long* done = bars + 8;   // [2] tcgen05.commit: the MMAs of the block have completed
+    unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 10);
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < S; i++) {
-            mbar_init(&full[i], 4);  // one arrival per warp of the producer group that owns the stage
-            mbar_init(&done[i], 1);  // one tcgen05.commit
-        }
-        for (int i = 0; i < T; i++) {
-            mbar_init(&tfull[i], 1);              // one tcgen05.commit
-            mbar_init(&tfree[i], MR_EPI_WARPS);   // one arrival per epilogue warp
-        }
+        for (int i = 0; i < S; i++) mbar_init(&raw_full[i], 1);  // the producer's arrive.expect_tx
+        for (int i = 0; i < 2; i++) mbar_init(&done[i], 1);      // one tcgen05.commit
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == MR_EPI_WARPS) {  // the first issuer warp owns the tensor memory
+    // rows of B' beyond the right-hand sides present stay zero for the whole kernel
+    for (unsigned i = threadIdx.x; i < 2 * bslot / 16; i += MR_THREADS)
+        reinterpret_cast<float4*>(sB)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    fence_proxy_async();
+    if (warp == MR_WARP_MMA) {  // the issuer warp owns the tensor memory
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
                      "n"(MR_TMEM_COLS)
                      : "memory");
@@ -241,235 +280,290 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
     __syncthreads();
     tc_fence_after();
     const unsigned tmem_base = *tmem_slot;
+    const unsigned tmem_acc = tmem_base + 2 * MR_A_COLS;
     const int nsites = (P.Vc - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;  // sites of this CTA
-    const int G = nsites * MR_HALVES;                                                   // stages of this CTA
+    const int G = nsites * MR_BLOCKS;                                                   // blocks of this CTA
 
     if (warp < MR_EPI_WARPS) {
-        // ===== epilogue: accumulator row 32 w + t lives in TMEM lane 32 w + t (UMMA M = 128) =====
+        // ===== epilogue: TMEM lane 64 h + r = row r of half h; warp q reads lanes 32 q .. 32 q + 31 =====
+        const int q = warp, h = q >> 1, row = 32 * (q & 1) + lane;
         int g = 0;
         for (int it = 0; it < nsites; it++) {
             const int X = blockIdx.x + it * gridDim.x;
             float acc[NCOL];
 #pragma unroll
-            for (int q = 0; q < NCOL; q++) acc[q] = 0.f;
-            for (int ch = 0; ch < MR_HALVES / MR_AS; ch++, g++) {  // g counts accumulator chains here
-                const int st = g % T;  // TMEM slot
-                if (warp == 0) MR_TRACE(2, g, 0);
-                mbar_wait(&tfull[st], (g / T) & 1, 1, g);
-                if (warp == 0) MR_TRACE(2, g, 1);
+            for (int c = 0; c < NCOL; c++) acc[c] = 0.f;
+            for (int d = 0; d < MR_BLOCKS; d++, g++) {
+                const int a = g & 1;
+                mbar_wait(&done[a], (unsigned)(g >> 1) & 1u);
                 tc_fence_after();
-                const unsigned taddr = tmem_base + ((unsigned)(32 * warp) << 16) + (unsigned)(st * 2 * NCOL);
+                // the columns of this half: main at h NCOL, small (lo.hi + hi.lo) at 2 NCOL + h NCOL
+                const unsigned taddr = tmem_acc + ((unsigned)(32 * q) << 16) + (unsigned)(a * ACC_COLS + h * NCOL);
 #pragma unroll
-                for (int c0 = 0; c0 < 2 * NCOL; c0 += 32) {  // 32 columns per round trip
-                    unsigned v[32];
-#pragma unroll
-                    for (int h = 0; h < 2; h++)
-                        asm volatile(
-                            "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-                            "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                            : "=r"(v[16 * h + 0]), "=r"(v[16 * h + 1]), "=r"(v[16 * h + 2]), "=r"(v[16 * h + 3]),
-                              "=r"(v[16 * h + 4]), "=r"(v[16 * h + 5]), "=r"(v[16 * h + 6]), "=r"(v[16 * h + 7]),
-                              "=r"(v[16 * h + 8]), "=r"(v[16 * h + 9]), "=r"(v[16 * h + 10]), "=r"(v[16 * h + 11]),
-                              "=r"(v[16 * h + 12]), "=r"(v[16 * h + 13]), "=r"(v[16 * h + 14]), "=r"(v[16 * h + 15])
-                            : "r"(taddr + c0 + 16 * h));
+                for (int c0 = 0; c0 < NCOL; c0 += 16) {  // 16 columns of main and of small per round trip
+                    unsigned vm[16], vs[16];
+                    tmem_ld16(taddr + c0, vm);
+                    tmem_ld16(taddr + 2 * NCOL + c0, vs);
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-                    for (int q = 0; q < 32; q++) acc[(c0 + q) % NCOL] += __uint_as_float(v[q]);
+                    for (int c = 0; c < 16; c++) acc[c0 + c] += __uint_as_float(vm[c]) + __uint_as_float(vs[c]);
                 }
                 tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&tfree[st]);
-                if (warp == 0) MR_TRACE(2, g, 2);
+                nbar_arrive(MR_BAR_ACC + a, (MR_EPI_WARPS + 1) * 32);
             }
-            // rows 64..127 hold the lo(A) products of rows 0..63: add them across warps through shared memory
-            if (warp >= 2) {
-                const int row = 32 * (warp - 2) + lane;
+            // the two halves of the contraction index meet through shared memory
+            if (h == 1) {
 #pragma unroll
-                for (int q = 0; q < NCOL; q++) xbuf[q * MR_ROWS + row] = acc[q];
+                for (int c = 0; c < NCOL; c++) xbuf[c * MR_ROWS + row] = acc[c];
             }
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (warp < 2) {
-                const int row = 32 * warp + lane;
+            nbar_sync(MR_BAR_EPI, MR_EPI_WARPS * 32);
+            if (h == 0) {
 #pragma unroll
-                for (int k = 0; k < NCOL / 2; k++)
+                for (int k = 0; k < KP; k++)
                     if (k < P.nrhs)
                         *reinterpret_cast<float2*>(out + k * P.vstride + ((long long)X * MR_ROWS + row) * 2) =
                             make_float2(acc[2 * k] + xbuf[(2 * k) * MR_ROWS + row],
                                         acc[2 * k + 1] + xbuf[(2 * k + 1) * MR_ROWS + row]);
             }
-            asm volatile("bar.sync 1, 128;" ::: "memory");
+            nbar_sync(MR_BAR_EPI, MR_EPI_WARPS * 32);
         }
-    } else if (warp < MR_EPI_WARPS + MR_ISSUERS) {
-        // ===== MMA issuers (one elected lane per warp) =====
-        // instruction descriptor: D fp32, A and B TF32, both K-major, M = 128 (hi rows | lo rows of A),
-        // N = 2 ncol (B'_hi rows | B'_lo rows): ONE MMA per k-step yields all four products hi.hi, lo.hi, hi.lo, lo.lo
-        const unsigned idesc =
-            (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)((2 * ncol) >> 3) << 17) | ((128u >> 4) << 24);
-        const unsigned s0 = smem_u32(smem);
-        const unsigned long long dA = umma_desc_sw128(s0);
-        const unsigned long long dB = umma_desc_sw128(s0 + 2 * MR_ROWS * MR_KT * 4);
-        // Issuer warp m takes the stages g = m, m + NG, ... (NG = P.groups divides S and T: a stage and a slot always
-        // have the same issuer).  A wait on a ready mbarrier still costs ~300 cycles of shared-memory latency under the producers'
-        // store traffic, a commit as much again: one issuer alone paced the kernel at ~1700 cycles per stage.
-        // Issuer warp m takes the accumulator chains c = m, m + MR_ISSUERS, ... (MR_AS stages each).  MR_ISSUERS * MR_AS
-        // divides S and MR_ISSUERS divides T, so a stage and a slot always have the same issuer (a parity wait cannot
-        // tell one completed phase from the one two phases earlier).  One issuer alone cannot keep up: a wait on a ready
-        // mbarrier costs ~300 cycles under the producers' store traffic, issuing 8 small MMAs ~500, a commit ~100.
-        const int mi = warp - MR_EPI_WARPS;
-        if (lane == 0) {
-            for (int c = mi; c < G / MR_AS; c += MR_ISSUERS) {
-                const int sl = c % T;
-                MR_TRACE(1, c * MR_AS, 0);
-                mbar_wait_lane(&tfree[sl], ((c / T) & 1) ^ 1, 2, c);
-                MR_TRACE(1, c * MR_AS, 1);
-                const unsigned tmem_d = tmem_base + (unsigned)(sl * 2 * NCOL);
+    } else if (warp < MR_WARP_B) {
+        // ===== converters: raw block (shared memory, as TMA wrote it) -> hi | lo -> tensor memory =====
+        // thread = one TMEM lane (64 h + r) and 32 of its 64 reals: segment seg = 2 h + ch of the 128-real row.  The
+        // TMA box of segment seg is [64 rows][128 B] at seg * 8 KB with chunk c of row r at c ^ (r & 7): 8 consecutive
+        // lanes (rows) read 8 different chunk positions -- conflict-free 128-bit loads.
+        const int cw = warp - MR_WARP_CONV, q = warp & 3, ch = cw >> 2, h = q >> 1, r = 32 * (q & 1) + lane;
+        const unsigned src_off = (unsigned)((2 * h + ch) * 8192 + r * 128);
+        const unsigned tlane = tmem_base + ((unsigned)(32 * q) << 16) + (unsigned)(32 * ch);
+        int s = 0, ph = 0;
+        for (int g = 0; g < G; g++) {
+            const int a = g & 1;
+            mbar_wait(&raw_full[s], (unsigned)ph);
+            mbar_wait(&done[a], ((unsigned)(g >> 1) & 1u) ^ 1u);  // the MMAs of block g - 2 have read A slot a
+            tc_fence_after();
+            const unsigned char* src = smem + (size_t)s * MR_RAW_BYTES + src_off;
+            const unsigned taddr = tlane + (unsigned)(a * MR_A_COLS);
 #pragma unroll
-                for (int hs = 0; hs < MR_AS; hs++) {
-                    const int g = c * MR_AS + hs, st = g % S;
-                    mbar_wait_lane(&full[st], (g / S) & 1, 3, g);
-                    MR_TRACE(1, g, 2);
-                    tc_fence_after();
-                    // descriptors differ from those of (stage 0, k-step 0) only in the 14-bit address field
-                    const unsigned long long so = (unsigned long long)(((unsigned)st * stage_bytes) >> 4);
+            for (int part = 0; part < 2; part++) {
+                float hi[16], lo[16];
 #pragma unroll
-                    for (int ks = 0; ks < MR_KT / 8; ks++) {  // 8 reals = 32 bytes of the 128-byte swizzled row
-                        const unsigned long long ao =
-                            so + (unsigned long long)(((ks >> 2) * 2 * MR_ROWS * 128 + (ks & 3) * 32) >> 4);
-                        const unsigned long long bo =
-                            so + (unsigned long long)(((ks >> 2) * 2 * ncol * 128 + (ks & 3) * 32) >> 4);
-                        tc_mma_tf32(tmem_d, dA + ao, dB + bo, idesc, (hs | ks) != 0);
+                for (int c = 0; c < 4; c++) {
+                    const int chunk = part * 4 + c;
+                    const V16<float> x = *reinterpret_cast<const V16<float>*>(src + ((chunk ^ (r & 7)) << 4));
+                    V16<float> xh, xl;
+                    split_tf32(x, xh, xl);
+#pragma unroll
+                    for (int e = 0; e < 4; e++) {
+                        hi[4 * c + e] = xh.r[e];
+                        lo[4 * c + e] = xl.r[e];
                     }
-                    MR_TRACE(1, g, 3);
-                    tc_commit(&done[st]);
-                    MR_TRACE(1, g, 4);
                 }
-                tc_commit(&tfull[sl]);
+                tmem_st16(taddr + 16 * part, hi);
+                tmem_st16(taddr + 64 + 16 * part, lo);
             }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            tc_fence_before();
+            nbar_arrive(MR_BAR_RAW + s, (MR_CONV_WARPS + 1) * 32);
+            nbar_arrive(MR_BAR_AB + a, (MR_CONV_WARPS + MR_B_WARPS + 1) * 32);
+            if (++s == S) {
+                s = 0;
+                ph ^= 1;
+            }
+        }
+    } else if (warp < MR_WARP_MMA) {
+        // ===== B' builders: warp bw takes the right-hand sides k = bw, bw + 4, ...; lane = 16-byte chunk of the 512-byte
+        // neighbour vector (2 complex): half h = lane >> 4, chunk kc = lane & 15 of that half's 64 reals =====
+        const int bw = warp - MR_WARP_B;
+        constexpr int NB = KP / MR_B_WARPS;  // right-hand sides per warp
+        const int hB = lane >> 4, kc = lane & 15;
+        int offB[NB];
+#pragma unroll
+        for (int j = 0; j < NB; j++) offB[j] = sw128_off(BROWS, hB * NCOL + 2 * (bw + MR_B_WARPS * j), kc);
+        V16<float> bq[NB];
+        int itB = 0, dB = 0, itP = 0, dP = 0, gP = 0;
+        // the vectors of block gP into L2, MR_B_AHEAD blocks before they are loaded: a neighbour in a direction the
+        // CTA has not visited lately comes from HBM, and the register loads run only one block ahead
+        auto prefetch = [&]() {
+            if (gP < G) {
+                const int X = blockIdx.x + itP * gridDim.x;
+                const float* Bb = in + (long long)coarse_neighbour(P, X, dP) * MR_REALS + lane * 4;
+#pragma unroll
+                for (int j = 0; j < NB; j++)
+                    if (bw + MR_B_WARPS * j < P.nrhs && (lane & 7) == 0)
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(Bb + (long long)(bw + MR_B_WARPS * j) * P.vstride));
+            }
+            gP++;
+            if (++dP == MR_BLOCKS) {
+                dP = 0;
+                itP++;
+            }
+        };
+        auto issue = [&]() {  // loads of the block (itB, dB); then advance
+            prefetch();
+            const int X = blockIdx.x + itB * gridDim.x;
+            const float* Bb = in + (long long)coarse_neighbour(P, X, dB) * MR_REALS + lane * 4;
+#pragma unroll
+            for (int j = 0; j < NB; j++)
+                if (bw + MR_B_WARPS * j < P.nrhs)
+                    bq[j] = *reinterpret_cast<const V16<float>*>(Bb + (long long)(bw + MR_B_WARPS * j) * P.vstride);
+            if (++dB == MR_BLOCKS) {
+                dB = 0;
+                itB++;
+            }
+        };
+        for (int i = 0; i < MR_B_AHEAD; i++) prefetch();
+        if (G > 0) issue();
+        for (int g = 0; g < G; g++) {
+            const int a = g & 1;
+            mbar_wait(&done[a], ((unsigned)(g >> 1) & 1u) ^ 1u);  // the MMAs of block g - 2 have read B' slot a
+            unsigned char* dst = sB + (size_t)a * bslot;
+#pragma unroll
+            for (int j = 0; j < NB; j++) {
+                if (bw + MR_B_WARPS * j < P.nrhs) {
+                    V16<float> h, l, t;
+                    split_tf32(bq[j], h, l);  // once per element: rounding to nearest is symmetric, hi(-x) = -hi(x)
+                    // row (k, re) = (b.re, -b.im), row (k, im) = (b.im, b.re) per complex entry; row 2k+1 = row 2k + 128
+                    // bytes with the swizzle bit 0 flipped (2k is even); the lo rows are 2 NCOL rows further
+                    t.r[0] = h.r[0]; t.r[1] = -h.r[1]; t.r[2] = h.r[2]; t.r[3] = -h.r[3];
+                    *reinterpret_cast<V16<float>*>(dst + offB[j]) = t;
+                    t.r[0] = l.r[0]; t.r[1] = -l.r[1]; t.r[2] = l.r[2]; t.r[3] = -l.r[3];
+                    *reinterpret_cast<V16<float>*>(dst + offB[j] + 2 * NCOL * 128) = t;
+                    t.r[0] = h.r[1]; t.r[1] = h.r[0]; t.r[2] = h.r[3]; t.r[3] = h.r[2];
+                    *reinterpret_cast<V16<float>*>(dst + (offB[j] ^ 16) + 128) = t;
+                    t.r[0] = l.r[1]; t.r[1] = l.r[0]; t.r[2] = l.r[3]; t.r[3] = l.r[2];
+                    *reinterpret_cast<V16<float>*>(dst + (offB[j] ^ 16) + 128 + 2 * NCOL * 128) = t;
+                }
+            }
+            fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async-proxy reads
+            nbar_arrive(MR_BAR_AB + a, (MR_CONV_WARPS + MR_B_WARPS + 1) * 32);
+            if (g + 1 < G) issue();  // after the hand-over: the fence and the arrive would wait for loads in flight
+        }
+    } else if (warp < MR_WARP_TMA) {
+        // ===== MMA issuers (one lane each; issuer m = slot m).  Per k-step of 8 reals (of both halves at once):
+        //   [main | small] (+)= A_hi . [B'_hi | B'_lo]^T   (M = 128, N = 4 NCOL)
+        //   small           += A_lo . B'_hi^T              (M = 128, N = 2 NCOL)
+        // instruction descriptor: D fp32, A and B TF32, K-major, N >> 3 at bit 17, M >> 4 at bit 24 =====
+        const unsigned idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((128u >> 4) << 24);
+        const unsigned idesc1 = idesc | ((unsigned)((4 * NCOL) >> 3) << 17);
+        const unsigned idesc2 = idesc | ((unsigned)((2 * NCOL) >> 3) << 17);
+        const unsigned long long dB0 = umma_desc_sw128(smem_u32(sB));
+        for (int g = warp - MR_WARP_MMA; g < G; g += MR_ISSUERS) {  // the whole warp runs the loop; one elected lane issues
+            const int a = g & 1;
+            if (g >= 2) nbar_sync(MR_BAR_ACC + a, (MR_EPI_WARPS + 1) * 32);  // the epilogue has read block g - 2
+            nbar_sync(MR_BAR_AB + a, (MR_CONV_WARPS + MR_B_WARPS + 1) * 32);
+            tc_fence_after();
+            const unsigned ta = tmem_base + (unsigned)(a * MR_A_COLS), td = tmem_acc + (unsigned)(a * ACC_COLS);
+            const unsigned long long db = dB0 + (unsigned long long)((a * bslot) >> 4);
+            if (elect_one()) {
+#pragma unroll
+                for (int ks = 0; ks < 8; ks++) {  // 8 reals = 32 bytes of the 128-byte swizzled row
+                    const unsigned long long bo = db + (unsigned long long)(((ks >> 2) * BROWS * 128 + (ks & 3) * 32) >> 4);
+                    tc_mma_tf32_ts(td, ta + 8 * ks, bo, idesc1, ks != 0);
+                    tc_mma_tf32_ts(td + 2 * NCOL, ta + 64 + 8 * ks, bo, idesc2, 1u);
+                }
+                tc_commit(&done[a]);
+            }
+            __syncwarp();
         }
         __syncwarp();
     } else {
-        // ===== producers: MR_PROD_GROUPS groups of 4 warps, group pg takes the stages g = pg, pg + MR_PROD_GROUPS, ... =====
-        // A group loads its NEXT stage into registers right after handing over the current one, and converts it a
-        // full round (MR_PROD_GROUPS stage times, > the HBM latency) later.  Why not a deeper register prefetch inside
-        // one group: fence.proxy.async / the releasing mbarrier arrive drain every outstanding load of the thread,
-        // so loads in flight across a hand-over serialise the pipeline (measured: ~2000 cycles per stage).
-        // Stage ownership: MR_PROD_GROUPS divides S, so a stage is always filled by the same group (a parity wait
-        // cannot tell one completed phase from the one two phases earlier).
-        const int pw = warp - MR_EPI_WARPS - MR_ISSUERS;  // 0..15
-        const int pg = pw >> 2, wq = pw & 3;              // group, warp in group
-        const int ptg = wq * 32 + lane;                   // 0..127
-        // A: a warp instruction reads 2 rows x 256 contiguous bytes (whole 128-byte lines); 8 consecutive lanes then
-        // store 8 chunks of ONE swizzled 128-byte row: conflict-free
-        const int rl = lane >> 4, kcA = lane & 15;
-        constexpr int kpad = NCOL / 2;
-        constexpr int NA = MR_ROWS * (MR_KT / 4) / 128;              // 8 A loads per thread
-        constexpr int NB = (kpad * (MR_KT / 4) + 127) / 128;          // B loads per thread
-        const int rowA = wq * 2 + rl;                                 // rows rowA + 8 i
-        const long long a_thr = (long long)rowA * 128 + kcA * 4;      // + i * 8 * 128 reals
-        const int offA = sw128_off(2 * MR_ROWS, rowA, kcA);           // + i * 8 * 128 bytes; lo: + 64 * 128 bytes
-        int kB[NB], offB[NB];
-        long long b_thr[NB];
+        // ===== TMA producer (one lane): four boxes of 32 reals x 64 rows per block, one transaction barrier =====
+        int s = 0, ph = 0, it = 0, d = 0;
+        for (int g = 0; g < G; g++) {
+            if (g >= S) nbar_sync(MR_BAR_RAW + s, (MR_CONV_WARPS + 1) * 32);  // the converters have read block g - S
+            if (elect_one()) {
+                mbar_arrive_expect_tx(&raw_full[s], MR_RAW_BYTES);
+                const int X = blockIdx.x + it * gridDim.x;
+                const int row0 = (X * MR_BLOCKS + d) * MR_ROWS;
+                unsigned char* dst = smem + (size_t)s * MR_RAW_BYTES;
 #pragma unroll
-        for (int j = 0; j < NB; j++) {
-            const int q = ptg + j * 128;
-            kB[j] = q >> 4;
-            offB[j] = sw128_off(2 * ncol, 2 * kB[j], q & 15);
-            b_thr[j] = (long long)kB[j] * P.vstride + (q & 15) * 4;
-        }
-        V16<float> a[NA], bq[NB];
-        auto issue = [&](int g) {  // global loads of stage g
-            const int it = g / MR_HALVES, hb = g - it * MR_HALVES, d = hb >> 1, half = hb & 1;
-            const int X = blockIdx.x + it * gridDim.x;
-            const float* Ab = A + ((long long)X * 9 + d) * (MR_ROWS * 128) + half * MR_KT + a_thr;
-#pragma unroll
-            for (int i = 0; i < NA; i++) a[i] = ldg_stream(Ab + i * 8 * 128);
-            const float* Bb = in + (long long)coarse_neighbour(P, X, d) * 128 + half * MR_KT;
-#pragma unroll
-            for (int j = 0; j < NB; j++) {  // 16 consecutive lanes read the 256 contiguous bytes of one right-hand side
-                if (kB[j] < kpad && kB[j] < P.nrhs)
-                    bq[j] = *reinterpret_cast<const V16<float>*>(Bb + b_thr[j]);
-                else
-                    bq[j].r[0] = bq[j].r[1] = bq[j].r[2] = bq[j].r[3] = 0.f;
+                for (int seg = 0; seg < 4; seg++) tma_load_2d(dst + seg * 8192, &tmA, &raw_full[s], seg * 32, row0);
             }
-        };
-        constexpr int NG = MR_PROD_GROUPS;
-        if (pg < G) issue(pg);
-        for (int g = pg; g < G; g += NG) {
-            const int st = g % S;
-            if (wq == 0) MR_TRACE(0, g, 0);
-            mbar_wait(&done[st], ((g / S) & 1) ^ 1, 4, g);
-            if (wq == 0) MR_TRACE(0, g, 1);
-            unsigned char* sA = smem + (size_t)st * stage_bytes;       // 128 rows: hi 0..63, lo 64..127
-            unsigned char* sB = sA + 2 * MR_ROWS * MR_KT * 4;          // 2 ncol rows: hi 0..ncol-1, lo ncol..
-#pragma unroll
-            for (int i = 0; i < NA; i++) {
-                V16<float> hi, lo;
-                split_tf32(a[i], hi, lo);
-                *reinterpret_cast<V16<float>*>(sA + offA + i * 8 * 128) = hi;
-                *reinterpret_cast<V16<float>*>(sA + offA + i * 8 * 128 + MR_ROWS * 128) = lo;
-            }
-            // B': rows (k, re) = (b.re, -b.im), (k, im) = (b.im, b.re) per complex entry; 16 chunks of 2 complex
-#pragma unroll
-            for (int j = 0; j < NB; j++) {
-                if (kB[j] < kpad) {
-                    const V16<float> b = bq[j];
-                    V16<float> re, im, hi, lo;
-                    re.r[0] = b.r[0]; re.r[1] = -b.r[1]; re.r[2] = b.r[2]; re.r[3] = -b.r[3];
-                    im.r[0] = b.r[1]; im.r[1] = b.r[0]; im.r[2] = b.r[3]; im.r[3] = b.r[2];
-                    // row 2k+1 = row 2k + 128 bytes with the swizzle bit 0 flipped (2k is even)
-                    split_tf32(re, hi, lo);
-                    *reinterpret_cast<V16<float>*>(sB + offB[j]) = hi;
-                    *reinterpret_cast<V16<float>*>(sB + offB[j] + ncol * 128) = lo;
-                    split_tf32(im, hi, lo);
-                    *reinterpret_cast<V16<float>*>(sB + (offB[j] ^ 16) + 128) = hi;
-                    *reinterpret_cast<V16<float>*>(sB + (offB[j] ^ 16) + 128 + ncol * 128) = lo;
-                }
-            }
-            if (wq == 0) MR_TRACE(0, g, 2);
-            fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async-proxy reads
             __syncwarp();
-            if (lane == 0) mbar_arrive(&full[st]);
-            if (wq == 0) MR_TRACE(0, g, 3);
-            if (g + NG < G) issue(g + NG);
-            if (wq == 0) MR_TRACE(0, g, 4);
+            if (++d == MR_BLOCKS) {
+                d = 0;
+                it++;
+            }
+            if (++s == S) {
+                s = 0;
+                ph ^= 1;
+            }
         }
+        __syncwarp();
     }
 
     tc_fence_before();
     __syncthreads();
-    if (warp == MR_EPI_WARPS) {
+    if (warp == MR_WARP_MMA) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(MR_TMEM_COLS)
                      : "memory");
     }
 }
 
-static int mrhs_max_smem() { return max_optin_smem(); }
-static int mrhs_sm_count() { return sm_count(); }
+// ---- host side ----------------------------------------------------------------------------------------------------
+// cuTensorMapEncodeTiled through the runtime's driver entry-point query: the library does not link libcuda, so it
+// still loads (and answers size queries) on a box without a driver.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres = cudaDriverEntryPointSymbolNotFound;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+            qres != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        cudaGetLastError();
+        fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+// The coarse matrix as a 2-D tensor [Vc * 9 * 64 rows][128 reals]; box = 32 reals x 64 rows (a quarter of a block),
+// written to shared memory with the 128-byte swizzle the converters read it with.
+static int make_matrix_tensor_map(CUtensorMap* tm, const float* A, long long Vc, const char* what) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) {
+        set_error("%s: cuTensorMapEncodeTiled is not available from this driver", what);
+        return LQCD_EUNSUPPORTED;
+    }
+    const cuuint64_t gdim[2] = {(cuuint64_t)MR_REALS, (cuuint64_t)Vc * MR_BLOCKS * MR_ROWS};
+    const cuuint64_t gstride[1] = {(cuuint64_t)MR_REALS * sizeof(float)};
+    const cuuint32_t box[2] = {32, (cuuint32_t)MR_ROWS};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(A), gdim, gstride, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("%s: cuTensorMapEncodeTiled failed (CUresult %d)", what, (int)r);
+        return LQCD_ECUDA;
+    }
+    return LQCD_OK;
+}
 
-// one tensor-core launch for up to 16 right-hand sides
+// one tensor-core launch for up to NCOL / 2 right-hand sides
 template <int NCOL>
-static int mrhs_launch_ncol(float* out, const float* in, const float* A, MrhsParams P, cudaStream_t st, const char* what) {
-    constexpr size_t stage = mr_stage_bytes(NCOL);
-    // S = 4 stages: a multiple of the producer groups and of MR_ISSUERS * MR_AS (stage ownership, see the kernel)
-    const int S = 4;
-    static_assert(4 % MR_PROD_GROUPS == 0 && 4 % (MR_ISSUERS * MR_AS) == 0, "stage ownership");
-    if ((size_t)mrhs_max_smem() < S * stage + MR_ROWS * NCOL * 4 + 1024) {
+static int mrhs_launch_ncol(float* out, const float* in, const CUtensorMap& tm, MrhsParams P, cudaStream_t st,
+                            const char* what) {
+    const size_t fixed = mr_smem_bytes(NCOL, 0);
+    int S = (int)(((size_t)max_optin_smem() - fixed) / MR_RAW_BYTES);
+    if ((size_t)max_optin_smem() < fixed + 2 * (size_t)MR_RAW_BYTES) {
         set_error("%s: not enough shared memory for the pipeline", what);
         return LQCD_EUNSUPPORTED;
     }
-    P.slots = mr_max_stages(NCOL) / MR_ISSUERS * MR_ISSUERS;
+    if (S > MR_MAX_STAGES) S = MR_MAX_STAGES;
+    if (g_knobs.mrhs_stages >= 2 && g_knobs.mrhs_stages < S) S = g_knobs.mrhs_stages;
     P.stages = S;
-    const size_t smem = S * stage + MR_ROWS * NCOL * 4 + (2 * S + 2 * 8) * 8 + 16;
     static unsigned long long attr = 0;
-    ensure_dynamic_smem(k_coarse_mrhs<NCOL>, mrhs_max_smem(), attr);
-    const int grid = P.Vc < mrhs_sm_count() ? P.Vc : mrhs_sm_count();
-    k_coarse_mrhs<NCOL><<<grid, MR_THREADS, smem, st>>>(out, in, A, P);
+    ensure_dynamic_smem(k_coarse_mrhs<NCOL>, max_optin_smem(), attr);
+    const int grid = P.Vc < sm_count() ? P.Vc : sm_count();
+    k_coarse_mrhs<NCOL><<<grid, MR_THREADS, mr_smem_bytes(NCOL, S), st>>>(out, in, tm, P);
     count_launch();
     return check_launch(what);
 }
 
-static int mrhs_tensor_launch(float* out, const float* in, const float* A, const int cdims[4], int nrhs, long long vstride,
-                              cudaStream_t st, const char* what) {
+static int mrhs_tensor_launch(float* out, const float* in, const CUtensorMap& tm, const int cdims[4], int nrhs,
+                              long long vstride, cudaStream_t st, const char* what) {
     MrhsParams P;
     for (int mu = 0; mu < 4; mu++) P.Lc[mu] = cdims[mu];
     for (int mu = 0; mu < 3; mu++) P.dLc[mu].set(cdims[mu]);
@@ -477,8 +571,8 @@ static int mrhs_tensor_launch(float* out, const float* in, const float* A, const
     P.nrhs = nrhs;
     P.vstride = vstride;
     P.stages = 0;
-    if (nrhs <= 8)  // UMMA with M = 128 needs N to be a multiple of 16 return mrhs_launch_ncol<16>(out, in, A, P, st, what);
-    return mrhs_launch_ncol<32>(out, in, A, P, st, what);
+    if (nrhs <= 8) return mrhs_launch_ncol<16>(out, in, tm, P, st, what);
+    return mrhs_launch_ncol<32>(out, in, tm, P, st, what);
 }
 
 }  // namespace lqcd
@@ -486,20 +580,6 @@ static int mrhs_tensor_launch(float* out, const float* in, const float* A, const
 using namespace lqcd;
 
 extern "C" {
-#ifdef LQCD_MRHS_TRACE
-int lqcd_debug_mrhs_trace(long long* host) {
-    return cudaMemcpyFromSymbol(host, g_mr_trace, sizeof(g_mr_trace)) == cudaSuccess ? 0 : -3;
-}
-int lqcd_debug_mrhs_hang(int* host) {
-    int n = 0;
-    cudaMemcpyFromSymbol(&n, g_mr_hang_n, sizeof(int));
-    cudaMemcpyFromSymbol(host, g_mr_hang, sizeof(g_mr_hang));
-    int z = 0;
-    cudaMemcpyToSymbol(g_mr_hang_n, &z, sizeof(int));
-    return n;
-}
-#endif
-
 
 int lqcd_coarse_mult_mrhs_f32(float* out, const float* in, const float* A, const int cdims[4], int nvec, int nrhs,
                               unsigned flags, void* stream) {
@@ -522,13 +602,16 @@ int lqcd_coarse_mult_mrhs_f32(float* out, const float* in, const float* A, const
             set_error("%s: coarse extent < 2", what);
             return LQCD_EINVAL;
         }
-    if (volume(cdims) * 9 * 64 * 64 > 0x7fffffffffffLL || volume(cdims) > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
+    if (volume(cdims) * 9 * 64 * 64 > 0x7fffffffffffLL || volume(cdims) * 9 * 64 > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
     const long long vstride = volume(cdims) * 4 * nvec;  // reals per coarse vector
     if (nvec == 32 && flags == 0 && g_knobs.mrhs_tensor >= 0) {
-        for (int k0 = 0; k0 < nrhs; k0 += 16) {  // 16 right-hand sides per launch (TMEM slots and registers)
+        CUtensorMap tm;
+        int rc = make_matrix_tensor_map(&tm, A, volume(cdims), what);
+        if (rc) return rc;
+        for (int k0 = 0; k0 < nrhs; k0 += 16) {  // 16 right-hand sides per launch (tensor-memory columns)
             const int kn = nrhs - k0 < 16 ? nrhs - k0 : 16;
-            int rc = mrhs_tensor_launch(out + k0 * vstride, in + k0 * vstride, A, cdims, kn, vstride,
-                                        (cudaStream_t)stream, what);
+            rc = mrhs_tensor_launch(out + k0 * vstride, in + k0 * vstride, tm, cdims, kn, vstride, (cudaStream_t)stream,
+                                    what);
             if (rc) return rc;
         }
         return LQCD_OK;

@@ -116,7 +116,12 @@ def test_mrhs_error_codes(lq):
 
     n0 = lq.launch_count()
     assert code(lambda: lq.coarse_mult_mrhs(x, x, d.A, cfg.cdims, cfg.nvec)) == lq.EINVAL
-    assert code(lambda: lq.coarse_mult_mrhs(y, x, d.A, (2, 2, 1, 2), cfg.nvec)) == lq.EINVAL
+    with pytest.raises(ValueError, match="needs"):  # sizes are checked by the binding before the C call ...
+        lq.coarse_mult_mrhs(y, x, d.A, (2, 2, 1, 2), cfg.nvec)
+    st = torch.cuda.current_stream().cuda_stream   # ... and the C call refuses the geometry itself
+    rc = lq.lib().lqcd_coarse_mult_mrhs_f32(y.data_ptr(), x.data_ptr(), d.A.data_ptr(), lq._i4((2, 2, 1, 2)), cfg.nvec,
+                                            2, 0, st)
+    assert rc == lq.EINVAL, "coarse extent 1"
     assert code(lambda: lq.coarse_mult_mrhs(y, x, d.A, cfg.cdims, 0)) == lq.EINVAL
     assert "lqcd_coarse_mult_mrhs_f32" in lq.last_error()
     assert lq.launch_count() == n0
