@@ -29,20 +29,25 @@
 // columns of half h, the other half of the products is discarded (the tensor pipe has the room: 64 % busy at the
 // HBM roofline for K = 16) -- and the two halves are added by the epilogue.
 //
-// One persistent CTA per SM, warp-specialised (608 threads):
+// One persistent CTA per SM, warp-specialised (704 threads):
 //   warps 0-3    epilogue: tcgen05.ld the accumulators of every block, add them in registers (fp32, round to
 //                nearest: the tensor core adds by truncation, so chains are kept to one block), store out_k(X)
-//   warps 4-11   converters: raw A tile -> (hi, lo) -> tensor memory (warp w owns TMEM lanes 32 (w % 4) ..)
-//   warps 12-19  B' builders: neighbour's input vectors (L2) -> rows (b.re, -b.im), (b.im, b.re), hi / lo, swizzled
-//   warp 20      MMA issuer  (one lane each): issuer m takes the blocks g = m, m + 2, ... (= accumulator / A / B' slot
-//                m), so every accumulator sees its MMAs in program order.  Two, because ISSUING is the narrow place:
-//                ptxas wraps every tcgen05.mma of a divergent region in an ELECT / BRA.U.ANY loop (~60 cycles per
-//                instruction, measured), more than these small MMAs (32-64 cycles) take to execute.  Warp 16 allocates
-//                and frees tensor memory
-//   warp 18      TMA producer (one lane): cp.async.bulk.tensor of the next block as soon as a ring slot is free
-// mbarriers where the hardware arrives: raw_full[S] (TMA complete_tx -> converters), done[2] (tcgen05.commit ->
-// converters, builders, epilogue); named barriers (bar.arrive / bar.sync) for the hand-overs between warps: converters
-// -> TMA producer (ring slot read), converters + builders -> issuer (operands written), epilogue -> issuer.
+//   warps 4-11   converters: raw A block -> (hi, lo) -> tensor memory (warp w owns TMEM lanes 32 (w % 4) ..)
+//   warps 12-19  B' builders, two groups of four (one per B' slot, taking the blocks in turn): neighbour's input
+//                vectors (L2, prefetched two blocks ahead) -> rows (b.re, -b.im), (b.im, b.re), hi / lo, swizzled
+//   warp 20      MMA issuer: the whole warp runs the loop, the lane chosen by elect.sync issues (under `lane == 0`
+//                ptxas wraps every tcgen05.mma in an ELECT / BRA.U.ANY loop, ~60 cycles per instruction -- more than
+//                these MMAs take to execute).  Allocates / frees tensor memory
+//   warp 21      TMA producer: cp.async.bulk.tensor of the next block as soon as a ring slot is free
+// Hand-overs: mbarriers where hardware arrives -- raw_full[S] (TMA complete_tx -> converters), done[2] / bdone[2]
+// (tcgen05.commit -> converters, epilogue / builders); named barriers (bar.arrive / bar.sync) between warps --
+// converters -> TMA producer (ring slot read), converters -> issuer (A slot written), builders -> issuer (B' slot
+// written), epilogue -> issuer (accumulators read).  An mbarrier operation queues behind the LDS / STS / tensor-core
+// traffic of the shared-memory pipe (300-550 cycles per wait here, even when the phase is complete); a named barrier
+// lives in the barrier unit.
+// Measured (c5, K = 16, 1965 MHz): 2.54 ms = 0.79 of the measured copy peak; K <= 8: 0.95-1.0.  What bounds K = 16 is
+// the shared-memory pipe (per block: 32 KB TMA write + 32 KB LDS + 32 KB B' STS + 48 KB tensor-core operand reads =
+// 1125 cycles at 128 B/clk against ~1200-1500 for the block at the HBM rate) -- DESIGN.md section 6.8.
 #include <cuda.h>  // CUtensorMap and its enums only: the encoder is fetched through cudaGetDriverEntryPoint
 
 #include "common.cuh"
@@ -53,15 +58,15 @@ namespace lqcd {
 constexpr int MR_ROWS = 64;     // N = 2 nvec = 64 rows per block
 constexpr int MR_REALS = 128;   // reals per row of a block
 constexpr int MR_BLOCKS = 9;    // blocks per coarse site
-constexpr int MR_EPI_WARPS = 4, MR_CONV_WARPS = 8, MR_B_WARPS = 8;
+constexpr int MR_EPI_WARPS = 4, MR_CONV_WARPS = 8, MR_B_WARPS = 8;  // B' builders: two groups of four
 constexpr int MR_WARP_CONV = MR_EPI_WARPS, MR_WARP_B = MR_WARP_CONV + MR_CONV_WARPS;
-constexpr int MR_B_AHEAD = 4;                       // blocks the B' builders' L2 prefetch runs ahead
-#ifndef LQCD_MR_ISSUERS
-#define LQCD_MR_ISSUERS 1
-#endif
-constexpr int MR_ISSUERS = LQCD_MR_ISSUERS;                       // = accumulator slots = A slots = B' slots
-constexpr int MR_WARP_MMA = MR_WARP_B + MR_B_WARPS, MR_WARP_TMA = MR_WARP_MMA + MR_ISSUERS;
-constexpr int MR_THREADS = (MR_WARP_TMA + 1) * 32;  // 608
+constexpr int MR_B_GROUP = 4;                       // warps per B' builder group (one group per B' slot)
+constexpr int MR_B_SLOTS = 2;                       // B' ring: the builders run a block ahead of the slot the MMAs read
+constexpr int MR_A_THREADS = (MR_CONV_WARPS + 1) * 32;  // named barrier: converters + issuer
+constexpr int MR_B_THREADS = (MR_B_GROUP + 1) * 32;     // named barrier: one builder group + issuer
+constexpr int MR_B_AHEAD = 2;                       // blocks the B' builders' L2 prefetch runs ahead
+constexpr int MR_WARP_MMA = MR_WARP_B + MR_B_WARPS, MR_WARP_TMA = MR_WARP_MMA + 1;
+constexpr int MR_THREADS = (MR_WARP_TMA + 1) * 32;  // 704
 constexpr int MR_TMEM_COLS = 512;                   // all of tensor memory
 constexpr int MR_A_COLS = 128;                      // one A slot: hi (64 columns) | lo (64 columns), 128 lanes
 constexpr unsigned MR_RAW_BYTES = MR_ROWS * MR_REALS * 4;  // 32 KB: one raw block
@@ -141,10 +146,11 @@ __device__ __forceinline__ void nbar_sync(int id, int threads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 constexpr int MR_BAR_EPI = 1;        // the epilogue's exchange of the two halves (128 threads)
-constexpr int MR_BAR_AB = 2;         // + slot: converters and builders -> issuer (A slot in TMEM and B' slot written)
+constexpr int MR_BAR_A = 2;          // + A slot: converters -> issuer (A slot in tensor memory written)
 constexpr int MR_BAR_ACC = 4;        // + slot: epilogue -> issuer (accumulator slot read)
-constexpr int MR_BAR_RAW = 6;        // + ring slot: converters -> TMA producer (raw block read)
-constexpr int MR_MAX_STAGES = 8;     // barrier ids 6 .. 13
+constexpr int MR_BAR_B = 6;          // + B' slot: builders -> issuer (B' slot written)
+constexpr int MR_BAR_RAW = 9;        // + ring slot: converters -> TMA producer (raw block read)
+constexpr int MR_MAX_STAGES = 6;     // barrier ids 9 .. 14
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -238,7 +244,7 @@ __device__ __forceinline__ int coarse_neighbour(const MrhsParams& P, int X, int 
 // lo rows) x 128 B.
 __host__ __device__ constexpr unsigned mr_bslot_bytes(int ncol) { return 2u * 4u * (unsigned)ncol * 128u; }
 __host__ __device__ constexpr size_t mr_smem_bytes(int ncol, int stages) {
-    return (size_t)stages * MR_RAW_BYTES + 2 * mr_bslot_bytes(ncol) + (size_t)MR_ROWS * ncol * 4 + (2 * 8 + 6) * 8 + 16;
+    return (size_t)stages * MR_RAW_BYTES + MR_B_SLOTS * mr_bslot_bytes(ncol) + (size_t)MR_ROWS * ncol * 4 + 16 * 8 + 16;
 }
 
 // NCOL = 2 Kp: accumulator columns per half of the contraction index (Kp = 8 or 16 right-hand sides, zero-padded)
@@ -255,19 +261,21 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
     constexpr int KP = NCOL / 2;
     static_assert(2 * MR_A_COLS + 2 * ACC_COLS <= MR_TMEM_COLS, "tensor memory: two A slots and two accumulator slots");
     unsigned char* sB = smem + (size_t)S * MR_RAW_BYTES;
-    float* xbuf = reinterpret_cast<float*>(sB + 2 * bslot);  // [NCOL][64]
+    float* xbuf = reinterpret_cast<float*>(sB + MR_B_SLOTS * bslot);  // [NCOL][64]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(xbuf + MR_ROWS * NCOL);
     unsigned long long* raw_full = bars;   // [<= 8] TMA complete_tx -> converters: the raw block has landed
-    unsigned long long* done = bars + 8;   // [2] tcgen05.commit: the MMAs of the block have completed
-    unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 10);
+    unsigned long long* done = bars + 8;   // [2] tcgen05.commit: the MMAs of the block have completed (A / accumulator slot)
+    unsigned long long* bdone = bars + 10; // [3] the same event per B' slot (a parity wait cannot look two phases back)
+    unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 14);
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < S; i++) mbar_init(&raw_full[i], 1);  // the producer's arrive.expect_tx
         for (int i = 0; i < 2; i++) mbar_init(&done[i], 1);      // one tcgen05.commit
+        for (int i = 0; i < MR_B_SLOTS; i++) mbar_init(&bdone[i], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // rows of B' beyond the right-hand sides present stay zero for the whole kernel
-    for (unsigned i = threadIdx.x; i < 2 * bslot / 16; i += MR_THREADS)
+    for (unsigned i = threadIdx.x; i < MR_B_SLOTS * bslot / 16; i += MR_THREADS)
         reinterpret_cast<float4*>(sB)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     fence_proxy_async();
     if (warp == MR_WARP_MMA) {  // the issuer warp owns the tensor memory
@@ -364,7 +372,7 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             tc_fence_before();
             nbar_arrive(MR_BAR_RAW + s, (MR_CONV_WARPS + 1) * 32);
-            nbar_arrive(MR_BAR_AB + a, (MR_CONV_WARPS + MR_B_WARPS + 1) * 32);
+            nbar_arrive(MR_BAR_A + a, MR_A_THREADS);
             if (++s == S) {
                 s = 0;
                 ph ^= 1;
@@ -373,53 +381,64 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
     } else if (warp < MR_WARP_MMA) {
         // ===== B' builders: warp bw takes the right-hand sides k = bw, bw + 4, ...; lane = 16-byte chunk of the 512-byte
         // neighbour vector (2 complex): half h = lane >> 4, chunk kc = lane & 15 of that half's 64 reals =====
-        const int bw = warp - MR_WARP_B;
-        constexpr int NB = KP / MR_B_WARPS;  // right-hand sides per warp
+        // Two groups of four warps: group m builds B' slot m, i.e. the blocks g = m, m + 2, ... -- a group's loop (wait
+        // for the slot, convert, proxy fence, arrive, next loads) takes longer than one block period, two run in turn.
+        const int bw = warp - MR_WARP_B, grp = bw / MR_B_GROUP, wq = bw % MR_B_GROUP;
+        constexpr int NB = KP / MR_B_GROUP;  // right-hand sides per warp: k = wq, wq + 4, ...
         const int hB = lane >> 4, kc = lane & 15;
         int offB[NB];
 #pragma unroll
-        for (int j = 0; j < NB; j++) offB[j] = sw128_off(BROWS, hB * NCOL + 2 * (bw + MR_B_WARPS * j), kc);
+        for (int j = 0; j < NB; j++) offB[j] = sw128_off(BROWS, hB * NCOL + 2 * (wq + MR_B_GROUP * j), kc);
         V16<float> bq[NB];
-        int itB = 0, dB = 0, itP = 0, dP = 0, gP = 0;
-        // the vectors of block gP into L2, MR_B_AHEAD blocks before they are loaded: a neighbour in a direction the
-        // CTA has not visited lately comes from HBM, and the register loads run only one block ahead
+        struct Walk {  // (site iteration, block) of the group's blocks g = grp, grp + 2, ...
+            int it, d, g;
+            __device__ void next() {
+                g += 2;
+                d += 2;
+                if (d >= MR_BLOCKS) {
+                    d -= MR_BLOCKS;
+                    it++;
+                }
+            }
+        } ld{0, grp, grp}, pf{0, grp, grp};
+        // the vectors of a block into L2, MR_B_AHEAD of the group's blocks before they are loaded: a neighbour in a
+        // direction the CTA has not visited lately comes from HBM, and the register loads run only one block ahead
         auto prefetch = [&]() {
-            if (gP < G) {
-                const int X = blockIdx.x + itP * gridDim.x;
-                const float* Bb = in + (long long)coarse_neighbour(P, X, dP) * MR_REALS + lane * 4;
+            if (pf.g < G) {
+                const int X = blockIdx.x + pf.it * gridDim.x;
+                const float* Bb = in + (long long)coarse_neighbour(P, X, pf.d) * MR_REALS + lane * 4;
 #pragma unroll
                 for (int j = 0; j < NB; j++)
-                    if (bw + MR_B_WARPS * j < P.nrhs && (lane & 7) == 0)
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(Bb + (long long)(bw + MR_B_WARPS * j) * P.vstride));
+                    if (wq + MR_B_GROUP * j < P.nrhs && (lane & 7) == 0)
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(Bb + (long long)(wq + MR_B_GROUP * j) * P.vstride));
             }
-            gP++;
-            if (++dP == MR_BLOCKS) {
-                dP = 0;
-                itP++;
-            }
+            pf.next();
         };
-        auto issue = [&]() {  // loads of the block (itB, dB); then advance
-            prefetch();
-            const int X = blockIdx.x + itB * gridDim.x;
-            const float* Bb = in + (long long)coarse_neighbour(P, X, dB) * MR_REALS + lane * 4;
+        // address of the group's next block's vectors (this lane's 16 bytes of right-hand side 0), computed ahead of
+        // the hand-over so that only the load instructions themselves follow it
+        auto next_src = [&]() -> const float* {
+            const int X = blockIdx.x + ld.it * gridDim.x;
+            const float* Bb = in + (long long)coarse_neighbour(P, X, ld.d) * MR_REALS + lane * 4;
+            ld.next();
+            return Bb;
+        };
+        auto issue = [&](const float* Bb) {
 #pragma unroll
             for (int j = 0; j < NB; j++)
-                if (bw + MR_B_WARPS * j < P.nrhs)
-                    bq[j] = *reinterpret_cast<const V16<float>*>(Bb + (long long)(bw + MR_B_WARPS * j) * P.vstride);
-            if (++dB == MR_BLOCKS) {
-                dB = 0;
-                itB++;
-            }
+                if (wq + MR_B_GROUP * j < P.nrhs)
+                    bq[j] = *reinterpret_cast<const V16<float>*>(Bb + (long long)(wq + MR_B_GROUP * j) * P.vstride);
         };
         for (int i = 0; i < MR_B_AHEAD; i++) prefetch();
-        if (G > 0) issue();
-        for (int g = 0; g < G; g++) {
-            const int a = g & 1;
-            mbar_wait(&done[a], ((unsigned)(g >> 1) & 1u) ^ 1u);  // the MMAs of block g - 2 have read B' slot a
-            unsigned char* dst = sB + (size_t)a * bslot;
+        if (grp < G) issue(next_src());
+        int sl = grp, ph = 0;  // B' slot g % 3 and the parity of its use count g / 3
+        for (int g = grp; g < G; g += 2) {
+            prefetch();
+            const float* nxt = g + 2 < G ? next_src() : in;  // while the slot is still busy
+            mbar_wait(&bdone[sl], (unsigned)ph ^ 1u);  // the MMAs of block g - 3 have read B' slot sl
+            unsigned char* dst = sB + (size_t)sl * bslot;
 #pragma unroll
             for (int j = 0; j < NB; j++) {
-                if (bw + MR_B_WARPS * j < P.nrhs) {
+                if (wq + MR_B_GROUP * j < P.nrhs) {
                     V16<float> h, l, t;
                     split_tf32(bq[j], h, l);  // once per element: rounding to nearest is symmetric, hi(-x) = -hi(x)
                     // row (k, re) = (b.re, -b.im), row (k, im) = (b.im, b.re) per complex entry; row 2k+1 = row 2k + 128
@@ -435,8 +454,13 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
                 }
             }
             fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async-proxy reads
-            nbar_arrive(MR_BAR_AB + a, (MR_CONV_WARPS + MR_B_WARPS + 1) * 32);
-            if (g + 1 < G) issue();  // after the hand-over: the fence and the arrive would wait for loads in flight
+            nbar_arrive(MR_BAR_B + sl, MR_B_THREADS);
+            if (g + 2 < G) issue(nxt);  // after the hand-over: the fence and the arrive would wait for loads in flight
+            sl += 2;  // g + 2
+            if (sl >= MR_B_SLOTS) {
+                sl -= MR_B_SLOTS;
+                ph ^= 1;
+            }
         }
     } else if (warp < MR_WARP_TMA) {
         // ===== MMA issuers (one lane each; issuer m = slot m).  Per k-step of 8 reals (of both halves at once):
@@ -447,13 +471,15 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
         const unsigned idesc1 = idesc | ((unsigned)((4 * NCOL) >> 3) << 17);
         const unsigned idesc2 = idesc | ((unsigned)((2 * NCOL) >> 3) << 17);
         const unsigned long long dB0 = umma_desc_sw128(smem_u32(sB));
-        for (int g = warp - MR_WARP_MMA; g < G; g += MR_ISSUERS) {  // the whole warp runs the loop; one elected lane issues
+        int sl = 0;  // B' slot g % 3
+        for (int g = 0; g < G; g++) {  // the whole warp runs the loop; one elected lane issues
             const int a = g & 1;
             if (g >= 2) nbar_sync(MR_BAR_ACC + a, (MR_EPI_WARPS + 1) * 32);  // the epilogue has read block g - 2
-            nbar_sync(MR_BAR_AB + a, (MR_CONV_WARPS + MR_B_WARPS + 1) * 32);
+            nbar_sync(MR_BAR_A + a, MR_A_THREADS);
+            nbar_sync(MR_BAR_B + sl, MR_B_THREADS);
             tc_fence_after();
             const unsigned ta = tmem_base + (unsigned)(a * MR_A_COLS), td = tmem_acc + (unsigned)(a * ACC_COLS);
-            const unsigned long long db = dB0 + (unsigned long long)((a * bslot) >> 4);
+            const unsigned long long db = dB0 + (unsigned long long)((sl * bslot) >> 4);
             if (elect_one()) {
 #pragma unroll
                 for (int ks = 0; ks < 8; ks++) {  // 8 reals = 32 bytes of the 128-byte swizzled row
@@ -462,8 +488,10 @@ __global__ void __launch_bounds__(MR_THREADS, 1)
                     tc_mma_tf32_ts(td + 2 * NCOL, ta + 64 + 8 * ks, bo, idesc2, 1u);
                 }
                 tc_commit(&done[a]);
+                tc_commit(&bdone[sl]);
             }
             __syncwarp();
+            if (++sl == MR_B_SLOTS) sl = 0;
         }
         __syncwarp();
     } else {
