@@ -398,6 +398,10 @@ class Workload:
         c = self.cfg
         self.lq.prolong(self.z[i], self.yc[i], self.v, c.dims, c.block, c.nvec)
 
+    def coarse_mult_half(self, i):
+        c = self.cfg
+        self.lq.coarse_mult_half(self.yc[i], self.xc[i], self.Ah, c.cdims, c.nvec, ws=self.half_ws)
+
 
 def time_steps(W: Workload, steps: int, warmup: int, ranks: Ranks):
     """K steps between one pair of events (whole-step time) with an event after every launch (per-kernel times)."""
@@ -728,6 +732,22 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "speedup_vs_16_single_applications": K * kernels["coarse_mult"]["us"] * 1e-6 / t,
             "frac_of_hbm_peak": (mc["bytes"] + vec_b) / t / 1e9 / peak, "bytes_per_launch": mc["bytes"] + vec_b,
             "path": "tcgen05 kind::tf32, hi/lo split of both operands (3xTF32), fp32 accumulation"}
+        # the coarse operator on half storage (A_0 and the forward blocks; the backward blocks are
+        # G5c A_+mu(X - mu)^dag G5c): 5/9 of the matrix traffic, every stored block read once for both sites it couples
+        prepare_row(W, "coarse_mult_half")
+        t = time_single(W, "coarse_mult_half", reps=max(10, args.steps))
+        mh = model_coarse_half(cfg)
+        yh, y9 = torch.empty_like(W.xc[0]), torch.empty_like(W.xc[0])
+        W.lq.coarse_mult_half(yh, W.xc[0], W.Ah, cfg.cdims, cfg.nvec, ws=W.half_ws)
+        W.lq.coarse_mult(y9, W.xc[0], W.A, cfg.cdims, cfg.nvec)
+        dev = (torch.linalg.vector_norm((yh - y9).to(torch.complex128)) /
+               torch.linalg.vector_norm(y9.to(torch.complex128))).item()
+        extra["coarse_mult_half_storage"] = {
+            "us": t * 1e6, "GBps": mh["bytes"] / t / 1e9, "GFLOPs": mh["flops"] / t / 1e9, "units_per_s": cfg.cvolume / t,
+            "frac_of_hbm_peak": mh["bytes"] / t / 1e9 / peak, "bytes_per_launch": mh["bytes"], "launches": 2,
+            "speedup_vs_nine_block_storage": kernels["coarse_mult"]["us"] * 1e-6 / t,
+            "rel_l2_vs_nine_block_kernel_on_this_operator": dev}
+        del W.Ah, W.half_ws, yh, y9
         # the coarse solver (1b) on the same 16 right-hand sides: 8 BiCGStab iterations, batched (D_c through the
         # tensor-core kernel) against one right-hand side at a time
         nb = int(W.lq.lib().lqcd_coarse_bicgstab_mrhs_workspace_bytes(W.lq._i4(cfg.cdims), cfg.nvec, K, 4))
@@ -868,6 +888,11 @@ def prepare_row(W: Workload, name: str):
     if name == "fine_mrhs" and not hasattr(W, "x2"):
         W.x2 = [torch.stack([W.x[0], W.x[1]]), torch.stack([W.x[2], W.x[3]])]
         W.y2 = [torch.empty_like(W.x2[0]), torch.empty_like(W.x2[1])]
+    if name == "coarse_mult_half" and not hasattr(W, "Ah"):
+        W.Ah = W.lq.pack_coarse_half(W.A, cfg.cdims, cfg.nvec)
+        W.half_ws = W.lq.coarse_half_workspace(cfg.cdims, cfg.nvec, dtype=W.v.dtype, device=W.dev)
+        for xc in W.xc:  # the rows that feed coarse_mult in the step are outputs of restrict; alone they need data
+            xc.copy_(torch.view_as_complex(torch.randn(xc.shape + (2,), device=W.dev, dtype=W.v.dtype)))
     if name == "coarse_mrhs" and not hasattr(W, "xcK"):
         gk = torch.Generator(device=W.dev)
         gk.manual_seed(4242)

@@ -156,6 +156,26 @@ int lqcd_coarse_mult_f32(float* out, const float* in, const float* A, const int 
 int lqcd_coarse_mult_f64(double* out, const double* in, const double* A, const int cdims[4], int nvec,
                          unsigned flags, void* stream);
 
+/* A3 on HALF storage.  gamma5-hermiticity (Eq. 2) makes the blocks of Eq. 7
+ * redundant:  A[X][2+2mu] = Gamma5c A[X-mu][1+2mu]^dag Gamma5c  for a Galerkin matrix, so the half layout
+ * keeps A_0 and the four forward blocks only,
+ *   Ah: complex[Vc][5][N][N],  Ah[X][0] = A[X][0],  Ah[X][1+mu] = A[X][1+2mu]
+ * (lqcd_native_coarse_half_reals reals; lqcd_pack_coarse_half copies them out of the nine-block matrix, device to
+ * device), and lqcd_coarse_mult_half applies
+ *   out(X) = Ah[X][0] in(X) + sum_mu ( Ah[X][1+mu] in(X+mu) + Gamma5c Ah[X-mu][1+mu]^dag Gamma5c in(X-mu) ),
+ * which IS lqcd_coarse_mult whenever A has the symmetry above (any Galerkin P^dag D P), at 5/9 of the matrix traffic:
+ * every stored block is read once and serves both sites it couples.  ws_dev: caller-owned device scratch of
+ * lqcd_coarse_half_workspace_bytes(cdims, nvec, sizeof(real)) bytes (four coarse vectors).  Two launches on `stream`,
+ * fixed summation order (no atomics).  Flags, errors and aliasing rules as for lqcd_coarse_mult. */
+size_t lqcd_native_coarse_half_reals(const int cdims[4], int nvec);
+size_t lqcd_coarse_half_workspace_bytes(const int cdims[4], int nvec, int real_bytes);
+int lqcd_pack_coarse_half_f32(float* Ah, const float* A, const int cdims[4], int nvec, void* stream);
+int lqcd_pack_coarse_half_f64(double* Ah, const double* A, const int cdims[4], int nvec, void* stream);
+int lqcd_coarse_mult_half_f32(float* out, const float* in, const float* Ah, const int cdims[4], int nvec,
+                              unsigned flags, void* ws_dev, void* stream);
+int lqcd_coarse_mult_half_f64(double* out, const double* in, const double* Ah, const int cdims[4], int nvec,
+                              unsigned flags, void* ws_dev, void* stream);
+
 /* ---- A4: restriction, Eq. 5:  out_c[X][chi][i] = <v_i restricted to (X,chi) | in_f> -- */
 int lqcd_restrict_f32(float* out_c, const float* in_f, const float* nullvecs, const int dims[4],
                       const int block[4], int nvec, void* stream);

@@ -438,6 +438,41 @@ def coarse_mult(out, inp, A, cdims, nvec, dagger=False, stream=None):
     return out
 
 
+def native_coarse_half_reals(cdims, nvec) -> int:
+    return int(lib().lqcd_native_coarse_half_reals(_i4(cdims), int(nvec)))
+
+
+def pack_coarse_half(A: torch.Tensor, cdims, nvec, stream=None) -> torch.Tensor:
+    """Half storage of a coarse matrix: A_0 and the four forward blocks, complex (Vc, 5, N, N)."""
+    sfx = _sfx(A)
+    _need_coarse(cdims, nvec, A=A)
+    n = 2 * int(nvec)
+    Ah = torch.empty((_vol(cdims), 5, n, n, 2), dtype=_rdtype(sfx), device=A.device)
+    _check(getattr(lib(), f"lqcd_pack_coarse_half_{sfx}")(_dev_ptr(Ah), _dev_ptr(A), _i4(cdims), int(nvec),
+                                                          _stream(stream, A)), "lqcd_pack_coarse_half")
+    return torch.view_as_complex(Ah)
+
+
+def coarse_half_workspace(cdims, nvec, dtype=torch.float32, device="cuda") -> torch.Tensor:
+    nb = int(lib().lqcd_coarse_half_workspace_bytes(_i4(cdims), int(nvec), 4 if dtype == torch.float32 else 8))
+    return torch.empty(max(nb, 16), dtype=torch.uint8, device=device)
+
+
+def coarse_mult_half(out, inp, Ah, cdims, nvec, dagger=False, ws=None, stream=None):
+    """A3 on half storage: out = D_c in from A_0 and the forward blocks, the backward blocks being
+    Gamma5c A_{+mu}(X - mu)^dag Gamma5c (Eqs. 2, 7)."""
+    sfx = _same_dtype(out, inp, Ah)
+    _need_coarse(cdims, nvec, (("out", out), ("in", inp)))
+    _need(Ah, native_coarse_half_reals(cdims, nvec), "Ah")
+    if ws is None:
+        ws = coarse_half_workspace(cdims, nvec, _rdtype(sfx), out.device)
+    _need_bytes(ws, int(lib().lqcd_coarse_half_workspace_bytes(_i4(cdims), int(nvec), 4 if sfx == "f32" else 8)), "ws")
+    _check(getattr(lib(), f"lqcd_coarse_mult_half_{sfx}")(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(Ah), _i4(cdims),
+                                                          int(nvec), DAGGER if dagger else 0, _dev_ptr(ws),
+                                                          _stream(stream, out, inp, Ah)), "lqcd_coarse_mult_half")
+    return out
+
+
 def restrict(out_c, in_f, nullvecs, dims, block, nvec, stream=None):
     """A4: Eq. 5.  (`restrict` is the paper's name; it shadows nothing in Python.)"""
     sfx = _same_dtype(out_c, in_f, nullvecs)

@@ -32,6 +32,8 @@ SIGNATURES = {
     "lqcd_native_nullvecs_reals": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_native_coarse_vec_reals": (C.c_size_t, [_i4, _ci]),
     "lqcd_native_coarse_mat_reals": (C.c_size_t, [_i4, _ci]),
+    "lqcd_native_coarse_half_reals": (C.c_size_t, [_i4, _ci]),
+    "lqcd_coarse_half_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci]),
     "lqcd_host_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_host_workspace_bytes_f64": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_galerkin_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci, _ci]),
@@ -55,6 +57,8 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_orthonormalize_blocks_{_p}": (_ci, [_vp, _i4, _i4, _ci, _vp]),
         f"lqcd_galerkin_coarse_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _vp, _vp]),
         f"lqcd_pack_nullvec_{_p}": (_ci, [_vp, _vp, _ci, _i4, _i4, _ci, _vp]),
+        f"lqcd_pack_coarse_half_{_p}": (_ci, [_vp, _vp, _i4, _ci, _vp]),
+        f"lqcd_coarse_mult_half_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _vp, _vp]),
         f"lqcd_unpack_nullvec_{_p}": (_ci, [_vp, _vp, _ci, _i4, _i4, _ci, _vp]),
         f"lqcd_wilson_clover_mult_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _cu, _vp]),
         f"lqcd_wilson_clover_dd_mult_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _cu, _vp]),

@@ -54,3 +54,19 @@ def rel_l2(a, b) -> float:
     a = np.asarray(a, dtype=np.complex128).ravel()
     b = np.asarray(b, dtype=np.complex128).ravel()
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def expand_half(Ah, cdims, nvec):
+    """Half storage of a coarse matrix -> the nine blocks: (Vc, 5, N, N) -> (Vc, 9, N, N) with d = 0 and
+    d = 1 + 2 mu taken from the half storage and d = 2 + 2 mu = G5c Ah[X - mu][1 + mu]^dag G5c (Eqs. 2, 7).  numpy only."""
+    Lc = tuple(int(l) for l in cdims)
+    Vc, n = Ah.shape[0], 2 * nvec
+    s = np.concatenate([np.ones(nvec), -np.ones(nvec)])
+    A9 = np.empty((Vc, 9, n, n), dtype=Ah.dtype)
+    A9[:, 0] = Ah[:, 0]
+    idx = np.arange(Vc).reshape(Lc[::-1])            # [t][z][y][x]
+    for mu in range(4):
+        A9[:, 1 + 2 * mu] = Ah[:, 1 + mu]
+        back = np.roll(idx, 1, axis=3 - mu).ravel()  # back[X] = X - mu (periodic)
+        A9[:, 2 + 2 * mu] = s[None, :, None] * np.conj(np.swapaxes(Ah[back, 1 + mu], 1, 2)) * s[None, None, :]
+    return A9

@@ -156,6 +156,63 @@ def test_fullsize_coarse_sampled(lq, name):
 
 
 @pytest.mark.parametrize("name", ["c4", "c5"])
+def test_fullsize_coarse_half_storage_sampled(lq, name):
+    """The coarse operator on half storage in bench.py's configuration: seeded forward blocks on
+    the device; for the sampled sites the nine blocks the oracle needs are put together on the HOST from the half
+    storage of the site and of its four backward neighbours (conjugate transpose and signs only)."""
+    import torch
+    cfg = li.CONFIGS[name]
+    Lc, Vc, nv = cfg.cdims, cfg.cvolume, cfg.nvec
+    n = 2 * nv
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed + 6)
+    Ah = torch.view_as_complex(0.05 * torch.randn((Vc, 5, n, n, 2), generator=gen, device="cuda", dtype=torch.float32))
+    Ah[:, 0] += torch.eye(n, device="cuda", dtype=torch.complex64)
+    sg = torch.cat([torch.ones(nv), -torch.ones(nv)]).to("cuda")
+    # (input preparation: the diagonal block of a Galerkin matrix obeys G5c A_0 G5c = A_0^dag -- needed by the
+    # whole-lattice property below, not by the sampled comparison)
+    Ah[:, 0] = 0.5 * (Ah[:, 0] + sg[None, :, None] * Ah[:, 0].conj().transpose(-1, -2) * sg[None, None, :])
+    xc = li.t_coarse_vector(gen, Vc, nv, "cuda", torch.float32)
+    yc = torch.empty_like(xc)
+    ws = lq.coarse_half_workspace(Lc, nv)
+    rng = np.random.default_rng(cfg.seed + 6)
+    Lca = np.array(Lc)
+    corners = np.array([[x, y, z, t] for x in (0, Lca[0] - 1) for y in (0, Lca[1] - 1) for z in (0, Lca[2] - 1)
+                        for t in (0, Lca[3] - 1)])
+    coords = np.concatenate([corners, np.stack([rng.integers(0, Lca[mu], 112) for mu in range(4)], axis=1)])
+    sites = site_index(Lc, coords).astype(np.int64)
+    sgn = np.concatenate([np.ones(nv), -np.ones(nv)])
+    A_s = np.empty((len(sites), 9, n, n), dtype=np.complex64)
+    own = Ah[torch.from_numpy(sites).cuda()].cpu().numpy()
+    A_s[:, 0] = own[:, 0]
+    for mu in range(4):
+        A_s[:, 1 + 2 * mu] = own[:, 1 + mu]
+        back = coords.copy()
+        back[:, mu] = (back[:, mu] - 1) % Lca[mu]
+        bsites = torch.from_numpy(site_index(Lc, back).astype(np.int64)).cuda()
+        fb = Ah[bsites, 1 + mu].cpu().numpy()
+        A_s[:, 2 + 2 * mu] = sgn[None, :, None] * np.conj(np.swapaxes(fb, 1, 2)) * sgn[None, None, :]
+    xc_h = xc.cpu().numpy()
+    for dag in (False, True):
+        lq.coarse_mult_half(yc, xc, Ah, Lc, nv, dagger=dag, ws=ws)
+        got = yc[torch.from_numpy(sites).cuda()].cpu().numpy()
+        ref = oracle.coarse_mult_sites(xc_h, A_s, Lc, sites, dagger=dag)
+        assert rel_l2(got, ref) <= TOL32, dag
+        per_site = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / np.linalg.norm(
+            ref.reshape(len(sites), -1), axis=1)
+        assert per_site.max() <= 5 * TOL32
+    # property on the whole lattice: <y, D_c x> = <D_c^dag y, x> (the half-storage operator and its dagger form)
+    z = li.t_coarse_vector(gen, Vc, nv, "cuda", torch.float32)
+    y1, y2 = torch.empty_like(xc), torch.empty_like(xc)
+    lq.coarse_mult_half(y1, xc, Ah, Lc, nv, ws=ws)
+    lq.coarse_mult_half(y2, z, Ah, Lc, nv, dagger=True, ws=ws)
+    lhs = torch.sum(torch.conj(z).to(torch.complex128) * y1.to(torch.complex128))
+    rhs = torch.sum(torch.conj(y2).to(torch.complex128) * xc.to(torch.complex128))
+    scale = torch.linalg.vector_norm(z.to(torch.complex128)) * torch.linalg.vector_norm(y1.to(torch.complex128))
+    assert (abs(lhs - rhs) / scale).item() <= TOL32
+
+
+@pytest.mark.parametrize("name", ["c4", "c5"])
 def test_fullsize_restrict_prolong_sampled(lq, name):
     import torch
     cfg = li.CONFIGS[name]

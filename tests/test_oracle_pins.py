@@ -374,6 +374,19 @@ def test_coarse_gamma5_block_relations(c1):
             assert np.max(np.abs(lhs - rhs)) < 1e-15
 
 
+def test_half_storage_expansion_reproduces_the_galerkin_matrix(c1):
+    """The test helper that turns half storage (A_0 and the forward blocks) back into nine blocks is
+    what the half-storage GPU tests hand to the oracle: on the true P^dag D P of config 1 (coarse extent 2 in every
+    direction: X + mu == X - mu) it must give back the oracle's own nine blocks, and the same on a lattice with
+    distinct neighbours."""
+    from problems import expand_half, make_problem, custom_config
+    cfg, A = c1["cfg"], c1["A"]
+    assert np.max(np.abs(expand_half(A[:, [0, 1, 3, 5, 7]], cfg.cdims, cfg.nvec) - A)) < 1e-15
+    prob = make_problem(custom_config((6, 4, 8, 4), (2, 2, 2, 2), 2))
+    A2 = prob.A
+    assert np.max(np.abs(expand_half(A2[:, [0, 1, 3, 5, 7]], prob.cfg.cdims, 2) - A2)) < 1e-15
+
+
 @pytest.mark.parametrize("dims,block,nvec,bc", [
     ((8, 4, 4, 8), (4, 2, 2, 2), 5, (1, 1, 1, -1)),
     ((4, 6, 4, 4), (2, 3, 1, 2), 3, (-1, 1, 1, -1)),
