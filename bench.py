@@ -38,6 +38,7 @@ import lqcd_inputs as li
 
 METRIC = "fp32 Wilson-clover & coarse mat-vec GB/s and GFLOP/s; % of HBM roofline"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+HBM_PIN_RATE_GBS = 3996e6 * 2 * 8192 / 8 / 1e9  # 8184 GB/s: memory clock x DDR x bus width (what ncu's DRAM % refers to)
 
 
 # ----------------------------------------------------------------------------------------------------------
@@ -446,6 +447,41 @@ def time_single(W: Workload, name: str, reps: int, warmup: int = 3):
     return e0.elapsed_time(e1) * 1e-3 / reps
 
 
+def measure_pcie(device, nbytes: int = 1 << 30, reps: int = 3) -> dict:
+    """Pinned-memory copy rates of this box, the ceiling of the e2e figure: H2D alone, D2H alone, and both directions at
+    once on two streams (PCIe is full duplex).  GB/s per direction, best of `reps`, CUDA events."""
+    import torch
+    h_in = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    h_out = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    d_a = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    d_b = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    s1, s2 = torch.cuda.Stream(device=device), torch.cuda.Stream(device=device)
+
+    def run(h2d: bool, d2h: bool) -> float:
+        best = float("inf")
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            s1.wait_event(e0)
+            s2.wait_event(e0)
+            if h2d:
+                with torch.cuda.stream(s1):
+                    d_a.copy_(h_in, non_blocking=True)
+            if d2h:
+                with torch.cuda.stream(s2):
+                    h_out.copy_(d_b, non_blocking=True)
+            torch.cuda.current_stream().wait_stream(s1)
+            torch.cuda.current_stream().wait_stream(s2)
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1) * 1e-3)
+        return nbytes / best / 1e9
+
+    return {"h2d_GBps": run(True, False), "d2h_GBps": run(False, True), "duplex_GBps_per_direction": run(True, True),
+            "bytes": nbytes}
+
+
 def time_e2e(W: Workload, steps: int, warmup: int, ranks: Ranks):
     """The same step through the host-vector C-ABI calls: canonical fp32 vectors in pinned host memory, H2D and D2H
     inside the timed region, every call synchronising."""
@@ -485,7 +521,8 @@ def time_e2e(W: Workload, steps: int, warmup: int, ranks: Ranks):
     pool = ThreadPoolExecutor(max_workers=3)
 
     def one():
-        futs = [pool.submit(f) for f in (chain_d, chain_ddag, chain_transfer)]
+        # the chain with the longest dependent compute first: its download then overlaps the uploads of the others
+        futs = [pool.submit(f) for f in (chain_transfer, chain_d, chain_ddag)]
         for f in futs:
             f.result()
 
@@ -521,6 +558,18 @@ def sample_config(cfg: li.Config) -> li.Config:
                      seed=cfg.seed, bc=cfg.bc)
 
 
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    import platform
+    return platform.processor() or "unknown"
+
+
 class OracleSample:
     """Host fields of the sample, fp32-rounded (the oracle promotes them and computes in fp64)."""
 
@@ -536,7 +585,8 @@ class OracleSample:
         self.clover = c64(0.025 * (g + np.conj(np.swapaxes(g, -1, -2))))
         self.v = c64(li.null_vectors(rng, s.nvec, s.volume) / np.sqrt(2.0 * 6 * (s.volume // s.cvolume)))
         self.A = c64(li.coarse_matrix_synthetic(rng, s.cvolume, s.nvec))
-        self.threads = oracle.threads()
+        self.cores = os.cpu_count() or 1
+        self.threads = oracle.set_threads(self.cores)
 
     def step(self):
         o, s = self.oracle, self.scfg
@@ -560,6 +610,65 @@ class OracleSample:
                 f"block {'x'.join(map(str, s.block))}, nvec {s.nvec}, fp32-rounded inputs, fp64 arithmetic")
 
 
+def oracle_full_rows(name: str = "c4") -> dict:
+    """SURVEY 8(d) "oracle beside it": the oracle's D, D^dag and coarse_mult at the FULL size of config 4 (32^3 x 64 fine,
+    8^3 x 16 coarse, N = 64), once with 1 thread (1 repeat) and with all cores (best of 3).  The fields have config 4's
+    shapes and fp32 storage but are plain Gaussian numbers: the oracle has no data-dependent control flow, and the exact
+    SU(3) recipe at 2 M sites costs minutes of host time for no change in what is measured.  Transfers (restrict,
+    prolong) are not timed at this size: their null vectors are 6.4 GB of host memory -- the sample above has them."""
+    import oracle
+    cfg = li.CONFIGS[name]
+    V, Vc, nv, n = cfg.volume, cfg.cvolume, cfg.nvec, 2 * cfg.nvec
+    rng = np.random.default_rng(cfg.seed)
+
+    def gauss(shape, scale=1.0):
+        a = rng.standard_normal(shape + (2,), dtype=np.float32)
+        if scale != 1.0:
+            a *= np.float32(scale)
+        return a.view(np.complex64).reshape(shape)
+
+    U, psi, clover = gauss((4, V, 3, 3), 0.5), gauss((V, 4, 3)), gauss((V, 2, 6, 6), 0.05)
+    A, xc = gauss((Vc, 9, n, n), 0.05), gauss((Vc, 2, nv))
+    m = model(cfg)
+    cores = os.cpu_count() or 1
+    rows = {
+        "wilson_clover": lambda: oracle.wilson_clover_mult(psi, U, clover, cfg.kappa, cfg.dims, cfg.bc),
+        "wilson_clover_dagger": lambda: oracle.wilson_clover_mult(psi, U, clover, cfg.kappa, cfg.dims, cfg.bc, dagger=True),
+        "coarse_mult": lambda: oracle.coarse_mult(xc, A, cfg.cdims),
+    }
+    out = {"workload": f"{name}: fine {'x'.join(map(str, cfg.dims))}, coarse {'x'.join(map(str, cfg.cdims))}, N = {n}; "
+                       "Gaussian fields of the config's shapes, fp32 storage, fp64 arithmetic", "rows": {}}
+    for label, fn in rows.items():
+        r = {}
+        for threads, reps in ((1, 1), (cores, 3)):
+            used = oracle.set_threads(threads)
+            best = min(_timed(fn) for _ in range(reps))
+            r[f"threads_{used}"] = {"s": best, "repeats": reps, "units_per_s": m[label]["units"] / best,
+                                    "GFLOPs": m[label]["flops"] / best / 1e9, "GBps": m[label]["bytes"] / best / 1e9}
+        out["rows"][label] = r
+    oracle.set_threads(cores)
+    return out
+
+
+def _timed(fn) -> float:
+    t0 = time.perf_counter()
+    fn()
+    return time.perf_counter() - t0
+
+
+def cpu_baseline_dict(cfg: li.Config, steps: int = 3, warmup: int = 1, full_rows: bool = True):
+    """The oracle as it stands on this box's host cores: the bounded sample of the workload (the line's value) and, per
+    SURVEY 8(d), the metric's rows at full config-4 size with 1 thread and with all cores."""
+    smp = OracleSample(cfg)
+    sec = smp.time(steps, warmup)
+    d = {"value": step_bytes(smp.scfg) / sec / 1e9, "unit": "GB/s", "cores": smp.threads, "kind": "oracle",
+         "sample": smp.describe(), "ms_per_step": sec * 1e3, "gflops": step_flops(smp.scfg) / sec / 1e9,
+         "cpu_model": cpu_model(), "host_cores": smp.cores}
+    if full_rows:
+        d["full_size_rows"] = oracle_full_rows("c4")
+    return d, smp, sec
+
+
 def step_bytes(cfg: li.Config) -> int:
     m = model(cfg)
     return sum(m[k]["bytes"] for k in STEP_ORDER)
@@ -570,9 +679,10 @@ def step_flops(cfg: li.Config) -> int:
     return sum(m[k]["flops"] for k in STEP_ORDER)
 
 
-def config_dict(cfg: li.Config, n_gpus: int) -> dict:
+def config_dict(cfg: li.Config, n_gpus: int, sample_of: str | None = None) -> dict:
     return {
-        "workload": (f"{cfg.name}: fine {'x'.join(map(str, cfg.dims))} ({cfg.volume} sites), block "
+        "workload": (("" if sample_of is None else f"bounded SAMPLE of {sample_of} -- what this line ran is ") +
+                     f"{cfg.name}: fine {'x'.join(map(str, cfg.dims))} ({cfg.volume} sites), block "
                      f"{'x'.join(map(str, cfg.block))} -> coarse {'x'.join(map(str, cfg.cdims))}, nvec {cfg.nvec} "
                      f"(N={2 * cfg.nvec}), {cfg.gauge} links, kappa {cfg.kappa}, bc {list(cfg.bc)}; step = D, D^dag, "
                      f"restrict, coarse_mult, prolong on one right-hand side"),
@@ -587,13 +697,20 @@ def run_reference(args, cfg: li.Config, ranks: Ranks):
     smp = OracleSample(cfg)
     sec = smp.time(args.steps, args.warmup)
     val = step_bytes(smp.scfg) / sec / 1e9
+    cb = {"value": val, "unit": "GB/s", "cores": smp.threads, "kind": "oracle", "sample": smp.describe(),
+          "cpu_model": cpu_model(), "host_cores": smp.cores}
+    if not args.no_extras:
+        cb["full_size_rows"] = oracle_full_rows("c4")
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(cfg, args.gpus),
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        # the line states what ran: the oracle is timed on a bounded sample (same recipe, smaller lattice), so this is
+        # NOT the same configuration as the GPU arm's line -- GB/s is intensive, but a 131 072-site lattice sits far
+        # better in the host caches than the full workload would
+        "config": config_dict(smp.scfg, args.gpus, sample_of=cfg.name), "same_config_as_gpu_arm": False,
         "gflops": step_flops(smp.scfg) / sec / 1e9,
-        "cpu_baseline": {"value": val, "unit": "GB/s", "cores": smp.threads, "kind": "oracle",
-                         "sample": smp.describe()},
+        "cpu_baseline": cb,
         "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -652,12 +769,21 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "GBps": m[name]["bytes"] / t / 1e9, "GFLOPs": m[name]["flops"] / t / 1e9,
             "units_per_s": m[name]["units"] / t, "frac_of_hbm_peak": m[name]["bytes"] / t / 1e9 / peak,
             "bytes_per_launch": m[name]["bytes"], "symbol": KERNEL_SYMBOL[name],
+            "frac_of_pin_rate": m[name]["bytes"] / t / 1e9 / HBM_PIN_RATE_GBS,
         }
     dominant = max(STEP_ORDER, key=lambda n: kernels[n]["us"])
     roofline = {
         "bound": "hbm", "kernel": dominant, "achieved": kernels[dominant]["GBps"], "peak": peak, "unit": "GB/s",
         "frac": kernels[dominant]["GBps"] / peak, "traffic": recorded_traffic(cfg.name + (":f64" if f64 else ""), dominant),
         "peak_source": peak_src, "algorithmic_bytes_per_launch": m[dominant]["bytes"],
+        "frac_of_pin_rate": kernels[dominant]["GBps"] / HBM_PIN_RATE_GBS, "pin_rate": HBM_PIN_RATE_GBS,
+        # the two kernels the metric names, next to the dominant one (restrict / prolong carry 70 % of the step's bytes)
+        "metric_kernels": {
+            n: {"us": kernels[n]["us"], "achieved": kernels[n]["GBps"], "frac": kernels[n]["GBps"] / peak,
+                "frac_of_pin_rate": kernels[n]["GBps"] / HBM_PIN_RATE_GBS, "GFLOPs": kernels[n]["GFLOPs"],
+                "traffic": recorded_traffic(cfg.name + (":f64" if f64 else ""), n),
+                "algorithmic_bytes_per_launch": m[n]["bytes"]}
+            for n in ("wilson_clover", "wilson_clover_dagger", "coarse_mult")},
     }
     # the 12-real-link variant of A1 (config 4 asks for both storages), timed alone
     extra = {}
@@ -829,9 +955,22 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)
     e2e_s = ranks.max(e2e_s)
+    pcie = measure_pcie(device)
+    # ceilings of one e2e step: (i) both directions perfectly overlapped; (ii) the dependency-aware bound: no result can
+    # leave before the first chain's input has arrived and its kernels have run, then the downloads run back to back
+    t_duplex = max(h2d, d2h) / (pcie["duplex_GBps_per_direction"] * 1e9)
+    fine_bytes = cfg.volume * 24 * (8 if f64 else 4)
+    t_chain = (fine_bytes / (pcie["h2d_GBps"] * 1e9) +
+               sum(kernels[n]["us"] for n in ("restrict", "coarse_mult", "prolong")) * 1e-6 + d2h / (pcie["d2h_GBps"] * 1e9))
     e2e = {"value": whole_job_value(sbytes, ranks.world, e2e_s) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps,
-           "note": "host-vector C-ABI calls, pinned canonical vectors, three independent chains on three streams; PCIe copies dominate"}
+           "pcie_measured": pcie, "ms_if_full_duplex": t_duplex * 1e3, "frac_of_full_duplex_pcie": t_duplex / e2e_s,
+           "ms_dependency_bound": t_chain * 1e3, "frac_of_dependency_bound": t_chain / e2e_s,
+           "GBps_per_direction": max(h2d, d2h) / e2e_s / 1e9,
+           "note": "host-vector C-ABI calls, pinned canonical vectors, three independent chains on three streams; PCIe "
+                   "copies dominate: every call needs its whole input on the device before the first output exists "
+                   "(the stencil wraps around the lattice), so the step cannot beat upload of one vector + its kernels "
+                   "+ all downloads (ms_dependency_bound)"}
 
     line = {
         "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": ranks.world, "steps": args.steps,
@@ -850,11 +989,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
                                                          "x".join(map(str, sharded["rank_grid"]))))
         line["sharded"] = sharded
     if ranks.rank == 0 and ranks.world == 1 and not args.no_cpu_baseline:
-        smp = OracleSample(cfg)
-        sec = smp.time(3, 1)
-        line["cpu_baseline"] = {"value": step_bytes(smp.scfg) / sec / 1e9, "unit": "GB/s", "cores": smp.threads,
-                                "kind": "oracle", "sample": smp.describe(), "ms_per_step": sec * 1e3,
-                                "gflops": step_flops(smp.scfg) / sec / 1e9}
+        line["cpu_baseline"], _, _ = cpu_baseline_dict(cfg, steps=3, warmup=1, full_rows=not args.no_extras)
     if ranks.rank == 0:
         print(json.dumps(line), flush=True)
 

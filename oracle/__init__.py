@@ -33,6 +33,11 @@ def threads() -> int:
     return int(lib().lqcd_oracle_threads_ref())
 
 
+def set_threads(n: int) -> int:
+    """OpenMP threads of the following oracle calls (1 ... all cores); returns the count in effect."""
+    return int(lib().lqcd_oracle_set_threads_ref(C.c_int(int(n))))
+
+
 def _i4(a):
     arr = (C.c_int * 4)(*[int(v) for v in a])
     return arr

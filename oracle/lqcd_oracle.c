@@ -92,6 +92,17 @@ int FN(lqcd_oracle_threads)(void) {
     return 1;
 #endif
 }
+/* number of OpenMP threads of the following calls (bench.py times the oracle with 1 thread and with all cores,
+ * SURVEY.md 8(d)); returns the count in effect.  Plumbing only: no arithmetic depends on it. */
+int FN(lqcd_oracle_set_threads)(int n) {
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+    return omp_get_max_threads();
+#else
+    (void)n;
+    return 1;
+#endif
+}
 
 /* ------------------------------------------------------------------------------------------
  * Geometry: s = x + Lx (y + Ly (z + Lz t))   (reading Q3: 0-based, x fastest)

@@ -430,8 +430,9 @@ def test_fullsize_fp64_five_rows_sampled(lq, name):
         ref = oracle.coarse_mult_sites(xc_h, A_s, Lc, csites, dagger=dag)
         assert rel_l2(got, ref) <= TOL64, dag
     del A, A_s
-    if name != "c4":
-        return  # restrict / prolong are aggregate-local: config 4 covers them (config 5's fp64 null vectors are 65 GB)
+    torch.cuda.empty_cache()
+    # (config 5: the fp64 null vectors are 65 GB on the device -- the size bench.py --precision f64 times; the oracle
+    # only ever sees the 16 gathered aggregates)
 
     # ---- A4 / A5: 16 sampled aggregates gathered into a fake 8^4 lattice of 2^4 blocks (see the fp32 test) ----
     Xs = np.stack([rng.integers(0, Lca[mu], 16) for mu in range(4)], axis=1)
@@ -459,3 +460,62 @@ def test_fullsize_fp64_five_rows_sampled(lq, name):
     assert rel_l2(out_c[Xreal_d].cpu().numpy(), ref_r) <= TOL64
     ref_p = oracle.prolong(xc[Xreal_d].cpu().numpy(), v_fake, fdims, b)
     assert rel_l2(lq.unpack_spinor(out_f, L)[real_d].cpu().numpy(), ref_p) <= TOL64
+
+
+def test_fullsize_device_setup_sampled(lq):
+    """The operators bench.py times are BUILT on the device (F2: clover term from the links, block-orthonormal null
+    vectors, Galerkin P^dag D P).  At config 4 the oracle cannot build them on the whole lattice, but all three are
+    local: the nine blocks A[X][.] of a coarse site, the orthonormal vectors on its aggregate and the clover term on
+    its sites depend only on the links and raw vectors of the 3^4 aggregates around X.  For sampled X those are
+    gathered into a 12^4 lattice (X in the middle; for the sample at the antiperiodic boundary X is placed last in t,
+    so that its forward t hop wraps -- and takes its phase -- in the small lattice as it does in the real one) and the
+    oracle runs its own set-up chain (O3, O4, O6) there from the RAW seeded inputs.  No oracle input is a CUDA output."""
+    import torch
+    cfg = li.CONFIGS["c4"]
+    L, b, Lc, nv, V = cfg.dims, cfg.block, cfg.cdims, cfg.nvec, cfg.volume
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(cfg.seed + 21)
+    U = li.t_gauge_field(cfg, gen, "cuda").to(torch.complex64)          # canonical (4, V, 3, 3), rounded once
+    U18 = lq.pack_gauge(U, L)
+    clover = lq.clover_from_links(U18, cfg.kappa, cfg.csw, L)
+    vn = torch.empty(lq.native_nullvecs_reals(L, b, nv), dtype=torch.float32, device="cuda")
+    # sampled coarse sites and the offset of X inside its 3^4 neighbourhood (mini coordinate of X)
+    samples = [((3, 5, 2, 9), (1, 1, 1, 1)), ((0, Lc[1] - 1, 4, Lc[3] - 1), (1, 1, 1, 2))]
+    mdims, mcd = (12, 12, 12, 12), (3, 3, 3, 3)
+    mc = li.site_coords(mdims)                                           # (20736, 4) fine coordinates in the mini lattice
+    gathers = []
+    for X, off in samples:
+        real_c = np.stack([((X[mu] + mc[:, mu] // b[mu] - off[mu]) % Lc[mu]) * b[mu] + mc[:, mu] % b[mu]
+                           for mu in range(4)], axis=1)
+        gathers.append(torch.from_numpy(site_index(L, real_c).astype(np.int64)).cuda())
+    raw = [np.empty((nv, len(mc), 4, 3), dtype=np.complex64) for _ in samples]
+    for i in range(nv):
+        vi = li.t_spinor(gen, V, "cuda", torch.float32)
+        lq.pack_nullvec(vn, vi, i, L, b, nv)
+        for k, g in enumerate(gathers):
+            raw[k][i] = vi[g].cpu().numpy()
+        del vi
+    lq.orthonormalize_blocks(vn, L, b, nv)
+    assert lq.orthonormalize_degenerate_count() == 0
+    A = lq.galerkin_coarse(U18, clover, vn, cfg.kappa, L, cfg.bc, b, nv)
+    clov_c = lq.unpack_clover(clover, L)                                 # canonical (V, 2, 6, 6)
+    for k, ((X, off), g) in enumerate(zip(samples, gathers)):
+        Um = np.ascontiguousarray(U[:, g].cpu().numpy())
+        clov_ref = oracle.clover_from_links(Um, cfg.kappa, cfg.csw, mdims)
+        v_ref = oracle.orthonormalize_blocks(raw[k], mdims, b)
+        A_ref = oracle.galerkin_coarse(Um, clov_ref, v_ref, cfg.kappa, mdims, cfg.bc, b)
+        mX = int(site_index(mcd, np.array(off)))                         # X inside the mini coarse lattice
+        Xr = int(site_index(Lc, np.array(X)))
+        in_X = np.nonzero(site_index(mcd, mc // 4) == mX)[0]             # its 256 fine sites (mini indices)
+        # O3: the clover term on the aggregate's sites
+        got_c = clov_c[g[torch.from_numpy(in_X).cuda()]].cpu().numpy()
+        assert rel_l2(got_c, clov_ref[in_X]) <= 4 * TOL32, ("clover", X)
+        # O4: the orthonormal vectors on the aggregate (the unique Q with positive diagonal, compared directly)
+        for i in (0, 1, nv // 2, nv - 1):
+            vi = lq.unpack_nullvec(vn, i, L, b, nv)
+            assert rel_l2(vi[g[torch.from_numpy(in_X).cuda()]].cpu().numpy(), v_ref[i][in_X]) <= 8 * TOL32, ("v", X, i)
+        # O6: all nine blocks of the coarse site
+        got_A = A[Xr].cpu().numpy()
+        assert rel_l2(got_A, A_ref[mX]) <= 2 * TOL32, ("A", X)
+        for d in range(9):
+            assert rel_l2(got_A[d], A_ref[mX][d]) <= 4 * TOL32, ("A block", X, d)

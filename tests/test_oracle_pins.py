@@ -180,7 +180,7 @@ def c1():
     clov = oracle.clover_from_links(f.U, cfg.kappa, cfg.csw, cfg.dims)
     v = oracle.orthonormalize_blocks(f.v, cfg.dims, cfg.block)
     A = oracle.galerkin_coarse(f.U, clov, v, cfg.kappa, cfg.dims, cfg.bc, cfg.block)
-    return dict(cfg=cfg, U=f.U, psi=f.psi, clov=clov, v=v, A=A)
+    return dict(cfg=cfg, U=f.U, psi=f.psi, clov=clov, v=v, A=A, vraw=f.v)
 
 
 def test_inputs_are_su3(c1):
@@ -306,6 +306,35 @@ def test_block_orthonormality_and_RP_identity(c1):
     for chi in range(2):
         W = v[:, mask][:, :, 2 * chi:2 * chi + 2, :].reshape(cfg.nvec, -1)
         assert np.max(np.abs(W.conj() @ W.T - np.eye(cfg.nvec))) < 1e-14
+
+
+def test_orthonormalisation_is_the_qr_factor_with_positive_diagonal(c1):
+    """Gram-Schmidt in index order (reading Q6) computes, per aggregate (X, chi), the Q of the QR factorisation whose R
+    has a positive diagonal -- and that Q is unique.  numpy.linalg.qr (Householder, LAPACK) is an independent route to
+    it: its Q, with every column re-phased by the phase of R's diagonal entry, must equal the oracle's vectors column
+    by column.  This pins the ORDER in which the vectors are orthogonalised (the Gram matrix and R P = 1 are blind to
+    it), which the device set-up's parity test relies on."""
+    cfg = c1["cfg"]
+    raw = c1["vraw"]                                      # the Gaussian vectors the oracle orthonormalised
+    v = c1["v"]
+    L, b, nv = cfg.dims, cfg.block, cfg.nvec
+    coords = li.site_coords(L)                           # (V, 4)
+    cidx = sum((coords[:, mu] // b[mu]) * int(np.prod(cfg.cdims[:mu])) for mu in range(4))
+    checked = 0
+    for X in range(cfg.cvolume):
+        sites = np.nonzero(cidx == X)[0]
+        for chi in range(2):
+            M = raw[:, sites][:, :, 2 * chi:2 * chi + 2, :].reshape(nv, -1).T      # columns = vectors
+            Q, R = np.linalg.qr(M)
+            d = np.diagonal(R)
+            Qp = Q * (d / np.abs(d))[None, :]                                     # R's diagonal made positive
+            got = v[:, sites][:, :, 2 * chi:2 * chi + 2, :].reshape(nv, -1).T
+            assert np.max(np.abs(got - Qp)) < 1e-13, (X, chi)
+            # triangularity: vector i lies in the span of the raw vectors 0..i
+            T = np.conj(got.T) @ M
+            assert np.max(np.abs(np.tril(T, -1))) < 1e-13
+            checked += 1
+    assert checked == 2 * cfg.cvolume
 
 
 def test_restrict_prolong_adjoint_and_definition(c1):
