@@ -323,6 +323,13 @@ int lqcd_coarse_bicgstab_f32(float* x, float* r_out, const float* b, const float
                              int niter, void* ws_dev, void* stream);
 int lqcd_coarse_bicgstab_f64(double* x, double* r_out, const double* b, const double* A, const int cdims[4], int nvec,
                              int niter, void* ws_dev, void* stream);
+/* The same solver on the HALF storage of the coarse matrix (Ah as for lqcd_coarse_mult_half): every application of D_c
+ * moves 5/9 of the matrix bytes.  Same workspace size; same recurrences, so the result differs from the nine-block
+ * solve only by the rounding of the operator applications. */
+int lqcd_coarse_bicgstab_half_f32(float* x, float* r_out, const float* b, const float* Ah, const int cdims[4], int nvec,
+                                  int niter, void* ws_dev, void* stream);
+int lqcd_coarse_bicgstab_half_f64(double* x, double* r_out, const double* b, const double* Ah, const int cdims[4],
+                                  int nvec, int niter, void* ws_dev, void* stream);
 
 /* The same for nrhs right-hand sides at once (x, r_out, b: nrhs coarse vectors back to back): nrhs independent
  * recurrences -- every right-hand side has its own alpha, omega, beta -- that share the applications of D_c through
@@ -349,6 +356,13 @@ int lqcd_mg_vcycle_f32(float* x, const float* b, const float* U, const float* cl
 int lqcd_mg_vcycle_f64(double* x, const double* b, const double* U, const double* clover, double kappa,
                        const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
                        const double* A, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
+/* The same V-cycle with the coarse matrix in half storage (its coarse solve is lqcd_coarse_bicgstab_half). */
+int lqcd_mg_vcycle_half_f32(float* x, const float* b, const float* U, const float* clover, float kappa,
+                            const int dims[4], const int bc[4], const int block[4], int nvec, const float* nullvecs,
+                            const float* Ah, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
+int lqcd_mg_vcycle_half_f64(double* x, const double* b, const double* U, const double* clover, double kappa,
+                            const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
+                            const double* Ah, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream);
 
 /* The V-cycle on nrhs right-hand sides at once (x, b: nrhs native spinors back to back): the restrictions, the coarse
  * solves (lqcd_coarse_bicgstab_mrhs, i.e. D_c on the tensor cores) and the prolongations are shared by all right-hand

@@ -34,6 +34,20 @@ class LqcdError(RuntimeError):
         super().__init__(f"{what} failed with code {code}: {msg}")
 
 
+_binding_error = None  # message of the most recent refusal by the binding itself (cleared by the next C call)
+
+
+class LqcdSizeError(LqcdError, ValueError):
+    """A call refused by the binding BEFORE it reaches the library: a tensor (or workspace, or face buffer) whose size
+    does not match the geometry.  Counts as LQCD_EINVAL (nothing is enqueued); also a ValueError."""
+
+    def __init__(self, msg: str):
+        global _binding_error
+        self.code = EINVAL
+        _binding_error = msg
+        RuntimeError.__init__(self, msg)
+
+
 def lib():
     return _lib.load()
 
@@ -86,6 +100,8 @@ def _stream(stream=None, *likes):
 
 
 def _check(rc: int, what: str):
+    global _binding_error
+    _binding_error = None
     if rc != 0:
         raise LqcdError(rc, what)
 
@@ -146,17 +162,17 @@ def _need(t, reals: int, name: str, exact: bool = True):
         return
     n = _reals(t)
     if (n != reals) if exact else (n < reals):
-        raise ValueError(f"{name}: tensor of {n} reals, the call needs {'' if exact else 'at least '}{reals}")
+        raise LqcdSizeError(f"{name}: tensor of {n} reals, the call needs {'' if exact else 'at least '}{reals}")
 
 
 def _need_bytes(t, nbytes: int, name: str):
     if t is None or isinstance(t, DevPtr):
         if nbytes > 0 and t is None:
-            raise ValueError(f"{name}: the call needs a workspace of {nbytes} bytes")
+            raise LqcdSizeError(f"{name}: the call needs a workspace of {nbytes} bytes")
         return
     have = int(t.numel()) * int(t.element_size())
     if have < nbytes:
-        raise ValueError(f"{name}: workspace of {have} bytes, the call needs {nbytes}")
+        raise LqcdSizeError(f"{name}: workspace of {have} bytes, the call needs {nbytes}")
 
 
 def _vol(dims) -> int:
@@ -169,11 +185,11 @@ def _vol(dims) -> int:
 def _need_faces(bufs, reals8, part_mask: int, name: str):
     """bufs[8]: a face buffer of at least reals8[f] reals for every face f of a partitioned direction."""
     if len(bufs) != 8:
-        raise ValueError(f"{name}: expected 8 face buffers (None for unpartitioned directions)")
+        raise LqcdSizeError(f"{name}: expected 8 face buffers (None for unpartitioned directions)")
     for f in range(8):
         if (int(part_mask) >> (f >> 1)) & 1:
             if bufs[f] is None:
-                raise ValueError(f"{name}[{f}]: missing face buffer of a partitioned direction")
+                raise LqcdSizeError(f"{name}[{f}]: missing face buffer of a partitioned direction")
             _need(bufs[f], int(reals8[f]), f"{name}[{f}]", exact=False)
 
 
@@ -222,7 +238,8 @@ def version() -> int:
 
 
 def last_error() -> str:
-    return lib().lqcd_last_error().decode()
+    """Text of the most recent failure: the library's (thread-local) string, or the binding's own refusal."""
+    return _binding_error if _binding_error is not None else lib().lqcd_last_error().decode()
 
 
 def launch_count() -> int:
@@ -568,16 +585,19 @@ def sap(x, r, b, U, clover, kappa, dims, bc, domain, n_sap=4, n_mr=6, initial_gu
                                              _ws_ptr(ws), _stream(stream, x, r, b, U)), "lqcd_sap")
     return x
 
-def coarse_bicgstab(x, b, A, cdims, nvec, niter, r_out=None, ws=None, stream=None):
-    """(1b) of PAPER.md:116: niter BiCGStab iterations (listing PAPER.md:71, M = 1, x0 = 0) for D_c x = b."""
+def coarse_bicgstab(x, b, A, cdims, nvec, niter, r_out=None, ws=None, half=False, stream=None):
+    """(1b) of PAPER.md:116: niter BiCGStab iterations (listing PAPER.md:71, M = 1, x0 = 0) for D_c x = b.
+    half: A is the half storage of the coarse matrix (pack_coarse_half)."""
     sfx = _same_dtype(x, b, A)
-    _need_coarse(cdims, nvec, (("x", x), ("b", b), ("r_out", r_out)), A)
+    _need_coarse(cdims, nvec, (("x", x), ("b", b), ("r_out", r_out)), None if half else A)
+    if half:
+        _need(A, native_coarse_half_reals(cdims, nvec), "Ah")
     if ws is None:
         nb = int(lib().lqcd_coarse_bicgstab_workspace_bytes(_i4(cdims), int(nvec), 4 if sfx == "f32" else 8))
         ws = torch.empty(nb, dtype=torch.uint8, device=x.device)
-    _check(getattr(lib(), f"lqcd_coarse_bicgstab_{sfx}")(_dev_ptr(x), _ws_ptr(r_out), _dev_ptr(b), _dev_ptr(A),
-                                                         _i4(cdims), int(nvec), int(niter), _dev_ptr(ws),
-                                                         _stream(stream, x, b, A, r_out)), "lqcd_coarse_bicgstab")
+    name = f"lqcd_coarse_bicgstab_{'half_' if half else ''}{sfx}"
+    _check(getattr(lib(), name)(_dev_ptr(x), _ws_ptr(r_out), _dev_ptr(b), _dev_ptr(A), _i4(cdims), int(nvec), int(niter),
+                                _dev_ptr(ws), _stream(stream, x, b, A, r_out)), name)
     return x
 
 
@@ -587,19 +607,22 @@ def mg_workspace(dims, block, nvec, dtype=torch.float32, device="cuda") -> torch
 
 
 def mg_vcycle(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, n_coarse=8, n_sap=4, n_mr=6, ws=None,
-              stream=None):
-    """x = M b: one V-cycle of the multigrid preconditioner."""
+              half=False, stream=None):
+    """x = M b: one V-cycle of the multigrid preconditioner.  half: A is the half storage."""
     sfx = _same_dtype(x, b, U, clover, nullvecs, A)
     _need_fine(dims, False, (("x", x), ("b", b)), U, clover)
     _need_transfer(dims, block, nvec, nullvecs=nullvecs)
-    _need_coarse(_cdims(dims, block), nvec, A=A)
+    if half:
+        _need(A, native_coarse_half_reals(_cdims(dims, block), nvec), "Ah")
+    else:
+        _need_coarse(_cdims(dims, block), nvec, A=A)
     if ws is None:
         ws = mg_workspace(dims, block, nvec, dtype=_rdtype(sfx), device=x.device)
     k = C.c_float(kappa) if sfx == "f32" else C.c_double(kappa)
-    _check(getattr(lib(), f"lqcd_mg_vcycle_{sfx}")(_dev_ptr(x), _dev_ptr(b), _dev_ptr(U), _dev_ptr(clover), k,
-                                                   _i4(dims), _i4(bc), _i4(block), int(nvec), _dev_ptr(nullvecs),
-                                                   _dev_ptr(A), int(n_coarse), int(n_sap), int(n_mr), _dev_ptr(ws),
-                                                   _stream(stream, x, b, U, clover)), "lqcd_mg_vcycle")
+    name = f"lqcd_mg_vcycle_{'half_' if half else ''}{sfx}"
+    _check(getattr(lib(), name)(_dev_ptr(x), _dev_ptr(b), _dev_ptr(U), _dev_ptr(clover), k, _i4(dims), _i4(bc),
+                                _i4(block), int(nvec), _dev_ptr(nullvecs), _dev_ptr(A), int(n_coarse), int(n_sap),
+                                int(n_mr), _dev_ptr(ws), _stream(stream, x, b, U, clover)), name)
     return x
 
 def coarse_mult_mrhs(out, inp, A, cdims, nvec, dagger=False, stream=None):

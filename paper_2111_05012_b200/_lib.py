@@ -70,7 +70,9 @@ for _p, _k in (("f32", _cf), ("f64", _cd)):
         f"lqcd_block_caxpy_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _vp]),
         f"lqcd_mr_domain_solve_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _cu, _ci, _vp, _vp]),
         f"lqcd_coarse_bicgstab_{_p}": (_ci, [_vp, _vp, _vp, _vp, _i4, _ci, _ci, _vp, _vp]),
+        f"lqcd_coarse_bicgstab_half_{_p}": (_ci, [_vp, _vp, _vp, _vp, _i4, _ci, _ci, _vp, _vp]),
         f"lqcd_mg_vcycle_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _vp, _vp, _ci, _ci, _ci, _vp, _vp]),
+        f"lqcd_mg_vcycle_half_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _i4, _ci, _vp, _vp, _ci, _ci, _ci, _vp, _vp]),
         f"lqcd_coarse_mult_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _i4, _ci, _ci, _cu, _vp]),
         f"lqcd_wilson_clover_mult_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _vp, _k, _i4, _i4, _ci, _cu, _vp]),
         f"lqcd_restrict_mrhs_{_p}": (_ci, [_vp, _vp, _vp, _i4, _i4, _ci, _ci, _vp]),

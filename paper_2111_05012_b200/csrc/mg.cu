@@ -226,10 +226,10 @@ static int red_ctas(int nrhs) {
 }
 
 template <typename T> struct BicgWs {  // carve-up of the caller's scratch (K vectors back to back each)
-    T *v, *s, *t, *p, *r, *part_a, *part_b, *sc;
-    static size_t bytes(long long n, int K) {
+    T *v, *s, *t, *p, *r, *part_a, *part_b, *sc, *half;
+    static size_t bytes(long long n, int K) {  // (+ the four scratch vectors of the half-storage operator)
         return 5 * align256((size_t)n * 2 * sizeof(T) * K) + 2 * align256((size_t)red_ctas(K) * K * 3 * sizeof(T)) +
-               align256((size_t)SC_COUNT * K * sizeof(T));
+               align256((size_t)SC_COUNT * K * sizeof(T)) + align256((size_t)n * 2 * sizeof(T) * 4);
     }
     void carve(void* ws, long long n, int K) {
         char* c = reinterpret_cast<char*>(ws);
@@ -241,13 +241,26 @@ template <typename T> struct BicgWs {  // carve-up of the caller's scratch (K ve
         r = (T*)c; c += vb;
         part_a = (T*)c; c += pb;
         part_b = (T*)c; c += pb;
-        sc = (T*)c;
+        sc = (T*)c; c += align256((size_t)SC_COUNT * K * sizeof(T));
+        half = (T*)c;
     }
 };
 
 // out_k = D_c in_k for K vectors back to back: one pass over A on the tensor cores where that applies (coarse_mrhs.cu)
 template <typename T>
 static int coarse_mult_any(T* out, const T* in, const T* A, const int cdims[4], int nvec, int K, void* st);
+template <typename T>
+static int coarse_mult_half_any(T* out, const T* in, const T* Ah, const int cdims[4], int nvec, void* ws, void* st);
+template <>
+int coarse_mult_half_any<float>(float* out, const float* in, const float* Ah, const int cdims[4], int nvec, void* ws,
+                                void* st) {
+    return lqcd_coarse_mult_half_f32(out, in, Ah, cdims, nvec, 0, ws, st);
+}
+template <>
+int coarse_mult_half_any<double>(double* out, const double* in, const double* Ah, const int cdims[4], int nvec, void* ws,
+                                 void* st) {
+    return lqcd_coarse_mult_half_f64(out, in, Ah, cdims, nvec, 0, ws, st);
+}
 template <>
 int coarse_mult_any<float>(float* out, const float* in, const float* A, const int cdims[4], int nvec, int K, void* st) {
     if (K == 1) return lqcd_coarse_mult_f32(out, in, A, cdims, nvec, 0, st);
@@ -272,8 +285,13 @@ struct BicgHooks {
 
 template <typename T>
 static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims[4], int nvec, int K, int niter,
-                         void* ws, void* stream, const char* what, const BicgHooks* H = nullptr) {
+                         void* ws, void* stream, const char* what, const BicgHooks* H = nullptr, bool half = false) {
+    // half: A is the half storage of the coarse matrix (lqcd_coarse_mult_half); single right-hand side only
     clear_error();
+    if (half && (K != 1 || (H && H->apply))) {
+        set_error("%s: half storage takes one right-hand side and no apply hook", what);
+        return LQCD_EINVAL;
+    }
     if (H && H->apply && !A) A = b;  // never read: the hook applies the operator
     if (!x || !b || !A || !ws || check_dims(cdims) || nvec < 1 || niter < 0 || K < 1 || K > 65535) {
         set_error("%s: null pointer, non-positive dim, nvec < 1, niter < 0 or nrhs outside 1..65535", what);
@@ -307,6 +325,7 @@ static int bicgstab_call(T* x, T* r_out, const T* b, const T* A, const int cdims
             }
             return LQCD_OK;
         }
+        if (half) return coarse_mult_half_any<T>(out, in, A, cdims, nvec, W.half, stream);
         return coarse_mult_any<T>(out, in, A, cdims, nvec, K, stream);
     };
     auto allreduce = [&](T* part) -> int {  // the partial sums of every rank, element by element
@@ -407,7 +426,7 @@ static size_t mg_ws_bytes(const int dims[4], const int block[4], int nvec, int K
 template <typename T>
 static int vcycle_call(T* x, const T* b, const T* U, const T* clover, T kappa, const int dims[4], const int bc[4],
                        const int block[4], int nvec, const T* nullvecs, const T* A, int K, int n_coarse, int n_sap,
-                       int n_mr, void* ws, void* stream, const char* what) {
+                       int n_mr, void* ws, void* stream, const char* what, bool half = false) {
     clear_error();
     int cd[4];
     if (!x || !b || !U || !clover || !nullvecs || !A || !ws || !bc || check_block(dims, block, nvec, cd)) {
@@ -445,7 +464,8 @@ static int vcycle_call(T* x, const T* b, const T* U, const T* clover, T kappa, c
     } else if ((rc = FineCalls<T>::restrict_mrhs_(bcv, b, nullvecs, dims, block, nvec, K, stream))) {
         return rc;
     }
-    if ((rc = bicgstab_call<T>(xcv, nullptr, bcv, A, cd, nvec, K, n_coarse, bicg_ws, stream, what))) return rc;  // (1b)
+    if ((rc = bicgstab_call<T>(xcv, nullptr, bcv, A, cd, nvec, K, n_coarse, bicg_ws, stream, what, nullptr, half)))
+        return rc;  // (1b)
     if (K == 1) {
         if ((rc = FineCalls<T>::prolong_(x, xcv, nullvecs, dims, block, nvec, stream))) return rc;         // (1c) Eq. 6
     } else if ((rc = FineCalls<T>::prolong_mrhs_(x, xcv, nullvecs, dims, block, nvec, K, stream))) {
@@ -514,6 +534,17 @@ int lqcd_coarse_bicgstab_f64(double* x, double* r_out, const double* b, const do
     return bicgstab_call<double>(x, r_out, b, A, cdims, nvec, 1, niter, ws_dev, stream, "lqcd_coarse_bicgstab_f64");
 }
 
+int lqcd_coarse_bicgstab_half_f32(float* x, float* r_out, const float* b, const float* Ah, const int cdims[4], int nvec,
+                                  int niter, void* ws_dev, void* stream) {
+    return bicgstab_call<float>(x, r_out, b, Ah, cdims, nvec, 1, niter, ws_dev, stream, "lqcd_coarse_bicgstab_half_f32",
+                                nullptr, true);
+}
+int lqcd_coarse_bicgstab_half_f64(double* x, double* r_out, const double* b, const double* Ah, const int cdims[4],
+                                  int nvec, int niter, void* ws_dev, void* stream) {
+    return bicgstab_call<double>(x, r_out, b, Ah, cdims, nvec, 1, niter, ws_dev, stream, "lqcd_coarse_bicgstab_half_f64",
+                                 nullptr, true);
+}
+
 size_t lqcd_mg_workspace_bytes(const int dims[4], const int block[4], int nvec, int real_bytes) {
     if (real_bytes != 4 && real_bytes != 8) return 0;
     return mg_ws_bytes(dims, block, nvec, 1, real_bytes);
@@ -545,5 +576,17 @@ int lqcd_mg_vcycle_f64(double* x, const double* b, const double* U, const double
                        const double* A, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream) {
     return vcycle_call<double>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, A, 1, n_coarse, n_sap, n_mr,
                                ws_dev, stream, "lqcd_mg_vcycle_f64");
+}
+int lqcd_mg_vcycle_half_f32(float* x, const float* b, const float* U, const float* clover, float kappa,
+                            const int dims[4], const int bc[4], const int block[4], int nvec, const float* nullvecs,
+                            const float* Ah, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream) {
+    return vcycle_call<float>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, Ah, 1, n_coarse, n_sap, n_mr,
+                              ws_dev, stream, "lqcd_mg_vcycle_half_f32", true);
+}
+int lqcd_mg_vcycle_half_f64(double* x, const double* b, const double* U, const double* clover, double kappa,
+                            const int dims[4], const int bc[4], const int block[4], int nvec, const double* nullvecs,
+                            const double* Ah, int n_coarse, int n_sap, int n_mr, void* ws_dev, void* stream) {
+    return vcycle_call<double>(x, b, U, clover, kappa, dims, bc, block, nvec, nullvecs, Ah, 1, n_coarse, n_sap, n_mr,
+                               ws_dev, stream, "lqcd_mg_vcycle_half_f64", true);
 }
 }

@@ -485,7 +485,9 @@ def test_fullsize_device_setup_sampled(lq):
     mc = li.site_coords(mdims)                                           # (20736, 4) fine coordinates in the mini lattice
     gathers = []
     for X, off in samples:
-        real_c = np.stack([((X[mu] + mc[:, mu] // b[mu] - off[mu]) % Lc[mu]) * b[mu] + mc[:, mu] % b[mu]
+        # mini aggregate m <-> real aggregate X + delta, delta = ((m - off + 1) mod 3) - 1 in {-1, 0, +1}: cyclic, so a
+        # hop that wraps the mini lattice arrives at the aggregate the real hop arrives at
+        real_c = np.stack([((X[mu] + (mc[:, mu] // b[mu] - off[mu] + 1) % 3 - 1) % Lc[mu]) * b[mu] + mc[:, mu] % b[mu]
                            for mu in range(4)], axis=1)
         gathers.append(torch.from_numpy(site_index(L, real_c).astype(np.int64)).cuda())
     raw = [np.empty((nv, len(mc), 4, 3), dtype=np.complex64) for _ in samples]
@@ -500,9 +502,10 @@ def test_fullsize_device_setup_sampled(lq):
     A = lq.galerkin_coarse(U18, clover, vn, cfg.kappa, L, cfg.bc, b, nv)
     clov_c = lq.unpack_clover(clover, L)                                 # canonical (V, 2, 6, 6)
     for k, ((X, off), g) in enumerate(zip(samples, gathers)):
-        Um = np.ascontiguousarray(U[:, g].cpu().numpy())
+        # the fp32-rounded inputs, promoted: the oracle's set-up chain runs in fp64 from here on
+        Um = np.ascontiguousarray(U[:, g].cpu().numpy()).astype(np.complex128)
         clov_ref = oracle.clover_from_links(Um, cfg.kappa, cfg.csw, mdims)
-        v_ref = oracle.orthonormalize_blocks(raw[k], mdims, b)
+        v_ref = oracle.orthonormalize_blocks(raw[k].astype(np.complex128), mdims, b)
         A_ref = oracle.galerkin_coarse(Um, clov_ref, v_ref, cfg.kappa, mdims, cfg.bc, b)
         mX = int(site_index(mcd, np.array(off)))                         # X inside the mini coarse lattice
         Xr = int(site_index(Lc, np.array(X)))

@@ -137,8 +137,49 @@ def test_half_storage_error_codes(lq):
     st = torch.cuda.current_stream().cuda_stream
     rc = lq.lib().lqcd_coarse_mult_half_f32(y.data_ptr(), x.data_ptr(), Ah.data_ptr(), lq._i4((2, 2, 1, 2)), cfg.nvec, 0,
                                             ws.data_ptr(), st)
-    assert rc == lq.EINVAL and "extent" in lq.last_error()
+    assert rc == lq.EINVAL and "extent" in lq.lib().lqcd_last_error().decode()
     rc = lq.lib().lqcd_coarse_mult_half_f32(y.data_ptr(), x.data_ptr(), Ah.data_ptr(), lq._i4(cfg.cdims), cfg.nvec, 4,
                                             ws.data_ptr(), st)
     assert rc == lq.EINVAL, "unknown flag"
     assert lq.launch_count() == n0, "an erroring call must not enqueue anything"
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_solvers_on_half_storage(lq, name, prec):
+    """The coarse BiCGStab and the V-cycle with the coarse matrix in half storage against the oracle's solver on the
+    nine-block Galerkin matrix (same recurrences; only the operator application differs)."""
+    import torch
+    from problems import check_bar
+    from test_gpu_parity import Dev
+    prob = config_problem(name, 16 if name == "c2" else 1)
+    cfg = prob.cfg
+    d = Dev(lq, prob, prec)
+    Ah = lq.pack_coarse_half(d.A, cfg.cdims, cfg.nvec)
+    M = np.zeros((cfg.cvolume * 2 * cfg.nvec,) * 2, dtype=np.complex128) if cfg.cvolume * 2 * cfg.nvec <= 512 else None
+    cond = 30.0
+    if M is not None:  # dense D_c from the oracle's operator, for the principled bound
+        n = M.shape[0]
+        for j in range(n):
+            e = np.zeros(n, dtype=np.complex128)
+            e[j] = 1
+            M[:, j] = oracle.coarse_mult(e.reshape(cfg.cvolume, 2, cfg.nvec), prob.A, cfg.cdims).ravel()
+        cond = float(np.linalg.cond(M))
+    b = to_dev(prob.xc, prec)
+    for niter in (1, 5):
+        x, r = torch.full_like(b, 3.0), torch.full_like(b, 3.0)
+        lq.coarse_bicgstab(x, b, Ah, cfg.cdims, cfg.nvec, niter, r_out=r, half=True)
+        rx, rr = oracle.coarse_bicgstab(rounded(prob.xc, prec), rounded(prob.A, prec), cfg.cdims, cfg.nvec, niter)
+        check_bar(rel_l2(x.cpu().numpy(), rx), 2 * niter * cond * TOL[prec], prec, f"bicgstab half {name} {niter}")
+        check_bar(np.linalg.norm(r.cpu().numpy() - rr) / np.linalg.norm(prob.xc), 2 * niter * cond * TOL[prec], prec,
+                  f"bicgstab half residual {name} {niter}")
+    n_coarse, n_sap, n_mr = 4, 2, 4
+    bn = lq.pack_spinor(to_dev(prob.psi[0], prec), cfg.dims)
+    xv = lq.empty_spinor(cfg.dims, dtype=bn.dtype)
+    lq.mg_vcycle(xv, bn, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, cfg.nvec, d.v, Ah, n_coarse=n_coarse,
+                 n_sap=n_sap, n_mr=n_mr, half=True)
+    ref = oracle.mg_vcycle(rounded(prob.psi[0], prec), rounded(prob.U, prec), rounded(prob.clover, prec), cfg.kappa,
+                           cfg.dims, cfg.bc, cfg.block, rounded(prob.v, prec), rounded(prob.A, prec), n_coarse=n_coarse,
+                           n_sap=n_sap, n_mr=n_mr)
+    bar = (2 * n_coarse * cond + 2 + 2 * n_sap * (n_mr + 1)) * TOL[prec]
+    check_bar(rel_l2(lq.unpack_spinor(xv, cfg.dims).cpu().numpy(), ref), bar, prec, f"vcycle half {name}")

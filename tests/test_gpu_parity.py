@@ -350,7 +350,7 @@ def test_error_codes(lq):
     i4, st = lq._i4, torch.cuda.current_stream().cuda_stream
     rc = lq.lib().lqcd_wilson_clover_mult_f32(y.data_ptr() + 4, x.data_ptr(), d.U.data_ptr(), d.clover.data_ptr(),
                                               cfg.kappa, i4(cfg.dims), i4(cfg.bc), 0, st)
-    assert rc == lq.EINVAL and "aligned" in lq.last_error()
+    assert rc == lq.EINVAL and "aligned" in lq.lib().lqcd_last_error().decode()
     xc = to_dev(prob.xc, "f32")
     yc = torch.empty_like(xc)
     with pytest.raises(ValueError, match="needs"):
