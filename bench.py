@@ -824,6 +824,15 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
                             "units_per_s": md["units"] / t, "frac_of_hbm_peak": md["bytes"] / t / 1e9 / peak,
                             "bytes_per_launch": md["bytes"],
                             "path": "generic" if nb else "shared-memory-resident"}
+            if label == "mr_domain_solve_even" and not nb and clocks.get("sm_mhz"):
+                # the resident solver is bound by SHARED-MEMORY bandwidth, not HBM: per site and
+                # iteration 8 neighbour spinors (96 B) + 8 links (72 B) + the clover term (288 B) + the store and the
+                # exchange of rho (2 x 96 B) = 1824 B of LDS / STS traffic; roof = 128 B/clk/SM x 148 SMs x SM clock
+                smem_b = 1824.0 * (cfg.volume / 2) * 6
+                roof = 128.0 * 148 * clocks["sm_mhz"] * 1e6
+                extra[label]["roofline"] = {"bound": "shared-memory bandwidth", "achieved": smem_b / t / 1e12,
+                                            "peak": roof / 1e12, "unit": "TB/s", "frac": smem_b / t / roof,
+                                            "bytes_per_site_iteration": 1824, "sm_mhz": clocks["sm_mhz"]}
         W.lq.set_knob("sap_fused", 0)
         # one V-cycle x = M b of the preconditioner: restrict, 8 BiCGStab iterations on D_c,
         # prolong, SAP(4, 6) -- everything on one stream, no host synchronisation
