@@ -23,8 +23,12 @@
  *   coarse mat  A[X][d][row][col], d = 0 diag, 1+2mu forward, 2+2mu backward   Vc*9*N*N complex
  *
  * NATIVE layouts (what the mult kernels consume; sizes from lqcd_native_*_reals; R = real type,
- * a "vec16" is 16 bytes = 4 floats or 2 doubles; sites are grouped in chunks of 32 canonical-
- * consecutive sites, chunk = s / 32, lane = s % 32, nchunk = ceil(V / 32)):
+ * a "vec16" is 16 bytes = 4 floats or 2 doubles; sites are grouped in chunks of 32: site s sits at
+ * native position n(s), chunk = n / 32, lane = n % 32, nchunk = ceil(V / 32).  Site order: when
+ * Lx % 4 == Ly % 4 == Lz % 2 == 0 a chunk is a 4 x 4 x 2 tile of sites (x, y, z), tiles in
+ * lexicographic order, n = 32 (x/4 + (Lx/4) (y/4 + (Ly/4) (z/2 + (Lz/2) t))) + x%4 + 4 (y%4) + 16 (z%2)
+ * -- every 128-byte line then belongs to one 4^4 domain; otherwise n(s) = s (canonical order).  The
+ * native layouts are opaque to callers: pack / unpack are the only calls that speak them):
  *   spinor   [chunk][j][lane] vec16, j = 0..24/nv-1 over the 24 reals r = 2*(3 alpha + c) + reim
  *   gauge18  [chunk][mu][18 reals as 18/nv full vec16 rows of 32 lanes, then (f32 only) one row of
  *            32 float2 holding reals 16,17], reals r = 2*(3a+b)+reim

@@ -3,6 +3,7 @@
 // |block|*6 complex per (X, chi, i).
 #pragma once
 #include "common.cuh"
+#include "layout.cuh"
 
 namespace lqcd {
 
@@ -11,21 +12,21 @@ struct TransferParams {
     int bv;    // sites per block
     int nvec;
     int LV;    // vec16 per (X, chi, i) vector = bv * 12 / NV
+    SiteOrder ord;  // native position of a fine site (layout.cuh)
 };
 
-// canonical fine site of local index l inside coarse site X
+// native position of the fine site with local index l inside coarse site X
 __device__ __forceinline__ int fine_site(const TransferParams& P, int X, int l) {
-    int s = 0, stride = 1;
+    int x[4];
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) {
         const int Xmu = X % P.Lc[mu];
         X /= P.Lc[mu];
         const int lmu = l % P.b[mu];
         l /= P.b[mu];
-        s += (Xmu * P.b[mu] + lmu) * stride;
-        stride *= P.L[mu];
+        x[mu] = Xmu * P.b[mu] + lmu;
     }
-    return s;
+    return P.ord.index(x);
 }
 
 template <typename T>
@@ -53,6 +54,7 @@ inline int transfer_setup(TransferParams& P, const void* a, const void* b, const
     }
     P.nvec = nvec;
     P.LV = P.bv * 12 / VecOf<T>::NV;
+    P.ord.set(dims);
     return LQCD_OK;
 }
 

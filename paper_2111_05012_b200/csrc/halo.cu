@@ -25,24 +25,22 @@ struct HaloParams {
     int fv[4];        // face volume V / L[mu]
     int phase[8];     // +1 / -1 per receive face (2 mu + dir)
     unsigned mask;    // partitioned directions
+    SiteOrder ord;    // native position of a site (layout.cuh)
 };
 
-// face site f of direction mu at x_mu = xm -> lexicographic site index
+// face site f of direction mu at x_mu = xm -> native position of that site
 __device__ __forceinline__ int face_site(const HaloParams& P, int mu, int f, int xm) {
-    int s = 0, stride = 1;
+    int x[4];
 #pragma unroll
     for (int nu = 0; nu < 4; nu++) {
-        int c;
         if (nu == mu) {
-            c = xm;
+            x[nu] = xm;
         } else {
-            c = f % P.L[nu];
+            x[nu] = f % P.L[nu];
             f /= P.L[nu];
         }
-        s += c * stride;
-        stride *= P.L[nu];
     }
-    return s;
+    return P.ord.index(x);
 }
 
 template <typename T> __device__ __forceinline__ void store_half(T* __restrict__ buf, int fv, int f, const T h[12]) {
@@ -165,6 +163,7 @@ static int halo_setup(HaloParams& P, const int dims[4], unsigned part_mask, unsi
     }
     for (int i = 0; i < 8; i++) P.phase[i] = 1;
     P.mask = part_mask;
+    P.ord.set(dims);
     return LQCD_OK;
 }
 

@@ -14,6 +14,8 @@ struct Knobs {
     int mrhs_stages = 0;              // pipeline stages of coarse_mult_mrhs, 0 = as many as fit
     int fine_mrhs = 0;                // -1 = wilson_clover_mult_mrhs applies the single-right-hand-side kernel per vector
     int sap_fused = 0;                // 0 = shared-memory-resident inner-domain solver when it fits; -1 = never
+    int site_order = 0;               // 0 = tiled site order (4 x 4 x 2 chunks) when the extents allow; -1 = canonical.
+                                      // Changes the NATIVE layout: every native field must be packed after setting it
     int sap_group_residual = 0;       // 0 = SAP's intermediate residuals on the next group's domains only; -1 = all sites
 };
 extern thread_local Knobs g_knobs;

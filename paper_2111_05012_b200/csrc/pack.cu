@@ -7,11 +7,11 @@
 namespace lqcd {
 
 template <typename T, bool UNPACK>
-__global__ void k_spinor(T* __restrict__ dst, const T* __restrict__ src, long long V) {
+__global__ void k_spinor(T* __restrict__ dst, const T* __restrict__ src, long long V, SiteOrder ord) {
     const long long n = V * 24;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
          idx += (long long)gridDim.x * blockDim.x) {
-        const long long s = idx / 24;
+        const long long s = ord.from_canonical((int)(idx / 24));  // native position of canonical site idx / 24
         const int r = (int)(idx % 24);
         if (UNPACK) dst[idx] = src[spinor_off<T>(s, r)];
         else dst[spinor_off<T>(s, r)] = src[idx];
@@ -19,13 +19,14 @@ __global__ void k_spinor(T* __restrict__ dst, const T* __restrict__ src, long lo
 }
 
 // canonical U[mu][s][a][b] -> native [chunk][mu][...]
-template <typename T, bool L12> __global__ void k_gauge(T* __restrict__ dst, const T* __restrict__ src, long long V) {
+template <typename T, bool L12>
+__global__ void k_gauge(T* __restrict__ dst, const T* __restrict__ src, long long V, SiteOrder ord) {
     const long long n = 4 * V * 18;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
          idx += (long long)gridDim.x * blockDim.x) {
         const int r = (int)(idx % 18);
         const long long ms = idx / 18;
-        const long long s = ms % V;
+        const long long s = ord.from_canonical((int)(ms % V));
         const int mu = (int)(ms / V);
         if (L12) {
             if (r < 12) dst[gauge12_off<T>(s, mu, r)] = src[idx];
@@ -37,7 +38,8 @@ template <typename T, bool L12> __global__ void k_gauge(T* __restrict__ dst, con
 
 // canonical F[s][chi][k][l] complex -> native 72 reals: diagonal real parts, strictly-lower entries.
 // The Hermitian part (F + F^dag)/2 of the input is what is stored.
-template <typename T> __global__ void k_clover(T* __restrict__ dst, const T* __restrict__ src, long long V) {
+template <typename T>
+__global__ void k_clover(T* __restrict__ dst, const T* __restrict__ src, long long V, SiteOrder ord) {
     const long long n = V * 72;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
          idx += (long long)gridDim.x * blockDim.x) {
@@ -57,16 +59,17 @@ template <typename T> __global__ void k_clover(T* __restrict__ dst, const T* __r
             const T up = blk[(l * 6 + k) * 2 + reim];
             val = reim ? (T)0.5 * (lo - up) : (T)0.5 * (lo + up);
         }
-        dst[clover_off<T>(s, r)] = val;
+        dst[clover_off<T>((long long)ord.from_canonical((int)s), r)] = val;
     }
 }
 
 // native 72 reals -> canonical full Hermitian blocks F[s][chi][k][l] complex
-template <typename T> __global__ void k_clover_unpack(T* __restrict__ dst, const T* __restrict__ src, long long V) {
+template <typename T>
+__global__ void k_clover_unpack(T* __restrict__ dst, const T* __restrict__ src, long long V, SiteOrder ord) {
     const long long n = V * 72;  // one thread per (site, chi, k, l)
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
          idx += (long long)gridDim.x * blockDim.x) {
-        const long long s = idx / 72;
+        const long long s = ord.from_canonical((int)(idx / 72));
         const int e = (int)(idx % 72), chi = e / 36, k = (e % 36) / 6, l = e % 6;
         T re, im;
         if (k == l) {
@@ -129,7 +132,10 @@ static int spinor_call(T* dst, const T* src, const int dims[4], void* stream, co
         return LQCD_EINVAL;
     }
     const long long V = volume(dims);
-    k_spinor<T, UNPACK><<<grid_for(V * 24), 256, 0, (cudaStream_t)stream>>>(dst, src, V);
+    if (V > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
+    SiteOrder ord;
+    ord.set(dims);
+    k_spinor<T, UNPACK><<<grid_for(V * 24), 256, 0, (cudaStream_t)stream>>>(dst, src, V, ord);
     count_launch();
     return check_launch(what);
 }
@@ -143,10 +149,13 @@ static int gauge_call(T* dst, const T* src, const int dims[4], unsigned flags, v
         return LQCD_EINVAL;
     }
     const long long V = volume(dims);
+    if (V > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
+    SiteOrder ord;
+    ord.set(dims);
     if (flags & LQCD_LINKS_12)
-        k_gauge<T, true><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V);
+        k_gauge<T, true><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V, ord);
     else
-        k_gauge<T, false><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V);
+        k_gauge<T, false><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V, ord);
     count_launch();
     return check_launch(what);
 }
@@ -158,7 +167,10 @@ template <typename T> static int clover_call(T* dst, const T* src, const int dim
         return LQCD_EINVAL;
     }
     const long long V = volume(dims);
-    k_clover<T><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V);
+    if (V > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
+    SiteOrder ord;
+    ord.set(dims);
+    k_clover<T><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V, ord);
     count_launch();
     return check_launch(what);
 }
@@ -171,7 +183,10 @@ static int clover_unpack_call(T* dst, const T* src, const int dims[4], void* str
         return LQCD_EINVAL;
     }
     const long long V = volume(dims);
-    k_clover_unpack<T><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V);
+    if (V > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
+    SiteOrder ord;
+    ord.set(dims);
+    k_clover_unpack<T><<<grid_for(V * 72), 256, 0, (cudaStream_t)stream>>>(dst, src, V, ord);
     count_launch();
     return check_launch(what);
 }

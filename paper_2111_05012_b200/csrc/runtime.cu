@@ -102,6 +102,7 @@ int lqcd_set_knob(const char* name, int value) {
     else if (!strcmp(name, "sap_group_residual")) g_knobs.sap_group_residual = value;
     else if (!strcmp(name, "fine_mrhs")) g_knobs.fine_mrhs = value;
     else if (!strcmp(name, "mrhs_tensor")) g_knobs.mrhs_tensor = value;
+    else if (!strcmp(name, "site_order")) g_knobs.site_order = value;
     else if (!strcmp(name, "mrhs_stages")) g_knobs.mrhs_stages = value;
     else {
         set_error("lqcd_set_knob: unknown knob '%s'", name);

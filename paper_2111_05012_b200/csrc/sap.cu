@@ -35,6 +35,7 @@ struct DomParams {
     int bv, Vc;
     int parity;    // 0 = all domains, 1 = even, 2 = odd
     int halfgrid;  // 1: the grid enumerates only the domains of the selected group (needs Lc[0] even)
+    SiteOrder ord; // native position of a site (layout.cuh)
 };
 
 // Coarse coordinates of the domain of CTA b; false if that domain is not in the selected group.
@@ -59,17 +60,16 @@ __device__ __forceinline__ bool domain_of_cta(const DomParams& P, int b, int Xc[
     return P.parity == 0 || ((Xc[0] + Xc[1] + Xc[2] + Xc[3]) & 1) == P.parity - 1;
 }
 
-// local coordinates of local index l (x fastest) and the canonical fine site
+// local coordinates of local index l (x fastest) and the NATIVE position of that fine site
 __device__ __forceinline__ int domain_site(const DomParams& P, const int Xc[4], int l, int lx[4]) {
-    int s = 0, stride = 1;
+    int x[4];
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) {
         lx[mu] = l % P.dom[mu];
         l /= P.dom[mu];
-        s += (Xc[mu] * P.dom[mu] + lx[mu]) * stride;
-        stride *= P.L[mu];
+        x[mu] = Xc[mu] * P.dom[mu] + lx[mu];
     }
-    return s;
+    return P.ord.index(x);
 }
 
 // Sum of NRED partial sums per thread over the CTA, same bits in every thread; fixed order (warp tree, then warps in
@@ -553,6 +553,7 @@ static int dom_setup(DomParams& P, const int dims[4], const int bc[4], const int
     }
     P.parity = 0;
     P.halfgrid = 0;
+    P.ord.set(dims);
     return LQCD_OK;
 }
 

@@ -55,6 +55,7 @@ template <bool ADJA, bool ADJB, typename T> __device__ __forceinline__ M3<T> mul
 struct CloverParams {
     int L[4];
     int V;
+    SiteOrder ord;  // native position of a site (layout.cuh)
 };
 
 __device__ __forceinline__ int shifted(const CloverParams& P, const int x[4], int mu, int dmu, int nu, int dnu) {
@@ -65,7 +66,7 @@ __device__ __forceinline__ int shifted(const CloverParams& P, const int x[4], in
     y[nu] += dnu;
     if (y[nu] >= P.L[nu]) y[nu] -= P.L[nu];
     if (y[nu] < 0) y[nu] += P.L[nu];
-    return y[0] + P.L[0] * (y[1] + P.L[1] * (y[2] + P.L[2] * y[3]));
+    return P.ord.index(y);  // native position
 }
 
 // Hermitian 3x3 F_{mu nu}(x) = (Q - Q^dag) / (8 i), Q = sum of the four plaquette leaves in the mu-nu plane that
@@ -129,13 +130,14 @@ __device__ void field_strength(T f[18], const T* __restrict__ U, const CloverPar
 template <typename T>
 __global__ void __launch_bounds__(128) k_clover_from_links(T* __restrict__ clover, const T* __restrict__ U, T coef,
                                                            CloverParams P) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= P.V) return;
-    int x[4], r = s;
+    const int sc = blockIdx.x * blockDim.x + threadIdx.x;  // canonical site index
+    if (sc >= P.V) return;
+    int x[4], r = sc;
     x[0] = r % P.L[0]; r /= P.L[0];
     x[1] = r % P.L[1]; r /= P.L[1];
     x[2] = r % P.L[2]; r /= P.L[2];
     x[3] = r;
+    const int s = P.ord.index(x);  // native position: what every field access below takes
     T B1[18], B2[18], B3[18], E[18];
     field_strength(B3, U, P, x, s, 0, 1);  // xy
     field_strength(B2, U, P, x, s, 0, 2);  // xz (enters with a minus sign)
@@ -202,6 +204,7 @@ static int clover_from_links_call(T* clover, const T* U, T kappa, T csw, const i
     CloverParams P;
     for (int mu = 0; mu < 4; mu++) P.L[mu] = dims[mu];
     P.V = (int)volume(dims);
+    P.ord.set(dims);
     k_clover_from_links<T><<<(P.V + 127) / 128, 128, 0, (cudaStream_t)stream>>>(clover, U, kappa * csw, P);
     count_launch();
     return check_launch(what);
@@ -353,31 +356,29 @@ __global__ void __launch_bounds__(256) k_prolongator_column(T* __restrict__ out_
 struct HopParams {
     int L[4], b[4], multi[4], bc[4];
     int V;
+    SiteOrder ord;  // native position of a site (layout.cuh)
 };
 
 // out(x) = -kappa beta (1 -+ g_mu) U in(x +- mu) if that hop leaves the aggregate of x, else 0
 template <typename T, int MU, bool FWD>
 __global__ void __launch_bounds__(128) k_hop_cross(T* __restrict__ out, const T* __restrict__ in, const T* __restrict__ U,
                                                    T kappa, HopParams P) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= P.V) return;
-    int x[4], r = s;
+    const int sc = blockIdx.x * blockDim.x + threadIdx.x;  // canonical site index
+    if (sc >= P.V) return;
+    int x[4], r = sc;
     x[0] = r % P.L[0]; r /= P.L[0];
     x[1] = r % P.L[1]; r /= P.L[1];
     x[2] = r % P.L[2]; r /= P.L[2];
     x[3] = r;
+    const int s = P.ord.index(x);  // native position
     T acc[24];
 #pragma unroll
     for (int k = 0; k < 24; k++) acc[k] = 0;
     const int lx = x[MU] % P.b[MU];
     const bool crosses = P.multi[MU] && (FWD ? lx == P.b[MU] - 1 : lx == 0);
     if (crosses) {
-        int stride = 1;
-#pragma unroll
-        for (int mu = 0; mu < MU; mu++) stride *= P.L[mu];
         const bool wraps = FWD ? x[MU] == P.L[MU] - 1 : x[MU] == 0;
-        const int nb = FWD ? (wraps ? s - (P.L[MU] - 1) * stride : s + stride)
-                           : (wraps ? s + (P.L[MU] - 1) * stride : s - stride);
+        const int nb = FWD ? P.ord.fwd(s, MU, x[MU]) : P.ord.bwd(s, MU, x[MU]);
         const T ph = -kappa * (wraps ? (T)P.bc[MU] : (T)1);
         T p[24], h[12], u[18], g[12];
         load_spinor<T>(p, in, nb);
@@ -454,6 +455,7 @@ static int galerkin_call(T* A, const T* U, const T* clover, const T* v, T kappa,
         H.bc[mu] = bc[mu];
     }
     H.V = (int)volume(dims);
+    H.ord.set(dims);
     cudaStream_t st = (cudaStream_t)stream;
     const long long Vc = volume(P.Lc);
     // vectors back to back, as restrict_mrhs_call expects them (every size is a multiple of 16 bytes)

@@ -24,6 +24,9 @@ struct FineParams {
     int ntile[4];  // tiles per direction
     int bc[4];     // +1 / -1
     int tilevol;   // threads that own a site (<= blockDim.x)
+    int warp_tiles;  // 1: tiled site order and a CTA tile made of whole 4 x 4 x 2 layout tiles: a warp owns one of them
+    int wt[3];       // ... layout tiles per CTA tile in x, y, z
+    FastDiv d_wt[3];
     int zslab;     // traversal slab extent in z tiles (0 = canonical tile order)
     int per_slab, nslab_full;  // zslab * ntile[3]; number of slabs of full height
     FastDiv d_ntile[3], d_tile[3], d_per_slab, d_zslab, d_dom[4];
@@ -33,6 +36,7 @@ struct FineParams {
     int parity;    // 0 = all domains, 1 = even domains only, 2 = odd domains only
     int keep;      // with parity != 0: 1 = leave the sites of the other group untouched instead of zeroing them
     int cut_lat;   // 1 = hops are cut where they leave the LATTICE (sharded interior pass), not where they leave a domain
+    SiteOrder ord;  // native position of a site (layout.cuh)
 };
 
 // Which site is mine: CTA -> tile (x tiles fastest; optionally z-slabbed traversal), thread -> site in tile.  All
@@ -62,12 +66,24 @@ __device__ __forceinline__ bool fine_decode(const FineParams& P, int x[4], int& 
         tc[3] = P.d_ntile[2].div(b);
         tc[2] = b - tc[3] * P.ntile[2];
     }
-    q = P.d_tile[0].div(tid); x[0] = tc[0] * P.tile[0] + (tid - q * P.tile[0]); tid = q;
-    q = P.d_tile[1].div(tid); x[1] = tc[1] * P.tile[1] + (tid - q * P.tile[1]); tid = q;
-    q = P.d_tile[2].div(tid); x[2] = tc[2] * P.tile[2] + (tid - q * P.tile[2]); tid = q;
-    x[3] = tc[3] * P.tile[3] + tid;
-    const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
-    s_out = x[0] + st1 * x[1] + st2 * x[2] + st3 * x[3];
+    if (P.warp_tiles) {
+        // lane = position inside a 4 x 4 x 2 layout tile (= chunk of the native layouts): every 128-bit access of the
+        // warp is one contiguous 512-byte row; warps enumerate the layout tiles of the CTA tile, x fastest
+        int w = tid >> 5;
+        q = P.d_wt[0].div(w); const int wx = w - q * P.wt[0]; w = q;
+        q = P.d_wt[1].div(w); const int wy = w - q * P.wt[1]; w = q;
+        q = P.d_wt[2].div(w); const int wz = w - q * P.wt[2]; w = q;
+        x[0] = tc[0] * P.tile[0] + 4 * wx + (tid & 3);
+        x[1] = tc[1] * P.tile[1] + 4 * wy + ((tid >> 2) & 3);
+        x[2] = tc[2] * P.tile[2] + 2 * wz + ((tid >> 4) & 1);
+        x[3] = tc[3] * P.tile[3] + w;
+    } else {
+        q = P.d_tile[0].div(tid); x[0] = tc[0] * P.tile[0] + (tid - q * P.tile[0]); tid = q;
+        q = P.d_tile[1].div(tid); x[1] = tc[1] * P.tile[1] + (tid - q * P.tile[1]); tid = q;
+        q = P.d_tile[2].div(tid); x[2] = tc[2] * P.tile[2] + (tid - q * P.tile[2]); tid = q;
+        x[3] = tc[3] * P.tile[3] + tid;
+    }
+    s_out = P.ord.index(x);  // native position: chunk = s >> 5, lane = s & 31
     return true;
 
 }
@@ -95,21 +111,17 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS)
                     const T* __restrict__ rhs, T kappa, FineParams P) {
     int x[4], s;
     if (!fine_decode(P, x, s)) return;
-    const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
 
-    // neighbour sites (halo-free, modulo L) and wrap phases
+    // neighbour sites (halo-free, modulo L; native positions) and wrap phases
     int sf[4], sb[4];
     T pf[4], pb[4];
-    {
-        const int stride[4] = {1, st1, st2, st3};
 #pragma unroll
-        for (int mu = 0; mu < 4; mu++) {
-            const bool wf = (x[mu] == P.L[mu] - 1), wb = (x[mu] == 0);
-            sf[mu] = wf ? s - (P.L[mu] - 1) * stride[mu] : s + stride[mu];
-            sb[mu] = wb ? s + (P.L[mu] - 1) * stride[mu] : s - stride[mu];
-            pf[mu] = wf ? (T)P.bc[mu] : (T)1;
-            pb[mu] = wb ? (T)P.bc[mu] : (T)1;
-        }
+    for (int mu = 0; mu < 4; mu++) {
+        const bool wf = (x[mu] == P.L[mu] - 1), wb = (x[mu] == 0);
+        sf[mu] = P.ord.fwd(s, mu, x[mu]);
+        sb[mu] = P.ord.bwd(s, mu, x[mu]);
+        pf[mu] = wf ? (T)P.bc[mu] : (T)1;
+        pb[mu] = wb ? (T)P.bc[mu] : (T)1;
     }
 
     T acc[24];
@@ -227,6 +239,7 @@ static int fine_setup(FineParams& P, long long& ntiles_out, const int dims[4], c
     P.parity = (flags & LQCD_DOMAIN_EVEN) ? 1 : (flags & LQCD_DOMAIN_ODD) ? 2 : 0;
     P.keep = 0;
     P.cut_lat = 0;
+    P.ord.set(dims);
     bool user_ok = g_knobs.fine_tile[0] > 0;
     for (int mu = 0; mu < 4 && user_ok; mu++) user_ok = dims[mu] % g_knobs.fine_tile[mu] == 0;
     if (user_ok)
@@ -242,6 +255,11 @@ static int fine_setup(FineParams& P, long long& ntiles_out, const int dims[4], c
         P.tilevol *= P.tile[mu];
         ntiles *= P.ntile[mu];
     }
+    P.warp_tiles = P.ord.tiled && P.tile[0] % 4 == 0 && P.tile[1] % 4 == 0 && P.tile[2] % 2 == 0;
+    P.wt[0] = P.warp_tiles ? P.tile[0] / 4 : 1;
+    P.wt[1] = P.warp_tiles ? P.tile[1] / 4 : 1;
+    P.wt[2] = P.warp_tiles ? P.tile[2] / 2 : 1;
+    for (int mu = 0; mu < 3; mu++) P.d_wt[mu].set(P.wt[mu]);
     // Traversal: canonical tile order keeps the +-t neighbours in L2 only while one time-slice of operands
     // (V3 * bytes/site) is well below the L2 capacity; beyond that, walk the lattice in z-slabs whose
     // per-time-slice footprint is <= ~32 MB (z faces of a slab are re-read: +2-3% traffic).
@@ -528,19 +546,15 @@ __global__ void __launch_bounds__(128, sizeof(T) == 4 ? 3 : 2)
         for (int mu = 0; mu < 4; mu++) par += P.d_dom[mu].div(x[mu]);
         if ((par & 1) != P.parity - 1) return;
     }
-    const int st1 = P.L[0], st2 = P.L[0] * P.L[1], st3 = st2 * P.L[2];
     int sf[4], sb[4];
     T pf[4], pb[4];
-    {
-        const int stride[4] = {1, st1, st2, st3};
 #pragma unroll
-        for (int mu = 0; mu < 4; mu++) {
-            const bool wf = (x[mu] == P.L[mu] - 1), wb = (x[mu] == 0);
-            sf[mu] = wf ? s - (P.L[mu] - 1) * stride[mu] : s + stride[mu];
-            sb[mu] = wb ? s + (P.L[mu] - 1) * stride[mu] : s - stride[mu];
-            pf[mu] = wf ? (T)P.bc[mu] : (T)1;
-            pb[mu] = wb ? (T)P.bc[mu] : (T)1;
-        }
+    for (int mu = 0; mu < 4; mu++) {
+        const bool wf = (x[mu] == P.L[mu] - 1), wb = (x[mu] == 0);
+        sf[mu] = P.ord.fwd(s, mu, x[mu]);
+        sb[mu] = P.ord.bwd(s, mu, x[mu]);
+        pf[mu] = wf ? (T)P.bc[mu] : (T)1;
+        pb[mu] = wb ? (T)P.bc[mu] : (T)1;
     }
     T acc[NRHS][24];
 #pragma unroll

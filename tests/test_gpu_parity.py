@@ -405,3 +405,34 @@ def test_host_entry_points(lq, prec):
     assert np.array_equal(yc.numpy(), d.R(prob.psi[0]))
     lq.prolong_host(out, xc, d.v, cfg.dims, cfg.block, cfg.nvec, ws)
     assert np.array_equal(out.numpy(), d.P(prob.xc))
+
+
+# ------------------------------------------------------------------------------------------------------
+# the native site order (tiled 4 x 4 x 2 chunks) is invisible through pack / unpack: the same
+# canonical fields packed in canonical order (knob site_order = -1) give the same bits
+# ------------------------------------------------------------------------------------------------------
+def test_results_do_not_depend_on_the_site_order(lq):
+    import torch
+    prob = config_problem("c2", 16)
+    cfg = prob.cfg
+    assert cfg.dims[0] % 4 == 0 and cfg.dims[1] % 4 == 0 and cfg.dims[2] % 2 == 0, "config 2 takes the tiled order"
+    outs = {}
+    try:
+        for order in (0, -1):
+            lq.set_knob("site_order", order)
+            d = Dev(lq, prob, "f32")                       # packs U, clover, null vectors in this order
+            x = lq.pack_spinor(to_dev(prob.psi[0], "f32"), cfg.dims)
+            r = lq.pack_spinor(to_dev(prob.psi[1], "f32"), cfg.dims)
+            z = lq.empty_spinor(cfg.dims)
+            lq.mr_domain_solve(z, r, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, parity=2, niter=3)
+            xs, rs = lq.empty_spinor(cfg.dims), lq.empty_spinor(cfg.dims)
+            lq.sap(xs, rs, x, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=3)
+            outs[order] = dict(
+                D=d.D(prob.psi[0]), Ddag=d.D(prob.psi[0], dagger=True), Dsap=d.Dsap(prob.psi[0], cfg.block, parity=1),
+                R=d.R(prob.psi[0]), P=d.P(prob.xc), mr=lq.unpack_spinor(z, cfg.dims).cpu().numpy(),
+                sap=lq.unpack_spinor(xs, cfg.dims).cpu().numpy(), packed=x.cpu().numpy())
+    finally:
+        lq.set_knob("site_order", 0)
+    assert not np.array_equal(outs[0]["packed"], outs[-1]["packed"]), "the two orders are different native layouts"
+    for k in ("D", "Ddag", "Dsap", "R", "P", "mr", "sap"):
+        assert np.array_equal(outs[0][k], outs[-1][k]), k
