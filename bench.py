@@ -526,8 +526,7 @@ def time_e2e(W: Workload, steps: int, warmup: int, ranks: Ranks):
     pool = ThreadPoolExecutor(max_workers=3)
 
     def one():
-        # the chain with the longest dependent compute first: its download then overlaps the uploads of the others
-        futs = [pool.submit(f) for f in (chain_transfer, chain_d, chain_ddag)]
+        futs = [pool.submit(f) for f in (chain_d, chain_ddag, chain_transfer)]
         for f in futs:
             f.result()
 
