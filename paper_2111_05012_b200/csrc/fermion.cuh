@@ -7,6 +7,22 @@
 
 namespace lqcd {
 
+// ---- packed fp32 arithmetic (sm_100a: fma.rn.f32x2 = SASS FFMA2) ---------------------------------------------
+// One FFMA2 does two IEEE fp32 FMAs (same rounding as two scalar fma()) for ONE issue slot; the FMA pipe's rate in
+// flops is unchanged (measured: 73 TFLOP/s either way), so this halves the ISSUE cost of the complex arithmetic below,
+// which is what the fp32 fine kernels are short of under a power-capped clock.  ptxas folds a scalar
+// broadcast (a, a), a negated broadcast and a swapped pair (hi, lo) into operand modifiers of FFMA2 (R.F32, -R.F32,
+// R.F32x2.LO_HI), so none of the pair constructors below costs an instruction as long as the two halves of a pair
+// are produced and consumed consistently.  fp64 keeps the scalar code, and so does a kernel that asks for it with
+// PACK = false: the shared-memory-resident domain solver, bound by LDS traffic at 4 warps per scheduler, was 1.5-2 %
+// SLOWER packed (half the independent FMA chains per thread to cover the pipe latency with).
+__device__ __forceinline__ float2 pk2(float lo, float hi) { return make_float2(lo, hi); }
+__device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 sw2(float2 v) { return make_float2(v.y, v.x); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+template <typename T> struct is_f32 { static constexpr bool value = false; };
+template <> struct is_f32<float> { static constexpr bool value = true; };
+
 // ---- loads --------------------------------------------------------------------------------------------
 // G64: 64-byte L2 fetch granularity (even/odd-domain mode, see common.cuh)
 template <typename T, bool G64 = false>
@@ -111,8 +127,39 @@ template <int MU, int SGN, typename T> __device__ __forceinline__ void project(T
 }
 
 // acc += ph * (1 + SGN g_mu)-reconstruction of g (g = link times projected half spinor)
-template <int MU, int SGN, typename T> __device__ __forceinline__ void reconstruct(T acc[24], const T g[12], T ph) {
+template <int MU, int SGN, typename T, bool PACK = true>
+__device__ __forceinline__ void reconstruct(T acc[24], const T g[12], T ph) {
     const T sp = (T)SGN * ph;
+    if constexpr (PACK && is_f32<T>::value) {
+        // pairs over the two spin components of a chirality half: (acc[2c+ri], acc[6+2c+ri]) and (acc[12+2c+ri],
+        // acc[18+2c+ri]); g comes from su3_mult in the same pairing, so every line is one FFMA2; lane by lane the
+        // same fma as the scalar code below
+        const float2 PH = bc2(ph), SP = bc2(sp), SN = bc2(-sp), SPN = pk2(sp, -sp), SNP = pk2(-sp, sp);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const float2 GR = pk2(g[2 * c], g[6 + 2 * c]), GI = pk2(g[2 * c + 1], g[6 + 2 * c + 1]);
+            float2 A01r = pk2(acc[2 * c], acc[6 + 2 * c]), A01i = pk2(acc[2 * c + 1], acc[6 + 2 * c + 1]);
+            float2 A23r = pk2(acc[12 + 2 * c], acc[18 + 2 * c]), A23i = pk2(acc[12 + 2 * c + 1], acc[18 + 2 * c + 1]);
+            A01r = fma2(PH, GR, A01r);
+            A01i = fma2(PH, GI, A01i);
+            if (MU == 0) {  // r2 = sg i g1 ; r3 = sg i g0
+                A23r = fma2(SN, sw2(GI), A23r);
+                A23i = fma2(SP, sw2(GR), A23i);
+            } else if (MU == 1) {  // r2 = sg g1 ; r3 = -sg g0
+                A23r = fma2(SPN, sw2(GR), A23r);
+                A23i = fma2(SPN, sw2(GI), A23i);
+            } else if (MU == 2) {  // r2 = sg i g0 ; r3 = -sg i g1
+                A23r = fma2(SNP, GI, A23r);
+                A23i = fma2(SPN, GR, A23i);
+            } else {  // r2 = sg g0 ; r3 = sg g1
+                A23r = fma2(SP, GR, A23r);
+                A23i = fma2(SP, GI, A23i);
+            }
+            acc[2 * c] = A01r.x, acc[6 + 2 * c] = A01r.y, acc[2 * c + 1] = A01i.x, acc[6 + 2 * c + 1] = A01i.y;
+            acc[12 + 2 * c] = A23r.x, acc[18 + 2 * c] = A23r.y, acc[12 + 2 * c + 1] = A23i.x, acc[18 + 2 * c + 1] = A23i.y;
+        }
+        return;
+    }
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         const T g0r = g[2 * c], g0i = g[2 * c + 1], g1r = g[6 + 2 * c], g1i = g[6 + 2 * c + 1];
@@ -145,7 +192,30 @@ template <int MU, int SGN, typename T> __device__ __forceinline__ void reconstru
 }
 
 // g = U h (FWD) or U^dag h (!FWD) for the two colour vectors of the half spinor
-template <bool FWD, typename T> __device__ __forceinline__ void su3_mult(T g[12], const T u[18], const T h[12]) {
+template <bool FWD, typename T, bool PACK = true>
+__device__ __forceinline__ void su3_mult(T g[12], const T u[18], const T h[12]) {
+    if constexpr (PACK && is_f32<T>::value) {
+        // the two colour vectors of the half spinor ride in the two lanes: a link element is a broadcast operand, no
+        // swap and no sign fix-up; lane by lane the same fma chain as the scalar code below
+        float2 HR[3], HI[3];
+#pragma unroll
+        for (int b = 0; b < 3; b++) HR[b] = pk2(h[2 * b], h[6 + 2 * b]), HI[b] = pk2(h[2 * b + 1], h[6 + 2 * b + 1]);
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            float2 GR = pk2(0.f, 0.f), GI = pk2(0.f, 0.f);
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                const float ur = FWD ? u[2 * (3 * a + b)] : u[2 * (3 * b + a)];
+                const float ui = FWD ? u[2 * (3 * a + b) + 1] : -u[2 * (3 * b + a) + 1];
+                GR = fma2(bc2(ur), HR[b], GR);
+                GR = fma2(bc2(-ui), HI[b], GR);
+                GI = fma2(bc2(ur), HI[b], GI);
+                GI = fma2(bc2(ui), HR[b], GI);
+            }
+            g[2 * a] = GR.x, g[6 + 2 * a] = GR.y, g[2 * a + 1] = GI.x, g[6 + 2 * a + 1] = GI.y;
+        }
+        return;
+    }
 #pragma unroll
     for (int sp = 0; sp < 2; sp++)
 #pragma unroll
@@ -174,7 +244,32 @@ template <bool FWD, typename T> __device__ __forceinline__ void su3_mult(T g[12]
 }
 
 // out6 += Hermitian 6x6 block (36 reals: 6 diagonal, 15 complex strictly-lower row-major) times in6
-template <typename T> __device__ __forceinline__ void herm6_madd(T out[12], const T cl[36], const T in[12]) {
+template <typename T, bool PACK = true>
+__device__ __forceinline__ void herm6_madd(T out[12], const T cl[36], const T in[12]) {
+    if constexpr (PACK && is_f32<T>::value) {
+        // (re, im) pairs: S collects a_r (x_r, x_i), Q collects +-a_i (x_i, x_r) (the swapped pair is an operand
+        // modifier); out = (S.re - Q.re, S.im + Q.im).  13 instructions per row instead of 22; the two partial sums are
+        // added at the end, so the rounding order differs from the scalar code (both are within the parity bars).
+        float2 X[6];
+#pragma unroll
+        for (int l = 0; l < 6; l++) X[l] = pk2(in[2 * l], in[2 * l + 1]);
+#pragma unroll
+        for (int k = 0; k < 6; k++) {
+            float2 S = fma2(bc2(cl[k]), X[k], pk2(out[2 * k], out[2 * k + 1]));
+            float2 Q = pk2(0.f, 0.f);
+#pragma unroll
+            for (int l = 0; l < 6; l++) {
+                if (l == k) continue;
+                const int t = l < k ? tri(k, l) : tri(l, k);
+                const float ar = cl[6 + 2 * t], ai = cl[6 + 2 * t + 1];
+                S = fma2(bc2(ar), X[l], S);
+                Q = fma2(bc2(l < k ? ai : -ai), sw2(X[l]), Q);
+            }
+            out[2 * k] = S.x - Q.x;
+            out[2 * k + 1] = S.y + Q.y;
+        }
+        return;
+    }
 #pragma unroll
     for (int k = 0; k < 6; k++) {
         T sr = fma(cl[k], in[2 * k], out[2 * k]);

@@ -151,8 +151,8 @@ __device__ __forceinline__ void hop_smem(T acc[24], const V16<T>* __restrict__ r
         u[17] = (T)v.y;
     }
     project<MU, SGN, T>(h, p);
-    su3_mult<FWD, T>(g, u, h);
-    reconstruct<MU, SGN, T>(acc, g, ph);
+    su3_mult<FWD, T, false>(g, u, h);  // scalar arithmetic here: see fermion.cuh
+    reconstruct<MU, SGN, T, false>(acc, g, ph);
 }
 
 // x (+)= M_SAP^(g) r: one domain per CTA, two threads per site (see above); ACC: accumulate into x.
@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
 #pragma unroll
                 for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
             }
-            herm6_madd<T>(p, cl, rho);
+            herm6_madd<T, false>(p, cl, rho);
         }
         // alpha = <p|rho>_X / <p|p>_X  (blocked dotc)
         T d[3] = {0, 0, 0};
