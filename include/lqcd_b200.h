@@ -180,6 +180,26 @@ int lqcd_coarse_mult_half_f32(float* out, const float* in, const float* Ah, cons
 int lqcd_coarse_mult_half_f64(double* out, const double* in, const double* Ah, const int cdims[4], int nvec,
                               unsigned flags, void* ws_dev, void* stream);
 
+/* lqcd_coarse_mult_half_f32 for callers that must not allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same two kernels, the same arithmetic and summation order --
+ * the result is bit-identical with lqcd_coarse_mult_half_f32 -- but the four scratch vectors live in a file-scope
+ * `static __device__` array inside the library instead of a caller-owned workspace.  The call itself calls no
+ * cudaMalloc, cudaFree or any allocating routine; out, in and Ah are the caller's, as above.
+ *   Limit: lqcd_coarse_half_workspace_bytes(cdims, nvec, 4) = Vc * 4 * 4 * nvec * 4 bytes must not exceed
+ *     LQCD_NOALLOC_SCRATCH_BYTES (16 MiB: up to config 4's coarse lattice, 8^3 x 16 sites at nvec = 32, or 32 768
+ *     sites at nvec = 8); a larger problem is refused with LQCD_EUNSUPPORTED and a message naming both sizes --
+ *     nothing is launched.  Every GPU that loads the library holds these 16 MiB until the process exits.
+ *   Sharing: every call on a device uses the SAME array.  Calls are safe back to back on one stream (stream order);
+ *     two calls that can overlap on the GPU (different streams, or graphs replayed concurrently) RACE on it and give
+ *     wrong results -- serialise them, or use the workspace form.  The array keeps the last call's contents; the
+ *     kernels overwrite every element they later read, so nothing needs clearing between calls of any sizes.
+ *   First call on a device: the array's device address is looked up once (cudaGetSymbolAddress, no allocation) and
+ *     cached per device; make that first call outside a graph capture.  LQCD_ECUDA if the lookup fails.
+ * Other errors, flags and aliasing rules as for lqcd_coarse_mult_half_f32. */
+#define LQCD_NOALLOC_SCRATCH_BYTES (16u << 20)
+int lqcd_coarse_mult_half_noalloc_f32(float* out, const float* in, const float* Ah, const int cdims[4], int nvec,
+                                      unsigned flags, void* stream);
+
 /* ---- A4: restriction, Eq. 5:  out_c[X][chi][i] = <v_i restricted to (X,chi) | in_f> -- */
 int lqcd_restrict_f32(float* out_c, const float* in_f, const float* nullvecs, const int dims[4],
                       const int block[4], int nvec, void* stream);

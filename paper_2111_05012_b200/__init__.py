@@ -475,6 +475,24 @@ def coarse_half_workspace(cdims, nvec, dtype=torch.float32, device="cuda") -> to
     return torch.empty(max(nb, 16), dtype=torch.uint8, device=device)
 
 
+NOALLOC_SCRATCH_BYTES = 16 << 20  # LQCD_NOALLOC_SCRATCH_BYTES of include/lqcd_b200.h
+
+
+def coarse_mult_half_noalloc(out, inp, Ah, cdims, nvec, dagger=False, stream=None):
+    """lqcd_coarse_mult_half_noalloc_f32: coarse_mult_half (fp32) with its scratch in a static device array of the
+    library (16 MiB) instead of a workspace -- the call allocates nothing.  Problems whose four scratch vectors exceed
+    that are refused (LqcdError, EUNSUPPORTED); calls that overlap on the GPU race on the shared array."""
+    sfx = _same_dtype(out, inp, Ah)
+    if sfx != "f32":
+        raise TypeError("coarse_mult_half_noalloc: fp32 only (the fp64 form takes a workspace: coarse_mult_half)")
+    _need_coarse(cdims, nvec, (("out", out), ("in", inp)))
+    _need(Ah, native_coarse_half_reals(cdims, nvec), "Ah")
+    _check(lib().lqcd_coarse_mult_half_noalloc_f32(_dev_ptr(out), _dev_ptr(inp), _dev_ptr(Ah), _i4(cdims), int(nvec),
+                                                   DAGGER if dagger else 0, _stream(stream, out, inp, Ah)),
+           "lqcd_coarse_mult_half_noalloc")
+    return out
+
+
 def coarse_mult_half(out, inp, Ah, cdims, nvec, dagger=False, ws=None, stream=None):
     """A3 on half storage: out = D_c in from A_0 and the forward blocks, the backward blocks being
     Gamma5c A_{+mu}(X - mu)^dag Gamma5c (Eqs. 2, 7)."""

@@ -32,6 +32,7 @@ SIGNATURES = {
     "lqcd_native_nullvecs_reals": (C.c_size_t, [_i4, _i4, _ci]),
     "lqcd_native_coarse_vec_reals": (C.c_size_t, [_i4, _ci]),
     "lqcd_native_coarse_mat_reals": (C.c_size_t, [_i4, _ci]),
+    "lqcd_coarse_mult_half_noalloc_f32": (_ci, [_vp, _vp, _vp, _i4, _ci, _cu, _vp]),
     "lqcd_native_coarse_half_reals": (C.c_size_t, [_i4, _ci]),
     "lqcd_coarse_half_workspace_bytes": (C.c_size_t, [_i4, _ci, _ci]),
     "lqcd_host_workspace_bytes": (C.c_size_t, [_i4, _i4, _ci]),

@@ -16,6 +16,7 @@
 // fixed order: results are bit-reproducible.  Two launches; scratch = 4 coarse vectors.
 // Coarse extent 2 (X + mu == X - mu) needs no special case: the block of Y still reaches Y + mu exactly once each way.
 // LQCD_DAGGER (G5c D_c G5c): the two G5c of the transposed term cancel, the forward terms take them as in coarse.cu.
+#include <mutex>
 #include "common.cuh"
 #include "knobs.h"
 
@@ -303,6 +304,40 @@ static int pack_half_call(T* Ah, const T* A, const int cdims[4], int nvec, void*
     return check_launch(what);
 }
 
+// ---- the variant that allocates nothing ----------------------------------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+// it): the four scratch vectors bw[0..3] live in a file-scope device array instead of a caller-supplied workspace.
+// Every GPU that loads the library holds these LQCD_NOALLOC_SCRATCH_BYTES until the process exits.
+//
+// In HOST code the name g_half_scratch is the host-side stand-in of the symbol, NOT a device address (a kernel handed
+// &g_half_scratch[0] from the host would fault or, where the GPU can reach host memory, quietly use the wrong memory):
+// the device address is asked for once per device with cudaGetSymbolAddress, with that device current, and cached.
+static __device__ __align__(256) unsigned char g_half_scratch[LQCD_NOALLOC_SCRATCH_BYTES];
+static void* g_half_scratch_addr[64] = {};  // per device ordinal; written once, under g_half_scratch_mutex
+static std::mutex g_half_scratch_mutex;
+
+static int half_scratch_ptr(void** out, const char* what) {
+    const int d = current_device();
+    if (d < 0 || d >= 64) {
+        set_error("%s: no current CUDA device (or ordinal %d >= 64)", what, d);
+        return LQCD_ECUDA;
+    }
+    std::lock_guard<std::mutex> lock(g_half_scratch_mutex);
+    if (!g_half_scratch_addr[d]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_half_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            set_error("%s: cudaGetSymbolAddress of the static scratch failed on device %d: %s", what, d,
+                      cudaGetErrorString(e));
+            return LQCD_ECUDA;
+        }
+        g_half_scratch_addr[d] = p;
+    }
+    *out = g_half_scratch_addr[d];
+    return LQCD_OK;
+}
+
 }  // namespace lqcd
 
 using namespace lqcd;
@@ -329,5 +364,28 @@ int lqcd_coarse_mult_half_f32(float* out, const float* in, const float* Ah, cons
 int lqcd_coarse_mult_half_f64(double* out, const double* in, const double* Ah, const int cdims[4], int nvec,
                               unsigned flags, void* ws_dev, void* stream) {
     return coarse_half_call<double>(out, in, Ah, cdims, nvec, flags, ws_dev, stream, "lqcd_coarse_mult_half_f64");
+}
+int lqcd_coarse_mult_half_noalloc_f32(float* out, const float* in, const float* Ah, const int cdims[4], int nvec,
+                                      unsigned flags, void* stream) {
+    const char* what = "lqcd_coarse_mult_half_noalloc_f32";
+    clear_error();
+    const size_t need = lqcd_coarse_half_workspace_bytes(cdims, nvec, (int)sizeof(float));
+    if (need == 0) {
+        set_error("%s: non-positive dim or nvec < 1", what);
+        return LQCD_EINVAL;
+    }
+    if (need > (size_t)LQCD_NOALLOC_SCRATCH_BYTES) {
+        set_error("%s: the problem needs %zu bytes of scratch (4 coarse vectors of %lld sites x %d complex), the static "
+                  "array holds LQCD_NOALLOC_SCRATCH_BYTES = %zu: use lqcd_coarse_mult_half_f32 with a caller-owned "
+                  "workspace", what, need, volume(cdims), 2 * nvec, (size_t)LQCD_NOALLOC_SCRATCH_BYTES);
+        return LQCD_EUNSUPPORTED;
+    }
+    void* ws = nullptr;
+    const int rc = half_scratch_ptr(&ws, what);
+    if (rc) return rc;
+    // Nothing has to start at zero: k_coarse_half writes every element of bw[0..3] of THIS problem (each site Y stores
+    // the whole vector bw[mu][Y + mu], and every site is some Y + mu) before k_coarse_half_sum reads it, so whatever
+    // an earlier call left in the array, of this or another size, is overwritten or never read.
+    return coarse_half_call<float>(out, in, Ah, cdims, nvec, flags, ws, stream, what);
 }
 }
