@@ -90,6 +90,33 @@ template <int NRED, typename T> __device__ __forceinline__ void cta_sum(T v[NRED
         v[q] = s;
     }
 }
+// The same for a CTA of NW warps known at compile time, fp32: the second stage reads the NW * NRED partial sums as
+// broadcast 128-bit loads (12 LDS.128 instead of 48 LDS.32 at NW = 16, NRED = 3) and adds them in the SAME order as
+// cta_sum (warps in index order), so the two give the same bits.  red must be 16-byte aligned.
+template <int NRED, int NW> __device__ __forceinline__ void cta_sum_v(float v[NRED], float* red) {
+    static_assert((NRED * NW) % 4 == 0, "partials must fill whole float4s");
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int q = 0; q < NRED; q++) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+        if (lane == 0) red[w * NRED + q] = v[q];
+    }
+    __syncthreads();
+    float t[NRED * NW];
+#pragma unroll
+    for (int j = 0; j < NRED * NW / 4; j++) {
+        const float4 f = reinterpret_cast<const float4*>(red)[j];
+        t[4 * j] = f.x, t[4 * j + 1] = f.y, t[4 * j + 2] = f.z, t[4 * j + 3] = f.w;
+    }
+#pragma unroll
+    for (int q = 0; q < NRED; q++) {
+        float s = t[q];
+#pragma unroll
+        for (int i = 1; i < NW; i++) s += t[i * NRED + q];
+        v[q] = s;
+    }
+}
 
 // ---- the shared-memory-resident inner-domain solver ------------------------------------------------------
 // Shared-memory image of one domain (bv sites, local index l, x fastest):
@@ -117,12 +144,16 @@ __device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
 __device__ __forceinline__ void cp_async_wait_all() {
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
 }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait_group() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
 
 template <typename T> struct MrSmem {
     static constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, NR = 72 / NV, NFULL = 18 / NV, TAIL = 18 - NFULL * NV;
     static __host__ __device__ size_t bytes(int bv, int bvp) {
         return (size_t)bv * (NJ + 4 * NFULL + NR) * 16 + (size_t)bv * 4 * TAIL * sizeof(T) +
-               (size_t)bvp * 2 * (NJ / 2) * 16 + 16 * 3 * sizeof(T);
+               (size_t)bvp * 2 * (NJ / 2) * 16 + 16 * 3 * sizeof(T) + 16;  // ... + the tensor-memory base address
     }
 };
 
@@ -155,10 +186,122 @@ __device__ __forceinline__ void hop_smem(T acc[24], const V16<T>* __restrict__ r
     reconstruct<MU, SGN, T, false>(acc, g, ph);
 }
 
+// ---- tensor memory as a second operand store (TM variant of k_mr_domain, fp32 4^4 domains) ---------------------
+// The solver is bound by the shared-memory pipe (ncu: LDS wavefronts 68 % of the pipe's peak, short-scoreboard and
+// MIO-throttle stalls on top), and 55 % of its LDS traffic are operands that are PRIVATE to a thread: the four links of
+// its four hops and its clover block never change during the n_mr iterations.  Blackwell's tensor memory (256 KB per SM,
+// 128 lanes x 512 columns of 32 bits, read by tcgen05.ld on a datapath of its own: measured 870 B/clk/SM against the
+// shared-memory pipe's 128) is addressed exactly that way -- lane = thread of a warp quarter, column = register index --
+// so the kernel parks them there: the first iteration reads them from shared memory (where cp.async staged them) and
+// stores them with tcgen05.st, the others read them back with tcgen05.ld.  No tensor-core instruction is issued; the
+// bits are the staged fp32 values, so the results are those of the shared-memory path.
+// Columns of a thread (warp w: lanes 32 (w % 4) ..., column block 128 (w / 4)): hop k's link at 20 k (18 reals),
+// clover block at 80 (36 reals).
+__device__ __forceinline__ void tm_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tm_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// tcgen05.ld is asynchronous: its destination registers are valid after tcgen05.wait::ld.  The registers are in/out
+// operands of the wait, so no use of them can be scheduled above it.
+__device__ __forceinline__ void tm_wait_ld18(float* v) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]), "+f"(v[8]),
+                   "+f"(v[9]), "+f"(v[10]), "+f"(v[11]), "+f"(v[12]), "+f"(v[13]), "+f"(v[14]), "+f"(v[15]), "+f"(v[16]),
+                   "+f"(v[17])::"memory");
+}
+__device__ __forceinline__ void tm_wait_ld36(float* v) {
+    tm_wait_ld18(v);  // (the second half is ordered behind the first wait by the same mechanism)
+    asm volatile("" : "+f"(v[18]), "+f"(v[19]), "+f"(v[20]), "+f"(v[21]), "+f"(v[22]), "+f"(v[23]), "+f"(v[24]), "+f"(v[25]),
+                 "+f"(v[26]), "+f"(v[27]), "+f"(v[28]), "+f"(v[29]), "+f"(v[30]), "+f"(v[31]), "+f"(v[32]), "+f"(v[33]),
+                 "+f"(v[34]), "+f"(v[35])::"memory");
+}
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_st16(unsigned ta, const float* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(ta),
+        "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]), "f"(v[8]), "f"(v[9]),
+        "f"(v[10]), "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15])
+        : "memory");
+}
+__device__ __forceinline__ void tm_st4(unsigned ta, const float* v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(ta), "f"(v[0]), "f"(v[1]), "f"(v[2]),
+                 "f"(v[3])
+                 : "memory");
+}
+__device__ __forceinline__ void tm_st2(unsigned ta, const float* v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(ta), "f"(v[0]), "f"(v[1]) : "memory");
+}
+__device__ __forceinline__ void tm_ld16(float* v, unsigned ta) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]), "=f"(v[8]),
+          "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
+        : "r"(ta));
+}
+__device__ __forceinline__ void tm_ld4(float* v, unsigned ta) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3])
+                 : "r"(ta));
+}
+__device__ __forceinline__ void tm_ld2(float* v, unsigned ta) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=f"(v[0]), "=f"(v[1]) : "r"(ta));
+}
+constexpr int TM_COLS = 512, TM_LINK = 20, TM_CLOVER = 80;
+
+// The first iteration's hop: operands from shared memory as in hop_smem, the link parked in tensor memory on the way.
+template <int MU, bool FWD, int SGN>
+__device__ __forceinline__ void hop_smem_park(float acc[24], const V16<float>* __restrict__ rho_s,
+                                              const V16<float>* __restrict__ U_s, const float* __restrict__ U_t, int bv,
+                                              int l_link, int l_nb, float ph, unsigned ta) {
+    float p[24], h[12], u[18], g[12];
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+        const V16<float> v = rho_s[j * bv + l_nb];
+#pragma unroll
+        for (int q = 0; q < 4; q++) p[j * 4 + q] = v.r[q];
+    }
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        const V16<float> v = U_s[(MU * 4 + j) * bv + l_link];
+#pragma unroll
+        for (int q = 0; q < 4; q++) u[j * 4 + q] = v.r[q];
+    }
+    const float2 v = *reinterpret_cast<const float2*>(U_t + (MU * bv + l_link) * 2);
+    u[16] = v.x;
+    u[17] = v.y;
+    tm_st16(ta, u);
+    tm_st2(ta + 16, u + 16);
+    project<MU, SGN, float>(h, p);
+    su3_mult<FWD, float, false>(g, u, h);
+    reconstruct<MU, SGN, float, false>(acc, g, ph);
+}
+// The other iterations' hop: the neighbour spinor from shared memory, the link from tensor memory.  un holds the link
+// requested one hop ahead; NEXT: request the following hop's link (at ta_next) before the arithmetic of this one.
+template <int MU, bool FWD, int SGN, bool NEXT>
+__device__ __forceinline__ void hop_tm(float acc[24], const V16<float>* __restrict__ rho_s, int bv, int l_nb, float ph,
+                                       float un[18], unsigned ta_next) {
+    float p[24], h[12], u[18], g[12];
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+        const V16<float> v = rho_s[j * bv + l_nb];
+#pragma unroll
+        for (int q = 0; q < 4; q++) p[j * 4 + q] = v.r[q];
+    }
+    tm_wait_ld18(un);
+#pragma unroll
+    for (int q = 0; q < 18; q++) u[q] = un[q];
+    if (NEXT) {
+        tm_ld16(un, ta_next);
+        tm_ld2(un + 16, ta_next + 16);
+    }
+    project<MU, SGN, float>(h, p);
+    su3_mult<FWD, float, false>(g, u, h);
+    reconstruct<MU, SGN, float, false>(acc, g, ph);
+}
+
 // x (+)= M_SAP^(g) r: one domain per CTA, two threads per site (see above); ACC: accumulate into x.
 // BVC: sites per domain as a compile-time constant (a multiple of 32; every shared-memory row offset then folds into
 // the immediate field of LDS/STS: -12 % instructions), 0 = run-time P.bv.
-template <typename T, bool ACC, int BVC>
+// TM: links and clover blocks parked in tensor memory after the first iteration (fp32, BVC = 256 only; above).
+template <typename T, bool ACC, int BVC, bool TM>
 __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits at most 151 sites (320 threads)
     k_mr_domain(T* __restrict__ x, const T* __restrict__ r, const T* __restrict__ U, const T* __restrict__ clover,
                 T kappa, DomParams P, int niter, int nrhs, long long rstride) {
@@ -209,6 +352,9 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
             for (int j = 0; j < NFULL; j++) cp_async16<T>(&U_s[(mu * NFULL + j) * bv + l], g + (j * CH + lane) * NV);
             if (S::TAIL) cp_async8(U_t + (mu * bv + l) * 2, g + NFULL * NV * CH + lane * 2);
         }
+    }
+    cp_async_commit();  // group "links": needed by the first hop phase
+    if (active) {
         const T* cbase = clover + (chunk * NR * CH + lane) * NV;
 #pragma unroll
         for (int j = 0; j < NR / 2; j++) {
@@ -216,7 +362,37 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
             cp_async16<T>(&C_s[row * bv + l], cbase + (long long)row * CH * NV);
         }
     }
-    cp_async_wait_all();
+    cp_async_commit();  // group "clover": first needed AFTER the hop phase of the first iteration, and only by the
+                        // thread that staged it (thread (l, h) stages and reads rows h * NR/2 ... of site l)
+    T rho[12];  // my half of the residual; the first right-hand side's is requested before any wait
+#pragma unroll
+    for (int j = 0; j < NH; j++) {
+        const V16<T> v = ld16_g64(r + sp_off + (long long)(NH * h + j) * CH * NV);
+#pragma unroll
+        for (int q = 0; q < NV; q++) rho[j * NV + q] = v.r[q];
+    }
+    if (ACC && active) {
+#pragma unroll
+        for (int j = 0; j < NH; j++)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(x + sp_off + (long long)(NH * h + j) * CH * NV));
+    }
+    unsigned& tm_slot = *reinterpret_cast<unsigned*>(red + 16 * 3);  // (dynamic shared memory: a static variable would
+                                                                     // not fit next to the opt-in maximum)
+    unsigned tm_base = 0;  // my lane quarter and column block of the CTA's tensor memory
+    if constexpr (TM) {
+        static_assert(!TM || (BVC == 256 && sizeof(T) == 4), "the tensor-memory variant is the fp32 4^4 one");
+        if (tid < 32) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                             (unsigned)__cvta_generic_to_shared(&tm_slot)),
+                         "n"(TM_COLS)
+                         : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+        tm_fence_before();
+        __syncthreads();
+        tm_fence_after();
+        tm_base = tm_slot + ((unsigned)(32 * ((tid >> 5) & 3)) << 16) + (unsigned)((tid >> 7) * 128);
+    }
 
     // neighbours inside the domain (local index, wrapped) and hop phases: a hop that leaves the domain is cut
     // (phase 0); in a direction spanned by ONE domain the wrap is the lattice's own and carries bc[mu].
@@ -239,15 +415,17 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
 
     // Right-hand sides one after the other on the resident operator: links and clover (86 % of the staged bytes) are
     // read from HBM once for all of them.
+    cp_async_wait_group<1>();  // my links have landed (everybody's after the first barrier below)
     for (int krhs = 0; krhs < nrhs; krhs++) {
     const T* rk = r + krhs * rstride;
     T* xk = x + krhs * rstride;
-    T rho[12];  // my half of the residual
+    if (krhs > 0) {
 #pragma unroll
-    for (int j = 0; j < NH; j++) {
-        const V16<T> v = ld16_g64(rk + sp_off + (long long)(NH * h + j) * CH * NV);
+        for (int j = 0; j < NH; j++) {
+            const V16<T> v = ld16_g64(rk + sp_off + (long long)(NH * h + j) * CH * NV);
 #pragma unroll
-        for (int q = 0; q < NV; q++) rho[j * NV + q] = v.r[q];
+            for (int q = 0; q < NV; q++) rho[j * NV + q] = v.r[q];
+        }
     }
     T z[12];
 #pragma unroll
@@ -270,7 +448,52 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
             T acc[24];
 #pragma unroll
             for (int q = 0; q < 24; q++) acc[q] = 0;
-            if (h == 0) {
+            bool hops_done = false;
+            if constexpr (TM) {
+                const bool first = krhs == 0 && it == 0;  // links still only in shared memory
+                if (first) {
+                    if (h == 0) {
+                        hop_smem_park<0, true, -1>(acc, rho_s, U_s, U_t, bv, l, nf[0], pf[0], tm_base);
+                        hop_smem_park<0, false, +1>(acc, rho_s, U_s, U_t, bv, nb[0], nb[0], pb[0], tm_base + TM_LINK);
+                        hop_smem_park<1, true, -1>(acc, rho_s, U_s, U_t, bv, l, nf[1], pf[1], tm_base + 2 * TM_LINK);
+                        hop_smem_park<1, false, +1>(acc, rho_s, U_s, U_t, bv, nb[1], nb[1], pb[1], tm_base + 3 * TM_LINK);
+                    } else {
+                        hop_smem_park<2, true, -1>(acc, rho_s, U_s, U_t, bv, l, nf[2], pf[2], tm_base);
+                        hop_smem_park<2, false, +1>(acc, rho_s, U_s, U_t, bv, nb[2], nb[2], pb[2], tm_base + TM_LINK);
+                        hop_smem_park<3, true, -1>(acc, rho_s, U_s, U_t, bv, l, nf[3], pf[3], tm_base + 2 * TM_LINK);
+                        hop_smem_park<3, false, +1>(acc, rho_s, U_s, U_t, bv, nb[3], nb[3], pb[3], tm_base + 3 * TM_LINK);
+                    }
+                    tm_wait_st();
+                } else {
+                    float un[18];
+                    tm_ld16(un, tm_base);
+                    tm_ld2(un + 16, tm_base + 16);
+                    if (h == 0) {
+                        hop_tm<0, true, -1, true>(acc, rho_s, bv, nf[0], pf[0], un, tm_base + TM_LINK);
+                        hop_tm<0, false, +1, true>(acc, rho_s, bv, nb[0], pb[0], un, tm_base + 2 * TM_LINK);
+                        hop_tm<1, true, -1, true>(acc, rho_s, bv, nf[1], pf[1], un, tm_base + 3 * TM_LINK);
+                        hop_tm<1, false, +1, false>(acc, rho_s, bv, nb[1], pb[1], un, 0u);
+                    } else {
+                        hop_tm<2, true, -1, true>(acc, rho_s, bv, nf[2], pf[2], un, tm_base + TM_LINK);
+                        hop_tm<2, false, +1, true>(acc, rho_s, bv, nb[2], pb[2], un, tm_base + 2 * TM_LINK);
+                        hop_tm<3, true, -1, true>(acc, rho_s, bv, nf[3], pf[3], un, tm_base + 3 * TM_LINK);
+                        hop_tm<3, false, +1, false>(acc, rho_s, bv, nb[3], pb[3], un, 0u);
+                    }
+                }
+                hops_done = true;
+            }
+            if (hops_done) {
+#pragma unroll
+                for (int j = 0; j < NH; j++) {
+                    V16<T> v;
+#pragma unroll
+                    for (int q = 0; q < NV; q++) {
+                        v.r[q] = h ? acc[j * NV + q] : acc[12 + j * NV + q];
+                        mine[j * NV + q] = h ? acc[12 + j * NV + q] : acc[j * NV + q];
+                    }
+                    xch_s[j * 2 * bvp + tid] = v;
+                }
+            } else if (h == 0) {
                 hop_smem<0, true, -1, T>(acc, rho_s, U_s, U_t, bv, l, nf[0], pf[0]);
                 hop_smem<0, false, +1, T>(acc, rho_s, U_s, U_t, bv, nb[0], nb[0], pb[0]);
                 hop_smem<1, true, -1, T>(acc, rho_s, U_s, U_t, bv, l, nf[1], pf[1]);
@@ -311,12 +534,31 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
             for (int q = 0; q < NV; q++) p[j * NV + q] = fma(-kappa, mine[j * NV + q] + v.r[q], rho[j * NV + q]);
         }
         {
+            cp_async_wait_group<0>();  // my clover rows (a no-op after the first iteration)
             T cl[36];
+            bool have = false;
+            if constexpr (TM) {
+                if (!(krhs == 0 && it == 0)) {  // parked in tensor memory by the first iteration
+                    tm_ld16(cl, tm_base + TM_CLOVER);
+                    tm_ld16(cl + 16, tm_base + TM_CLOVER + 16);
+                    tm_ld4(cl + 32, tm_base + TM_CLOVER + 32);
+                    tm_wait_ld36(cl);
+                    have = true;
+                }
+            }
+            if (!have) {
 #pragma unroll
-            for (int j = 0; j < 36 / NV; j++) {
-                const V16<T> v = C_s[(h * (36 / NV) + j) * bv + l];
+                for (int j = 0; j < 36 / NV; j++) {
+                    const V16<T> v = C_s[(h * (36 / NV) + j) * bv + l];
 #pragma unroll
-                for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
+                    for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
+                }
+                if constexpr (TM) {
+                    tm_st16(tm_base + TM_CLOVER, cl);
+                    tm_st16(tm_base + TM_CLOVER + 16, cl + 16);
+                    tm_st4(tm_base + TM_CLOVER + 32, cl + 32);
+                    tm_wait_st();
+                }
             }
             herm6_madd<T, false>(p, cl, rho);
         }
@@ -333,7 +575,8 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
                 d[2] = fma(p[2 * k + 1], p[2 * k + 1], d[2]);
             }
         }
-        cta_sum<3, T>(d, red);
+        if constexpr (BVC == 256 && sizeof(T) == 4) cta_sum_v<3, 16>(d, red);
+        else cta_sum<3, T>(d, red);
         const T ar = d[2] > 0 ? d[0] / d[2] : (T)0, ai = d[2] > 0 ? d[1] / d[2] : (T)0;
         // z += alpha rho ; rho -= alpha p  (blocked axpy)
 #pragma unroll
@@ -368,6 +611,12 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
         }
     }
     }  // right-hand sides
+    if constexpr (TM) {
+        tm_fence_before();
+        __syncthreads();
+        if (tid < 32)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_slot), "n"(TM_COLS) : "memory");
+    }
 }
 
 // ---- blocked BLAS-1: one CTA per domain, sites strided over the threads ------------------------
@@ -602,18 +851,25 @@ static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa
             grid = (unsigned)(P.Vc / 2);
         }
         const long long rstride = (long long)nchunks(dims) * CH * 24;  // right-hand sides back to back
-#define LAUNCH_MR(ACC, BVC)                                                                                   \
+#define LAUNCH_MR(ACC, BVC, TM)                                                                                 \
     do {                                                                                                      \
         static unsigned long long attr = 0;                                                                   \
-        ensure_dynamic_smem(k_mr_domain<T, ACC, BVC>, max_optin_smem(), attr);                                \
-        k_mr_domain<T, ACC, BVC><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter, K, rstride);   \
+        ensure_dynamic_smem(k_mr_domain<T, ACC, BVC, TM>, max_optin_smem(), attr);                            \
+        k_mr_domain<T, ACC, BVC, TM><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter, K, rstride); \
     } while (0)
         if (sizeof(T) == 4 && P.bv == 256) {  // the paper's typical 4^4 domain
-            if (acc) LAUNCH_MR(true, (sizeof(T) == 4 ? 256 : 0));
-            else LAUNCH_MR(false, (sizeof(T) == 4 ? 256 : 0));
+            constexpr int B = sizeof(T) == 4 ? 256 : 0;
+            constexpr bool F32 = sizeof(T) == 4;
+            if (g_knobs.sap_tmem >= 0) {  // links and clover parked in tensor memory
+                if (acc) LAUNCH_MR(true, B, F32);
+                else LAUNCH_MR(false, B, F32);
+            } else {
+                if (acc) LAUNCH_MR(true, B, false);
+                else LAUNCH_MR(false, B, false);
+            }
         } else {
-            if (acc) LAUNCH_MR(true, 0);
-            else LAUNCH_MR(false, 0);
+            if (acc) LAUNCH_MR(true, 0, false);
+            else LAUNCH_MR(false, 0, false);
         }
 #undef LAUNCH_MR
         count_launch();

@@ -28,12 +28,15 @@ def lq():
     return lq
 
 
-@pytest.fixture(params=[0, -1], ids=["resident", "generic"])
+@pytest.fixture(params=[(0, 0), (0, -1), (-1, 0)], ids=["resident", "resident-smem", "generic"])
 def path(lq, request):
-    """both implementations of the inner-domain solver"""
-    lq.set_knob("sap_fused", request.param)
-    yield request.param
+    """the implementations of the inner-domain solver: shared-memory-resident with the links and clover blocks parked
+    in tensor memory (fp32 4^4 domains; elsewhere the same as the next), shared memory only, generic"""
+    lq.set_knob("sap_fused", request.param[0])
+    lq.set_knob("sap_tmem", request.param[1])
+    yield request.param[0]
     lq.set_knob("sap_fused", 0)
+    lq.set_knob("sap_tmem", 0)
 
 
 def fields(prob, prec):
@@ -290,6 +293,46 @@ def test_sap_mrhs_4x4_domains(lq):
     for k in range(4):
         lq.sap(x1, r1, b[k], d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=6)
         assert torch.equal(x[k], x1) and torch.equal(r[k], r1), k
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 8, 4, 8)])
+def test_mr_tensor_memory_is_bit_identical(lq, dims):
+    """fp32, 4^4 domains: the resident solver parks each thread's links and clover block in tensor memory after the
+    first iteration (knob sap_tmem).  The parked bits are the staged fp32 values and the
+    arithmetic is the same, so every result is bit-identical with the shared-memory-only kernel: all groups, with and
+    without accumulation, 0 ... 7 iterations, several right-hand sides on the resident operator, SAP.  (Against the
+    oracle both run in test_mr_edge_lattices / test_c2_lattice_sap.)  (12, 8, 4, 8): odd Lc[0] (full grid in
+    accumulate mode), a direction spanned by one domain."""
+    import torch
+    cfg = custom_config(dims, (4, 4, 4, 4), 1, gauge="exp", eps=0.5, kappa=0.135, csw=1.0, seed=21)
+    prob = make_problem(cfg, n_rhs=3, coarse="none")
+    d = Dev(lq, prob, "f32", coarse=False)
+    b = torch.stack([lq.pack_spinor(to_dev(p, "f32"), cfg.dims) for p in prob.psi])
+    out = {}
+    for knob in (0, -1):
+        lq.set_knob("sap_tmem", knob)
+        try:
+            res = []
+            for parity in (0, 1, 2):
+                for niter in (0, 1, 2, 7):
+                    z = torch.full_like(b[0], 5.0)
+                    lq.mr_domain_solve(z, b[0], d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, parity=parity,
+                                       niter=niter)
+                    y = b[1].clone()
+                    lq.mr_domain_solve(y, b[0], d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, parity=parity,
+                                       niter=niter, accumulate=True)
+                    res += [z, y]
+            x, r = torch.full_like(b, 3.0), torch.full_like(b, 3.0)
+            lq.sap_mrhs(x, r, b, d.U, d.clover, cfg.kappa, cfg.dims, cfg.bc, cfg.block, n_sap=2, n_mr=5)
+            res += [x, r]
+            torch.cuda.synchronize()
+            out[knob] = res
+        finally:
+            lq.set_knob("sap_tmem", 0)
+    assert len(out[0]) == len(out[-1])
+    for k, (a, c) in enumerate(zip(out[0], out[-1])):
+        assert torch.equal(a, c), k
+    assert float(out[0][-2].abs().max()) > 0
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
