@@ -814,7 +814,10 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             W.lq.set_knob("sap_fused", knob)
             nb = int(W.lq.lib().lqcd_mr_workspace_bytes(W.lq._i4(cfg.dims), W.lq._i4(cfg.block), 4))
             W.mr_ws = torch.empty(nb, dtype=torch.uint8, device=W.dev) if nb else None
-            t = time_single(W, name, reps=max(3, min(10, args.steps)), warmup=1)
+            row_sampler = ClockSampler(0)  # this row's own clock: an ALU-bound kernel runs into the power cap
+            row_sampler.start()
+            t = time_single(W, name, reps=max(3, min(10, args.steps)) * (3 if key == "mr" else 1), warmup=1)
+            row_clocks = row_sampler.stop()
             W.mr_ws = None
             md = ms[key]
             label = {("mr_even", 0): "mr_domain_solve_even", ("mr_even", -1): "mr_domain_solve_even_generic",
@@ -823,15 +826,29 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
                             "units_per_s": md["units"] / t, "frac_of_hbm_peak": md["bytes"] / t / 1e9 / peak,
                             "bytes_per_launch": md["bytes"],
                             "path": "generic" if nb else "shared-memory-resident"}
-            if label == "mr_domain_solve_even" and not nb and clocks.get("sm_mhz"):
-                # the resident solver is bound by SHARED-MEMORY bandwidth, not HBM: per site and
-                # iteration 8 neighbour spinors (96 B) + 8 links (72 B) + the clover term (288 B) + the store and the
-                # exchange of rho (2 x 96 B) = 1824 B of LDS / STS traffic; roof = 128 B/clk/SM x 148 SMs x SM clock
-                smem_b = 1824.0 * (cfg.volume / 2) * 6
-                roof = 128.0 * 148 * clocks["sm_mhz"] * 1e6
-                extra[label]["roofline"] = {"bound": "shared-memory bandwidth", "achieved": smem_b / t / 1e12,
-                                            "peak": roof / 1e12, "unit": "TB/s", "frac": smem_b / t / roof,
-                                            "bytes_per_site_iteration": 1824, "sm_mhz": clocks["sm_mhz"]}
+            if label == "mr_domain_solve_even" and not nb and row_clocks.get("sm_mhz"):
+                # The resident solver is bound on the SM, not by HBM.  With the links and clover blocks
+                # parked in tensor memory (fp32 4^4 domains on the tiled site order: persistent kernel) the binding
+                # roof is the fp32 pipe: 1472 FFMA / FADD per site and iteration (SASS count of the iteration body,
+                # two threads per site) against 128 lanes/clk/SM x 148 SMs x SM clock; the shared-memory pipe carries
+                # 8 neighbour spinors (96 B) + the store and the exchange of rho (96 + 192 B) = 1056 B per site and
+                # iteration (1824 B when links and clover term are read from shared memory too) at 128 B/clk/SM.
+                tm = cfg.block == (4, 4, 4, 4) and all(d % 4 == 0 for d in cfg.dims[:2]) and cfg.dims[2] % 2 == 0
+                sites_it = (cfg.volume / 2) * 6
+                clk = row_clocks["sm_mhz"] * 1e6
+                alu_roof, smem_roof = 128.0 * 148 * clk, 128.0 * 148 * clk
+                smem_b = (1056.0 if tm else 1824.0) * sites_it
+                extra[label]["path"] = "persistent, operands in tensor memory" if tm else "shared-memory-resident"
+                extra[label]["roofline"] = {
+                    "bound": "alu" if tm else "shared-memory bandwidth",
+                    "achieved": (1472.0 * sites_it / t / 1e12) if tm else smem_b / t / 1e12,
+                    "peak": (alu_roof if tm else smem_roof) / 1e12,
+                    "unit": "T fp32 lane-instructions/s" if tm else "TB/s",
+                    "frac": (1472.0 * sites_it / t / alu_roof) if tm else smem_b / t / smem_roof,
+                    "fp32_instructions_per_site_iteration": 1472,
+                    "shared_memory": {"bytes_per_site_iteration": 1056 if tm else 1824,
+                                      "achieved_TBps": smem_b / t / 1e12, "frac": smem_b / t / smem_roof},
+                    "sm_mhz": row_clocks["sm_mhz"], "clock_reasons": row_clocks.get("reasons", [])}
         W.lq.set_knob("sap_fused", 0)
         # one V-cycle x = M b of the preconditioner: restrict, 8 BiCGStab iterations on D_c,
         # prolong, SAP(4, 6) -- everything on one stream, no host synchronisation

@@ -35,28 +35,30 @@ struct DomParams {
     int bv, Vc;
     int parity;    // 0 = all domains, 1 = even, 2 = odd
     int halfgrid;  // 1: the grid enumerates only the domains of the selected group (needs Lc[0] even)
+    FastDiv d_Lc[3], d_half, d_dom[3];  // reciprocals of Lc[0..2], Lc[0] / 2 and dom[0..2] for the index decode
     SiteOrder ord; // native position of a site (layout.cuh)
 };
 
 // Coarse coordinates of the domain of CTA b; false if that domain is not in the selected group.
 __device__ __forceinline__ bool domain_of_cta(const DomParams& P, int b, int Xc[4]) {
+    // (divisions by run-time extents as multiply-high with host-computed reciprocals: the decode with hardware-less
+    // integer division was 1.6 k issue cycles per CTA of 16 warps)
+    int q;
     if (P.halfgrid) {
         const int h = P.Lc[0] >> 1;
-        const int hx = b % h;
-        b /= h;
-        Xc[1] = b % P.Lc[1];
-        b /= P.Lc[1];
-        Xc[2] = b % P.Lc[2];
-        Xc[3] = b / P.Lc[2];
+        q = P.d_half.div(b);
+        const int hx = b - q * h;
+        b = q;
+        q = P.d_Lc[1].div(b); Xc[1] = b - q * P.Lc[1]; b = q;
+        q = P.d_Lc[2].div(b); Xc[2] = b - q * P.Lc[2];
+        Xc[3] = q;
         Xc[0] = 2 * hx + ((Xc[1] + Xc[2] + Xc[3] + P.parity - 1) & 1);
         return true;
     }
-    Xc[0] = b % P.Lc[0];
-    b /= P.Lc[0];
-    Xc[1] = b % P.Lc[1];
-    b /= P.Lc[1];
-    Xc[2] = b % P.Lc[2];
-    Xc[3] = b / P.Lc[2];
+    q = P.d_Lc[0].div(b); Xc[0] = b - q * P.Lc[0]; b = q;
+    q = P.d_Lc[1].div(b); Xc[1] = b - q * P.Lc[1]; b = q;
+    q = P.d_Lc[2].div(b); Xc[2] = b - q * P.Lc[2];
+    Xc[3] = q;
     return P.parity == 0 || ((Xc[0] + Xc[1] + Xc[2] + Xc[3]) & 1) == P.parity - 1;
 }
 
@@ -64,11 +66,14 @@ __device__ __forceinline__ bool domain_of_cta(const DomParams& P, int b, int Xc[
 __device__ __forceinline__ int domain_site(const DomParams& P, const int Xc[4], int l, int lx[4]) {
     int x[4];
 #pragma unroll
-    for (int mu = 0; mu < 4; mu++) {
-        lx[mu] = l % P.dom[mu];
-        l /= P.dom[mu];
+    for (int mu = 0; mu < 3; mu++) {
+        const int q = P.d_dom[mu].div(l);
+        lx[mu] = l - q * P.dom[mu];
+        l = q;
         x[mu] = Xc[mu] * P.dom[mu] + lx[mu];
     }
+    lx[3] = l;
+    x[3] = Xc[3] * P.dom[3] + l;
     return P.ord.index(x);
 }
 
@@ -153,7 +158,7 @@ template <typename T> struct MrSmem {
     static constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, NR = 72 / NV, NFULL = 18 / NV, TAIL = 18 - NFULL * NV;
     static __host__ __device__ size_t bytes(int bv, int bvp) {
         return (size_t)bv * (NJ + 4 * NFULL + NR) * 16 + (size_t)bv * 4 * TAIL * sizeof(T) +
-               (size_t)bvp * 2 * (NJ / 2) * 16 + 16 * 3 * sizeof(T) + 16;  // ... + the tensor-memory base address
+               (size_t)bvp * 2 * (NJ / 2) * 16 + 16 * 3 * sizeof(T);
     }
 };
 
@@ -186,122 +191,10 @@ __device__ __forceinline__ void hop_smem(T acc[24], const V16<T>* __restrict__ r
     reconstruct<MU, SGN, T, false>(acc, g, ph);
 }
 
-// ---- tensor memory as a second operand store (TM variant of k_mr_domain, fp32 4^4 domains) ---------------------
-// The solver is bound by the shared-memory pipe (ncu: LDS wavefronts 68 % of the pipe's peak, short-scoreboard and
-// MIO-throttle stalls on top), and 55 % of its LDS traffic are operands that are PRIVATE to a thread: the four links of
-// its four hops and its clover block never change during the n_mr iterations.  Blackwell's tensor memory (256 KB per SM,
-// 128 lanes x 512 columns of 32 bits, read by tcgen05.ld on a datapath of its own: measured 870 B/clk/SM against the
-// shared-memory pipe's 128) is addressed exactly that way -- lane = thread of a warp quarter, column = register index --
-// so the kernel parks them there: the first iteration reads them from shared memory (where cp.async staged them) and
-// stores them with tcgen05.st, the others read them back with tcgen05.ld.  No tensor-core instruction is issued; the
-// bits are the staged fp32 values, so the results are those of the shared-memory path.
-// Columns of a thread (warp w: lanes 32 (w % 4) ..., column block 128 (w / 4)): hop k's link at 20 k (18 reals),
-// clover block at 80 (36 reals).
-__device__ __forceinline__ void tm_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tm_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-// tcgen05.ld is asynchronous: its destination registers are valid after tcgen05.wait::ld.  The registers are in/out
-// operands of the wait, so no use of them can be scheduled above it.
-__device__ __forceinline__ void tm_wait_ld18(float* v) {
-    asm volatile("tcgen05.wait::ld.sync.aligned;"
-                 : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]), "+f"(v[8]),
-                   "+f"(v[9]), "+f"(v[10]), "+f"(v[11]), "+f"(v[12]), "+f"(v[13]), "+f"(v[14]), "+f"(v[15]), "+f"(v[16]),
-                   "+f"(v[17])::"memory");
-}
-__device__ __forceinline__ void tm_wait_ld36(float* v) {
-    tm_wait_ld18(v);  // (the second half is ordered behind the first wait by the same mechanism)
-    asm volatile("" : "+f"(v[18]), "+f"(v[19]), "+f"(v[20]), "+f"(v[21]), "+f"(v[22]), "+f"(v[23]), "+f"(v[24]), "+f"(v[25]),
-                 "+f"(v[26]), "+f"(v[27]), "+f"(v[28]), "+f"(v[29]), "+f"(v[30]), "+f"(v[31]), "+f"(v[32]), "+f"(v[33]),
-                 "+f"(v[34]), "+f"(v[35])::"memory");
-}
-__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tm_st16(unsigned ta, const float* v) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(ta),
-        "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]), "f"(v[8]), "f"(v[9]),
-        "f"(v[10]), "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15])
-        : "memory");
-}
-__device__ __forceinline__ void tm_st4(unsigned ta, const float* v) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(ta), "f"(v[0]), "f"(v[1]), "f"(v[2]),
-                 "f"(v[3])
-                 : "memory");
-}
-__device__ __forceinline__ void tm_st2(unsigned ta, const float* v) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(ta), "f"(v[0]), "f"(v[1]) : "memory");
-}
-__device__ __forceinline__ void tm_ld16(float* v, unsigned ta) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-        : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]), "=f"(v[8]),
-          "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
-        : "r"(ta));
-}
-__device__ __forceinline__ void tm_ld4(float* v, unsigned ta) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3])
-                 : "r"(ta));
-}
-__device__ __forceinline__ void tm_ld2(float* v, unsigned ta) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=f"(v[0]), "=f"(v[1]) : "r"(ta));
-}
-constexpr int TM_COLS = 512, TM_LINK = 20, TM_CLOVER = 80;
-
-// The first iteration's hop: operands from shared memory as in hop_smem, the link parked in tensor memory on the way.
-template <int MU, bool FWD, int SGN>
-__device__ __forceinline__ void hop_smem_park(float acc[24], const V16<float>* __restrict__ rho_s,
-                                              const V16<float>* __restrict__ U_s, const float* __restrict__ U_t, int bv,
-                                              int l_link, int l_nb, float ph, unsigned ta) {
-    float p[24], h[12], u[18], g[12];
-#pragma unroll
-    for (int j = 0; j < 6; j++) {
-        const V16<float> v = rho_s[j * bv + l_nb];
-#pragma unroll
-        for (int q = 0; q < 4; q++) p[j * 4 + q] = v.r[q];
-    }
-#pragma unroll
-    for (int j = 0; j < 4; j++) {
-        const V16<float> v = U_s[(MU * 4 + j) * bv + l_link];
-#pragma unroll
-        for (int q = 0; q < 4; q++) u[j * 4 + q] = v.r[q];
-    }
-    const float2 v = *reinterpret_cast<const float2*>(U_t + (MU * bv + l_link) * 2);
-    u[16] = v.x;
-    u[17] = v.y;
-    tm_st16(ta, u);
-    tm_st2(ta + 16, u + 16);
-    project<MU, SGN, float>(h, p);
-    su3_mult<FWD, float, false>(g, u, h);
-    reconstruct<MU, SGN, float, false>(acc, g, ph);
-}
-// The other iterations' hop: the neighbour spinor from shared memory, the link from tensor memory.  un holds the link
-// requested one hop ahead; NEXT: request the following hop's link (at ta_next) before the arithmetic of this one.
-template <int MU, bool FWD, int SGN, bool NEXT>
-__device__ __forceinline__ void hop_tm(float acc[24], const V16<float>* __restrict__ rho_s, int bv, int l_nb, float ph,
-                                       float un[18], unsigned ta_next) {
-    float p[24], h[12], u[18], g[12];
-#pragma unroll
-    for (int j = 0; j < 6; j++) {
-        const V16<float> v = rho_s[j * bv + l_nb];
-#pragma unroll
-        for (int q = 0; q < 4; q++) p[j * 4 + q] = v.r[q];
-    }
-    tm_wait_ld18(un);
-#pragma unroll
-    for (int q = 0; q < 18; q++) u[q] = un[q];
-    if (NEXT) {
-        tm_ld16(un, ta_next);
-        tm_ld2(un + 16, ta_next + 16);
-    }
-    project<MU, SGN, float>(h, p);
-    su3_mult<FWD, float, false>(g, u, h);
-    reconstruct<MU, SGN, float, false>(acc, g, ph);
-}
-
 // x (+)= M_SAP^(g) r: one domain per CTA, two threads per site (see above); ACC: accumulate into x.
 // BVC: sites per domain as a compile-time constant (a multiple of 32; every shared-memory row offset then folds into
 // the immediate field of LDS/STS: -12 % instructions), 0 = run-time P.bv.
-// TM: links and clover blocks parked in tensor memory after the first iteration (fp32, BVC = 256 only; above).
-template <typename T, bool ACC, int BVC, bool TM>
+template <typename T, bool ACC, int BVC>
 __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits at most 151 sites (320 threads)
     k_mr_domain(T* __restrict__ x, const T* __restrict__ r, const T* __restrict__ U, const T* __restrict__ clover,
                 T kappa, DomParams P, int niter, int nrhs, long long rstride) {
@@ -376,23 +269,6 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
         for (int j = 0; j < NH; j++)
             asm volatile("prefetch.global.L2 [%0];" ::"l"(x + sp_off + (long long)(NH * h + j) * CH * NV));
     }
-    unsigned& tm_slot = *reinterpret_cast<unsigned*>(red + 16 * 3);  // (dynamic shared memory: a static variable would
-                                                                     // not fit next to the opt-in maximum)
-    unsigned tm_base = 0;  // my lane quarter and column block of the CTA's tensor memory
-    if constexpr (TM) {
-        static_assert(!TM || (BVC == 256 && sizeof(T) == 4), "the tensor-memory variant is the fp32 4^4 one");
-        if (tid < 32) {
-            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
-                             (unsigned)__cvta_generic_to_shared(&tm_slot)),
-                         "n"(TM_COLS)
-                         : "memory");
-            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-        }
-        tm_fence_before();
-        __syncthreads();
-        tm_fence_after();
-        tm_base = tm_slot + ((unsigned)(32 * ((tid >> 5) & 3)) << 16) + (unsigned)((tid >> 7) * 128);
-    }
 
     // neighbours inside the domain (local index, wrapped) and hop phases: a hop that leaves the domain is cut
     // (phase 0); in a direction spanned by ONE domain the wrap is the lattice's own and carries bc[mu].
@@ -448,52 +324,7 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
             T acc[24];
 #pragma unroll
             for (int q = 0; q < 24; q++) acc[q] = 0;
-            bool hops_done = false;
-            if constexpr (TM) {
-                const bool first = krhs == 0 && it == 0;  // links still only in shared memory
-                if (first) {
-                    if (h == 0) {
-                        hop_smem_park<0, true, -1>(acc, rho_s, U_s, U_t, bv, l, nf[0], pf[0], tm_base);
-                        hop_smem_park<0, false, +1>(acc, rho_s, U_s, U_t, bv, nb[0], nb[0], pb[0], tm_base + TM_LINK);
-                        hop_smem_park<1, true, -1>(acc, rho_s, U_s, U_t, bv, l, nf[1], pf[1], tm_base + 2 * TM_LINK);
-                        hop_smem_park<1, false, +1>(acc, rho_s, U_s, U_t, bv, nb[1], nb[1], pb[1], tm_base + 3 * TM_LINK);
-                    } else {
-                        hop_smem_park<2, true, -1>(acc, rho_s, U_s, U_t, bv, l, nf[2], pf[2], tm_base);
-                        hop_smem_park<2, false, +1>(acc, rho_s, U_s, U_t, bv, nb[2], nb[2], pb[2], tm_base + TM_LINK);
-                        hop_smem_park<3, true, -1>(acc, rho_s, U_s, U_t, bv, l, nf[3], pf[3], tm_base + 2 * TM_LINK);
-                        hop_smem_park<3, false, +1>(acc, rho_s, U_s, U_t, bv, nb[3], nb[3], pb[3], tm_base + 3 * TM_LINK);
-                    }
-                    tm_wait_st();
-                } else {
-                    float un[18];
-                    tm_ld16(un, tm_base);
-                    tm_ld2(un + 16, tm_base + 16);
-                    if (h == 0) {
-                        hop_tm<0, true, -1, true>(acc, rho_s, bv, nf[0], pf[0], un, tm_base + TM_LINK);
-                        hop_tm<0, false, +1, true>(acc, rho_s, bv, nb[0], pb[0], un, tm_base + 2 * TM_LINK);
-                        hop_tm<1, true, -1, true>(acc, rho_s, bv, nf[1], pf[1], un, tm_base + 3 * TM_LINK);
-                        hop_tm<1, false, +1, false>(acc, rho_s, bv, nb[1], pb[1], un, 0u);
-                    } else {
-                        hop_tm<2, true, -1, true>(acc, rho_s, bv, nf[2], pf[2], un, tm_base + TM_LINK);
-                        hop_tm<2, false, +1, true>(acc, rho_s, bv, nb[2], pb[2], un, tm_base + 2 * TM_LINK);
-                        hop_tm<3, true, -1, true>(acc, rho_s, bv, nf[3], pf[3], un, tm_base + 3 * TM_LINK);
-                        hop_tm<3, false, +1, false>(acc, rho_s, bv, nb[3], pb[3], un, 0u);
-                    }
-                }
-                hops_done = true;
-            }
-            if (hops_done) {
-#pragma unroll
-                for (int j = 0; j < NH; j++) {
-                    V16<T> v;
-#pragma unroll
-                    for (int q = 0; q < NV; q++) {
-                        v.r[q] = h ? acc[j * NV + q] : acc[12 + j * NV + q];
-                        mine[j * NV + q] = h ? acc[12 + j * NV + q] : acc[j * NV + q];
-                    }
-                    xch_s[j * 2 * bvp + tid] = v;
-                }
-            } else if (h == 0) {
+            if (h == 0) {
                 hop_smem<0, true, -1, T>(acc, rho_s, U_s, U_t, bv, l, nf[0], pf[0]);
                 hop_smem<0, false, +1, T>(acc, rho_s, U_s, U_t, bv, nb[0], nb[0], pb[0]);
                 hop_smem<1, true, -1, T>(acc, rho_s, U_s, U_t, bv, l, nf[1], pf[1]);
@@ -536,29 +367,11 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
         {
             cp_async_wait_group<0>();  // my clover rows (a no-op after the first iteration)
             T cl[36];
-            bool have = false;
-            if constexpr (TM) {
-                if (!(krhs == 0 && it == 0)) {  // parked in tensor memory by the first iteration
-                    tm_ld16(cl, tm_base + TM_CLOVER);
-                    tm_ld16(cl + 16, tm_base + TM_CLOVER + 16);
-                    tm_ld4(cl + 32, tm_base + TM_CLOVER + 32);
-                    tm_wait_ld36(cl);
-                    have = true;
-                }
-            }
-            if (!have) {
 #pragma unroll
-                for (int j = 0; j < 36 / NV; j++) {
-                    const V16<T> v = C_s[(h * (36 / NV) + j) * bv + l];
+            for (int j = 0; j < 36 / NV; j++) {
+                const V16<T> v = C_s[(h * (36 / NV) + j) * bv + l];
 #pragma unroll
-                    for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
-                }
-                if constexpr (TM) {
-                    tm_st16(tm_base + TM_CLOVER, cl);
-                    tm_st16(tm_base + TM_CLOVER + 16, cl + 16);
-                    tm_st4(tm_base + TM_CLOVER + 32, cl + 32);
-                    tm_wait_st();
-                }
+                for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
             }
             herm6_madd<T, false>(p, cl, rho);
         }
@@ -611,12 +424,435 @@ __global__ void __launch_bounds__(sizeof(T) == 4 ? 512 : 320, 1)  // fp64 fits a
         }
     }
     }  // right-hand sides
-    if constexpr (TM) {
-        tm_fence_before();
-        __syncthreads();
-        if (tid < 32)
-            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_slot), "n"(TM_COLS) : "memory");
+}
+
+// ---- the persistent tensor-memory form of the resident solver (fp32, 4^4 domains, tiled site order) ----------
+// k_mr_domain is bound by the shared-memory pipe (ncu: LDS wavefronts 68 % of the pipe's peak, short-scoreboard and
+// MIO-throttle stalls on top), and 55 % of its LDS traffic are operands that are PRIVATE to a thread and constant over
+// the n_mr iterations: the four links of its four hops and its clover block.  Blackwell's tensor memory (256 KB per
+// SM, 128 lanes x 512 columns of 32 bits, read by tcgen05.ld on a datapath of its own: measured 870 B/clk/SM against
+// the shared-memory pipe's 128) is addressed exactly that way -- lane = thread of a warp quarter, column = register
+// index -- so this kernel parks them there: the first iteration of a domain reads them from shared memory and stores
+// them with tcgen05.st, the others read them back with tcgen05.ld (shared-memory pipe 68 -> 47 % busy).  No
+// tensor-core instruction is issued; the parked bits are the staged fp32 values.
+// One CTA per SM walks the domains b = blockIdx.x, blockIdx.x + gridDim.x, ...; tensor memory is allocated once.  From
+// the second iteration on the staging buffers are idle, so the NEXT domain is staged under the remaining iterations:
+// on the tiled site order a 4^4 domain is 8 whole chunks, i.e. 8 contiguous 9216-byte blocks of links, 8 of clover
+// term, requested as 16 bulk copies (cp.async.bulk, completion on two mbarriers: links, clover) instead of 22 cp.async
+// instructions in every thread, and the HBM reads that the one-CTA-per-domain kernel exposes at the start of every
+// CTA disappear behind the arithmetic.
+// Shared memory mirrors the native chunk layouts (local site l = 32 c + lane, c = (z >> 1) + 2 t).
+// Columns of a thread in tensor memory (warp w: lanes 32 (w % 4) ..., column block 128 (w / 4)): hop k's link at 20 k
+// (18 reals), clover block at 80 (36 reals).
+// Preconditions (host): tiled site order, every enumerated domain selected (all domains, or the half grid of one
+// group), niter >= 2.  Same arithmetic in the same order as k_mr_domain: bit-identical results (tested).
+__device__ __forceinline__ void tm_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tm_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// tcgen05.ld is asynchronous: its destination registers are valid after tcgen05.wait::ld.  The registers are in/out
+// operands of the wait, so no use of them can be scheduled above it.
+__device__ __forceinline__ void tm_wait_ld18(float* v) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7]), "+f"(v[8]),
+                   "+f"(v[9]), "+f"(v[10]), "+f"(v[11]), "+f"(v[12]), "+f"(v[13]), "+f"(v[14]), "+f"(v[15]), "+f"(v[16]),
+                   "+f"(v[17])::"memory");
+}
+__device__ __forceinline__ void tm_wait_ld36(float* v) {
+    tm_wait_ld18(v);  // (the second half is ordered behind the first wait by the same mechanism)
+    asm volatile("" : "+f"(v[18]), "+f"(v[19]), "+f"(v[20]), "+f"(v[21]), "+f"(v[22]), "+f"(v[23]), "+f"(v[24]), "+f"(v[25]),
+                 "+f"(v[26]), "+f"(v[27]), "+f"(v[28]), "+f"(v[29]), "+f"(v[30]), "+f"(v[31]), "+f"(v[32]), "+f"(v[33]),
+                 "+f"(v[34]), "+f"(v[35])::"memory");
+}
+__device__ __forceinline__ void tm_st16(unsigned ta, const float* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(ta),
+        "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]), "f"(v[8]), "f"(v[9]),
+        "f"(v[10]), "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15])
+        : "memory");
+}
+__device__ __forceinline__ void tm_st4(unsigned ta, const float* v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(ta), "f"(v[0]), "f"(v[1]), "f"(v[2]),
+                 "f"(v[3])
+                 : "memory");
+}
+__device__ __forceinline__ void tm_st2(unsigned ta, const float* v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(ta), "f"(v[0]), "f"(v[1]) : "memory");
+}
+__device__ __forceinline__ void tm_ld16(float* v, unsigned ta) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]), "=f"(v[8]),
+          "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
+        : "r"(ta));
+}
+__device__ __forceinline__ void tm_ld4(float* v, unsigned ta) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3])
+                 : "r"(ta));
+}
+__device__ __forceinline__ void tm_ld2(float* v, unsigned ta) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=f"(v[0]), "=f"(v[1]) : "r"(ta));
+}
+constexpr int TM_COLS = 512, TM_LINK = 20, TM_CLOVER = 80;
+
+// mbarrier + bulk-copy plumbing of the staging
+__device__ __forceinline__ unsigned sm_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(sm_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void sbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(sm_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void sbar_wait(unsigned long long* bar, unsigned parity) {
+    unsigned ok;
+    long long t0 = 0;
+    for (unsigned n = 0;; n++) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(sm_u32(bar)), "r"(parity)
+            : "memory");
+        if (ok) return;
+        if ((n & 1023u) == 1023u) {  // a wait of seconds can only be a protocol error: fail the launch, do not hang
+            const long long t = clock64();
+            if (t0 == 0) t0 = t;
+            else if (t - t0 > 4000000000ll) __trap();
+        }
     }
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(sm_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(sm_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+
+// Shared-memory image of the persistent kernel (offsets in floats): chunk-major copies of the native layouts
+struct TmSmem {
+    static constexpr int RHO = 0;                    // [6][256] float4: the current residual (as in k_mr_domain)
+    static constexpr int LINKS = RHO + 6 * 256 * 4;  // [8 chunks][4 mu][576]: rows 0..3 [lane] float4, tail [lane] float2
+    static constexpr int CLOVER = LINKS + 8 * 2304;  // [8][18 rows][32] float4
+    static constexpr int RNEXT = CLOVER + 8 * 2304;  // [8][6 rows][32] float4: first residual of the staged domain
+    static constexpr int XCH = RNEXT + 8 * 768;      // [3][512] float4
+    static constexpr int RED = XCH + 3 * 512 * 4;    // 48 partial sums
+    static constexpr int SLOT = RED + 48;            // tensor-memory base address (+ pad)
+    static constexpr int BARS = SLOT + 4;            // two mbarriers (16 bytes)
+    static constexpr int FLOATS = BARS + 4;
+    static constexpr size_t BYTES = (size_t)FLOATS * 4;
+};
+
+// The first iteration's hop: operands from shared memory (chunk layout), the link parked in tensor memory on the way.
+template <int MU, bool FWD, int SGN>
+__device__ __forceinline__ void hop_chunk_park(float acc[24], const V16<float>* __restrict__ rho_s,
+                                               const float* __restrict__ links_s, int l_link, int l_nb, float ph,
+                                               unsigned ta) {
+    float p[24], h[12], u[18], g[12];
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+        const V16<float> v = rho_s[j * 256 + l_nb];
+#pragma unroll
+        for (int q = 0; q < 4; q++) p[j * 4 + q] = v.r[q];
+    }
+    const float* lk = links_s + ((l_link >> 5) * 4 + MU) * 576;
+    const int lane = l_link & 31;
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        const V16<float> v = *reinterpret_cast<const V16<float>*>(lk + j * 128 + lane * 4);
+#pragma unroll
+        for (int q = 0; q < 4; q++) u[j * 4 + q] = v.r[q];
+    }
+    const float2 v = *reinterpret_cast<const float2*>(lk + 512 + lane * 2);
+    u[16] = v.x;
+    u[17] = v.y;
+    tm_st16(ta, u);
+    tm_st2(ta + 16, u + 16);
+    project<MU, SGN, float>(h, p);
+    su3_mult<FWD, float, false>(g, u, h);
+    reconstruct<MU, SGN, float, false>(acc, g, ph);
+}
+// The other iterations' hop: the neighbour spinor from shared memory, the link from tensor memory.  un holds the link
+// requested one hop ahead; NEXT: request the following hop's link (at ta_next) before the arithmetic of this one.
+template <int MU, bool FWD, int SGN, bool NEXT>
+__device__ __forceinline__ void hop_tm(float acc[24], const V16<float>* __restrict__ rho_s, int l_nb, float ph,
+                                       float un[18], unsigned ta_next) {
+    float p[24], h[12], u[18], g[12];
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+        const V16<float> v = rho_s[j * 256 + l_nb];
+#pragma unroll
+        for (int q = 0; q < 4; q++) p[j * 4 + q] = v.r[q];
+    }
+    tm_wait_ld18(un);
+#pragma unroll
+    for (int q = 0; q < 18; q++) u[q] = un[q];
+    if (NEXT) {
+        tm_ld16(un, ta_next);
+        tm_ld2(un + 16, ta_next + 16);
+    }
+    project<MU, SGN, float>(h, p);
+    su3_mult<FWD, float, false>(g, u, h);
+    reconstruct<MU, SGN, float, false>(acc, g, ph);
+}
+
+template <bool ACC>
+__global__ void __launch_bounds__(512, 1)
+    k_mr_domain_tm(float* __restrict__ x, const float* __restrict__ r, const float* __restrict__ U,
+                   const float* __restrict__ clover, float kappa, DomParams P, int niter, int nrhs, long long rstride,
+                   int ndom) {
+    using T = float;
+    constexpr int NV = 4, NH = 3, bv = 256, bvp = 256;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* sm = reinterpret_cast<float*>(smem_raw);
+    const int tid = threadIdx.x;
+    V16<T>* rho_s = reinterpret_cast<V16<T>*>(sm + TmSmem::RHO);
+    const float* links_s = sm + TmSmem::LINKS;
+    const float* clover_s = sm + TmSmem::CLOVER;
+    const float* rnext_s = sm + TmSmem::RNEXT;
+    V16<T>* xch_s = reinterpret_cast<V16<T>*>(sm + TmSmem::XCH);
+    T* red = sm + TmSmem::RED;
+    unsigned& tm_slot = *reinterpret_cast<unsigned*>(sm + TmSmem::SLOT);
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(sm + TmSmem::BARS);  // [0] links + residual, [1] clover
+
+    const int h = tid >= bvp;  // warp-uniform
+    const int l = tid - h * bvp;
+    const int partner = h ? tid - bvp : tid + bvp;
+    const int lc = l >> 5, lane = l & 31;  // my chunk of the domain and my lane in it (= native lane: tiled order)
+    const int cstep_z = P.ord.T[2] >> 5, cstep_t = P.ord.T[3] >> 5;  // chunk stride between z pairs / time slices
+
+    // first chunk of domain b
+    auto chunk0 = [&](int b) {
+        int Xc[4];
+        domain_of_cta(P, b, Xc);
+        return P.ord.index(Xc[0] * 4, Xc[1] * 4, Xc[2] * 4, Xc[3] * 4) >> 5;
+    };
+    // staging of domain b.  Links and clover term: 16 bulk copies on two mbarriers, one per warp (lane 0) -- the SM
+    // accepts one bulk request per ~80 cycles and its issuer waits for it, so their number is what counts: with the
+    // residual and the L2 prefetch of the solution as bulk requests too (32) they were 2.6 k cycles on the critical
+    // path of every domain.  Those two are per-thread instead: cp.async of my half of the (first) residual, which only I
+    // read, and prefetch.global.L2 of my lines of the solution.
+    // (The copies of the other warps may complete before thread 0's expect_tx: the phase cannot, it needs that arrival.)
+    auto stage = [&](int b) {
+        const long long c0 = chunk0(b);
+        {
+            const long long so = ((c0 + (lc & 1) * cstep_z + (lc >> 1) * cstep_t) * 6 * CH + lane) * NV;
+#pragma unroll
+            for (int j = 0; j < NH; j++) {
+                cp_async16<T>(sm + TmSmem::RNEXT + lc * 768 + (NH * h + j) * 128 + lane * 4,
+                              r + so + (long long)(NH * h + j) * CH * NV);
+                if (ACC) asm volatile("prefetch.global.L2 [%0];" ::"l"(x + so + (long long)(NH * h + j) * CH * NV));
+            }
+            cp_async_commit();
+        }
+        if (tid == 0) {
+            sbar_expect_tx(&bars[0], 8 * 9216);
+            sbar_expect_tx(&bars[1], 8 * 9216);
+        }
+        if ((tid & 31) == 0) {
+            const int i = tid >> 5, c = i & 7;
+            const long long ch = c0 + (c & 1) * cstep_z + (c >> 1) * cstep_t;
+            if (i < 8) bulk_g2s(sm + TmSmem::LINKS + c * 2304, U + ch * 2304, 9216, &bars[0]);
+            else bulk_g2s(sm + TmSmem::CLOVER + c * 2304, clover + ch * 2304, 9216, &bars[1]);
+        }
+    };
+    if (tid == 0) {
+        sbar_init(&bars[0], 1);
+        sbar_init(&bars[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (tid < 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sm_u32(&tm_slot)),
+                     "n"(TM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tm_fence_before();
+    __syncthreads();
+    tm_fence_after();
+    const unsigned tm_base = tm_slot + ((unsigned)(32 * ((tid >> 5) & 3)) << 16) + (unsigned)((tid >> 7) * 128);
+    int b = blockIdx.x;
+    if (b < ndom) stage(b);
+
+    // neighbours inside the domain and hop phases: the same for every domain
+    int nf[4], nb[4];
+    T pf[4], pb[4];
+    {
+        const int lxm[4] = {l & 3, (l >> 2) & 3, (l >> 4) & 3, l >> 6};
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const int ls = 1 << (2 * mu);
+            const bool wf = lxm[mu] == 3, wb = lxm[mu] == 0;
+            nf[mu] = wf ? l - 3 * ls : l + ls;
+            nb[mu] = wb ? l + 3 * ls : l - ls;
+            const T wrap = P.multi[mu] ? (T)0 : (T)P.bc[mu];
+            pf[mu] = wf ? wrap : (T)1;
+            pb[mu] = wb ? wrap : (T)1;
+        }
+    }
+    unsigned phase = 0;
+    for (; b < ndom; b += gridDim.x, phase ^= 1u) {
+        const long long ch = chunk0(b) + (lc & 1) * cstep_z + (lc >> 1) * cstep_t;  // my native chunk
+        const long long sp_off = (ch * 6 * CH + lane) * NV;
+        sbar_wait(&bars[0], phase);  // the links of this domain have landed
+        cp_async_wait_group<0>();    // ... and my half of its first residual
+        T rho[12];
+#pragma unroll
+        for (int j = 0; j < NH; j++) {
+            const V16<T> v = *reinterpret_cast<const V16<T>*>(rnext_s + lc * 768 + (NH * h + j) * 128 + lane * 4);
+#pragma unroll
+            for (int q = 0; q < NV; q++) rho[j * NV + q] = v.r[q];
+        }
+        for (int krhs = 0; krhs < nrhs; krhs++) {
+            const T* rk = r + krhs * rstride;
+            T* xk = x + krhs * rstride;
+            if (krhs > 0) {
+#pragma unroll
+                for (int j = 0; j < NH; j++) {
+                    const V16<T> v = ld16_g64(rk + sp_off + (long long)(NH * h + j) * CH * NV);
+#pragma unroll
+                    for (int q = 0; q < NV; q++) rho[j * NV + q] = v.r[q];
+                }
+            }
+            T z[12];
+#pragma unroll
+            for (int q = 0; q < 12; q++) z[q] = 0;
+            for (int it = 0; it < niter; it++) {
+                const bool first = krhs == 0 && it == 0;  // operands still only in shared memory
+#pragma unroll
+                for (int j = 0; j < NH; j++) {
+                    V16<T> v;
+#pragma unroll
+                    for (int q = 0; q < NV; q++) v.r[q] = rho[j * NV + q];
+                    rho_s[(NH * h + j) * bv + l] = v;
+                }
+                __syncthreads();
+                T mine[12];
+                {
+                    T acc[24];
+#pragma unroll
+                    for (int q = 0; q < 24; q++) acc[q] = 0;
+                    if (first) {
+                        if (h == 0) {
+                            hop_chunk_park<0, true, -1>(acc, rho_s, links_s, l, nf[0], pf[0], tm_base);
+                            hop_chunk_park<0, false, +1>(acc, rho_s, links_s, nb[0], nb[0], pb[0], tm_base + TM_LINK);
+                            hop_chunk_park<1, true, -1>(acc, rho_s, links_s, l, nf[1], pf[1], tm_base + 2 * TM_LINK);
+                            hop_chunk_park<1, false, +1>(acc, rho_s, links_s, nb[1], nb[1], pb[1], tm_base + 3 * TM_LINK);
+                        } else {
+                            hop_chunk_park<2, true, -1>(acc, rho_s, links_s, l, nf[2], pf[2], tm_base);
+                            hop_chunk_park<2, false, +1>(acc, rho_s, links_s, nb[2], nb[2], pb[2], tm_base + TM_LINK);
+                            hop_chunk_park<3, true, -1>(acc, rho_s, links_s, l, nf[3], pf[3], tm_base + 2 * TM_LINK);
+                            hop_chunk_park<3, false, +1>(acc, rho_s, links_s, nb[3], nb[3], pb[3], tm_base + 3 * TM_LINK);
+                        }
+                        tm_wait_st();
+                    } else {
+                        float un[18];
+                        tm_ld16(un, tm_base);
+                        tm_ld2(un + 16, tm_base + 16);
+                        if (h == 0) {
+                            hop_tm<0, true, -1, true>(acc, rho_s, nf[0], pf[0], un, tm_base + TM_LINK);
+                            hop_tm<0, false, +1, true>(acc, rho_s, nb[0], pb[0], un, tm_base + 2 * TM_LINK);
+                            hop_tm<1, true, -1, true>(acc, rho_s, nf[1], pf[1], un, tm_base + 3 * TM_LINK);
+                            hop_tm<1, false, +1, false>(acc, rho_s, nb[1], pb[1], un, 0u);
+                        } else {
+                            hop_tm<2, true, -1, true>(acc, rho_s, nf[2], pf[2], un, tm_base + TM_LINK);
+                            hop_tm<2, false, +1, true>(acc, rho_s, nb[2], pb[2], un, tm_base + 2 * TM_LINK);
+                            hop_tm<3, true, -1, true>(acc, rho_s, nf[3], pf[3], un, tm_base + 3 * TM_LINK);
+                            hop_tm<3, false, +1, false>(acc, rho_s, nb[3], pb[3], un, 0u);
+                        }
+                    }
+#pragma unroll
+                    for (int j = 0; j < NH; j++) {
+                        V16<T> v;
+#pragma unroll
+                        for (int q = 0; q < NV; q++) {
+                            v.r[q] = h ? acc[j * NV + q] : acc[12 + j * NV + q];
+                            mine[j * NV + q] = h ? acc[12 + j * NV + q] : acc[j * NV + q];
+                        }
+                        xch_s[j * 2 * bvp + tid] = v;
+                    }
+                }
+                __syncthreads();
+                T p[12];
+#pragma unroll
+                for (int j = 0; j < NH; j++) {
+                    const V16<T> v = xch_s[j * 2 * bvp + partner];
+#pragma unroll
+                    for (int q = 0; q < NV; q++) p[j * NV + q] = fma(-kappa, mine[j * NV + q] + v.r[q], rho[j * NV + q]);
+                }
+                {
+                    T cl[36];
+                    if (first) {
+                        sbar_wait(&bars[1], phase);  // the clover term of this domain has landed
+#pragma unroll
+                        for (int j = 0; j < 9; j++) {
+                            const V16<T> v =
+                                *reinterpret_cast<const V16<T>*>(clover_s + lc * 2304 + (h * 9 + j) * 128 + lane * 4);
+#pragma unroll
+                            for (int q = 0; q < NV; q++) cl[j * NV + q] = v.r[q];
+                        }
+                        tm_st16(tm_base + TM_CLOVER, cl);
+                        tm_st16(tm_base + TM_CLOVER + 16, cl + 16);
+                        tm_st4(tm_base + TM_CLOVER + 32, cl + 32);
+                        tm_wait_st();
+                    } else {
+                        tm_ld16(cl, tm_base + TM_CLOVER);
+                        tm_ld16(cl + 16, tm_base + TM_CLOVER + 16);
+                        tm_ld4(cl + 32, tm_base + TM_CLOVER + 32);
+                        tm_wait_ld36(cl);
+                    }
+                    herm6_madd<T, false>(p, cl, rho);
+                }
+                T d[3] = {0, 0, 0};
+#pragma unroll
+                for (int k = 0; k < 6; k++) {
+                    d[0] = fma(p[2 * k], rho[2 * k], d[0]);
+                    d[0] = fma(p[2 * k + 1], rho[2 * k + 1], d[0]);
+                    d[1] = fma(p[2 * k], rho[2 * k + 1], d[1]);
+                    d[1] = fma(-p[2 * k + 1], rho[2 * k], d[1]);
+                    d[2] = fma(p[2 * k], p[2 * k], d[2]);
+                    d[2] = fma(p[2 * k + 1], p[2 * k + 1], d[2]);
+                }
+                cta_sum_v<3, 16>(d, red);
+                // every thread is past its last read of the staging buffers of this domain: stage the next one
+                if (first && b + (int)gridDim.x < ndom) stage(b + gridDim.x);
+                const T ar = d[2] > 0 ? d[0] / d[2] : (T)0, ai = d[2] > 0 ? d[1] / d[2] : (T)0;
+#pragma unroll
+                for (int k = 0; k < 6; k++) {
+                    const T rr = rho[2 * k], ri = rho[2 * k + 1];
+                    z[2 * k] = fma(ar, rr, z[2 * k]);
+                    z[2 * k] = fma(-ai, ri, z[2 * k]);
+                    z[2 * k + 1] = fma(ar, ri, z[2 * k + 1]);
+                    z[2 * k + 1] = fma(ai, rr, z[2 * k + 1]);
+                    rho[2 * k] = fma(-ar, p[2 * k], rho[2 * k]);
+                    rho[2 * k] = fma(ai, p[2 * k + 1], rho[2 * k]);
+                    rho[2 * k + 1] = fma(-ar, p[2 * k + 1], rho[2 * k + 1]);
+                    rho[2 * k + 1] = fma(-ai, p[2 * k], rho[2 * k + 1]);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < NH; j++) {
+                T* px = xk + sp_off + (long long)(NH * h + j) * CH * NV;
+                V16<T> v;
+#pragma unroll
+                for (int q = 0; q < NV; q++) v.r[q] = z[j * NV + q];
+                if (ACC) {
+                    const V16<T> xo = ld16_g64(px);
+#pragma unroll
+                    for (int q = 0; q < NV; q++) v.r[q] += xo.r[q];
+                }
+                st16(px, v);
+            }
+        }  // right-hand sides
+    }  // domains
+    tm_fence_before();
+    __syncthreads();
+    if (tid < 32)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_slot), "n"(TM_COLS) : "memory");
 }
 
 // ---- blocked BLAS-1: one CTA per domain, sites strided over the threads ------------------------
@@ -803,6 +1039,19 @@ static int dom_setup(DomParams& P, const int dims[4], const int bc[4], const int
     P.parity = 0;
     P.halfgrid = 0;
     P.ord.set(dims);
+    {  // reciprocals of the index decode: exact while (CTA or site index) * divisor < 2^32
+        long long dmax = 1;
+        for (int mu = 0; mu < 3; mu++) dmax = P.Lc[mu] > dmax ? P.Lc[mu] : dmax;
+        if ((long long)P.Vc * dmax >= 0x100000000LL || (long long)P.bv * P.bv >= 0x100000000LL) {
+            set_error("%s: lattice too large for the 32-bit index decode", what);
+            return LQCD_EUNSUPPORTED;
+        }
+        for (int mu = 0; mu < 3; mu++) {
+            P.d_Lc[mu].set(P.Lc[mu]);
+            P.d_dom[mu].set(P.dom[mu]);
+        }
+        P.d_half.set(P.Lc[0] > 1 ? P.Lc[0] / 2 : 1);
+    }
     return LQCD_OK;
 }
 
@@ -851,25 +1100,36 @@ static int mr_domain_call(T* z, const T* r, const T* U, const T* clover, T kappa
             grid = (unsigned)(P.Vc / 2);
         }
         const long long rstride = (long long)nchunks(dims) * CH * 24;  // right-hand sides back to back
-#define LAUNCH_MR(ACC, BVC, TM)                                                                                 \
+        if constexpr (sizeof(T) == 4) {
+            if (g_knobs.sap_tmem >= 0 && niter >= 2 && (P.parity == 0 || P.halfgrid) && P.ord.tiled && domain[0] == 4 &&
+                domain[1] == 4 && domain[2] == 4 && domain[3] == 4 && TmSmem::BYTES <= (size_t)max_optin_smem()) {
+                // persistent form: one CTA per SM walks the domains, links and clover blocks parked in tensor memory
+                const int ndom = (int)grid;
+                const unsigned g = grid < (unsigned)sm_count() ? grid : (unsigned)sm_count();
+                static unsigned long long attr_a = 0, attr_b = 0;
+                if (acc) {
+                    ensure_dynamic_smem(k_mr_domain_tm<true>, (int)TmSmem::BYTES, attr_a);
+                    k_mr_domain_tm<true><<<g, 512, TmSmem::BYTES, st>>>(z, r, U, clover, kappa, P, niter, K, rstride, ndom);
+                } else {
+                    ensure_dynamic_smem(k_mr_domain_tm<false>, (int)TmSmem::BYTES, attr_b);
+                    k_mr_domain_tm<false><<<g, 512, TmSmem::BYTES, st>>>(z, r, U, clover, kappa, P, niter, K, rstride, ndom);
+                }
+                count_launch();
+                return check_launch(what);
+            }
+        }
+#define LAUNCH_MR(ACC, BVC)                                                                                   \
     do {                                                                                                      \
         static unsigned long long attr = 0;                                                                   \
-        ensure_dynamic_smem(k_mr_domain<T, ACC, BVC, TM>, max_optin_smem(), attr);                            \
-        k_mr_domain<T, ACC, BVC, TM><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter, K, rstride); \
+        ensure_dynamic_smem(k_mr_domain<T, ACC, BVC>, max_optin_smem(), attr);                                \
+        k_mr_domain<T, ACC, BVC><<<grid, threads, smem, st>>>(z, r, U, clover, kappa, P, niter, K, rstride);   \
     } while (0)
         if (sizeof(T) == 4 && P.bv == 256) {  // the paper's typical 4^4 domain
-            constexpr int B = sizeof(T) == 4 ? 256 : 0;
-            constexpr bool F32 = sizeof(T) == 4;
-            if (g_knobs.sap_tmem >= 0) {  // links and clover parked in tensor memory
-                if (acc) LAUNCH_MR(true, B, F32);
-                else LAUNCH_MR(false, B, F32);
-            } else {
-                if (acc) LAUNCH_MR(true, B, false);
-                else LAUNCH_MR(false, B, false);
-            }
+            if (acc) LAUNCH_MR(true, (sizeof(T) == 4 ? 256 : 0));
+            else LAUNCH_MR(false, (sizeof(T) == 4 ? 256 : 0));
         } else {
-            if (acc) LAUNCH_MR(true, 0, false);
-            else LAUNCH_MR(false, 0, false);
+            if (acc) LAUNCH_MR(true, 0);
+            else LAUNCH_MR(false, 0);
         }
 #undef LAUNCH_MR
         count_launch();

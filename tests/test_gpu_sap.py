@@ -30,8 +30,9 @@ def lq():
 
 @pytest.fixture(params=[(0, 0), (0, -1), (-1, 0)], ids=["resident", "resident-smem", "generic"])
 def path(lq, request):
-    """the implementations of the inner-domain solver: shared-memory-resident with the links and clover blocks parked
-    in tensor memory (fp32 4^4 domains; elsewhere the same as the next), shared memory only, generic"""
+    """the implementations of the inner-domain solver: resident (persistent, links and clover blocks parked in tensor
+    memory, for fp32 4^4 domains on the tiled site order; elsewhere the same as the next), resident in shared memory
+    only (one CTA per domain), generic"""
     lq.set_knob("sap_fused", request.param[0])
     lq.set_knob("sap_tmem", request.param[1])
     yield request.param[0]
@@ -295,14 +296,17 @@ def test_sap_mrhs_4x4_domains(lq):
         assert torch.equal(x[k], x1) and torch.equal(r[k], r1), k
 
 
-@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 8, 4, 8)])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (12, 8, 4, 8), (16, 16, 16, 20)])
 def test_mr_tensor_memory_is_bit_identical(lq, dims):
-    """fp32, 4^4 domains: the resident solver parks each thread's links and clover block in tensor memory after the
-    first iteration (knob sap_tmem).  The parked bits are the staged fp32 values and the
-    arithmetic is the same, so every result is bit-identical with the shared-memory-only kernel: all groups, with and
-    without accumulation, 0 ... 7 iterations, several right-hand sides on the resident operator, SAP.  (Against the
-    oracle both run in test_mr_edge_lattices / test_c2_lattice_sap.)  (12, 8, 4, 8): odd Lc[0] (full grid in
-    accumulate mode), a direction spanned by one domain."""
+    """fp32, 4^4 domains, tiled site order: the persistent form of the resident solver (one CTA per SM walks the
+    domains, the next domain staged by bulk copies under the current one's iterations) parks each thread's links and
+    clover block in tensor memory after the first iteration (knob sap_tmem).  The parked bits
+    are the staged fp32 values and the arithmetic is the same, so every result is bit-identical with the
+    one-CTA-per-domain shared-memory kernel: all groups, with and without accumulation, 0 ... 7 iterations (fewer than
+    2 iterations and the full grid of an odd Lc[0] take the other kernel by design), several right-hand sides on the
+    resident operator, SAP.  (Against the oracle both run in test_mr_edge_lattices / test_c2_lattice_sap.)
+    (12, 8, 4, 8): odd Lc[0], a direction spanned by one domain; (16, 16, 16, 20): more domains than SMs, so a CTA walks
+    several domains (320, 160 per group, on 148 SMs: a ragged second round)."""
     import torch
     cfg = custom_config(dims, (4, 4, 4, 4), 1, gauge="exp", eps=0.5, kappa=0.135, csw=1.0, seed=21)
     prob = make_problem(cfg, n_rhs=3, coarse="none")
