@@ -992,21 +992,26 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     e2e_s, h2d, d2h = time_e2e(W, e2e_steps, 1, ranks)
     e2e_s = ranks.max(e2e_s)
     pcie = measure_pcie(device)
-    # ceilings of one e2e step: (i) both directions perfectly overlapped; (ii) the dependency-aware bound: no result can
-    # leave before the first chain's input has arrived and its kernels have run, then the downloads run back to back
+    # Ceilings of one e2e step.  (i) Both directions perfectly overlapped.  (ii) The dependency-aware bound: inside a call
+    # the vector travels in slabs (upload of slab k+1 under the kernels of slab k under the download of slab k-1,
+    # host_api.cu), so the two operator chains keep both directions busy; but prolong's result (one fine vector) can
+    # only leave after restrict's input (one fine vector) has arrived, and while that input occupies a share s of the
+    # upload link the operator chains' uploads -- hence their downloads -- lose exactly that share: whatever the
+    # interleaving, the download link idles for one fine-vector upload:  t >= t_duplex + fine_bytes / h2d rate.
     t_duplex = max(h2d, d2h) / (pcie["duplex_GBps_per_direction"] * 1e9)
     fine_bytes = cfg.volume * 24 * (8 if f64 else 4)
-    t_chain = (fine_bytes / (pcie["h2d_GBps"] * 1e9) +
-               sum(kernels[n]["us"] for n in ("restrict", "coarse_mult", "prolong")) * 1e-6 + d2h / (pcie["d2h_GBps"] * 1e9))
+    t_chain = t_duplex + fine_bytes / (pcie["h2d_GBps"] * 1e9)
     e2e = {"value": whole_job_value(sbytes, ranks.world, e2e_s) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps,
            "pcie_measured": pcie, "ms_if_full_duplex": t_duplex * 1e3, "frac_of_full_duplex_pcie": t_duplex / e2e_s,
            "ms_dependency_bound": t_chain * 1e3, "frac_of_dependency_bound": t_chain / e2e_s,
            "GBps_per_direction": max(h2d, d2h) / e2e_s / 1e9,
            "note": "host-vector C-ABI calls, pinned canonical vectors, three independent chains on three streams; PCIe "
-                   "copies dominate: every call needs its whole input on the device before the first output exists "
-                   "(the stencil wraps around the lattice), so the step cannot beat upload of one vector + its kernels "
-                   "+ all downloads (ms_dependency_bound)"}
+                   "copies dominate.  Inside a call the vector travels in slabs of time slices: upload of slab k+1 under "
+                   "pack / kernel / unpack of slab k under the download of slab k-1.  The transfer chain (restrict -> "
+                   "coarse operator -> prolong) has its one-vector download strictly after its one-vector upload, which "
+                   "leaves the download link idle for one upload whatever the interleaving: ms_dependency_bound = "
+                   "ms_if_full_duplex + one fine vector / h2d rate"}
 
     line = {
         "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": ranks.world, "steps": args.steps,

@@ -519,7 +519,14 @@ int lqcd_coarse_bicgstab_hooks_f64(double* x, double* r_out, const double* b, co
  * The operator fields (U, clover, A, nullvecs) stay resident on the device in native layout; the
  * right-hand side comes from and the result goes back to HOST memory in CANONICAL layout (pinned
  * memory recommended).  Each call: cudaMemcpyAsync H2D -> pack -> the mult kernel -> unpack ->
- * cudaMemcpyAsync D2H -> cudaStreamSynchronize.  ws_dev is caller-owned device scratch of at least
+ * cudaMemcpyAsync D2H -> cudaStreamSynchronize.  A fine vector of at least three slabs of ~16 MB
+ * (knob "host_slab_mb": smallest slab in MB, -1 = never) travels in SLABS of time slices: the upload
+ * of slab k+1 runs under pack / kernel / unpack of slab k (on `stream`) and under the download of
+ * slab k-1, on two copy streams and a set of events that the library creates ONCE per calling host
+ * thread and device and keeps (the only state of these calls; nothing is allocated per call).  The
+ * kernels are the same ones on a range of tiles / aggregates: results are bit-identical with the
+ * one-shot path.  The call returns after everything it enqueued has completed, as before.
+ * ws_dev is caller-owned device scratch of at least
  * lqcd_host_workspace_bytes(...) bytes (the _f32 calls) or lqcd_host_workspace_bytes_f64(...) bytes
  * (the _f64 calls; host and device data are then all double).  Same errors as the device calls. */
 size_t lqcd_host_workspace_bytes(const int dims[4], const int block[4], int nvec);

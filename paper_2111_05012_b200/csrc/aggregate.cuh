@@ -12,6 +12,7 @@ struct TransferParams {
     int bv;    // sites per block
     int nvec;
     int LV;    // vec16 per (X, chi, i) vector = bv * 12 / NV
+    int agg_off;  // first aggregate (X, chi) of the launch (range forms of restrict / prolong; 0 otherwise)
     SiteOrder ord;  // native position of a fine site (layout.cuh)
 };
 
@@ -53,6 +54,7 @@ inline int transfer_setup(TransferParams& P, const void* a, const void* b, const
         P.bv *= block[mu];
     }
     P.nvec = nvec;
+    P.agg_off = 0;
     P.LV = P.bv * 12 / VecOf<T>::NV;
     P.ord.set(dims);
     return LQCD_OK;

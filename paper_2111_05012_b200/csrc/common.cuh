@@ -163,6 +163,23 @@ struct FastDiv {
     __device__ __forceinline__ int div(int n) const { return (int)(__umulhi((unsigned)n, m) + (unsigned)n * one); }
 };
 
+// ---- internal range forms of the hot-path calls (host_api.cu pipelines a host vector through them slab by slab) -----
+// canonical <-> native re-layout of the sites [s0, s1) (canonical index) of a spinor
+template <typename T, bool UNPACK>
+int spinor_range_call(T* dst, const T* src, const int dims[4], long long s0, long long s1, void* stream, const char* what);
+// D (or D^dag) on the time slices [t0, t1) only; both multiples of fine_tile_extent_t(); canonical tile traversal
+template <typename T>
+int wilson_clover_slab_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4], const int bc[4],
+                            unsigned flags, int t0, int t1, void* stream, const char* what);
+int fine_tile_extent_t(const int dims[4], const int bc[4], int real_bytes);  // extent in t of the fine kernel's CTA tile
+// restrict / prolong on the aggregates (X, chi) with X in [X0, X1) only
+template <typename T>
+int restrict_range_call(T* out_c, const T* in_f, const T* v, const int dims[4], const int block[4], int nvec, long long X0,
+                        long long X1, void* stream, const char* what);
+template <typename T>
+int prolong_range_call(T* out_f, const T* in_c, const T* v, const int dims[4], const int block[4], int nvec, long long X0,
+                       long long X1, void* stream, const char* what);
+
 // ---- geometry passed to kernels by value ---------------------------------------------------------
 struct Geom {
     int L[4];        // fine dims

@@ -17,6 +17,8 @@ struct Knobs {
     int site_order = 0;               // 0 = tiled site order (4 x 4 x 2 chunks) when the extents allow; -1 = canonical.
                                       // Changes the NATIVE layout: every native field must be packed after setting it
     int sap_group_residual = 0;       // 0 = SAP's intermediate residuals on the next group's domains only; -1 = all sites
+    int host_slab_mb = 0;             // host-vector calls: smallest slab of the upload / compute / download pipeline in MB;
+                                      // 0 = 16; -1 = never pipeline (one-shot path)
     int sap_tmem = 0;                 // 0 = the resident solver parks links and clover blocks in tensor memory (fp32 4^4
                                       // domains); -1 = shared memory only
 };

@@ -7,9 +7,9 @@
 namespace lqcd {
 
 template <typename T, bool UNPACK>
-__global__ void k_spinor(T* __restrict__ dst, const T* __restrict__ src, long long V, SiteOrder ord) {
-    const long long n = V * 24;
-    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
+__global__ void k_spinor(T* __restrict__ dst, const T* __restrict__ src, long long n0, long long n, SiteOrder ord) {
+    // canonical reals [n0, n) (24 per site)
+    for (long long idx = n0 + blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
          idx += (long long)gridDim.x * blockDim.x) {
         const long long s = ord.from_canonical((int)(idx / 24));  // native position of canonical site idx / 24
         const int r = (int)(idx % 24);
@@ -135,10 +135,25 @@ static int spinor_call(T* dst, const T* src, const int dims[4], void* stream, co
     if (V > 0x7fffffffLL) return LQCD_EUNSUPPORTED;
     SiteOrder ord;
     ord.set(dims);
-    k_spinor<T, UNPACK><<<grid_for(V * 24), 256, 0, (cudaStream_t)stream>>>(dst, src, V, ord);
+    k_spinor<T, UNPACK><<<grid_for(V * 24), 256, 0, (cudaStream_t)stream>>>(dst, src, 0, V * 24, ord);
     count_launch();
     return check_launch(what);
 }
+
+// the sites [s0, s1) only (arguments validated by the caller, host_api.cu)
+template <typename T, bool UNPACK>
+int spinor_range_call(T* dst, const T* src, const int dims[4], long long s0, long long s1, void* stream, const char* what) {
+    if (s1 <= s0) return LQCD_OK;
+    SiteOrder ord;
+    ord.set(dims);
+    k_spinor<T, UNPACK><<<grid_for((s1 - s0) * 24), 256, 0, (cudaStream_t)stream>>>(dst, src, s0 * 24, s1 * 24, ord);
+    count_launch();
+    return check_launch(what);
+}
+template int spinor_range_call<float, false>(float*, const float*, const int*, long long, long long, void*, const char*);
+template int spinor_range_call<float, true>(float*, const float*, const int*, long long, long long, void*, const char*);
+template int spinor_range_call<double, false>(double*, const double*, const int*, long long, long long, void*, const char*);
+template int spinor_range_call<double, true>(double*, const double*, const int*, long long, long long, void*, const char*);
 
 template <typename T>
 static int gauge_call(T* dst, const T* src, const int dims[4], unsigned flags, void* stream, const char* what) {

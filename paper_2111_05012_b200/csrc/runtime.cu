@@ -101,6 +101,7 @@ int lqcd_set_knob(const char* name, int value) {
     else if (!strcmp(name, "sap_fused")) g_knobs.sap_fused = value;
     else if (!strcmp(name, "sap_group_residual")) g_knobs.sap_group_residual = value;
     else if (!strcmp(name, "sap_tmem")) g_knobs.sap_tmem = value;
+    else if (!strcmp(name, "host_slab_mb")) g_knobs.host_slab_mb = value;
     else if (!strcmp(name, "fine_mrhs")) g_knobs.fine_mrhs = value;
     else if (!strcmp(name, "mrhs_tensor")) g_knobs.mrhs_tensor = value;
     else if (!strcmp(name, "site_order")) g_knobs.site_order = value;

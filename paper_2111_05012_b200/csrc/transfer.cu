@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(256) k_restrict(T* __restrict__ out_c, const T
     constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, JH = 12 / NV;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* sm = reinterpret_cast<T*>(smem_raw);  // [l][12 reals of chirality chi]
-    const int agg = blockIdx.x;              // (X, chi)
+    const int agg = blockIdx.x + P.agg_off;  // (X, chi)
     const int X = agg >> 1, chi = agg & 1;
     // stage the aggregate's slice of in_f
     for (int idx = threadIdx.x; idx < P.LV; idx += blockDim.x) {
@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(256) k_restrict_mrhs(T* __restrict__ out_c, lo
     constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, JH = 12 / NV;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* sm = reinterpret_cast<T*>(smem_raw);  // [r][l][12 reals of chirality chi]
-    const int agg = blockIdx.x;              // (X, chi)
+    const int agg = blockIdx.x + P.agg_off;  // (X, chi)
     const int X = agg >> 1, chi = agg & 1;
     for (int idx = threadIdx.x; idx < P.LV; idx += blockDim.x) {
         const int l = idx / JH, jj = idx % JH;
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(256) k_prolong(T* __restrict__ out_f, const T*
     constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, JH = 12 / NV;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* xc = reinterpret_cast<T*>(smem_raw);  // nvec complex
-    const int agg = blockIdx.x;
+    const int agg = blockIdx.x + P.agg_off;
     const int X = agg >> 1, chi = agg & 1;
     for (int i = threadIdx.x; i < 2 * P.nvec; i += blockDim.x) xc[i] = in_c[(long long)agg * P.nvec * 2 + i];
     __syncthreads();
@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(256) k_prolong_mrhs(T* __restrict__ out_f, lon
     constexpr int NV = VecOf<T>::NV, NJ = 24 / NV, JH = 12 / NV;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* xc = reinterpret_cast<T*>(smem_raw);  // [r][nvec] complex
-    const int agg = blockIdx.x;
+    const int agg = blockIdx.x + P.agg_off;
     const int X = agg >> 1, chi = agg & 1;
     for (int q = threadIdx.x; q < nr * 2 * P.nvec; q += blockDim.x) {
         const int r = q / (2 * P.nvec), i = q % (2 * P.nvec);
@@ -274,6 +274,34 @@ static int restrict_call(T* out_c, const T* in_f, const T* v, const int dims[4],
     return check_launch(what);
 }
 
+// restrict on the aggregates of the coarse sites [X0, X1) only (host_api.cu: under the upload of the next slab)
+template <typename T>
+int restrict_range_call(T* out_c, const T* in_f, const T* v, const int dims[4], const int block[4], int nvec, long long X0,
+                        long long X1, void* stream, const char* what) {
+    TransferParams P;
+    int rc = transfer_setup<T>(P, out_c, in_f, v, dims, block, nvec, what);
+    if (rc) return rc;
+    const size_t smem = (size_t)P.bv * 12 * sizeof(T);
+    if (smem > 200 * 1024) {
+        set_error("%s: block of %d sites does not fit in shared memory", what, P.bv);
+        return LQCD_EUNSUPPORTED;
+    }
+    if (X1 <= X0) return LQCD_OK;
+    auto kern = k_restrict<T, 8>;
+    if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    int warps = g_knobs.transfer_warps > 0 ? g_knobs.transfer_warps : 8;
+    if (warps > 8) warps = 8;
+    if (warps > nvec) warps = nvec;
+    P.agg_off = (int)(2 * X0);
+    kern<<<(unsigned)(2 * (X1 - X0)), warps * 32, smem, (cudaStream_t)stream>>>(out_c, in_f, v, P);
+    count_launch();
+    return check_launch(what);
+}
+template int restrict_range_call<float>(float*, const float*, const float*, const int*, const int*, int, long long,
+                                        long long, void*, const char*);
+template int restrict_range_call<double>(double*, const double*, const double*, const int*, const int*, int, long long,
+                                         long long, void*, const char*);
+
 // nrhs fine vectors back to back -> nrhs coarse vectors back to back; the null vectors are read once per group of
 // NRMAX vectors (as many as fit in shared memory next to each other: 9 in fp32, 4 in fp64 for 4^4 blocks)
 template <typename T>
@@ -331,6 +359,31 @@ static int prolong_call(T* out_f, const T* in_c, const T* v, const int dims[4], 
     count_launch();
     return check_launch(what);
 }
+
+// prolong on the aggregates of the coarse sites [X0, X1) only (host_api.cu: the download of a slab runs under the
+// prolongation of the next)
+template <typename T>
+int prolong_range_call(T* out_f, const T* in_c, const T* v, const int dims[4], const int block[4], int nvec, long long X0,
+                       long long X1, void* stream, const char* what) {
+    TransferParams P;
+    int rc = transfer_setup<T>(P, out_f, in_c, v, dims, block, nvec, what);
+    if (rc) return rc;
+    const size_t smem = (size_t)nvec * 2 * sizeof(T);
+    if (smem > 48 * 1024) {
+        set_error("%s: nvec = %d outside the compiled range", what, nvec);
+        return LQCD_EUNSUPPORTED;
+    }
+    if (X1 <= X0) return LQCD_OK;
+    const int threads = P.LV >= 256 ? 256 : (P.LV + 31) / 32 * 32;
+    P.agg_off = (int)(2 * X0);
+    k_prolong<T, 8><<<(unsigned)(2 * (X1 - X0)), threads, smem, (cudaStream_t)stream>>>(out_f, in_c, v, P);
+    count_launch();
+    return check_launch(what);
+}
+template int prolong_range_call<float>(float*, const float*, const float*, const int*, const int*, int, long long,
+                                       long long, void*, const char*);
+template int prolong_range_call<double>(double*, const double*, const double*, const int*, const int*, int, long long,
+                                        long long, void*, const char*);
 
 // nrhs coarse vectors back to back -> nrhs fine vectors back to back, null vectors read once per group of 8
 template <typename T>

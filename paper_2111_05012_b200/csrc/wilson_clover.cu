@@ -24,6 +24,7 @@ struct FineParams {
     int ntile[4];  // tiles per direction
     int bc[4];     // +1 / -1
     int tilevol;   // threads that own a site (<= blockDim.x)
+    int tile_off;  // first tile of the launch (slab form: the grid covers a range of time slices; 0 otherwise)
     int warp_tiles;  // 1: tiled site order and a CTA tile made of whole 4 x 4 x 2 layout tiles: a warp owns one of them
     int wt[3];       // ... layout tiles per CTA tile in x, y, z
     FastDiv d_wt[3];
@@ -45,7 +46,7 @@ struct FineParams {
 __device__ __forceinline__ bool fine_decode(const FineParams& P, int x[4], int& s_out) {
     int tid = threadIdx.x;
     if (tid >= P.tilevol) return false;
-    int b = blockIdx.x, q;
+    int b = blockIdx.x + P.tile_off, q;
     int tc[4];
     q = P.d_ntile[0].div(b); tc[0] = b - q * P.ntile[0]; b = q;
     q = P.d_ntile[1].div(b); tc[1] = b - q * P.ntile[1]; b = q;
@@ -239,6 +240,7 @@ static int fine_setup(FineParams& P, long long& ntiles_out, const int dims[4], c
     P.parity = (flags & LQCD_DOMAIN_EVEN) ? 1 : (flags & LQCD_DOMAIN_ODD) ? 2 : 0;
     P.keep = 0;
     P.cut_lat = 0;
+    P.tile_off = 0;
     P.ord.set(dims);
     bool user_ok = g_knobs.fine_tile[0] > 0;
     for (int mu = 0; mu < 4 && user_ok; mu++) user_ok = dims[mu] % g_knobs.fine_tile[mu] == 0;
@@ -373,6 +375,60 @@ int wilson_clover_call(T* out, const T* in, const T* U, const T* clover, const T
     count_launch();
     return check_launch(what);
 }
+// D (D^dag) on the time slices [t0, t1) only: the tiles of those slices in canonical tile order (tiles of one time
+// slice are then consecutive), as host_api.cu needs to run the operator slab by slab under the upload of the next
+// slab.  Arguments were validated by the caller; t0, t1 multiples of the CTA tile's extent in t.
+int fine_tile_extent_t(const int dims[4], const int bc[4], int real_bytes) {
+    FineParams P;
+    long long ntiles = 0;
+    if (fine_setup(P, ntiles, dims, bc, nullptr, 0u, real_bytes, "fine_tile_extent_t")) return 0;
+    return P.tile[3];
+}
+template <typename T>
+int wilson_clover_slab_call(T* out, const T* in, const T* U, const T* clover, T kappa, const int dims[4], const int bc[4],
+                            unsigned flags, int t0, int t1, void* stream, const char* what) {
+    FineParams P;
+    long long ntiles = 0;
+    {
+        const int rc = fine_setup(P, ntiles, dims, bc, nullptr, 0u, (int)sizeof(T), what);
+        if (rc) return rc;
+    }
+    if (t0 % P.tile[3] || t1 % P.tile[3] || t0 < 0 || t1 > dims[3] || t1 <= t0) {
+        set_error("%s: slab [%d, %d) is not made of whole tiles", what, t0, t1);
+        return LQCD_EINVAL;
+    }
+    P.zslab = 0;  // canonical tile order: x, y, z, t
+    P.per_slab = P.ntile[3];
+    P.nslab_full = 0;
+    const long long per_t = (long long)P.ntile[0] * P.ntile[1] * P.ntile[2];
+    P.tile_off = (int)(per_t * (t0 / P.tile[3]));
+    const unsigned grid = (unsigned)(per_t * ((t1 - t0) / P.tile[3]));
+    const int threads = (P.tilevol + 31) / 32 * 32;
+    const bool dag = flags & LQCD_DAGGER, l12 = flags & LQCD_LINKS_12;
+    cudaStream_t st = (cudaStream_t)stream;
+    const T* rhs = nullptr;
+#define LAUNCH_S(DAG, L12)                                                                                   \
+    do {                                                                                                     \
+        if (threads <= 128)                                                                                  \
+            k_wilson_clover<T, DAG, L12, 0, false, 128, (sizeof(T) == 4 ? 4 : 3)>                            \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);                               \
+        else                                                                                                 \
+            k_wilson_clover<T, DAG, L12, 0, false, 256, (sizeof(T) == 4 ? 2 : 1)>                            \
+                <<<grid, threads, 0, st>>>(out, in, U, clover, rhs, kappa, P);                               \
+    } while (0)
+    if (dag && l12) LAUNCH_S(true, true);
+    else if (dag) LAUNCH_S(true, false);
+    else if (l12) LAUNCH_S(false, true);
+    else LAUNCH_S(false, false);
+#undef LAUNCH_S
+    count_launch();
+    return check_launch(what);
+}
+template int wilson_clover_slab_call<float>(float*, const float*, const float*, const float*, float, const int*,
+                                            const int*, unsigned, int, int, void*, const char*);
+template int wilson_clover_slab_call<double>(double*, const double*, const double*, const double*, double, const int*,
+                                             const int*, unsigned, int, int, void*, const char*);
+
 // r := b - D x on the domains of ONE group only (flags: LQCD_DOMAIN_EVEN / ODD), the other sites of r untouched: what
 // SAP needs between two half sweeps, where only the group solved next reads the residual (sap.cu).  The full operator
 // (no hop is cut): the even/odd kernel variant with the cut switched off, the residual epilogue and no zero fill.

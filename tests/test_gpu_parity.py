@@ -407,6 +407,69 @@ def test_host_entry_points(lq, prec):
     assert np.array_equal(out.numpy(), d.P(prob.xc))
 
 
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("dims,block", [((16, 16, 8, 24), (4, 4, 4, 4)), ((8, 8, 8, 36), (4, 4, 2, 3)),
+                                        ((10, 10, 10, 36), (5, 5, 2, 3))])
+def test_host_entry_points_slab_pipeline(lq, prec, dims, block):
+    """A host vector travels in slabs of time slices: upload of slab k + 1 under pack / kernel / unpack of slab k under
+    the download of slab k - 1 (host_api.cu; knob host_slab_mb sets the smallest slab, -1 the one-shot path).  The
+    kernels are the same ones on a range of tiles / aggregates, so every result is bit-identical with the one-shot
+    path and with the device-pointer calls; the launch counts show that the pipeline was taken.  Random native operator
+    fields (the comparison is between paths, not against the oracle); (10, 10, 10, 36): canonical site order."""
+    import torch
+    nvec = 4
+    rdt = torch.float32 if prec == "f32" else torch.float64
+    cd = tuple(d // b for d, b in zip(dims, block))
+    V, Vc = int(np.prod(dims)), int(np.prod(cd))
+    g = torch.Generator(device="cuda")
+    g.manual_seed(7)
+    rnd = lambda n, s=1.0: torch.randn(n, generator=g, device="cuda", dtype=rdt) * s
+    bc = (1, 1, 1, -1)
+    U, U12 = rnd(lq.native_gauge_reals(dims)), rnd(lq.native_gauge_reals(dims, links12=True))
+    clov, v = rnd(lq.native_clover_reals(dims), 0.1), rnd(lq.native_nullvecs_reals(dims, block, nvec))
+    ws = torch.empty(lq.host_workspace_bytes(dims, block, nvec, dtype=rdt), dtype=torch.uint8, device="cuda")
+    x_h = torch.randn((V, 4, 3, 2), dtype=rdt).pin_memory()
+    xc_h = torch.randn((Vc, 2, nvec, 2), dtype=rdt).pin_memory()
+    xn = lq.pack_spinor(x_h.cuda(), dims)
+    # device-pointer results, canonical
+    ref = {}
+    for key, kw in (("D", {}), ("Ddag", {"dagger": True}), ("D12", {"links12": True})):
+        y = lq.empty_spinor(dims, dtype=rdt)
+        lq.wilson_clover_mult(y, xn, U12 if kw.get("links12") else U, clov, 0.13, dims, bc, **kw)
+        ref[key] = torch.view_as_real(lq.unpack_spinor(y, dims)).cpu()
+    yc = torch.zeros((Vc, 2, nvec, 2), dtype=rdt, device="cuda")
+    lq.restrict(yc, xn, v, dims, block, nvec)
+    ref["R"] = yc.cpu()
+    y = lq.empty_spinor(dims, dtype=rdt)
+    lq.prolong(y, xc_h.cuda(), v, dims, block, nvec)
+    ref["P"] = torch.view_as_real(lq.unpack_spinor(y, dims)).cpu()
+    launches = {}
+    for knob in (1, -1):  # slabs of >= 1 MB / one-shot
+        lq.set_knob("host_slab_mb", knob)
+        try:
+            out = torch.zeros_like(x_h).pin_memory()
+            n0 = lq.launch_count()
+            lq.wilson_clover_mult_host(out, x_h, U, clov, 0.13, dims, bc, ws)
+            launches[knob] = lq.launch_count() - n0
+            assert torch.equal(out, ref["D"]), knob
+            lq.wilson_clover_mult_host(out, x_h, U, clov, 0.13, dims, bc, ws, dagger=True)
+            assert torch.equal(out, ref["Ddag"]), knob
+            lq.wilson_clover_mult_host(out, x_h, U12, clov, 0.13, dims, bc, ws, links12=True)
+            assert torch.equal(out, ref["D12"]), knob
+            oc = torch.zeros_like(xc_h).pin_memory()
+            lq.restrict_host(oc, x_h, v, dims, block, nvec, ws)
+            assert torch.equal(oc, ref["R"]), knob
+            out.zero_()
+            lq.prolong_host(out, xc_h, v, dims, block, nvec, ws)
+            assert torch.equal(out, ref["P"]), knob
+        finally:
+            lq.set_knob("host_slab_mb", 0)
+    assert launches[-1] == 3
+    slab_big_enough = V * 24 * x_h.element_size() >= 3 * (1 << 20)
+    if slab_big_enough:
+        assert launches[1] >= 9, "the slab pipeline was not taken"
+
+
 # ------------------------------------------------------------------------------------------------------
 # the native site order (tiled 4 x 4 x 2 chunks, DESIGN.md section 5) is invisible through pack / unpack: the same
 # canonical fields packed in canonical order (knob site_order = -1) give the same bits
