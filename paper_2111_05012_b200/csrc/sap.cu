@@ -654,6 +654,9 @@ __global__ void __launch_bounds__(512, 1)
             sbar_expect_tx(&bars[1], 8 * 9216);
         }
         if ((tid & 31) == 0) {
+            // (the buffers were last READ through the generic proxy, before the CTA barrier that precedes this call;
+            // the fence orders those accesses before the async-proxy writes of the copies -- cheap insurance)
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             const int i = tid >> 5, c = i & 7;
             const long long ch = c0 + (c & 1) * cstep_z + (c >> 1) * cstep_t;
             if (i < 8) bulk_g2s(sm + TmSmem::LINKS + c * 2304, U + ch * 2304, 9216, &bars[0]);
