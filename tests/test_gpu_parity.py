@@ -462,6 +462,11 @@ def test_host_entry_points_slab_pipeline(lq, prec, dims, block):
             out.zero_()
             lq.prolong_host(out, xc_h, v, dims, block, nvec, ws)
             assert torch.equal(out, ref["P"]), knob
+            # pageable host memory (the copies then block the host; the order of the pipeline still holds)
+            xp, op = x_h.clone(), torch.zeros((V, 4, 3, 2), dtype=rdt)
+            assert not xp.is_pinned() and not op.is_pinned()
+            lq.wilson_clover_mult_host(op, xp, U, clov, 0.13, dims, bc, ws)
+            assert torch.equal(op, ref["D"]), knob
         finally:
             lq.set_knob("host_slab_mb", 0)
     assert launches[-1] == 3
