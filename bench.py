@@ -1086,6 +1086,12 @@ def run_rows(args, cfg: li.Config):
     W = Workload(cfg, device, seed=cfg.seed, synthetic_operators=args.synthetic_operators, precision=args.precision)
     m = model(cfg, real_bytes=8 if args.precision == "f64" else 4)
     peak, peak_src = measured_peak()
+    # tuning knobs of the library for this run (results never depend on them)
+    if args.fine_tile:
+        W.lq.set_fine_tile(tuple(int(v) for v in args.fine_tile.split("x")))
+    for kv in args.knob or []:
+        k, v = kv.split("=")
+        W.lq.set_knob(k, int(v))
     sampler = ClockSampler(0)
     sampler.start()
     out = {}
@@ -1098,7 +1104,8 @@ def run_rows(args, cfg: li.Config):
     clocks = sampler.stop()
     print(json.dumps({"metric": METRIC, "rows": out, "unit": "GB/s", "peak": peak, "peak_source": peak_src,
                       "workload": cfg.name, "dtype": args.precision, "data": "synthetic", "steps": args.steps,
-                      "warmup": args.warmup, "clocks": clocks}), flush=True)
+                      "warmup": args.warmup, "clocks": clocks, "fine_tile": args.fine_tile or "auto",
+                      "knobs": args.knob or []}), flush=True)
 
 
 def run_sweep(args):
@@ -1185,6 +1192,10 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="config 5's bandwidth-roofline sweep over volumes (1 GPU)")
     ap.add_argument("--rows", default=None, metavar="ROW[,ROW...]",
                     help="time the named rows alone (1 GPU; %s)" % ", ".join(sorted(ROW_MODELS)))
+    ap.add_argument("--fine-tile", default=None, metavar="AxBxCxD",
+                    help="with --rows: sites per CTA of the fine kernels (lqcd_set_fine_tile), e.g. 4x4x4x2")
+    ap.add_argument("--knob", action="append", metavar="NAME=VALUE",
+                    help="with --rows: lqcd_set_knob(NAME, VALUE) before timing; may be repeated")
     args = ap.parse_args()
     cfg = li.CONFIGS[args.workload]
     if args.sweep:
