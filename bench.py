@@ -792,7 +792,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     # the 12-real-link variant of A1 (config 4 asks for both storages), timed alone
     extra = {}
     if not args.no_extras and sharded is None:
-        t12 = time_single(W, "wilson_clover_12", reps=max(10, args.steps))
+        t12 = time_single(W, "wilson_clover_12", reps=max(50, args.steps))
         m12 = model(cfg, links12=True, real_bytes=rb)["wilson_clover"]
         extra["wilson_clover_links12"] = {"us": t12 * 1e6, "GBps": m12["bytes"] / t12 / 1e9,
                                           "GFLOPs": m12["flops"] / t12 / 1e9, "units_per_s": m12["units"] / t12,
@@ -800,7 +800,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     if not args.no_extras and sharded is None and not f64:
         # F1 (next row of SURVEY 8(f)): the domain-decomposed operator D_SAP, all domains and the even group
         for name, par in (("wilson_clover_dd", 0), ("wilson_clover_dd_even", 1)):
-            t = time_single(W, name, reps=max(10, args.steps))
+            t = time_single(W, name, reps=max(50, args.steps))
             md = model_dsap(cfg, par)
             extra[name] = {"us": t * 1e6, "GBps": md["bytes"] / t / 1e9, "GFLOPs": md["flops"] / t / 1e9,
                            "units_per_s": md["units"] / t, "frac_of_hbm_peak": md["bytes"] / t / 1e9 / peak,
@@ -879,7 +879,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         W.xcK = torch.view_as_complex(torch.randn((K, cfg.cvolume, 2, cfg.nvec, 2), generator=gk, device=W.dev,
                                                   dtype=torch.float32))
         W.ycK = torch.empty_like(W.xcK)
-        t = time_single(W, "coarse_mrhs", reps=max(5, min(20, args.steps)), warmup=2)
+        t = time_single(W, "coarse_mrhs", reps=max(30, args.steps), warmup=3)
         mc = m["coarse_mult"]
         vec_b = 2 * K * cfg.cvolume * 2 * cfg.nvec * 8
         extra["coarse_mult_mrhs_16"] = {
@@ -891,7 +891,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         # the coarse operator on half storage (A_0 and the forward blocks; the backward blocks are
         # G5c A_+mu(X - mu)^dag G5c): 5/9 of the matrix traffic, every stored block read once for both sites it couples
         prepare_row(W, "coarse_mult_half")
-        t = time_single(W, "coarse_mult_half", reps=max(10, args.steps))
+        t = time_single(W, "coarse_mult_half", reps=max(50, args.steps))
         mh = model_coarse_half(cfg)
         yh, y9 = torch.empty_like(W.xc[0]), torch.empty_like(W.xc[0])
         W.lq.coarse_mult_half(yh, W.xc[0], W.Ah, cfg.cdims, cfg.nvec, ws=W.half_ws)
@@ -923,7 +923,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         # F4, fine half: D on two right-hand sides at once (links and clover read once for both)
         W.x2 = [torch.stack([W.x[0], W.x[1]]), torch.stack([W.x[2], W.x[3]])]
         W.y2 = [torch.empty_like(W.x2[0]), torch.empty_like(W.x2[1])]
-        t = time_single(W, "fine_mrhs", reps=max(10, args.steps))
+        t = time_single(W, "fine_mrhs", reps=max(50, args.steps))
         fb, ff = (576 + 2 * 192) * cfg.volume, 2 * m["wilson_clover"]["flops"]
         extra["wilson_clover_mrhs_2"] = {
             "us": t * 1e6, "us_per_rhs": t * 1e6 / 2, "GBps": fb / t / 1e9, "GFLOPs": ff / t / 1e9,
