@@ -194,6 +194,9 @@ _REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown"
             0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
 
 
+SETTLE_S = 0.5  # untimed run-in of a single-kernel extra row (time_single)
+
+
 class ClockSampler(threading.Thread):
     def __init__(self, device_index: int, period_s: float = 0.004):
         super().__init__(daemon=True)
@@ -436,19 +439,36 @@ def time_steps(W: Workload, steps: int, warmup: int, ranks: Ranks):
     return total_s, per_kernel, launches
 
 
-def time_single(W: Workload, name: str, reps: int, warmup: int = 3):
-    """one row alone, rotating buffers (used for the 12-real-link variant and the sweep)"""
+def time_single(W: Workload, name: str, reps: int, warmup: int = 3, settle_s: float = 0.0, clocks: dict = None):
+    """one row alone, rotating buffers (used for the 12-real-link variant and the sweep).
+    settle_s > 0: the row is first run back to back for that long, untimed, so that the SM clock of the power-capped
+    box has settled on THIS row's load (after a tensor-core row it stays near 1.3 GHz for > 100 ms, which made the
+    next bandwidth row read 10-15 % slow: profiles/r02c_fine_c5.md); clocks: a dict that receives the SM clock sampled
+    during the timed launches."""
     import torch
     f = getattr(W, name)
     for k in range(warmup):
         f(k % W.NBUF)
+    if settle_s > 0:
+        t_end, k = time.perf_counter() + settle_s, 0
+        while time.perf_counter() < t_end:
+            for _ in range(4):
+                f(k % W.NBUF)
+                k += 1
+            torch.cuda.synchronize()
     torch.cuda.synchronize()
+    sampler = ClockSampler(torch.cuda.current_device()) if clocks is not None else None
+    if sampler:
+        sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for k in range(reps):
         f(k % W.NBUF)
     e1.record()
     torch.cuda.synchronize()
+    if sampler:
+        c = sampler.stop()
+        clocks.update({"sm_mhz": c.get("sm_mhz"), "clock_reasons": c.get("reasons", [])})
     return e0.elapsed_time(e1) * 1e-3 / reps
 
 
@@ -792,19 +812,21 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
     # the 12-real-link variant of A1 (config 4 asks for both storages), timed alone
     extra = {}
     if not args.no_extras and sharded is None:
-        t12 = time_single(W, "wilson_clover_12", reps=max(50, args.steps))
+        c12 = {}
+        t12 = time_single(W, "wilson_clover_12", reps=max(50, args.steps), settle_s=SETTLE_S, clocks=c12)
         m12 = model(cfg, links12=True, real_bytes=rb)["wilson_clover"]
         extra["wilson_clover_links12"] = {"us": t12 * 1e6, "GBps": m12["bytes"] / t12 / 1e9,
                                           "GFLOPs": m12["flops"] / t12 / 1e9, "units_per_s": m12["units"] / t12,
-                                          "frac_of_hbm_peak": m12["bytes"] / t12 / 1e9 / peak}
+                                          "frac_of_hbm_peak": m12["bytes"] / t12 / 1e9 / peak, **c12}
     if not args.no_extras and sharded is None and not f64:
         # F1 (next row of SURVEY 8(f)): the domain-decomposed operator D_SAP, all domains and the even group
         for name, par in (("wilson_clover_dd", 0), ("wilson_clover_dd_even", 1)):
-            t = time_single(W, name, reps=max(50, args.steps))
+            cr = {}
+            t = time_single(W, name, reps=max(50, args.steps), settle_s=SETTLE_S, clocks=cr)
             md = model_dsap(cfg, par)
             extra[name] = {"us": t * 1e6, "GBps": md["bytes"] / t / 1e9, "GFLOPs": md["flops"] / t / 1e9,
                            "units_per_s": md["units"] / t, "frac_of_hbm_peak": md["bytes"] / t / 1e9 / peak,
-                           "bytes_per_launch": md["bytes"]}
+                           "bytes_per_launch": md["bytes"], **cr}
 
         # F3: the inner-domain solver (6 minimal-residual iterations, even domains), shared-memory-resident and
         # generic, and the SAP smoother with the paper's parameters (n = 4, 6 inner iterations)
@@ -879,7 +901,11 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         W.xcK = torch.view_as_complex(torch.randn((K, cfg.cvolume, 2, cfg.nvec, 2), generator=gk, device=W.dev,
                                                   dtype=torch.float32))
         W.ycK = torch.empty_like(W.xcK)
-        t = time_single(W, "coarse_mrhs", reps=max(30, args.steps), warmup=3)
+        ck, ckb = {}, {}
+        # burst (the row's first launches, the box still at the clock of whatever ran before) and sustained (after
+        # the run-in: this kernel alone pulls the power-capped box down to ~1.3 GHz)
+        t_burst = time_single(W, "coarse_mrhs", reps=max(30, args.steps), warmup=3, clocks=ckb)
+        t = time_single(W, "coarse_mrhs", reps=max(30, args.steps), warmup=3, settle_s=SETTLE_S, clocks=ck)
         mc = m["coarse_mult"]
         vec_b = 2 * K * cfg.cvolume * 2 * cfg.nvec * 8
         extra["coarse_mult_mrhs_16"] = {
@@ -887,11 +913,14 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "GFLOPs": K * mc["flops"] / t / 1e9, "units_per_s": K * cfg.cvolume / t,
             "speedup_vs_16_single_applications": K * kernels["coarse_mult"]["us"] * 1e-6 / t,
             "frac_of_hbm_peak": (mc["bytes"] + vec_b) / t / 1e9 / peak, "bytes_per_launch": mc["bytes"] + vec_b,
-            "path": "tcgen05 kind::tf32, hi/lo split of both operands (3xTF32), fp32 accumulation"}
+            "path": "tcgen05 kind::tf32, hi/lo split of both operands (3xTF32), fp32 accumulation", **ck,
+            "burst": {"us": t_burst * 1e6, "frac_of_hbm_peak": (mc["bytes"] + vec_b) / t_burst / 1e9 / peak,
+                      "sm_mhz": ckb.get("sm_mhz")}}
         # the coarse operator on half storage (A_0 and the forward blocks; the backward blocks are
         # G5c A_+mu(X - mu)^dag G5c): 5/9 of the matrix traffic, every stored block read once for both sites it couples
         prepare_row(W, "coarse_mult_half")
-        t = time_single(W, "coarse_mult_half", reps=max(50, args.steps))
+        ch = {}
+        t = time_single(W, "coarse_mult_half", reps=max(50, args.steps), settle_s=SETTLE_S, clocks=ch)
         mh = model_coarse_half(cfg)
         yh, y9 = torch.empty_like(W.xc[0]), torch.empty_like(W.xc[0])
         W.lq.coarse_mult_half(yh, W.xc[0], W.Ah, cfg.cdims, cfg.nvec, ws=W.half_ws)
@@ -902,7 +931,7 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
             "us": t * 1e6, "GBps": mh["bytes"] / t / 1e9, "GFLOPs": mh["flops"] / t / 1e9, "units_per_s": cfg.cvolume / t,
             "frac_of_hbm_peak": mh["bytes"] / t / 1e9 / peak, "bytes_per_launch": mh["bytes"], "launches": 2,
             "speedup_vs_nine_block_storage": kernels["coarse_mult"]["us"] * 1e-6 / t,
-            "rel_l2_vs_nine_block_kernel_on_this_operator": dev}
+            "rel_l2_vs_nine_block_kernel_on_this_operator": dev, **ch}
         # ... and the V-cycle with its coarse solve on the half storage (16 applications of D_c at 5/9 of the bytes)
         W.mg_ws = W.lq.mg_workspace(cfg.dims, cfg.block, cfg.nvec, device=W.dev)
         tvh = time_single(W, "vcycle_half", reps=3, warmup=1)
@@ -923,13 +952,14 @@ def run_ours(args, cfg: li.Config, ranks: Ranks):
         # F4, fine half: D on two right-hand sides at once (links and clover read once for both)
         W.x2 = [torch.stack([W.x[0], W.x[1]]), torch.stack([W.x[2], W.x[3]])]
         W.y2 = [torch.empty_like(W.x2[0]), torch.empty_like(W.x2[1])]
-        t = time_single(W, "fine_mrhs", reps=max(50, args.steps))
+        cf = {}
+        t = time_single(W, "fine_mrhs", reps=max(50, args.steps), settle_s=SETTLE_S, clocks=cf)
         fb, ff = (576 + 2 * 192) * cfg.volume, 2 * m["wilson_clover"]["flops"]
         extra["wilson_clover_mrhs_2"] = {
             "us": t * 1e6, "us_per_rhs": t * 1e6 / 2, "GBps": fb / t / 1e9, "GFLOPs": ff / t / 1e9,
             "units_per_s": 2 * cfg.volume / t,
             "speedup_vs_2_single_applications": 2 * kernels["wilson_clover"]["us"] * 1e-6 / t,
-            "frac_of_hbm_peak": fb / t / 1e9 / peak, "bytes_per_launch": fb}
+            "frac_of_hbm_peak": fb / t / 1e9 / peak, "bytes_per_launch": fb, **cf}
         del W.x2, W.y2
         # SURVEY 8(e), the sharded operators' own cost on one GPU: directions marked partitioned with the rank as its
         # own neighbour (pack -> interior -> add; nothing crosses a link, so this is the kernels' overhead over the
