@@ -4,7 +4,6 @@
 namespace lqcd {
 struct Knobs {
     int fine_tile[4] = {0, 0, 0, 0};  // 0 = automatic
-    int fine_variant = 0;             // 0 = automatic choice of fine-kernel variant
     int fine_tslab = 0;               // 0 = automatic; >0 = z tiles per traversal slab; <0 = canonical order
     int coarse_rows_per_warp = 0;     // row tiles per warp, 0 = automatic
     int coarse_R = 0;                 // rows in flight per lane (1, 2, 4), 0 = automatic (2)

@@ -92,8 +92,7 @@ int lqcd_set_fine_tile(const int tile[4]) {
 
 int lqcd_set_knob(const char* name, int value) {
     if (!name) return LQCD_EINVAL;
-    if (!strcmp(name, "fine_variant")) g_knobs.fine_variant = value;
-    else if (!strcmp(name, "coarse_rows_per_warp")) g_knobs.coarse_rows_per_warp = value;
+    if (!strcmp(name, "coarse_rows_per_warp")) g_knobs.coarse_rows_per_warp = value;
     else if (!strcmp(name, "coarse_R")) g_knobs.coarse_R = value;
     else if (!strcmp(name, "coarse_warps")) g_knobs.coarse_warps = value;
     else if (!strcmp(name, "transfer_warps")) g_knobs.transfer_warps = value;
