@@ -275,6 +275,51 @@ def test_wilson_clover_edge_lattices(lq, prec, dims, bc):
             assert rel_l2(got, oracle_D(prob, prob.psi[0], prec, dagger=dagger)) <= TOL[prec]
 
 
+def _random_lattices(n, seed):
+    """Seeded lattice shapes for the sweep below: extents 2..12, volume <= 6000 (the oracle stays fast); about half of
+    them satisfy 4 | Lx, 4 | Ly, 2 | Lz (tiled native site order, a warp per layout tile), the others fall back to the
+    canonical order with ragged chunks."""
+    rng = np.random.default_rng(seed)
+    out = []
+    while len(out) < n:
+        if len(out) % 2 == 0:
+            dims = (int(rng.choice([4, 8, 12])), int(rng.choice([4, 8])), int(rng.choice([2, 4, 6])),
+                    int(rng.integers(2, 9)))
+        else:
+            dims = tuple(int(rng.integers(2, 8)) for _ in range(4))
+        if int(np.prod(dims)) > 6000:
+            continue
+        bc = tuple(int(b) for b in rng.choice([1, -1], size=4))
+        domain = tuple(int(rng.choice([d for d in range(1, L + 1) if L % d == 0])) for L in dims)
+        tile = tuple(int(rng.choice([d for d in (1, 2, 4) if L % d == 0])) for L in dims)
+        out.append((dims, bc, domain, tile, bool(rng.integers(2)), bool(rng.integers(2)), int(rng.integers(3))))
+    return out
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("case", _random_lattices(10, 20211105), ids=lambda c: "x".join(map(str, c[0])))
+def test_wilson_clover_random_lattices(lq, prec, case):
+    """D, D^dag and D_SAP (all / even / odd domains) on seeded random lattice shapes, boundary conditions, domains,
+    link storage and CTA tiles against the oracle: every index-decode path of the fine kernels (tiled and canonical
+    site order, a warp per layout tile or not, automatic and user tiles)."""
+    dims, bc, domain, tile, links12, dagger, parity = case
+    cfg = custom_config(dims, (1, 1, 1, 1), 1, bc=bc)
+    prob = make_problem(cfg, coarse="none")
+    d = Dev(lq, prob, prec, links12=links12, coarse=False)
+    psi = prob.psi[0]
+    try:
+        for user_tile in (None, tile):
+            lq.set_fine_tile(user_tile)
+            got = d.D(psi, dagger=dagger)
+            assert rel_l2(got, oracle_D(prob, psi, prec, dagger=dagger)) <= TOL[prec], (case, user_tile)
+            got = d.Dsap(psi, domain, parity=parity, dagger=dagger)
+            ref = oracle_Dsap(prob, psi, prec, domain, parity=parity, dagger=dagger)
+            assert rel_l2(got, ref) <= TOL[prec], (case, user_tile)
+            assert np.array_equal(got == 0, ref == 0), (case, user_tile)
+    finally:
+        lq.set_fine_tile(None)
+
+
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("dims,block,nvec", [
     ((16, 8, 8, 8), (8, 4, 4, 4), 4),    # the paper's 8x4x4x4 block; coarse 2^4
