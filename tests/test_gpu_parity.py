@@ -347,6 +347,39 @@ def test_coarse_and_transfer_edge_sizes(lq, prec, dims, block, nvec):
     assert rel_l2(d.P(prob.xc), oracle.prolong(rounded(prob.xc, prec), v, cfg.dims, cfg.block)) <= TOL[prec]
 
 
+def _random_coarse_sizes(n, seed):
+    rng = np.random.default_rng(seed)
+    out = []
+    while len(out) < n:
+        block = tuple(int(rng.choice([1, 2, 3, 4])) for _ in range(4))
+        cdims = tuple(int(rng.integers(2, 5)) for _ in range(4))
+        dims = tuple(b * c for b, c in zip(block, cdims))
+        nvec = int(rng.choice([1, 2, 3, 5, 7, 8, 12, 16, 17, 24, 32, 33]))
+        bvol, cvol = int(np.prod(block)), int(np.prod(cdims))
+        if bvol < 2 or bvol * cvol > 6000 or cvol * nvec * nvec > 60000:
+            continue
+        out.append((dims, block, nvec))
+    return out
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dims,block,nvec", _random_coarse_sizes(8, 5012),
+                         ids=lambda v: "x".join(map(str, v)) if isinstance(v, tuple) else str(v))
+def test_coarse_and_transfer_random_sizes(lq, prec, dims, block, nvec):
+    """coarse_mult (and its dagger), restrict and prolong on seeded random block shapes, coarse extents 2..4 and numbers
+    of null vectors (rows spread over part of a warp, one warp, several vec16 per lane; ragged aggregates)."""
+    cfg = custom_config(dims, block, nvec)
+    prob = make_problem(cfg, coarse="synthetic")
+    d = Dev(lq, prob, prec)
+    v, A = rounded(prob.v, prec), rounded(prob.A, prec)
+    for dagger in (False, True):
+        ref = oracle.coarse_mult(rounded(prob.xc, prec), A, cfg.cdims, dagger=dagger)
+        assert rel_l2(d.Dc(prob.xc, dagger=dagger), ref) <= TOL[prec], dagger
+    psi = prob.psi[0]
+    assert rel_l2(d.R(psi), oracle.restrict(rounded(psi, prec), v, cfg.dims, cfg.block)) <= TOL[prec]
+    assert rel_l2(d.P(prob.xc), oracle.prolong(rounded(prob.xc, prec), v, cfg.dims, cfg.block)) <= TOL[prec]
+
+
 def test_results_do_not_depend_on_tuning_knobs(lq):
     prob = config_problem("c2", 16)
     d = Dev(lq, prob, "f32")
