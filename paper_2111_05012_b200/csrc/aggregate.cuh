@@ -13,6 +13,7 @@ struct TransferParams {
     int nvec;
     int LV;    // vec16 per (X, chi, i) vector = bv * 12 / NV
     int agg_off;  // first aggregate (X, chi) of the launch (range forms of restrict / prolong; 0 otherwise)
+    int zero;     // always 0, but only known at run time: the dependency fence of the streaming batches (transfer.cu)
     SiteOrder ord;  // native position of a fine site (layout.cuh)
 };
 
@@ -55,6 +56,7 @@ inline int transfer_setup(TransferParams& P, const void* a, const void* b, const
     }
     P.nvec = nvec;
     P.agg_off = 0;
+    P.zero = 0;
     P.LV = P.bv * 12 / VecOf<T>::NV;
     P.ord.set(dims);
     return LQCD_OK;
